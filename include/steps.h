@@ -1,0 +1,156 @@
+/*
+ * steps.h -- C ABI of steps-b200: the data-parallel hot path of StePS (arXiv:1811.05903)
+ * on one NVIDIA B200 (sm_100a).
+ *
+ * What the library computes (citations: PAPER.md line numbers / equation numbers;
+ * "reading #k": DESIGN.md section "Readings of the paper"):
+ *
+ *   (1) the O(N^2) direct-summation force of Eq. 8 (L88), first term, with G = 1 and
+ *       without the a(t)^-3 factor (both enter through the kick coefficients):
+ *
+ *           acc_i = sum_{j != i} m_j g(|x_j - x_i|, h_i + h_j) (x_j - x_i),   g = calF / r,
+ *
+ *       calF(r, h) the spline-softened 1/r^2 of Eq. 3-4 (L53-61), evaluated with the PAIR
+ *       softening h_i + h_j (Eq. 2, Eq. 8; reading #3).  j = i is skipped and a
+ *       coincident distinct pair (r = 0) contributes 0 (reading #4).  This is "the most
+ *       time-consuming part" (L96, L131) and the only super-linear step.
+ *   (2) the kick-drift-kick leapfrog of Eq. 9-11 (L98-109) applied to Eq. 8 in comoving
+ *       coordinates, as one fused O(N) kernel driven by scalar coefficients the host
+ *       derives from the Friedmann equation (Eq. 1, RK4 per L127), followed by the one
+ *       force evaluation per step the paper asks for (L96).
+ *
+ * Conventions common to every call
+ *   - All array arguments are DEVICE pointers unless the name ends in _host.  The caller
+ *     owns every buffer; the library keeps no pointer after the call returns.
+ *   - Layout: pos, vel, acc are SoA, 3N contiguous doubles [x_0..x_{N-1} | y_0.. | z_0..];
+ *     mass and soft are N doubles.  Pointers must be 16-byte aligned.  soft[i] is the
+ *     paper's h_i (Eq. 7, support radius of the spline), NOT a Plummer epsilon.
+ *   - Calls are stream-ordered on `stream` (a cudaStream_t; NULL = legacy default stream)
+ *     and never synchronise the host, except that the FIRST call for a larger N than any
+ *     seen before on this device (re)allocates the internal workspace with cudaMalloc.
+ *     steps_reserve(N) does that allocation up front; steps_shutdown() frees it.
+ *   - Results do not depend on particle order beyond rounding.  Radially sorted input
+ *     (|x| ascending) is the fast path: the kernels classify (i-group, j-tile) pairs by
+ *     their radial intervals into "far" (no pair can have r < h_i + h_j; branch-free
+ *     Newtonian body) and "near" (full per-pair spline test).  Unsorted input only makes
+ *     more tiles "near" -- slower, never wrong.
+ *   - Return value: STEPS_OK (0) or a negative error code; steps_strerror() gives text.
+ *     Nothing throws or aborts.  N = 1 is valid (acc = 0).  Non-finite inputs give
+ *     non-finite outputs, not an error.  Numerical domain of the fast (far) bodies:
+ *     pair separations must satisfy 2^-63 < r < 2^63 (r^2 is seeded through fp32).
+ *   - The device must be compute capability 10.x (sm_100a cubin only; no PTX fallback,
+ *     no CPU fallback): otherwise STEPS_EUNSUPPORTED.
+ */
+#ifndef STEPS_B200_STEPS_H
+#define STEPS_B200_STEPS_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct CUstream_st *steps_stream_t; /* cudaStream_t */
+
+enum {
+    STEPS_OK = 0,
+    STEPS_EINVAL = -1,       /* null pointer, N < 1, misaligned pointer, bad range */
+    STEPS_ECUDA = -2,        /* CUDA runtime / launch error (steps_last_cuda_error() has the code) */
+    STEPS_EUNSUPPORTED = -3, /* current device is not sm_100 */
+    STEPS_ENOMEM = -4        /* workspace allocation failed */
+};
+
+/* ---- force evaluation --------------------------------- */
+
+/* fp64 path: every pair in fp64 (the reciprocal square root is seeded by the fp32 SFU and
+ * refined in fp64).  Bar: max_i |acc_i - oracle_i| / |oracle_i| <= 1e-12.
+ * Overwrites acc[0..3N).  pos/mass/soft are read only. */
+int steps_forces(const double *pos, const double *mass, const double *soft, long long N,
+                 double *acc, steps_stream_t stream);
+
+/* mixed path: pair arithmetic in fp32 (the paper's GPU runs were single precision, L159),
+ * per-tile fp32 partial sums flushed into fp64 accumulators.
+ * Bar: RMS relative error <= 2e-6, max <= 1e-4. */
+int steps_forces_mixed(const double *pos, const double *mass, const double *soft, long long N,
+                       double *acc, steps_stream_t stream);
+
+/* The paper's multi-node decomposition (L139: node k computes floor(N/N_node) force
+ * vectors against all particles): forces on particles i in [i_begin, i_end) only, against
+ * all N sources.  acc_out is SoA over the range: 3*(i_end-i_begin) doubles
+ * [ax | ay | az].  mixed != 0 selects the mixed path. */
+int steps_forces_range(const double *pos, const double *mass, const double *soft, long long N,
+                       long long i_begin, long long i_end, double *acc_out, int mixed,
+                       steps_stream_t stream);
+
+/* End-to-end convenience with HOST buffers (pageable or pinned): copies pos/mass/soft to
+ * the device, evaluates the forces, copies acc back and synchronises `stream` before
+ * returning.  Used by bench.py's e2e figure. */
+int steps_forces_host(const double *pos_host, const double *mass_host, const double *soft_host,
+                      long long N, double *acc_host, int mixed, steps_stream_t stream);
+
+/* ---- time integration ---------------------------------- */
+
+/* Coefficients of one fused kick/drift pass.  With g_i = acc_i + B x_i the pass does
+ *     v <- alpha_close v + beta_close g     (closing half kick of the PREVIOUS step)
+ *     v <- alpha_open  v + beta_open  g     (opening half kick of THIS step)
+ *     x <- x + gamma v                      (drift)
+ * For Eq. 8 with reading #6 (the background term carries a^-3) and reading #8 (drag
+ * explicit in the opening, implicit in the closing half kick), a step a_n -> a_{n+1} of
+ * length dt has
+ *     alpha_open = 1 - H_n dt            beta_open  = G a_n^-3 dt/2         gamma = dt
+ *     alpha_close = 1/(1 + H_{n+1} dt)   beta_close = G a_{n+1}^-3 (dt/2)/(1 + H_{n+1} dt)
+ * and B = (4 pi/3) rho_bar (G = 1 units).  The identity kick is alpha = 1, beta = 0.
+ * steps_kdk_schedule() fills these from the cosmology.  `mixed` selects the force path. */
+typedef struct {
+    double alpha_close, beta_close;
+    double alpha_open, beta_open;
+    double gamma;
+    double B;
+    int mixed;
+} steps_kdk_coeffs;
+
+/* The fused O(N) pass alone (Eq. 9-10): updates vel and pos in place from acc. */
+int steps_kick_drift(double *pos, double *vel, const double *acc, long long N,
+                     const steps_kdk_coeffs *c, steps_stream_t stream);
+
+/* One integrator step: steps_kick_drift, then ONE force evaluation at the new positions
+ * into acc (L96).  Driver pattern: steps_forces once; per step one steps_kdk_step whose
+ * *_close are the previous step's closing coefficients (identity on the first step);
+ * a final steps_kick_drift with gamma = 0 and an identity opening kick closes the run. */
+int steps_kdk_step(double *pos, double *vel, double *acc, const double *mass, const double *soft,
+                   long long N, const steps_kdk_coeffs *c, steps_stream_t stream);
+
+/* Host-side scalars (no device work).  Friedmann equation, Eq. 1 (L37). */
+typedef struct {
+    double H0, Omega_m, Omega_r, Omega_L, Omega_k; /* present-day values, code units */
+} steps_cosmology;
+
+double steps_hubble(double a, const steps_cosmology *c);
+/* a(t + dt) by classical RK4 on da/dt = a H(a) (L127). */
+double steps_scale_factor_rk4(double a, double dt, const steps_cosmology *c);
+/* Fills the opening half kick, drift and closing half kick of the step a_n -> a_{n+1}
+ * (a_{n+1} by RK4, H0 = 0 means static Newtonian mode, L92) into
+ * out[0..5] = {alpha_open, beta_open, gamma, alpha_close, beta_close, a_next}. */
+int steps_kdk_schedule(double a_n, double dt, double G, const steps_cosmology *c, double *out6);
+
+/* Diagnostics (row a7): out4 (device, 4 doubles) = {sum m v_x, sum m v_y, sum m v_z,
+ * sum m |v|}.  Deterministic fixed-order reduction. */
+int steps_momentum(const double *vec, const double *mass, long long N, double *out4,
+                   steps_stream_t stream);
+
+/* ---- housekeeping ------------------------------------------------------------------ */
+
+int steps_reserve(long long N);          /* allocate workspace for up to N particles now */
+void steps_shutdown(void);               /* free all workspace on all devices */
+long long steps_workspace_bytes(long long N); /* bytes steps_reserve(N) allocates */
+const char *steps_strerror(int code);
+int steps_last_cuda_error(void);         /* cudaError_t of the last STEPS_ECUDA on this thread */
+int steps_version(void);                 /* major*10000 + minor*100 + patch */
+/* Number of kernels this library has launched since load (for bench.py's gpu_launches). */
+long long steps_kernel_launch_count(void);
+/* Tuning / testing knobs.  "driver": 0 = default force driver, 1 = the simple one-CTA-per-
+ * i-block driver kept as an in-library cross-check.  Unknown key: STEPS_EINVAL. */
+int steps_set_option(const char *key, long long value);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* STEPS_B200_STEPS_H */

@@ -1,0 +1,304 @@
+// steps.cu -- C ABI of steps-b200 (include/steps.h): argument checks, workspace, launches.
+// Every step of the hot path runs in the kernels of this translation unit; there is no CPU
+// fallback and no dependency on oracle/.
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+
+#include "../../include/steps.h"
+#include "common.cuh"
+#include "prep.cuh"
+#include "force_mixed.cuh"
+#include "force_fp64.cuh"
+#include "force_v1.cuh"
+#include "kdk.cuh"
+
+using namespace steps;
+
+namespace {
+
+std::atomic<long long> g_launches{0};
+thread_local int g_last_cuda_error = 0;
+std::atomic<int> g_driver{0};   // 0 = default, 1 = simple v1 driver (cross-check)
+
+constexpr int MAX_DEVICES = 16;
+
+struct Workspace {
+    void* tiles = nullptr;          // max(sizeof(TileF32), sizeof(TileF64)) * ntiles
+    long long cap_particles = 0;
+    double* mom_partial = nullptr;  // MOM_BLOCKS * 4
+    // staging buffers of steps_forces_host
+    double* h_pos = nullptr; double* h_mass = nullptr; double* h_soft = nullptr; double* h_acc = nullptr;
+    long long h_cap = 0;
+    int cc_major = -1;
+};
+Workspace g_ws[MAX_DEVICES];
+std::mutex g_mutex;
+
+inline long long ntiles_of(long long N) { return (N + TJ - 1) / TJ; }
+
+int cuda_fail(cudaError_t e)
+{
+    g_last_cuda_error = (int)e;
+    return STEPS_ECUDA;
+}
+#define STEPS_CUDA(call)                                   \
+    do {                                                   \
+        cudaError_t e__ = (call);                          \
+        if (e__ != cudaSuccess) return cuda_fail(e__);     \
+    } while (0)
+
+int current_device(int* dev)
+{
+    STEPS_CUDA(cudaGetDevice(dev));
+    if (*dev < 0 || *dev >= MAX_DEVICES) return STEPS_EUNSUPPORTED;
+    Workspace& w = g_ws[*dev];
+    if (w.cc_major < 0) {
+        int major = 0;
+        STEPS_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, *dev));
+        w.cc_major = major;
+    }
+    if (w.cc_major != 10) return STEPS_EUNSUPPORTED;   // sm_100a cubin only
+    return STEPS_OK;
+}
+
+int ensure_workspace(int dev, long long N)
+{
+    std::lock_guard<std::mutex> lock(g_mutex);
+    Workspace& w = g_ws[dev];
+    if (!w.mom_partial) {
+        if (cudaMalloc(&w.mom_partial, sizeof(double) * MOM_BLOCKS * 4) != cudaSuccess) return STEPS_ENOMEM;
+    }
+    if (N <= w.cap_particles) return STEPS_OK;
+    if (w.tiles) { cudaFree(w.tiles); w.tiles = nullptr; w.cap_particles = 0; }
+    const size_t tile_bytes = sizeof(TileF64) > sizeof(TileF32) ? sizeof(TileF64) : sizeof(TileF32);
+    if (cudaMalloc(&w.tiles, tile_bytes * (size_t)ntiles_of(N)) != cudaSuccess) {
+        cudaGetLastError();
+        return STEPS_ENOMEM;
+    }
+    w.cap_particles = ntiles_of(N) * TJ;
+    return STEPS_OK;
+}
+
+bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+
+template <typename Path>
+int launch_forces(const double* pos, const double* mass, const double* soft, long long N, long long i_begin,
+                  long long i_end, double* acc_out, cudaStream_t st, Workspace& w)
+{
+    using Tile = typename Path::Tile;
+    const int nt = (int)ntiles_of(N);
+    Tile* tiles = reinterpret_cast<Tile*>(w.tiles);
+    prep_tiles<Tile><<<nt, TJ, 0, st>>>(pos, mass, soft, N, tiles);
+    g_launches++;
+    const long long cnt = i_end - i_begin;
+    const int nblk = (int)((cnt + IB - 1) / IB);
+    forces_v1_kernel<Path><<<nblk, CTA_THREADS, 0, st>>>(pos, soft, N, tiles, nt, i_begin, i_end, acc_out);
+    g_launches++;
+    STEPS_CUDA(cudaGetLastError());
+    return STEPS_OK;
+}
+
+int forces_impl(const double* pos, const double* mass, const double* soft, long long N, long long i_begin,
+                long long i_end, double* acc_out, int mixed, steps_stream_t stream)
+{
+    if (!pos || !mass || !soft || !acc_out || N < 1) return STEPS_EINVAL;
+    if (i_begin < 0 || i_end > N || i_begin >= i_end) return STEPS_EINVAL;
+    if (N > (1ll << 31) - TJ) return STEPS_EINVAL;
+    if (misaligned(pos) || misaligned(mass) || misaligned(soft) || misaligned(acc_out)) return STEPS_EINVAL;
+    int dev;
+    int rc = current_device(&dev);
+    if (rc != STEPS_OK) return rc;
+    rc = ensure_workspace(dev, N);
+    if (rc != STEPS_OK) return rc;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    return mixed ? launch_forces<MixedPath>(pos, mass, soft, N, i_begin, i_end, acc_out, st, g_ws[dev])
+                 : launch_forces<Fp64Path>(pos, mass, soft, N, i_begin, i_end, acc_out, st, g_ws[dev]);
+}
+
+}  // namespace
+
+extern "C" {
+
+int steps_forces(const double* pos, const double* mass, const double* soft, long long N, double* acc,
+                 steps_stream_t stream)
+{
+    return forces_impl(pos, mass, soft, N, 0, N, acc, 0, stream);
+}
+
+int steps_forces_mixed(const double* pos, const double* mass, const double* soft, long long N, double* acc,
+                       steps_stream_t stream)
+{
+    return forces_impl(pos, mass, soft, N, 0, N, acc, 1, stream);
+}
+
+int steps_forces_range(const double* pos, const double* mass, const double* soft, long long N, long long i_begin,
+                       long long i_end, double* acc_out, int mixed, steps_stream_t stream)
+{
+    return forces_impl(pos, mass, soft, N, i_begin, i_end, acc_out, mixed, stream);
+}
+
+int steps_forces_host(const double* pos_host, const double* mass_host, const double* soft_host, long long N,
+                      double* acc_host, int mixed, steps_stream_t stream)
+{
+    if (!pos_host || !mass_host || !soft_host || !acc_host || N < 1) return STEPS_EINVAL;
+    int dev;
+    int rc = current_device(&dev);
+    if (rc != STEPS_OK) return rc;
+    Workspace& w = g_ws[dev];
+    {
+        std::lock_guard<std::mutex> lock(g_mutex);
+        if (N > w.h_cap) {
+            cudaFree(w.h_pos); cudaFree(w.h_mass); cudaFree(w.h_soft); cudaFree(w.h_acc);
+            w.h_pos = w.h_mass = w.h_soft = w.h_acc = nullptr; w.h_cap = 0;
+            if (cudaMalloc(&w.h_pos, sizeof(double) * 3 * N) != cudaSuccess ||
+                cudaMalloc(&w.h_mass, sizeof(double) * N) != cudaSuccess ||
+                cudaMalloc(&w.h_soft, sizeof(double) * N) != cudaSuccess ||
+                cudaMalloc(&w.h_acc, sizeof(double) * 3 * N) != cudaSuccess) {
+                cudaGetLastError();
+                return STEPS_ENOMEM;
+            }
+            w.h_cap = N;
+        }
+    }
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    STEPS_CUDA(cudaMemcpyAsync(w.h_pos, pos_host, sizeof(double) * 3 * N, cudaMemcpyHostToDevice, st));
+    STEPS_CUDA(cudaMemcpyAsync(w.h_mass, mass_host, sizeof(double) * N, cudaMemcpyHostToDevice, st));
+    STEPS_CUDA(cudaMemcpyAsync(w.h_soft, soft_host, sizeof(double) * N, cudaMemcpyHostToDevice, st));
+    rc = forces_impl(w.h_pos, w.h_mass, w.h_soft, N, 0, N, w.h_acc, mixed, stream);
+    if (rc != STEPS_OK) return rc;
+    STEPS_CUDA(cudaMemcpyAsync(acc_host, w.h_acc, sizeof(double) * 3 * N, cudaMemcpyDeviceToHost, st));
+    STEPS_CUDA(cudaStreamSynchronize(st));
+    return STEPS_OK;
+}
+
+int steps_kick_drift(double* pos, double* vel, const double* acc, long long N, const steps_kdk_coeffs* c,
+                     steps_stream_t stream)
+{
+    if (!pos || !vel || !acc || !c || N < 1) return STEPS_EINVAL;
+    if (misaligned(pos) || misaligned(vel) || misaligned(acc)) return STEPS_EINVAL;
+    int dev;
+    int rc = current_device(&dev);
+    if (rc != STEPS_OK) return rc;
+    KdkScalars k{c->alpha_close, c->beta_close, c->alpha_open, c->beta_open, c->gamma, c->B};
+    const long long M = 3 * N;
+    long long blocks = (M + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    kick_drift_kernel<<<(int)blocks, 256, 0, reinterpret_cast<cudaStream_t>(stream)>>>(pos, vel, acc, M, k);
+    g_launches++;
+    STEPS_CUDA(cudaGetLastError());
+    return STEPS_OK;
+}
+
+int steps_kdk_step(double* pos, double* vel, double* acc, const double* mass, const double* soft, long long N,
+                   const steps_kdk_coeffs* c, steps_stream_t stream)
+{
+    if (!mass || !soft) return STEPS_EINVAL;
+    int rc = steps_kick_drift(pos, vel, acc, N, c, stream);
+    if (rc != STEPS_OK) return rc;
+    return forces_impl(pos, mass, soft, N, 0, N, acc, c->mixed, stream);
+}
+
+double steps_hubble(double a, const steps_cosmology* c)
+{
+    return c->H0 * std::sqrt(c->Omega_m / (a * a * a) + c->Omega_r / (a * a * a * a) + c->Omega_L +
+                             c->Omega_k / (a * a));
+}
+
+double steps_scale_factor_rk4(double a, double dt, const steps_cosmology* c)
+{
+    auto f = [c](double s) { return s * steps_hubble(s, c); };
+    const double k1 = f(a), k2 = f(a + 0.5 * dt * k1), k3 = f(a + 0.5 * dt * k2), k4 = f(a + dt * k3);
+    return a + dt / 6.0 * (k1 + 2.0 * (k2 + k3) + k4);
+}
+
+int steps_kdk_schedule(double a_n, double dt, double G, const steps_cosmology* c, double* out6)
+{
+    if (!c || !out6 || !(a_n > 0.0)) return STEPS_EINVAL;
+    const bool is_static = (c->H0 == 0.0);
+    const double H_n = is_static ? 0.0 : steps_hubble(a_n, c);
+    const double a_1 = is_static ? a_n : steps_scale_factor_rk4(a_n, dt, c);
+    const double H_1 = is_static ? 0.0 : steps_hubble(a_1, c);
+    out6[0] = 1.0 - H_n * dt;
+    out6[1] = 0.5 * dt * G / (a_n * a_n * a_n);
+    out6[2] = dt;
+    out6[3] = 1.0 / (1.0 + H_1 * dt);
+    out6[4] = 0.5 * dt * G / (a_1 * a_1 * a_1) * out6[3];
+    out6[5] = a_1;
+    return STEPS_OK;
+}
+
+int steps_momentum(const double* vec, const double* mass, long long N, double* out4, steps_stream_t stream)
+{
+    if (!vec || !mass || !out4 || N < 1) return STEPS_EINVAL;
+    int dev;
+    int rc = current_device(&dev);
+    if (rc != STEPS_OK) return rc;
+    rc = ensure_workspace(dev, 1);
+    if (rc != STEPS_OK) return rc;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    momentum_stage1<<<MOM_BLOCKS, 256, 0, st>>>(vec, mass, N, g_ws[dev].mom_partial);
+    momentum_stage2<<<1, 32, 0, st>>>(g_ws[dev].mom_partial, MOM_BLOCKS, out4);
+    g_launches += 2;
+    STEPS_CUDA(cudaGetLastError());
+    return STEPS_OK;
+}
+
+int steps_reserve(long long N)
+{
+    if (N < 1) return STEPS_EINVAL;
+    int dev;
+    int rc = current_device(&dev);
+    if (rc != STEPS_OK) return rc;
+    return ensure_workspace(dev, N);
+}
+
+void steps_shutdown(void)
+{
+    std::lock_guard<std::mutex> lock(g_mutex);
+    int cur = 0;
+    cudaGetDevice(&cur);
+    for (int d = 0; d < MAX_DEVICES; ++d) {
+        Workspace& w = g_ws[d];
+        if (!w.tiles && !w.mom_partial && !w.h_pos) continue;
+        cudaSetDevice(d);
+        cudaFree(w.tiles); cudaFree(w.mom_partial);
+        cudaFree(w.h_pos); cudaFree(w.h_mass); cudaFree(w.h_soft); cudaFree(w.h_acc);
+        w = Workspace();
+    }
+    cudaSetDevice(cur);
+}
+
+long long steps_workspace_bytes(long long N)
+{
+    if (N < 1) return 0;
+    const size_t tile_bytes = sizeof(TileF64) > sizeof(TileF32) ? sizeof(TileF64) : sizeof(TileF32);
+    return (long long)(tile_bytes * (size_t)ntiles_of(N) + sizeof(double) * MOM_BLOCKS * 4);
+}
+
+const char* steps_strerror(int code)
+{
+    switch (code) {
+        case STEPS_OK: return "ok";
+        case STEPS_EINVAL: return "invalid argument (null or misaligned pointer, N < 1, or bad range)";
+        case STEPS_ECUDA: return "CUDA runtime error (see steps_last_cuda_error)";
+        case STEPS_EUNSUPPORTED: return "device is not compute capability 10.x (sm_100a build, no fallback)";
+        case STEPS_ENOMEM: return "workspace allocation failed";
+        default: return "unknown error code";
+    }
+}
+
+int steps_last_cuda_error(void) { return g_last_cuda_error; }
+int steps_version(void) { return 100; }
+long long steps_kernel_launch_count(void) { return g_launches.load(); }
+
+int steps_set_option(const char* key, long long value)
+{
+    if (!key) return STEPS_EINVAL;
+    if (std::strcmp(key, "driver") == 0) { g_driver = (int)value; return STEPS_OK; }
+    return STEPS_EINVAL;
+}
+
+}  // extern "C"

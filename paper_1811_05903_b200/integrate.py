@@ -1,0 +1,26 @@
+"""Host-side driver of the KDK run (row a6: the O(1) scalar bookkeeping; all O(N) and O(N^2)
+work is in the kernels).  Follows the driver pattern documented at steps_kdk_step in
+include/steps.h: forces once, then one fused kick/drift + force evaluation per step, the
+closing half kick of step n fused with the opening half kick of step n+1."""
+from __future__ import annotations
+
+from . import steps as S
+
+
+def run_kdk(pos, vel, acc, mass, soft, a0: float, dts, cosmo: S.Cosmology, G: float, B: float,
+            mixed: bool = False, on_step=None) -> float:
+    """Integrate in place over the time steps `dts` starting at scale factor a0.  `acc` must
+    hold the forces at the initial positions on entry (steps_forces) and holds the forces at
+    the final positions on return.  Returns the final scale factor.  on_step(k, a) is called
+    after each step's force evaluation with velocities still lacking the closing half kick."""
+    a = a0
+    alpha_c, beta_c = 1.0, 0.0                      # identity closing kick before the first step
+    for k, dt in enumerate(dts):
+        sc = S.steps_kdk_schedule(a, float(dt), G, cosmo)
+        co = S.KdkCoeffs(alpha_c, beta_c, sc["alpha_open"], sc["beta_open"], sc["gamma"], B, int(mixed))
+        S.steps_kdk_step(pos, vel, acc, mass, soft, co)
+        alpha_c, beta_c, a = sc["alpha_close"], sc["beta_close"], sc["a_next"]
+        if on_step is not None:
+            on_step(k, a)
+    S.steps_kick_drift(pos, vel, acc, S.KdkCoeffs(alpha_c, beta_c, 1.0, 0.0, 0.0, B, int(mixed)))
+    return a

@@ -1,0 +1,187 @@
+"""Thin ctypes binding of the C ABI in include/steps.h -- same names, argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of libsteps_b200.so; PyTorch is used
+for device memory and streams.  There is no CPU fallback: if the library is missing it is
+built (nvcc, in-tree) or the import of the symbol fails loudly."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsteps_b200.so")
+
+OK, EINVAL, ECUDA, EUNSUPPORTED, ENOMEM = 0, -1, -2, -3, -4
+
+EXPORTS = [
+    "steps_forces", "steps_forces_mixed", "steps_forces_range", "steps_forces_host", "steps_kick_drift",
+    "steps_kdk_step", "steps_hubble", "steps_scale_factor_rk4", "steps_kdk_schedule", "steps_momentum",
+    "steps_reserve", "steps_shutdown", "steps_workspace_bytes", "steps_strerror", "steps_last_cuda_error",
+    "steps_version", "steps_kernel_launch_count", "steps_set_option",
+]
+
+
+class KdkCoeffs(C.Structure):
+    _fields_ = [("alpha_close", C.c_double), ("beta_close", C.c_double), ("alpha_open", C.c_double),
+                ("beta_open", C.c_double), ("gamma", C.c_double), ("B", C.c_double), ("mixed", C.c_int)]
+
+
+class Cosmology(C.Structure):
+    _fields_ = [("H0", C.c_double), ("Omega_m", C.c_double), ("Omega_r", C.c_double),
+                ("Omega_L", C.c_double), ("Omega_k", C.c_double)]
+
+
+class StepsError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Load (building first if the .so is absent or stale) the C-ABI library."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    from . import build as _build
+    path = _build.build()
+    L = C.CDLL(path)
+    vp, ll, dbl, i32 = C.c_void_p, C.c_longlong, C.c_double, C.c_int
+    L.steps_forces.argtypes = [vp, vp, vp, ll, vp, vp]
+    L.steps_forces_mixed.argtypes = [vp, vp, vp, ll, vp, vp]
+    L.steps_forces_range.argtypes = [vp, vp, vp, ll, ll, ll, vp, i32, vp]
+    L.steps_forces_host.argtypes = [vp, vp, vp, ll, vp, i32, vp]
+    L.steps_kick_drift.argtypes = [vp, vp, vp, ll, C.POINTER(KdkCoeffs), vp]
+    L.steps_kdk_step.argtypes = [vp, vp, vp, vp, vp, ll, C.POINTER(KdkCoeffs), vp]
+    L.steps_hubble.argtypes = [dbl, C.POINTER(Cosmology)]
+    L.steps_hubble.restype = dbl
+    L.steps_scale_factor_rk4.argtypes = [dbl, dbl, C.POINTER(Cosmology)]
+    L.steps_scale_factor_rk4.restype = dbl
+    L.steps_kdk_schedule.argtypes = [dbl, dbl, dbl, C.POINTER(Cosmology), C.POINTER(dbl)]
+    L.steps_momentum.argtypes = [vp, vp, ll, vp, vp]
+    L.steps_reserve.argtypes = [ll]
+    L.steps_shutdown.restype = None
+    L.steps_workspace_bytes.argtypes = [ll]
+    L.steps_workspace_bytes.restype = ll
+    L.steps_strerror.argtypes = [i32]
+    L.steps_strerror.restype = C.c_char_p
+    L.steps_kernel_launch_count.restype = ll
+    L.steps_set_option.argtypes = [C.c_char_p, ll]
+    _lib = L
+    return L
+
+
+def _check(rc: int) -> None:
+    if rc != OK:
+        L = lib()
+        msg = L.steps_strerror(rc).decode()
+        if rc == ECUDA:
+            msg += f" [cudaError {L.steps_last_cuda_error()}]"
+        raise StepsError(f"steps error {rc}: {msg}")
+
+
+def _stream(stream=None) -> int:
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return int(s.cuda_stream)
+
+
+def _dev(t, n_elem: int):
+    import torch
+    if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and t.numel() == n_elem):
+        raise StepsError(f"expected a contiguous CUDA float64 tensor with {n_elem} elements, got "
+                         f"{tuple(t.shape)} {t.dtype} {t.device}")
+    return t.data_ptr()
+
+
+def _host(a, n_elem: int):
+    import numpy as np
+    import torch
+    if isinstance(a, torch.Tensor):
+        if a.is_cuda or a.dtype != torch.float64 or not a.is_contiguous() or a.numel() != n_elem:
+            raise StepsError("expected a contiguous CPU float64 tensor")
+        return a.data_ptr()
+    if not (isinstance(a, np.ndarray) and a.dtype == np.float64 and a.flags.c_contiguous and a.size == n_elem):
+        raise StepsError("expected a C-contiguous float64 numpy array")
+    return a.ctypes.data
+
+
+# ---- the calls of include/steps.h, same names -------------------------------------------------
+
+def steps_forces(pos, mass, soft, acc, stream=None) -> None:
+    n = mass.numel()
+    _check(lib().steps_forces(_dev(pos, 3 * n), _dev(mass, n), _dev(soft, n), n, _dev(acc, 3 * n), _stream(stream)))
+
+
+def steps_forces_mixed(pos, mass, soft, acc, stream=None) -> None:
+    n = mass.numel()
+    _check(lib().steps_forces_mixed(_dev(pos, 3 * n), _dev(mass, n), _dev(soft, n), n, _dev(acc, 3 * n),
+                                    _stream(stream)))
+
+
+def steps_forces_range(pos, mass, soft, i_begin: int, i_end: int, acc_out, mixed: bool = False, stream=None) -> None:
+    n = mass.numel()
+    _check(lib().steps_forces_range(_dev(pos, 3 * n), _dev(mass, n), _dev(soft, n), n, i_begin, i_end,
+                                    _dev(acc_out, 3 * (i_end - i_begin)), int(mixed), _stream(stream)))
+
+
+def steps_forces_host(pos_host, mass_host, soft_host, acc_host, mixed: bool = False, stream=None) -> None:
+    n = int(mass_host.size if hasattr(mass_host, "size") and not callable(mass_host.size) else mass_host.numel())
+    _check(lib().steps_forces_host(_host(pos_host, 3 * n), _host(mass_host, n), _host(soft_host, n), n,
+                                   _host(acc_host, 3 * n), int(mixed), _stream(stream)))
+
+
+def steps_kick_drift(pos, vel, acc, coeffs: KdkCoeffs, stream=None) -> None:
+    n = pos.numel() // 3
+    _check(lib().steps_kick_drift(_dev(pos, 3 * n), _dev(vel, 3 * n), _dev(acc, 3 * n), n, C.byref(coeffs),
+                                  _stream(stream)))
+
+
+def steps_kdk_step(pos, vel, acc, mass, soft, coeffs: KdkCoeffs, stream=None) -> None:
+    n = mass.numel()
+    _check(lib().steps_kdk_step(_dev(pos, 3 * n), _dev(vel, 3 * n), _dev(acc, 3 * n), _dev(mass, n), _dev(soft, n),
+                                n, C.byref(coeffs), _stream(stream)))
+
+
+def steps_hubble(a: float, cosmo: Cosmology) -> float:
+    return lib().steps_hubble(a, C.byref(cosmo))
+
+
+def steps_scale_factor_rk4(a: float, dt: float, cosmo: Cosmology) -> float:
+    return lib().steps_scale_factor_rk4(a, dt, C.byref(cosmo))
+
+
+def steps_kdk_schedule(a_n: float, dt: float, G: float, cosmo: Cosmology) -> dict:
+    out = (C.c_double * 6)()
+    _check(lib().steps_kdk_schedule(a_n, dt, G, C.byref(cosmo), out))
+    return dict(alpha_open=out[0], beta_open=out[1], gamma=out[2], alpha_close=out[3], beta_close=out[4],
+                a_next=out[5])
+
+
+def steps_momentum(vec, mass, out4, stream=None) -> None:
+    n = mass.numel()
+    _check(lib().steps_momentum(_dev(vec, 3 * n), _dev(mass, n), n, _dev(out4, 4), _stream(stream)))
+
+
+def steps_reserve(n: int) -> None:
+    _check(lib().steps_reserve(n))
+
+
+def steps_shutdown() -> None:
+    lib().steps_shutdown()
+
+
+def steps_workspace_bytes(n: int) -> int:
+    return int(lib().steps_workspace_bytes(n))
+
+
+def steps_version() -> int:
+    return int(lib().steps_version())
+
+
+def steps_kernel_launch_count() -> int:
+    return int(lib().steps_kernel_launch_count())
+
+
+def steps_set_option(key: str, value: int) -> None:
+    _check(lib().steps_set_option(key.encode(), value))

@@ -1,0 +1,279 @@
+"""-m gpu: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Tolerances are BASELINE.json's north_star:
+  fp64 path : max_i |a_gpu - a_ref|_2 / |a_ref|_2 <= 1e-12
+  mixed path: RMS <= 2e-6, max <= 1e-4."""
+import ctypes as C
+import math
+
+import numpy as np
+import pytest
+
+from paper_1811_05903_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+FP64_MAX = 1e-12
+MIXED_RMS, MIXED_MAX = 2e-6, 1e-4
+LCDM = dict(H0=0.0288675134594813, Omega_m=0.3, Omega_r=0.0, Omega_L=0.7, Omega_k=0.0)
+
+
+@pytest.fixture(scope="module")
+def S():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_1811_05903_b200 import steps
+    steps.lib()
+    return steps
+
+
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def gpu_forces(S, ps_or_arrays, mixed, idx=None):
+    import torch
+    pos, mass, soft = (ps_or_arrays.pos, ps_or_arrays.mass, ps_or_arrays.soft) if hasattr(ps_or_arrays, "pos") else ps_or_arrays
+    dpos, dm, dh = dev(pos), dev(mass), dev(soft)
+    acc = torch.full_like(dpos, float("nan"))
+    (S.steps_forces_mixed if mixed else S.steps_forces)(dpos, dm, dh, acc)
+    torch.cuda.synchronize()
+    out = acc.cpu().numpy()
+    return out if idx is None else out[:, idx]
+
+
+def rel_err(got, ref):
+    return np.linalg.norm(got - ref, axis=0) / np.linalg.norm(ref, axis=0)
+
+
+def check(got, ref, mixed, label=""):
+    assert np.all(np.isfinite(got)), label
+    e = rel_err(got, ref)
+    if mixed:
+        rms = math.sqrt(np.mean(e * e))
+        assert rms <= MIXED_RMS and e.max() <= MIXED_MAX, f"{label}: mixed rms {rms:.3e} max {e.max():.3e}"
+    else:
+        assert e.max() <= FP64_MAX, f"{label}: fp64 max {e.max():.3e} (rms {math.sqrt(np.mean(e*e)):.3e})"
+    return e
+
+
+@pytest.mark.parametrize("mixed", [False, True], ids=["fp64", "mixed"])
+def test_config0_forces(S, oracle, mixed):
+    ps = synth.config(0)
+    check(gpu_forces(S, ps, mixed), oracle.forces(ps.pos, ps.mass, ps.soft), mixed, "config0")
+
+
+@pytest.mark.parametrize("mixed", [False, True], ids=["fp64", "mixed"])
+def test_config1_forces_65536(S, oracle, mixed, request):
+    ps = synth.config(1)
+    ref = _oracle_cached(oracle, ps, "c1")
+    check(gpu_forces(S, ps, mixed), ref, mixed, "config1")
+
+
+_CACHE = {}
+
+
+def _oracle_cached(oracle, ps, key, idx=None):
+    if key not in _CACHE:
+        _CACHE[key] = oracle.forces(ps.pos, ps.mass, ps.soft, idx=idx)
+    return _CACHE[key]
+
+
+@pytest.mark.parametrize("mixed", [False, True], ids=["fp64", "mixed"])
+@pytest.mark.parametrize("eps0", [0.1, 1.0])
+def test_softening_stress(S, oracle, mixed, eps0):
+    """h_min inflated 10x / 100x: thousands of pairs in both softened branches of Eq. 4."""
+    ps = synth.g0(4096, seed=77, eps0=eps0)
+    d = ps.pos[:, :, None] - ps.pos[:, None, :512]
+    u = np.linalg.norm(d, axis=0) / (ps.soft[:, None] + ps.soft[None, :512])
+    assert ((u > 0) & (u < 0.5)).sum() > 50 and ((u >= 0.5) & (u < 1)).sum() > 200
+    check(gpu_forces(S, ps, mixed), oracle.forces(ps.pos, ps.mass, ps.soft), mixed, f"stress eps0={eps0}")
+
+
+@pytest.mark.parametrize("mixed", [False, True], ids=["fp64", "mixed"])
+@pytest.mark.parametrize("n", [1, 2, 3, 31, 255, 256, 257, 1000, 1025, 2049, 5000])
+def test_ragged_sizes(S, oracle, mixed, n):
+    ps = synth.g0(n, seed=1000 + n, eps0=0.05)
+    got = gpu_forces(S, ps, mixed)
+    if n == 1:
+        assert np.all(got == 0.0)
+        return
+    check(got, oracle.forces(ps.pos, ps.mass, ps.soft), mixed, f"n={n}")
+
+
+@pytest.mark.parametrize("mixed", [False, True], ids=["fp64", "mixed"])
+def test_unsorted_input_is_still_correct(S, oracle, mixed):
+    ps = synth.g0(6000, seed=5, sort=False)
+    perm = np.random.default_rng(3).permutation(ps.n)
+    arrays = (np.ascontiguousarray(ps.pos[:, perm]), ps.mass[perm].copy(), ps.soft[perm].copy())
+    check(gpu_forces(S, arrays, mixed), oracle.forces(*arrays), mixed, "unsorted")
+
+
+@pytest.mark.parametrize("mixed", [False, True], ids=["fp64", "mixed"])
+def test_coincident_particles_and_zero_softening(S, oracle, mixed):
+    rng = np.random.default_rng(9)
+    pos = rng.normal(size=(3, 600))
+    pos[:, 100] = pos[:, 7]                     # a coincident distinct pair (reading #4: contributes 0)
+    mass = rng.uniform(0.5, 1.5, 600)
+    soft = np.full(600, 0.05)
+    check(gpu_forces(S, (pos, mass, soft), mixed), oracle.forces(pos, mass, soft), mixed, "coincident")
+    soft0 = np.zeros(600)                       # pure Newtonian: h = 0 everywhere, self pair still skipped
+    pos2 = rng.normal(size=(3, 600))
+    check(gpu_forces(S, (pos2, mass, soft0), mixed), oracle.forces(pos2, mass, soft0), mixed, "h=0")
+
+
+@pytest.mark.parametrize("mixed", [False, True], ids=["fp64", "mixed"])
+def test_config2_zoom_core_sampled(S, oracle, mixed):
+    ps = synth.config(2)
+    assert ps.soft.max() / ps.soft.min() >= 100.0
+    idx = synth.stratified_sample(ps.n, 2048)
+    ref = _oracle_cached(oracle, ps, "c2", idx)
+    check(gpu_forces(S, ps, mixed, idx), ref, mixed, "config2")
+
+
+@pytest.mark.parametrize("mixed", [False, True], ids=["fp64", "mixed"])
+def test_config3_one_million_sampled(S, oracle, mixed):
+    """Full BASELINE size, in the launch configuration bench.py times; oracle on a stratified i-sample."""
+    ps = synth.config(3)
+    idx = synth.stratified_sample(ps.n, 2048)
+    ref = _oracle_cached(oracle, ps, "c3", idx)
+    check(gpu_forces(S, ps, mixed, idx), ref, mixed, "config3")
+
+
+def test_newtons_third_law_and_determinism_on_device(S):
+    import torch
+    ps = synth.config(1)
+    a1 = gpu_forces(S, ps, False)
+    a2 = gpu_forces(S, ps, False)
+    assert np.array_equal(a1, a2)               # bitwise run-to-run
+    m1, m2 = gpu_forces(S, ps, True), gpu_forces(S, ps, True)
+    assert np.array_equal(m1, m2)
+    net = np.linalg.norm(a1 @ ps.mass) / np.sum(ps.mass * np.linalg.norm(a1, axis=0))
+    assert net < 1e-13
+
+
+def test_forces_range_and_host_entry_points(S, oracle):
+    import torch
+    ps = synth.g0(5000, seed=21)
+    full = gpu_forces(S, ps, False)
+    dpos, dm, dh = dev(ps.pos), dev(ps.mass), dev(ps.soft)
+    for (b, e) in [(0, 5000), (0, 1), (4999, 5000), (1000, 3077), (2048, 2049)]:
+        out = torch.empty(3 * (e - b), dtype=torch.float64, device="cuda")
+        S.steps_forces_range(dpos, dm, dh, b, e, out, mixed=False)
+        torch.cuda.synchronize()
+        assert np.array_equal(out.cpu().numpy().reshape(3, e - b), full[:, b:e]), (b, e)
+    acc_h = np.empty((3, ps.n))
+    S.steps_forces_host(ps.pos, ps.mass, ps.soft, acc_h, mixed=False)
+    assert np.array_equal(acc_h, full)
+    acc_m = np.empty((3, ps.n))
+    S.steps_forces_host(ps.pos, ps.mass, ps.soft, acc_m, mixed=True)
+    check(acc_m, oracle.forces(ps.pos, ps.mass, ps.soft), True, "host mixed")
+    L = S.lib()
+    assert L.steps_forces(dpos.data_ptr(), dm.data_ptr(), dh.data_ptr(), 0, dpos.data_ptr(), None) == S.EINVAL
+    assert L.steps_forces(dpos.data_ptr() + 8, dm.data_ptr(), dh.data_ptr(), 10, dpos.data_ptr(), None) == S.EINVAL
+    assert L.steps_forces_range(dpos.data_ptr(), dm.data_ptr(), dh.data_ptr(), 5000, 10, 10, dpos.data_ptr(), 0, None) == S.EINVAL
+
+
+def test_config0_one_kdk_step(S, oracle):
+    """Config 0: one force evaluation plus one KDK step (first step of config 4's schedule, v = 0)."""
+    import torch
+    ps = synth.config(0)
+    B = 1.0 / ps.r_cut ** 3
+    dt = float(oracle.ln_a_schedule(1 / 51, 1.0, 200, LCDM)[0])
+    pos, vel = ps.pos.copy(), ps.vel.copy()
+    acc = oracle.forces(pos, ps.mass, ps.soft)
+    a1 = oracle.kdk_step(pos, vel, acc, ps.mass, ps.soft, 1 / 51, dt, 1.0, B, LCDM)
+
+    from paper_1811_05903_b200 import integrate
+    dpos, dvel, dm, dh = dev(ps.pos), dev(ps.vel), dev(ps.mass), dev(ps.soft)
+    dacc = torch.empty_like(dpos)
+    S.steps_forces(dpos, dm, dh, dacc)
+    a1_gpu = integrate.run_kdk(dpos, dvel, dacc, dm, dh, 1 / 51, [dt], S.Cosmology(**LCDM), 1.0, B)
+    torch.cuda.synchronize()
+    assert a1_gpu == pytest.approx(a1, rel=1e-14)
+    np.testing.assert_allclose(dpos.cpu().numpy(), pos, rtol=1e-13, atol=1e-15)
+    assert rel_err(dacc.cpu().numpy(), acc).max() <= FP64_MAX
+    assert rel_err(dvel.cpu().numpy(), vel).max() <= 1e-11
+
+
+def test_momentum_diagnostic(S, oracle):
+    import torch
+    ps = synth.config4_ics(10000, synth.SEED_BASE + 4, vel_factor=0.7)
+    out = torch.empty(4, dtype=torch.float64, device="cuda")
+    S.steps_momentum(dev(ps.vel), dev(ps.mass), out)
+    want = oracle.momentum(ps.vel, ps.mass)
+    got = out.cpu().numpy()
+    assert got[3] == pytest.approx(want[3], rel=1e-13)
+    assert np.linalg.norm(got[:3] - want[:3]) < 1e-14 * want[3]
+
+
+def _config4(oracle, n):
+    vf = oracle.hubble(1 / 51, LCDM) * oracle.growth_rate(1 / 51, LCDM)
+    return synth.config4_ics(n, synth.SEED_BASE + 4, vel_factor=vf)
+
+
+def test_config4_trajectory_vs_oracle_8192(S, oracle):
+    """200 comoving KDK steps, a: 1/51 -> 1, N = 8192: final positions against the oracle run,
+    judged against the chaos floor = oracle vs oracle with every step's force sum in reversed order
+    (SURVEY.md 8(c.5)); absolute cap 1e-6 of the local spacing."""
+    import torch
+    from paper_1811_05903_b200 import integrate
+    n = 8192
+    ps = _config4(oracle, n)
+    B = 1.0 / ps.r_cut ** 3
+    dts = oracle.ln_a_schedule(1 / 51, 1.0, 200, LCDM)
+
+    pos, vel = ps.pos.copy(), ps.vel.copy()
+    acc = oracle.forces(pos, ps.mass, ps.soft)
+    a = 1 / 51
+    for dt in dts:
+        a = oracle.kdk_step(pos, vel, acc, ps.mass, ps.soft, a, float(dt), 1.0, B, LCDM)
+
+    # chaos floor: perturb the oracle's own initial forces at the 1e-16 level by reversing the sum
+    pos2, vel2 = ps.pos.copy(), ps.vel.copy()
+    acc2 = oracle.forces(pos2, ps.mass, ps.soft, reverse_j=True)
+    a2 = 1 / 51
+    for dt in dts:
+        a2 = oracle.kdk_step(pos2, vel2, acc2, ps.mass, ps.soft, a2, float(dt), 1.0, B, LCDM)
+    floor = np.max(np.linalg.norm(pos2 - pos, axis=0) / ps.spacing)
+
+    dpos, dvel, dm, dh = dev(ps.pos), dev(ps.vel), dev(ps.mass), dev(ps.soft)
+    dacc = torch.empty_like(dpos)
+    S.steps_forces(dpos, dm, dh, dacc)
+    a_gpu = integrate.run_kdk(dpos, dvel, dacc, dm, dh, 1 / 51, dts, S.Cosmology(**LCDM), 1.0, B)
+    torch.cuda.synchronize()
+    assert a_gpu == pytest.approx(a, rel=1e-12) and a == pytest.approx(1.0, rel=1e-8)
+    dev_pos = np.max(np.linalg.norm(dpos.cpu().numpy() - pos, axis=0) / ps.spacing)
+    print(f"config4 N={n}: max |dx|/s GPU-vs-oracle {dev_pos:.3e}, chaos floor {floor:.3e}")
+    assert dev_pos <= 1e-6
+    assert dev_pos <= max(1000 * floor, 1e-9)
+    p = oracle.momentum(dvel.cpu().numpy(), ps.mass)
+    assert np.linalg.norm(p[:3]) / p[3] <= 1e-10
+
+
+def test_config4_momentum_drift_262144(S, oracle):
+    """Config 4 at its full size: total momentum drift <= 1e-10 relative in fp64 through 200 steps."""
+    import torch
+    from paper_1811_05903_b200 import integrate
+    ps = _config4(oracle, 262144)
+    B = 1.0 / ps.r_cut ** 3
+    dts = oracle.ln_a_schedule(1 / 51, 1.0, 200, LCDM)
+    dpos, dvel, dm, dh = dev(ps.pos), dev(ps.vel), dev(ps.mass), dev(ps.soft)
+    dacc = torch.empty_like(dpos)
+    out = torch.empty(4, dtype=torch.float64, device="cuda")
+    S.steps_forces(dpos, dm, dh, dacc)
+    worst = []
+
+    def on_step(k, a):
+        if k % 20 == 19:
+            S.steps_momentum(dvel, dm, out)
+            o = out.cpu().numpy()
+            worst.append(np.linalg.norm(o[:3]) / o[3])
+
+    integrate.run_kdk(dpos, dvel, dacc, dm, dh, 1 / 51, dts, S.Cosmology(**LCDM), 1.0, B, on_step=on_step)
+    S.steps_momentum(dvel, dm, out)
+    o = out.cpu().numpy()
+    worst.append(np.linalg.norm(o[:3]) / o[3])
+    print("config4 N=262144 momentum |P|/sum m|v| per 20 steps:", ["%.2e" % w for w in worst])
+    assert np.all(np.isfinite(dpos.cpu().numpy()))
+    assert max(worst) <= 1e-10
