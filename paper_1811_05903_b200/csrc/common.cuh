@@ -19,10 +19,6 @@ constexpr int WARP_I = 32 * R_I;          // contiguous i-particles owned by one
 // any sane |x_i|; if it overflows, rsqrt(inf) = 0 and the term is still exactly 0.
 #define STEPS_PAD_POS 1.0e18
 
-// MQ_SCALE = 1.5^-1.5: the fp64 far body works with the scaled seed Y0 = sqrt(1.5)/r, so the
-// mass is pre-divided by Y0^3/y0^3 once per particle by the prep kernel (one rounding, ~1e-16).
-#define STEPS_MQ_SCALE 0.54433105395181735517
-
 // ---- j-tile records (built by the prep kernels, streamed to shared memory as ONE bulk copy) ----
 // Radial interval and largest softening of the REAL particles in the tile (pads excluded),
 // rounded outwards, used for the far/near classification (triangle inequality:
@@ -35,7 +31,7 @@ struct alignas(16) TileF32 {              // mixed path: 5136 B
     TileMeta meta;
 };
 struct alignas(16) TileF64 {              // fp64 path: 10256 B
-    double x[TJ], y[TJ], z[TJ], mq[TJ];   // mq = m / 1.5^1.5 (see force_fp64.cuh)
+    double x[TJ], y[TJ], z[TJ], m[TJ];
     double h[TJ];
     TileMeta meta;
 };

@@ -1,0 +1,232 @@
+// force_driver.cuh -- the two force drivers that move j-tiles past register-blocked i-particles.
+//
+//  forces_persistent_kernel  (default): persistent CTAs (grid = SMs x resident CTAs), the
+//      (i-block, j-tile) iteration space is linearised and cut into equal contiguous shares
+//      ("stream-K"), so every CTA streams the same number of tiles no matter how N divides.
+//      j-tiles arrive in shared memory by 1-D bulk TMA copies (cp.async.bulk -> UBLKCP in SASS)
+//      through a STAGES-deep mbarrier ring; one elected thread is the producer.  A CTA whose
+//      share crosses an i-block boundary writes one partial record per i-block it touched;
+//      forces_reduce_kernel sums the records of each i-block in fixed CTA order (deterministic).
+//  forces_v1_kernel: one CTA per i-block, plain loads + __syncthreads.  Kept as the in-library
+//      cross-check of the persistent driver (steps_set_option("driver", 1)).
+//
+// Both share the Path bodies (force_mixed.cuh / force_fp64.cuh) and the per-thread accumulator
+// block in shared memory: element (c, k) of thread t at acc[(c * R_I + k) * CTA_THREADS + t].
+#pragma once
+#include "common.cuh"
+
+namespace steps {
+
+// ---- mbarrier / bulk-copy PTX ------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra LAB_DONE;\n"
+        "bra LAB_WAIT;\n"
+        "LAB_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// 1-D bulk copy global -> shared, completion signalled on an mbarrier (TMA engine, no tensor map).
+__device__ __forceinline__ void bulk_load(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// ---- shared helpers ----------------------------------------------------------------------------
+template <typename Path>
+__device__ __forceinline__ void load_i_block(typename Path::IState& S, const double* __restrict__ pos,
+                                             const double* __restrict__ soft, long long N, long long i0,
+                                             long long i_end, float& rlo, float& rhi, float& hh)
+{
+    long long idx[R_I];
+#pragma unroll
+    for (int k = 0; k < R_I; ++k) {
+        const long long i = i0 + 32 * k;
+        idx[k] = i < i_end ? i : i_end - 1;     // clamp: duplicates a real particle, result not stored
+    }
+    rlo = __int_as_float(0x7f800000); rhi = 0.0f; hh = 0.0f;
+    Path::load_i(S, pos, soft, N, idx, rlo, rhi, hh);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {          // bounds of the warp's 128 contiguous i-particles
+        rlo = fminf(rlo, __shfl_xor_sync(0xffffffffu, rlo, o));
+        rhi = fmaxf(rhi, __shfl_xor_sync(0xffffffffu, rhi, o));
+        hh = fmaxf(hh, __shfl_xor_sync(0xffffffffu, hh, o));
+    }
+}
+
+__host__ __device__ constexpr int stage_stride(int tile_bytes) { return (tile_bytes + 127) / 128 * 128; }
+
+template <typename Path, int STAGES>
+constexpr int persistent_smem_bytes()
+{
+    return STAGES * stage_stride((int)sizeof(typename Path::Tile)) + Path::NOUT * R_I * CTA_THREADS * (int)sizeof(double);
+}
+
+// ---- persistent stream-K driver ------------------------------------------------------------------
+// partials: [nb + gridDim.x slots][Path::NOUT][IB] doubles; CTA p's record for i-block b is slot b + p.
+template <typename Path, int STAGES>
+__global__ void __launch_bounds__(CTA_THREADS, 2)
+forces_persistent_kernel(const double* __restrict__ pos, const double* __restrict__ soft, long long N,
+                         const typename Path::Tile* __restrict__ tiles, int nt, long long i_begin, long long i_end,
+                         int nb, double* __restrict__ partials)
+{
+    using Tile = typename Path::Tile;
+    constexpr int STRIDE = stage_stride((int)sizeof(Tile));
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ uint64_t full_bar[STAGES], empty_bar[STAGES];
+    double* acc = reinterpret_cast<double*>(smem_raw + STAGES * STRIDE) + threadIdx.x;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const long long W = (long long)nb * nt;
+    const long long w0 = (long long)blockIdx.x * W / gridDim.x;
+    const long long w1 = ((long long)blockIdx.x + 1) * W / gridDim.x;
+    const int total = (int)(w1 - w0);                       // tiles this CTA streams
+    if (total <= 0) return;
+
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < STAGES; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], CTA_THREADS / 32); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    // producer (thread 0): tile number k of this CTA's stream is tiles[(w0 + k) % nt], stage k % STAGES
+    auto produce = [&](int k) {
+        const int s = k % STAGES;
+        if (k >= STAGES) mbar_wait(&empty_bar[s], ((k / STAGES) - 1) & 1);
+        mbar_expect_tx(&full_bar[s], (uint32_t)sizeof(Tile));
+        bulk_load(smem_raw + s * STRIDE, tiles + (w0 + k) % nt, (uint32_t)sizeof(Tile), &full_bar[s]);
+    };
+    if (threadIdx.x == 0) {
+        for (int k = 0; k < STAGES - 1 && k < total; ++k) produce(k);
+    }
+
+    int it = 0;                                             // tiles consumed so far
+    long long w = w0;
+    while (w < w1) {
+        const int b = (int)(w / nt);
+        const int t0 = (int)(w - (long long)b * nt);
+        const int cnt = (int)min((long long)(nt - t0), w1 - w);
+
+        typename Path::IState S;
+        float rlo, rhi, hh;
+        const long long i0 = i_begin + (long long)b * IB + warp * WARP_I + lane;
+        load_i_block<Path>(S, pos, soft, N, i0, i_end, rlo, rhi, hh);
+#pragma unroll
+        for (int q = 0; q < Path::NOUT * R_I; ++q) acc[q * CTA_THREADS] = 0.0;
+
+        for (int c = 0; c < cnt; ++c, ++it) {
+            if (threadIdx.x == 0 && it + STAGES - 1 < total) produce(it + STAGES - 1);
+            const int s = it % STAGES;
+            mbar_wait(&full_bar[s], (it / STAGES) & 1);
+            const Tile& T = *reinterpret_cast<const Tile*>(smem_raw + s * STRIDE);
+            if (tile_is_far(rlo, rhi, hh, T.meta)) Path::far(T, S, acc);
+            else Path::near(T, S, acc);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty_bar[s]);
+        }
+
+        double* out = partials + ((long long)(b + blockIdx.x) * Path::NOUT) * IB + warp * WARP_I + lane;
+#pragma unroll
+        for (int cc = 0; cc < Path::NOUT; ++cc)
+#pragma unroll
+            for (int k = 0; k < R_I; ++k) out[(long long)cc * IB + 32 * k] = acc[(cc * R_I + k) * CTA_THREADS];
+        w += cnt;
+    }
+}
+
+// Fixed-order sum of the partial records of each i-block -> acc_out (SoA over [i_begin, i_end)).
+template <int NOUT>
+__global__ void __launch_bounds__(256) forces_reduce_kernel(const double* __restrict__ partials, int nt, int nb, int P,
+                                                            long long cnt, double* __restrict__ acc_out)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= cnt) return;
+    const int b = (int)(i / IB), off = (int)(i - (long long)b * IB);
+    const long long W = (long long)nb * nt;
+    // CTA p owns w in [floor(p W / P), floor((p+1) W / P));  the CTA that owns w is floor(((w+1) P - 1) / W)
+    const int p_lo = (int)((((long long)b * nt + 1) * P - 1) / W);
+    const int p_hi = (int)((((long long)(b + 1) * nt) * P - 1) / W);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        double hi = 0.0, lo = 0.0;
+        for (int p = p_lo; p <= p_hi; ++p) {
+            const long long w0 = (long long)p * W / P, w1 = ((long long)p + 1) * W / P;
+            if (w1 <= w0) continue;                                    // idle CTA wrote nothing
+            const double* rec = partials + ((long long)(b + p) * NOUT) * IB + off;
+            const double v = rec[(long long)c * IB];
+            const double s = hi + v, bb = s - hi;
+            lo += (hi - (s - bb)) + (v - bb);                          // TwoSum
+            hi = s;
+            if (NOUT == 6) lo += rec[(long long)(3 + c) * IB];
+        }
+        acc_out[(long long)c * cnt + i] = hi + lo;
+    }
+}
+
+// ---- simple driver (cross-check) -----------------------------------------------------------------
+template <typename Path>
+__global__ void __launch_bounds__(CTA_THREADS, 2)
+forces_v1_kernel(const double* __restrict__ pos, const double* __restrict__ soft, long long N,
+                 const typename Path::Tile* __restrict__ tiles, int ntiles, long long i_begin, long long i_end,
+                 double* __restrict__ acc_out)
+{
+    using Tile = typename Path::Tile;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    Tile& tile = *reinterpret_cast<Tile*>(smem_raw);
+    double* acc = reinterpret_cast<double*>(smem_raw + stage_stride((int)sizeof(Tile))) + threadIdx.x;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const long long i0 = i_begin + (long long)blockIdx.x * IB + (long long)warp * WARP_I + lane;
+    typename Path::IState S;
+    float rlo, rhi, hh;
+    load_i_block<Path>(S, pos, soft, N, i0, i_end, rlo, rhi, hh);
+#pragma unroll
+    for (int q = 0; q < Path::NOUT * R_I; ++q) acc[q * CTA_THREADS] = 0.0;
+    for (int t = 0; t < ntiles; ++t) {
+        __syncthreads();
+        {
+            const uint4* src = reinterpret_cast<const uint4*>(tiles + t);
+            uint4* dst = reinterpret_cast<uint4*>(&tile);
+            for (int q = threadIdx.x; q < (int)(sizeof(Tile) / 16); q += CTA_THREADS) dst[q] = src[q];
+        }
+        __syncthreads();
+        if (tile_is_far(rlo, rhi, hh, tile.meta)) Path::far(tile, S, acc);
+        else Path::near(tile, S, acc);
+    }
+    const long long cnt = i_end - i_begin;
+#pragma unroll
+    for (int k = 0; k < R_I; ++k) {
+        const long long i = i0 + 32 * k;
+        if (i < i_end) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                double v = acc[(c * R_I + k) * CTA_THREADS];
+                if (Path::NOUT == 6) v += acc[((3 + c) * R_I + k) * CTA_THREADS];
+                acc_out[(long long)c * cnt + (i - i_begin)] = v;
+            }
+        }
+    }
+}
+
+}  // namespace steps

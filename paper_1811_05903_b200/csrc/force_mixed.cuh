@@ -33,10 +33,18 @@ __device__ __noinline__ float spline_g_soft_from_f32(float r2, float hs)
 struct MixedPath {
     using Tile = TileF32;
 
+    static constexpr int NOUT = 3;            // doubles per i-particle in the accumulator / partial record
+
     struct IState {
         float x[R_I], y[R_I], z[R_I], h[R_I];
-        double ax[R_I], ay[R_I], az[R_I];
     };
+
+    // acc: this thread's fp64 accumulators in shared memory, element (c, k) at acc[(c * R_I + k) * CTA_THREADS].
+    static __device__ __forceinline__ void flush(double* acc, int c, int k, float partial)
+    {
+        double* a = acc + (c * R_I + k) * CTA_THREADS;
+        *a += (double)partial;
+    }
 
     // Loads the thread's R_I i-particles (indices already clamped into [0, N)).
     static __device__ __forceinline__ void load_i(IState& S, const double* __restrict__ pos,
@@ -47,7 +55,6 @@ struct MixedPath {
         for (int k = 0; k < R_I; ++k) {
             const double x = pos[idx[k]], y = pos[N + idx[k]], z = pos[2 * N + idx[k]], h = soft[idx[k]];
             S.x[k] = (float)x; S.y[k] = (float)y; S.z[k] = (float)z; S.h[k] = (float)h;
-            S.ax[k] = S.ay[k] = S.az[k] = 0.0;
             const double r = sqrt(x * x + y * y + z * z);
             rlo = fminf(rlo, __double2float_rd(r));
             rhi = fmaxf(rhi, __double2float_ru(r));
@@ -70,7 +77,7 @@ struct MixedPath {
         az = fma2(dz, s, az);
     }
 
-    static __device__ __forceinline__ void far(const Tile& T, IState& S)
+    static __device__ __forceinline__ void far(const Tile& T, const IState& S, double* acc)
     {
         u64 xi[R_I], yi[R_I], zi[R_I], ax[R_I], ay[R_I], az[R_I];
 #pragma unroll
@@ -93,13 +100,13 @@ struct MixedPath {
 #pragma unroll
         for (int k = 0; k < R_I; ++k) {
             float lo, hi;
-            unpack2(ax[k], lo, hi); S.ax[k] += (double)(lo + hi);
-            unpack2(ay[k], lo, hi); S.ay[k] += (double)(lo + hi);
-            unpack2(az[k], lo, hi); S.az[k] += (double)(lo + hi);
+            unpack2(ax[k], lo, hi); flush(acc, 0, k, lo + hi);
+            unpack2(ay[k], lo, hi); flush(acc, 1, k, lo + hi);
+            unpack2(az[k], lo, hi); flush(acc, 2, k, lo + hi);
         }
     }
 
-    static __device__ __forceinline__ void near(const Tile& T, IState& S)
+    static __device__ __forceinline__ void near(const Tile& T, const IState& S, double* acc)
     {
         float ax[R_I], ay[R_I], az[R_I];
 #pragma unroll
@@ -123,7 +130,7 @@ struct MixedPath {
         }
 #pragma unroll
         for (int k = 0; k < R_I; ++k) {
-            S.ax[k] += (double)ax[k]; S.ay[k] += (double)ay[k]; S.az[k] += (double)az[k];
+            flush(acc, 0, k, ax[k]); flush(acc, 1, k, ay[k]); flush(acc, 2, k, az[k]);
         }
     }
 };

@@ -43,7 +43,7 @@ __global__ void __launch_bounds__(TJ) prep_tiles(const double* __restrict__ pos,
         T.m[threadIdx.x] = (float)m; T.h[threadIdx.x] = (float)h;
     } else {
         T.x[threadIdx.x] = x; T.y[threadIdx.x] = y; T.z[threadIdx.x] = z;
-        T.mq[threadIdx.x] = m * STEPS_MQ_SCALE; T.h[threadIdx.x] = h;
+        T.m[threadIdx.x] = m; T.h[threadIdx.x] = h;
     }
     const double r = sqrt(x * x + y * y + z * z);
     float rlo = real ? __double2float_rd(r) : __int_as_float(0x7f800000);

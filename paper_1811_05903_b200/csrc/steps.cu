@@ -12,7 +12,7 @@
 #include "prep.cuh"
 #include "force_mixed.cuh"
 #include "force_fp64.cuh"
-#include "force_v1.cuh"
+#include "force_driver.cuh"
 #include "kdk.cuh"
 
 using namespace steps;
@@ -24,10 +24,15 @@ thread_local int g_last_cuda_error = 0;
 std::atomic<int> g_driver{0};   // 0 = default, 1 = simple v1 driver (cross-check)
 
 constexpr int MAX_DEVICES = 16;
+constexpr int STAGES = 4;
+constexpr int MAX_GRID = 148 * 4;
 
 struct Workspace {
     void* tiles = nullptr;          // max(sizeof(TileF32), sizeof(TileF64)) * ntiles
+    double* partials = nullptr;     // (nb + grid) * 6 * IB doubles (persistent driver's split-j records)
     long long cap_particles = 0;
+    int num_sms = 0;
+    int grid_mixed = 0, grid_fp64 = 0;   // persistent grids: SMs x resident CTAs
     double* mom_partial = nullptr;  // MOM_BLOCKS * 4
     // staging buffers of steps_forces_host
     double* h_pos = nullptr; double* h_mass = nullptr; double* h_soft = nullptr; double* h_acc = nullptr;
@@ -38,6 +43,8 @@ Workspace g_ws[MAX_DEVICES];
 std::mutex g_mutex;
 
 inline long long ntiles_of(long long N) { return (N + TJ - 1) / TJ; }
+inline long long nblocks_of(long long cnt) { return (cnt + IB - 1) / IB; }
+inline size_t partial_bytes(long long N) { return sizeof(double) * 6 * IB * (size_t)(nblocks_of(N) + MAX_GRID); }
 
 int cuda_fail(cudaError_t e)
 {
@@ -59,6 +66,7 @@ int current_device(int* dev)
         int major = 0;
         STEPS_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, *dev));
         w.cc_major = major;
+        STEPS_CUDA(cudaDeviceGetAttribute(&w.num_sms, cudaDevAttrMultiProcessorCount, *dev));
     }
     if (w.cc_major != 10) return STEPS_EUNSUPPORTED;   // sm_100a cubin only
     return STEPS_OK;
@@ -72,10 +80,12 @@ int ensure_workspace(int dev, long long N)
         if (cudaMalloc(&w.mom_partial, sizeof(double) * MOM_BLOCKS * 4) != cudaSuccess) return STEPS_ENOMEM;
     }
     if (N <= w.cap_particles) return STEPS_OK;
-    if (w.tiles) { cudaFree(w.tiles); w.tiles = nullptr; w.cap_particles = 0; }
+    if (w.tiles) { cudaFree(w.tiles); cudaFree(w.partials); w.tiles = nullptr; w.partials = nullptr; w.cap_particles = 0; }
     const size_t tile_bytes = sizeof(TileF64) > sizeof(TileF32) ? sizeof(TileF64) : sizeof(TileF32);
-    if (cudaMalloc(&w.tiles, tile_bytes * (size_t)ntiles_of(N)) != cudaSuccess) {
+    if (cudaMalloc(&w.tiles, tile_bytes * (size_t)ntiles_of(N)) != cudaSuccess ||
+        cudaMalloc(&w.partials, partial_bytes(N)) != cudaSuccess) {
         cudaGetLastError();
+        cudaFree(w.tiles); w.tiles = nullptr;
         return STEPS_ENOMEM;
     }
     w.cap_particles = ntiles_of(N) * TJ;
@@ -86,7 +96,7 @@ bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) !
 
 template <typename Path>
 int launch_forces(const double* pos, const double* mass, const double* soft, long long N, long long i_begin,
-                  long long i_end, double* acc_out, cudaStream_t st, Workspace& w)
+                  long long i_end, double* acc_out, cudaStream_t st, Workspace& w, int& grid_cache)
 {
     using Tile = typename Path::Tile;
     const int nt = (int)ntiles_of(N);
@@ -94,9 +104,28 @@ int launch_forces(const double* pos, const double* mass, const double* soft, lon
     prep_tiles<Tile><<<nt, TJ, 0, st>>>(pos, mass, soft, N, tiles);
     g_launches++;
     const long long cnt = i_end - i_begin;
-    const int nblk = (int)((cnt + IB - 1) / IB);
-    forces_v1_kernel<Path><<<nblk, CTA_THREADS, 0, st>>>(pos, soft, N, tiles, nt, i_begin, i_end, acc_out);
-    g_launches++;
+    const int nb = (int)nblocks_of(cnt);
+    if (g_driver.load() == 1) {
+        const int smem = stage_stride((int)sizeof(Tile)) + Path::NOUT * R_I * CTA_THREADS * (int)sizeof(double);
+        STEPS_CUDA(cudaFuncSetAttribute(forces_v1_kernel<Path>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        forces_v1_kernel<Path><<<nb, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, i_begin, i_end, acc_out);
+        g_launches++;
+    } else {
+        constexpr int smem = persistent_smem_bytes<Path, STAGES>();
+        auto kern = forces_persistent_kernel<Path, STAGES>;
+        if (grid_cache == 0) {
+            STEPS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            int per_sm = 0;
+            STEPS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, CTA_THREADS, smem));
+            if (per_sm < 1) return STEPS_EUNSUPPORTED;
+            int g = w.num_sms * per_sm;
+            grid_cache = g > MAX_GRID ? MAX_GRID : g;
+        }
+        const int P = grid_cache;
+        kern<<<P, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, i_begin, i_end, nb, w.partials);
+        forces_reduce_kernel<Path::NOUT><<<(int)((cnt + 255) / 256), 256, 0, st>>>(w.partials, nt, nb, P, cnt, acc_out);
+        g_launches += 2;
+    }
     STEPS_CUDA(cudaGetLastError());
     return STEPS_OK;
 }
@@ -114,8 +143,9 @@ int forces_impl(const double* pos, const double* mass, const double* soft, long 
     rc = ensure_workspace(dev, N);
     if (rc != STEPS_OK) return rc;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-    return mixed ? launch_forces<MixedPath>(pos, mass, soft, N, i_begin, i_end, acc_out, st, g_ws[dev])
-                 : launch_forces<Fp64Path>(pos, mass, soft, N, i_begin, i_end, acc_out, st, g_ws[dev]);
+    Workspace& w = g_ws[dev];
+    return mixed ? launch_forces<MixedPath>(pos, mass, soft, N, i_begin, i_end, acc_out, st, w, w.grid_mixed)
+                 : launch_forces<Fp64Path>(pos, mass, soft, N, i_begin, i_end, acc_out, st, w, w.grid_fp64);
 }
 
 }  // namespace
@@ -264,7 +294,7 @@ void steps_shutdown(void)
         Workspace& w = g_ws[d];
         if (!w.tiles && !w.mom_partial && !w.h_pos) continue;
         cudaSetDevice(d);
-        cudaFree(w.tiles); cudaFree(w.mom_partial);
+        cudaFree(w.tiles); cudaFree(w.partials); cudaFree(w.mom_partial);
         cudaFree(w.h_pos); cudaFree(w.h_mass); cudaFree(w.h_soft); cudaFree(w.h_acc);
         w = Workspace();
     }
@@ -275,7 +305,7 @@ long long steps_workspace_bytes(long long N)
 {
     if (N < 1) return 0;
     const size_t tile_bytes = sizeof(TileF64) > sizeof(TileF32) ? sizeof(TileF64) : sizeof(TileF32);
-    return (long long)(tile_bytes * (size_t)ntiles_of(N) + sizeof(double) * MOM_BLOCKS * 4);
+    return (long long)(tile_bytes * (size_t)ntiles_of(N) + partial_bytes(N) + sizeof(double) * MOM_BLOCKS * 4);
 }
 
 const char* steps_strerror(int code)
