@@ -1,0 +1,320 @@
+#!/usr/bin/env python
+"""bench.py -- BASELINE.json's metric: ordered pairwise interactions/s per force evaluation at
+N = 1,048,576 (config 3), and the fraction of the FP32 (mixed path) / FP64 (fp64 path) peak.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl native|reference] [--n N_PARTICLES]
+
+A "step" is one pass of the whole hot path through the C ABI: steps_kdk_step (fused kick/drift,
+tile prep, the O(N^2) force kernel, the split-j reduce) plus the momentum diagnostic -- rows
+a0-a7 of SURVEY.md 8(a); a6 is a handful of host doubles.  Both paths are timed; `value` is the
+mixed path (the FP32 target), `paths.fp64` carries the fp64 path.  One JSON line on stdout.
+
+  * inputs resident in HBM for `value`; `e2e` goes through steps_forces_host with pinned HOST
+    buffers (H2D of pos/mass/soft and D2H of acc inside the timed region);
+  * every step is bracketed by CUDA events on the launch stream, L2 is flushed (256 MiB write)
+    between timed steps, >= 3 warm-up steps; the force kernel alone is bracketed by the library
+    ("profile" option) for the roofline figure;
+  * clocks / throttle reasons are sampled through NVML during the timed region;
+  * `cpu_baseline` / `--impl reference`: the CPU oracle as it stands, on a bounded i-sample.
+  * N > 1 GPUs (torchrun): the paper's decomposition (L139) -- each rank evaluates the forces of
+    its i-range against all sources (steps_forces_range), kicks/drifts its slice, and the drifted
+    positions are all-gathered (NCCL): total work fixed => "strong" scaling.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+FLOP_PER_INTERACTION = 20.0      # stated convention
+SM_COUNT, SM_MAX_MHZ = 148, 1965.0
+PEAK_FP32_TFLOPS = SM_COUNT * 128 * 2 * SM_MAX_MHZ * 1e6 / 1e12     # 74.45
+PEAK_FP64_TFLOPS = SM_COUNT * 64 * 2 * SM_MAX_MHZ * 1e6 / 1e12      # 37.22 (64 FP64 lanes/SM, measured)
+METRIC = "pairwise interactions/s per force eval at N=1M"
+UNIT = "interactions/s"
+LCDM = dict(H0=0.0288675134594813, Omega_m=0.3, Omega_r=0.0, Omega_L=0.7, Omega_k=0.0)
+# DRAM bytes per launch of the force kernel from the committed `ncu --set full` capture
+# (profiles/r01_force_kernels_ncu.md); None until captured.
+NCU_DRAM_BYTES = {"mixed": None, "fp64": None}
+
+
+class ClockSampler:
+    """NVML sampler thread: SM clock and throttle reasons while the timed region runs."""
+
+    def __init__(self, index: int, period: float = 0.1):
+        self.samples, self.reasons, self.period, self._stop = [], set(), period, threading.Event()
+        self.max_mhz, self.ok = None, False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            pass
+        self.t = threading.Thread(target=self._run, daemon=True)
+
+    def _run(self):
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def __enter__(self):
+        if self.ok:
+            self.t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self.ok:
+            self.t.join(timeout=2)
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["nvml unavailable"]}
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(s)}
+
+
+def cpu_oracle_rate(ps, budget_s: float = 12.0):
+    """The oracle as it stands on this host's cores, on a bounded stratified i-sample x all j."""
+    from oracle import steps_oracle as oracle
+    from paper_1811_05903_b200 import synth
+    n = ps.n
+    probe = synth.stratified_sample(n, max(64, min(n, 4 * oracle.num_threads() * 16)))
+    t0 = time.perf_counter()
+    oracle.forces(ps.pos, ps.mass, ps.soft, idx=probe)
+    dt = time.perf_counter() - t0
+    rate = len(probe) * (n - 1.0) / dt
+    n_idx = int(min(n, max(len(probe), budget_s * rate / (n - 1.0))))
+    idx = synth.stratified_sample(n, n_idx)
+    t0 = time.perf_counter()
+    oracle.forces(ps.pos, ps.mass, ps.soft, idx=idx)
+    dt = time.perf_counter() - t0
+    return {"value": len(idx) * (n - 1.0) / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"{len(idx)} stratified i-particles x all {n} sources of the same workload, {dt:.1f} s"}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle (fp64 pairwise spline sum), each step a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import steps_oracle as oracle
+    from paper_1811_05903_b200 import synth
+    n = args.n or 1048576
+    ps = synth.g0(n, synth.SEED_BASE + 3)
+    per_step = max(64, min(n, int(args.ref_pairs / n)))
+    idx = synth.stratified_sample(n, per_step)
+    for _ in range(args.warmup):
+        oracle.forces(ps.pos, ps.mass, ps.soft, idx=idx[: max(16, len(idx) // 8)])
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.forces(ps.pos, ps.mass, ps.soft, idx=idx)
+    dt = time.perf_counter() - t0
+    value = args.steps * len(idx) * (n - 1.0) / dt
+    sample = f"{len(idx)} stratified i-particles x all {n} sources per step"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"config3: compactified g0 set, N={n}, CPU oracle on a bounded i-sample", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="native", choices=["native", "reference"])
+    ap.add_argument("--n", type=int, default=0, help="override the particle count (default: config 3, 1,048,576)")
+    ap.add_argument("--paths", default="mixed,fp64")
+    ap.add_argument("--ref-pairs", type=float, default=4e9, help="--impl reference: pair budget per step")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    from paper_1811_05903_b200 import shard, synth
+    from paper_1811_05903_b200 import steps as S
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    args.warmup = max(args.warmup, 3)
+
+    n = args.n or 1048576
+    ps = synth.g0(n, synth.SEED_BASE + 3)          # config 3 (identical on every rank: seeded)
+    b, e = shard.i_range(rank, world, n)
+    cnt = e - b
+    pos = torch.from_numpy(ps.pos).cuda()           # replicated sources
+    mass, soft = torch.from_numpy(ps.mass).cuda(), torch.from_numpy(ps.soft).cuda()
+    S.steps_reserve(n)
+    S.steps_set_option("profile", 1)
+    flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    mom = torch.empty(4, dtype=torch.float64, device="cuda")
+    cosmo = S.Cosmology(**LCDM)
+    B = 1.0 / ps.r_cut ** 3
+    sched = S.steps_kdk_schedule(1.0 / 51.0, 1.0e-3, 1.0, cosmo)
+    stream = torch.cuda.current_stream()
+    inter_step = float(n) * (n - 1.0)               # ordered pairs of one whole-job force evaluation
+    paths = [p for p in args.paths.split(",") if p in ("mixed", "fp64")]
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    results, launches_total = {}, 0
+    sampler = ClockSampler(local_rank)
+    with sampler:
+        for path in paths:
+            mixed = path == "mixed"
+            x = pos.clone()
+            co = S.KdkCoeffs(1.0, 0.0, sched["alpha_open"], sched["beta_open"], sched["gamma"], B, int(mixed))
+            if world == 1:
+                v, acc = torch.zeros_like(x), torch.empty_like(x)
+                (S.steps_forces_mixed if mixed else S.steps_forces)(x, mass, soft, acc)
+
+                def step():
+                    S.steps_kdk_step(x, v, acc, mass, soft, co)
+                    S.steps_momentum(v, mass, mom)
+            else:
+                xl = x[:, b:e].contiguous()
+                vl, al = torch.zeros_like(xl), torch.empty(3 * cnt, dtype=torch.float64, device="cuda")
+                ml = mass[b:e].contiguous()
+                S.steps_forces_range(x, mass, soft, b, e, al, mixed=mixed)
+                state = {"x": x}
+
+                def step():
+                    S.steps_kick_drift(xl, vl, al, co)
+                    state["x"] = shard.gather_soa(xl, n)
+                    S.steps_forces_range(state["x"], mass, soft, b, e, al, mixed=mixed)
+                    S.steps_momentum(vl, ml, mom)
+
+            for _ in range(args.warmup):
+                step()
+            barrier()
+            l0 = S.steps_kernel_launch_count()
+            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+            kernel_ms = []
+            for k in range(args.steps):
+                flush_buf.fill_(k & 0xFF)                       # L2 flush between timed steps (outside the events)
+                ev[k][0].record(stream)
+                step()
+                ev[k][1].record(stream)
+                ev[k][1].synchronize()
+                kernel_ms.append(S.steps_last_force_kernel_ms())
+            barrier()
+            launches = S.steps_kernel_launch_count() - l0
+            t_ms = torch.tensor([sum(a.elapsed_time(c) for a, c in ev)], dtype=torch.float64, device="cuda")
+            if world > 1:
+                dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
+            total_ms = float(t_ms.item())
+            k_ms = sum(kernel_ms) / len(kernel_ms)
+            peak = PEAK_FP32_TFLOPS if mixed else PEAK_FP64_TFLOPS
+            kern_inter = float(cnt) * (n - 1.0)                 # this rank's launch
+            achieved = FLOP_PER_INTERACTION * kern_inter / (k_ms * 1e-3) / 1e12
+            results[path] = {
+                "value": args.steps * inter_step / (total_ms * 1e-3), "unit": UNIT,
+                "ms_per_step": total_ms / args.steps, "force_kernel_ms": k_ms, "gpu_launches": int(launches),
+                "dtype": "f32 pairs, f64 accumulate" if mixed else "f64",
+                "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                             "frac": achieved / peak, "traffic": NCU_DRAM_BYTES[path],
+                             "flop_per_interaction": FLOP_PER_INTERACTION,
+                             "peak_source": "148 SM x %d lanes x 2 x 1965 MHz (DESIGN.md; lanes/SM measured)" % (128 if mixed else 64),
+                             "kernel": "forces_persistent_kernel<%s>" % ("MixedPath" if mixed else "Fp64Path"),
+                             "kernel_share_of_step": k_ms * args.steps / total_ms},
+            }
+            launches_total += launches
+
+        # end to end through the C ABI with HOST buffers (N = 1 process only: the call is single-GPU)
+        e2e = None
+        if world == 1 and "mixed" in paths:
+            hp, hm, hh = (torch.from_numpy(a).pin_memory() for a in (ps.pos, ps.mass, ps.soft))
+            ha = torch.empty((3, n), dtype=torch.float64).pin_memory()
+            for _ in range(2):
+                S.steps_forces_host(hp, hm, hh, ha, mixed=True)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            reps = max(2, min(args.steps, 5))
+            e0.record(stream)
+            for _ in range(reps):
+                S.steps_forces_host(hp, hm, hh, ha, mixed=True)
+            e1.record(stream)
+            e1.synchronize()
+            e2e = {"value": reps * inter_step / (e0.elapsed_time(e1) * 1e-3), "unit": UNIT,
+                   "h2d_bytes_per_step": 5 * n * 8, "d2h_bytes_per_step": 3 * n * 8,
+                   "call": "steps_forces_host(mixed=1), pinned host buffers"}
+    clocks = sampler.summary()
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    head = "mixed" if "mixed" in results else paths[0]
+    r = results[head]
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        cpu = cpu_oracle_rate(ps)
+    if clocks.get("sm_mhz"):
+        for p in results.values():
+            p["roofline"]["frac_at_sampled_clock"] = p["roofline"]["frac"] * SM_MAX_MHZ / clocks["sm_mhz"]
+    out = {
+        "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True,
+        "scaling": "strong", "vs_baseline": None, "dtype": r["dtype"], "data": "synthetic",
+        "config": {"workload": f"config3: compactified g0 set (S^3 stereographic, m~(1+r^2/4R^2)^3, eps_i=0.01(m_i/m_min)^(1/3)), N={n}, "
+                               f"one steps_kdk_step (kick+drift+prep+force+reduce) + momentum per step",
+                   "headline_path": head, "l2": "256 MiB flush write between timed steps (inputs 42 MB fit L2; ALU-bound)",
+                   "i_sharding": "none" if world == 1 else f"i-range per rank (PAPER L139), all-gather of positions, {world} ranks",
+                   "persistent_grid": {p: S.steps_persistent_grid(p == "mixed") for p in results}},
+        "roofline": r["roofline"], "paths": results, "clocks": clocks, "gpu_launches": int(launches_total),
+        "e2e": e2e, "cpu_baseline": cpu,
+        "context": "paper (other hardware): 9.3 Tflop/s on 4x GTX 1080 Ti, ~24% of peak (L159); K80 ~9.7e9 interactions/s/GPU (Table 1, derived)",
+    }
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -146,9 +146,17 @@ int steps_last_cuda_error(void);         /* cudaError_t of the last STEPS_ECUDA 
 int steps_version(void);                 /* major*10000 + minor*100 + patch */
 /* Number of kernels this library has launched since load (for bench.py's gpu_launches). */
 long long steps_kernel_launch_count(void);
-/* Tuning / testing knobs.  "driver": 0 = default force driver, 1 = the simple one-CTA-per-
- * i-block driver kept as an in-library cross-check.  Unknown key: STEPS_EINVAL. */
+/* Tuning / testing knobs.  "driver": 0 = default force driver (persistent, bulk-TMA), 1 = the
+ * simple one-CTA-per-i-block driver kept as an in-library cross-check.  "profile": 1 = bracket
+ * the force kernel of every later call with CUDA events recorded on the call's stream.
+ * Unknown key: STEPS_EINVAL. */
 int steps_set_option(const char *key, long long value);
+/* With "profile" on: device time in ms of the most recent force kernel launched on the current
+ * device (waits for it to finish); -1 if none was recorded. */
+double steps_last_force_kernel_ms(void);
+/* Grid (CTA count) of the persistent force kernel on the current device: SMs x resident CTAs;
+ * 0 before the first call of that path. */
+int steps_persistent_grid(int mixed);
 
 #ifdef __cplusplus
 }

@@ -22,6 +22,7 @@ namespace {
 std::atomic<long long> g_launches{0};
 thread_local int g_last_cuda_error = 0;
 std::atomic<int> g_driver{0};   // 0 = default, 1 = simple v1 driver (cross-check)
+std::atomic<int> g_profile{0};  // 1 = bracket the force kernel with CUDA events on its stream
 
 constexpr int MAX_DEVICES = 16;
 constexpr int STAGES = 4;
@@ -38,6 +39,8 @@ struct Workspace {
     double* h_pos = nullptr; double* h_mass = nullptr; double* h_soft = nullptr; double* h_acc = nullptr;
     long long h_cap = 0;
     int cc_major = -1;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;   // "profile" option: around the last force kernel
+    bool ev_valid = false;
 };
 Workspace g_ws[MAX_DEVICES];
 std::mutex g_mutex;
@@ -122,7 +125,13 @@ int launch_forces(const double* pos, const double* mass, const double* soft, lon
             grid_cache = g > MAX_GRID ? MAX_GRID : g;
         }
         const int P = grid_cache;
+        const bool prof = g_profile.load() != 0;
+        if (prof) {
+            if (!w.ev0) { STEPS_CUDA(cudaEventCreate(&w.ev0)); STEPS_CUDA(cudaEventCreate(&w.ev1)); }
+            STEPS_CUDA(cudaEventRecord(w.ev0, st));
+        }
         kern<<<P, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, i_begin, i_end, nb, w.partials);
+        if (prof) { STEPS_CUDA(cudaEventRecord(w.ev1, st)); w.ev_valid = true; }
         forces_reduce_kernel<Path::NOUT><<<(int)((cnt + 255) / 256), 256, 0, st>>>(w.partials, nt, nb, P, cnt, acc_out);
         g_launches += 2;
     }
@@ -296,6 +305,7 @@ void steps_shutdown(void)
         cudaSetDevice(d);
         cudaFree(w.tiles); cudaFree(w.partials); cudaFree(w.mom_partial);
         cudaFree(w.h_pos); cudaFree(w.h_mass); cudaFree(w.h_soft); cudaFree(w.h_acc);
+        if (w.ev0) { cudaEventDestroy(w.ev0); cudaEventDestroy(w.ev1); }
         w = Workspace();
     }
     cudaSetDevice(cur);
@@ -328,7 +338,26 @@ int steps_set_option(const char* key, long long value)
 {
     if (!key) return STEPS_EINVAL;
     if (std::strcmp(key, "driver") == 0) { g_driver = (int)value; return STEPS_OK; }
+    if (std::strcmp(key, "profile") == 0) { g_profile = (int)value; return STEPS_OK; }
     return STEPS_EINVAL;
+}
+
+double steps_last_force_kernel_ms(void)
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= MAX_DEVICES) return -1.0;
+    Workspace& w = g_ws[dev];
+    if (!w.ev_valid) return -1.0;
+    float ms = 0.0f;
+    if (cudaEventSynchronize(w.ev1) != cudaSuccess || cudaEventElapsedTime(&ms, w.ev0, w.ev1) != cudaSuccess) return -1.0;
+    return (double)ms;
+}
+
+int steps_persistent_grid(int mixed)
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= MAX_DEVICES) return 0;
+    return mixed ? g_ws[dev].grid_mixed : g_ws[dev].grid_fp64;
 }
 
 }  // extern "C"

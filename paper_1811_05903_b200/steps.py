@@ -17,7 +17,8 @@ EXPORTS = [
     "steps_forces", "steps_forces_mixed", "steps_forces_range", "steps_forces_host", "steps_kick_drift",
     "steps_kdk_step", "steps_hubble", "steps_scale_factor_rk4", "steps_kdk_schedule", "steps_momentum",
     "steps_reserve", "steps_shutdown", "steps_workspace_bytes", "steps_strerror", "steps_last_cuda_error",
-    "steps_version", "steps_kernel_launch_count", "steps_set_option",
+    "steps_version", "steps_kernel_launch_count", "steps_set_option", "steps_last_force_kernel_ms",
+    "steps_persistent_grid",
 ]
 
 
@@ -67,6 +68,8 @@ def lib() -> C.CDLL:
     L.steps_strerror.restype = C.c_char_p
     L.steps_kernel_launch_count.restype = ll
     L.steps_set_option.argtypes = [C.c_char_p, ll]
+    L.steps_last_force_kernel_ms.restype = dbl
+    L.steps_persistent_grid.argtypes = [i32]
     _lib = L
     return L
 
@@ -185,3 +188,11 @@ def steps_kernel_launch_count() -> int:
 
 def steps_set_option(key: str, value: int) -> None:
     _check(lib().steps_set_option(key.encode(), value))
+
+
+def steps_last_force_kernel_ms() -> float:
+    return float(lib().steps_last_force_kernel_ms())
+
+
+def steps_persistent_grid(mixed: bool) -> int:
+    return int(lib().steps_persistent_grid(int(mixed)))
