@@ -86,7 +86,7 @@ constexpr int persistent_smem_bytes()
 // ---- persistent stream-K driver ------------------------------------------------------------------
 // partials: [nb + gridDim.x slots][Path::NOUT][IB] doubles; CTA p's record for i-block b is slot b + p.
 template <typename Path, int STAGES>
-__global__ void __launch_bounds__(CTA_THREADS, 2)
+__global__ void __launch_bounds__(CTA_THREADS, 1)
 forces_persistent_kernel(const double* __restrict__ pos, const double* __restrict__ soft, long long N,
                          const typename Path::Tile* __restrict__ tiles, int nt, long long i_begin, long long i_end,
                          int nb, double* __restrict__ partials)
@@ -187,7 +187,7 @@ __global__ void __launch_bounds__(256) forces_reduce_kernel(const double* __rest
 
 // ---- simple driver (cross-check) -----------------------------------------------------------------
 template <typename Path>
-__global__ void __launch_bounds__(CTA_THREADS, 2)
+__global__ void __launch_bounds__(CTA_THREADS, 1)
 forces_v1_kernel(const double* __restrict__ pos, const double* __restrict__ soft, long long N,
                  const typename Path::Tile* __restrict__ tiles, int ntiles, long long i_begin, long long i_end,
                  double* __restrict__ acc_out)

@@ -2,21 +2,26 @@
 //
 // Rows a1/a2 of the hot path (Eq. 8 L88 first term; Eq. 3-4).
 //
-// Far body budget: 16 FP64-pipe instructions per interaction, nothing else on that pipe:
-//   3 DADD  d = x_j - x_i                       (exact input differences, no cancellation loss)
-//   1 DMUL + 2 DFMA  r2 = dx^2 + dy^2 + dz^2
-//   7 for s = m r^-3:  y2 = y0*y0;  e = fma(-r2, y2, 1);  q = m*y0;  q3 = q*y2;  t = q3*e;
-//                      c = fma(1.875, e, 1.5);  s = fma(t, c, q3)
-//   3 DFMA  acc += s * d
-// The reciprocal square root is seeded on the otherwise idle pipes: r2 is truncated to fp32
-// with two integer ops, MUFU.RSQ gives y0 ~ r^-1 (|delta| <~ 2e-7), three integer ops widen it
-// back to fp64.  With e = 1 - r2*y0^2 (exact to 1e-16: y0 has 24 bits, so y0^2 is exact) the
-// exact factor is r^-3 = y0^3 (1-e)^(-3/2) = y0^3 (1 + 1.5 e + 1.875 e^2 + 2.1875 e^3 ...);
-// the body keeps the quadratic term, leaving 2.19 e^3 < 3e-19 per pair.
-// Why not cheaper: a linear-only correction (14 instructions) leaves a one-signed 1.875 e^2 <=
-// 5e-13 per pair.  The bar is the MAX over particles, and the unluckiest of 1e6 particles has a
-// net force ~100x below its largest pair terms, which amplifies any per-pair error that is
-// not a few ulp; measured on config 1 the 14-instruction body gave max 4.3e-12 (rms 5e-14).
+// Far body (scaled sources, see TileT in common.cuh): 15 FP64-pipe instructions per interaction,
+// nothing else on that pipe:
+//   3 DFMA  dX = X_j - c_j x_i = c_j (x_j - x_i)
+//   1 DMUL + 2 DFMA  r2 = dX.dX                      (= c_j^2 r^2)
+//   6 for s = r2^(-3/2) = m_j / r^3 / c_j:  y2 = y0*y0;  e = fma(-r2, y2, 1);  q3 = y0*y2;  t = q3*e;
+//                      p = fma(1.875, e, 1.5);  s = fma(t, p, q3)
+//   3 DFMA  acc += s * dX
+// The reciprocal square root is seeded by ONE instruction on the otherwise idle SFU:
+// rsqrt.approx.ftz.f64 (MUFU.RSQ64H) reads the high word of r2 and returns a double whose low
+// word is zero, y0 ~ r2^(-1/2) with |delta| <~ 2^-20.  y0 has <= 21 significant bits, so y0*y0 is
+// exact and e = 1 - r2*y0^2 is exact to 1e-16.  The exact factor is
+//   r2^(-3/2) = y0^3 (1-e)^(-3/2) = y0^3 (1 + 1.5 e + 1.875 e^2 + 2.1875 e^3 ...);
+// the body keeps the quadratic term, leaving 2.19 e^3 < 3e-18 per pair.
+// Why not cheaper: a linear-only correction leaves a one-signed 1.875 e^2 ~ 1e-12 per pair whose
+// pair-to-pair fluctuation is amplified by the cancellation in the net force (the bar is the MAX
+// over particles, and the unluckiest of 1e6 particles has a net force ~100x below its largest
+// pair terms); an fp32-computed p = 1.5 + 1.875 e has 1e-7 resolution and spoils the linear term.
+// What the scaling costs: X_j = fl(c_j x_j) carries one rounding, 1.1e-16 |x_j| / r relative to
+// dX -- a few 1e-15 for the closest far pairs of these sets, random in sign (measured in the
+// parity tests; the unscaled 16-instruction body had exact differences).
 //
 // Accumulation: the compactified sets put ~87 % of the mass in the outer 1 % of the particles,
 // whose large pulls cancel almost exactly (shell theorem); a single running fp64 sum over all
@@ -29,15 +34,13 @@
 
 namespace steps {
 
-// y0 ~ 1 / sqrt(r2) to fp32-SFU accuracy, as an fp64 number, without touching the FP64 pipe.
-// Valid for 2^-126 <= r2 < 2^128.
+// y0 ~ 1 / sqrt(r2) with ~20 good bits as an fp64 number whose low word is 0: one MUFU.RSQ64H,
+// nothing on the FP64 pipe.
 __device__ __forceinline__ double rsqrt_seed(double r2)
 {
-    const int hi = __double2hiint(r2), lo = __double2loint(r2);
-    const unsigned fb = __funnelshift_l((unsigned)lo, (unsigned)(hi - 0x38000000), 3);   // fp64 -> fp32 bits (truncate)
-    const float y = rsqrt_approx(__uint_as_float(fb));
-    const unsigned yb = __float_as_uint(y);
-    return __hiloint2double((int)((yb >> 3) + 0x38000000u), (int)(yb << 29));            // fp32 -> fp64 bits (exact)
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(r2));
+    return y;
 }
 
 // Softened branches of Eq. 4 as g = calF / r in fp64.  Caller guarantees 0 < r2 < h^2.
@@ -86,16 +89,16 @@ struct Fp64Path {
         }
     }
 
-    // m * r2^(-3/2), 7 FP64-pipe instructions, relative error a few ulp.
-    static __device__ __forceinline__ double newton_s(double r2, double m)
+    // r2^(-3/2), 6 FP64-pipe instructions, relative error a few ulp.
+    static __device__ __forceinline__ double rcube(double r2)
     {
         const double y0 = rsqrt_seed(r2);
         const double y2 = y0 * y0;
         const double e = fma(-r2, y2, 1.0);
-        const double q3 = (m * y0) * y2;
+        const double q3 = y0 * y2;
         const double t = q3 * e;
-        const double c = fma(1.875, e, 1.5);
-        return fma(t, c, q3);
+        const double p = fma(1.875, e, 1.5);
+        return fma(t, p, q3);
     }
 
     static __device__ __forceinline__ void far(const Tile& T, const IState& S, double* acc)
@@ -105,23 +108,21 @@ struct Fp64Path {
         for (int k = 0; k < R_I; ++k) ax[k] = ay[k] = az[k] = 0.0;
 #pragma unroll 2
         for (int j = 0; j < TJ; j += 2) {
-            const double2 X = *reinterpret_cast<const double2*>(&T.x[j]);
-            const double2 Y = *reinterpret_cast<const double2*>(&T.y[j]);
-            const double2 Z = *reinterpret_cast<const double2*>(&T.z[j]);
-            const double2 M = *reinterpret_cast<const double2*>(&T.m[j]);
+            const double2 X = *reinterpret_cast<const double2*>(&T.X[j]);
+            const double2 Y = *reinterpret_cast<const double2*>(&T.Y[j]);
+            const double2 Z = *reinterpret_cast<const double2*>(&T.Z[j]);
+            const double2 Cc = *reinterpret_cast<const double2*>(&T.c[j]);
 #pragma unroll
             for (int k = 0; k < R_I; ++k) {
                 {
-                    const double dx = X.x - S.x[k], dy = Y.x - S.y[k], dz = Z.x - S.z[k];
-                    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-                    const double s = newton_s(r2, M.x);
-                    ax[k] = fma(dx, s, ax[k]); ay[k] = fma(dy, s, ay[k]); az[k] = fma(dz, s, az[k]);
+                    const double dX = fma(-S.x[k], Cc.x, X.x), dY = fma(-S.y[k], Cc.x, Y.x), dZ = fma(-S.z[k], Cc.x, Z.x);
+                    const double s = rcube(fma(dZ, dZ, fma(dY, dY, dX * dX)));
+                    ax[k] = fma(dX, s, ax[k]); ay[k] = fma(dY, s, ay[k]); az[k] = fma(dZ, s, az[k]);
                 }
                 {
-                    const double dx = X.y - S.x[k], dy = Y.y - S.y[k], dz = Z.y - S.z[k];
-                    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-                    const double s = newton_s(r2, M.y);
-                    ax[k] = fma(dx, s, ax[k]); ay[k] = fma(dy, s, ay[k]); az[k] = fma(dz, s, az[k]);
+                    const double dX = fma(-S.x[k], Cc.y, X.y), dY = fma(-S.y[k], Cc.y, Y.y), dZ = fma(-S.z[k], Cc.y, Z.y);
+                    const double s = rcube(fma(dZ, dZ, fma(dY, dY, dX * dX)));
+                    ax[k] = fma(dX, s, ax[k]); ay[k] = fma(dY, s, ay[k]); az[k] = fma(dZ, s, az[k]);
                 }
             }
         }
@@ -142,7 +143,7 @@ struct Fp64Path {
                 const double dx = xj - S.x[k], dy = yj - S.y[k], dz = zj - S.z[k];
                 const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
                 const double hs = S.h[k] + hj;
-                double s = newton_s(r2, mq);
+                double s = mq * rcube(r2);
                 if (r2 < hs * hs || r2 == 0.0)                        // Eq. 4 branches 1-2; readings #2, #4
                     s = (r2 == 0.0) ? 0.0 : mq * spline_g_soft_f64(r2, hs);
                 ax[k] = fma(dx, s, ax[k]); ay[k] = fma(dy, s, ay[k]); az[k] = fma(dz, s, az[k]);

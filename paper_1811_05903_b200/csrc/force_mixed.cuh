@@ -4,17 +4,21 @@
 //   far  tile: acc_i += m_j (x_j - x_i) / r^3                 (calF = 1/r^2 for r >= h, Eq. 4 third case)
 //   near tile: acc_i += m_j g(r, h_i + h_j) (x_j - x_i)       (all three branches; j = i and r = 0 add 0)
 //
-// Far body: two j-particles per instruction with the sm_100a packed fp32x2 pipe ops
-// (FADD2/FMUL2/FFMA2): 12 packed FP32-pipe instructions + 2 MUFU.RSQ per TWO interactions,
-// i.e. 12 FP32-lane-cycles and 7 issue slots per interaction.  j-data is read from the
-// shared-memory tile with broadcast LDS.128 (4 j per load per component), amortised over
-// R_I = 4 register-blocked i-particles per thread.  Partial sums live in fp32 for one tile
-// (<= 256 terms per packed half) and are then flushed into fp64 accumulators.
+// Far body (scaled sources, see TileT in common.cuh): two j-particles per instruction with the
+// sm_100a packed fp32x2 pipe ops (FADD2/FMUL2/FFMA2):
+//     dX = X_j - c_j x_i (3 FFMA2)   r2 = dX.dX (FMUL2 + 2 FFMA2)   y = rsqrt(r2) (2 MUFU.RSQ)
+//     y3 = y y y (2 FMUL2)           acc += y3 dX (3 FFMA2)
+// = 11 packed FP32-pipe instructions + 2 MUFU per TWO interactions, i.e. 11 FP32-lane-cycles and
+// 6.5 issue slots per interaction.  j-data is read from the shared-memory tile with broadcast
+// LDS.128 (4 j per load per component), amortised over R_I = 4 register-blocked i-particles per
+// thread.  Partial sums live in fp32 for one tile (<= 128 terms per packed half) and are then
+// flushed into fp64 accumulators.
+// Near body: same packing on the plain copy, plus h_i + h_j, its square and the r2 < h^2 test per
+// pair (14 packed + 2 MUFU per two interactions); the rare softened pair is patched in fp64.
 #pragma once
 #include "common.cuh"
 
 namespace steps {
-
 // Softened branches of Eq. 4 as g = calF / r, evaluated in fp64 (rare path: ~1e-4 of the pairs
 // of a near tile), r^2 and h = h_i + h_j given in fp32.  Caller guarantees 0 < r^2 < h^2.
 __device__ __noinline__ float spline_g_soft_from_f32(float r2, float hs)
@@ -62,39 +66,39 @@ struct MixedPath {
         }
     }
 
-    // One packed pair-of-interactions: i against (j, j+1).
-    static __device__ __forceinline__ void pair2(u64 xj, u64 yj, u64 zj, u64 mj, u64 xi, u64 yi, u64 zi,
+    // One packed pair of far interactions: i against the scaled sources (j, j+1).  nxi = (-x_i, -x_i).
+    static __device__ __forceinline__ void pair2(u64 Xj, u64 Yj, u64 Zj, u64 cj, u64 nxi, u64 nyi, u64 nzi,
                                                  u64& ax, u64& ay, u64& az)
     {
-        const u64 dx = sub2(xj, xi), dy = sub2(yj, yi), dz = sub2(zj, zi);
-        const u64 r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+        const u64 dX = fma2(nxi, cj, Xj), dY = fma2(nyi, cj, Yj), dZ = fma2(nzi, cj, Zj);
+        const u64 r2 = fma2(dZ, dZ, fma2(dY, dY, mul2(dX, dX)));
         float a, b;
         unpack2(r2, a, b);
-        const u64 rinv = pack2(rsqrt_approx(a), rsqrt_approx(b));
-        const u64 s = mul2(mul2(mj, rinv), mul2(rinv, rinv));
-        ax = fma2(dx, s, ax);
-        ay = fma2(dy, s, ay);
-        az = fma2(dz, s, az);
+        const u64 y = pack2(rsqrt_approx(a), rsqrt_approx(b));
+        const u64 y3 = mul2(mul2(y, y), y);
+        ax = fma2(dX, y3, ax);
+        ay = fma2(dY, y3, ay);
+        az = fma2(dZ, y3, az);
     }
 
     static __device__ __forceinline__ void far(const Tile& T, const IState& S, double* acc)
     {
-        u64 xi[R_I], yi[R_I], zi[R_I], ax[R_I], ay[R_I], az[R_I];
+        u64 nxi[R_I], nyi[R_I], nzi[R_I], ax[R_I], ay[R_I], az[R_I];
 #pragma unroll
         for (int k = 0; k < R_I; ++k) {
-            xi[k] = pack2(S.x[k], S.x[k]); yi[k] = pack2(S.y[k], S.y[k]); zi[k] = pack2(S.z[k], S.z[k]);
+            nxi[k] = pack2(-S.x[k], -S.x[k]); nyi[k] = pack2(-S.y[k], -S.y[k]); nzi[k] = pack2(-S.z[k], -S.z[k]);
             ax[k] = ay[k] = az[k] = 0ull;
         }
 #pragma unroll 2
         for (int j = 0; j < TJ; j += 4) {
-            const ulonglong2 X = *reinterpret_cast<const ulonglong2*>(&T.x[j]);
-            const ulonglong2 Y = *reinterpret_cast<const ulonglong2*>(&T.y[j]);
-            const ulonglong2 Z = *reinterpret_cast<const ulonglong2*>(&T.z[j]);
-            const ulonglong2 M = *reinterpret_cast<const ulonglong2*>(&T.m[j]);
+            const ulonglong2 X = *reinterpret_cast<const ulonglong2*>(&T.X[j]);
+            const ulonglong2 Y = *reinterpret_cast<const ulonglong2*>(&T.Y[j]);
+            const ulonglong2 Z = *reinterpret_cast<const ulonglong2*>(&T.Z[j]);
+            const ulonglong2 Cc = *reinterpret_cast<const ulonglong2*>(&T.c[j]);
 #pragma unroll
             for (int k = 0; k < R_I; ++k) {
-                pair2(X.x, Y.x, Z.x, M.x, xi[k], yi[k], zi[k], ax[k], ay[k], az[k]);
-                pair2(X.y, Y.y, Z.y, M.y, xi[k], yi[k], zi[k], ax[k], ay[k], az[k]);
+                pair2(X.x, Y.x, Z.x, Cc.x, nxi[k], nyi[k], nzi[k], ax[k], ay[k], az[k]);
+                pair2(X.y, Y.y, Z.y, Cc.y, nxi[k], nyi[k], nzi[k], ax[k], ay[k], az[k]);
             }
         }
 #pragma unroll
@@ -106,31 +110,55 @@ struct MixedPath {
         }
     }
 
+    // Pair factor of one half of a packed near pair that failed the Newtonian test.
+    static __device__ __forceinline__ float patch(float r2, float hs2, float hs, float m, float s_newton)
+    {
+        if (r2 == 0.0f) return 0.0f;                                   // j = i or coincident (reading #4)
+        if (r2 < hs2) return m * spline_g_soft_from_f32(r2, hs);       // Eq. 4 branches 1-2 (reading #2)
+        return s_newton;
+    }
+
     static __device__ __forceinline__ void near(const Tile& T, const IState& S, double* acc)
     {
-        float ax[R_I], ay[R_I], az[R_I];
+        u64 xi[R_I], yi[R_I], zi[R_I], hi[R_I], ax[R_I], ay[R_I], az[R_I];
 #pragma unroll
-        for (int k = 0; k < R_I; ++k) ax[k] = ay[k] = az[k] = 0.0f;
+        for (int k = 0; k < R_I; ++k) {
+            xi[k] = pack2(S.x[k], S.x[k]); yi[k] = pack2(S.y[k], S.y[k]); zi[k] = pack2(S.z[k], S.z[k]);
+            hi[k] = pack2(S.h[k], S.h[k]);
+            ax[k] = ay[k] = az[k] = 0ull;
+        }
 #pragma unroll 2
-        for (int j = 0; j < TJ; ++j) {
-            const float xj = T.x[j], yj = T.y[j], zj = T.z[j], mj = T.m[j], hj = T.h[j];
+        for (int j = 0; j < TJ; j += 2) {
+            const u64 xj = *reinterpret_cast<const u64*>(&T.x[j]), yj = *reinterpret_cast<const u64*>(&T.y[j]);
+            const u64 zj = *reinterpret_cast<const u64*>(&T.z[j]), mj = *reinterpret_cast<const u64*>(&T.m[j]);
+            const u64 hj = *reinterpret_cast<const u64*>(&T.h[j]);
 #pragma unroll
             for (int k = 0; k < R_I; ++k) {
-                const float dx = xj - S.x[k], dy = yj - S.y[k], dz = zj - S.z[k];
-                const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                const float hs = S.h[k] + hj;
-                const float rinv = rsqrt_approx(r2);
-                float s = mj * rinv * (rinv * rinv);
-                if (r2 < hs * hs || r2 == 0.0f)                       // Eq. 4 branches 1-2; readings #2, #4
-                    s = (r2 == 0.0f) ? 0.0f : mj * spline_g_soft_from_f32(r2, hs);
-                ax[k] = fmaf(dx, s, ax[k]);
-                ay[k] = fmaf(dy, s, ay[k]);
-                az[k] = fmaf(dz, s, az[k]);
+                const u64 dx = sub2(xj, xi[k]), dy = sub2(yj, yi[k]), dz = sub2(zj, zi[k]);
+                const u64 r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+                const u64 hs = add2(hj, hi[k]);
+                const u64 hs2 = mul2(hs, hs);
+                float ra, rb, ha, hb;
+                unpack2(r2, ra, rb);
+                unpack2(hs2, ha, hb);
+                const u64 rinv = pack2(rsqrt_approx(ra), rsqrt_approx(rb));
+                u64 s = mul2(mul2(mj, rinv), mul2(rinv, rinv));
+                if (!(ra >= ha && rb >= hb && fminf(ra, rb) > 0.0f)) {   // some half is softened, coincident or NaN
+                    float sa, sb, ma, mb, hsa, hsb;
+                    unpack2(s, sa, sb); unpack2(mj, ma, mb); unpack2(hs, hsa, hsb);
+                    s = pack2(patch(ra, ha, hsa, ma, sa), patch(rb, hb, hsb, mb, sb));
+                }
+                ax[k] = fma2(dx, s, ax[k]);
+                ay[k] = fma2(dy, s, ay[k]);
+                az[k] = fma2(dz, s, az[k]);
             }
         }
 #pragma unroll
         for (int k = 0; k < R_I; ++k) {
-            flush(acc, 0, k, ax[k]); flush(acc, 1, k, ay[k]); flush(acc, 2, k, az[k]);
+            float lo, hi2;
+            unpack2(ax[k], lo, hi2); flush(acc, 0, k, lo + hi2);
+            unpack2(ay[k], lo, hi2); flush(acc, 1, k, lo + hi2);
+            unpack2(az[k], lo, hi2); flush(acc, 2, k, lo + hi2);
         }
     }
 };

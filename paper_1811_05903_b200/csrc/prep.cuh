@@ -38,17 +38,37 @@ __global__ void __launch_bounds__(TJ) prep_tiles(const double* __restrict__ pos,
     const double m = real ? mass[j] : 0.0;
     const double h = real ? soft[j] : 0.0;
     Tile& T = tiles[blockIdx.x];
+    const int t = threadIdx.x;
+    // Scaled copy (see TileT in common.cuh).  A source whose scaled coordinates would leave the
+    // safe range of the arithmetic type (or with m < 0) cannot use the far body: it then forces
+    // its whole tile onto the near body (hmax = +inf) -- slower, never wrong.
+    bool scaled_ok = real && m > 0.0;
     if constexpr (sizeof(Tile) == sizeof(TileF32)) {
-        T.x[threadIdx.x] = (float)x; T.y[threadIdx.x] = (float)y; T.z[threadIdx.x] = (float)z;
-        T.m[threadIdx.x] = (float)m; T.h[threadIdx.x] = (float)h;
+        T.x[t] = (float)x; T.y[t] = (float)y; T.z[t] = (float)z; T.m[t] = (float)m; T.h[t] = (float)h;
+        // c is rounded to fp32 FIRST and X = fl32(x * c32), so that X - c32 x_i = c32 (x_j - x_i) up
+        // to the one rounding of X (the same size as the fp32 rounding of x_j itself).
+        const float c32 = scaled_ok ? (float)(1.0 / sqrt(m)) : STEPS_PAD_C32;
+        const double lim = 1.0e18, c = (double)c32;
+        scaled_ok = scaled_ok && c < lim && fabs(x * c) < lim && fabs(y * c) < lim && fabs(z * c) < lim;
+        T.c[t] = scaled_ok ? c32 : STEPS_PAD_C32;
+        T.X[t] = scaled_ok ? (float)(x * c) : STEPS_PAD_X32;
+        T.Y[t] = scaled_ok ? (float)(y * c) : STEPS_PAD_X32;
+        T.Z[t] = scaled_ok ? (float)(z * c) : STEPS_PAD_X32;
     } else {
-        T.x[threadIdx.x] = x; T.y[threadIdx.x] = y; T.z[threadIdx.x] = z;
-        T.m[threadIdx.x] = m; T.h[threadIdx.x] = h;
+        T.x[t] = x; T.y[t] = y; T.z[t] = z; T.m[t] = m; T.h[t] = h;
+        const double lim = 1.0e100, c = scaled_ok ? 1.0 / sqrt(m) : STEPS_PAD_C64;
+        scaled_ok = scaled_ok && c < lim && fabs(x * c) < lim && fabs(y * c) < lim && fabs(z * c) < lim;
+        T.c[t] = scaled_ok ? c : STEPS_PAD_C64;
+        T.X[t] = scaled_ok ? x * c : STEPS_PAD_X64;
+        T.Y[t] = scaled_ok ? y * c : STEPS_PAD_X64;
+        T.Z[t] = scaled_ok ? z * c : STEPS_PAD_X64;
     }
+    const bool force_near = real && m != 0.0 && !scaled_ok;
     const double r = sqrt(x * x + y * y + z * z);
     float rlo = real ? __double2float_rd(r) : __int_as_float(0x7f800000);
     float rhi = real ? __double2float_ru(r) : 0.0f;
     float hh = real ? __double2float_ru(h) : 0.0f;
+    if (force_near) hh = __int_as_float(0x7f800000);
     block_bounds(rlo, rhi, hh);
     if (threadIdx.x == 0) {
         T.meta.rmin = rlo; T.meta.rmax = rhi; T.meta.hmax = hh; T.meta.pad = 0.0f;

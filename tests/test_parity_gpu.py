@@ -175,11 +175,18 @@ def test_forces_range_and_host_entry_points(S, oracle):
     ps = synth.g0(5000, seed=21)
     full = gpu_forces(S, ps, False)
     dpos, dm, dh = dev(ps.pos), dev(ps.mass), dev(ps.soft)
-    for (b, e) in [(0, 5000), (0, 1), (4999, 5000), (1000, 3077), (2048, 2049)]:
+    # A range whose warp groups (128 consecutive i) coincide with the full call's groups classifies
+    # every (group, tile) pair the same way and is bit-identical; any other range may evaluate a
+    # Newtonian pair through the other body (scaled far / plain near), which differs by rounding.
+    for (b, e) in [(0, 5000), (1024, 5000), (2048, 4096), (0, 1), (4999, 5000), (1000, 3077), (2048, 2049)]:
         out = torch.empty(3 * (e - b), dtype=torch.float64, device="cuda")
         S.steps_forces_range(dpos, dm, dh, b, e, out, mixed=False)
         torch.cuda.synchronize()
-        assert np.array_equal(out.cpu().numpy().reshape(3, e - b), full[:, b:e]), (b, e)
+        got = out.cpu().numpy().reshape(3, e - b)
+        if b % 128 == 0 and (e % 128 == 0 or e == ps.n):
+            assert np.array_equal(got, full[:, b:e]), (b, e)
+        else:
+            assert rel_err(got, full[:, b:e]).max() <= 1e-13, (b, e)
     acc_h = np.empty((3, ps.n))
     S.steps_forces_host(ps.pos, ps.mass, ps.soft, acc_h, mixed=False)
     assert np.array_equal(acc_h, full)
