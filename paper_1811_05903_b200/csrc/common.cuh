@@ -9,9 +9,24 @@ namespace steps {
 typedef unsigned long long u64;
 
 // ---- decomposition constants -------------------------------------------------------------
-constexpr int TJ = 256;                   // particles per j-tile (one bulk copy, one far/near decision)
-constexpr int R_I = 4;                    // register-blocked i-particles per thread
-constexpr int CTA_THREADS = 512;          // threads per CTA (16 warps); ONE persistent CTA per SM
+// (overridable with -DSTEPS_TJ / -DSTEPS_R_I / -DSTEPS_CTA_THREADS for tuning sweeps; the defaults are the product)
+#ifndef STEPS_TJ
+#define STEPS_TJ 256
+#endif
+#ifndef STEPS_R_I
+#define STEPS_R_I 4
+#endif
+#ifndef STEPS_CTA_THREADS
+#define STEPS_CTA_THREADS 512
+#endif
+#ifndef STEPS_FAR_UNROLL
+#define STEPS_FAR_UNROLL 1
+#endif
+#define STEPS_PRAGMA_(x) _Pragma(#x)
+#define STEPS_UNROLL(n) STEPS_PRAGMA_(unroll n)
+constexpr int TJ = STEPS_TJ;              // particles per j-tile (one bulk copy, one far/near decision)
+constexpr int R_I = STEPS_R_I;            // register-blocked i-particles per thread
+constexpr int CTA_THREADS = STEPS_CTA_THREADS;   // threads per CTA; ONE persistent CTA per SM
 constexpr int IB = CTA_THREADS * R_I;     // i-particles per CTA work item (2048)
 constexpr int WARP_I = 32 * R_I;          // contiguous i-particles owned by one warp (128)
 

@@ -141,8 +141,12 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
             const int s = it % STAGES;
             mbar_wait(&full_bar[s], (it / STAGES) & 1);
             const Tile& T = *reinterpret_cast<const Tile*>(smem_raw + s * STRIDE);
+#ifdef STEPS_DIAG_ALLFAR                                   // timing diagnostic only (wrong forces): no near body
+            Path::far(T, S, acc);
+#else
             if (tile_is_far(rlo, rhi, hh, T.meta)) Path::far(T, S, acc);
             else Path::near(T, S, acc);
+#endif
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty_bar[s]);
         }

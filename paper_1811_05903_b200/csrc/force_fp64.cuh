@@ -106,7 +106,7 @@ struct Fp64Path {
         double ax[R_I], ay[R_I], az[R_I];
 #pragma unroll
         for (int k = 0; k < R_I; ++k) ax[k] = ay[k] = az[k] = 0.0;
-#pragma unroll 2
+STEPS_UNROLL(STEPS_FAR_UNROLL)
         for (int j = 0; j < TJ; j += 2) {
             const double2 X = *reinterpret_cast<const double2*>(&T.X[j]);
             const double2 Y = *reinterpret_cast<const double2*>(&T.Y[j]);

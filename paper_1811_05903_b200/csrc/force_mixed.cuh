@@ -66,47 +66,56 @@ struct MixedPath {
         }
     }
 
-    // One packed pair of far interactions: i against the scaled sources (j, j+1).  nxi = (-x_i, -x_i).
-    static __device__ __forceinline__ void pair2(u64 Xj, u64 Yj, u64 Zj, u64 cj, u64 nxi, u64 nyi, u64 nzi,
-                                                 u64& ax, u64& ay, u64& az)
-    {
-        const u64 dX = fma2(nxi, cj, Xj), dY = fma2(nyi, cj, Yj), dZ = fma2(nzi, cj, Zj);
-        const u64 r2 = fma2(dZ, dZ, fma2(dY, dY, mul2(dX, dX)));
-        float a, b;
-        unpack2(r2, a, b);
-        const u64 y = pack2(rsqrt_approx(a), rsqrt_approx(b));
-        const u64 y3 = mul2(mul2(y, y), y);
-        ax = fma2(dX, y3, ax);
-        ay = fma2(dY, y3, ay);
-        az = fma2(dZ, y3, az);
-    }
-
+    // Far body.  TWO i-particles per packed instruction (the register-blocked i's of a thread are
+    // packed in pairs), the scaled source (X_j, Y_j, Z_j, c_j) enters as 32-bit scalars that FFMA2
+    // broadcasts to both halves (SASS: Rn.F32 operands), so every packed instruction except the
+    // three accumulates reads <= 4 distinct register words -- measured on B200: an FFMA2 with three
+    // distinct 64-bit register operands costs 3 clk instead of 2 (register-file read bandwidth is
+    // 2 words/clk/lane), see DESIGN.md "what limits the mixed far body".
     static __device__ __forceinline__ void far(const Tile& T, const IState& S, double* acc)
     {
-        u64 nxi[R_I], nyi[R_I], nzi[R_I], ax[R_I], ay[R_I], az[R_I];
+        static_assert(R_I % 2 == 0, "i-particles are packed in pairs");
+        constexpr int NP = R_I / 2;
+        u64 nx[NP], ny[NP], nz[NP], ax[NP], ay[NP], az[NP];
 #pragma unroll
-        for (int k = 0; k < R_I; ++k) {
-            nxi[k] = pack2(-S.x[k], -S.x[k]); nyi[k] = pack2(-S.y[k], -S.y[k]); nzi[k] = pack2(-S.z[k], -S.z[k]);
-            ax[k] = ay[k] = az[k] = 0ull;
+        for (int p = 0; p < NP; ++p) {
+            nx[p] = pack2(-S.x[2 * p], -S.x[2 * p + 1]);
+            ny[p] = pack2(-S.y[2 * p], -S.y[2 * p + 1]);
+            nz[p] = pack2(-S.z[2 * p], -S.z[2 * p + 1]);
+            ax[p] = ay[p] = az[p] = 0ull;
         }
-#pragma unroll 2
+STEPS_UNROLL(STEPS_FAR_UNROLL)
         for (int j = 0; j < TJ; j += 4) {
-            const ulonglong2 X = *reinterpret_cast<const ulonglong2*>(&T.X[j]);
-            const ulonglong2 Y = *reinterpret_cast<const ulonglong2*>(&T.Y[j]);
-            const ulonglong2 Z = *reinterpret_cast<const ulonglong2*>(&T.Z[j]);
-            const ulonglong2 Cc = *reinterpret_cast<const ulonglong2*>(&T.c[j]);
+            const float4 X = *reinterpret_cast<const float4*>(&T.X[j]);
+            const float4 Y = *reinterpret_cast<const float4*>(&T.Y[j]);
+            const float4 Z = *reinterpret_cast<const float4*>(&T.Z[j]);
+            const float4 Cc = *reinterpret_cast<const float4*>(&T.c[j]);
+            const float Xs[4] = {X.x, X.y, X.z, X.w}, Ys[4] = {Y.x, Y.y, Y.z, Y.w};
+            const float Zs[4] = {Z.x, Z.y, Z.z, Z.w}, Cs[4] = {Cc.x, Cc.y, Cc.z, Cc.w};
 #pragma unroll
-            for (int k = 0; k < R_I; ++k) {
-                pair2(X.x, Y.x, Z.x, Cc.x, nxi[k], nyi[k], nzi[k], ax[k], ay[k], az[k]);
-                pair2(X.y, Y.y, Z.y, Cc.y, nxi[k], nyi[k], nzi[k], ax[k], ay[k], az[k]);
+            for (int q = 0; q < 4; ++q) {
+                const u64 cq = pack2(Cs[q], Cs[q]), Xq = pack2(Xs[q], Xs[q]);
+                const u64 Yq = pack2(Ys[q], Ys[q]), Zq = pack2(Zs[q], Zs[q]);
+#pragma unroll
+                for (int p = 0; p < NP; ++p) {
+                    const u64 dX = fma2(nx[p], cq, Xq), dY = fma2(ny[p], cq, Yq), dZ = fma2(nz[p], cq, Zq);
+                    const u64 r2 = fma2(dZ, dZ, fma2(dY, dY, mul2(dX, dX)));
+                    float a, b;
+                    unpack2(r2, a, b);
+                    const u64 y = pack2(rsqrt_approx(a), rsqrt_approx(b));
+                    const u64 y3 = mul2(mul2(y, y), y);
+                    ax[p] = fma2(dX, y3, ax[p]);
+                    ay[p] = fma2(dY, y3, ay[p]);
+                    az[p] = fma2(dZ, y3, az[p]);
+                }
             }
         }
 #pragma unroll
-        for (int k = 0; k < R_I; ++k) {
+        for (int p = 0; p < NP; ++p) {
             float lo, hi;
-            unpack2(ax[k], lo, hi); flush(acc, 0, k, lo + hi);
-            unpack2(ay[k], lo, hi); flush(acc, 1, k, lo + hi);
-            unpack2(az[k], lo, hi); flush(acc, 2, k, lo + hi);
+            unpack2(ax[p], lo, hi); flush(acc, 0, 2 * p, lo); flush(acc, 0, 2 * p + 1, hi);
+            unpack2(ay[p], lo, hi); flush(acc, 1, 2 * p, lo); flush(acc, 1, 2 * p + 1, hi);
+            unpack2(az[p], lo, hi); flush(acc, 2, 2 * p, lo); flush(acc, 2, 2 * p + 1, hi);
         }
     }
 

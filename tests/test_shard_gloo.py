@@ -1,0 +1,71 @@
+"""-m "not gpu": the N > 1 plumbing of bench.py on CPU -- the paper's i-range decomposition
+(node k computes floor(N/N_node) force vectors against all particles, the
+main node also takes the remainder; one exchange of positions per step).  world_size 2 and 3,
+`gloo` backend, 127.0.0.1 rendezvous.  The per-rank force call is played by the oracle's
+idx-restricted sum (the CUDA path needs a GPU); what is under test is the host-side plan:
+ranges tile [0, N) exactly, the all-gather rebuilds the replicated SoA array, and the sharded
+evaluation equals the unsharded one bit for bit."""
+import os
+import socket
+
+import numpy as np
+import pytest
+
+from paper_1811_05903_b200 import shard, synth
+
+
+def _free_port() -> int:
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+@pytest.mark.parametrize("world,n", [(1, 7), (2, 4096), (3, 1000), (8, 1048576), (5, 3)])
+def test_i_ranges_tile_the_particles(world, n):
+    ranges = shard.all_ranges(world, n)
+    assert ranges[0][0] == 0 and ranges[-1][1] == n
+    for (b0, e0), (b1, e1) in zip(ranges, ranges[1:]):
+        assert e0 == b1 and e0 >= b0
+    base, rem = divmod(n, world)
+    assert ranges[0][1] - ranges[0][0] == base + rem          # the main rank takes mod(N, P) (L139)
+    assert all(e - b == base for b, e in ranges[1:])
+
+
+def _worker(rank: int, world: int, port: int, n: int, out_dir: str) -> None:
+    import torch
+    import torch.distributed as dist
+
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        from oracle import steps_oracle as oracle
+        ps = synth.g0(n, seed=77)                              # identical on every rank (seeded)
+        b, e = shard.i_range(rank, world, n)
+        # one "step": every rank moves ITS slice (a stand-in drift), the slices are all-gathered ...
+        x_local = torch.from_numpy(ps.pos[:, b:e].copy()) * (1.0 + 1e-3 * (rank + 1))
+        x_all = shard.gather_soa(x_local, n)
+        # ... and every rank evaluates the forces of its i-range against ALL sources
+        pos = np.ascontiguousarray(x_all.numpy())
+        acc_local = oracle.forces(pos, ps.mass, ps.soft, idx=np.arange(b, e, dtype=np.int64))
+        np.save(os.path.join(out_dir, f"pos_{rank}.npy"), pos)
+        np.save(os.path.join(out_dir, f"acc_{rank}.npy"), acc_local)
+        dist.barrier()
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world,n", [(2, 1501), (3, 1000)])
+def test_sharded_step_equals_unsharded(world, n, tmp_path, oracle):
+    import torch.multiprocessing as mp
+
+    port = _free_port()
+    mp.spawn(_worker, args=(world, port, n, str(tmp_path)), nprocs=world, join=True)
+    ps = synth.g0(n, seed=77)
+    expect_pos = ps.pos.copy()
+    for r, (b, e) in enumerate(shard.all_ranges(world, n)):
+        expect_pos[:, b:e] *= 1.0 + 1e-3 * (r + 1)
+    full = oracle.forces(expect_pos, ps.mass, ps.soft)
+    for r, (b, e) in enumerate(shard.all_ranges(world, n)):
+        assert np.array_equal(np.load(tmp_path / f"pos_{r}.npy"), expect_pos), f"rank {r}: gathered positions"
+        assert np.array_equal(np.load(tmp_path / f"acc_{r}.npy"), full[:, b:e]), f"rank {r}: forces of its range"
