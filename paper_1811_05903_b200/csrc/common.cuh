@@ -22,6 +22,9 @@ typedef unsigned long long u64;
 #ifndef STEPS_FAR_UNROLL
 #define STEPS_FAR_UNROLL 1
 #endif
+#ifndef STEPS_FP64_P_OFFPIPE
+#define STEPS_FP64_P_OFFPIPE 1
+#endif
 #define STEPS_PRAGMA_(x) _Pragma(#x)
 #define STEPS_UNROLL(n) STEPS_PRAGMA_(unroll n)
 constexpr int TJ = STEPS_TJ;              // particles per j-tile (one bulk copy, one far/near decision)

@@ -43,6 +43,27 @@ __device__ __forceinline__ double rsqrt_seed(double r2)
     return y;
 }
 
+// p = 1.5 + 1.875 e built WITHOUT the FP64 pipe (|e| < 2^-17; p is needed to 2^-36 absolute only,
+// because it multiplies t = q3 e ~ 2^-19 q3):
+//   f  = e 2^128 as an fp32 number: (hi word of e) << 3 keeps the low 8 exponent bits and the top 20
+//        mantissa bits (valid for 2^-255 <= |e| < 2, and for e = 0); the sign is merged back  [SHL, LOP3]
+//   g  = fma(f, 1.875 2^(38-128), 1.5 2^23): the magic-number add leaves K = rint(1.875 e 2^38) in the
+//        low mantissa bits of g in two's complement, g = 0x4B400000 + K                       [FFMA]
+//   p  = 1.5 + K 2^-38 as fp64 bits: (0x3FF80000'00000000 + (K << 14)); both words come straight
+//        from g because 0x4B400000 is a multiple of 2^18                                     [SHF, SHF, IADD]
+// Error: 2^-20 relative truncation of e (2^-39 on p) + 2^-39 rounding of K  ->  < 2^-57 relative on s.
+__device__ __forceinline__ double poly_p_offpipe(double e)
+{
+    const unsigned H = (unsigned)__double2hiint(e);
+    unsigned fb;                                               // (H << 3 & 0x7fffffff) | (H & 0x80000000): one LOP3
+    asm("lop3.b32 %0, %1, %2, 0x80000000, 0xd8;" : "=r"(fb) : "r"(H << 3), "r"(H));
+    const float f = __uint_as_float(fb);
+    const unsigned g = __float_as_uint(fmaf(f, 0x1.ep-90f, 12582912.0f));
+    const int hi = (int)(g >> 18) + (0x3ff80000 - (0x4b400000 >> 18));
+    const int lo = (int)(g << 14);
+    return __hiloint2double(hi, lo);
+}
+
 // Softened branches of Eq. 4 as g = calF / r in fp64.  Caller guarantees 0 < r2 < h^2.
 __device__ __noinline__ double spline_g_soft_f64(double r2, double h)
 {
@@ -97,7 +118,11 @@ struct Fp64Path {
         const double e = fma(-r2, y2, 1.0);
         const double q3 = y0 * y2;
         const double t = q3 * e;
+#if STEPS_FP64_P_OFFPIPE
+        const double p = poly_p_offpipe(e);
+#else
         const double p = fma(1.875, e, 1.5);
+#endif
         return fma(t, p, q3);
     }
 
