@@ -23,7 +23,15 @@ typedef unsigned long long u64;
 #define STEPS_FAR_UNROLL 1
 #endif
 #ifndef STEPS_FP64_P_OFFPIPE
-#define STEPS_FP64_P_OFFPIPE 1
+#define STEPS_FP64_P_OFFPIPE 0
+#endif
+#ifndef STEPS_MIXED_ACC_SCALAR
+#define STEPS_MIXED_ACC_SCALAR 0
+#endif
+// fp32 tiles store c[] with adjacent elements swapped (c[j ^ 1]): after the LDS.128 loads of the far
+// body the scalar c_q then sits in a register of the opposite parity (bank) to X_q / Y_q / Z_q.
+#ifndef STEPS_C_SWIZZLE
+#define STEPS_C_SWIZZLE 1
 #endif
 #define STEPS_PRAGMA_(x) _Pragma(#x)
 #define STEPS_UNROLL(n) STEPS_PRAGMA_(unroll n)

@@ -43,6 +43,10 @@ __device__ __forceinline__ double rsqrt_seed(double r2)
     return y;
 }
 
+// [Measured slower, kept behind STEPS_FP64_P_OFFPIPE=1 as a documented experiment: on B200 every non-FP64
+//  instruction issued next to a saturated DFMA stream costs 0.3-1 clk of DFMA issue (micro-benchmark:
+//  8 DFMA alone 2.37 clk each; + 4 LOP3 -> 2.84; + 4 FFMA -> 2.54), so the 6 ALU/FMA instructions that
+//  replace one DFMA made the N = 1M evaluation 1224 ms instead of 1091 ms.]
 // p = 1.5 + 1.875 e built WITHOUT the FP64 pipe (|e| < 2^-17; p is needed to 2^-36 absolute only,
 // because it multiplies t = q3 e ~ 2^-19 q3):
 //   f  = e 2^128 as an fp32 number: (hi word of e) << 3 keeps the low 8 exponent bits and the top 20

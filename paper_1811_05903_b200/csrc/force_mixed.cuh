@@ -94,7 +94,7 @@ STEPS_UNROLL(STEPS_FAR_UNROLL)
             const float Zs[4] = {Z.x, Z.y, Z.z, Z.w}, Cs[4] = {Cc.x, Cc.y, Cc.z, Cc.w};
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
-                const u64 cq = pack2(Cs[q], Cs[q]), Xq = pack2(Xs[q], Xs[q]);
+                const u64 cq = pack2(Cs[q ^ STEPS_C_SWIZZLE], Cs[q ^ STEPS_C_SWIZZLE]), Xq = pack2(Xs[q], Xs[q]);
                 const u64 Yq = pack2(Ys[q], Ys[q]), Zq = pack2(Zs[q], Zs[q]);
 #pragma unroll
                 for (int p = 0; p < NP; ++p) {
@@ -104,9 +104,19 @@ STEPS_UNROLL(STEPS_FAR_UNROLL)
                     unpack2(r2, a, b);
                     const u64 y = pack2(rsqrt_approx(a), rsqrt_approx(b));
                     const u64 y3 = mul2(mul2(y, y), y);
+#if STEPS_MIXED_ACC_SCALAR
+                    {
+                        float dl, dh, yl, yh, al, ah;
+                        unpack2(y3, yl, yh);
+                        unpack2(dX, dl, dh); unpack2(ax[p], al, ah); ax[p] = pack2(fmaf(dl, yl, al), fmaf(dh, yh, ah));
+                        unpack2(dY, dl, dh); unpack2(ay[p], al, ah); ay[p] = pack2(fmaf(dl, yl, al), fmaf(dh, yh, ah));
+                        unpack2(dZ, dl, dh); unpack2(az[p], al, ah); az[p] = pack2(fmaf(dl, yl, al), fmaf(dh, yh, ah));
+                    }
+#else
                     ax[p] = fma2(dX, y3, ax[p]);
                     ay[p] = fma2(dY, y3, ay[p]);
                     az[p] = fma2(dZ, y3, az[p]);
+#endif
                 }
             }
         }

@@ -50,7 +50,7 @@ __global__ void __launch_bounds__(TJ) prep_tiles(const double* __restrict__ pos,
         const float c32 = scaled_ok ? (float)(1.0 / sqrt(m)) : STEPS_PAD_C32;
         const double lim = 1.0e18, c = (double)c32;
         scaled_ok = scaled_ok && c < lim && fabs(x * c) < lim && fabs(y * c) < lim && fabs(z * c) < lim;
-        T.c[t] = scaled_ok ? c32 : STEPS_PAD_C32;
+        T.c[t ^ STEPS_C_SWIZZLE] = scaled_ok ? c32 : STEPS_PAD_C32;   // see STEPS_C_SWIZZLE in common.cuh
         T.X[t] = scaled_ok ? (float)(x * c) : STEPS_PAD_X32;
         T.Y[t] = scaled_ok ? (float)(y * c) : STEPS_PAD_X32;
         T.Z[t] = scaled_ok ? (float)(z * c) : STEPS_PAD_X32;
