@@ -22,9 +22,8 @@ typedef unsigned long long u64;
 #ifndef STEPS_FAR_UNROLL
 #define STEPS_FAR_UNROLL 1
 #endif
-#ifndef STEPS_FP64_P_OFFPIPE
-#define STEPS_FP64_P_OFFPIPE 0
-#endif
+// Constant folded into the scaled copy of the fp64 tiles: c_j = (STEPS_FP64_FOLD m_j)^(-1/2) (force_fp64.cuh).
+#define STEPS_FP64_FOLD 1.875
 #ifndef STEPS_MIXED_ACC_SCALAR
 #define STEPS_MIXED_ACC_SCALAR 0
 #endif

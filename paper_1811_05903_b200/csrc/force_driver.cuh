@@ -10,6 +10,9 @@
 //  forces_v1_kernel: one CTA per i-block, plain loads + __syncthreads.  Kept as the in-library
 //      cross-check of the persistent driver (steps_set_option("driver", 1)).
 //
+// `zero` is a kernel argument that is always 0 and that the compiler cannot know to be 0: the fp64 far
+// body tests bits of it to place never-taken branches between its stages (see force_fp64.cuh).
+//
 // Both share the Path bodies (force_mixed.cuh / force_fp64.cuh) and the per-thread accumulator
 // block in shared memory: element (c, k) of thread t at acc[(c * R_I + k) * CTA_THREADS + t].
 #pragma once
@@ -89,7 +92,7 @@ template <typename Path, int STAGES>
 __global__ void __launch_bounds__(CTA_THREADS, 1)
 forces_persistent_kernel(const double* __restrict__ pos, const double* __restrict__ soft, long long N,
                          const typename Path::Tile* __restrict__ tiles, int nt, long long i_begin, long long i_end,
-                         int nb, double* __restrict__ partials)
+                         int nb, double* __restrict__ partials, int zero)
 {
     using Tile = typename Path::Tile;
     constexpr int STRIDE = stage_stride((int)sizeof(Tile));
@@ -142,9 +145,9 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
             mbar_wait(&full_bar[s], (it / STAGES) & 1);
             const Tile& T = *reinterpret_cast<const Tile*>(smem_raw + s * STRIDE);
 #ifdef STEPS_DIAG_ALLFAR                                   // timing diagnostic only (wrong forces): no near body
-            Path::far(T, S, acc);
+            Path::far(T, S, acc, zero);
 #else
-            if (tile_is_far(rlo, rhi, hh, T.meta)) Path::far(T, S, acc);
+            if (tile_is_far(rlo, rhi, hh, T.meta)) Path::far(T, S, acc, zero);
             else Path::near(T, S, acc);
 #endif
             __syncwarp();
@@ -194,7 +197,7 @@ template <typename Path>
 __global__ void __launch_bounds__(CTA_THREADS, 1)
 forces_v1_kernel(const double* __restrict__ pos, const double* __restrict__ soft, long long N,
                  const typename Path::Tile* __restrict__ tiles, int ntiles, long long i_begin, long long i_end,
-                 double* __restrict__ acc_out)
+                 double* __restrict__ acc_out, int zero)
 {
     using Tile = typename Path::Tile;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -215,7 +218,7 @@ forces_v1_kernel(const double* __restrict__ pos, const double* __restrict__ soft
             for (int q = threadIdx.x; q < (int)(sizeof(Tile) / 16); q += CTA_THREADS) dst[q] = src[q];
         }
         __syncthreads();
-        if (tile_is_far(rlo, rhi, hh, tile.meta)) Path::far(tile, S, acc);
+        if (tile_is_far(rlo, rhi, hh, tile.meta)) Path::far(tile, S, acc, zero);
         else Path::near(tile, S, acc);
     }
     const long long cnt = i_end - i_begin;

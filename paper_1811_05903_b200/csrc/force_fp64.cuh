@@ -2,26 +2,41 @@
 //
 // Rows a1/a2 of the hot path (Eq. 8 L88 first term; Eq. 3-4).
 //
-// Far body (scaled sources, see TileT in common.cuh): 15 FP64-pipe instructions per interaction,
+// Far body (scaled sources, see TileT in common.cuh): 14 FP64-pipe instructions per interaction,
 // nothing else on that pipe:
-//   3 DFMA  dX = X_j - c_j x_i = c_j (x_j - x_i)
-//   1 DMUL + 2 DFMA  r2 = dX.dX                      (= c_j^2 r^2)
-//   6 for s = r2^(-3/2) = m_j / r^3 / c_j:  y2 = y0*y0;  e = fma(-r2, y2, 1);  q3 = y0*y2;  t = q3*e;
-//                      p = fma(1.875, e, 1.5);  s = fma(t, p, q3)
+//   3 DFMA  dX = X_j - c_j x_i = c_j (x_j - x_i)          (c_j = (1.875 m_j)^(-1/2), see below)
+//   1 DMUL + 2 DFMA  r2 = dX.dX                            (= c_j^2 r^2)
+//   5 for s = r2^(-3/2) / 1.875:   y2 = y0*y0;  w = fma(r2, y2, -1.4);  g = fma(w, w, C0);
+//                                  q3 = y0*y2;  s = q3*g
 //   3 DFMA  acc += s * dX
 // The reciprocal square root is seeded by ONE instruction on the otherwise idle SFU:
 // rsqrt.approx.ftz.f64 (MUFU.RSQ64H) reads the high word of r2 and returns a double whose low
-// word is zero, y0 ~ r2^(-1/2) with |delta| <~ 2^-20.  y0 has <= 21 significant bits, so y0*y0 is
-// exact and e = 1 - r2*y0^2 is exact to 1e-16.  The exact factor is
-//   r2^(-3/2) = y0^3 (1-e)^(-3/2) = y0^3 (1 + 1.5 e + 1.875 e^2 + 2.1875 e^3 ...);
-// the body keeps the quadratic term, leaving 2.19 e^3 < 3e-18 per pair.
-// Why not cheaper: a linear-only correction leaves a one-signed 1.875 e^2 ~ 1e-12 per pair whose
-// pair-to-pair fluctuation is amplified by the cancellation in the net force (the bar is the MAX
-// over particles, and the unluckiest of 1e6 particles has a net force ~100x below its largest
-// pair terms); an fp32-computed p = 1.5 + 1.875 e has 1e-7 resolution and spoils the linear term.
+// word is zero, y0 ~ r2^(-1/2) with |1 - r2 y0^2| = |e| <= 2^-19.05 (measured over 1.6e7 arguments).
+// y0 has <= 21 significant bits, so y2 = y0*y0 is exact.  With u = r2 y0^2 = 1 - e the exact factor is
+//   r2^(-3/2) = y0^3 u^(-3/2) = y0^3 (1 + 1.5 e + 1.875 e^2 + 2.1875 e^3 ...)
+// and the quadratic Taylor polynomial 4.375 - 5.25 u + 1.875 u^2 completes to the square
+//   1.875 [ (u - 1.4)^2 + 0.7/1.875 ],
+// which costs two FMAs (w, g) instead of the three of Horner's rule; the factor 1.875 is folded into the
+// tile's scaled copy: prep_tiles stores c_j = (1.875 m_j)^(-1/2), so s dX = c_j^-2 (x_j - x_i) / (1.875 r^3)
+// = m_j (x_j - x_i) / r^3 with s = (c_j r)^-3 / 1.875 as the body returns it.
+// Remainder 2.19 e^3 < 3e-18 per pair; measured max relative error of s 9.5e-16, mean +2e-18.
+// Why not cheaper: a linear-only correction leaves 1.875 e^2 ~ 1e-12 per pair whose pair-to-pair
+// fluctuation is amplified by the cancellation in the net force (the bar is the MAX over particles,
+// and the unluckiest of 1e6 particles has a net force ~100x below its largest pair terms).
+//
+// Instruction ORDER matters on this pipe (micro-benchmarked on B200): a DFMA
+// whose three source operands are three different registers that all have to come from the register
+// file occupies the FP64 pipe for 3 clk instead of 2; an operand that the PREVIOUS FP64 instruction of
+// the warp held in the same operand slot (SASS `.reuse`) is not read again.  So the body is written in
+// stages over the R_I register-blocked i-particles of ONE source j -- all differences (they share c_j
+// and X_j/Y_j/Z_j), then the <= 2-register r2 / polynomial instructions, then the accumulate triples
+// (they share s) -- and the stages are separated by never-taken branches on bits of the kernel argument
+// `zero`, because ptxas otherwise interleaves the stages to hide latency and loses the operand reuse
+// (89-90 % instead of 84 % FP64-pipe occupancy).  Latency is hidden by the other 3 warps of the SMSP.
+//
 // What the scaling costs: X_j = fl(c_j x_j) carries one rounding, 1.1e-16 |x_j| / r relative to
 // dX -- a few 1e-15 for the closest far pairs of these sets, random in sign (measured in the
-// parity tests; the unscaled 16-instruction body had exact differences).
+// parity tests).
 //
 // Accumulation: the compactified sets put ~87 % of the mass in the outer 1 % of the particles,
 // whose large pulls cancel almost exactly (shell theorem); a single running fp64 sum over all
@@ -43,30 +58,11 @@ __device__ __forceinline__ double rsqrt_seed(double r2)
     return y;
 }
 
-// [Measured slower, kept behind STEPS_FP64_P_OFFPIPE=1 as a documented experiment: on B200 every non-FP64
-//  instruction issued next to a saturated DFMA stream costs 0.3-1 clk of DFMA issue (micro-benchmark:
-//  8 DFMA alone 2.37 clk each; + 4 LOP3 -> 2.84; + 4 FFMA -> 2.54), so the 6 ALU/FMA instructions that
-//  replace one DFMA made the N = 1M evaluation 1224 ms instead of 1091 ms.]
-// p = 1.5 + 1.875 e built WITHOUT the FP64 pipe (|e| < 2^-17; p is needed to 2^-36 absolute only,
-// because it multiplies t = q3 e ~ 2^-19 q3):
-//   f  = e 2^128 as an fp32 number: (hi word of e) << 3 keeps the low 8 exponent bits and the top 20
-//        mantissa bits (valid for 2^-255 <= |e| < 2, and for e = 0); the sign is merged back  [SHL, LOP3]
-//   g  = fma(f, 1.875 2^(38-128), 1.5 2^23): the magic-number add leaves K = rint(1.875 e 2^38) in the
-//        low mantissa bits of g in two's complement, g = 0x4B400000 + K                       [FFMA]
-//   p  = 1.5 + K 2^-38 as fp64 bits: (0x3FF80000'00000000 + (K << 14)); both words come straight
-//        from g because 0x4B400000 is a multiple of 2^18                                     [SHF, SHF, IADD]
-// Error: 2^-20 relative truncation of e (2^-39 on p) + 2^-39 rounding of K  ->  < 2^-57 relative on s.
-__device__ __forceinline__ double poly_p_offpipe(double e)
-{
-    const unsigned H = (unsigned)__double2hiint(e);
-    unsigned fb;                                               // (H << 3 & 0x7fffffff) | (H & 0x80000000): one LOP3
-    asm("lop3.b32 %0, %1, %2, 0x80000000, 0xd8;" : "=r"(fb) : "r"(H << 3), "r"(H));
-    const float f = __uint_as_float(fb);
-    const unsigned g = __float_as_uint(fmaf(f, 0x1.ep-90f, 12582912.0f));
-    const int hi = (int)(g >> 18) + (0x3ff80000 - (0x4b400000 >> 18));
-    const int lo = (int)(g << 14);
-    return __hiloint2double(hi, lo);
-}
+// Never-taken branch on bit n of `zero` (always 0, unknown to the compiler): ends a basic block, which
+// is the only ordering ptxas respects.  One uniform-datapath branch per use, no FP64-pipe work.
+#define STEPS_STAGE_FENCE(zero, n)                                                              \
+    asm volatile("{\n.reg .pred p;\n.reg .b32 t;\nand.b32 t, %0, %1;\nsetp.ne.s32 p, t, 0;\n@p trap;\n}" \
+                 :: "r"(zero), "r"(1 << (n)))
 
 // Softened branches of Eq. 4 as g = calF / r in fp64.  Caller guarantees 0 < r2 < h^2.
 __device__ __noinline__ double spline_g_soft_f64(double r2, double h)
@@ -114,7 +110,7 @@ struct Fp64Path {
         }
     }
 
-    // r2^(-3/2), 6 FP64-pipe instructions, relative error a few ulp.
+    // r2^(-3/2), 6 FP64-pipe instructions, relative error a few ulp (near body; the far body inlines the 5-op form).
     static __device__ __forceinline__ double rcube(double r2)
     {
         const double y0 = rsqrt_seed(r2);
@@ -122,37 +118,45 @@ struct Fp64Path {
         const double e = fma(-r2, y2, 1.0);
         const double q3 = y0 * y2;
         const double t = q3 * e;
-#if STEPS_FP64_P_OFFPIPE
-        const double p = poly_p_offpipe(e);
-#else
         const double p = fma(1.875, e, 1.5);
-#endif
         return fma(t, p, q3);
     }
 
-    static __device__ __forceinline__ void far(const Tile& T, const IState& S, double* acc)
+    static __device__ __forceinline__ void far(const Tile& T, const IState& S, double* acc, int zero)
     {
+        constexpr double A = 1.4;
+        constexpr double C0 = 1.0 / STEPS_FP64_FOLD - (1.0 - A) * (1.0 - A);   // (u - A)^2 + C0 = 1/1.875 at u = 1
         double ax[R_I], ay[R_I], az[R_I];
 #pragma unroll
         for (int k = 0; k < R_I; ++k) ax[k] = ay[k] = az[k] = 0.0;
-STEPS_UNROLL(STEPS_FAR_UNROLL)
-        for (int j = 0; j < TJ; j += 2) {
-            const double2 X = *reinterpret_cast<const double2*>(&T.X[j]);
-            const double2 Y = *reinterpret_cast<const double2*>(&T.Y[j]);
-            const double2 Z = *reinterpret_cast<const double2*>(&T.Z[j]);
-            const double2 Cc = *reinterpret_cast<const double2*>(&T.c[j]);
+#pragma unroll 1
+        for (int j = 0; j < TJ; ++j) {
+            const double X = T.X[j], Y = T.Y[j], Z = T.Z[j], C = T.c[j];
+            double dX[R_I], dY[R_I], dZ[R_I], r2[R_I], y0[R_I], y2[R_I], w[R_I];
+            STEPS_STAGE_FENCE(zero, 0);
+#pragma unroll
+            for (int k = 0; k < R_I; ++k) dX[k] = fma(-S.x[k], C, X);
+#pragma unroll
+            for (int k = 0; k < R_I; ++k) dY[k] = fma(-S.y[k], C, Y);
+#pragma unroll
+            for (int k = 0; k < R_I; ++k) dZ[k] = fma(-S.z[k], C, Z);
+            STEPS_STAGE_FENCE(zero, 1);
+#pragma unroll
+            for (int k = 0; k < R_I; ++k) r2[k] = fma(dZ[k], dZ[k], fma(dY[k], dY[k], dX[k] * dX[k]));
+#pragma unroll
+            for (int k = 0; k < R_I; ++k) y0[k] = rsqrt_seed(r2[k]);
 #pragma unroll
             for (int k = 0; k < R_I; ++k) {
-                {
-                    const double dX = fma(-S.x[k], Cc.x, X.x), dY = fma(-S.y[k], Cc.x, Y.x), dZ = fma(-S.z[k], Cc.x, Z.x);
-                    const double s = rcube(fma(dZ, dZ, fma(dY, dY, dX * dX)));
-                    ax[k] = fma(dX, s, ax[k]); ay[k] = fma(dY, s, ay[k]); az[k] = fma(dZ, s, az[k]);
-                }
-                {
-                    const double dX = fma(-S.x[k], Cc.y, X.y), dY = fma(-S.y[k], Cc.y, Y.y), dZ = fma(-S.z[k], Cc.y, Z.y);
-                    const double s = rcube(fma(dZ, dZ, fma(dY, dY, dX * dX)));
-                    ax[k] = fma(dX, s, ax[k]); ay[k] = fma(dY, s, ay[k]); az[k] = fma(dZ, s, az[k]);
-                }
+                y2[k] = y0[k] * y0[k];
+                w[k] = fma(r2[k], y2[k], -A);
+                y2[k] = y0[k] * y2[k];
+                w[k] = fma(w[k], w[k], C0);
+                w[k] = y2[k] * w[k];
+            }
+            STEPS_STAGE_FENCE(zero, 2);
+#pragma unroll
+            for (int k = 0; k < R_I; ++k) {
+                ax[k] = fma(dX[k], w[k], ax[k]); ay[k] = fma(dY[k], w[k], ay[k]); az[k] = fma(dZ[k], w[k], az[k]);
             }
         }
 #pragma unroll

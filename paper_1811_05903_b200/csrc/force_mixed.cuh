@@ -72,7 +72,7 @@ struct MixedPath {
     // three accumulates reads <= 4 distinct register words -- measured on B200: an FFMA2 with three
     // distinct 64-bit register operands costs 3 clk instead of 2 (register-file read bandwidth is
     // 2 words/clk/lane), see DESIGN.md "what limits the mixed far body".
-    static __device__ __forceinline__ void far(const Tile& T, const IState& S, double* acc)
+    static __device__ __forceinline__ void far(const Tile& T, const IState& S, double* acc, int /*zero*/)
     {
         static_assert(R_I % 2 == 0, "i-particles are packed in pairs");
         constexpr int NP = R_I / 2;

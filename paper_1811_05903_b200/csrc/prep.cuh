@@ -56,7 +56,9 @@ __global__ void __launch_bounds__(TJ) prep_tiles(const double* __restrict__ pos,
         T.Z[t] = scaled_ok ? (float)(z * c) : STEPS_PAD_X32;
     } else {
         T.x[t] = x; T.y[t] = y; T.z[t] = z; T.m[t] = m; T.h[t] = h;
-        const double lim = 1.0e100, c = scaled_ok ? 1.0 / sqrt(m) : STEPS_PAD_C64;
+        // c_j = (1.875 m_j)^(-1/2): the fp64 far body returns s = r2^(-3/2) / 1.875 (force_fp64.cuh), so that
+        // s dX = c_j^-2 (x_j - x_i) / (1.875 r^3) = m_j (x_j - x_i) / r^3
+        const double lim = 1.0e100, c = scaled_ok ? 1.0 / sqrt(STEPS_FP64_FOLD * m) : STEPS_PAD_C64;
         scaled_ok = scaled_ok && c < lim && fabs(x * c) < lim && fabs(y * c) < lim && fabs(z * c) < lim;
         T.c[t] = scaled_ok ? c : STEPS_PAD_C64;
         T.X[t] = scaled_ok ? x * c : STEPS_PAD_X64;

@@ -111,7 +111,7 @@ int launch_forces(const double* pos, const double* mass, const double* soft, lon
     if (g_driver.load() == 1) {
         const int smem = stage_stride((int)sizeof(Tile)) + Path::NOUT * R_I * CTA_THREADS * (int)sizeof(double);
         STEPS_CUDA(cudaFuncSetAttribute(forces_v1_kernel<Path>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        forces_v1_kernel<Path><<<nb, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, i_begin, i_end, acc_out);
+        forces_v1_kernel<Path><<<nb, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, i_begin, i_end, acc_out, 0);
         g_launches++;
     } else {
         constexpr int smem = persistent_smem_bytes<Path, STAGES>();
@@ -130,7 +130,7 @@ int launch_forces(const double* pos, const double* mass, const double* soft, lon
             if (!w.ev0) { STEPS_CUDA(cudaEventCreate(&w.ev0)); STEPS_CUDA(cudaEventCreate(&w.ev1)); }
             STEPS_CUDA(cudaEventRecord(w.ev0, st));
         }
-        kern<<<P, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, i_begin, i_end, nb, w.partials);
+        kern<<<P, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, i_begin, i_end, nb, w.partials, 0);
         if (prof) { STEPS_CUDA(cudaEventRecord(w.ev1, st)); w.ev_valid = true; }
         forces_reduce_kernel<Path::NOUT><<<(int)((cnt + 255) / 256), 256, 0, st>>>(w.partials, nt, nb, P, cnt, acc_out);
         g_launches += 2;
