@@ -74,7 +74,18 @@ struct alignas(16) TileT {
     TileMeta meta;
 };
 typedef TileT<float> TileF32;             // mixed path:  9232 B
-typedef TileT<double> TileF64;            // fp64 path:  18448 B
+// fp64 path, 18448 B: the scaled copy is stored per source, (X, Y, Z, c) in 32 contiguous bytes, because the
+// fp64 far body handles ONE source per loop pass and every shared-memory load costs FP64-pipe issue time on
+// B200 (measured: ~1.8 clk per LDS.64, ~2.5 clk per LDS.128 next to a saturated DFMA stream): two LDS.128 per
+// source instead of four LDS.64.
+struct alignas(16) FarSrcF64 {
+    double X, Y, Z, c;
+};
+struct alignas(16) TileF64 {
+    FarSrcF64 far[TJ];
+    double x[TJ], y[TJ], z[TJ], m[TJ], h[TJ];
+    TileMeta meta;
+};
 static_assert(sizeof(TileF32) == 9 * TJ * 4 + 16, "TileF32 layout");
 static_assert(sizeof(TileF64) == 9 * TJ * 8 + 16, "TileF64 layout");
 static_assert(sizeof(TileF32) % 16 == 0 && sizeof(TileF64) % 16 == 0, "bulk copies need 16 B multiples");
@@ -89,6 +100,12 @@ __device__ __forceinline__ bool tile_is_far(float rminI, float rmaxI, float hmax
     const float need = (hmaxI + J.hmax) * 1.0001f + 1.0e-5f * fmaxf(rmaxI, J.rmax);
     return gap > need;
 }
+
+// Never-taken branch on bit n of `zero` (always 0, unknown to the compiler): ends a basic block, which
+// is the only ordering ptxas respects.  One uniform-datapath branch per use, no FP64-pipe work.
+#define STEPS_STAGE_FENCE(zero, n)                                                              \
+    asm volatile("{\n.reg .pred p;\n.reg .b32 t;\nand.b32 t, %0, %1;\nsetp.ne.s32 p, t, 0;\n@p trap;\n}" \
+                 :: "r"(zero), "r"(1 << (n)))
 
 // ---- packed fp32x2 arithmetic (sm_100a FADD2 / FMUL2 / FFMA2) ------------------------------
 __device__ __forceinline__ u64 pack2(float lo, float hi)

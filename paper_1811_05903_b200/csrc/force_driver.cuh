@@ -147,7 +147,8 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
 #ifdef STEPS_DIAG_ALLFAR                                   // timing diagnostic only (wrong forces): no near body
             Path::far(T, S, acc, zero);
 #else
-            if (tile_is_far(rlo, rhi, hh, T.meta)) Path::far(T, S, acc, zero);
+            // the decision is warp-uniform by construction (warp-reduced bounds); the vote tells the compiler so
+            if (__all_sync(0xffffffffu, tile_is_far(rlo, rhi, hh, T.meta))) Path::far(T, S, acc, zero);
             else Path::near(T, S, acc);
 #endif
             __syncwarp();

@@ -58,12 +58,6 @@ __device__ __forceinline__ double rsqrt_seed(double r2)
     return y;
 }
 
-// Never-taken branch on bit n of `zero` (always 0, unknown to the compiler): ends a basic block, which
-// is the only ordering ptxas respects.  One uniform-datapath branch per use, no FP64-pipe work.
-#define STEPS_STAGE_FENCE(zero, n)                                                              \
-    asm volatile("{\n.reg .pred p;\n.reg .b32 t;\nand.b32 t, %0, %1;\nsetp.ne.s32 p, t, 0;\n@p trap;\n}" \
-                 :: "r"(zero), "r"(1 << (n)))
-
 // Softened branches of Eq. 4 as g = calF / r in fp64.  Caller guarantees 0 < r2 < h^2.
 __device__ __noinline__ double spline_g_soft_f64(double r2, double h)
 {
@@ -131,7 +125,9 @@ struct Fp64Path {
         for (int k = 0; k < R_I; ++k) ax[k] = ay[k] = az[k] = 0.0;
 #pragma unroll 1
         for (int j = 0; j < TJ; ++j) {
-            const double X = T.X[j], Y = T.Y[j], Z = T.Z[j], C = T.c[j];
+            const double2 XY = *reinterpret_cast<const double2*>(&T.far[j].X);
+            const double2 ZC = *reinterpret_cast<const double2*>(&T.far[j].Z);
+            const double X = XY.x, Y = XY.y, Z = ZC.x, C = ZC.y;
             double dX[R_I], dY[R_I], dZ[R_I], r2[R_I], y0[R_I], y2[R_I], w[R_I];
             STEPS_STAGE_FENCE(zero, 0);
 #pragma unroll

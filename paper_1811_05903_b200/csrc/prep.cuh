@@ -60,10 +60,10 @@ __global__ void __launch_bounds__(TJ) prep_tiles(const double* __restrict__ pos,
         // s dX = c_j^-2 (x_j - x_i) / (1.875 r^3) = m_j (x_j - x_i) / r^3
         const double lim = 1.0e100, c = scaled_ok ? 1.0 / sqrt(STEPS_FP64_FOLD * m) : STEPS_PAD_C64;
         scaled_ok = scaled_ok && c < lim && fabs(x * c) < lim && fabs(y * c) < lim && fabs(z * c) < lim;
-        T.c[t] = scaled_ok ? c : STEPS_PAD_C64;
-        T.X[t] = scaled_ok ? x * c : STEPS_PAD_X64;
-        T.Y[t] = scaled_ok ? y * c : STEPS_PAD_X64;
-        T.Z[t] = scaled_ok ? z * c : STEPS_PAD_X64;
+        T.far[t].c = scaled_ok ? c : STEPS_PAD_C64;
+        T.far[t].X = scaled_ok ? x * c : STEPS_PAD_X64;
+        T.far[t].Y = scaled_ok ? y * c : STEPS_PAD_X64;
+        T.far[t].Z = scaled_ok ? z * c : STEPS_PAD_X64;
     }
     const bool force_near = real && m != 0.0 && !scaled_ok;
     const double r = sqrt(x * x + y * y + z * z);

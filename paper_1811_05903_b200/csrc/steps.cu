@@ -25,7 +25,10 @@ std::atomic<int> g_driver{0};   // 0 = default, 1 = simple v1 driver (cross-chec
 std::atomic<int> g_profile{0};  // 1 = bracket the force kernel with CUDA events on its stream
 
 constexpr int MAX_DEVICES = 16;
-constexpr int STAGES = 4;
+#ifndef STEPS_STAGES
+#define STEPS_STAGES 4
+#endif
+constexpr int STAGES = STEPS_STAGES;   // depth of the bulk-copy ring
 constexpr int MAX_GRID = 148 * 4;
 
 struct Workspace {
