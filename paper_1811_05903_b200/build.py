@@ -43,6 +43,19 @@ def build(force: bool = False, verbose: bool = False) -> str:
         print(log)
     if res.returncode != 0:
         raise RuntimeError("nvcc failed; see paper_1811_05903_b200/build.log")
+    # Post-link pass: operand-reuse hints on the FP64 instructions of the fp64 force kernels (sass_reuse.py).
+    # It verifies its own output by re-disassembly and restores the library if anything but the hints changed;
+    # the unpatched library is equally correct (slower), so a failure here is logged, not fatal.
+    try:
+        from . import sass_reuse
+        n = sass_reuse.patch(LIB)
+        note = f"sass_reuse: {n} instructions patched"
+    except Exception as exc:  # noqa: BLE001
+        note = f"sass_reuse: skipped ({exc})"
+    with open(os.path.join(HERE, "build.log"), "a") as f:
+        f.write("\n" + note + "\n")
+    if verbose:
+        print(note)
     return LIB
 
 

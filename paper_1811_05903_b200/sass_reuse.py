@@ -1,0 +1,219 @@
+"""Post-link pass over libsteps_b200.so: add operand-reuse hints to the FP64 instructions of the fp64 force kernels.
+
+Why (measured on B200): an FP64-pipe instruction occupies the pipe for max(2, R) clk, R = the
+number of its 64-bit register source operands that have to be read from the register file.  An operand is NOT read again
+when the previous FP64 instruction of the warp held the same register in the same operand slot and carried the SASS
+`.reuse` flag on it.  ptxas sets that flag only on part of the eligible pairs (it clears it wherever it also sets the
+scheduler's yield hint), which leaves ~10 of the 56 FP64 instructions of one pass of the far loop at 3 clk.
+
+What this pass does: inside every straight-line run of an fp64 force kernel it looks at each pair of consecutive DFMA/DMUL
+instructions (only register-neutral integer/uniform bookkeeping instructions may sit between them); where both read the
+same register pair in the same slot and nothing in between writes it, it sets the reuse bit of that slot (bits 58/59/60
+of the instruction's second word = slots A/B/C) and the no-yield bit (bit 45) on the FIRST instruction, exactly what
+ptxas emits itself for the pairs it does flag.  Nothing else changes: the pass re-disassembles the patched library and
+requires every instruction to be textually identical except for the added `.reuse` suffixes; otherwise it restores
+the original file and raises.  The flag is a hint to the operand collector (values are identical with and without it);
+the GPU parity tests run on the patched library.
+
+Usage: python -m paper_1811_05903_b200.sass_reuse [path/to/libsteps_b200.so]   (build.py calls patch() after nvcc)
+"""
+from __future__ import annotations
+
+import os
+import re
+import shutil
+import struct
+import subprocess
+import sys
+
+KERNEL_PATTERNS = ("forces_persistent_kernelINS_8Fp64Path", "forces_v1_kernelINS_8Fp64Path")
+FP64_OPS = ("DFMA", "DMUL")
+# instructions that may sit between the two FP64 instructions of a pair (ptxas itself keeps `.reuse` across these)
+NEUTRAL_OPS = ("ISETP", "VIADD", "IADD3", "IMAD", "MOV", "LOP3", "UMOV", "ULOP3", "UIADD3", "UISETP", "ULEA", "LEA", "NOP")
+BLOCK_END_OPS = ("BRA", "BSYNC", "BSSY", "EXIT", "CALL", "RET", "BAR", "WARPSYNC", "BPT", "JMP", "BRX", "YIELD", "NANOSLEEP")
+REUSE_BIT = (58, 59, 60)
+NO_YIELD_BIT = 45
+
+
+def _cuobjdump() -> str:
+    for c in ("/usr/local/cuda/bin/cuobjdump", "cuobjdump"):
+        if shutil.which(c):
+            return c
+    raise RuntimeError("cuobjdump not found")
+
+
+def disassemble(path: str) -> dict[str, list[tuple[int, str, int, int]]]:
+    """{mangled kernel name: [(address, text, word0, word1), ...]} from `cuobjdump -sass`."""
+    out = subprocess.run([_cuobjdump(), "-sass", path], capture_output=True, text=True, check=True).stdout
+    lines = out.splitlines()
+    funcs: dict[str, list[tuple[int, str, int, int]]] = {}
+    cur = None
+    for i, line in enumerate(lines):
+        m = re.search(r"Function : (\S+)", line)
+        if m:
+            cur = m.group(1)
+            funcs[cur] = []
+            continue
+        m = re.match(r"\s*/\*([0-9a-f]{4,})\*/\s+(.*?)\s*;\s*/\* (0x[0-9a-f]{16}) \*/", line)
+        if m and cur is not None:
+            hi = re.match(r"\s*/\* (0x[0-9a-f]{16}) \*/", lines[i + 1])
+            funcs[cur].append((int(m.group(1), 16), m.group(2).strip(), int(m.group(3), 16), int(hi.group(1), 16)))
+    return funcs
+
+
+def _split(text: str):
+    """-> (predicated, opcode, [operands])"""
+    pred = False
+    m = re.match(r"^@!?U?P\w+\s+", text)
+    if m:
+        pred = True
+        text = text[m.end():]
+    op = text.split()[0]
+    rest = text[len(op):].strip()
+    args = [a.strip() for a in rest.split(",")] if rest else []
+    return pred, op, args
+
+
+def _reg(arg: str):
+    """register number of a plain (possibly negated / absolute / .reuse) R operand, else None"""
+    m = re.match(r"^[-~]?\|?R(\d+)(\.reuse)?\|?$", arg)
+    return int(m.group(1)) if m else None
+
+
+def _written(op: str, args: list[str]) -> set[int]:
+    """registers a neutral instruction may write (conservative: destination and its upper neighbour)"""
+    w: set[int] = set()
+    if args:
+        r = _reg(args[0])
+        if r is not None:
+            w.update((r, r + 1))
+    return w
+
+
+def plan(ins: list[tuple[int, str, int, int]]) -> dict[int, int]:
+    """{instruction index: bits to OR into word1} for one kernel."""
+    targets = set()
+    for _, text, _, _ in ins:
+        _, op, args = _split(text)
+        if op.split(".")[0] in ("BRA", "BSSY", "CALL", "JMP"):
+            for a in args:
+                m = re.match(r"^`?\(?(0x[0-9a-f]+)\)?$", a)
+                if m:
+                    targets.add(int(m.group(1), 16))
+    patches: dict[int, int] = {}
+    prev = None                 # (index, src regs per slot, dest reg) of the previous FP64 instruction of this run
+    between: set[int] = set()   # registers written since then
+    for idx, (addr, text, _, w1) in enumerate(ins):
+        if addr in targets:
+            prev = None
+        pred, op, args = _split(text)
+        base = op.split(".")[0]
+        if base in FP64_OPS and not pred:
+            srcs = [_reg(a) for a in args[1:]]
+            dest = _reg(args[0])
+            if prev is not None:
+                pidx, psrcs, pdest = prev
+                bits = 0
+                for s in range(min(len(srcs), len(psrcs), 3)):
+                    r = srcs[s]
+                    if r is None or r != psrcs[s]:
+                        continue
+                    if pdest is not None and pdest in (r, r + 1, r - 1):
+                        continue                      # the first instruction overwrites (part of) the operand
+                    if r in between or (r + 1) in between:
+                        continue
+                    bits |= 1 << REUSE_BIT[s]
+                if bits:
+                    bits |= 1 << NO_YIELD_BIT
+                    if (ins[pidx][3] | bits) != ins[pidx][3]:
+                        patches[pidx] = patches.get(pidx, 0) | bits
+            prev = (idx, srcs, dest)
+            between = set()
+        elif base in BLOCK_END_OPS or base not in NEUTRAL_OPS or pred:
+            prev = None
+            between = set()
+        else:
+            between |= _written(op, args)
+    return patches
+
+
+def _calibrate(funcs) -> None:
+    """The bit assignment must reproduce the flags ptxas set itself, on every FP64 instruction of the library."""
+    seen = 0
+    for ins in funcs.values():
+        for _, text, _, w1 in ins:
+            pred, op, args = _split(text)
+            if op.split(".")[0] not in FP64_OPS:
+                continue
+            for s, a in enumerate(args[1:4]):
+                flagged = a.endswith(".reuse") or ".reuse|" in a
+                if _reg(a) is None and not flagged:
+                    continue
+                if bool(w1 >> REUSE_BIT[s] & 1) != flagged:
+                    raise RuntimeError(f"reuse-bit calibration failed on '{text}' (slot {s}, word1 {w1:#018x})")
+                seen += flagged
+    if seen == 0:
+        raise RuntimeError("no ptxas-set .reuse flag found to calibrate against")
+
+
+def patch(path: str, verbose: bool = False) -> int:
+    """Patch the library in place; returns the number of instructions changed.  Restores the file on any mismatch."""
+    funcs = disassemble(path)
+    _calibrate(funcs)
+    data = bytearray(open(path, "rb").read())
+    original = bytes(data)
+    changed = 0
+    expect: dict[str, dict[int, int]] = {}
+    for name, ins in funcs.items():
+        if not any(p in name for p in KERNEL_PATTERNS):
+            continue
+        code = b"".join(struct.pack("<QQ", w0, w1) for _, _, w0, w1 in ins)
+        if data.count(code) != 1:
+            raise RuntimeError(f"code of {name} not found exactly once in {path}")
+        off = data.find(code)
+        patches = plan(ins)
+        expect[name] = patches
+        for idx, bits in patches.items():
+            w1 = ins[idx][3] | bits
+            data[off + 16 * idx + 8: off + 16 * idx + 16] = struct.pack("<Q", w1)
+            changed += 1
+    if not changed:
+        return 0
+    tmp = path + ".patched"
+    with open(tmp, "wb") as f:
+        f.write(data)
+    os.chmod(tmp, os.stat(path).st_mode)
+    try:
+        after = disassemble(tmp)
+        for name, ins in funcs.items():
+            new = after[name]
+            if len(new) != len(ins):
+                raise RuntimeError(f"{name}: instruction count changed")
+            for idx, (old_i, new_i) in enumerate(zip(ins, new)):
+                if old_i[1] == new_i[1] and old_i[2:] == new_i[2:]:
+                    continue
+                if idx not in expect.get(name, {}):
+                    raise RuntimeError(f"{name}+{old_i[0]:#x}: unexpected change '{old_i[1]}' -> '{new_i[1]}'")
+                if new_i[1].replace(".reuse", "") != old_i[1].replace(".reuse", "") or old_i[2] != new_i[2]:
+                    raise RuntimeError(f"{name}+{old_i[0]:#x}: '{old_i[1]}' -> '{new_i[1]}' is not a pure reuse hint")
+                want = expect[name][idx]
+                nf = [a.endswith(".reuse") for a in _split(new_i[1])[2][1:4]]
+                for s in range(3):
+                    if want >> REUSE_BIT[s] & 1 and not (s < len(nf) and nf[s]):
+                        raise RuntimeError(f"{name}+{old_i[0]:#x}: slot {s} hint did not land: '{new_i[1]}'")
+                if verbose:
+                    print(f"{name[:40]}+{old_i[0]:#06x}: {old_i[1]}  ->  {new_i[1]}")
+        os.replace(tmp, path)
+    except Exception:
+        if os.path.exists(tmp):
+            os.remove(tmp)
+        with open(path, "wb") as f:
+            f.write(original)
+        raise
+    return changed
+
+
+if __name__ == "__main__":
+    here = os.path.dirname(os.path.abspath(__file__))
+    target = sys.argv[1] if len(sys.argv) > 1 and not sys.argv[1].startswith("-") else os.path.join(here, "libsteps_b200.so")
+    print(f"{patch(target, verbose='-v' in sys.argv)} instructions patched in {target}")
