@@ -26,10 +26,13 @@ import struct
 import subprocess
 import sys
 
-KERNEL_PATTERNS = ("forces_persistent_kernelINS_8Fp64Path", "forces_v1_kernelINS_8Fp64Path")
-FP64_OPS = ("DFMA", "DMUL")
-# instructions that may sit between the two FP64 instructions of a pair (ptxas itself keeps `.reuse` across these)
-NEUTRAL_OPS = ("ISETP", "VIADD", "IADD3", "IMAD", "MOV", "LOP3", "UMOV", "ULOP3", "UIADD3", "UISETP", "ULEA", "LEA", "NOP")
+KERNEL_PATTERNS = ("forces_persistent_kernelINS_8Fp64Path", "forces_v1_kernelINS_8Fp64Path",
+                   "forces_persistent_kernelINS_9MixedPath", "forces_v1_kernelINS_9MixedPath")
+# the 2-clk-per-warp arithmetic instructions with 64-bit register operands: FP64 and packed fp32x2
+FP64_OPS = ("DFMA", "DMUL", "FFMA2", "FMUL2")
+# instructions that may sit between the two instructions of a pair (ptxas itself keeps `.reuse` across these)
+NEUTRAL_OPS = ("ISETP", "VIADD", "IADD3", "IMAD", "MOV", "LOP3", "UMOV", "ULOP3", "UIADD3", "UISETP", "ULEA", "LEA", "NOP",
+               "MUFU")
 BLOCK_END_OPS = ("BRA", "BSYNC", "BSSY", "EXIT", "CALL", "RET", "BAR", "WARPSYNC", "BPT", "JMP", "BRX", "YIELD", "NANOSLEEP")
 REUSE_BIT = (58, 59, 60)
 NO_YIELD_BIT = 45
@@ -76,8 +79,17 @@ def _split(text: str):
 
 def _reg(arg: str):
     """register number of a plain (possibly negated / absolute / .reuse) R operand, else None"""
-    m = re.match(r"^[-~]?\|?R(\d+)(\.reuse)?\|?$", arg)
+    m = re.match(r"^[-~]?\|?R(\d+)(\.reuse)?(\.F32x2\.HI_LO|\.F32)?\|?$", arg)
     return int(m.group(1)) if m else None
+
+
+def _flagged(arg: str) -> bool:
+    return ".reuse" in arg
+
+
+def _kind(arg: str) -> str:
+    """operand width class: a packed/64-bit pair and a broadcast 32-bit scalar of the same number are different operands"""
+    return "s" if arg.endswith(".F32") or arg.endswith(".F32|") else "p"
 
 
 def _written(op: str, args: list[str]) -> set[int]:
@@ -109,15 +121,15 @@ def plan(ins: list[tuple[int, str, int, int]]) -> dict[int, int]:
         pred, op, args = _split(text)
         base = op.split(".")[0]
         if base in FP64_OPS and not pred:
-            srcs = [_reg(a) for a in args[1:]]
+            srcs = [(_reg(a), _kind(a)) if _reg(a) is not None else None for a in args[1:]]
             dest = _reg(args[0])
             if prev is not None:
                 pidx, psrcs, pdest = prev
                 bits = 0
                 for s in range(min(len(srcs), len(psrcs), 3)):
-                    r = srcs[s]
-                    if r is None or r != psrcs[s]:
+                    if srcs[s] is None or srcs[s] != psrcs[s]:
                         continue
+                    r = srcs[s][0]
                     if pdest is not None and pdest in (r, r + 1, r - 1):
                         continue                      # the first instruction overwrites (part of) the operand
                     if r in between or (r + 1) in between:
@@ -146,7 +158,7 @@ def _calibrate(funcs) -> None:
             if op.split(".")[0] not in FP64_OPS:
                 continue
             for s, a in enumerate(args[1:4]):
-                flagged = a.endswith(".reuse") or ".reuse|" in a
+                flagged = _flagged(a)
                 if _reg(a) is None and not flagged:
                     continue
                 if bool(w1 >> REUSE_BIT[s] & 1) != flagged:
@@ -197,7 +209,7 @@ def patch(path: str, verbose: bool = False) -> int:
                 if new_i[1].replace(".reuse", "") != old_i[1].replace(".reuse", "") or old_i[2] != new_i[2]:
                     raise RuntimeError(f"{name}+{old_i[0]:#x}: '{old_i[1]}' -> '{new_i[1]}' is not a pure reuse hint")
                 want = expect[name][idx]
-                nf = [a.endswith(".reuse") for a in _split(new_i[1])[2][1:4]]
+                nf = [_flagged(a) for a in _split(new_i[1])[2][1:4]]
                 for s in range(3):
                     if want >> REUSE_BIT[s] & 1 and not (s < len(nf) and nf[s]):
                         raise RuntimeError(f"{name}+{old_i[0]:#x}: slot {s} hint did not land: '{new_i[1]}'")
