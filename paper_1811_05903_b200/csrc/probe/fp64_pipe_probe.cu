@@ -90,6 +90,8 @@ __global__ void __launch_bounds__(THREADS, 1) lds_kernel(const double* in, doubl
 // ---- 3. the 14-instruction far body in isolation ----------------------------------------------------------------------------
 // ORDER 0: two sources x 4 i per pass, written interaction by interaction (ptxas schedules freely)
 // ORDER 1: one source x 4 i per pass in three stages separated by never-taken branches (the body of force_fp64.cuh)
+// ORDER 2: as 1, the tile walked by pointer increment: ptxas then addresses the loads through a uniform register
+//          (LDS [UR]) instead of a per-lane register (LDS [R+UR]), which needs no register-file read
 __device__ __forceinline__ double seed64h(double r2) { double y; asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(r2)); return y; }
 #define FENCE(zero, n) asm volatile("{\n.reg .pred p;\n.reg .b32 t;\nand.b32 t, %0, %1;\nsetp.ne.s32 p, t, 0;\n@p trap;\n}" :: "r"(zero), "r"(1 << (n)))
 template <int ORDER>
@@ -121,9 +123,16 @@ __global__ void __launch_bounds__(THREADS, 1) far_kernel(const double* __restric
                 }
             }
         } else {
+            const double* src = &T[0][0];
 #pragma unroll 1
             for (int j = 0; j < 256; ++j) {
-                const double2 XY = *reinterpret_cast<const double2*>(&T[j][0]), ZC = *reinterpret_cast<const double2*>(&T[j][2]);
+                double2 XY, ZC;
+                if (ORDER == 2) {
+                    XY = *reinterpret_cast<const double2*>(src); ZC = *reinterpret_cast<const double2*>(src + 2);
+                    src += 4;
+                } else {
+                    XY = *reinterpret_cast<const double2*>(&T[j][0]); ZC = *reinterpret_cast<const double2*>(&T[j][2]);
+                }
                 double dX[RI], dY[RI], dZ[RI], r2[RI], y0[RI], y2[RI], w[RI];
                 FENCE(zero, 0);
 #pragma unroll
@@ -210,5 +219,6 @@ int main()
     run_lds<2>("56 two-source DFMA + 2 LDS.128 per pass", 2.0);
     run_far<0>("14 instr, 2 sources x 4 i per pass, free order");
     run_far<1>("14 instr, 1 source x 4 i per pass, staged with fences");
+    run_far<2>("14 instr, staged with fences, uniform-register LDS address");
     return 0;
 }
