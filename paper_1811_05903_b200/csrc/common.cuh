@@ -22,6 +22,10 @@ typedef unsigned long long u64;
 #ifndef STEPS_FAR_UNROLL
 #define STEPS_FAR_UNROLL 1
 #endif
+// fp64 path: far tiles summed in registers between two additions to the double-double accumulator (force_fp64.cuh)
+#ifndef STEPS_FP64_FAR_TILES_PER_FLUSH
+#define STEPS_FP64_FAR_TILES_PER_FLUSH 4
+#endif
 // Constant folded into the scaled copy of the fp64 tiles: c_j = (STEPS_FP64_FOLD m_j)^(-1/2) (force_fp64.cuh).
 #define STEPS_FP64_FOLD 1.875
 #ifndef STEPS_MIXED_ACC_SCALAR

@@ -78,6 +78,14 @@ __device__ __forceinline__ void load_i_block(typename Path::IState& S, const dou
     }
 }
 
+// FarSums of the fp64 path are register sums (zeroed); those of the mixed path only carry the accumulator pointer.
+template <typename Path>
+__device__ __forceinline__ void init_far_sums(typename Path::FarSums& F, double* acc)
+{
+    if constexpr (Path::NOUT == 3) F.acc = acc;
+    else Path::far_zero(F);
+}
+
 __host__ __device__ constexpr int stage_stride(int tile_bytes) { return (tile_bytes + 127) / 128 * 128; }
 
 template <typename Path, int STAGES>
@@ -139,22 +147,32 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
 #pragma unroll
         for (int q = 0; q < Path::NOUT * R_I; ++q) acc[q * CTA_THREADS] = 0.0;
 
+        typename Path::FarSums F;
+        init_far_sums<Path>(F, acc);
+        int pending = 0;                                    // far tiles summed in F since its last flush
         for (int c = 0; c < cnt; ++c, ++it) {
             if (threadIdx.x == 0 && it + STAGES - 1 < total) produce(it + STAGES - 1);
             const int s = it % STAGES;
             mbar_wait(&full_bar[s], (it / STAGES) & 1);
             const Tile& T = *reinterpret_cast<const Tile*>(smem_raw + s * STRIDE);
 #ifdef STEPS_DIAG_ALLFAR                                   // timing diagnostic only (wrong forces): no near body
-            Path::far(T, S, acc, zero);
+            Path::far(T, S, F, zero);
+            if (++pending >= Path::FAR_TILES_PER_FLUSH) { Path::far_flush(F, acc); pending = 0; }
 #else
             // the decision is warp-uniform by construction (warp-reduced bounds); the vote tells the compiler so
-            if (__all_sync(0xffffffffu, tile_is_far(rlo, rhi, hh, T.meta))) Path::far(T, S, acc, zero);
-            else Path::near(T, S, acc);
+            if (__all_sync(0xffffffffu, tile_is_far(rlo, rhi, hh, T.meta))) {
+                Path::far(T, S, F, zero);
+                if (++pending >= Path::FAR_TILES_PER_FLUSH) { Path::far_flush(F, acc); pending = 0; }
+            } else {
+                if (pending) { Path::far_flush(F, acc); pending = 0; }
+                Path::near(T, S, acc);
+            }
 #endif
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty_bar[s]);
         }
 
+        if (pending) Path::far_flush(F, acc);
         double* out = partials + ((long long)(b + blockIdx.x) * Path::NOUT) * IB + warp * WARP_I + lane;
 #pragma unroll
         for (int cc = 0; cc < Path::NOUT; ++cc)
@@ -219,8 +237,14 @@ forces_v1_kernel(const double* __restrict__ pos, const double* __restrict__ soft
             for (int q = threadIdx.x; q < (int)(sizeof(Tile) / 16); q += CTA_THREADS) dst[q] = src[q];
         }
         __syncthreads();
-        if (tile_is_far(rlo, rhi, hh, tile.meta)) Path::far(tile, S, acc, zero);
-        else Path::near(tile, S, acc);
+        if (tile_is_far(rlo, rhi, hh, tile.meta)) {
+            typename Path::FarSums F;
+            init_far_sums<Path>(F, acc);
+            Path::far(tile, S, F, zero);
+            Path::far_flush(F, acc);                       // the cross-check driver flushes at every tile
+        } else {
+            Path::near(tile, S, acc);
+        }
     }
     const long long cnt = i_end - i_begin;
 #pragma unroll

@@ -116,13 +116,30 @@ struct Fp64Path {
         return fma(t, p, q3);
     }
 
-    static __device__ __forceinline__ void far(const Tile& T, const IState& S, double* acc, int zero)
+    // Running sums of the far tiles, kept in registers ACROSS tiles: the persistent driver adds them to the double-double
+    // accumulator only every FAR_TILES_PER_FLUSH far tiles (and before a near tile / at the end of the i-block), so
+    // the far loop of the next tile starts without waiting for the last DFMAs of this one to drain.
+    struct FarSums {
+        double ax[R_I], ay[R_I], az[R_I];
+    };
+    static constexpr int FAR_TILES_PER_FLUSH = STEPS_FP64_FAR_TILES_PER_FLUSH;
+    static __device__ __forceinline__ void far_zero(FarSums& F)
+    {
+#pragma unroll
+        for (int k = 0; k < R_I; ++k) F.ax[k] = F.ay[k] = F.az[k] = 0.0;
+    }
+    static __device__ __forceinline__ void far_flush(FarSums& F, double* acc)
+    {
+#pragma unroll
+        for (int k = 0; k < R_I; ++k) { flush(acc, 0, k, F.ax[k]); flush(acc, 1, k, F.ay[k]); flush(acc, 2, k, F.az[k]); }
+        far_zero(F);
+    }
+
+    static __device__ __forceinline__ void far(const Tile& T, const IState& S, FarSums& F, int zero)
     {
         constexpr double A = 1.4;
         constexpr double C0 = 1.0 / STEPS_FP64_FOLD - (1.0 - A) * (1.0 - A);   // (u - A)^2 + C0 = 1/1.875 at u = 1
-        double ax[R_I], ay[R_I], az[R_I];
-#pragma unroll
-        for (int k = 0; k < R_I; ++k) ax[k] = ay[k] = az[k] = 0.0;
+        double (&ax)[R_I] = F.ax, (&ay)[R_I] = F.ay, (&az)[R_I] = F.az;
 #pragma unroll 1
         for (int j = 0; j < TJ; ++j) {
             const double2 XY = *reinterpret_cast<const double2*>(&T.far[j].X);
@@ -155,8 +172,6 @@ struct Fp64Path {
                 ax[k] = fma(dX[k], w[k], ax[k]); ay[k] = fma(dY[k], w[k], ay[k]); az[k] = fma(dZ[k], w[k], az[k]);
             }
         }
-#pragma unroll
-        for (int k = 0; k < R_I; ++k) { flush(acc, 0, k, ax[k]); flush(acc, 1, k, ay[k]); flush(acc, 2, k, az[k]); }
     }
 
     static __device__ __forceinline__ void near(const Tile& T, const IState& S, double* acc)
