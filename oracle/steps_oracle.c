@@ -21,7 +21,8 @@
  * continuity, the two-body closed form, exact Newtonian r >= h, shell theorem on
  * regular polyhedra and a Fibonacci shell, Newton's third law, symmetries, an
  * independent numpy longdouble brute force on N <= 8, RK4 a(t) vs closed forms, drag
- * and background-term closed forms with 2nd-order convergence, Kepler orbit.
+ * and background-term closed forms with 2nd-order convergence, Kepler orbit; Eq. 12 time step against the two-body
+ * closed form, its scaling laws, the dt_max clamp and a numpy brute force.
  * Parity status: every function below is pinned (none "parity unpinned"); the choice
  * of how the drag enters the kick (reading #8) is a reading the paper does not fix.
  */
@@ -200,6 +201,32 @@ void oracle_momentum(const double *vel, const double *mass, long long N, double 
         neumaier_add(&sa, &ca, mass[i] * sqrt(vx * vx + vy * vy + vz * vz));
     }
     out4[0] = s[0] + c[0]; out4[1] = s[1] + c[1]; out4[2] = s[2] + c[2]; out4[3] = sa + ca;
+}
+
+/*
+ * Adaptive time step, Eq. 12 (L113-116):
+ *     dt = min[ dt_max, min_i sqrt( 2 eta_i eps / |A_i| ) ],   eta_i = 2.8 h_i  (L116, literal).
+ * Readings (#11): one global step, the minimum over all particles (the integrator of Eq. 9-11 advances
+ * every particle with the same dt); A_i is the acceleration that the kick applies, without the velocity-dependent
+ * drag: A_i = coef (acc_i + B x_i) with coef = G a^-3 (Eq. 8, reading #6).  |A_i| = 0 puts no limit on dt.
+ * Plain loop, fp64, in the order of the formula.
+ */
+double oracle_timestep(const double *pos, const double *acc, const double *soft, long long N, double coef, double B,
+                       double eps, double dt_max)
+{
+    double dt = dt_max;
+    for (long long i = 0; i < N; ++i) {
+        const double Ax = coef * (acc[i] + B * pos[i]);
+        const double Ay = coef * (acc[N + i] + B * pos[N + i]);
+        const double Az = coef * (acc[2 * N + i] + B * pos[2 * N + i]);
+        const double A = sqrt(Ax * Ax + Ay * Ay + Az * Az);
+        if (A > 0.0) {
+            const double eta = 2.8 * soft[i];
+            const double dti = sqrt(2.0 * eta * eps / A);
+            if (dti < dt) dt = dti;
+        }
+    }
+    return dt;
 }
 
 int oracle_num_threads(void)

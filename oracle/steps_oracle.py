@@ -50,6 +50,8 @@ def lib():
         L.oracle_kdk_coeffs.argtypes = [C.c_double, C.c_double, C.c_double, C.POINTER(Cosmo), dp]
         L.oracle_momentum.restype = None
         L.oracle_momentum.argtypes = [dp, dp, C.c_longlong, dp]
+        L.oracle_timestep.restype = C.c_double
+        L.oracle_timestep.argtypes = [dp, dp, dp, C.c_longlong, C.c_double, C.c_double, C.c_double, C.c_double]
         L.oracle_num_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -122,6 +124,15 @@ def momentum(vel, mass) -> np.ndarray:
     out = np.empty(4)
     lib().oracle_momentum(_dp(vel), _dp(mass), mass.shape[0], _dp(out))
     return out
+
+
+def timestep(pos, acc, soft, coef: float, B: float, eps: float, dt_max: float) -> float:
+    """PAPER.md Eq. 12 (L113-116): global adaptive step min[dt_max, min_i sqrt(2 * 2.8 h_i * eps / |A_i|)],
+    A_i = coef (acc_i + B x_i)."""
+    pos, acc, soft = _f64(pos), _f64(acc), _f64(soft)
+    n = soft.shape[0]
+    assert pos.shape == (3, n) and acc.shape == (3, n)
+    return float(lib().oracle_timestep(_dp(pos), _dp(acc), _dp(soft), n, coef, B, eps, dt_max))
 
 
 def num_threads() -> int:

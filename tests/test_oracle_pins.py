@@ -417,3 +417,50 @@ def test_kdk_coefficient_form_equals_literal_step(oracle):
     np.testing.assert_allclose(vel, v2, rtol=1e-12, atol=1e-18)
     p = oracle.momentum(vel, ps.mass)
     assert np.linalg.norm(p[:3]) / p[3] < 1e-12
+
+
+# ---- Eq. 12 (L113-116): adaptive global time step --------------------------------------------------------------
+def _two_body(d, m1, m2, h1, h2):
+    pos = np.array([[0.0, d], [0.0, 0.0], [0.0, 0.0]])
+    return pos, np.array([m1, m2]), np.array([h1, h2])
+
+
+def test_timestep_two_body_closed_form(oracle):
+    """Two bodies at separation d >= h1 + h2: |A_1| = G m_2 / d^2, |A_2| = G m_1 / d^2 (Eq. 4 third case), so
+    dt = min_i sqrt(2 * 2.8 h_i * eps * d^2 / (G m_other)) -- typed out here from Eq. 12, not from the oracle."""
+    d, m1, m2, h1, h2, G, eps = 3.0, 2.0, 5.0, 0.3, 0.1, 1.7, 0.025
+    pos, mass, soft = _two_body(d, m1, m2, h1, h2)
+    acc = oracle.forces(pos, mass, soft)
+    dt = oracle.timestep(pos, acc, soft, G, 0.0, eps, 1e30)
+    dt1 = math.sqrt(2 * 2.8 * h1 * eps * d * d / (G * m2))
+    dt2 = math.sqrt(2 * 2.8 * h2 * eps * d * d / (G * m1))
+    assert dt == pytest.approx(min(dt1, dt2), rel=1e-14)
+    assert min(dt1, dt2) == dt2 and dt1 / dt2 > 1.05          # the pin would notice the wrong particle being picked
+
+
+def test_timestep_scalings_clamp_and_zero_acceleration(oracle):
+    rng = np.random.default_rng(12)
+    n = 200
+    pos = rng.normal(size=(3, n)); acc = rng.normal(size=(3, n)); soft = rng.uniform(0.01, 0.1, n)
+    base = oracle.timestep(pos, acc, soft, 1.0, 0.0, 0.01, 1e30)
+    # dt ~ sqrt(eps), ~ sqrt(h), ~ |A|^-1/2 (Eq. 12)
+    assert oracle.timestep(pos, acc, soft, 1.0, 0.0, 0.04, 1e30) == pytest.approx(2 * base, rel=1e-14)
+    assert oracle.timestep(pos, acc, 4 * soft, 1.0, 0.0, 0.01, 1e30) == pytest.approx(2 * base, rel=1e-14)
+    assert oracle.timestep(pos, acc, soft, 4.0, 0.0, 0.01, 1e30) == pytest.approx(base / 2, rel=1e-14)
+    assert oracle.timestep(pos, 4 * acc, soft, 1.0, 0.0, 0.01, 1e30) == pytest.approx(base / 2, rel=1e-14)
+    # dt_max clamps; a particle at rest in the force field puts no limit
+    assert oracle.timestep(pos, acc, soft, 1.0, 0.0, 0.01, base / 3) == base / 3
+    assert oracle.timestep(pos, 0 * acc, soft, 1.0, 0.0, 0.01, 7.5) == 7.5
+    # the background term enters A_i = coef (acc_i + B x_i): with acc = -B x the particle feels nothing
+    assert oracle.timestep(pos, -0.3 * pos, soft, 2.0, 0.3, 0.01, 7.5) == 7.5
+
+
+def test_timestep_against_numpy_brute_force(oracle):
+    rng = np.random.default_rng(13)
+    n = 1000
+    pos = rng.normal(size=(3, n)); acc = rng.normal(size=(3, n)) * 10.0 ** rng.uniform(-3, 3, n)
+    soft = 10.0 ** rng.uniform(-3, 0, n)
+    coef, B, eps = 0.37, 0.011, 0.025
+    A = np.linalg.norm(coef * (acc + B * pos), axis=0)
+    want = float(np.min(np.sqrt(2 * 2.8 * soft * eps / A)))
+    assert oracle.timestep(pos, acc, soft, coef, B, eps, 1e30) == pytest.approx(want, rel=1e-14)
