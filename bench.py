@@ -43,7 +43,7 @@ UNIT = "interactions/s"
 LCDM = dict(H0=0.0288675134594813, Omega_m=0.3, Omega_r=0.0, Omega_L=0.7, Omega_k=0.0)
 # DRAM bytes per launch of the force kernel from the committed `ncu --set full` capture
 # (profiles/r01_force_kernels_ncu.md); None until captured.
-NCU_DRAM_BYTES = {"mixed": 84.516096e6 + 19.605248e6, "fp64": 5.559068e9 + 79.579904e6}
+NCU_DRAM_BYTES = {"mixed": 84.567040e6 + 18.440448e6, "fp64": 5.357882e9 + 89.916160e6}
 
 
 class ClockSampler:

@@ -136,6 +136,15 @@ int steps_kdk_schedule(double a_n, double dt, double G, const steps_cosmology *c
 int steps_momentum(const double *vec, const double *mass, long long N, double *out4,
                    steps_stream_t stream);
 
+/* Adaptive global time step, Eq. 12 (L113-116):
+ *     dt = min[ dt_max, min_i sqrt(2 eta_i eps / |A_i|) ],  eta_i = 2.8 soft[i]  (L116, literal),
+ * A_i = coef (acc_i + B pos_i) = the acceleration the kick applies, without the drag (coef = G a^-3, reading #6/#11);
+ * |A_i| = 0 puts no limit.  pos, acc: SoA 3N device doubles; soft: N; dt_out: ONE device double (stream-ordered, the
+ * host is not synchronised -- read it back when the next step's coefficients are needed).  Exact minimum, so the
+ * result does not depend on the reduction order.  STEPS_EINVAL for null pointers, N < 1, eps <= 0 or dt_max <= 0. */
+int steps_timestep(const double *pos, const double *acc, const double *soft, long long N, double coef,
+                   double B, double eps, double dt_max, double *dt_out, steps_stream_t stream);
+
 /* ---- housekeeping ------------------------------------------------------------------ */
 
 int steps_reserve(long long N);          /* allocate workspace for up to N particles now */

@@ -62,4 +62,41 @@ __global__ void momentum_stage2(const double* __restrict__ partial, int nblocks,
     }
 }
 
+// ---- adaptive global time step, Eq. 12 (L113-116) ---------------------------------------------------------
+// dt = min[dt_max, min_i sqrt(2 eta_i eps / |A_i|)], eta_i = 2.8 h_i, A_i = coef (acc_i + B x_i) (reading #11).
+// Each particle's candidate is formed exactly as the formula reads (IEEE fp64 sqrt and divide); the minimum is exact, so
+// the result does not depend on the reduction order.  |A_i| = 0 puts no limit.  48 B read per particle, HBM/L2-bound.
+__global__ void __launch_bounds__(256) timestep_stage1(const double* __restrict__ pos, const double* __restrict__ acc,
+                                                        const double* __restrict__ soft, long long N, double coef, double B,
+                                                        double eps, double dt_max, double* __restrict__ partial)
+{
+    double dt = dt_max;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
+        const double Ax = coef * (acc[i] + B * pos[i]);
+        const double Ay = coef * (acc[N + i] + B * pos[N + i]);
+        const double Az = coef * (acc[2 * N + i] + B * pos[2 * N + i]);
+        const double A = sqrt(Ax * Ax + Ay * Ay + Az * Az);
+        if (A > 0.0) dt = fmin(dt, sqrt(2.0 * (2.8 * soft[i]) * eps / A));
+    }
+    __shared__ double sh[8];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) dt = fmin(dt, __shfl_down_sync(0xffffffffu, dt, o));
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = dt;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < 8; ++w) dt = fmin(dt, sh[w]);
+        partial[blockIdx.x] = dt;
+    }
+}
+
+__global__ void timestep_stage2(const double* __restrict__ partial, int nblocks, double* __restrict__ out)
+{
+    if (threadIdx.x == 0) {
+        double dt = partial[0];
+        for (int b = 1; b < nblocks; ++b) dt = fmin(dt, partial[b]);
+        out[0] = dt;
+    }
+}
+
 }  // namespace steps

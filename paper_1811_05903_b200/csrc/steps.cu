@@ -288,6 +288,24 @@ int steps_momentum(const double* vec, const double* mass, long long N, double* o
     return STEPS_OK;
 }
 
+int steps_timestep(const double* pos, const double* acc, const double* soft, long long N, double coef, double B,
+                   double eps, double dt_max, double* dt_out, steps_stream_t stream)
+{
+    if (!pos || !acc || !soft || !dt_out || N < 1) return STEPS_EINVAL;
+    if (!(eps > 0.0) || !(dt_max > 0.0)) return STEPS_EINVAL;
+    int dev;
+    int rc = current_device(&dev);
+    if (rc != STEPS_OK) return rc;
+    rc = ensure_workspace(dev, 1);
+    if (rc != STEPS_OK) return rc;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    timestep_stage1<<<MOM_BLOCKS, 256, 0, st>>>(pos, acc, soft, N, coef, B, eps, dt_max, g_ws[dev].mom_partial);
+    timestep_stage2<<<1, 32, 0, st>>>(g_ws[dev].mom_partial, MOM_BLOCKS, dt_out);
+    g_launches += 2;
+    STEPS_CUDA(cudaGetLastError());
+    return STEPS_OK;
+}
+
 int steps_reserve(long long N)
 {
     if (N < 1) return STEPS_EINVAL;

@@ -237,6 +237,55 @@ def _config4(oracle, n):
     return synth.config4_ics(n, synth.SEED_BASE + 4, vel_factor=vf)
 
 
+# ---- Eq. 12 (L113-116): adaptive global time step -----------------------------------------------------------------
+@pytest.mark.gpu
+@pytest.mark.parametrize("n", [1, 2, 255, 4096, 65536, 100003])
+def test_timestep_matches_oracle(S, oracle, n):
+    import torch
+    ps = synth.config(0, n) if n >= 2 else synth.config(0, 1)
+    rng = np.random.default_rng(1200 + n)
+    acc = rng.normal(size=(3, n)) * 10.0 ** rng.uniform(-4, 2, n)
+    out = torch.empty(1, dtype=torch.float64, device="cuda")
+    for coef, B, eps, dt_max in [(1.0, 0.0, 0.025, 1e30), (51.0 ** 3, 1.25e-4, 0.01, 1e30), (1.0, 1.25e-4, 0.025, 1e-6)]:
+        S.steps_timestep(dev(ps.pos), dev(acc), dev(ps.soft), coef, B, eps, dt_max, out)
+        want = oracle.timestep(ps.pos, acc, ps.soft, coef, B, eps, dt_max)
+        # sqrt and divide are IEEE on both sides; the only freedom is FMA contraction inside |A_i| (<= 2 ulp)
+        assert out.item() == pytest.approx(want, rel=4e-16), (n, coef, out.item(), want)
+    # no acceleration anywhere: dt_max comes back exactly
+    S.steps_timestep(dev(ps.pos), dev(0 * acc), dev(ps.soft), 1.0, 0.0, 0.025, 0.75, out)
+    assert out.item() == 0.75
+
+
+@pytest.mark.gpu
+def test_adaptive_kdk_run_follows_the_oracle(S, oracle):
+    """20 comoving KDK steps whose length is set by Eq. 12 from the forces of the previous step, library vs oracle:
+    the step lengths agree to rounding and so do the trajectories."""
+    import torch
+    from paper_1811_05903_b200 import integrate
+    ps = _config4(oracle, 2048)
+    B, G, eps, dt_max = 1.0 / ps.r_cut ** 3, 1.0, 0.025, 0.5
+    dpos, dvel, dm, dh = dev(ps.pos), dev(ps.vel), dev(ps.mass), dev(ps.soft)
+    dacc = torch.empty_like(dpos)
+    S.steps_forces(dpos, dm, dh, dacc)
+    pos, vel = ps.pos.copy(), ps.vel.copy()
+    acc = oracle.forces(pos, ps.mass, ps.soft)
+    a_lib = a_ref = 1 / 51
+    out = torch.empty(1, dtype=torch.float64, device="cuda")
+    cosmo = S.Cosmology(**LCDM)
+    for step in range(20):
+        S.steps_timestep(dpos, dacc, dh, G / a_lib ** 3, B, eps, dt_max, out)
+        dt_lib = out.item()
+        dt_ref = oracle.timestep(pos, acc, ps.soft, G / a_ref ** 3, B, eps, dt_max)
+        assert dt_lib == pytest.approx(dt_ref, rel=1e-11), step
+        a_lib = integrate.run_kdk(dpos, dvel, dacc, dm, dh, a_lib, [dt_lib], cosmo, G, B)
+        a_ref = oracle.kdk_step(pos, vel, acc, ps.mass, ps.soft, a_ref, dt_ref, G, B, LCDM)
+    assert a_lib == pytest.approx(a_ref, rel=1e-11)
+    s = (ps.mass * (4 * np.pi / 3) * ps.r_cut ** 3) ** (1 / 3)
+    dx = np.linalg.norm(dpos.cpu().numpy() - pos, axis=0) / s
+    print(f"adaptive run, 20 steps: a = {a_ref:.6f}, max |dx|/s library-vs-oracle {dx.max():.3e}")
+    assert dx.max() < 1e-9
+
+
 def test_config4_lockstep_200_steps_8192(S, oracle):
     """Config 4 at N = 8192, every one of the 200 comoving KDK steps (a: 1/51 -> 1): the library steps
     from the ORACLE's state (x_n, v_n, acc_n) and must land on the oracle's (x_{n+1}, v_{n+1},
