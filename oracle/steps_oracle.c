@@ -229,6 +229,29 @@ double oracle_timestep(const double *pos, const double *acc, const double *soft,
     return dt;
 }
 
+/*
+ * Net-force residual, the convergence monitor of glass generation (section 3.1 "the net gravitational
+ * force acting on each particle is as small as possible"; L245 "integrating Eq. 8 with reversed gravity"):
+ *     g_i = acc_i + B x_i        (the bracket of Eq. 8 L88 with reading #6: pair sum + background term, G = 1)
+ *     out[0] = sum_i |g_i|^2     out[1] = max_i |g_i|
+ * Neumaier-compensated sum, plain loop.  (Reversed gravity itself needs no function: it is G < 0 in the kick.)
+ */
+void oracle_force_residual(const double *pos, const double *acc, long long N, double B, double *out2)
+{
+    double s = 0.0, c = 0.0, mx = 0.0;
+    for (long long i = 0; i < N; ++i) {
+        const double gx = acc[i] + B * pos[i];
+        const double gy = acc[N + i] + B * pos[N + i];
+        const double gz = acc[2 * N + i] + B * pos[2 * N + i];
+        const double g2 = gx * gx + gy * gy + gz * gz;
+        neumaier_add(&s, &c, g2);
+        const double g = sqrt(g2);
+        if (g > mx) mx = g;
+    }
+    out2[0] = s + c;
+    out2[1] = mx;
+}
+
 int oracle_num_threads(void)
 {
 #ifdef _OPENMP

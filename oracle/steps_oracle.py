@@ -52,6 +52,8 @@ def lib():
         L.oracle_momentum.argtypes = [dp, dp, C.c_longlong, dp]
         L.oracle_timestep.restype = C.c_double
         L.oracle_timestep.argtypes = [dp, dp, dp, C.c_longlong, C.c_double, C.c_double, C.c_double, C.c_double]
+        L.oracle_force_residual.restype = None
+        L.oracle_force_residual.argtypes = [dp, dp, C.c_longlong, C.c_double, dp]
         L.oracle_num_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -133,6 +135,15 @@ def timestep(pos, acc, soft, coef: float, B: float, eps: float, dt_max: float) -
     n = soft.shape[0]
     assert pos.shape == (3, n) and acc.shape == (3, n)
     return float(lib().oracle_timestep(_dp(pos), _dp(acc), _dp(soft), n, coef, B, eps, dt_max))
+
+
+def force_residual(pos, acc, B: float) -> np.ndarray:
+    """Glass-generation monitor: [sum_i |acc_i + B x_i|^2, max_i |acc_i + B x_i|]."""
+    pos, acc = _f64(pos), _f64(acc)
+    assert pos.shape == acc.shape and pos.shape[0] == 3
+    out = np.zeros(2)
+    lib().oracle_force_residual(_dp(pos), _dp(acc), pos.shape[1], B, _dp(out))
+    return out
 
 
 def num_threads() -> int:

@@ -464,3 +464,46 @@ def test_timestep_against_numpy_brute_force(oracle):
     A = np.linalg.norm(coef * (acc + B * pos), axis=0)
     want = float(np.min(np.sqrt(2 * 2.8 * soft * eps / A)))
     assert oracle.timestep(pos, acc, soft, coef, B, eps, 1e30) == pytest.approx(want, rel=1e-14)
+
+
+# ---- glass generation monitor (section 3.1): net force residual g_i = acc_i + B x_i -------------------
+def test_force_residual_closed_forms_and_brute_force(oracle):
+    rng = np.random.default_rng(31)
+    n, B = 500, 0.37
+    pos = rng.normal(size=(3, n))
+    # a particle alone in the background (pair sum 0): g = B x exactly; a particle in exact balance: g = 0
+    r = oracle.force_residual(pos, np.zeros((3, n)), B)
+    assert r[0] == pytest.approx(B * B * np.sum(pos ** 2), rel=1e-14)
+    assert r[1] == pytest.approx(B * np.max(np.linalg.norm(pos, axis=0)), rel=1e-15)
+    assert np.all(oracle.force_residual(pos, -B * pos, B) == 0.0)
+    acc = rng.normal(size=(3, n))
+    g = np.linalg.norm(acc.astype(np.longdouble) + np.longdouble(B) * pos.astype(np.longdouble), axis=0)
+    r = oracle.force_residual(pos, acc, B)
+    assert r[0] == pytest.approx(float(np.sum(g * g)), rel=1e-15)
+    assert r[1] == pytest.approx(float(np.max(g)), rel=1e-15)
+
+
+def test_force_residual_of_a_uniform_ball_is_small_and_reversed_gravity_lowers_it(oracle):
+    """Shell theorem (L86): inside a uniform ball of total mass M and radius R the pair sum is -(M/R^3) x, so with
+    B = M/R^3 (reading #7) the residual of a dense random sampling is only its Poisson noise.  Evolving that sampling
+    with REVERSED gravity in EdS (L245: G < 0 in the kick, nothing else changes) must lower the rms residual."""
+    rng = np.random.default_rng(32)
+    n, R = 1500, 1.0
+    u = rng.normal(size=(3, n)); u /= np.linalg.norm(u, axis=0)
+    pos = np.ascontiguousarray(u * R * rng.uniform(0, 1, n) ** (1 / 3))
+    mass = np.full(n, 1.0 / n); soft = np.full(n, 0.5 * (4 * np.pi / 3 / n) ** (1 / 3) * R)
+    B = 1.0 / R ** 3
+    acc = oracle.forces(pos, mass, soft)
+    inner = np.linalg.norm(pos, axis=0) < 0.6 * R
+    rms_pair = np.sqrt(np.mean(np.sum(acc[:, inner] ** 2, axis=0)))
+    g = acc + B * pos
+    rms0 = np.sqrt(np.mean(np.sum(g[:, inner] ** 2, axis=0)))
+    assert rms0 < 0.5 * rms_pair                      # background term cancels the mean pull (sign and size of B)
+    cosmo = dict(H0=math.sqrt(2 * B), Omega_m=1.0, Omega_r=0.0, Omega_L=0.0, Omega_k=0.0)
+    vel = np.zeros_like(pos); a = 0.05
+    r_start = oracle.force_residual(pos, acc, B)[0]
+    for _ in range(40):
+        dt = oracle.timestep(pos, acc, soft, 1.0 / a ** 3, B, 0.025, 1e30)
+        a = oracle.kdk_step(pos, vel, acc, mass, soft, a, dt, -1.0, B, cosmo)        # G = -1: reversed gravity
+    r_end = oracle.force_residual(pos, acc, B)[0]
+    assert r_end < 0.5 * r_start, (r_start, r_end)
