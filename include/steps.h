@@ -145,6 +145,14 @@ int steps_momentum(const double *vec, const double *mass, long long N, double *o
 int steps_timestep(const double *pos, const double *acc, const double *soft, long long N, double coef,
                    double B, double eps, double dt_max, double *dt_out, steps_stream_t stream);
 
+/* Glass generation (section 3.1).  Reversed gravity needs no call of its
+ * own: it is G < 0 in steps_kdk_schedule (both the pair sum and the background term change sign, the uniform sphere
+ * stays static).  This is its convergence monitor, the net force per particle g_i = acc_i + B pos_i:
+ *     out2 (device, 2 doubles) = { sum_i |g_i|^2, max_i |g_i| }.
+ * pos, acc: SoA 3N device doubles.  Deterministic fixed-order reduction, stream-ordered. */
+int steps_force_residual(const double *pos, const double *acc, long long N, double B, double *out2,
+                         steps_stream_t stream);
+
 /* ---- housekeeping ------------------------------------------------------------------ */
 
 int steps_reserve(long long N);          /* allocate workspace for up to N particles now */

@@ -99,4 +99,40 @@ __global__ void timestep_stage2(const double* __restrict__ partial, int nblocks,
     }
 }
 
+// ---- net-force residual, the convergence monitor of glass generation (section 3.1) --------------
+// g_i = acc_i + B x_i;  out = {sum_i |g_i|^2, max_i |g_i|}.  Fixed assignment + fixed-order tree: deterministic.
+__global__ void __launch_bounds__(256) residual_stage1(const double* __restrict__ pos, const double* __restrict__ acc,
+                                                        long long N, double B, double* __restrict__ partial)
+{
+    double s = 0.0, mx = 0.0;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
+        const double gx = fma(B, pos[i], acc[i]), gy = fma(B, pos[N + i], acc[N + i]), gz = fma(B, pos[2 * N + i], acc[2 * N + i]);
+        const double g2 = fma(gz, gz, fma(gy, gy, gx * gx));
+        s += g2;
+        mx = fmax(mx, sqrt(g2));
+    }
+    __shared__ double sh[8][2];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        s += __shfl_down_sync(0xffffffffu, s, o);
+        mx = fmax(mx, __shfl_down_sync(0xffffffffu, mx, o));
+    }
+    if ((threadIdx.x & 31) == 0) { sh[threadIdx.x >> 5][0] = s; sh[threadIdx.x >> 5][1] = mx; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < 8; ++w) { s += sh[w][0]; mx = fmax(mx, sh[w][1]); }
+        partial[2 * blockIdx.x] = s; partial[2 * blockIdx.x + 1] = mx;
+    }
+}
+
+__global__ void residual_stage2(const double* __restrict__ partial, int nblocks, double* __restrict__ out2)
+{
+    if (threadIdx.x == 0) {
+        double s = 0.0, mx = 0.0;
+        for (int b = 0; b < nblocks; ++b) { s += partial[2 * b]; mx = fmax(mx, partial[2 * b + 1]); }
+        out2[0] = s; out2[1] = mx;
+    }
+}
+
 }  // namespace steps

@@ -306,6 +306,22 @@ int steps_timestep(const double* pos, const double* acc, const double* soft, lon
     return STEPS_OK;
 }
 
+int steps_force_residual(const double* pos, const double* acc, long long N, double B, double* out2, steps_stream_t stream)
+{
+    if (!pos || !acc || !out2 || N < 1) return STEPS_EINVAL;
+    int dev;
+    int rc = current_device(&dev);
+    if (rc != STEPS_OK) return rc;
+    rc = ensure_workspace(dev, 1);
+    if (rc != STEPS_OK) return rc;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    residual_stage1<<<MOM_BLOCKS, 256, 0, st>>>(pos, acc, N, B, g_ws[dev].mom_partial);
+    residual_stage2<<<1, 32, 0, st>>>(g_ws[dev].mom_partial, MOM_BLOCKS, out2);
+    g_launches += 2;
+    STEPS_CUDA(cudaGetLastError());
+    return STEPS_OK;
+}
+
 int steps_reserve(long long N)
 {
     if (N < 1) return STEPS_EINVAL;

@@ -24,3 +24,22 @@ def run_kdk(pos, vel, acc, mass, soft, a0: float, dts, cosmo: S.Cosmology, G: fl
             on_step(k, a)
     S.steps_kick_drift(pos, vel, acc, S.KdkCoeffs(alpha_c, beta_c, 1.0, 0.0, 0.0, B, int(mixed)))
     return a
+
+
+def run_adaptive(pos, vel, acc, mass, soft, a0: float, n_steps: int, cosmo: S.Cosmology, G: float, B: float,
+                 eps: float, dt_max: float, mixed: bool = False, on_step=None):
+    """n_steps KDK steps whose length is the global adaptive step of Eq. 12 (steps_timestep) evaluated on the forces
+    at the start of each step.  G < 0 is the reversed gravity of glass generation.  `acc` holds the
+    forces at the current positions on entry and on return.  Returns (final scale factor, list of step lengths).
+    One device->host read of the step length per step (the next step's coefficients need it)."""
+    import torch
+    dt_dev = torch.empty(1, dtype=torch.float64, device=pos.device)
+    a, dts = a0, []
+    for k in range(n_steps):
+        S.steps_timestep(pos, acc, soft, abs(G) / a ** 3, B, eps, dt_max, dt_dev)
+        dt = float(dt_dev.item())
+        a = run_kdk(pos, vel, acc, mass, soft, a, [dt], cosmo, G, B, mixed=mixed)
+        dts.append(dt)
+        if on_step is not None:
+            on_step(k, a)
+    return a, dts

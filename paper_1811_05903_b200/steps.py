@@ -16,7 +16,7 @@ OK, EINVAL, ECUDA, EUNSUPPORTED, ENOMEM = 0, -1, -2, -3, -4
 EXPORTS = [
     "steps_forces", "steps_forces_mixed", "steps_forces_range", "steps_forces_host", "steps_kick_drift",
     "steps_kdk_step", "steps_hubble", "steps_scale_factor_rk4", "steps_kdk_schedule", "steps_momentum",
-    "steps_timestep",
+    "steps_timestep", "steps_force_residual",
     "steps_reserve", "steps_shutdown", "steps_workspace_bytes", "steps_strerror", "steps_last_cuda_error",
     "steps_version", "steps_kernel_launch_count", "steps_set_option", "steps_last_force_kernel_ms",
     "steps_persistent_grid",
@@ -62,6 +62,7 @@ def lib() -> C.CDLL:
     L.steps_kdk_schedule.argtypes = [dbl, dbl, dbl, C.POINTER(Cosmology), C.POINTER(dbl)]
     L.steps_momentum.argtypes = [vp, vp, ll, vp, vp]
     L.steps_timestep.argtypes = [vp, vp, vp, ll, dbl, dbl, dbl, dbl, vp, vp]
+    L.steps_force_residual.argtypes = [vp, vp, ll, dbl, vp, vp]
     L.steps_reserve.argtypes = [ll]
     L.steps_shutdown.restype = None
     L.steps_workspace_bytes.argtypes = [ll]
@@ -173,6 +174,12 @@ def steps_timestep(pos, acc, soft, coef: float, B: float, eps: float, dt_max: fl
     n = soft.numel()
     _check(lib().steps_timestep(_dev(pos, 3 * n), _dev(acc, 3 * n), _dev(soft, n), n, coef, B, eps, dt_max,
                                 _dev(dt_out, 1), _stream(stream)))
+
+
+def steps_force_residual(pos, acc, B: float, out2, stream=None) -> None:
+    """Glass-generation monitor: out2 = [sum_i |acc_i + B x_i|^2, max_i |acc_i + B x_i|] (2-element device tensor)."""
+    n = pos.numel() // 3
+    _check(lib().steps_force_residual(_dev(pos, 3 * n), _dev(acc, 3 * n), n, B, _dev(out2, 2), _stream(stream)))
 
 
 def steps_reserve(n: int) -> None:

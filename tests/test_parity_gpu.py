@@ -286,6 +286,63 @@ def test_adaptive_kdk_run_follows_the_oracle(S, oracle):
     assert dx.max() < 1e-9
 
 
+# ---- glass generation (section 3.1): reversed gravity + net-force residual --------------------------------
+@pytest.mark.gpu
+@pytest.mark.parametrize("n", [1, 3, 257, 65536, 100003])
+def test_force_residual_matches_oracle(S, oracle, n):
+    import torch
+    rng = np.random.default_rng(3100 + n)
+    pos = rng.normal(size=(3, n)) * 5.0
+    acc = rng.normal(size=(3, n)) * 10.0 ** rng.uniform(-4, 1, n)
+    out = torch.empty(2, dtype=torch.float64, device="cuda")
+    for B in (0.0, 1.25e-4, 0.37):
+        S.steps_force_residual(dev(pos), dev(acc), B, out)
+        want = oracle.force_residual(pos, acc, B)
+        got = out.cpu().numpy()
+        assert got[0] == pytest.approx(want[0], rel=1e-13), (n, B)     # plain fp64 tree sum vs compensated sum
+        assert got[1] == pytest.approx(want[1], rel=4e-16), (n, B)
+
+
+@pytest.mark.gpu
+def test_glass_run_reversed_gravity_follows_the_oracle(S, oracle):
+    """40 adaptive KDK steps with REVERSED gravity (G = -1) in an EdS background on the compactified g0 set (random on
+    S^3, i.e. the starting point of glass making): the library follows the oracle step by step, and the net-force
+    residual -- the quantity glass generation minimises -- goes down."""
+    import torch
+    from paper_1811_05903_b200 import integrate
+    ps = synth.config(0, 2048)
+    B = 1.0 / ps.r_cut ** 3
+    eds = dict(H0=math.sqrt(2 * B), Omega_m=1.0, Omega_r=0.0, Omega_L=0.0, Omega_k=0.0)
+    G, eps, dt_max, a0, n_steps = -1.0, 0.025, 1e30, 0.05, 40
+    dpos, dvel, dm, dh = dev(ps.pos), dev(np.zeros_like(ps.pos)), dev(ps.mass), dev(ps.soft)
+    dacc = torch.empty_like(dpos)
+    S.steps_forces(dpos, dm, dh, dacc)
+    out = torch.empty(2, dtype=torch.float64, device="cuda")
+    S.steps_force_residual(dpos, dacc, B, out)
+    res0 = out.cpu().numpy().copy()
+    a_lib, dts = integrate.run_adaptive(dpos, dvel, dacc, dm, dh, a0, n_steps, S.Cosmology(**eds), G, B, eps, dt_max)
+    S.steps_force_residual(dpos, dacc, B, out)
+    res1 = out.cpu().numpy().copy()
+
+    pos, vel = ps.pos.copy(), np.zeros_like(ps.pos)
+    acc = oracle.forces(pos, ps.mass, ps.soft)
+    want0 = oracle.force_residual(pos, acc, B)
+    a = a0
+    for k in range(n_steps):
+        dt = oracle.timestep(pos, acc, ps.soft, 1.0 / a ** 3, B, eps, dt_max)
+        assert dts[k] == pytest.approx(dt, rel=1e-10), k
+        a = oracle.kdk_step(pos, vel, acc, ps.mass, ps.soft, a, dt, G, B, eds)
+    want1 = oracle.force_residual(pos, acc, B)
+    assert a_lib == pytest.approx(a, rel=1e-11)
+    assert res0[0] == pytest.approx(want0[0], rel=1e-12) and res1[0] == pytest.approx(want1[0], rel=1e-9)
+    s = (ps.mass * (4 * np.pi / 3) * ps.r_cut ** 3) ** (1 / 3)
+    dx = np.linalg.norm(dpos.cpu().numpy() - pos, axis=0) / s
+    print(f"glass run, {n_steps} steps: a {a0} -> {a:.4f}, residual sum |g|^2 {want0[0]:.4e} -> {want1[0]:.4e}, "
+          f"max |dx|/s library-vs-oracle {dx.max():.3e}")
+    assert dx.max() < 1e-9
+    assert res1[0] < res0[0]
+
+
 def test_config4_lockstep_200_steps_8192(S, oracle):
     """Config 4 at N = 8192, every one of the 200 comoving KDK steps (a: 1/51 -> 1): the library steps
     from the ORACLE's state (x_n, v_n, acc_n) and must land on the oracle's (x_{n+1}, v_{n+1},
