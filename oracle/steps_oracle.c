@@ -93,6 +93,38 @@ void oracle_forces(const double *pos, const double *mass, const double *soft, lo
     }
 }
 
+/* Quasi-periodic boundary conditions, Eq. 5 (L65-70): "only the leading term of the sum in Eq. 5 is kept
+ * for each pair of particles", i.e. of all images x - nL of the separation vector the one of smallest length, in a cubic
+ * box of side L.  Reading (#16): the leading term is taken component by component, n_c = round-half-even of
+ * (x_c / L) (nearbyint under the default rounding mode), so a component of exactly L/2 keeps its sign; otherwise as
+ * oracle_forces above (pair softening h_i + h_j, j = i skipped, r = 0 adds 0, G = 1, compensated sums). */
+void oracle_forces_quasi_periodic(const double *pos, const double *mass, const double *soft, long long N, double L,
+                                  double *acc)
+{
+    const double *x = pos, *y = pos + N, *z = pos + 2 * N;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (long long i = 0; i < N; ++i) {
+        double sx = 0, sy = 0, sz = 0, cx = 0, cy = 0, cz = 0;
+        for (long long j = 0; j < N; ++j) {
+            if (j == i) continue;
+            double dx = x[i] - x[j], dy = y[i] - y[j], dz = z[i] - z[j];          /* x_i - x_j */
+            dx -= L * nearbyint(dx / L);                                          /* leading image, Eq. 5 */
+            dy -= L * nearbyint(dy / L);
+            dz -= L * nearbyint(dz / L);
+            const double r = sqrt(dx * dx + dy * dy + dz * dz);
+            if (r == 0.0) continue;
+            const double h = soft[i] + soft[j];
+            const double f = -mass[j] * oracle_spline_F(r, h);
+            neumaier_add(&sx, &cx, f * (dx / r));
+            neumaier_add(&sy, &cy, f * (dy / r));
+            neumaier_add(&sz, &cz, f * (dz / r));
+        }
+        acc[i] = sx + cx;
+        acc[N + i] = sy + cy;
+        acc[2 * N + i] = sz + cz;
+    }
+}
+
 /* ------------------------------------------------------------------ background */
 
 typedef struct {

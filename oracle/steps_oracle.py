@@ -37,6 +37,8 @@ def lib():
         L.oracle_spline_F.argtypes = [C.c_double, C.c_double]
         L.oracle_forces.restype = None
         L.oracle_forces.argtypes = [dp, dp, dp, C.c_longlong, llp, C.c_longlong, dp, C.c_int]
+        L.oracle_forces_quasi_periodic.restype = None
+        L.oracle_forces_quasi_periodic.argtypes = [dp, dp, dp, C.c_longlong, C.c_double, dp]
         L.oracle_hubble.restype = C.c_double
         L.oracle_hubble.argtypes = [C.c_double, C.POINTER(Cosmo)]
         L.oracle_rk4_scale_factor.restype = C.c_double
@@ -86,6 +88,16 @@ def forces(pos, mass, soft, idx=None, reverse_j: bool = False) -> np.ndarray:
         lib().oracle_forces(_dp(pos), _dp(mass), _dp(soft), n,
                             idx.ctypes.data_as(C.POINTER(C.c_longlong)), idx.shape[0], _dp(acc),
                             int(reverse_j))
+    return acc
+
+
+def forces_quasi_periodic(pos, mass, soft, L: float) -> np.ndarray:
+    """Eq. 5 (L65-70) leading term only: nearest-image pair forces in a cubic box of side L; acc (3, N), G = 1."""
+    pos, mass, soft = _f64(pos), _f64(mass), _f64(soft)
+    n = mass.shape[0]
+    assert pos.shape == (3, n) and soft.shape == (n,)
+    acc = np.empty((3, n))
+    lib().oracle_forces_quasi_periodic(_dp(pos), _dp(mass), _dp(soft), n, float(L), _dp(acc))
     return acc
 
 

@@ -507,3 +507,56 @@ def test_force_residual_of_a_uniform_ball_is_small_and_reversed_gravity_lowers_i
         a = oracle.kdk_step(pos, vel, acc, mass, soft, a, dt, -1.0, B, cosmo)        # G = -1: reversed gravity
     r_end = oracle.force_residual(pos, acc, B)[0]
     assert r_end < 0.5 * r_start, (r_start, r_end)
+
+
+# ---- Eq. 5 (L65-70), quasi-periodic boundary: only the leading (nearest) image of each pair --------------------------
+def _box(rng, n, L):
+    pos = rng.uniform(0, L, size=(3, n))
+    mass = rng.uniform(0.5, 1.5, n) / n
+    soft = np.full(n, 0.02 * L)
+    return np.ascontiguousarray(pos), mass, soft
+
+
+def test_quasi_periodic_two_body_across_the_boundary(oracle):
+    """x_1 = 0.05 L, x_2 = 0.95 L: the leading image of the separation has length 0.1 L and points THROUGH the boundary,
+    so particle 1 is pulled towards -x with m_2 / (0.1 L)^2 (Eq. 4 third case), not towards +x with m_2 / (0.9 L)^2."""
+    L, m1, m2 = 2.0, 3.0, 5.0
+    pos = np.array([[0.05 * L, 0.95 * L], [0.3, 0.3], [0.7, 0.7]])
+    acc = oracle.forces_quasi_periodic(pos, np.array([m1, m2]), np.array([0.01, 0.01]), L)
+    assert acc[0, 0] == pytest.approx(-m2 / (0.1 * L) ** 2, rel=1e-13)
+    assert acc[0, 1] == pytest.approx(+m1 / (0.1 * L) ** 2, rel=1e-13)
+    assert np.all(acc[1:] == 0.0)
+
+
+def test_quasi_periodic_lattice_translation_newton3_and_open_limit(oracle):
+    rng = np.random.default_rng(55)
+    L = 1.7
+    # odd simple-cubic lattice (no separation component of exactly L/2): every particle sits at a centre of symmetry
+    g = (np.arange(5) + 0.5) * L / 5
+    lat = np.ascontiguousarray(np.array(np.meshgrid(g, g, g, indexing="ij")).reshape(3, -1))
+    acc = oracle.forces_quasi_periodic(lat, np.full(125, 1 / 125), np.full(125, 0.01), L)
+    assert np.abs(acc).max() < 1e-13 * (1 / 125) / (L / 5) ** 2 * 125
+    pos, mass, soft = _box(rng, 300, L)
+    ref = oracle.forces_quasi_periodic(pos, mass, soft, L)
+    # translation by any vector, positions wrapped back into the box: same forces (this is what the wrap is for)
+    shift = np.array([[0.61 * L], [-2.3 * L], [0.123]])
+    moved = np.ascontiguousarray(np.mod(pos + shift, L))
+    err = np.linalg.norm(oracle.forces_quasi_periodic(moved, mass, soft, L) - ref, axis=0) / np.linalg.norm(ref, axis=0)
+    assert err.max() < 1e-11
+    # Newton's third law survives the wrap (the leading image of x_i - x_j is minus that of x_j - x_i)
+    assert np.linalg.norm((mass * ref).sum(axis=1)) < 1e-14 * np.sum(mass * np.linalg.norm(ref, axis=0))
+    # all particles within a region smaller than L/2: no wrap is active, result = the open-boundary oracle
+    small = np.ascontiguousarray(0.3 * L + pos * 0.45)
+    assert np.array_equal(oracle.forces_quasi_periodic(small, mass, soft, L), oracle.forces(small, mass, soft))
+    # brute force with numpy longdouble on a few particles
+    p8, m8, h8 = pos[:, :8].astype(np.longdouble), mass[:8], soft[:8]
+    want = np.zeros((3, 8), dtype=np.longdouble)
+    for i in range(8):
+        for j in range(8):
+            if i != j:
+                d = p8[:, j] - p8[:, i]
+                d = d - L * np.rint(d / L)
+                r = np.sqrt(np.sum(d * d))
+                want[:, i] += m8[j] * oracle.spline_F(float(r), h8[i] + h8[j]) * d / r
+    got = oracle.forces_quasi_periodic(np.ascontiguousarray(pos[:, :8]), m8, h8, L)
+    assert np.abs(got - want.astype(np.float64)).max() < 1e-13 * np.abs(got).max()
