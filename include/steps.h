@@ -136,6 +136,16 @@ int steps_kdk_schedule(double a_n, double dt, double G, const steps_cosmology *c
 int steps_momentum(const double *vec, const double *mass, long long N, double *out4,
                    steps_stream_t stream);
 
+/* Quasi-periodic boundary conditions, Eq. 5 (L65-70, first part): "only the leading
+ * term of the sum in Eq. 5 is kept for each pair of particles" -- every separation x_j - x_i is replaced by its image of
+ * smallest length in a cubic box of side L (component-wise d - L rint(d / L), ties to even), otherwise exactly
+ * steps_forces / steps_forces_mixed (mixed != 0): same layout, same pair law with pair softening soft_i + soft_j, G = 1,
+ * acc overwritten.  Positions need not lie inside [0, L).  First version: every tile pair goes through the per-pair
+ * softening test (no far/near split in a periodic box) in the persistent stream-K driver.  The full Ewald image
+ * sum of Eq. 5 (|x - nL| < 2.6 L) is not built.  STEPS_EINVAL additionally for L <= 0. */
+int steps_forces_quasi_periodic(const double *pos, const double *mass, const double *soft, long long N,
+                                double L, double *acc, int mixed, steps_stream_t stream);
+
 /* Adaptive global time step, Eq. 12 (L113-116):
  *     dt = min[ dt_max, min_i sqrt(2 eta_i eps / |A_i|) ],  eta_i = 2.8 soft[i]  (L116, literal),
  * A_i = coef (acc_i + B pos_i) = the acceleration the kick applies, without the drag (coef = G a^-3, reading #6/#11);

@@ -96,11 +96,14 @@ constexpr int persistent_smem_bytes()
 
 // ---- persistent stream-K driver ------------------------------------------------------------------
 // partials: [nb + gridDim.x slots][Path::NOUT][IB] doubles; CTA p's record for i-block b is slot b + p.
-template <typename Path, int STAGES>
+// PERIODIC (quasi-periodic boundary, Eq. 5): every tile goes through the near body
+// with leading-image separations in a cubic box of side box_L -- the radial far/near classification of the compactified
+// sets does not apply in a periodic box.
+template <typename Path, int STAGES, bool PERIODIC = false>
 __global__ void __launch_bounds__(CTA_THREADS, 1)
 forces_persistent_kernel(const double* __restrict__ pos, const double* __restrict__ soft, long long N,
                          const typename Path::Tile* __restrict__ tiles, int nt, long long i_begin, long long i_end,
-                         int nb, double* __restrict__ partials, int zero)
+                         int nb, double* __restrict__ partials, int zero, double box_L, double box_invL)
 {
     using Tile = typename Path::Tile;
     constexpr int STRIDE = stage_stride((int)sizeof(Tile));
@@ -155,6 +158,9 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
             const int s = it % STAGES;
             mbar_wait(&full_bar[s], (it / STAGES) & 1);
             const Tile& T = *reinterpret_cast<const Tile*>(smem_raw + s * STRIDE);
+            if constexpr (PERIODIC) {
+                Path::template near_box<true>(T, S, acc, box_L, box_invL);
+            } else {
 #ifdef STEPS_DIAG_ALLFAR                                   // timing diagnostic only (wrong forces): no near body
             Path::far(T, S, F, zero);
             if (++pending >= Path::FAR_TILES_PER_FLUSH) { Path::far_flush(F, acc); pending = 0; }
@@ -168,6 +174,7 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
                 Path::near(T, S, acc);
             }
 #endif
+            }
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty_bar[s]);
         }

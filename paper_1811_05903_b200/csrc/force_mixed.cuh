@@ -147,8 +147,22 @@ STEPS_UNROLL(STEPS_FAR_UNROLL)
         return s_newton;
     }
 
-    static __device__ __forceinline__ void near(const Tile& T, const IState& S, double* acc)
+    // Leading periodic image of a packed pair of separation components (Eq. 5): d - L rint(d/L) with the
+    // round-to-nearest-even shift trick in fp32 (valid for |d/L| < 2^22), 3 packed instructions.
+    static __device__ __forceinline__ u64 wrap2(u64 d, u64 negL, u64 invL)
     {
+        const u64 SHIFT = pack2(12582912.0f, 12582912.0f), NSHIFT = pack2(-12582912.0f, -12582912.0f);   // 1.5 * 2^23
+        const u64 n = add2(fma2(d, invL, SHIFT), NSHIFT);
+        return fma2(negL, n, d);
+    }
+
+    static __device__ __forceinline__ void near(const Tile& T, const IState& S, double* acc) { near_box<false>(T, S, acc, 0.0, 0.0); }
+
+    // PERIODIC: every separation is replaced by its leading image in a cubic box of side L (row 8(f)-3).
+    template <bool PERIODIC>
+    static __device__ __forceinline__ void near_box(const Tile& T, const IState& S, double* acc, double Ld, double invLd)
+    {
+        const u64 negL = pack2(-(float)Ld, -(float)Ld), invL = pack2((float)invLd, (float)invLd);
         u64 xi[R_I], yi[R_I], zi[R_I], hi[R_I], ax[R_I], ay[R_I], az[R_I];
 #pragma unroll
         for (int k = 0; k < R_I; ++k) {
@@ -163,7 +177,8 @@ STEPS_UNROLL(STEPS_FAR_UNROLL)
             const u64 hj = *reinterpret_cast<const u64*>(&T.h[j]);
 #pragma unroll
             for (int k = 0; k < R_I; ++k) {
-                const u64 dx = sub2(xj, xi[k]), dy = sub2(yj, yi[k]), dz = sub2(zj, zi[k]);
+                u64 dx = sub2(xj, xi[k]), dy = sub2(yj, yi[k]), dz = sub2(zj, zi[k]);
+                if (PERIODIC) { dx = wrap2(dx, negL, invL); dy = wrap2(dy, negL, invL); dz = wrap2(dz, negL, invL); }
                 const u64 r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
                 const u64 hs = add2(hj, hi[k]);
                 const u64 hs2 = mul2(hs, hs);

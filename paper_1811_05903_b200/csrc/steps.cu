@@ -37,6 +37,7 @@ struct Workspace {
     long long cap_particles = 0;
     int num_sms = 0;
     int grid_mixed = 0, grid_fp64 = 0;   // persistent grids: SMs x resident CTAs
+    int grid_mixed_periodic = 0, grid_fp64_periodic = 0;
     double* mom_partial = nullptr;  // MOM_BLOCKS * 4
     // staging buffers of steps_forces_host
     double* h_pos = nullptr; double* h_mass = nullptr; double* h_soft = nullptr; double* h_acc = nullptr;
@@ -133,7 +134,7 @@ int launch_forces(const double* pos, const double* mass, const double* soft, lon
             if (!w.ev0) { STEPS_CUDA(cudaEventCreate(&w.ev0)); STEPS_CUDA(cudaEventCreate(&w.ev1)); }
             STEPS_CUDA(cudaEventRecord(w.ev0, st));
         }
-        kern<<<P, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, i_begin, i_end, nb, w.partials, 0);
+        kern<<<P, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, i_begin, i_end, nb, w.partials, 0, 0.0, 0.0);
         if (prof) { STEPS_CUDA(cudaEventRecord(w.ev1, st)); w.ev_valid = true; }
         forces_reduce_kernel<Path::NOUT><<<(int)((cnt + 255) / 256), 256, 0, st>>>(w.partials, nt, nb, P, cnt, acc_out);
         g_launches += 2;
@@ -160,9 +161,53 @@ int forces_impl(const double* pos, const double* mass, const double* soft, long 
                  : launch_forces<Fp64Path>(pos, mass, soft, N, i_begin, i_end, acc_out, st, w, w.grid_fp64);
 }
 
+template <typename Path>
+int launch_forces_periodic(const double* pos, const double* mass, const double* soft, long long N, double L, double* acc_out,
+                           cudaStream_t st, Workspace& w, int& grid_cache)
+{
+    using Tile = typename Path::Tile;
+    const int nt = (int)ntiles_of(N);
+    Tile* tiles = reinterpret_cast<Tile*>(w.tiles);
+    prep_tiles<Tile><<<nt, TJ, 0, st>>>(pos, mass, soft, N, tiles);
+    const int nb = (int)nblocks_of(N);
+    constexpr int smem = persistent_smem_bytes<Path, STAGES>();
+    auto kern = forces_persistent_kernel<Path, STAGES, true>;
+    if (grid_cache == 0) {
+        STEPS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        int per_sm = 0;
+        STEPS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, CTA_THREADS, smem));
+        if (per_sm < 1) return STEPS_EUNSUPPORTED;
+        const int g = w.num_sms * per_sm;
+        grid_cache = g > MAX_GRID ? MAX_GRID : g;
+    }
+    const int P = grid_cache;
+    kern<<<P, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, 0, N, nb, w.partials, 0, L, 1.0 / L);
+    forces_reduce_kernel<Path::NOUT><<<(int)((N + 255) / 256), 256, 0, st>>>(w.partials, nt, nb, P, N, acc_out);
+    g_launches += 3;
+    STEPS_CUDA(cudaGetLastError());
+    return STEPS_OK;
+}
+
 }  // namespace
 
 extern "C" {
+
+int steps_forces_quasi_periodic(const double* pos, const double* mass, const double* soft, long long N, double L,
+                                double* acc, int mixed, steps_stream_t stream)
+{
+    if (!pos || !mass || !soft || !acc || N < 1 || !(L > 0.0)) return STEPS_EINVAL;
+    if (N > (1ll << 31) - TJ) return STEPS_EINVAL;
+    if (misaligned(pos) || misaligned(mass) || misaligned(soft) || misaligned(acc)) return STEPS_EINVAL;
+    int dev;
+    int rc = current_device(&dev);
+    if (rc != STEPS_OK) return rc;
+    rc = ensure_workspace(dev, N);
+    if (rc != STEPS_OK) return rc;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    Workspace& w = g_ws[dev];
+    return mixed ? launch_forces_periodic<MixedPath>(pos, mass, soft, N, L, acc, st, w, w.grid_mixed_periodic)
+                 : launch_forces_periodic<Fp64Path>(pos, mass, soft, N, L, acc, st, w, w.grid_fp64_periodic);
+}
 
 int steps_forces(const double* pos, const double* mass, const double* soft, long long N, double* acc,
                  steps_stream_t stream)

@@ -16,7 +16,7 @@ OK, EINVAL, ECUDA, EUNSUPPORTED, ENOMEM = 0, -1, -2, -3, -4
 EXPORTS = [
     "steps_forces", "steps_forces_mixed", "steps_forces_range", "steps_forces_host", "steps_kick_drift",
     "steps_kdk_step", "steps_hubble", "steps_scale_factor_rk4", "steps_kdk_schedule", "steps_momentum",
-    "steps_timestep", "steps_force_residual",
+    "steps_timestep", "steps_force_residual", "steps_forces_quasi_periodic",
     "steps_reserve", "steps_shutdown", "steps_workspace_bytes", "steps_strerror", "steps_last_cuda_error",
     "steps_version", "steps_kernel_launch_count", "steps_set_option", "steps_last_force_kernel_ms",
     "steps_persistent_grid",
@@ -61,6 +61,7 @@ def lib() -> C.CDLL:
     L.steps_scale_factor_rk4.restype = dbl
     L.steps_kdk_schedule.argtypes = [dbl, dbl, dbl, C.POINTER(Cosmology), C.POINTER(dbl)]
     L.steps_momentum.argtypes = [vp, vp, ll, vp, vp]
+    L.steps_forces_quasi_periodic.argtypes = [vp, vp, vp, ll, dbl, vp, i32, vp]
     L.steps_timestep.argtypes = [vp, vp, vp, ll, dbl, dbl, dbl, dbl, vp, vp]
     L.steps_force_residual.argtypes = [vp, vp, ll, dbl, vp, vp]
     L.steps_reserve.argtypes = [ll]
@@ -167,6 +168,13 @@ def steps_kdk_schedule(a_n: float, dt: float, G: float, cosmo: Cosmology) -> dic
 def steps_momentum(vec, mass, out4, stream=None) -> None:
     n = mass.numel()
     _check(lib().steps_momentum(_dev(vec, 3 * n), _dev(mass, n), n, _dev(out4, 4), _stream(stream)))
+
+
+def steps_forces_quasi_periodic(pos, mass, soft, L: float, acc, mixed: bool = False, stream=None) -> None:
+    """Eq. 5 leading term (nearest image in a cubic box of side L); otherwise as steps_forces / steps_forces_mixed."""
+    n = mass.numel()
+    _check(lib().steps_forces_quasi_periodic(_dev(pos, 3 * n), _dev(mass, n), _dev(soft, n), n, float(L), _dev(acc, 3 * n),
+                                             int(mixed), _stream(stream)))
 
 
 def steps_timestep(pos, acc, soft, coef: float, B: float, eps: float, dt_max: float, dt_out, stream=None) -> None:
