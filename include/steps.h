@@ -155,6 +155,21 @@ int steps_forces_quasi_periodic(const double *pos, const double *mass, const dou
 int steps_timestep(const double *pos, const double *acc, const double *soft, long long N, double coef,
                    double B, double eps, double dt_max, double *dt_out, steps_stream_t stream);
 
+/* Device-resident adaptive stepping (second half): one KDK step whose length is Eq. 12 and whose
+ * coefficients (Eq. 1 / RK4 of L127 / readings #8-#9, the arithmetic of steps_kdk_schedule) are computed ON THE DEVICE,
+ * so that a run needs no host round trip between steps and a sequence of these calls can be captured in a CUDA graph.
+ * state5 (device, 5 doubles) = {a, dt of the last step, alpha_close, beta_close, steps taken}; initialise it to
+ * {a_0, 0, 1, 0, 0}.  Per call: dt = Eq. 12 from (pos, acc, soft) with coef = |G| a^-3; closing kick of the previous
+ * step + opening kick + drift; force evaluation at the new positions into acc; state advanced to a_{n+1}.  acc must hold
+ * the forces at the current positions on entry (steps_forces before the first call).  steps_kick_close_adaptive applies
+ * the pending closing half kick (end of a run, or before velocities are read) and resets it to the identity.
+ * G < 0 = reversed gravity (glass generation).  cosmo is read on the host at call time. */
+int steps_kdk_step_adaptive(double *pos, double *vel, double *acc, const double *mass, const double *soft,
+                            long long N, double *state5, const steps_cosmology *cosmo, double G, double B,
+                            double eps, double dt_max, int mixed, steps_stream_t stream);
+int steps_kick_close_adaptive(double *pos, double *vel, const double *acc, long long N, double *state5,
+                              double B, steps_stream_t stream);
+
 /* Glass generation (section 3.1).  Reversed gravity needs no call of its
  * own: it is G < 0 in steps_kdk_schedule (both the pair sum and the background term change sign, the uniform sphere
  * stays static).  This is its convergence monitor, the net force per particle g_i = acc_i + B pos_i:

@@ -135,4 +135,105 @@ __global__ void residual_stage2(const double* __restrict__ partial, int nblocks,
     }
 }
 
+// ---- device-resident adaptive stepping (second half): no host round trip between steps -----------
+// Run state in device memory: {a, dt, alpha_close, beta_close, steps taken}.
+struct RunState {
+    double a, dt, alpha_close, beta_close, steps;
+};
+struct CosmoScalars {
+    double H0, Om, Or, OL, Ok;
+};
+__device__ __forceinline__ double hubble_dev(double a, const CosmoScalars& c)          // PAPER.md Eq. 1 (L37)
+{
+    return c.H0 * sqrt(c.Om / (a * a * a) + c.Or / (a * a * a * a) + c.OL + c.Ok / (a * a));
+}
+
+// Eq. 12 with coef = |G| a^-3 taken from the run state (stage 1 of the two-stage exact minimum).
+__global__ void __launch_bounds__(256) timestep_state_stage1(const double* __restrict__ pos, const double* __restrict__ acc,
+                                                              const double* __restrict__ soft, long long N,
+                                                              const RunState* __restrict__ st, double absG, double B,
+                                                              double eps, double dt_max, double* __restrict__ partial)
+{
+    const double a = st->a;
+    const double coef = absG / (a * a * a);
+    double dt = dt_max;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
+        const double Ax = coef * (acc[i] + B * pos[i]);
+        const double Ay = coef * (acc[N + i] + B * pos[N + i]);
+        const double Az = coef * (acc[2 * N + i] + B * pos[2 * N + i]);
+        const double A = sqrt(Ax * Ax + Ay * Ay + Az * Az);
+        if (A > 0.0) dt = fmin(dt, sqrt(2.0 * (2.8 * soft[i]) * eps / A));
+    }
+    __shared__ double sh[8];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) dt = fmin(dt, __shfl_down_sync(0xffffffffu, dt, o));
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = dt;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < 8; ++w) dt = fmin(dt, sh[w]);
+        partial[blockIdx.x] = dt;
+    }
+}
+
+// Stage 2 + the step's coefficients (the arithmetic of steps_kdk_schedule, on the device): writes the six kick/drift
+// scalars of THIS step to coef6 = {alpha_close(prev), beta_close(prev), alpha_open, beta_open, gamma, B} and advances
+// the state to a_{n+1} with the new closing coefficients.
+__global__ void step_coefficients_kernel(const double* __restrict__ partial, int nblocks, RunState* __restrict__ st,
+                                         CosmoScalars c, double G, double B, double* __restrict__ coef6)
+{
+    if (threadIdx.x != 0) return;
+    double dt = partial[0];
+    for (int b = 1; b < nblocks; ++b) dt = fmin(dt, partial[b]);
+    const double a_n = st->a;
+    const bool is_static = (c.H0 == 0.0);
+    const double H_n = is_static ? 0.0 : hubble_dev(a_n, c);
+    double a_1 = a_n;
+    if (!is_static) {                                                   // classical RK4 on da/dt = a H(a) (L127)
+        const double k1 = a_n * hubble_dev(a_n, c);
+        const double s2 = a_n + 0.5 * dt * k1, k2 = s2 * hubble_dev(s2, c);
+        const double s3 = a_n + 0.5 * dt * k2, k3 = s3 * hubble_dev(s3, c);
+        const double s4 = a_n + dt * k3, k4 = s4 * hubble_dev(s4, c);
+        a_1 = a_n + dt / 6.0 * (k1 + 2.0 * (k2 + k3) + k4);
+    }
+    const double H_1 = is_static ? 0.0 : hubble_dev(a_1, c);
+    coef6[0] = st->alpha_close; coef6[1] = st->beta_close;
+    coef6[2] = 1.0 - H_n * dt;
+    coef6[3] = 0.5 * dt * G / (a_n * a_n * a_n);
+    coef6[4] = dt;
+    coef6[5] = B;
+    const double ac = 1.0 / (1.0 + H_1 * dt);
+    st->alpha_close = ac;
+    st->beta_close = 0.5 * dt * G / (a_1 * a_1 * a_1) * ac;
+    st->a = a_1;
+    st->dt = dt;
+    st->steps += 1.0;
+}
+
+// The final closing half kick of a run: coefficients from the state, which is reset to the identity.
+__global__ void close_coefficients_kernel(RunState* __restrict__ st, double B, double* __restrict__ coef6)
+{
+    if (threadIdx.x != 0) return;
+    coef6[0] = st->alpha_close; coef6[1] = st->beta_close; coef6[2] = 1.0; coef6[3] = 0.0; coef6[4] = 0.0; coef6[5] = B;
+    st->alpha_close = 1.0; st->beta_close = 0.0;
+}
+
+// kick_drift_kernel with its six scalars read from device memory.
+__global__ void __launch_bounds__(256) kick_drift_dev_kernel(double* __restrict__ pos, double* __restrict__ vel,
+                                                             const double* __restrict__ acc, long long M,
+                                                             const double* __restrict__ coef6)
+{
+    const double ac = coef6[0], bc = coef6[1], ao = coef6[2], bo = coef6[3], gamma = coef6[4], B = coef6[5];
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < M; k += stride) {
+        const double x = pos[k];
+        const double g = fma(B, x, acc[k]);
+        double v = vel[k];
+        v = fma(bc, g, ac * v);
+        v = fma(bo, g, ao * v);
+        vel[k] = v;
+        pos[k] = fma(gamma, v, x);
+    }
+}
+
 }  // namespace steps

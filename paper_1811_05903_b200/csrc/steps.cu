@@ -288,6 +288,55 @@ int steps_kdk_step(double* pos, double* vel, double* acc, const double* mass, co
     return forces_impl(pos, mass, soft, N, 0, N, acc, c->mixed, stream);
 }
 
+int steps_kdk_step_adaptive(double* pos, double* vel, double* acc, const double* mass, const double* soft, long long N,
+                            double* state5, const steps_cosmology* c, double G, double B, double eps, double dt_max,
+                            int mixed, steps_stream_t stream)
+{
+    if (!pos || !vel || !acc || !mass || !soft || !state5 || !c || N < 1) return STEPS_EINVAL;
+    if (!(eps > 0.0) || !(dt_max > 0.0)) return STEPS_EINVAL;
+    if (misaligned(pos) || misaligned(vel) || misaligned(acc)) return STEPS_EINVAL;
+    int dev;
+    int rc = current_device(&dev);
+    if (rc != STEPS_OK) return rc;
+    rc = ensure_workspace(dev, N);
+    if (rc != STEPS_OK) return rc;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    double* partial = g_ws[dev].mom_partial;
+    double* coef6 = partial + 2 * MOM_BLOCKS;
+    RunState* rs = reinterpret_cast<RunState*>(state5);
+    const CosmoScalars cs{c->H0, c->Omega_m, c->Omega_r, c->Omega_L, c->Omega_k};
+    timestep_state_stage1<<<MOM_BLOCKS, 256, 0, st>>>(pos, acc, soft, N, rs, std::fabs(G), B, eps, dt_max, partial);
+    step_coefficients_kernel<<<1, 32, 0, st>>>(partial, MOM_BLOCKS, rs, cs, G, B, coef6);
+    const long long M = 3 * N;
+    long long blocks = (M + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    kick_drift_dev_kernel<<<(int)blocks, 256, 0, st>>>(pos, vel, acc, M, coef6);
+    g_launches += 3;
+    STEPS_CUDA(cudaGetLastError());
+    return forces_impl(pos, mass, soft, N, 0, N, acc, mixed, stream);
+}
+
+int steps_kick_close_adaptive(double* pos, double* vel, const double* acc, long long N, double* state5, double B,
+                              steps_stream_t stream)
+{
+    if (!pos || !vel || !acc || !state5 || N < 1) return STEPS_EINVAL;
+    int dev;
+    int rc = current_device(&dev);
+    if (rc != STEPS_OK) return rc;
+    rc = ensure_workspace(dev, 1);
+    if (rc != STEPS_OK) return rc;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    double* coef6 = g_ws[dev].mom_partial + 2 * MOM_BLOCKS;
+    close_coefficients_kernel<<<1, 32, 0, st>>>(reinterpret_cast<RunState*>(state5), B, coef6);
+    const long long M = 3 * N;
+    long long blocks = (M + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    kick_drift_dev_kernel<<<(int)blocks, 256, 0, st>>>(pos, vel, acc, M, coef6);
+    g_launches += 2;
+    STEPS_CUDA(cudaGetLastError());
+    return STEPS_OK;
+}
+
 double steps_hubble(double a, const steps_cosmology* c)
 {
     return c->H0 * std::sqrt(c->Omega_m / (a * a * a) + c->Omega_r / (a * a * a * a) + c->Omega_L +

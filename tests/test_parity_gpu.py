@@ -417,6 +417,88 @@ def test_quasi_periodic_translation_invariance_and_unwrapped_positions_on_device
     assert float(p.norm()) < 1e-13 * float((torch.from_numpy(mass).cuda() * a0.norm(dim=0)).sum())
 
 
+# ---- device-resident adaptive stepping (8(f)-1, second half) ---------------------------------------------------------
+def _oracle_adaptive(oracle, ps, vel0, cosmo, G, B, eps, dt_max, a0, n_steps):
+    pos, vel = ps.pos.copy(), vel0.copy()
+    acc = oracle.forces(pos, ps.mass, ps.soft)
+    a, dts = a0, []
+    for _ in range(n_steps):
+        dt = oracle.timestep(pos, acc, ps.soft, abs(G) / a ** 3, B, eps, dt_max)
+        a = oracle.kdk_step(pos, vel, acc, ps.mass, ps.soft, a, dt, G, B, cosmo)
+        dts.append(dt)
+    return pos, vel, a, dts
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("mode", ["lcdm", "glass"])
+def test_device_resident_adaptive_run_matches_oracle(S, oracle, mode):
+    """steps_kdk_step_adaptive computes the step length (Eq. 12), a(t) (RK4) and the kick/drift coefficients on the
+    device; 20 steps without any host round trip must land where the oracle's host-driven loop lands."""
+    import torch
+    n_steps, eps, dt_max = 20, 0.025, 0.5
+    if mode == "lcdm":
+        ps = _config4(oracle, 2048); vel0 = ps.vel; cosmo = LCDM; G = 1.0; a0 = 1 / 51
+    else:
+        ps = synth.config(0, 2048); vel0 = np.zeros_like(ps.pos); G = -1.0; a0 = 0.05
+        cosmo = dict(H0=math.sqrt(2.0 / ps.r_cut ** 3), Omega_m=1.0, Omega_r=0.0, Omega_L=0.0, Omega_k=0.0)
+    B = 1.0 / ps.r_cut ** 3
+    dpos, dvel, dm, dh = dev(ps.pos), dev(vel0), dev(ps.mass), dev(ps.soft)
+    dacc = torch.empty_like(dpos)
+    S.steps_forces(dpos, dm, dh, dacc)
+    state = torch.tensor([a0, 0.0, 1.0, 0.0, 0.0], dtype=torch.float64, device="cuda")
+    c = S.Cosmology(**cosmo)
+    for _ in range(n_steps):
+        S.steps_kdk_step_adaptive(dpos, dvel, dacc, dm, dh, state, c, G, B, eps, dt_max)
+    S.steps_kick_close_adaptive(dpos, dvel, dacc, state, B)
+    st = state.cpu().numpy()
+    pos, vel, a, dts = _oracle_adaptive(oracle, ps, vel0, cosmo, G, B, eps, dt_max, a0, n_steps)
+    assert st[4] == n_steps and st[2] == 1.0 and st[3] == 0.0
+    assert st[0] == pytest.approx(a, rel=1e-11) and st[1] == pytest.approx(dts[-1], rel=1e-9)
+    s = (ps.mass * (4 * np.pi / 3) * ps.r_cut ** 3) ** (1 / 3)
+    dx = np.linalg.norm(dpos.cpu().numpy() - pos, axis=0) / s
+    dv = np.linalg.norm(dvel.cpu().numpy() - vel, axis=0) / np.maximum(np.linalg.norm(vel, axis=0), 1e-300)
+    print(f"device-resident adaptive run [{mode}]: a = {a:.6f}, max |dx|/s {dx.max():.3e}, max |dv|/|v| {dv.max():.3e}")
+    assert dx.max() < 1e-9 and dv.max() < 1e-8
+
+
+@pytest.mark.gpu
+def test_device_resident_steps_replay_from_a_cuda_graph(S, oracle):
+    """Five adaptive steps captured ONCE in a CUDA graph and replayed four times give bit for bit the state of twenty
+    eager calls: the whole step (time-step criterion, coefficients, kick/drift, tile prep, forces, reduce) is
+    stream-ordered device work with no host dependence."""
+    import torch
+    ps = _config4(oracle, 4096)
+    B, G, eps, dt_max, a0 = 1.0 / ps.r_cut ** 3, 1.0, 0.025, 0.5, 1 / 51
+    c = S.Cosmology(**LCDM)
+    dm, dh = dev(ps.mass), dev(ps.soft)
+
+    def fresh():
+        dpos, dvel = dev(ps.pos), dev(ps.vel)
+        dacc = torch.empty_like(dpos)
+        S.steps_forces(dpos, dm, dh, dacc)
+        return dpos, dvel, dacc, torch.tensor([a0, 0.0, 1.0, 0.0, 0.0], dtype=torch.float64, device="cuda")
+
+    pos_e, vel_e, acc_e, st_e = fresh()
+    for _ in range(20):
+        S.steps_kdk_step_adaptive(pos_e, vel_e, acc_e, dm, dh, st_e, c, G, B, eps, dt_max)
+    torch.cuda.synchronize()
+
+    pos_g, vel_g, acc_g, st_g = fresh()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(g, stream=side):
+            for _ in range(5):
+                S.steps_kdk_step_adaptive(pos_g, vel_g, acc_g, dm, dh, st_g, c, G, B, eps, dt_max)
+    torch.cuda.current_stream().wait_stream(side)
+    for _ in range(4):
+        g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(st_g, st_e) and st_g[4].item() == 20.0
+    assert torch.equal(pos_g, pos_e) and torch.equal(vel_g, vel_e) and torch.equal(acc_g, acc_e)
+
+
 def test_config4_lockstep_200_steps_8192(S, oracle):
     """Config 4 at N = 8192, every one of the 200 comoving KDK steps (a: 1/51 -> 1): the library steps
     from the ORACLE's state (x_n, v_n, acc_n) and must land on the oracle's (x_{n+1}, v_{n+1},
