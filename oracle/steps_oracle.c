@@ -125,6 +125,43 @@ void oracle_forces_quasi_periodic(const double *pos, const double *mass, const d
     }
 }
 
+/* Periodic boundary conditions, Eq. 5 (L65-70) with the paper's cut: F(x, h) = sum over integer triplets n of
+ * -G calF(|x - nL|, h) (x - nL)/|x - nL|, "the only valid triplets are where |x - nL| < 2.6 L is fulfilled".
+ * Reading (#17): x is the separation x_i - x_j as it is (no prior wrapping: the set {x - nL} is the same for
+ * every representative of x modulo L, so the sum does not depend on it); the triplets are searched in |n_c| <= 4 around
+ * the nearest image, which contains every n with |x - nL| < 2.6 L; strict inequality as printed; the pair law with pair
+ * softening h_i + h_j is applied to every image.  Plain loops, compensated sums. */
+void oracle_forces_periodic_images(const double *pos, const double *mass, const double *soft, long long N, double L,
+                                   double *acc)
+{
+    const double *x = pos, *y = pos + N, *z = pos + 2 * N;
+    const double cut = 2.6 * L;
+#pragma omp parallel for schedule(dynamic, 4)
+    for (long long i = 0; i < N; ++i) {
+        double sx = 0, sy = 0, sz = 0, cx = 0, cy = 0, cz = 0;
+        for (long long j = 0; j < N; ++j) {
+            if (j == i) continue;
+            const double h = soft[i] + soft[j];
+            const double bx = x[i] - x[j], by = y[i] - y[j], bz = z[i] - z[j];
+            const double ox = nearbyint(bx / L), oy = nearbyint(by / L), oz = nearbyint(bz / L);
+            for (int n1 = -4; n1 <= 4; ++n1)
+                for (int n2 = -4; n2 <= 4; ++n2)
+                    for (int n3 = -4; n3 <= 4; ++n3) {
+                        const double dx = bx - (ox + n1) * L, dy = by - (oy + n2) * L, dz = bz - (oz + n3) * L;
+                        const double r = sqrt(dx * dx + dy * dy + dz * dz);
+                        if (!(r < cut) || r == 0.0) continue;
+                        const double f = -mass[j] * oracle_spline_F(r, h);
+                        neumaier_add(&sx, &cx, f * (dx / r));
+                        neumaier_add(&sy, &cy, f * (dy / r));
+                        neumaier_add(&sz, &cz, f * (dz / r));
+                    }
+        }
+        acc[i] = sx + cx;
+        acc[N + i] = sy + cy;
+        acc[2 * N + i] = sz + cz;
+    }
+}
+
 /* ------------------------------------------------------------------ background */
 
 typedef struct {

@@ -39,6 +39,8 @@ def lib():
         L.oracle_forces.argtypes = [dp, dp, dp, C.c_longlong, llp, C.c_longlong, dp, C.c_int]
         L.oracle_forces_quasi_periodic.restype = None
         L.oracle_forces_quasi_periodic.argtypes = [dp, dp, dp, C.c_longlong, C.c_double, dp]
+        L.oracle_forces_periodic_images.restype = None
+        L.oracle_forces_periodic_images.argtypes = [dp, dp, dp, C.c_longlong, C.c_double, dp]
         L.oracle_hubble.restype = C.c_double
         L.oracle_hubble.argtypes = [C.c_double, C.POINTER(Cosmo)]
         L.oracle_rk4_scale_factor.restype = C.c_double
@@ -98,6 +100,16 @@ def forces_quasi_periodic(pos, mass, soft, L: float) -> np.ndarray:
     assert pos.shape == (3, n) and soft.shape == (n,)
     acc = np.empty((3, n))
     lib().oracle_forces_quasi_periodic(_dp(pos), _dp(mass), _dp(soft), n, float(L), _dp(acc))
+    return acc
+
+
+def forces_periodic_images(pos, mass, soft, L: float) -> np.ndarray:
+    """Eq. 5 (L65-70) with the paper's cut |x - nL| < 2.6 L over the periodic images; acc (3, N), G = 1."""
+    pos, mass, soft = _f64(pos), _f64(mass), _f64(soft)
+    n = mass.shape[0]
+    assert pos.shape == (3, n) and soft.shape == (n,)
+    acc = np.empty((3, n))
+    lib().oracle_forces_periodic_images(_dp(pos), _dp(mass), _dp(soft), n, float(L), _dp(acc))
     return acc
 
 

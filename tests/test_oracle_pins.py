@@ -560,3 +560,42 @@ def test_quasi_periodic_lattice_translation_newton3_and_open_limit(oracle):
                 want[:, i] += m8[j] * oracle.spline_F(float(r), h8[i] + h8[j]) * d / r
     got = oracle.forces_quasi_periodic(np.ascontiguousarray(pos[:, :8]), m8, h8, L)
     assert np.abs(got - want.astype(np.float64)).max() < 1e-13 * np.abs(got).max()
+
+
+# ---- Eq. 5 (L65-70) with the cut |x - nL| < 2.6 L: periodic image sum ------------------------------------------------
+def test_periodic_images_count_and_two_body_sum(oracle):
+    """One source at the origin, one test particle at x: the force is the sum over the images inside the 2.6 L sphere
+    around x, typed out here with numpy; at x -> 0+ there are 81 such triplets minus the coincident one."""
+    L = 1.0
+    n = np.array([(a, b, c) for a in range(-4, 5) for b in range(-4, 5) for c in range(-4, 5)], dtype=float)
+    assert int(np.sum(np.sum(n * n, axis=1) < 2.6 ** 2)) == 81
+    xt = np.array([0.21, -0.13, 0.34])
+    v = xt[None, :] - n * L                                     # x_i - x_j - nL with x_j = 0
+    r = np.linalg.norm(v, axis=1)
+    keep = r < 2.6 * L
+    want = -(2.0 * v[keep] / r[keep, None] ** 3).sum(axis=0)    # m_j = 2, calF = 1/r^2 beyond the softening
+    pos = np.ascontiguousarray(np.array([xt, [0.0, 0.0, 0.0]]).T)
+    acc = oracle.forces_periodic_images(pos, np.array([1.0, 2.0]), np.array([0.01, 0.01]), L)
+    assert np.allclose(acc[:, 0], want, rtol=1e-13, atol=1e-15)
+
+
+def test_periodic_images_symmetries(oracle):
+    rng = np.random.default_rng(66)
+    L = 1.3
+    g = (np.arange(3) + 0.5) * L / 3
+    lat = np.ascontiguousarray(np.array(np.meshgrid(g, g, g, indexing="ij")).reshape(3, -1))
+    acc = oracle.forces_periodic_images(lat, np.full(27, 1 / 27), np.full(27, 0.01), L)
+    assert np.abs(acc).max() < 1e-12                            # every lattice site is a centre of symmetry
+    pos, mass, soft = _box(rng, 60, L)
+    ref = oracle.forces_periodic_images(pos, mass, soft, L)
+    # the image set of a separation does not depend on its representative: shifting particles by lattice vectors or
+    # translating the whole set (without wrapping) leaves the forces unchanged
+    moved = pos.copy(); moved[:, ::3] += np.array([[2 * L], [-L], [3 * L]])
+    assert np.abs(oracle.forces_periodic_images(np.ascontiguousarray(moved), mass, soft, L) - ref).max() < 1e-11 * np.abs(ref).max()
+    shifted = np.ascontiguousarray(pos + np.array([[0.37], [-1.9], [0.05]]))
+    assert np.abs(oracle.forces_periodic_images(shifted, mass, soft, L) - ref).max() < 1e-11 * np.abs(ref).max()
+    # Newton III
+    assert np.linalg.norm((mass * ref).sum(axis=1)) < 1e-13 * np.sum(mass * np.linalg.norm(ref, axis=0))
+    # the nearest image is one of the terms: removing the cut's other images gives back the quasi-periodic force
+    qp = oracle.forces_quasi_periodic(pos, mass, soft, L)
+    assert np.abs(ref - qp).max() > 1e-3 * np.abs(qp).max()     # the other images do contribute
