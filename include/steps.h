@@ -141,10 +141,18 @@ int steps_momentum(const double *vec, const double *mass, long long N, double *o
  * smallest length in a cubic box of side L (component-wise d - L rint(d / L), ties to even), otherwise exactly
  * steps_forces / steps_forces_mixed (mixed != 0): same layout, same pair law with pair softening soft_i + soft_j, G = 1,
  * acc overwritten.  Positions need not lie inside [0, L).  First version: every tile pair goes through the per-pair
- * softening test (no far/near split in a periodic box) in the persistent stream-K driver.  The full Ewald image
- * sum of Eq. 5 (|x - nL| < 2.6 L) is not built.  STEPS_EINVAL additionally for L <= 0. */
+ * softening test (no far/near split in a periodic box) in the persistent stream-K driver.  The image sum of Eq. 5 with the
+ * 2.6 L cut is steps_forces_periodic below.  STEPS_EINVAL additionally for L <= 0. */
 int steps_forces_quasi_periodic(const double *pos, const double *mass, const double *soft, long long N,
                                 double L, double *acc, int mixed, steps_stream_t stream);
+
+/* Periodic boundary conditions, Eq. 5 (L65-70, second part): the sum over the periodic
+ * images x - nL of every separation with the paper's cut |x - nL| < 2.6 L (strict), each image through the pair law with
+ * pair softening soft_i + soft_j; fp64 path only (the images of a homogeneous box cancel to a small remainder).  Layout,
+ * G = 1 and error behaviour as steps_forces_quasi_periodic; the result does not depend on which representative modulo L
+ * the positions are given in.  Cost: 343 candidate images per pair. */
+int steps_forces_periodic(const double *pos, const double *mass, const double *soft, long long N, double L,
+                          double *acc, steps_stream_t stream);
 
 /* Adaptive global time step, Eq. 12 (L113-116):
  *     dt = min[ dt_max, min_i sqrt(2 eta_i eps / |A_i|) ],  eta_i = 2.8 soft[i]  (L116, literal),

@@ -96,10 +96,10 @@ constexpr int persistent_smem_bytes()
 
 // ---- persistent stream-K driver ------------------------------------------------------------------
 // partials: [nb + gridDim.x slots][Path::NOUT][IB] doubles; CTA p's record for i-block b is slot b + p.
-// PERIODIC (quasi-periodic boundary, Eq. 5): every tile goes through the near body
-// with leading-image separations in a cubic box of side box_L -- the radial far/near classification of the compactified
+// BOX != 0 (periodic boundaries, Eq. 5): every tile goes through the near body with
+// leading-image separations (BOX = 1, quasi-periodic) or the image sum (BOX = 2) in a cubic box of side box_L -- the radial far/near classification of the compactified
 // sets does not apply in a periodic box.
-template <typename Path, int STAGES, bool PERIODIC = false>
+template <typename Path, int STAGES, int BOX = 0>   // BOX: 0 open boundary, 1 nearest image, 2 image sum with the 2.6 L cut
 __global__ void __launch_bounds__(CTA_THREADS, 1)
 forces_persistent_kernel(const double* __restrict__ pos, const double* __restrict__ soft, long long N,
                          const typename Path::Tile* __restrict__ tiles, int nt, long long i_begin, long long i_end,
@@ -158,8 +158,10 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
             const int s = it % STAGES;
             mbar_wait(&full_bar[s], (it / STAGES) & 1);
             const Tile& T = *reinterpret_cast<const Tile*>(smem_raw + s * STRIDE);
-            if constexpr (PERIODIC) {
+            if constexpr (BOX == 1) {
                 Path::template near_box<true>(T, S, acc, box_L, box_invL);
+            } else if constexpr (BOX == 2) {
+                Path::near_images(T, S, acc, box_L, box_invL);
             } else {
 #ifdef STEPS_DIAG_ALLFAR                                   // timing diagnostic only (wrong forces): no near body
             Path::far(T, S, F, zero);

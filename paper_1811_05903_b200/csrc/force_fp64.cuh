@@ -185,6 +185,48 @@ struct Fp64Path {
 
     static __device__ __forceinline__ void near(const Tile& T, const IState& S, double* acc) { near_box<false>(T, S, acc, 0.0, 0.0); }
 
+    // Periodic image sum, Eq. 5 (L65-70) with the paper's cut: every image x - nL of the separation with
+    // |x - nL| < 2.6 L contributes through the pair law.  Around the nearest image (|d_c| <= L/2) these are among the
+    // 343 triplets |n_c| <= 3; the loop walks all of them and applies the cut (row 8(f)-3, second part).  The 4
+    // register-blocked i-particles run in lockstep inside the image loop.
+    static __device__ __forceinline__ void near_images(const Tile& T, const IState& S, double* acc, double L, double invL)
+    {
+        const double cut2 = (2.6 * L) * (2.6 * L);
+        double ax[R_I], ay[R_I], az[R_I];
+#pragma unroll
+        for (int k = 0; k < R_I; ++k) ax[k] = ay[k] = az[k] = 0.0;
+#pragma unroll 1
+        for (int j = 0; j < TJ; ++j) {
+            const double xj = T.x[j], yj = T.y[j], zj = T.z[j], mq = T.m[j], hj = T.h[j];
+            if (mq == 0.0) continue;                                   // pads and massless sources (warp-uniform)
+            double dx[R_I], dy[R_I], dz[R_I], hs2[R_I], hs[R_I];
+#pragma unroll
+            for (int k = 0; k < R_I; ++k) {
+                dx[k] = wrap(xj - S.x[k], L, invL); dy[k] = wrap(yj - S.y[k], L, invL); dz[k] = wrap(zj - S.z[k], L, invL);
+                hs[k] = S.h[k] + hj; hs2[k] = hs[k] * hs[k];
+            }
+#pragma unroll 1
+            for (int n1 = -3; n1 <= 3; ++n1)
+#pragma unroll 1
+                for (int n2 = -3; n2 <= 3; ++n2)
+#pragma unroll 1
+                    for (int n3 = -3; n3 <= 3; ++n3) {
+                        const double ox = n1 * L, oy = n2 * L, oz = n3 * L;
+#pragma unroll
+                        for (int k = 0; k < R_I; ++k) {
+                            const double vx = dx[k] - ox, vy = dy[k] - oy, vz = dz[k] - oz;
+                            const double r2 = fma(vz, vz, fma(vy, vy, vx * vx));
+                            double s = mq * rcube(r2);
+                            if (r2 < hs2[k] || r2 == 0.0) s = (r2 == 0.0) ? 0.0 : mq * spline_g_soft_f64(r2, hs[k]);
+                            if (!(r2 < cut2)) s = 0.0;                 // "|x - nL| < 2.6 L" (strict, as printed)
+                            ax[k] = fma(vx, s, ax[k]); ay[k] = fma(vy, s, ay[k]); az[k] = fma(vz, s, az[k]);
+                        }
+                    }
+        }
+#pragma unroll
+        for (int k = 0; k < R_I; ++k) { flush(acc, 0, k, ax[k]); flush(acc, 1, k, ay[k]); flush(acc, 2, k, az[k]); }
+    }
+
     // PERIODIC: every separation is replaced by its leading image in a cubic box of side L (row 8(f)-3).
     template <bool PERIODIC>
     static __device__ __forceinline__ void near_box(const Tile& T, const IState& S, double* acc, double L, double invL)

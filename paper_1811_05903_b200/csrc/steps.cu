@@ -37,7 +37,7 @@ struct Workspace {
     long long cap_particles = 0;
     int num_sms = 0;
     int grid_mixed = 0, grid_fp64 = 0;   // persistent grids: SMs x resident CTAs
-    int grid_mixed_periodic = 0, grid_fp64_periodic = 0;
+    int grid_mixed_periodic = 0, grid_fp64_periodic = 0, grid_fp64_images = 0;
     double* mom_partial = nullptr;  // MOM_BLOCKS * 4
     // staging buffers of steps_forces_host
     double* h_pos = nullptr; double* h_mass = nullptr; double* h_soft = nullptr; double* h_acc = nullptr;
@@ -161,7 +161,7 @@ int forces_impl(const double* pos, const double* mass, const double* soft, long 
                  : launch_forces<Fp64Path>(pos, mass, soft, N, i_begin, i_end, acc_out, st, w, w.grid_fp64);
 }
 
-template <typename Path>
+template <typename Path, int BOX>
 int launch_forces_periodic(const double* pos, const double* mass, const double* soft, long long N, double L, double* acc_out,
                            cudaStream_t st, Workspace& w, int& grid_cache)
 {
@@ -171,7 +171,7 @@ int launch_forces_periodic(const double* pos, const double* mass, const double* 
     prep_tiles<Tile><<<nt, TJ, 0, st>>>(pos, mass, soft, N, tiles);
     const int nb = (int)nblocks_of(N);
     constexpr int smem = persistent_smem_bytes<Path, STAGES>();
-    auto kern = forces_persistent_kernel<Path, STAGES, true>;
+    auto kern = forces_persistent_kernel<Path, STAGES, BOX>;
     if (grid_cache == 0) {
         STEPS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         int per_sm = 0;
@@ -205,8 +205,24 @@ int steps_forces_quasi_periodic(const double* pos, const double* mass, const dou
     if (rc != STEPS_OK) return rc;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     Workspace& w = g_ws[dev];
-    return mixed ? launch_forces_periodic<MixedPath>(pos, mass, soft, N, L, acc, st, w, w.grid_mixed_periodic)
-                 : launch_forces_periodic<Fp64Path>(pos, mass, soft, N, L, acc, st, w, w.grid_fp64_periodic);
+    return mixed ? launch_forces_periodic<MixedPath, 1>(pos, mass, soft, N, L, acc, st, w, w.grid_mixed_periodic)
+                 : launch_forces_periodic<Fp64Path, 1>(pos, mass, soft, N, L, acc, st, w, w.grid_fp64_periodic);
+}
+
+int steps_forces_periodic(const double* pos, const double* mass, const double* soft, long long N, double L, double* acc,
+                          steps_stream_t stream)
+{
+    if (!pos || !mass || !soft || !acc || N < 1 || !(L > 0.0)) return STEPS_EINVAL;
+    if (N > (1ll << 31) - TJ) return STEPS_EINVAL;
+    if (misaligned(pos) || misaligned(mass) || misaligned(soft) || misaligned(acc)) return STEPS_EINVAL;
+    int dev;
+    int rc = current_device(&dev);
+    if (rc != STEPS_OK) return rc;
+    rc = ensure_workspace(dev, N);
+    if (rc != STEPS_OK) return rc;
+    Workspace& w = g_ws[dev];
+    return launch_forces_periodic<Fp64Path, 2>(pos, mass, soft, N, L, acc, reinterpret_cast<cudaStream_t>(stream), w,
+                                               w.grid_fp64_images);
 }
 
 int steps_forces(const double* pos, const double* mass, const double* soft, long long N, double* acc,

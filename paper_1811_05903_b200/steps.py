@@ -16,7 +16,7 @@ OK, EINVAL, ECUDA, EUNSUPPORTED, ENOMEM = 0, -1, -2, -3, -4
 EXPORTS = [
     "steps_forces", "steps_forces_mixed", "steps_forces_range", "steps_forces_host", "steps_kick_drift",
     "steps_kdk_step", "steps_hubble", "steps_scale_factor_rk4", "steps_kdk_schedule", "steps_momentum",
-    "steps_timestep", "steps_force_residual", "steps_forces_quasi_periodic",
+    "steps_timestep", "steps_force_residual", "steps_forces_quasi_periodic", "steps_forces_periodic",
     "steps_kdk_step_adaptive", "steps_kick_close_adaptive",
     "steps_reserve", "steps_shutdown", "steps_workspace_bytes", "steps_strerror", "steps_last_cuda_error",
     "steps_version", "steps_kernel_launch_count", "steps_set_option", "steps_last_force_kernel_ms",
@@ -63,6 +63,7 @@ def lib() -> C.CDLL:
     L.steps_kdk_schedule.argtypes = [dbl, dbl, dbl, C.POINTER(Cosmology), C.POINTER(dbl)]
     L.steps_momentum.argtypes = [vp, vp, ll, vp, vp]
     L.steps_forces_quasi_periodic.argtypes = [vp, vp, vp, ll, dbl, vp, i32, vp]
+    L.steps_forces_periodic.argtypes = [vp, vp, vp, ll, dbl, vp, vp]
     L.steps_kdk_step_adaptive.argtypes = [vp, vp, vp, vp, vp, ll, vp, C.POINTER(Cosmology), dbl, dbl, dbl, dbl, i32, vp]
     L.steps_kick_close_adaptive.argtypes = [vp, vp, vp, ll, vp, dbl, vp]
     L.steps_timestep.argtypes = [vp, vp, vp, ll, dbl, dbl, dbl, dbl, vp, vp]
@@ -178,6 +179,13 @@ def steps_forces_quasi_periodic(pos, mass, soft, L: float, acc, mixed: bool = Fa
     n = mass.numel()
     _check(lib().steps_forces_quasi_periodic(_dev(pos, 3 * n), _dev(mass, n), _dev(soft, n), n, float(L), _dev(acc, 3 * n),
                                              int(mixed), _stream(stream)))
+
+
+def steps_forces_periodic(pos, mass, soft, L: float, acc, stream=None) -> None:
+    """Eq. 5 image sum with the cut |x - nL| < 2.6 L in a cubic box of side L (fp64 path)."""
+    n = mass.numel()
+    _check(lib().steps_forces_periodic(_dev(pos, 3 * n), _dev(mass, n), _dev(soft, n), n, float(L), _dev(acc, 3 * n),
+                                       _stream(stream)))
 
 
 def steps_kdk_step_adaptive(pos, vel, acc, mass, soft, state5, cosmo: "Cosmology", G: float, B: float, eps: float,

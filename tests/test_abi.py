@@ -58,6 +58,7 @@ def test_argument_checks_without_a_device():
     assert L.steps_forces_host(None, None, None, 4, None, 0, None) == S.EINVAL
     assert L.steps_kick_drift(None, None, None, 4, None, None) == S.EINVAL
     assert L.steps_momentum(None, None, 4, None, None) == S.EINVAL
+    assert L.steps_forces_periodic(None, None, None, 4, 1.0, None, None) == S.EINVAL
     assert L.steps_forces_quasi_periodic(None, None, None, 4, 1.0, None, 0, None) == S.EINVAL
     assert L.steps_kdk_step_adaptive(None, None, None, None, None, 4, None, None, 1.0, 0.0, 0.025, 1.0, 0, None) == S.EINVAL
     assert L.steps_kick_close_adaptive(None, None, None, 4, None, 0.0, None) == S.EINVAL

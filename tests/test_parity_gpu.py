@@ -499,6 +499,36 @@ def test_device_resident_steps_replay_from_a_cuda_graph(S, oracle):
     assert torch.equal(pos_g, pos_e) and torch.equal(vel_g, vel_e) and torch.equal(acc_g, acc_e)
 
 
+# ---- Eq. 5 (L65-70) with the cut |x - nL| < 2.6 L: periodic image sum (fp64) ------------------------------------------
+@pytest.mark.gpu
+@pytest.mark.parametrize("n", [2, 27, 300, 1500])
+def test_periodic_image_sum_matches_oracle(S, oracle, n):
+    import torch
+    L = 1.3
+    pos, mass, soft = _periodic_box(n, L, 6600 + n)
+    if n == 27:                                  # simple-cubic lattice: every site a centre of symmetry, force 0
+        g = (np.arange(3) + 0.5) * L / 3
+        pos = np.ascontiguousarray(np.array(np.meshgrid(g, g, g, indexing="ij")).reshape(3, -1))
+    acc = torch.empty(3, n, dtype=torch.float64, device="cuda")
+    S.steps_forces_periodic(dev(pos), dev(mass), dev(soft), L, acc)
+    got = acc.cpu().numpy()
+    ref = oracle.forces_periodic_images(pos, mass, soft, L)
+    if n == 27:
+        assert np.abs(got).max() < 1e-12 and np.abs(ref).max() < 1e-12
+        return
+    # ~80 images per pair cancel to a remainder: the error is measured against the scale of what is summed
+    scale = _pair_force_abs_sum(pos, mass, soft, L)
+    e_abs = np.linalg.norm(got - ref, axis=0) / scale
+    e = rel_err(got, ref)
+    print(f"[image sum n={n}] relative to net force: max {e.max():.3e}; relative to sum_j |f_ij|: max {e_abs.max():.3e}")
+    assert e_abs.max() <= 1e-12 and e.max() <= 1e-10
+    # representative independence on the device: shift a third of the particles by lattice vectors
+    moved = pos.copy(); moved[:, ::3] += np.array([[2 * L], [-L], [3 * L]])
+    acc2 = torch.empty_like(acc)
+    S.steps_forces_periodic(dev(np.ascontiguousarray(moved)), dev(mass), dev(soft), L, acc2)
+    assert np.abs(acc2.cpu().numpy() - got).max() <= 1e-10 * np.abs(got).max()
+
+
 def test_config4_lockstep_200_steps_8192(S, oracle):
     """Config 4 at N = 8192, every one of the 200 comoving KDK steps (a: 1/51 -> 1): the library steps
     from the ORACLE's state (x_n, v_n, acc_n) and must land on the oracle's (x_{n+1}, v_{n+1},

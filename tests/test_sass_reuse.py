@@ -62,5 +62,5 @@ def test_built_library_is_calibrated_and_fully_patched():
     for n in names:
         assert sass_reuse.plan(funcs[n]) == {}, n     # the build step left nothing to patch (idempotent)
     # the fp64 far loop: every accumulate triple shares s through the reuse cache
-    text = [t for _, t, _, _ in funcs[[n for n in names if "persistent" in n and "Fp64" in n and "Lb0" in n][0]]]
+    text = [t for _, t, _, _ in funcs[[n for n in names if "persistent" in n and "Fp64" in n and "Li4ELi0E" in n][0]]]
     assert sum(".reuse" in t and t.startswith("DFMA") for t in text) >= 20
