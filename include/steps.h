@@ -150,7 +150,7 @@ int steps_forces_quasi_periodic(const double *pos, const double *mass, const dou
  * images x - nL of every separation with the paper's cut |x - nL| < 2.6 L (strict), each image through the pair law with
  * pair softening soft_i + soft_j; fp64 path only (the images of a homogeneous box cancel to a small remainder).  Layout,
  * G = 1 and error behaviour as steps_forces_quasi_periodic; the result does not depend on which representative modulo L
- * the positions are given in.  Cost: 343 candidate images per pair. */
+ * the positions are given in.  Cost: 179 candidate images per pair (about 81 of them inside the cut). */
 int steps_forces_periodic(const double *pos, const double *mass, const double *soft, long long N, double L,
                           double *acc, steps_stream_t stream);
 

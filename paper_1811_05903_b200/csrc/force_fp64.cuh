@@ -67,6 +67,21 @@ __device__ __noinline__ double spline_g_soft_f64(double r2, double h)
     return ih3 * (64.0 / 3.0 + u * (-48.0 + u * (38.4 - (32.0 / 3.0) * u))) - 1.0 / (15.0 * r * r2);
 }
 
+// Integer triplets n with n.n <= 12: a superset of every n with |d - nL| < 2.6 L for |d_c| <= L/2 (Eq. 5 cut).
+constexpr int EWALD_NTRIPLETS = 179;
+struct EwaldTriplets {
+    double3 v[EWALD_NTRIPLETS];
+    constexpr EwaldTriplets() : v{}
+    {
+        int c = 0;
+        for (int a = -3; a <= 3; ++a)
+            for (int b = -3; b <= 3; ++b)
+                for (int d = -3; d <= 3; ++d)
+                    if (a * a + b * b + d * d <= 12) { v[c].x = a; v[c].y = b; v[c].z = d; ++c; }
+    }
+};
+__constant__ double3 ewald_triplets[EWALD_NTRIPLETS];
+
 struct Fp64Path {
     using Tile = TileF64;
 
@@ -187,8 +202,9 @@ struct Fp64Path {
 
     // Periodic image sum, Eq. 5 (L65-70) with the paper's cut: every image x - nL of the separation with
     // |x - nL| < 2.6 L contributes through the pair law.  Around the nearest image (|d_c| <= L/2) these are among the
-    // 343 triplets |n_c| <= 3; the loop walks all of them and applies the cut (row 8(f)-3, second part).  The 4
-    // register-blocked i-particles run in lockstep inside the image loop.
+    // triplets with |n| < 2.6 + sqrt(3)/2, i.e. n.n <= 12: 179 of them (constant-memory table ewald_triplets); the loop
+    // walks these and applies the cut per image (row 8(f)-3, second part).  The 4 register-blocked i-particles run in
+    // lockstep inside the image loop.
     static __device__ __forceinline__ void near_images(const Tile& T, const IState& S, double* acc, double L, double invL)
     {
         const double cut2 = (2.6 * L) * (2.6 * L);
@@ -206,22 +222,18 @@ struct Fp64Path {
                 hs[k] = S.h[k] + hj; hs2[k] = hs[k] * hs[k];
             }
 #pragma unroll 1
-            for (int n1 = -3; n1 <= 3; ++n1)
-#pragma unroll 1
-                for (int n2 = -3; n2 <= 3; ++n2)
-#pragma unroll 1
-                    for (int n3 = -3; n3 <= 3; ++n3) {
-                        const double ox = n1 * L, oy = n2 * L, oz = n3 * L;
+            for (int c = 0; c < EWALD_NTRIPLETS; ++c) {
+                const double ox = ewald_triplets[c].x * L, oy = ewald_triplets[c].y * L, oz = ewald_triplets[c].z * L;
 #pragma unroll
-                        for (int k = 0; k < R_I; ++k) {
-                            const double vx = dx[k] - ox, vy = dy[k] - oy, vz = dz[k] - oz;
-                            const double r2 = fma(vz, vz, fma(vy, vy, vx * vx));
-                            double s = mq * rcube(r2);
-                            if (r2 < hs2[k] || r2 == 0.0) s = (r2 == 0.0) ? 0.0 : mq * spline_g_soft_f64(r2, hs[k]);
-                            if (!(r2 < cut2)) s = 0.0;                 // "|x - nL| < 2.6 L" (strict, as printed)
-                            ax[k] = fma(vx, s, ax[k]); ay[k] = fma(vy, s, ay[k]); az[k] = fma(vz, s, az[k]);
-                        }
-                    }
+                for (int k = 0; k < R_I; ++k) {
+                    const double vx = dx[k] - ox, vy = dy[k] - oy, vz = dz[k] - oz;
+                    const double r2 = fma(vz, vz, fma(vy, vy, vx * vx));
+                    double s = mq * rcube(r2);
+                    if (r2 < hs2[k] || r2 == 0.0) s = (r2 == 0.0) ? 0.0 : mq * spline_g_soft_f64(r2, hs[k]);
+                    if (!(r2 < cut2)) s = 0.0;                         // "|x - nL| < 2.6 L" (strict, as printed)
+                    ax[k] = fma(vx, s, ax[k]); ay[k] = fma(vy, s, ay[k]); az[k] = fma(vz, s, az[k]);
+                }
+            }
         }
 #pragma unroll
         for (int k = 0; k < R_I; ++k) { flush(acc, 0, k, ax[k]); flush(acc, 1, k, ay[k]); flush(acc, 2, k, az[k]); }

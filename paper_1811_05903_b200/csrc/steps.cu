@@ -221,6 +221,14 @@ int steps_forces_periodic(const double* pos, const double* mass, const double* s
     rc = ensure_workspace(dev, N);
     if (rc != STEPS_OK) return rc;
     Workspace& w = g_ws[dev];
+    if (w.grid_fp64_images == 0) {                       // first use on this device: upload the triplet table
+        static const EwaldTriplets table;
+        int count = 0;
+        for (int c = 0; c < EWALD_NTRIPLETS; ++c) count += (table.v[c].x * table.v[c].x + table.v[c].y * table.v[c].y +
+                                                             table.v[c].z * table.v[c].z <= 12.0);
+        if (count != EWALD_NTRIPLETS) return STEPS_EUNSUPPORTED;
+        STEPS_CUDA(cudaMemcpyToSymbol(ewald_triplets, table.v, sizeof(table.v)));
+    }
     return launch_forces_periodic<Fp64Path, 2>(pos, mass, soft, N, L, acc, reinterpret_cast<cudaStream_t>(stream), w,
                                                w.grid_fp64_images);
 }
