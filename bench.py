@@ -35,7 +35,14 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 FLOP_PER_INTERACTION = 20.0      # stated convention
-SM_COUNT, SM_MAX_MHZ = 148, 1965.0
+SM_COUNT, SM_MAX_MHZ, SM_MHZ_SOURCE = 148, 1965.0, "profiling guide (1965 MHz)"
+try:                                   # driver-written per pod; absent -> the guide's B200 boost clock
+    with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as _f:
+        _mhz = float(json.load(_f).get("sm_max_mhz", 0.0))
+    if 1000.0 < _mhz < 3000.0:
+        SM_MAX_MHZ, SM_MHZ_SOURCE = _mhz, "MEASURED_PEAKS.json sm_max_mhz"
+except (OSError, ValueError):
+    pass
 PEAK_FP32_TFLOPS = SM_COUNT * 128 * 2 * SM_MAX_MHZ * 1e6 / 1e12     # 74.45
 PEAK_FP64_TFLOPS = SM_COUNT * 64 * 2 * SM_MAX_MHZ * 1e6 / 1e12      # 37.22 (64 FP64 lanes/SM, measured)
 METRIC = "pairwise interactions/s per force eval at N=1M"
@@ -261,7 +268,7 @@ def main():
                 "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                              "frac": achieved / peak, "traffic": NCU_DRAM_BYTES[path],
                              "flop_per_interaction": FLOP_PER_INTERACTION,
-                             "peak_source": "148 SM x %d lanes x 2 x 1965 MHz (DESIGN.md; lanes/SM measured)" % (128 if mixed else 64),
+                             "peak_source": "148 SM x %d lanes x 2 x %.0f MHz (%s; DESIGN.md section 6; lanes/SM measured)" % (128 if mixed else 64, SM_MAX_MHZ, SM_MHZ_SOURCE),
                              "kernel": "forces_persistent_kernel<%s>" % ("MixedPath" if mixed else "Fp64Path"),
                              "kernel_share_of_step": k_ms * args.steps / total_ms},
             }
