@@ -55,7 +55,9 @@ enum {
     STEPS_EINVAL = -1,       /* null pointer, N < 1, misaligned pointer, bad range */
     STEPS_ECUDA = -2,        /* CUDA runtime / launch error (steps_last_cuda_error() has the code) */
     STEPS_EUNSUPPORTED = -3, /* current device is not sm_100 */
-    STEPS_ENOMEM = -4        /* workspace allocation failed */
+    STEPS_ENOMEM = -4,       /* workspace allocation failed */
+    STEPS_ECAPTURE = -5      /* the call would have to allocate workspace while its stream is being captured into a CUDA
+                                graph: call steps_reserve(N) (and, for steps_forces_periodic, one un-captured call) first */
 };
 
 /* ---- force evaluation --------------------------------- */

@@ -22,7 +22,9 @@
  * regular polyhedra and a Fibonacci shell, Newton's third law, symmetries, an
  * independent numpy longdouble brute force on N <= 8, RK4 a(t) vs closed forms, drag
  * and background-term closed forms with 2nd-order convergence, Kepler orbit; Eq. 12 time step against the two-body
- * closed form, its scaling laws, the dt_max clamp and a numpy brute force.
+ * closed form, its scaling laws, the dt_max clamp and a numpy brute force; the momentum diagnostic against hand-typed
+ * three-particle values and a numpy longdouble brute force; the growth rate (oracle/steps_oracle.py, config-4 initial
+ * velocities) against the hypergeometric closed form of flat LCDM.
  * Parity status: every function below is pinned (none "parity unpinned"); the choice
  * of how the drag enters the kick (reading #8) is a reading the paper does not fix.
  */

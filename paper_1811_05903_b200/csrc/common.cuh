@@ -28,9 +28,6 @@ typedef unsigned long long u64;
 #endif
 // Constant folded into the scaled copy of the fp64 tiles: c_j = (STEPS_FP64_FOLD m_j)^(-1/2) (force_fp64.cuh).
 #define STEPS_FP64_FOLD 1.875
-#ifndef STEPS_MIXED_ACC_SCALAR
-#define STEPS_MIXED_ACC_SCALAR 0
-#endif
 // fp32 tiles store c[] with adjacent elements swapped (c[j ^ 1]): after the LDS.128 loads of the far
 // body the scalar c_q then sits in a register of the opposite parity (bank) to X_q / Y_q / Z_q.
 #ifndef STEPS_C_SWIZZLE

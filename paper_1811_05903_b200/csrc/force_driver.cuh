@@ -94,17 +94,45 @@ constexpr int persistent_smem_bytes()
     return STAGES * stage_stride((int)sizeof(typename Path::Tile)) + Path::NOUT * R_I * CTA_THREADS * (int)sizeof(double);
 }
 
+// ---- band mode (force_sym.cuh) ---------------------------------------------------------------------
+// Device-resident plan of a pair-symmetric force evaluation (written by sym_band_width + sym_plan_finalize in force_sym.cuh).
+// In BAND mode the persistent driver only visits, for i-block b, the tiles of the blocks c with |c - b| <= W; the far block
+// pairs beyond the band are the work items of forces_sym_kernel.
+struct SymPlan {
+    int W;            // band half-width in blocks of IB particles
+    int nb;           // blocks
+    int Km;           // rows that own symmetric items: max(0, nb - 1 - W)
+    int nt;           // j-tiles, padded to whole blocks: nb * (IB / TJ)
+    long long K;      // symmetric items: Km (Km + 1) / 2
+    long long T;      // band tile visits: cum[nb]
+};
+// followed in memory by  long long cum[nb + 1]: band tile visits of the rows before b
+__device__ __forceinline__ const long long* plan_cum(const SymPlan* plan) { return reinterpret_cast<const long long*>(plan + 1); }
+// row b of the band with cum[b] <= w < cum[b + 1]
+__device__ __forceinline__ int band_row_of(const long long* __restrict__ cum, int nb, long long w)
+{
+    int lo = 0, hi = nb - 1;
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (cum[mid] <= w) lo = mid; else hi = mid - 1;
+    }
+    return lo;
+}
+
 // ---- persistent stream-K driver ------------------------------------------------------------------
 // partials: [nb + gridDim.x slots][Path::NOUT][IB] doubles; CTA p's record for i-block b is slot b + p.
 // BOX != 0 (periodic boundaries, Eq. 5): every tile goes through the near body with
 // leading-image separations (BOX = 1, quasi-periodic) or the image sum (BOX = 2) in a cubic box of side box_L -- the radial far/near classification of the compactified
 // sets does not apply in a periodic box.
-template <typename Path, int STAGES, int BOX = 0>   // BOX: 0 open boundary, 1 nearest image, 2 image sum with the 2.6 L cut
+// BAND (open boundary only): the iteration space is the band of `plan` instead of all nb x nt (i-block, tile) pairs.
+template <typename Path, int STAGES, int BOX = 0, bool BAND = false>   // BOX: 0 open boundary, 1 nearest image, 2 image sum with the 2.6 L cut
 __global__ void __launch_bounds__(CTA_THREADS, 1)
 forces_persistent_kernel(const double* __restrict__ pos, const double* __restrict__ soft, long long N,
                          const typename Path::Tile* __restrict__ tiles, int nt, long long i_begin, long long i_end,
-                         int nb, double* __restrict__ partials, int zero, double box_L, double box_invL)
+                         int nb, double* __restrict__ partials, int zero, double box_L, double box_invL,
+                         const SymPlan* __restrict__ plan)
 {
+    static_assert(!BAND || BOX == 0, "the band split applies to the open boundary only");
     using Tile = typename Path::Tile;
     constexpr int STRIDE = stage_stride((int)sizeof(Tile));
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -112,7 +140,9 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
     double* acc = reinterpret_cast<double*>(smem_raw + STAGES * STRIDE) + threadIdx.x;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const long long W = (long long)nb * nt;
+    const long long* cum = BAND ? plan_cum(plan) : nullptr;
+    const int bandW = BAND ? plan->W : 0;
+    const long long W = BAND ? plan->T : (long long)nb * nt;
     const long long w0 = (long long)blockIdx.x * W / gridDim.x;
     const long long w1 = ((long long)blockIdx.x + 1) * W / gridDim.x;
     const int total = (int)(w1 - w0);                       // tiles this CTA streams
@@ -130,7 +160,14 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
         const int s = k % STAGES;
         if (k >= STAGES) mbar_wait(&empty_bar[s], ((k / STAGES) - 1) & 1);
         mbar_expect_tx(&full_bar[s], (uint32_t)sizeof(Tile));
-        bulk_load(smem_raw + s * STRIDE, tiles + (w0 + k) % nt, (uint32_t)sizeof(Tile), &full_bar[s]);
+        long long tile;
+        if constexpr (BAND) {                                   // band mode: row of the linear index, then its tile
+            const int pb = band_row_of(cum, nb, w0 + k);
+            tile = (long long)max(0, pb - bandW) * (IB / TJ) + (w0 + k - cum[pb]);
+        } else {
+            tile = (w0 + k) % nt;
+        }
+        bulk_load(smem_raw + s * STRIDE, tiles + tile, (uint32_t)sizeof(Tile), &full_bar[s]);
     };
     if (threadIdx.x == 0) {
         for (int k = 0; k < STAGES - 1 && k < total; ++k) produce(k);
@@ -139,9 +176,15 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
     int it = 0;                                             // tiles consumed so far
     long long w = w0;
     while (w < w1) {
-        const int b = (int)(w / nt);
-        const int t0 = (int)(w - (long long)b * nt);
-        const int cnt = (int)min((long long)(nt - t0), w1 - w);
+        int b, cnt;
+        if constexpr (BAND) {
+            b = band_row_of(cum, nb, w);
+            cnt = (int)min(cum[b + 1] - w, w1 - w);
+        } else {
+            b = (int)(w / nt);
+            const int t0 = (int)(w - (long long)b * nt);
+            cnt = (int)min((long long)(nt - t0), w1 - w);
+        }
 
         typename Path::IState S;
         float rlo, rhi, hh;
@@ -163,10 +206,6 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
             } else if constexpr (BOX == 2) {
                 Path::near_images(T, S, acc, box_L, box_invL);
             } else {
-#ifdef STEPS_DIAG_ALLFAR                                   // timing diagnostic only (wrong forces): no near body
-            Path::far(T, S, F, zero);
-            if (++pending >= Path::FAR_TILES_PER_FLUSH) { Path::far_flush(F, acc); pending = 0; }
-#else
             // the decision is warp-uniform by construction (warp-reduced bounds); the vote tells the compiler so
             if (__all_sync(0xffffffffu, tile_is_far(rlo, rhi, hh, T.meta))) {
                 Path::far(T, S, F, zero);
@@ -175,7 +214,6 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
                 if (pending) { Path::far_flush(F, acc); pending = 0; }
                 Path::near(T, S, acc);
             }
-#endif
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty_bar[s]);
@@ -217,6 +255,38 @@ __global__ void __launch_bounds__(256) forces_reduce_kernel(const double* __rest
             if (NOUT == 6) lo += rec[(long long)(3 + c) * IB];
         }
         acc_out[(long long)c * cnt + i] = hi + lo;
+    }
+}
+
+// The same for the BAND mode (rows of different lengths: the owners of a row come from the plan's cumulative counts).
+// to_dd != 0: the result stays double-double in (acc_hi, acc_lo) for forces_sym_reduce_kernel to add its records to.
+template <int NOUT>
+__global__ void __launch_bounds__(256) forces_band_reduce_kernel(const double* __restrict__ partials, const SymPlan* __restrict__ plan,
+                                                                 int P, long long cnt, double* __restrict__ acc_out,
+                                                                 int to_dd, double* __restrict__ acc_hi, double* __restrict__ acc_lo)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= cnt) return;
+    const long long* cum = plan_cum(plan);
+    const long long W = plan->T;
+    const int b = (int)(i / IB), off = (int)(i - (long long)b * IB);
+    const int p_lo = (int)(((cum[b] + 1) * P - 1) / W);
+    const int p_hi = (int)((cum[b + 1] * P - 1) / W);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        double hi = 0.0, lo = 0.0;
+        for (int p = p_lo; p <= p_hi; ++p) {
+            const long long w0 = (long long)p * W / P, w1 = ((long long)p + 1) * W / P;
+            if (w1 <= w0) continue;
+            const double* rec = partials + ((long long)(b + p) * NOUT) * IB + off;
+            const double v = rec[(long long)c * IB];
+            const double s = hi + v, bb = s - hi;
+            lo += (hi - (s - bb)) + (v - bb);                          // TwoSum
+            hi = s;
+            if (NOUT == 6) lo += rec[(long long)(3 + c) * IB];
+        }
+        if (to_dd) { acc_hi[(long long)c * cnt + i] = hi; acc_lo[(long long)c * cnt + i] = lo; }
+        else acc_out[(long long)c * cnt + i] = hi + lo;
     }
 }
 

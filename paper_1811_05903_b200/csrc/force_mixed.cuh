@@ -114,19 +114,9 @@ STEPS_UNROLL(STEPS_FAR_UNROLL)
                     unpack2(r2, a, b);
                     const u64 y = pack2(rsqrt_approx(a), rsqrt_approx(b));
                     const u64 y3 = mul2(mul2(y, y), y);
-#if STEPS_MIXED_ACC_SCALAR
-                    {
-                        float dl, dh, yl, yh, al, ah;
-                        unpack2(y3, yl, yh);
-                        unpack2(dX, dl, dh); unpack2(ax[p], al, ah); ax[p] = pack2(fmaf(dl, yl, al), fmaf(dh, yh, ah));
-                        unpack2(dY, dl, dh); unpack2(ay[p], al, ah); ay[p] = pack2(fmaf(dl, yl, al), fmaf(dh, yh, ah));
-                        unpack2(dZ, dl, dh); unpack2(az[p], al, ah); az[p] = pack2(fmaf(dl, yl, al), fmaf(dh, yh, ah));
-                    }
-#else
                     ax[p] = fma2(dX, y3, ax[p]);
                     ay[p] = fma2(dY, y3, ay[p]);
                     az[p] = fma2(dZ, y3, az[p]);
-#endif
                 }
             }
         }

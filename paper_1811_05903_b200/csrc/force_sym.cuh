@@ -1,0 +1,315 @@
+// force_sym.cuh -- the pair-symmetric force driver: every unordered FAR pair is evaluated ONCE and applied to both
+// particles (Newton's third law; PAPER.md L131 counts the cost of the force calculation as N(N-1)/2 pair evaluations).
+//
+// Rows a1 + a3 of the hot path (Eq. 8 L88 first term, Eq. 4 third case L59) for the bulk of the pairs:
+//
+//   * The particles are cut into BLOCKS of IB = 2048 consecutive (radially sorted) particles = 8 j-tiles.  A block pair
+//     (b, c) is "far" when the radial intervals of the two blocks are separated by more than hmax_b + hmax_c (the same
+//     triangle-inequality test as tile_is_far, on block bounds): then no pair of it can be softened and every pair
+//     is exactly Newtonian.  W = max |c - b| over the block pairs that are NOT far (a device scalar, sym_band_width):
+//     for radially sorted input W = 1 (only neighbouring blocks touch), for unsorted input W = nb - 1.
+//   * Block pairs with |c - b| <= W (the "band": the diagonal, all softened pairs, the self pairs) go through the
+//     asymmetric persistent kernel of force_driver.cuh, restricted to the band's tiles.
+//   * Every block pair with c - b > W is ONE work item of forces_sym_kernel: the CTA's 16 warps hold the 2048 particles of
+//     block b in registers (4 per lane, as the asymmetric kernel does), block c's scaled sources sit in shared memory, and
+//     warp w meets the sixteen 128-source subgroups of c in the order (w + q) mod 16, q = 0..15 (one __syncthreads per
+//     round, so each subgroup's reaction sums in shared memory have one owner at a time).  Inside a (warp, subgroup)
+//     meeting the sources are handed round the warp: at step s lane l works on source (l - s) mod 32 of the current
+//     32-source set against its own 4 particles and then passes that source's reaction sums (3 doubles, 6 SHFL) on to
+//     lane l + 1; after 32 steps every source has met all 128 particles of the warp and its sums are back in the
+//     lane they started in.
+//   * Per pair: 3 DFMA differences, 3 for r^2, 5 for r^-3 (the body of force_fp64.cuh), 1 DMUL s_i = m_i s and
+//     2 x 3 DFMA accumulates = 18 FP64-pipe instructions per UNORDERED pair = 9 per ordered interaction (14 in the
+//     asymmetric body).  The seven instructions of the accumulate stage are ordered so that each reads at most two new
+//     register operands (w, then dZ, then s_i stay in the operand-reuse cache), i.e. all hold the pipe for 2 clk.
+//   * An item writes two partial records of 3 x 2048 doubles: the forces of c on the particles of b (row record) and of b on
+//     the particles of c (column record: the reaction sums B_j = sum_i m_i s dX times -1.875 c_j^2 = -1/m_j, see below).
+//     forces_sym_reduce_kernel adds the records of each particle in fixed order (TwoSum, double-double) to the band's
+//     result: bit-reproducible, no atomics.  Record memory is bounded by running the items in panels.
+//
+// Scaled sources (common.cuh): dX = X_j - c_j x_i = c_j (x_j - x_i), s = (c_j r)^-3 / 1.875, c_j = (1.875 m_j)^(-1/2):
+//   force per unit mass on i:  m_j (x_j - x_i) / r^3 = s dX
+//   force per unit mass on j:  m_i (x_i - x_j) / r^3 = -(m_i s dX) / m_j = -(1.875 c_j^2) (m_i s) dX
+// Massless or unscalable particles cannot take part (their reaction sum cannot be divided by m_j): prep_tiles marks their
+// tile hmax = +inf, which makes every block pair of that block "not far", W = nb - 1, and the whole evaluation runs
+// through the asymmetric kernel -- slower, never wrong.
+#pragma once
+#include "common.cuh"
+#include "force_fp64.cuh"
+#include "force_driver.cuh"
+
+namespace steps {
+
+constexpr int TPB = IB / TJ;                 // j-tiles per block (8)
+constexpr int SUBGROUPS = CTA_THREADS / 32;  // 128-particle subgroups per block = warps per CTA (16)
+static_assert(IB % TJ == 0 && WARP_I * SUBGROUPS == IB, "block = whole tiles = one subgroup per warp");
+
+// SymPlan (the device-resident plan of one force evaluation) is declared in force_driver.cuh.
+__host__ __device__ inline long long sym_row_start(long long b, long long Km) { return b * Km - b * (b - 1) / 2; }
+
+struct BlockMeta {
+    float rmin, rmax, hmax;
+};
+template <typename Tile>
+__device__ __forceinline__ BlockMeta block_meta(const Tile* __restrict__ tiles, int b)
+{
+    BlockMeta m{__int_as_float(0x7f800000), 0.0f, 0.0f};
+#pragma unroll
+    for (int t = 0; t < TPB; ++t) {
+        const TileMeta tm = tiles[(long long)b * TPB + t].meta;
+        m.rmin = fminf(m.rmin, tm.rmin); m.rmax = fmaxf(m.rmax, tm.rmax); m.hmax = fmaxf(m.hmax, tm.hmax);
+    }
+    return m;
+}
+
+// W = max |c - b| over the block pairs that are not far.  plan->W must be 0 on entry (prep_tiles resets it).
+template <typename Tile>
+__global__ void __launch_bounds__(128) sym_band_width(const Tile* __restrict__ tiles, int nb, SymPlan* __restrict__ plan)
+{
+    const int b = blockIdx.x;
+    const BlockMeta I = block_meta(tiles, b);
+    int far_from = 0;
+    for (int c = threadIdx.x; c < nb; c += blockDim.x) {
+        const BlockMeta J = block_meta(tiles, c);
+        const TileMeta Jm{J.rmin, J.rmax, J.hmax, 0.0f};
+        if (!tile_is_far(I.rmin, I.rmax, I.hmax, Jm)) far_from = max(far_from, abs(c - b));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) far_from = max(far_from, __shfl_xor_sync(0xffffffffu, far_from, o));
+    if ((threadIdx.x & 31) == 0 && far_from > 0) atomicMax(&plan->W, far_from);
+}
+
+// One CTA: the item count and the band's cumulative tile counts from W.
+__global__ void __launch_bounds__(1024) sym_plan_finalize(SymPlan* __restrict__ plan, int nb, int sym_min_items)
+{
+    long long* cum = reinterpret_cast<long long*>(plan + 1);
+    __shared__ long long part[1024];
+    __shared__ int sW;
+    if (threadIdx.x == 0) {
+        int W = plan->W;
+        long long Km = nb - 1 - W;
+        if (Km < 0) Km = 0;
+        // too few items to balance over the SMs: everything through the band (W = nb - 1)
+        if (Km * (Km + 1) / 2 < sym_min_items) { W = nb - 1; Km = 0; }
+        plan->W = W; plan->nb = nb; plan->Km = (int)Km; plan->nt = nb * TPB; plan->K = Km * (Km + 1) / 2;
+        sW = W;
+    }
+    __syncthreads();
+    const int W = sW;
+    const int per = (nb + blockDim.x - 1) / blockDim.x;
+    const int b0 = min(nb, (int)threadIdx.x * per), b1 = min(nb, b0 + per);
+    auto width = [&](int b) { return (long long)(min(nb - 1, b + W) - max(0, b - W) + 1) * TPB; };
+    long long s = 0;
+    for (int b = b0; b < b1; ++b) s += width(b);
+    part[threadIdx.x] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        long long run = 0;
+        for (int t = 0; t < (int)blockDim.x; ++t) { const long long v = part[t]; part[t] = run; run += v; }
+        plan->T = run;
+        cum[nb] = run;
+    }
+    __syncthreads();
+    s = part[threadIdx.x];
+    for (int b = b0; b < b1; ++b) { cum[b] = s; s += width(b); }
+}
+
+constexpr int sym_smem_bytes() { return 2 * IB * (int)sizeof(FarSrcF64) + 3 * IB * (int)sizeof(double); }
+
+// Items [k_begin, k_end) of the plan's item list (one panel), shared out evenly over the grid.
+// rowrec / colrec: [k - k_begin][3][IB] doubles.
+__global__ void __launch_bounds__(CTA_THREADS, 1)
+forces_sym_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__ plan, long long k_begin, long long k_end,
+                  double* __restrict__ rowrec, double* __restrict__ colrec, int zero)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ uint64_t full_bar[2];
+    FarSrcF64* col = reinterpret_cast<FarSrcF64*>(smem_raw);                       // [2][IB]
+    double* Bsm = reinterpret_cast<double*>(smem_raw + 2 * IB * sizeof(FarSrcF64));   // [3][IB]
+
+    const long long K = plan->K;
+    if (k_end > K) k_end = K;
+    if (k_begin >= k_end) return;
+    const int W = plan->W, nb = plan->nb, Km = plan->Km;
+    const long long n_items = k_end - k_begin;
+    const long long kk0 = k_begin + (long long)blockIdx.x * n_items / gridDim.x;
+    const long long kk1 = k_begin + ((long long)blockIdx.x + 1) * n_items / gridDim.x;
+    const int total = (int)(kk1 - kk0);
+    if (total <= 0) return;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // decode the first item: row b = the largest b with sym_row_start(b) <= kk0
+    int b, c;
+    {
+        const double t = 2.0 * Km + 1.0;
+        int bb = (int)((t - sqrt(fmax(t * t - 8.0 * (double)kk0, 0.0))) * 0.5);
+        bb = max(0, min(bb, Km - 1));
+        while (bb + 1 < Km && sym_row_start(bb + 1, Km) <= kk0) ++bb;
+        while (bb > 0 && sym_row_start(bb, Km) > kk0) --bb;
+        b = bb;
+        c = bb + W + 1 + (int)(kk0 - sym_row_start(bb, Km));
+    }
+
+    if (threadIdx.x == 0) {
+        mbar_init(&full_bar[0], 1); mbar_init(&full_bar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    // producer cursor (thread 0): the column block of item `it` goes to stage it & 1 by TPB bulk copies of the tiles' far[]
+    int pb = b, pc = c;
+    auto produce = [&](int it) {
+        const int s = it & 1;
+        mbar_expect_tx(&full_bar[s], (uint32_t)(IB * sizeof(FarSrcF64)));
+#pragma unroll
+        for (int t = 0; t < TPB; ++t)
+            bulk_load(col + (size_t)s * IB + t * TJ, &tiles[(long long)pc * TPB + t].far[0], (uint32_t)(TJ * sizeof(FarSrcF64)),
+                      &full_bar[s]);
+        if (++pc == nb) { ++pb; pc = pb + W + 1; }
+    };
+    if (threadIdx.x == 0) {
+        produce(0);
+        if (total > 1) produce(1);
+    }
+
+    constexpr double A = 1.4;
+    constexpr double C0 = 1.0 / STEPS_FP64_FOLD - (1.0 - A) * (1.0 - A);
+    double xi[R_I], yi[R_I], zi[R_I], mi[R_I];
+    int cur_b = -1;
+    const int src_lane = (lane + 31) & 31;                       // reaction sums come from lane - 1
+
+    for (int it = 0; it < total; ++it) {
+        if (b != cur_b) {                                        // the row block's particles (plain copy of the tiles; pads: m = 0)
+            cur_b = b;
+#pragma unroll
+            for (int k = 0; k < R_I; ++k) {
+                const int i = warp * WARP_I + lane + 32 * k;     // within the block
+                const TileF64& T = tiles[(long long)b * TPB + i / TJ];
+                xi[k] = T.x[i % TJ]; yi[k] = T.y[i % TJ]; zi[k] = T.z[i % TJ]; mi[k] = T.m[i % TJ];
+            }
+        }
+        double ax[R_I], ay[R_I], az[R_I];
+#pragma unroll
+        for (int k = 0; k < R_I; ++k) ax[k] = ay[k] = az[k] = 0.0;
+        for (int q = threadIdx.x; q < 3 * IB; q += CTA_THREADS) Bsm[q] = 0.0;
+        const int s = it & 1;
+        mbar_wait(&full_bar[s], (it >> 1) & 1);
+        __syncthreads();
+        const FarSrcF64* cs = col + (size_t)s * IB;
+
+        for (int q = 0; q < SUBGROUPS; ++q) {
+            const int u = (warp + q) & (SUBGROUPS - 1);
+            for (int t = 0; t < WARP_I / 32; ++t) {
+                const FarSrcF64* set = cs + u * WARP_I + t * 32;
+                double bx = 0.0, by = 0.0, bz = 0.0;
+#pragma unroll 1
+                for (int st = 0; st < 32; ++st) {
+                    const FarSrcF64* src = set + ((lane - st) & 31);
+                    const double2 XY = *reinterpret_cast<const double2*>(&src->X);
+                    const double2 ZC = *reinterpret_cast<const double2*>(&src->Z);
+                    const double X = XY.x, Y = XY.y, Z = ZC.x, C = ZC.y;
+                    double dX[R_I], dY[R_I], dZ[R_I], r2[R_I], y0[R_I], y2[R_I], w[R_I];
+                    STEPS_STAGE_FENCE(zero, 0);
+#pragma unroll
+                    for (int k = 0; k < R_I; ++k) dX[k] = fma(-xi[k], C, X);
+#pragma unroll
+                    for (int k = 0; k < R_I; ++k) dY[k] = fma(-yi[k], C, Y);
+#pragma unroll
+                    for (int k = 0; k < R_I; ++k) dZ[k] = fma(-zi[k], C, Z);
+                    STEPS_STAGE_FENCE(zero, 1);
+#pragma unroll
+                    for (int k = 0; k < R_I; ++k) r2[k] = fma(dZ[k], dZ[k], fma(dY[k], dY[k], dX[k] * dX[k]));
+#pragma unroll
+                    for (int k = 0; k < R_I; ++k) y0[k] = rsqrt_seed(r2[k]);
+#pragma unroll
+                    for (int k = 0; k < R_I; ++k) {
+                        y2[k] = y0[k] * y0[k];
+                        w[k] = fma(r2[k], y2[k], -A);
+                        y2[k] = y0[k] * y2[k];
+                        w[k] = fma(w[k], w[k], C0);
+                        w[k] = y2[k] * w[k];
+                    }
+                    STEPS_STAGE_FENCE(zero, 2);
+#pragma unroll
+                    for (int k = 0; k < R_I; ++k) {
+                        const double si = mi[k] * w[k];
+                        ax[k] = fma(dX[k], w[k], ax[k]);
+                        ay[k] = fma(dY[k], w[k], ay[k]);
+                        az[k] = fma(dZ[k], w[k], az[k]);
+                        bz = fma(dZ[k], si, bz);
+                        by = fma(dY[k], si, by);
+                        bx = fma(dX[k], si, bx);
+                    }
+                    bx = __shfl_sync(0xffffffffu, bx, src_lane);
+                    by = __shfl_sync(0xffffffffu, by, src_lane);
+                    bz = __shfl_sync(0xffffffffu, bz, src_lane);
+                }
+                // 32 hand-overs later the sums of source `lane` of the set are back in this lane
+                const int j = u * WARP_I + t * 32 + lane;
+                Bsm[j] += bx; Bsm[IB + j] += by; Bsm[2 * IB + j] += bz;
+            }
+            __syncthreads();
+        }
+
+        // partial records of the item
+        const long long rec = (kk0 + it - k_begin) * 3 * IB;
+#pragma unroll
+        for (int k = 0; k < R_I; ++k) {
+            const int i = warp * WARP_I + lane + 32 * k;
+            rowrec[rec + i] = ax[k]; rowrec[rec + IB + i] = ay[k]; rowrec[rec + 2 * IB + i] = az[k];
+        }
+        for (int j = threadIdx.x; j < IB; j += CTA_THREADS) {
+            const double cj = cs[j].c;
+            const double f = -STEPS_FP64_FOLD * cj * cj;
+            colrec[rec + j] = f * Bsm[j]; colrec[rec + IB + j] = f * Bsm[IB + j]; colrec[rec + 2 * IB + j] = f * Bsm[2 * IB + j];
+        }
+        __syncthreads();                                          // stage s and Bsm are free again
+        if (threadIdx.x == 0 && it + 2 < total) produce(it + 2);
+        if (++c == nb) { ++b; c = b + W + 1; }
+    }
+}
+
+// acc (double-double, SoA over all N particles) += the records of one panel, in fixed order; `last` writes acc_out = hi + lo.
+__global__ void __launch_bounds__(256)
+forces_sym_reduce_kernel(const SymPlan* __restrict__ plan, const double* __restrict__ rowrec, const double* __restrict__ colrec,
+                         long long k_begin, long long k_end, long long N, double* __restrict__ acc_hi,
+                         double* __restrict__ acc_lo, int last, double* __restrict__ acc_out)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const long long K = plan->K;
+    if (k_end > K) k_end = K;
+    const int W = plan->W, Km = plan->Km;
+    const int b = (int)(i / IB), off = (int)(i - (long long)b * IB);
+    double hi[3], lo[3];
+#pragma unroll
+    for (int cc = 0; cc < 3; ++cc) { hi[cc] = acc_hi[cc * N + i]; lo[cc] = acc_lo[cc * N + i]; }
+    auto add = [&](const double* rec, long long k) {
+        const double* p = rec + (k - k_begin) * 3 * IB + off;
+#pragma unroll
+        for (int cc = 0; cc < 3; ++cc) {
+            const double v = p[(long long)cc * IB];
+            const double s = hi[cc] + v, bb = s - hi[cc];
+            lo[cc] += (hi[cc] - (s - bb)) + (v - bb);              // TwoSum
+            hi[cc] = s;
+        }
+    };
+    if (k_begin < k_end) {
+        if (b < Km) {                                              // this block as the row of its items
+            const long long r0 = sym_row_start(b, Km), r1 = r0 + (Km - b);
+            for (long long k = max(r0, k_begin); k < min(r1, k_end); ++k) add(rowrec, k);
+        }
+        const int rows = min(Km, b - W);                           // this block as the column of item (bb, b), bb + W < b
+        for (int bb = 0; bb < rows; ++bb) {
+            const long long k = sym_row_start(bb, Km) + (b - bb - W - 1);
+            if (k >= k_begin && k < k_end) add(colrec, k);
+        }
+    }
+#pragma unroll
+    for (int cc = 0; cc < 3; ++cc) {
+        if (last) acc_out[cc * N + i] = hi[cc] + lo[cc];
+        else { acc_hi[cc * N + i] = hi[cc]; acc_lo[cc * N + i] = lo[cc]; }
+    }
+}
+
+}  // namespace steps

@@ -26,10 +26,13 @@ __device__ __forceinline__ void block_bounds(float& rlo, float& rhi, float& hh)
     }
 }
 
+// band_width_reset (nullable): the plan's W of a pair-symmetric evaluation (force_sym.cuh), reset here for sym_band_width.
 template <typename Tile>
 __global__ void __launch_bounds__(TJ) prep_tiles(const double* __restrict__ pos, const double* __restrict__ mass,
-                                                 const double* __restrict__ soft, long long N, Tile* __restrict__ tiles)
+                                                 const double* __restrict__ soft, long long N, Tile* __restrict__ tiles,
+                                                 int* __restrict__ band_width_reset)
 {
+    if (band_width_reset != nullptr && blockIdx.x == 0 && threadIdx.x == 0) *band_width_reset = 0;
     const long long j = (long long)blockIdx.x * TJ + threadIdx.x;
     const bool real = j < N;
     const double x = real ? pos[j] : STEPS_PAD_POS;

@@ -13,6 +13,7 @@
 #include "force_mixed.cuh"
 #include "force_fp64.cuh"
 #include "force_driver.cuh"
+#include "force_sym.cuh"
 #include "kdk.cuh"
 
 using namespace steps;
@@ -31,27 +32,47 @@ constexpr int MAX_DEVICES = 16;
 constexpr int STAGES = STEPS_STAGES;   // depth of the bulk-copy ring
 constexpr int MAX_GRID = 148 * 4;
 
+// Pair-symmetric evaluation (force_sym.cuh) of the fp64 path: used for full evaluations of at least SYM_MIN_BLOCKS blocks;
+// its partial records are produced and consumed in panels of at most g_sym_panel_items items (96 KiB of records each).
+constexpr int SYM_MIN_BLOCKS = 64;
+std::atomic<long long> g_sym_panel_items{16384};
+std::atomic<int> g_sym_enabled{1};
+
 struct Workspace {
-    void* tiles = nullptr;          // max(sizeof(TileF32), sizeof(TileF64)) * ntiles
+    void* tiles = nullptr;          // max(sizeof(TileF32), sizeof(TileF64)) * ntiles (padded to whole blocks)
     double* partials = nullptr;     // (nb + grid) * 6 * IB doubles (persistent driver's split-j records)
     long long cap_particles = 0;
+    SymPlan* plan = nullptr;        // SymPlan + cum[nb + 1]
+    double* acc_dd = nullptr;       // 6 N doubles: (hi, lo) of the band result, the symmetric records are added to it
+    double* sym_records = nullptr;  // 2 * panel_items * 3 * IB doubles (row records, then column records)
+    long long sym_cap_particles = 0, sym_panel_items = 0;
     int num_sms = 0;
-    int grid_mixed = 0, grid_fp64 = 0;   // persistent grids: SMs x resident CTAs
+    int grid_mixed = 0, grid_fp64 = 0, grid_fp64_band = 0, grid_sym = 0;   // persistent grids: SMs x resident CTAs
     int grid_mixed_periodic = 0, grid_fp64_periodic = 0, grid_fp64_images = 0;
     double* mom_partial = nullptr;  // MOM_BLOCKS * 4
     // staging buffers of steps_forces_host
     double* h_pos = nullptr; double* h_mass = nullptr; double* h_soft = nullptr; double* h_acc = nullptr;
     long long h_cap = 0;
     int cc_major = -1;
-    cudaEvent_t ev0 = nullptr, ev1 = nullptr;   // "profile" option: around the last force kernel
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;   // "profile" option: around the last force kernel(s)
     bool ev_valid = false;
+    // One scratch area per device: calls on different streams are serialised through this event (see claim_scratch).
+    cudaEvent_t scratch_done = nullptr;
+    cudaStream_t scratch_stream = nullptr;
+    bool scratch_used = false;
 };
 Workspace g_ws[MAX_DEVICES];
 std::mutex g_mutex;
 
-inline long long ntiles_of(long long N) { return (N + TJ - 1) / TJ; }
 inline long long nblocks_of(long long cnt) { return (cnt + IB - 1) / IB; }
+inline long long ntiles_of(long long N) { return (N + TJ - 1) / TJ; }
+inline long long ntiles_padded(long long N) { return nblocks_of(N) * TPB; }       // whole blocks (force_sym.cuh)
 inline size_t partial_bytes(long long N) { return sizeof(double) * 6 * IB * (size_t)(nblocks_of(N) + MAX_GRID); }
+inline size_t tile_bytes_max() { return sizeof(TileF64) > sizeof(TileF32) ? sizeof(TileF64) : sizeof(TileF32); }
+inline long long sym_items_max(long long N) { const long long nb = nblocks_of(N); return nb * (nb - 1) / 2; }
+inline long long sym_panel_items_for(long long N) { return std::max(1ll, std::min(sym_items_max(N), g_sym_panel_items.load())); }
+inline size_t sym_record_bytes(long long items) { return sizeof(double) * 2 * 3 * IB * (size_t)items; }
+inline bool sym_eligible(long long N) { return g_sym_enabled.load() != 0 && nblocks_of(N) >= SYM_MIN_BLOCKS; }
 
 int cuda_fail(cudaError_t e)
 {
@@ -68,47 +89,162 @@ int current_device(int* dev)
 {
     STEPS_CUDA(cudaGetDevice(dev));
     if (*dev < 0 || *dev >= MAX_DEVICES) return STEPS_EUNSUPPORTED;
+    std::lock_guard<std::mutex> lock(g_mutex);
     Workspace& w = g_ws[*dev];
     if (w.cc_major < 0) {
         int major = 0;
         STEPS_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, *dev));
-        w.cc_major = major;
         STEPS_CUDA(cudaDeviceGetAttribute(&w.num_sms, cudaDevAttrMultiProcessorCount, *dev));
+        w.cc_major = major;
     }
     if (w.cc_major != 10) return STEPS_EUNSUPPORTED;   // sm_100a cubin only
     return STEPS_OK;
 }
 
-int ensure_workspace(int dev, long long N)
+bool stream_is_capturing(cudaStream_t st)
+{
+    cudaStreamCaptureStatus status = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &status) != cudaSuccess) { cudaGetLastError(); return false; }
+    return status != cudaStreamCaptureStatusNone;
+}
+
+// (Re)allocates the per-device scratch for N particles.  Never allocates while `st` is being captured into a CUDA graph
+// (cudaMalloc/cudaFree are not capturable): STEPS_ECAPTURE tells the caller to steps_reserve(N) before the capture.
+int ensure_workspace(int dev, long long N, cudaStream_t st)
 {
     std::lock_guard<std::mutex> lock(g_mutex);
     Workspace& w = g_ws[dev];
-    if (!w.mom_partial) {
-        if (cudaMalloc(&w.mom_partial, sizeof(double) * MOM_BLOCKS * 4) != cudaSuccess) return STEPS_ENOMEM;
+    const bool need_small = !w.mom_partial;
+    const bool need_tiles = N > w.cap_particles;
+    const bool need_sym = sym_eligible(N) && (N > w.sym_cap_particles || sym_panel_items_for(N) > w.sym_panel_items);
+    if (!need_small && !need_tiles && !need_sym) return STEPS_OK;
+    if (stream_is_capturing(st)) return STEPS_ECAPTURE;
+    if (need_small) {
+        // first use of this device: the reduction scratch and the image-sum triplet table (Eq. 5) in constant memory
+        static const EwaldTriplets table;
+        STEPS_CUDA(cudaMemcpyToSymbol(ewald_triplets, table.v, sizeof(table.v)));
+        if (cudaMalloc(&w.mom_partial, sizeof(double) * MOM_BLOCKS * 4) != cudaSuccess) { cudaGetLastError(); return STEPS_ENOMEM; }
     }
-    if (N <= w.cap_particles) return STEPS_OK;
-    if (w.tiles) { cudaFree(w.tiles); cudaFree(w.partials); w.tiles = nullptr; w.partials = nullptr; w.cap_particles = 0; }
-    const size_t tile_bytes = sizeof(TileF64) > sizeof(TileF32) ? sizeof(TileF64) : sizeof(TileF32);
-    if (cudaMalloc(&w.tiles, tile_bytes * (size_t)ntiles_of(N)) != cudaSuccess ||
-        cudaMalloc(&w.partials, partial_bytes(N)) != cudaSuccess) {
-        cudaGetLastError();
-        cudaFree(w.tiles); w.tiles = nullptr;
-        return STEPS_ENOMEM;
+    if (need_tiles || need_sym) STEPS_CUDA(cudaDeviceSynchronize());      // nothing in flight may still use the old scratch
+    if (need_tiles) {
+        cudaFree(w.tiles); cudaFree(w.partials); cudaFree(w.plan);
+        w.tiles = nullptr; w.partials = nullptr; w.plan = nullptr; w.cap_particles = 0;
+        if (cudaMalloc(&w.tiles, tile_bytes_max() * (size_t)ntiles_padded(N)) != cudaSuccess ||
+            cudaMalloc(&w.partials, partial_bytes(N)) != cudaSuccess ||
+            cudaMalloc(&w.plan, sizeof(SymPlan) + sizeof(long long) * (size_t)(nblocks_of(N) + 1)) != cudaSuccess) {
+            cudaGetLastError();
+            cudaFree(w.tiles); cudaFree(w.partials); w.tiles = nullptr; w.partials = nullptr;
+            return STEPS_ENOMEM;
+        }
+        w.cap_particles = nblocks_of(N) * IB;
     }
-    w.cap_particles = ntiles_of(N) * TJ;
+    if (need_sym) {
+        cudaFree(w.acc_dd); cudaFree(w.sym_records);
+        w.acc_dd = nullptr; w.sym_records = nullptr; w.sym_cap_particles = 0; w.sym_panel_items = 0;
+        const long long items = sym_panel_items_for(N);
+        if (cudaMalloc(&w.acc_dd, sizeof(double) * 6 * (size_t)N) != cudaSuccess ||
+            cudaMalloc(&w.sym_records, sym_record_bytes(items)) != cudaSuccess) {
+            cudaGetLastError();
+            cudaFree(w.acc_dd); w.acc_dd = nullptr;
+            return STEPS_ENOMEM;
+        }
+        w.sym_cap_particles = N; w.sym_panel_items = items;
+    }
+    return STEPS_OK;
+}
+
+// The scratch area (tiles, partial records, reduction partials, run coefficients) is ONE per device.  Calls are
+// stream-ordered on their own stream; a call on a DIFFERENT stream than the previous user first waits (on the device,
+// cudaStreamWaitEvent) for the previous user's last kernel, so concurrent streams are serialised instead of racing.
+// Streams under graph capture are left alone (events cannot cross a capture): one capturing stream per device at a time.
+int claim_scratch(Workspace& w, cudaStream_t st)
+{
+    std::lock_guard<std::mutex> lock(g_mutex);
+    if (stream_is_capturing(st)) return STEPS_OK;
+    if (!w.scratch_done) STEPS_CUDA(cudaEventCreateWithFlags(&w.scratch_done, cudaEventDisableTiming));
+    if (w.scratch_used && w.scratch_stream != st) STEPS_CUDA(cudaStreamWaitEvent(st, w.scratch_done, 0));
+    return STEPS_OK;
+}
+int release_scratch(Workspace& w, cudaStream_t st)
+{
+    std::lock_guard<std::mutex> lock(g_mutex);
+    if (stream_is_capturing(st)) return STEPS_OK;
+    STEPS_CUDA(cudaEventRecord(w.scratch_done, st));
+    w.scratch_stream = st; w.scratch_used = true;
     return STEPS_OK;
 }
 
 bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+
+template <typename Kernel>
+int persistent_grid(Kernel kern, int smem, const Workspace& w, int& grid_cache)
+{
+    if (grid_cache == 0) {
+        STEPS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        int per_sm = 0;
+        STEPS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, CTA_THREADS, smem));
+        if (per_sm < 1) return STEPS_EUNSUPPORTED;
+        const int g = w.num_sms * per_sm;
+        grid_cache = g > MAX_GRID ? MAX_GRID : g;
+    }
+    return STEPS_OK;
+}
+
+// Full fp64 evaluation, pair-symmetric (force_sym.cuh): band through the asymmetric persistent kernel, every far block
+// pair once through forces_sym_kernel, panel by panel; all decisions that depend on the data (W) are taken on the device.
+int launch_forces_sym(const double* pos, const double* mass, const double* soft, long long N, double* acc_out,
+                      cudaStream_t st, Workspace& w)
+{
+    using Path = Fp64Path;
+    const int nb = (int)nblocks_of(N);
+    const int ntp = nb * TPB;
+    TileF64* tiles = reinterpret_cast<TileF64*>(w.tiles);
+    constexpr int smem_band = persistent_smem_bytes<Path, STAGES>();
+    auto band = forces_persistent_kernel<Path, STAGES, 0, true>;
+    int rc = persistent_grid(band, smem_band, w, w.grid_fp64_band);
+    if (rc != STEPS_OK) return rc;
+    rc = persistent_grid(forces_sym_kernel, sym_smem_bytes(), w, w.grid_sym);
+    if (rc != STEPS_OK) return rc;
+    const int P = w.grid_fp64_band, Ps = w.grid_sym;
+    const bool prof = g_profile.load() != 0;
+    if (prof && !w.ev0) { STEPS_CUDA(cudaEventCreate(&w.ev0)); STEPS_CUDA(cudaEventCreate(&w.ev1)); }
+
+    prep_tiles<TileF64><<<ntp, TJ, 0, st>>>(pos, mass, soft, N, tiles, &w.plan->W);
+    sym_band_width<TileF64><<<nb, 128, 0, st>>>(tiles, nb, w.plan);
+    sym_plan_finalize<<<1, 1024, 0, st>>>(w.plan, nb, 8 * Ps);
+    if (prof) STEPS_CUDA(cudaEventRecord(w.ev0, st));
+    band<<<P, CTA_THREADS, smem_band, st>>>(pos, soft, N, tiles, ntp, 0, N, nb, w.partials, 0, 0.0, 0.0, w.plan);
+    double* hi = w.acc_dd;
+    double* lo = w.acc_dd + 3 * N;
+    forces_band_reduce_kernel<Path::NOUT><<<(int)((N + 255) / 256), 256, 0, st>>>(w.partials, w.plan, P, N, acc_out, 1, hi, lo);
+    g_launches += 5;
+    const long long items = w.sym_panel_items, kmax = sym_items_max(N);
+    double* rowrec = w.sym_records;
+    double* colrec = w.sym_records + (size_t)items * 3 * IB;
+    for (long long k0 = 0; k0 < kmax; k0 += items) {
+        const long long k1 = std::min(kmax, k0 + items);
+        forces_sym_kernel<<<Ps, CTA_THREADS, sym_smem_bytes(), st>>>(tiles, w.plan, k0, k1, rowrec, colrec, 0);
+        forces_sym_reduce_kernel<<<(int)((N + 255) / 256), 256, 0, st>>>(w.plan, rowrec, colrec, k0, k1, N, hi, lo,
+                                                                          k1 == kmax ? 1 : 0, acc_out);
+        g_launches += 2;
+    }
+    if (prof) { STEPS_CUDA(cudaEventRecord(w.ev1, st)); w.ev_valid = true; }
+    STEPS_CUDA(cudaGetLastError());
+    return STEPS_OK;
+}
 
 template <typename Path>
 int launch_forces(const double* pos, const double* mass, const double* soft, long long N, long long i_begin,
                   long long i_end, double* acc_out, cudaStream_t st, Workspace& w, int& grid_cache)
 {
     using Tile = typename Path::Tile;
+    if constexpr (Path::NOUT == 6) {
+        if (i_begin == 0 && i_end == N && g_driver.load() == 0 && sym_eligible(N) && w.sym_records)
+            return launch_forces_sym(pos, mass, soft, N, acc_out, st, w);
+    }
     const int nt = (int)ntiles_of(N);
     Tile* tiles = reinterpret_cast<Tile*>(w.tiles);
-    prep_tiles<Tile><<<nt, TJ, 0, st>>>(pos, mass, soft, N, tiles);
+    prep_tiles<Tile><<<nt, TJ, 0, st>>>(pos, mass, soft, N, tiles, nullptr);
     g_launches++;
     const long long cnt = i_end - i_begin;
     const int nb = (int)nblocks_of(cnt);
@@ -120,21 +256,15 @@ int launch_forces(const double* pos, const double* mass, const double* soft, lon
     } else {
         constexpr int smem = persistent_smem_bytes<Path, STAGES>();
         auto kern = forces_persistent_kernel<Path, STAGES>;
-        if (grid_cache == 0) {
-            STEPS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-            int per_sm = 0;
-            STEPS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, CTA_THREADS, smem));
-            if (per_sm < 1) return STEPS_EUNSUPPORTED;
-            int g = w.num_sms * per_sm;
-            grid_cache = g > MAX_GRID ? MAX_GRID : g;
-        }
+        const int rc = persistent_grid(kern, smem, w, grid_cache);
+        if (rc != STEPS_OK) return rc;
         const int P = grid_cache;
         const bool prof = g_profile.load() != 0;
         if (prof) {
             if (!w.ev0) { STEPS_CUDA(cudaEventCreate(&w.ev0)); STEPS_CUDA(cudaEventCreate(&w.ev1)); }
             STEPS_CUDA(cudaEventRecord(w.ev0, st));
         }
-        kern<<<P, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, i_begin, i_end, nb, w.partials, 0, 0.0, 0.0);
+        kern<<<P, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, i_begin, i_end, nb, w.partials, 0, 0.0, 0.0, nullptr);
         if (prof) { STEPS_CUDA(cudaEventRecord(w.ev1, st)); w.ev_valid = true; }
         forces_reduce_kernel<Path::NOUT><<<(int)((cnt + 255) / 256), 256, 0, st>>>(w.partials, nt, nb, P, cnt, acc_out);
         g_launches += 2;
@@ -148,17 +278,21 @@ int forces_impl(const double* pos, const double* mass, const double* soft, long 
 {
     if (!pos || !mass || !soft || !acc_out || N < 1) return STEPS_EINVAL;
     if (i_begin < 0 || i_end > N || i_begin >= i_end) return STEPS_EINVAL;
-    if (N > (1ll << 31) - TJ) return STEPS_EINVAL;
+    if (N > (1ll << 31) - IB) return STEPS_EINVAL;
     if (misaligned(pos) || misaligned(mass) || misaligned(soft) || misaligned(acc_out)) return STEPS_EINVAL;
     int dev;
     int rc = current_device(&dev);
     if (rc != STEPS_OK) return rc;
-    rc = ensure_workspace(dev, N);
-    if (rc != STEPS_OK) return rc;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    rc = ensure_workspace(dev, N, st);
+    if (rc != STEPS_OK) return rc;
     Workspace& w = g_ws[dev];
-    return mixed ? launch_forces<MixedPath>(pos, mass, soft, N, i_begin, i_end, acc_out, st, w, w.grid_mixed)
-                 : launch_forces<Fp64Path>(pos, mass, soft, N, i_begin, i_end, acc_out, st, w, w.grid_fp64);
+    rc = claim_scratch(w, st);
+    if (rc != STEPS_OK) return rc;
+    rc = mixed ? launch_forces<MixedPath>(pos, mass, soft, N, i_begin, i_end, acc_out, st, w, w.grid_mixed)
+               : launch_forces<Fp64Path>(pos, mass, soft, N, i_begin, i_end, acc_out, st, w, w.grid_fp64);
+    if (rc != STEPS_OK) return rc;
+    return release_scratch(w, st);
 }
 
 template <typename Path, int BOX>
@@ -168,24 +302,20 @@ int launch_forces_periodic(const double* pos, const double* mass, const double* 
     using Tile = typename Path::Tile;
     const int nt = (int)ntiles_of(N);
     Tile* tiles = reinterpret_cast<Tile*>(w.tiles);
-    prep_tiles<Tile><<<nt, TJ, 0, st>>>(pos, mass, soft, N, tiles);
+    int rc = claim_scratch(w, st);
+    if (rc != STEPS_OK) return rc;
+    prep_tiles<Tile><<<nt, TJ, 0, st>>>(pos, mass, soft, N, tiles, nullptr);
     const int nb = (int)nblocks_of(N);
     constexpr int smem = persistent_smem_bytes<Path, STAGES>();
     auto kern = forces_persistent_kernel<Path, STAGES, BOX>;
-    if (grid_cache == 0) {
-        STEPS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        int per_sm = 0;
-        STEPS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, CTA_THREADS, smem));
-        if (per_sm < 1) return STEPS_EUNSUPPORTED;
-        const int g = w.num_sms * per_sm;
-        grid_cache = g > MAX_GRID ? MAX_GRID : g;
-    }
+    rc = persistent_grid(kern, smem, w, grid_cache);
+    if (rc != STEPS_OK) return rc;
     const int P = grid_cache;
-    kern<<<P, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, 0, N, nb, w.partials, 0, L, 1.0 / L);
+    kern<<<P, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, 0, N, nb, w.partials, 0, L, 1.0 / L, nullptr);
     forces_reduce_kernel<Path::NOUT><<<(int)((N + 255) / 256), 256, 0, st>>>(w.partials, nt, nb, P, N, acc_out);
     g_launches += 3;
     STEPS_CUDA(cudaGetLastError());
-    return STEPS_OK;
+    return release_scratch(w, st);
 }
 
 }  // namespace
@@ -196,12 +326,12 @@ int steps_forces_quasi_periodic(const double* pos, const double* mass, const dou
                                 double* acc, int mixed, steps_stream_t stream)
 {
     if (!pos || !mass || !soft || !acc || N < 1 || !(L > 0.0)) return STEPS_EINVAL;
-    if (N > (1ll << 31) - TJ) return STEPS_EINVAL;
+    if (N > (1ll << 31) - IB) return STEPS_EINVAL;
     if (misaligned(pos) || misaligned(mass) || misaligned(soft) || misaligned(acc)) return STEPS_EINVAL;
     int dev;
     int rc = current_device(&dev);
     if (rc != STEPS_OK) return rc;
-    rc = ensure_workspace(dev, N);
+    rc = ensure_workspace(dev, N, reinterpret_cast<cudaStream_t>(stream));
     if (rc != STEPS_OK) return rc;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     Workspace& w = g_ws[dev];
@@ -213,22 +343,14 @@ int steps_forces_periodic(const double* pos, const double* mass, const double* s
                           steps_stream_t stream)
 {
     if (!pos || !mass || !soft || !acc || N < 1 || !(L > 0.0)) return STEPS_EINVAL;
-    if (N > (1ll << 31) - TJ) return STEPS_EINVAL;
+    if (N > (1ll << 31) - IB) return STEPS_EINVAL;
     if (misaligned(pos) || misaligned(mass) || misaligned(soft) || misaligned(acc)) return STEPS_EINVAL;
     int dev;
     int rc = current_device(&dev);
     if (rc != STEPS_OK) return rc;
-    rc = ensure_workspace(dev, N);
+    rc = ensure_workspace(dev, N, reinterpret_cast<cudaStream_t>(stream));
     if (rc != STEPS_OK) return rc;
     Workspace& w = g_ws[dev];
-    if (w.grid_fp64_images == 0) {                       // first use on this device: upload the triplet table
-        static const EwaldTriplets table;
-        int count = 0;
-        for (int c = 0; c < EWALD_NTRIPLETS; ++c) count += (table.v[c].x * table.v[c].x + table.v[c].y * table.v[c].y +
-                                                             table.v[c].z * table.v[c].z <= 12.0);
-        if (count != EWALD_NTRIPLETS) return STEPS_EUNSUPPORTED;
-        STEPS_CUDA(cudaMemcpyToSymbol(ewald_triplets, table.v, sizeof(table.v)));
-    }
     return launch_forces_periodic<Fp64Path, 2>(pos, mass, soft, N, L, acc, reinterpret_cast<cudaStream_t>(stream), w,
                                                w.grid_fp64_images);
 }
@@ -322,9 +444,11 @@ int steps_kdk_step_adaptive(double* pos, double* vel, double* acc, const double*
     int dev;
     int rc = current_device(&dev);
     if (rc != STEPS_OK) return rc;
-    rc = ensure_workspace(dev, N);
+    rc = ensure_workspace(dev, N, reinterpret_cast<cudaStream_t>(stream));
     if (rc != STEPS_OK) return rc;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    rc = claim_scratch(g_ws[dev], st);                      // released by the force evaluation at the end of this call
+    if (rc != STEPS_OK) return rc;
     double* partial = g_ws[dev].mom_partial;
     double* coef6 = partial + 2 * MOM_BLOCKS;
     RunState* rs = reinterpret_cast<RunState*>(state5);
@@ -347,9 +471,11 @@ int steps_kick_close_adaptive(double* pos, double* vel, const double* acc, long 
     int dev;
     int rc = current_device(&dev);
     if (rc != STEPS_OK) return rc;
-    rc = ensure_workspace(dev, 1);
+    rc = ensure_workspace(dev, 1, reinterpret_cast<cudaStream_t>(stream));
     if (rc != STEPS_OK) return rc;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    rc = claim_scratch(g_ws[dev], st);
+    if (rc != STEPS_OK) return rc;
     double* coef6 = g_ws[dev].mom_partial + 2 * MOM_BLOCKS;
     close_coefficients_kernel<<<1, 32, 0, st>>>(reinterpret_cast<RunState*>(state5), B, coef6);
     const long long M = 3 * N;
@@ -358,7 +484,7 @@ int steps_kick_close_adaptive(double* pos, double* vel, const double* acc, long 
     kick_drift_dev_kernel<<<(int)blocks, 256, 0, st>>>(pos, vel, acc, M, coef6);
     g_launches += 2;
     STEPS_CUDA(cudaGetLastError());
-    return STEPS_OK;
+    return release_scratch(g_ws[dev], st);
 }
 
 double steps_hubble(double a, const steps_cosmology* c)
@@ -396,14 +522,16 @@ int steps_momentum(const double* vec, const double* mass, long long N, double* o
     int dev;
     int rc = current_device(&dev);
     if (rc != STEPS_OK) return rc;
-    rc = ensure_workspace(dev, 1);
+    rc = ensure_workspace(dev, 1, reinterpret_cast<cudaStream_t>(stream));
     if (rc != STEPS_OK) return rc;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    rc = claim_scratch(g_ws[dev], st);
+    if (rc != STEPS_OK) return rc;
     momentum_stage1<<<MOM_BLOCKS, 256, 0, st>>>(vec, mass, N, g_ws[dev].mom_partial);
     momentum_stage2<<<1, 32, 0, st>>>(g_ws[dev].mom_partial, MOM_BLOCKS, out4);
     g_launches += 2;
     STEPS_CUDA(cudaGetLastError());
-    return STEPS_OK;
+    return release_scratch(g_ws[dev], st);
 }
 
 int steps_timestep(const double* pos, const double* acc, const double* soft, long long N, double coef, double B,
@@ -414,14 +542,16 @@ int steps_timestep(const double* pos, const double* acc, const double* soft, lon
     int dev;
     int rc = current_device(&dev);
     if (rc != STEPS_OK) return rc;
-    rc = ensure_workspace(dev, 1);
+    rc = ensure_workspace(dev, 1, reinterpret_cast<cudaStream_t>(stream));
     if (rc != STEPS_OK) return rc;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    rc = claim_scratch(g_ws[dev], st);
+    if (rc != STEPS_OK) return rc;
     timestep_stage1<<<MOM_BLOCKS, 256, 0, st>>>(pos, acc, soft, N, coef, B, eps, dt_max, g_ws[dev].mom_partial);
     timestep_stage2<<<1, 32, 0, st>>>(g_ws[dev].mom_partial, MOM_BLOCKS, dt_out);
     g_launches += 2;
     STEPS_CUDA(cudaGetLastError());
-    return STEPS_OK;
+    return release_scratch(g_ws[dev], st);
 }
 
 int steps_force_residual(const double* pos, const double* acc, long long N, double B, double* out2, steps_stream_t stream)
@@ -430,14 +560,16 @@ int steps_force_residual(const double* pos, const double* acc, long long N, doub
     int dev;
     int rc = current_device(&dev);
     if (rc != STEPS_OK) return rc;
-    rc = ensure_workspace(dev, 1);
+    rc = ensure_workspace(dev, 1, reinterpret_cast<cudaStream_t>(stream));
     if (rc != STEPS_OK) return rc;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    rc = claim_scratch(g_ws[dev], st);
+    if (rc != STEPS_OK) return rc;
     residual_stage1<<<MOM_BLOCKS, 256, 0, st>>>(pos, acc, N, B, g_ws[dev].mom_partial);
     residual_stage2<<<1, 32, 0, st>>>(g_ws[dev].mom_partial, MOM_BLOCKS, out2);
     g_launches += 2;
     STEPS_CUDA(cudaGetLastError());
-    return STEPS_OK;
+    return release_scratch(g_ws[dev], st);
 }
 
 int steps_reserve(long long N)
@@ -446,7 +578,7 @@ int steps_reserve(long long N)
     int dev;
     int rc = current_device(&dev);
     if (rc != STEPS_OK) return rc;
-    return ensure_workspace(dev, N);
+    return ensure_workspace(dev, N, nullptr);
 }
 
 void steps_shutdown(void)
@@ -458,9 +590,12 @@ void steps_shutdown(void)
         Workspace& w = g_ws[d];
         if (!w.tiles && !w.mom_partial && !w.h_pos) continue;
         cudaSetDevice(d);
-        cudaFree(w.tiles); cudaFree(w.partials); cudaFree(w.mom_partial);
+        cudaDeviceSynchronize();
+        cudaFree(w.tiles); cudaFree(w.partials); cudaFree(w.plan); cudaFree(w.acc_dd); cudaFree(w.sym_records);
+        cudaFree(w.mom_partial);
         cudaFree(w.h_pos); cudaFree(w.h_mass); cudaFree(w.h_soft); cudaFree(w.h_acc);
         if (w.ev0) { cudaEventDestroy(w.ev0); cudaEventDestroy(w.ev1); }
+        if (w.scratch_done) cudaEventDestroy(w.scratch_done);
         w = Workspace();
     }
     cudaSetDevice(cur);
@@ -469,8 +604,10 @@ void steps_shutdown(void)
 long long steps_workspace_bytes(long long N)
 {
     if (N < 1) return 0;
-    const size_t tile_bytes = sizeof(TileF64) > sizeof(TileF32) ? sizeof(TileF64) : sizeof(TileF32);
-    return (long long)(tile_bytes * (size_t)ntiles_of(N) + partial_bytes(N) + sizeof(double) * MOM_BLOCKS * 4);
+    size_t bytes = tile_bytes_max() * (size_t)ntiles_padded(N) + partial_bytes(N) + sizeof(double) * MOM_BLOCKS * 4 +
+                   sizeof(SymPlan) + sizeof(long long) * (size_t)(nblocks_of(N) + 1);
+    if (sym_eligible(N)) bytes += sizeof(double) * 6 * (size_t)N + sym_record_bytes(sym_panel_items_for(N));
+    return (long long)bytes;
 }
 
 const char* steps_strerror(int code)
@@ -481,6 +618,7 @@ const char* steps_strerror(int code)
         case STEPS_ECUDA: return "CUDA runtime error (see steps_last_cuda_error)";
         case STEPS_EUNSUPPORTED: return "device is not compute capability 10.x (sm_100a build, no fallback)";
         case STEPS_ENOMEM: return "workspace allocation failed";
+        case STEPS_ECAPTURE: return "workspace must be allocated (steps_reserve) before the stream is captured into a CUDA graph";
         default: return "unknown error code";
     }
 }
@@ -494,6 +632,12 @@ int steps_set_option(const char* key, long long value)
     if (!key) return STEPS_EINVAL;
     if (std::strcmp(key, "driver") == 0) { g_driver = (int)value; return STEPS_OK; }
     if (std::strcmp(key, "profile") == 0) { g_profile = (int)value; return STEPS_OK; }
+    if (std::strcmp(key, "sym") == 0) { g_sym_enabled = value != 0; return STEPS_OK; }
+    if (std::strcmp(key, "sym_panel_items") == 0) {
+        if (value < 1) return STEPS_EINVAL;
+        g_sym_panel_items = value;
+        return STEPS_OK;
+    }
     return STEPS_EINVAL;
 }
 

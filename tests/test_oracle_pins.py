@@ -310,6 +310,21 @@ def test_growth_rate_limits(oracle):
     assert oracle.growth_rate(1.0, LCDM) == pytest.approx(0.3 ** 0.55, abs=5e-3)    # textbook fit
 
 
+def test_growth_rate_flat_lcdm_closed_form(oracle):
+    """Flat LCDM (Omega_r = Omega_k = 0): the growing mode of PAPER.md Eq. 19 (L255) has the closed form
+    D(a) ~ a 2F1(1/3, 1; 11/6; x), x = -a^3 Omega_L/Omega_m, hence
+    f = dlnD/dlna = 1 + 3 x F'(x)/F(x) with F' = (1/3 * 1 / (11/6)) 2F1(4/3, 2; 17/6; x).
+    scipy's hypergeometric routine is independent of the oracle's quadrature of Eq. 19 (a wrong power of a'H, a wrong
+    dlnH/dlna term or a sloppy quadrature fails at 1e-7).  f sets the initial velocities of config 4."""
+    from scipy.special import hyp2f1
+    for a in (1 / 51, 0.1, 0.3, 0.6, 1.0):
+        x = -a ** 3 * LCDM["Omega_L"] / LCDM["Omega_m"]
+        F = hyp2f1(1 / 3, 1.0, 11 / 6, x)
+        dF = (1 / 3) / (11 / 6) * hyp2f1(4 / 3, 2.0, 17 / 6, x)
+        f = 1.0 + 3.0 * x * dF / F
+        assert oracle.growth_rate(a, LCDM) == pytest.approx(f, rel=2e-7), a
+
+
 # ------------------------------------------------------------------ KDK integrator (Eq. 8-11)
 
 def _one_particle(x0, v0):
@@ -417,6 +432,27 @@ def test_kdk_coefficient_form_equals_literal_step(oracle):
     np.testing.assert_allclose(vel, v2, rtol=1e-12, atol=1e-18)
     p = oracle.momentum(vel, ps.mass)
     assert np.linalg.norm(p[:3]) / p[3] < 1e-12
+
+
+# ---- diagnostics: P = sum m v, sum m |v| -----------------------------------------------------
+def test_momentum_hand_values_and_brute_force(oracle):
+    """Three particles with hand-typed values: m = (1, 2, 4), v_1 = (3, 4, 0), v_2 = (0, -6, 8), v_3 = (-2, 1, 2),
+    |v| = (5, 10, 3):  sum m v = (3 - 8, 4 - 12 + 4, 16 + 8) = (-5, -4, 24),  sum m |v| = 5 + 20 + 12 = 37.
+    All four outputs differ, the components differ from each other, and sum m v^2 = 261 != 37, so a swapped index,
+    a missing square root or a missing mass fails.  Then a numpy-longdouble brute force on random data."""
+    vel = np.array([[3.0, 0.0, -2.0], [4.0, -6.0, 1.0], [0.0, 8.0, 2.0]])
+    mass = np.array([1.0, 2.0, 4.0])
+    np.testing.assert_array_equal(oracle.momentum(vel, mass), [-5.0, -4.0, 24.0, 37.0])
+    rng = np.random.default_rng(7)
+    n = 1000
+    vel = rng.normal(size=(3, n)) * np.array([[1.0], [10.0], [100.0]])
+    mass = rng.uniform(0.1, 5.0, size=n) * 10.0 ** rng.integers(-6, 3, size=n)
+    vl, ml = vel.astype(np.longdouble), mass.astype(np.longdouble)
+    want = np.array([*(ml * vl).sum(axis=1), (ml * np.sqrt((vl * vl).sum(axis=0))).sum()], dtype=np.longdouble)
+    got = oracle.momentum(vel, mass)
+    scale = (ml * np.abs(vl)).sum(axis=1)
+    assert np.all(np.abs(got[:3] - want[:3]) <= 4e-16 * scale)          # compensated: error ~ 1 ulp of sum |m v|
+    assert abs(got[3] - want[3]) <= 4e-16 * want[3]
 
 
 # ---- Eq. 12 (L113-116): adaptive global time step --------------------------------------------------------------
