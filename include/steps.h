@@ -27,8 +27,16 @@
  *     paper's h_i (Eq. 7, support radius of the spline), NOT a Plummer epsilon.
  *   - Calls are stream-ordered on `stream` (a cudaStream_t; NULL = legacy default stream)
  *     and never synchronise the host, except that the FIRST call for a larger N than any
- *     seen before on this device (re)allocates the internal workspace with cudaMalloc.
- *     steps_reserve(N) does that allocation up front; steps_shutdown() frees it.
+ *     seen before on this device (re)allocates the internal workspace (cudaDeviceSynchronize +
+ *     cudaMalloc).  steps_reserve(N) does that allocation up front; steps_shutdown() frees it.
+ *   - The workspace (tile records, partial records, reduction scratch) is ONE per device.  Calls
+ *     on different streams of one device are therefore SERIALISED, not concurrent: a call on
+ *     another stream than the previous one first waits on the device (cudaStreamWaitEvent) for
+ *     the previous call's last kernel.  Host threads may call concurrently (internal mutex).
+ *   - CUDA graphs: every call can be captured provided the workspace exists already; a call that
+ *     would have to allocate while `stream` is being captured returns STEPS_ECAPTURE and launches
+ *     nothing.  The cross-stream serialisation above does not reach into a capture: use one
+ *     capturing stream per device at a time.
  *   - Results do not depend on particle order beyond rounding.  Radially sorted input
  *     (|x| ascending) is the fast path: the kernels classify (i-group, j-tile) pairs by
  *     their radial intervals into "far" (no pair can have r < h_i + h_j; branch-free
@@ -37,7 +45,10 @@
  *   - Return value: STEPS_OK (0) or a negative error code; steps_strerror() gives text.
  *     Nothing throws or aborts.  N = 1 is valid (acc = 0).  Non-finite inputs give
  *     non-finite outputs, not an error.  Numerical domain of the fast (far) bodies:
- *     pair separations must satisfy 2^-63 < r < 2^63 (r^2 is seeded through fp32).
+ *     pair separations must satisfy 2^-63 < r < 2^63 (r^2 is seeded through fp32), and the
+ *     mixed path, which works on r / sqrt(m_j) in fp32, needs 1e-12 < r / sqrt(m_j) < 1e18
+ *     for every far pair (sources that cannot guarantee it from their own softening and
+ *     coordinates are routed through the slower exact body).
  *   - The device must be compute capability 10.x (sm_100a cubin only; no PTX fallback,
  *     no CPU fallback): otherwise STEPS_EUNSUPPORTED.
  */
@@ -64,7 +75,13 @@ enum {
 
 /* fp64 path: every pair in fp64 (the reciprocal square root is seeded by the fp32 SFU and
  * refined in fp64).  Bar: max_i |acc_i - oracle_i| / |oracle_i| <= 1e-12.
- * Overwrites acc[0..3N).  pos/mass/soft are read only. */
+ * Overwrites acc[0..3N).  pos/mass/soft are read only.
+ * From N = 131,072 (64 blocks of 2,048 particles) the evaluation is PAIR-SYMMETRIC: every block pair whose radial
+ * intervals are further apart than the largest pair softening is evaluated once and applied to both blocks (Newton's
+ * third law; PAPER.md L131 counts the cost as N(N-1)/2 pair evaluations), the band of block pairs around the diagonal
+ * goes through the one-sided kernel.  The split is decided on the device from the data; unsorted input, massless
+ * particles or too few blocks fall back to the one-sided kernel for everything.  Results are bit-reproducible either way.
+ * The symmetric part needs 48 B per particle + up to 1.5 GiB of partial records (steps_workspace_bytes). */
 int steps_forces(const double *pos, const double *mass, const double *soft, long long N,
                  double *acc, steps_stream_t stream);
 
@@ -164,6 +181,9 @@ int steps_forces_periodic(const double *pos, const double *mass, const double *s
  * result does not depend on the reduction order.  STEPS_EINVAL for null pointers, N < 1, eps <= 0 or dt_max <= 0. */
 int steps_timestep(const double *pos, const double *acc, const double *soft, long long N, double coef,
                    double B, double eps, double dt_max, double *dt_out, steps_stream_t stream);
+/* Host scalar: the `coef` of steps_timestep at scale factor a, |G| a^-3 (Eq. 8 L88 with reading #6; |G| because the
+ * reversed gravity of glass generation, G < 0, changes the direction of A_i, not its size). */
+double steps_timestep_coefficient(double G, double a);
 
 /* Device-resident adaptive stepping (second half): one KDK step whose length is Eq. 12 and whose
  * coefficients (Eq. 1 / RK4 of L127 / readings #8-#9, the arithmetic of steps_kdk_schedule) are computed ON THE DEVICE,
@@ -200,11 +220,14 @@ int steps_version(void);                 /* major*10000 + minor*100 + patch */
 long long steps_kernel_launch_count(void);
 /* Tuning / testing knobs.  "driver": 0 = default force driver (persistent, bulk-TMA), 1 = the
  * simple one-CTA-per-i-block driver kept as an in-library cross-check.  "profile": 1 = bracket
- * the force kernel of every later call with CUDA events recorded on the call's stream.
- * Unknown key: STEPS_EINVAL. */
+ * the force kernel(s) of every later call with CUDA events recorded on the call's stream.
+ * "sym": 0 = never use the pair-symmetric evaluation (default 1).  "sym_panel_items": how many
+ * block-pair items (96 KiB of partial records each) the symmetric evaluation keeps in flight
+ * (default 16384 = 1.5 GiB; the items are run in panels of this size).  Unknown key: STEPS_EINVAL. */
 int steps_set_option(const char *key, long long value);
 /* With "profile" on: device time in ms of the most recent force kernel launched on the current
- * device (waits for it to finish); -1 if none was recorded. */
+ * device (waits for it to finish); -1 if none was recorded.  For a pair-symmetric evaluation: from the
+ * start of the band kernel to the end of the last panel's reduce (all force kernels of the evaluation). */
 double steps_last_force_kernel_ms(void);
 /* Grid (CTA count) of the persistent force kernel on the current device: SMs x resident CTAs;
  * 0 before the first call of that path. */

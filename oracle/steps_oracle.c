@@ -101,11 +101,13 @@ void oracle_forces(const double *pos, const double *mass, const double *soft, lo
  * (x_c / L) (nearbyint under the default rounding mode), so a component of exactly L/2 keeps its sign; otherwise as
  * oracle_forces above (pair softening h_i + h_j, j = i skipped, r = 0 adds 0, G = 1, compensated sums). */
 void oracle_forces_quasi_periodic(const double *pos, const double *mass, const double *soft, long long N, double L,
-                                  double *acc)
+                                  const long long *idx, long long n_idx, double *acc)
 {
     const double *x = pos, *y = pos + N, *z = pos + 2 * N;
+    const long long count = idx ? n_idx : N;               /* idx: the particles to evaluate, as in oracle_forces */
 #pragma omp parallel for schedule(dynamic, 16)
-    for (long long i = 0; i < N; ++i) {
+    for (long long k = 0; k < count; ++k) {
+        const long long i = idx ? idx[k] : k;
         double sx = 0, sy = 0, sz = 0, cx = 0, cy = 0, cz = 0;
         for (long long j = 0; j < N; ++j) {
             if (j == i) continue;
@@ -121,9 +123,9 @@ void oracle_forces_quasi_periodic(const double *pos, const double *mass, const d
             neumaier_add(&sy, &cy, f * (dy / r));
             neumaier_add(&sz, &cz, f * (dz / r));
         }
-        acc[i] = sx + cx;
-        acc[N + i] = sy + cy;
-        acc[2 * N + i] = sz + cz;
+        acc[k] = sx + cx;
+        acc[count + k] = sy + cy;
+        acc[2 * count + k] = sz + cz;
     }
 }
 
@@ -134,12 +136,14 @@ void oracle_forces_quasi_periodic(const double *pos, const double *mass, const d
  * the nearest image, which contains every n with |x - nL| < 2.6 L; strict inequality as printed; the pair law with pair
  * softening h_i + h_j is applied to every image.  Plain loops, compensated sums. */
 void oracle_forces_periodic_images(const double *pos, const double *mass, const double *soft, long long N, double L,
-                                   double *acc)
+                                   const long long *idx, long long n_idx, double *acc)
 {
     const double *x = pos, *y = pos + N, *z = pos + 2 * N;
     const double cut = 2.6 * L;
+    const long long count = idx ? n_idx : N;               /* idx: the particles to evaluate, as in oracle_forces */
 #pragma omp parallel for schedule(dynamic, 4)
-    for (long long i = 0; i < N; ++i) {
+    for (long long k = 0; k < count; ++k) {
+        const long long i = idx ? idx[k] : k;
         double sx = 0, sy = 0, sz = 0, cx = 0, cy = 0, cz = 0;
         for (long long j = 0; j < N; ++j) {
             if (j == i) continue;
@@ -158,9 +162,9 @@ void oracle_forces_periodic_images(const double *pos, const double *mass, const 
                         neumaier_add(&sz, &cz, f * (dz / r));
                     }
         }
-        acc[i] = sx + cx;
-        acc[N + i] = sy + cy;
-        acc[2 * N + i] = sz + cz;
+        acc[k] = sx + cx;
+        acc[count + k] = sy + cy;
+        acc[2 * count + k] = sz + cz;
     }
 }
 

@@ -38,9 +38,9 @@ def lib():
         L.oracle_forces.restype = None
         L.oracle_forces.argtypes = [dp, dp, dp, C.c_longlong, llp, C.c_longlong, dp, C.c_int]
         L.oracle_forces_quasi_periodic.restype = None
-        L.oracle_forces_quasi_periodic.argtypes = [dp, dp, dp, C.c_longlong, C.c_double, dp]
+        L.oracle_forces_quasi_periodic.argtypes = [dp, dp, dp, C.c_longlong, C.c_double, llp, C.c_longlong, dp]
         L.oracle_forces_periodic_images.restype = None
-        L.oracle_forces_periodic_images.argtypes = [dp, dp, dp, C.c_longlong, C.c_double, dp]
+        L.oracle_forces_periodic_images.argtypes = [dp, dp, dp, C.c_longlong, C.c_double, llp, C.c_longlong, dp]
         L.oracle_hubble.restype = C.c_double
         L.oracle_hubble.argtypes = [C.c_double, C.POINTER(Cosmo)]
         L.oracle_rk4_scale_factor.restype = C.c_double
@@ -93,24 +93,31 @@ def forces(pos, mass, soft, idx=None, reverse_j: bool = False) -> np.ndarray:
     return acc
 
 
-def forces_quasi_periodic(pos, mass, soft, L: float) -> np.ndarray:
-    """Eq. 5 (L65-70) leading term only: nearest-image pair forces in a cubic box of side L; acc (3, N), G = 1."""
+def _periodic(fn, pos, mass, soft, L, idx):
     pos, mass, soft = _f64(pos), _f64(mass), _f64(soft)
     n = mass.shape[0]
     assert pos.shape == (3, n) and soft.shape == (n,)
-    acc = np.empty((3, n))
-    lib().oracle_forces_quasi_periodic(_dp(pos), _dp(mass), _dp(soft), n, float(L), _dp(acc))
+    if idx is None:
+        acc = np.empty((3, n))
+        fn(_dp(pos), _dp(mass), _dp(soft), n, float(L), None, 0, _dp(acc))
+    else:
+        idx = np.ascontiguousarray(idx, dtype=np.int64)
+        assert idx.ndim == 1 and (idx >= 0).all() and (idx < n).all()
+        acc = np.empty((3, idx.shape[0]))
+        fn(_dp(pos), _dp(mass), _dp(soft), n, float(L), idx.ctypes.data_as(C.POINTER(C.c_longlong)), idx.shape[0], _dp(acc))
     return acc
 
 
-def forces_periodic_images(pos, mass, soft, L: float) -> np.ndarray:
-    """Eq. 5 (L65-70) with the paper's cut |x - nL| < 2.6 L over the periodic images; acc (3, N), G = 1."""
-    pos, mass, soft = _f64(pos), _f64(mass), _f64(soft)
-    n = mass.shape[0]
-    assert pos.shape == (3, n) and soft.shape == (n,)
-    acc = np.empty((3, n))
-    lib().oracle_forces_periodic_images(_dp(pos), _dp(mass), _dp(soft), n, float(L), _dp(acc))
-    return acc
+def forces_quasi_periodic(pos, mass, soft, L: float, idx=None) -> np.ndarray:
+    """Eq. 5 (L65-70) leading term only: nearest-image pair forces in a cubic box of side L; acc (3, N), G = 1.
+    idx: evaluate only these particles (against all N sources); acc is then (3, len(idx))."""
+    return _periodic(lib().oracle_forces_quasi_periodic, pos, mass, soft, L, idx)
+
+
+def forces_periodic_images(pos, mass, soft, L: float, idx=None) -> np.ndarray:
+    """Eq. 5 (L65-70) with the paper's cut |x - nL| < 2.6 L over the periodic images; acc (3, N), G = 1.
+    idx: evaluate only these particles (against all N sources); acc is then (3, len(idx))."""
+    return _periodic(lib().oracle_forces_periodic_images, pos, mass, soft, L, idx)
 
 
 def hubble(a: float, cosmo: dict) -> float:

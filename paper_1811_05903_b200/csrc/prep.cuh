@@ -53,6 +53,9 @@ __global__ void __launch_bounds__(TJ) prep_tiles(const double* __restrict__ pos,
         const float c32 = scaled_ok ? (float)(1.0 / sqrt(m)) : STEPS_PAD_C32;
         const double lim = 1.0e18, c = (double)c32;
         scaled_ok = scaled_ok && c < lim && fabs(x * c) < lim && fabs(y * c) < lim && fabs(z * c) < lim;
+        // lower end: the far body works on c r = r / sqrt(m_j) in fp32 and y^3 = (c r)^-3 must stay finite.  A far pair has
+        // r >= h_i + h_j >= h_j, so c h_j bounds c r from below (h_j = 0: the documented domain of steps.h applies).
+        scaled_ok = scaled_ok && !(h > 0.0 && c * h < 1.0e-12);
         T.c[t ^ STEPS_C_SWIZZLE] = scaled_ok ? c32 : STEPS_PAD_C32;   // see STEPS_C_SWIZZLE in common.cuh
         T.X[t] = scaled_ok ? (float)(x * c) : STEPS_PAD_X32;
         T.Y[t] = scaled_ok ? (float)(y * c) : STEPS_PAD_X32;

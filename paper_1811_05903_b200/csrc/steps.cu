@@ -554,6 +554,8 @@ int steps_timestep(const double* pos, const double* acc, const double* soft, lon
     return release_scratch(g_ws[dev], st);
 }
 
+double steps_timestep_coefficient(double G, double a) { return std::fabs(G) / (a * a * a); }
+
 int steps_force_residual(const double* pos, const double* acc, long long N, double B, double* out2, steps_stream_t stream)
 {
     if (!pos || !acc || !out2 || N < 1) return STEPS_EINVAL;

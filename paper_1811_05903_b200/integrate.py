@@ -36,7 +36,7 @@ def run_adaptive(pos, vel, acc, mass, soft, a0: float, n_steps: int, cosmo: S.Co
     dt_dev = torch.empty(1, dtype=torch.float64, device=pos.device)
     a, dts = a0, []
     for k in range(n_steps):
-        S.steps_timestep(pos, acc, soft, abs(G) / a ** 3, B, eps, dt_max, dt_dev)
+        S.steps_timestep(pos, acc, soft, S.steps_timestep_coefficient(G, a), B, eps, dt_max, dt_dev)
         dt = float(dt_dev.item())
         a = run_kdk(pos, vel, acc, mass, soft, a, [dt], cosmo, G, B, mixed=mixed)
         dts.append(dt)

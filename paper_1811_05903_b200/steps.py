@@ -11,12 +11,12 @@ import os
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsteps_b200.so")
 
-OK, EINVAL, ECUDA, EUNSUPPORTED, ENOMEM = 0, -1, -2, -3, -4
+OK, EINVAL, ECUDA, EUNSUPPORTED, ENOMEM, ECAPTURE = 0, -1, -2, -3, -4, -5
 
 EXPORTS = [
     "steps_forces", "steps_forces_mixed", "steps_forces_range", "steps_forces_host", "steps_kick_drift",
     "steps_kdk_step", "steps_hubble", "steps_scale_factor_rk4", "steps_kdk_schedule", "steps_momentum",
-    "steps_timestep", "steps_force_residual", "steps_forces_quasi_periodic", "steps_forces_periodic",
+    "steps_timestep", "steps_timestep_coefficient", "steps_force_residual", "steps_forces_quasi_periodic", "steps_forces_periodic",
     "steps_kdk_step_adaptive", "steps_kick_close_adaptive",
     "steps_reserve", "steps_shutdown", "steps_workspace_bytes", "steps_strerror", "steps_last_cuda_error",
     "steps_version", "steps_kernel_launch_count", "steps_set_option", "steps_last_force_kernel_ms",
@@ -47,7 +47,19 @@ def lib() -> C.CDLL:
     if _lib is not None:
         return _lib
     from . import build as _build
-    path = _build.build()
+    _lib = load_library(_build.build())
+    return _lib
+
+
+def build_info() -> dict:
+    """What the build did to the loaded library (nvcc command, operand-reuse pass): build.py's buildinfo record."""
+    from . import build as _build
+    return _build.build_info()
+
+
+def load_library(path: str) -> C.CDLL:
+    """dlopen a build of the C-ABI library and declare its prototypes (lib() does this for the product build; the A/B
+    test of the post-link pass loads the unpatched build next to it)."""
     L = C.CDLL(path)
     vp, ll, dbl, i32 = C.c_void_p, C.c_longlong, C.c_double, C.c_int
     L.steps_forces.argtypes = [vp, vp, vp, ll, vp, vp]
@@ -68,6 +80,8 @@ def lib() -> C.CDLL:
     L.steps_kick_close_adaptive.argtypes = [vp, vp, vp, ll, vp, dbl, vp]
     L.steps_timestep.argtypes = [vp, vp, vp, ll, dbl, dbl, dbl, dbl, vp, vp]
     L.steps_force_residual.argtypes = [vp, vp, ll, dbl, vp, vp]
+    L.steps_timestep_coefficient.argtypes = [dbl, dbl]
+    L.steps_timestep_coefficient.restype = dbl
     L.steps_reserve.argtypes = [ll]
     L.steps_shutdown.restype = None
     L.steps_workspace_bytes.argtypes = [ll]
@@ -78,7 +92,6 @@ def lib() -> C.CDLL:
     L.steps_set_option.argtypes = [C.c_char_p, ll]
     L.steps_last_force_kernel_ms.restype = dbl
     L.steps_persistent_grid.argtypes = [i32]
-    _lib = L
     return L
 
 
@@ -208,6 +221,10 @@ def steps_timestep(pos, acc, soft, coef: float, B: float, eps: float, dt_max: fl
     n = soft.numel()
     _check(lib().steps_timestep(_dev(pos, 3 * n), _dev(acc, 3 * n), _dev(soft, n), n, coef, B, eps, dt_max,
                                 _dev(dt_out, 1), _stream(stream)))
+
+
+def steps_timestep_coefficient(G: float, a: float) -> float:
+    return float(lib().steps_timestep_coefficient(G, a))
 
 
 def steps_force_residual(pos, acc, B: float, out2, stream=None) -> None:

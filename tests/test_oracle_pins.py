@@ -435,6 +435,16 @@ def test_kdk_coefficient_form_equals_literal_step(oracle):
 
 
 # ---- diagnostics: P = sum m v, sum m |v| -----------------------------------------------------
+def test_periodic_oracles_sampled_equals_full(oracle):
+    """The idx argument of the two periodic oracles only selects which particles are evaluated."""
+    rng = np.random.default_rng(11)
+    n, L = 40, 1.1
+    pos, mass, soft = rng.uniform(0, L, (3, n)), rng.uniform(0.5, 1.5, n), np.full(n, 0.02)
+    idx = np.array([3, 17, 39, 0])
+    for fn in (oracle.forces_quasi_periodic, oracle.forces_periodic_images):
+        np.testing.assert_array_equal(fn(pos, mass, soft, L, idx=idx), fn(pos, mass, soft, L)[:, idx])
+
+
 def test_momentum_hand_values_and_brute_force(oracle):
     """Three particles with hand-typed values: m = (1, 2, 4), v_1 = (3, 4, 0), v_2 = (0, -6, 8), v_3 = (-2, 1, 2),
     |v| = (5, 10, 3):  sum m v = (3 - 8, 4 - 12 + 4, 16 + 8) = (-5, -4, 24),  sum m |v| = 5 + 20 + 12 = 37.
