@@ -48,9 +48,26 @@ PEAK_FP64_TFLOPS = SM_COUNT * 64 * 2 * SM_MAX_MHZ * 1e6 / 1e12      # 37.22 (64 
 METRIC = "pairwise interactions/s per force eval at N=1M"
 UNIT = "interactions/s"
 LCDM = dict(H0=0.0288675134594813, Omega_m=0.3, Omega_r=0.0, Omega_L=0.7, Omega_k=0.0)
-# DRAM bytes per launch of the force kernel from the committed `ncu --set full` capture
-# (profiles/r01_force_kernels_ncu.md); None until captured.
-NCU_DRAM_BYTES = {"mixed": 84.567040e6 + 18.440448e6, "fp64": 5.357882e9 + 89.916160e6}
+
+
+def ncu_traffic(path: str, n: int):
+    """DRAM bytes per force evaluation (dram__bytes_read.sum + dram__bytes_write.sum of its force kernels) from the newest
+    committed `ncu --set full` capture, profiles/r*_dram_traffic.csv: rows `path,N,kernel,read_bytes,write_bytes`.  The
+    figure is a record of that capture, not measured in this run: returned only for the captured (path, N), else None."""
+    import csv
+    import glob
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_dram_traffic.csv")))
+    if not files:
+        return None, "no ncu capture committed"
+    total, kernels = 0.0, []
+    with open(files[-1]) as f:
+        for row in csv.DictReader(f):
+            if row["path"] == path and int(row["N"]) == n:
+                total += float(row["read_bytes"]) + float(row["write_bytes"])
+                kernels.append(row["kernel"])
+    if not kernels:
+        return None, f"{os.path.basename(files[-1])} has no capture of path={path} N={n}"
+    return total, f"{os.path.basename(files[-1])}: " + " + ".join(kernels)
 
 
 class ClockSampler:
@@ -129,6 +146,66 @@ def cpu_oracle_rate(ps, budget_s: float = 12.0):
             "sample": f"{len(idx)} stratified i-particles x all {n} sources of the same workload, {dt:.1f} s"}
 
 
+def bench_next_rows(S, synth, torch, stream, reps: int = 3):
+    """SURVEY.md 8(f) rows, each timed on its own workload (3 warm-up + `reps` timed calls, CUDA events on the launch
+    stream, L2 not flushed: these kernels are ALU-bound and their inputs fit L2 anyway).  Periodic boxes: uniform random
+    particles of equal mass in a cube of side 1, softening 1/30 of the mean spacing (the state glass making starts from,
+    as in the parity tests).  The roofline fraction uses the same 20 flop per evaluated pair term as the headline."""
+    import numpy as np
+
+    def timed(fn):
+        for _ in range(3):
+            fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(reps):
+            fn()
+        e1.record(stream)
+        e1.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    def box(n, seed):
+        rng = np.random.default_rng(seed)
+        pos = torch.from_numpy(np.ascontiguousarray(rng.uniform(0.0, 1.0, size=(3, n)))).cuda()
+        mass = torch.full((n,), 1.0 / n, dtype=torch.float64, device="cuda")
+        soft = torch.full((n,), 1.0 / n ** (1 / 3) / 30, dtype=torch.float64, device="cuda")
+        return pos, mass, soft, torch.empty_like(pos)
+
+    rows = {}
+    n = 262144
+    pos, mass, soft, acc = box(n, 9001)
+    for mixed in (False, True):
+        ms = timed(lambda: S.steps_forces_quasi_periodic(pos, mass, soft, 1.0, acc, mixed=mixed))
+        rate = n * (n - 1.0) / (ms * 1e-3)
+        peak = PEAK_FP32_TFLOPS if mixed else PEAK_FP64_TFLOPS
+        rows["quasi_periodic_" + ("mixed" if mixed else "fp64")] = {
+            "value": rate, "unit": UNIT, "ms": ms, "N": n, "workload": "uniform periodic box, leading image (Eq. 5)",
+            "roofline": {"bound": "alu", "achieved": FLOP_PER_INTERACTION * rate / 1e12, "peak": peak, "unit": "TFLOP/s",
+                         "frac": FLOP_PER_INTERACTION * rate / 1e12 / peak}}
+    n = 32768
+    pos, mass, soft, acc = box(n, 9002)
+    ms = timed(lambda: S.steps_forces_periodic(pos, mass, soft, 1.0, acc))
+    images = 4.0 / 3.0 * math.pi * 2.6 ** 3                        # mean number of images inside the 2.6 L cut per pair
+    rate = n * (n - 1.0) / (ms * 1e-3)
+    rows["periodic_images"] = {
+        "value": rate, "unit": "pairs/s (each summed over its images inside |x - nL| < 2.6 L)", "ms": ms, "N": n,
+        "images_per_pair_in_cut": images, "image_terms_per_s": rate * images,
+        "roofline": {"bound": "alu", "achieved": FLOP_PER_INTERACTION * rate * images / 1e12, "peak": PEAK_FP64_TFLOPS,
+                     "unit": "TFLOP/s", "frac": FLOP_PER_INTERACTION * rate * images / 1e12 / PEAK_FP64_TFLOPS}}
+    # device-resident adaptive step (Eq. 12 + KDK + force evaluation), config 0 size and 32,768
+    for n in (4096, 32768):
+        ps = synth.g0(n, synth.SEED_BASE)
+        x, m, h = (torch.from_numpy(a).cuda() for a in (ps.pos, ps.mass, ps.soft))
+        v, a = torch.zeros_like(x), torch.empty_like(x)
+        S.steps_forces(x, m, h, a)
+        st = torch.tensor([1.0 / 51.0, 0.0, 1.0, 0.0, 0.0], dtype=torch.float64, device="cuda")
+        cosmo = S.Cosmology(**LCDM)
+        ms = timed(lambda: S.steps_kdk_step_adaptive(x, v, a, m, h, st, cosmo, 1.0, 1.25e-4, 0.025, 0.05))
+        rows[f"adaptive_step_{n}"] = {"value": n * (n - 1.0) / (ms * 1e-3), "unit": UNIT, "us_per_step": 1e3 * ms, "N": n,
+                                       "workload": "steps_kdk_step_adaptive, fp64, compactified g0 set"}
+    return rows
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle (fp64 pairwise spline sum), each step a bounded sample."""
     rank = int(os.environ.get("RANK", "0"))
@@ -169,6 +246,7 @@ def main():
     ap.add_argument("--paths", default="mixed,fp64")
     ap.add_argument("--ref-pairs", type=float, default=4e9, help="--impl reference: pair budget per step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-next-rows", action="store_true", help="skip the periodic / adaptive-step rows (SURVEY 8(f))")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -261,15 +339,21 @@ def main():
             peak = PEAK_FP32_TFLOPS if mixed else PEAK_FP64_TFLOPS
             kern_inter = float(cnt) * (n - 1.0)                 # this rank's launch
             achieved = FLOP_PER_INTERACTION * kern_inter / (k_ms * 1e-3) / 1e12
+            traffic, traffic_source = ncu_traffic(path, n) if world == 1 else (None, "multi-GPU run")
+            symmetric = world == 1 and S.steps_pair_symmetric(n)
             results[path] = {
                 "value": args.steps * inter_step / (total_ms * 1e-3), "unit": UNIT,
                 "ms_per_step": total_ms / args.steps, "force_kernel_ms": k_ms, "gpu_launches": int(launches),
                 "dtype": "f32 pairs, f64 accumulate" if mixed else "f64",
                 "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                             "frac": achieved / peak, "traffic": NCU_DRAM_BYTES[path],
+                             "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_source,
                              "flop_per_interaction": FLOP_PER_INTERACTION,
+                             "pair_evaluation": ("each far block pair once, applied to both blocks (Newton III, PAPER L131); "
+                                                 "band around the diagonal one-sided") if symmetric else "one-sided (every ordered pair)",
                              "peak_source": "148 SM x %d lanes x 2 x %.0f MHz (%s; DESIGN.md section 6; lanes/SM measured)" % (128 if mixed else 64, SM_MAX_MHZ, SM_MHZ_SOURCE),
-                             "kernel": "forces_persistent_kernel<%s>" % ("MixedPath" if mixed else "Fp64Path"),
+                             "kernel": (("forces_sym_mixed_kernel" if mixed else "forces_sym_kernel") +
+                                        " + band forces_persistent_kernel + reduces (one event pair around all of them)") if symmetric
+                                       else "forces_persistent_kernel<%s>" % ("MixedPath" if mixed else "Fp64Path"),
                              "kernel_share_of_step": k_ms * args.steps / total_ms},
             }
             launches_total += launches
@@ -291,6 +375,8 @@ def main():
             e2e = {"value": reps * inter_step / (e0.elapsed_time(e1) * 1e-3), "unit": UNIT,
                    "h2d_bytes_per_step": 5 * n * 8, "d2h_bytes_per_step": 3 * n * 8,
                    "call": "steps_forces_host(mixed=1), pinned host buffers"}
+        # the section 8(f) NEXT rows (one GPU; their own short repetition, not --steps)
+        next_rows = bench_next_rows(S, synth, torch, stream) if world == 1 and not args.no_next_rows else None
     clocks = sampler.summary()
 
     if rank != 0:
@@ -315,7 +401,7 @@ def main():
                    "i_sharding": "none" if world == 1 else f"i-range per rank (PAPER L139), all-gather of positions, {world} ranks",
                    "persistent_grid": {p: S.steps_persistent_grid(p == "mixed") for p in results}},
         "roofline": r["roofline"], "paths": results, "clocks": clocks, "gpu_launches": int(launches_total),
-        "e2e": e2e, "cpu_baseline": cpu,
+        "e2e": e2e, "cpu_baseline": cpu, "next_rows": next_rows, "build": S.build_info(),
         "context": "paper (other hardware): 9.3 Tflop/s on 4x GTX 1080 Ti, ~24% of peak (L159); K80 ~9.7e9 interactions/s/GPU (Table 1, derived)",
     }
     print(json.dumps(out))

@@ -229,6 +229,10 @@ int steps_set_option(const char *key, long long value);
  * device (waits for it to finish); -1 if none was recorded.  For a pair-symmetric evaluation: from the
  * start of the band kernel to the end of the last panel's reduce (all force kernels of the evaluation). */
 double steps_last_force_kernel_ms(void);
+/* 1 if a full force evaluation of N particles is set up pair-symmetrically (see steps_forces; N >= 131,072 and the
+ * "sym" option on), else 0.  Host-side eligibility only: the device still routes everything through the one-sided
+ * kernel when the data do not allow the split (unsorted input, massless particles). */
+int steps_pair_symmetric(long long N);
 /* Grid (CTA count) of the persistent force kernel on the current device: SMs x resident CTAs;
  * 0 before the first call of that path. */
 int steps_persistent_grid(int mixed);

@@ -36,6 +36,7 @@
 #pragma once
 #include "common.cuh"
 #include "force_fp64.cuh"
+#include "force_mixed.cuh"
 #include "force_driver.cuh"
 
 namespace steps {
@@ -270,6 +271,167 @@ forces_sym_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__
             colrec[rec + j] = f * Bsm[j]; colrec[rec + IB + j] = f * Bsm[IB + j]; colrec[rec + 2 * IB + j] = f * Bsm[2 * IB + j];
         }
         __syncthreads();                                          // stage s and Bsm are free again
+        if (threadIdx.x == 0 && it + 2 < total) produce(it + 2);
+        if (++c == nb) { ++b; c = b + W + 1; }
+    }
+}
+
+// ---- the same for the MIXED path (fp32 pairs, fp64 accumulation) ------------------------------------------------------
+// Per step a lane meets one source with its 4 particles packed in two pairs (FFMA2 / FMUL2, the source's scalars broadcast to
+// both halves): per packed pair 3 differences, 3 for r^2, 2 MUFU.RSQ, 2 for y^3, 1 for s_i = m_i y^3 and 2 x 3 accumulates
+// = 15 packed FP32-pipe instructions + 2 MUFU per FOUR ordered interactions (11 + 2 per two in the asymmetric body).
+// fp32 sums never hold more than 128 terms: the particles' sums are flushed into fp64 accumulators in shared memory after
+// every 128-source subgroup, the sources' reaction sums (two packed halves, 64 terms each) into fp64 shared memory after the
+// 32 hand-overs of a set.  Scaled sources: c_j = m_j^(-1/2) in fp32, dX = X_j - c_j x_i, y = 1/(c_j r):
+//   on i:  m_j (x_j - x_i)/r^3 = y^3 dX          on j:  -(m_i y^3 dX) c_j^2
+__host__ __device__ constexpr int sym_mixed_stage_bytes() { return TPB * 4 * TJ * (int)sizeof(float); }     // (X, Y, Z, c) of the block's tiles
+__host__ __device__ constexpr int sym_mixed_smem_bytes() { return 2 * sym_mixed_stage_bytes() + 3 * IB * (int)sizeof(double) + 3 * R_I * CTA_THREADS * (int)sizeof(double); }
+
+__global__ void __launch_bounds__(CTA_THREADS, 1)
+forces_sym_mixed_kernel(const TileF32* __restrict__ tiles, const SymPlan* __restrict__ plan, long long k_begin, long long k_end,
+                        double* __restrict__ rowrec, double* __restrict__ colrec)
+{
+    static_assert(R_I == 4, "two packed pairs per lane");
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ uint64_t full_bar[2];
+    constexpr int STAGE = sym_mixed_stage_bytes();
+    float* col = reinterpret_cast<float*>(smem_raw);                                   // [2][TPB][4][TJ]
+    double* Bsm = reinterpret_cast<double*>(smem_raw + 2 * STAGE);                     // [3][IB]
+    double* Asm = Bsm + 3 * IB + threadIdx.x;                                          // [3][R_I][CTA_THREADS], this thread's column
+
+    const long long K = plan->K;
+    if (k_end > K) k_end = K;
+    if (k_begin >= k_end) return;
+    const int W = plan->W, nb = plan->nb, Km = plan->Km;
+    const long long n_items = k_end - k_begin;
+    const long long kk0 = k_begin + (long long)blockIdx.x * n_items / gridDim.x;
+    const long long kk1 = k_begin + ((long long)blockIdx.x + 1) * n_items / gridDim.x;
+    const int total = (int)(kk1 - kk0);
+    if (total <= 0) return;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    int b, c;
+    {
+        const double t = 2.0 * Km + 1.0;
+        int bb = (int)((t - sqrt(fmax(t * t - 8.0 * (double)kk0, 0.0))) * 0.5);
+        bb = max(0, min(bb, Km - 1));
+        while (bb + 1 < Km && sym_row_start(bb + 1, Km) <= kk0) ++bb;
+        while (bb > 0 && sym_row_start(bb, Km) > kk0) --bb;
+        b = bb;
+        c = bb + W + 1 + (int)(kk0 - sym_row_start(bb, Km));
+    }
+    if (threadIdx.x == 0) {
+        mbar_init(&full_bar[0], 1); mbar_init(&full_bar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    int pb = b, pc = c;
+    auto produce = [&](int it) {
+        const int s = it & 1;
+        mbar_expect_tx(&full_bar[s], (uint32_t)STAGE);
+#pragma unroll
+        for (int t = 0; t < TPB; ++t)          // X[], Y[], Z[], c[] are the first 4 TJ floats of a tile record
+            bulk_load(reinterpret_cast<unsigned char*>(col) + (size_t)s * STAGE + t * (4 * TJ * sizeof(float)),
+                      &tiles[(long long)pc * TPB + t].X[0], (uint32_t)(4 * TJ * sizeof(float)), &full_bar[s]);
+        if (++pc == nb) { ++pb; pc = pb + W + 1; }
+    };
+    if (threadIdx.x == 0) {
+        produce(0);
+        if (total > 1) produce(1);
+    }
+
+    constexpr int NP = R_I / 2;
+    u64 nx[NP], ny[NP], nz[NP], m2[NP];
+    int cur_b = -1;
+    const int src_lane = (lane + 31) & 31;
+
+    for (int it = 0; it < total; ++it) {
+        if (b != cur_b) {
+            cur_b = b;
+            float x[R_I], y[R_I], z[R_I], m[R_I];
+#pragma unroll
+            for (int k = 0; k < R_I; ++k) {
+                const int i = warp * WARP_I + lane + 32 * k;
+                const TileF32& T = tiles[(long long)b * TPB + i / TJ];
+                x[k] = T.x[i % TJ]; y[k] = T.y[i % TJ]; z[k] = T.z[i % TJ]; m[k] = T.m[i % TJ];
+            }
+#pragma unroll
+            for (int p = 0; p < NP; ++p) {
+                nx[p] = pack2(-x[2 * p], -x[2 * p + 1]); ny[p] = pack2(-y[2 * p], -y[2 * p + 1]);
+                nz[p] = pack2(-z[2 * p], -z[2 * p + 1]); m2[p] = pack2(m[2 * p], m[2 * p + 1]);
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < 3 * R_I; ++q) Asm[q * CTA_THREADS] = 0.0;
+        for (int q = threadIdx.x; q < 3 * IB; q += CTA_THREADS) Bsm[q] = 0.0;
+        const int s = it & 1;
+        mbar_wait(&full_bar[s], (it >> 1) & 1);
+        __syncthreads();
+        const float* cs = col + (size_t)s * (STAGE / sizeof(float));
+
+        for (int q = 0; q < SUBGROUPS; ++q) {
+            const int u = (warp + q) & (SUBGROUPS - 1);
+            u64 ax[NP], ay[NP], az[NP];
+#pragma unroll
+            for (int p = 0; p < NP; ++p) ax[p] = ay[p] = az[p] = 0ull;
+            for (int t = 0; t < WARP_I / 32; ++t) {
+                const int j0 = u * WARP_I + t * 32;                                   // first source of the set (within the block)
+                const float* set = cs + (j0 / TJ) * (4 * TJ) + (j0 % TJ);           // X of source j0; Y, Z, c follow at + TJ each
+                u64 bx = 0ull, by = 0ull, bz = 0ull;
+#pragma unroll 2
+                for (int st = 0; st < 32; ++st) {
+                    const int r = (lane - st) & 31;
+                    const float X = set[r], Y = set[TJ + r], Z = set[2 * TJ + r], C = set[3 * TJ + (r ^ STEPS_C_SWIZZLE)];
+                    const u64 cq = pack2(C, C), Xq = pack2(X, X), Yq = pack2(Y, Y), Zq = pack2(Z, Z);
+#pragma unroll
+                    for (int p = 0; p < NP; ++p) {
+                        const u64 dX = fma2(nx[p], cq, Xq), dY = fma2(ny[p], cq, Yq), dZ = fma2(nz[p], cq, Zq);
+                        const u64 r2 = fma2(dZ, dZ, fma2(dY, dY, mul2(dX, dX)));
+                        float ra, rb;
+                        unpack2(r2, ra, rb);
+                        const u64 y = pack2(rsqrt_approx(ra), rsqrt_approx(rb));
+                        const u64 y3 = mul2(mul2(y, y), y);
+                        const u64 si = mul2(y3, m2[p]);
+                        ax[p] = fma2(dX, y3, ax[p]);
+                        ay[p] = fma2(dY, y3, ay[p]);
+                        az[p] = fma2(dZ, y3, az[p]);
+                        bz = fma2(dZ, si, bz);
+                        by = fma2(dY, si, by);
+                        bx = fma2(dX, si, bx);
+                    }
+                    bx = __shfl_sync(0xffffffffu, bx, src_lane);
+                    by = __shfl_sync(0xffffffffu, by, src_lane);
+                    bz = __shfl_sync(0xffffffffu, bz, src_lane);
+                }
+                float lo, hi;
+                const int j = j0 + lane;
+                unpack2(bx, lo, hi); Bsm[j] += (double)lo + (double)hi;
+                unpack2(by, lo, hi); Bsm[IB + j] += (double)lo + (double)hi;
+                unpack2(bz, lo, hi); Bsm[2 * IB + j] += (double)lo + (double)hi;
+            }
+#pragma unroll
+            for (int p = 0; p < NP; ++p) {                   // 128 sources per particle: into the fp64 accumulators
+                float lo, hi;
+                unpack2(ax[p], lo, hi); Asm[(0 * R_I + 2 * p) * CTA_THREADS] += (double)lo; Asm[(0 * R_I + 2 * p + 1) * CTA_THREADS] += (double)hi;
+                unpack2(ay[p], lo, hi); Asm[(1 * R_I + 2 * p) * CTA_THREADS] += (double)lo; Asm[(1 * R_I + 2 * p + 1) * CTA_THREADS] += (double)hi;
+                unpack2(az[p], lo, hi); Asm[(2 * R_I + 2 * p) * CTA_THREADS] += (double)lo; Asm[(2 * R_I + 2 * p + 1) * CTA_THREADS] += (double)hi;
+            }
+            __syncthreads();
+        }
+
+        const long long rec = (kk0 + it - k_begin) * 3 * IB;
+#pragma unroll
+        for (int k = 0; k < R_I; ++k) {
+            const int i = warp * WARP_I + lane + 32 * k;
+#pragma unroll
+            for (int cc = 0; cc < 3; ++cc) rowrec[rec + cc * IB + i] = Asm[(cc * R_I + k) * CTA_THREADS];
+        }
+        for (int j = threadIdx.x; j < IB; j += CTA_THREADS) {
+            const double cj = (double)cs[(j / TJ) * (4 * TJ) + 3 * TJ + ((j % TJ) ^ STEPS_C_SWIZZLE)];
+            const double f = -cj * cj;
+            colrec[rec + j] = f * Bsm[j]; colrec[rec + IB + j] = f * Bsm[IB + j]; colrec[rec + 2 * IB + j] = f * Bsm[2 * IB + j];
+        }
+        __syncthreads();
         if (threadIdx.x == 0 && it + 2 < total) produce(it + 2);
         if (++c == nb) { ++b; c = b + W + 1; }
     }

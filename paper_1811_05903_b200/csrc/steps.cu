@@ -47,7 +47,7 @@ struct Workspace {
     double* sym_records = nullptr;  // 2 * panel_items * 3 * IB doubles (row records, then column records)
     long long sym_cap_particles = 0, sym_panel_items = 0;
     int num_sms = 0;
-    int grid_mixed = 0, grid_fp64 = 0, grid_fp64_band = 0, grid_sym = 0;   // persistent grids: SMs x resident CTAs
+    int grid_mixed = 0, grid_fp64 = 0, grid_fp64_band = 0, grid_mixed_band = 0, grid_sym = 0, grid_sym_mixed = 0;   // persistent grids: SMs x resident CTAs
     int grid_mixed_periodic = 0, grid_fp64_periodic = 0, grid_fp64_images = 0;
     double* mom_partial = nullptr;  // MOM_BLOCKS * 4
     // staging buffers of steps_forces_host
@@ -190,27 +190,30 @@ int persistent_grid(Kernel kern, int smem, const Workspace& w, int& grid_cache)
     return STEPS_OK;
 }
 
-// Full fp64 evaluation, pair-symmetric (force_sym.cuh): band through the asymmetric persistent kernel, every far block
-// pair once through forces_sym_kernel, panel by panel; all decisions that depend on the data (W) are taken on the device.
+// Full evaluation, pair-symmetric (force_sym.cuh): band through the asymmetric persistent kernel, every far block pair once
+// through the symmetric kernel, panel by panel; all decisions that depend on the data (W) are taken on the device.
+template <typename Path>
 int launch_forces_sym(const double* pos, const double* mass, const double* soft, long long N, double* acc_out,
                       cudaStream_t st, Workspace& w)
 {
-    using Path = Fp64Path;
+    using Tile = typename Path::Tile;
+    constexpr bool FP64 = Path::NOUT == 6;
     const int nb = (int)nblocks_of(N);
     const int ntp = nb * TPB;
-    TileF64* tiles = reinterpret_cast<TileF64*>(w.tiles);
+    Tile* tiles = reinterpret_cast<Tile*>(w.tiles);
     constexpr int smem_band = persistent_smem_bytes<Path, STAGES>();
     auto band = forces_persistent_kernel<Path, STAGES, 0, true>;
-    int rc = persistent_grid(band, smem_band, w, w.grid_fp64_band);
+    int rc = persistent_grid(band, smem_band, w, FP64 ? w.grid_fp64_band : w.grid_mixed_band);
     if (rc != STEPS_OK) return rc;
-    rc = persistent_grid(forces_sym_kernel, sym_smem_bytes(), w, w.grid_sym);
+    if constexpr (FP64) rc = persistent_grid(forces_sym_kernel, sym_smem_bytes(), w, w.grid_sym);
+    else rc = persistent_grid(forces_sym_mixed_kernel, sym_mixed_smem_bytes(), w, w.grid_sym_mixed);
     if (rc != STEPS_OK) return rc;
-    const int P = w.grid_fp64_band, Ps = w.grid_sym;
+    const int P = FP64 ? w.grid_fp64_band : w.grid_mixed_band, Ps = FP64 ? w.grid_sym : w.grid_sym_mixed;
     const bool prof = g_profile.load() != 0;
     if (prof && !w.ev0) { STEPS_CUDA(cudaEventCreate(&w.ev0)); STEPS_CUDA(cudaEventCreate(&w.ev1)); }
 
-    prep_tiles<TileF64><<<ntp, TJ, 0, st>>>(pos, mass, soft, N, tiles, &w.plan->W);
-    sym_band_width<TileF64><<<nb, 128, 0, st>>>(tiles, nb, w.plan);
+    prep_tiles<Tile><<<ntp, TJ, 0, st>>>(pos, mass, soft, N, tiles, &w.plan->W);
+    sym_band_width<Tile><<<nb, 128, 0, st>>>(tiles, nb, w.plan);
     sym_plan_finalize<<<1, 1024, 0, st>>>(w.plan, nb, 8 * Ps);
     if (prof) STEPS_CUDA(cudaEventRecord(w.ev0, st));
     band<<<P, CTA_THREADS, smem_band, st>>>(pos, soft, N, tiles, ntp, 0, N, nb, w.partials, 0, 0.0, 0.0, w.plan);
@@ -223,7 +226,8 @@ int launch_forces_sym(const double* pos, const double* mass, const double* soft,
     double* colrec = w.sym_records + (size_t)items * 3 * IB;
     for (long long k0 = 0; k0 < kmax; k0 += items) {
         const long long k1 = std::min(kmax, k0 + items);
-        forces_sym_kernel<<<Ps, CTA_THREADS, sym_smem_bytes(), st>>>(tiles, w.plan, k0, k1, rowrec, colrec, 0);
+        if constexpr (FP64) forces_sym_kernel<<<Ps, CTA_THREADS, sym_smem_bytes(), st>>>(tiles, w.plan, k0, k1, rowrec, colrec, 0);
+        else forces_sym_mixed_kernel<<<Ps, CTA_THREADS, sym_mixed_smem_bytes(), st>>>(tiles, w.plan, k0, k1, rowrec, colrec);
         forces_sym_reduce_kernel<<<(int)((N + 255) / 256), 256, 0, st>>>(w.plan, rowrec, colrec, k0, k1, N, hi, lo,
                                                                           k1 == kmax ? 1 : 0, acc_out);
         g_launches += 2;
@@ -238,10 +242,9 @@ int launch_forces(const double* pos, const double* mass, const double* soft, lon
                   long long i_end, double* acc_out, cudaStream_t st, Workspace& w, int& grid_cache)
 {
     using Tile = typename Path::Tile;
-    if constexpr (Path::NOUT == 6) {
-        if (i_begin == 0 && i_end == N && g_driver.load() == 0 && sym_eligible(N) && w.sym_records)
-            return launch_forces_sym(pos, mass, soft, N, acc_out, st, w);
-    }
+    if (i_begin == 0 && i_end == N && g_driver.load() == 0 && sym_eligible(N) && w.sym_records &&
+        (Path::NOUT == 6 || g_sym_enabled.load() != 2))      // "sym" = 2: fp64 path only
+        return launch_forces_sym<Path>(pos, mass, soft, N, acc_out, st, w);
     const int nt = (int)ntiles_of(N);
     Tile* tiles = reinterpret_cast<Tile*>(w.tiles);
     prep_tiles<Tile><<<nt, TJ, 0, st>>>(pos, mass, soft, N, tiles, nullptr);
@@ -634,7 +637,7 @@ int steps_set_option(const char* key, long long value)
     if (!key) return STEPS_EINVAL;
     if (std::strcmp(key, "driver") == 0) { g_driver = (int)value; return STEPS_OK; }
     if (std::strcmp(key, "profile") == 0) { g_profile = (int)value; return STEPS_OK; }
-    if (std::strcmp(key, "sym") == 0) { g_sym_enabled = value != 0; return STEPS_OK; }
+    if (std::strcmp(key, "sym") == 0) { g_sym_enabled = (int)value; return STEPS_OK; }
     if (std::strcmp(key, "sym_panel_items") == 0) {
         if (value < 1) return STEPS_EINVAL;
         g_sym_panel_items = value;
@@ -653,6 +656,8 @@ double steps_last_force_kernel_ms(void)
     if (cudaEventSynchronize(w.ev1) != cudaSuccess || cudaEventElapsedTime(&ms, w.ev0, w.ev1) != cudaSuccess) return -1.0;
     return (double)ms;
 }
+
+int steps_pair_symmetric(long long N) { return N >= 1 && sym_eligible(N) && g_driver.load() == 0 ? 1 : 0; }
 
 int steps_persistent_grid(int mixed)
 {

@@ -26,7 +26,7 @@ import struct
 import subprocess
 import sys
 
-KERNEL_PATTERNS = ("forces_persistent_kernelINS_8Fp64Path", "forces_v1_kernelINS_8Fp64Path", "forces_sym_kernel",
+KERNEL_PATTERNS = ("forces_persistent_kernelINS_8Fp64Path", "forces_v1_kernelINS_8Fp64Path", "forces_sym_kernel", "forces_sym_mixed_kernel",
                    "forces_persistent_kernelINS_9MixedPath", "forces_v1_kernelINS_9MixedPath")
 # the 2-clk-per-warp arithmetic instructions with 64-bit register operands: FP64 and packed fp32x2
 FP64_OPS = ("DFMA", "DMUL", "FFMA2", "FMUL2")

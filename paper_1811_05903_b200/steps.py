@@ -20,7 +20,7 @@ EXPORTS = [
     "steps_kdk_step_adaptive", "steps_kick_close_adaptive",
     "steps_reserve", "steps_shutdown", "steps_workspace_bytes", "steps_strerror", "steps_last_cuda_error",
     "steps_version", "steps_kernel_launch_count", "steps_set_option", "steps_last_force_kernel_ms",
-    "steps_persistent_grid",
+    "steps_persistent_grid", "steps_pair_symmetric",
 ]
 
 
@@ -92,6 +92,7 @@ def load_library(path: str) -> C.CDLL:
     L.steps_set_option.argtypes = [C.c_char_p, ll]
     L.steps_last_force_kernel_ms.restype = dbl
     L.steps_persistent_grid.argtypes = [i32]
+    L.steps_pair_symmetric.argtypes = [ll]
     return L
 
 
@@ -263,3 +264,7 @@ def steps_last_force_kernel_ms() -> float:
 
 def steps_persistent_grid(mixed: bool) -> int:
     return int(lib().steps_persistent_grid(int(mixed)))
+
+
+def steps_pair_symmetric(n: int) -> bool:
+    return bool(lib().steps_pair_symmetric(n))
