@@ -150,7 +150,7 @@ def bench_next_rows(S, synth, torch, stream, reps: int = 3):
     """SURVEY.md 8(f) rows, each timed on its own workload (3 warm-up + `reps` timed calls, CUDA events on the launch
     stream, L2 not flushed: these kernels are ALU-bound and their inputs fit L2 anyway).  Periodic boxes: uniform random
     particles of equal mass in a cube of side 1, softening 1/30 of the mean spacing (the state glass making starts from,
-    as in the parity tests).  The roofline fraction uses the same 20 flop per evaluated pair term as the headline."""
+    as in the parity tests), in Morton (cell) order -- the periodic counterpart of the radial order.  The roofline fraction uses the same 20 flop per evaluated pair term as the headline."""
     import numpy as np
 
     def timed(fn):
@@ -165,10 +165,7 @@ def bench_next_rows(S, synth, torch, stream, reps: int = 3):
         return e0.elapsed_time(e1) / reps
 
     def box(n, seed):
-        rng = np.random.default_rng(seed)
-        pos = torch.from_numpy(np.ascontiguousarray(rng.uniform(0.0, 1.0, size=(3, n)))).cuda()
-        mass = torch.full((n,), 1.0 / n, dtype=torch.float64, device="cuda")
-        soft = torch.full((n,), 1.0 / n ** (1 / 3) / 30, dtype=torch.float64, device="cuda")
+        pos, mass, soft = (torch.from_numpy(a).cuda() for a in synth.periodic_box(n, 1.0, seed))
         return pos, mass, soft, torch.empty_like(pos)
 
     rows = {}
@@ -179,7 +176,7 @@ def bench_next_rows(S, synth, torch, stream, reps: int = 3):
         rate = n * (n - 1.0) / (ms * 1e-3)
         peak = PEAK_FP32_TFLOPS if mixed else PEAK_FP64_TFLOPS
         rows["quasi_periodic_" + ("mixed" if mixed else "fp64")] = {
-            "value": rate, "unit": UNIT, "ms": ms, "N": n, "workload": "uniform periodic box, leading image (Eq. 5)",
+            "value": rate, "unit": UNIT, "ms": ms, "N": n, "workload": "uniform periodic box in Morton order, leading image (Eq. 5)",
             "roofline": {"bound": "alu", "achieved": FLOP_PER_INTERACTION * rate / 1e12, "peak": peak, "unit": "TFLOP/s",
                          "frac": FLOP_PER_INTERACTION * rate / 1e12 / peak}}
     n = 32768

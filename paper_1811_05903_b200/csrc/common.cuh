@@ -57,7 +57,12 @@ constexpr int WARP_I = 32 * R_I;          // contiguous i-particles owned by one
 // | |x_i| - |x_j| | <= |x_i - x_j|).
 struct TileMeta {
     float rmin, rmax, hmax, pad;
+    // Axis-aligned bounding box of the REAL particles (rounded outwards), used by the periodic-box kernels: a
+    // (i-group, j-tile) pair whose boxes are compact (cell-ordered input) shares ONE periodic image shift per
+    // component, so the per-pair wrap of Eq. 5's leading term is only paid where the boxes straddle half the box.
+    float lo[3], hi[3], pad2[2];
 };
+static_assert(sizeof(TileMeta) == 48, "TileMeta layout");
 //
 // Each tile carries its sources twice:
 //   (X, Y, Z, c)    mass-scaled copy for the FAR body:  c_j = m_j^(-1/2),  X_j = c_j x_j.  With
@@ -74,8 +79,8 @@ struct alignas(16) TileT {
     T x[TJ], y[TJ], z[TJ], m[TJ], h[TJ];
     TileMeta meta;
 };
-typedef TileT<float> TileF32;             // mixed path:  9232 B
-// fp64 path, 18448 B: the scaled copy is stored per source, (X, Y, Z, c) in 32 contiguous bytes, because the
+typedef TileT<float> TileF32;             // mixed path:  9264 B
+// fp64 path, 18480 B: the scaled copy is stored per source, (X, Y, Z, c) in 32 contiguous bytes, because the
 // fp64 far body handles ONE source per loop pass and every shared-memory load costs FP64-pipe issue time on
 // B200 (measured: ~1.8 clk per LDS.64, ~2.5 clk per LDS.128 next to a saturated DFMA stream): two LDS.128 per
 // source instead of four LDS.64.
@@ -87,8 +92,8 @@ struct alignas(16) TileF64 {
     double x[TJ], y[TJ], z[TJ], m[TJ], h[TJ];
     TileMeta meta;
 };
-static_assert(sizeof(TileF32) == 9 * TJ * 4 + 16, "TileF32 layout");
-static_assert(sizeof(TileF64) == 9 * TJ * 8 + 16, "TileF64 layout");
+static_assert(sizeof(TileF32) == 9 * TJ * 4 + sizeof(TileMeta), "TileF32 layout");
+static_assert(sizeof(TileF64) == 9 * TJ * 8 + sizeof(TileMeta), "TileF64 layout");
 static_assert(sizeof(TileF32) % 16 == 0 && sizeof(TileF64) % 16 == 0, "bulk copies need 16 B multiples");
 
 // Far iff the radial gap between the i-group and the j-tile exceeds the largest possible
@@ -100,6 +105,52 @@ __device__ __forceinline__ bool tile_is_far(float rminI, float rmaxI, float hmax
     const float gap = fmaxf(J.rmin - rmaxI, rminI - J.rmax);
     const float need = (hmaxI + J.hmax) * 1.0001f + 1.0e-5f * fmaxf(rmaxI, J.rmax);
     return gap > need;
+}
+
+// ---- periodic boxes (Eq. 5, leading image): one image shift per (i-group, j-tile) pair -----------------
+// With cell-ordered input (each tile a compact cell) the separations x_j - x_i of a tile pair span, per component, an
+// interval [dmin, dmax] much shorter than L.  With n = floor(dmin / L) every d' = d - n L lies in [lo, hi], lo in [0, L):
+//   hi <= L/2           all pairs take image n          (shift n L, no per-pair wrap)
+//   lo >= L/2           all pairs take image n + 1      (shift (n + 1) L, no per-pair wrap; needs hi <= 3L/2)
+//   otherwise           the interval straddles L/2: shift n L and, per pair, d' -= L where d' > L/2 (needs hi < 3L/2)
+// gmin = the smallest |leading-image separation| any pair of the two boxes can have in this component.
+// kind: 0 = no common shift possible (boxes too wide: unsorted input) or a softened pair is possible -> general body;
+//       1 = far, uniform shift;  2 = far, per-pair conditional subtraction.
+struct BoxShift {
+    int kind;
+    double s[3];
+};
+__device__ __forceinline__ BoxShift box_shift(const float (&loI)[3], const float (&hiI)[3], float hmaxI, const TileMeta& J, float L)
+{
+    BoxShift d;
+    d.kind = 1;
+    float g2 = 0.0f;
+    const float half = 0.5f * L, eps = 1.0e-5f * L;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const float dmin = (J.lo[c] - hiI[c]) - eps, dmax = (J.hi[c] - loI[c]) + eps;   // outward (fp32 rounding of the bounds)
+        const float n = floorf(dmin / L);
+        const float lo = dmin - n * L, hi = dmax - n * L;
+        float gmin;
+        if (!(dmax - dmin < 0.45f * L)) { d.kind = 0; d.s[c] = 0.0; continue; }       // also catches NaN / inf bounds
+        if (hi <= half - eps) { d.s[c] = (double)n * (double)L; gmin = lo; }
+        else if (lo >= half + eps) { d.s[c] = ((double)n + 1.0) * (double)L; gmin = fmaxf(L - hi, 0.0f); }
+        else { d.s[c] = (double)n * (double)L; gmin = fmaxf(fminf(lo, L - hi), 0.0f); if (d.kind == 1) d.kind = 2; }
+        g2 = fmaf(gmin, gmin, g2);
+    }
+    if (d.kind != 0) {
+        const float need = (hmaxI + J.hmax) * 1.0001f + 1.0e-5f * L;
+        if (!(g2 > need * need)) d.kind = 0;
+    }
+    return d;
+}
+
+// d -= period where d > half, both as bit patterns (valid for half > 0; d <= 0 never subtracts): one 64-bit integer compare
+// on the ALU pipe and ONE predicated DADD, instead of the compare + add + two selects the compiler makes of the C form.
+__device__ __forceinline__ void sub_if_above(double& d, long long half_bits, double neg_period)
+{
+    asm("{\n.reg .pred p;\nsetp.gt.s64 p, %1, %2;\n@p add.f64 %0, %0, %3;\n}"
+        : "+d"(d) : "l"(__double_as_longlong(d)), "l"(half_bits), "d"(neg_period));
 }
 
 // Never-taken branch on bit n of `zero` (always 0, unknown to the compiler): ends a basic block, which

@@ -17,6 +17,7 @@
 // block in shared memory: element (c, k) of thread t at acc[(c * R_I + k) * CTA_THREADS + t].
 #pragma once
 #include "common.cuh"
+#include "force_fp64.cuh"   // EWALD_NTRIPLETS / ewald_triplets (image-sum table of BOX = 2)
 
 namespace steps {
 
@@ -76,6 +77,28 @@ __device__ __forceinline__ void load_i_block(typename Path::IState& S, const dou
         rhi = fmaxf(rhi, __shfl_xor_sync(0xffffffffu, rhi, o));
         hh = fmaxf(hh, __shfl_xor_sync(0xffffffffu, hh, o));
     }
+}
+
+// Bounding box of the warp's 128 i-particles, rounded outwards (periodic boxes: box_shift in common.cuh).
+template <typename Path>
+__device__ __forceinline__ void warp_box(const typename Path::IState& S, float (&lo)[3], float (&hi)[3])
+{
+    const float inf = __int_as_float(0x7f800000);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { lo[c] = inf; hi[c] = -inf; }
+#pragma unroll
+    for (int k = 0; k < R_I; ++k) {
+        const double v[3] = {(double)S.x[k], (double)S.y[k], (double)S.z[k]};
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { lo[c] = fminf(lo[c], __double2float_rd(v[c])); hi[c] = fmaxf(hi[c], __double2float_ru(v[c])); }
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            lo[c] = fminf(lo[c], __shfl_xor_sync(0xffffffffu, lo[c], o));
+            hi[c] = fmaxf(hi[c], __shfl_xor_sync(0xffffffffu, hi[c], o));
+        }
 }
 
 // FarSums of the fp64 path are register sums (zeroed); those of the mixed path only carry the accumulator pointer.
@@ -138,6 +161,13 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ uint64_t full_bar[STAGES], empty_bar[STAGES];
     double* acc = reinterpret_cast<double*>(smem_raw + STAGES * STRIDE) + threadIdx.x;
+    __shared__ double img_tab[BOX == 2 ? 3 * EWALD_NTRIPLETS : 1];     // image offsets n L of Eq. 5 (BOX = 2 only)
+    if constexpr (BOX == 2) {
+        for (int q = threadIdx.x; q < EWALD_NTRIPLETS; q += CTA_THREADS) {
+            img_tab[3 * q] = ewald_triplets[q].x * box_L; img_tab[3 * q + 1] = ewald_triplets[q].y * box_L;
+            img_tab[3 * q + 2] = ewald_triplets[q].z * box_L;
+        }
+    }
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const long long* cum = BAND ? plan_cum(plan) : nullptr;
@@ -190,6 +220,8 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
         float rlo, rhi, hh;
         const long long i0 = i_begin + (long long)b * IB + warp * WARP_I + lane;
         load_i_block<Path>(S, pos, soft, N, i0, i_end, rlo, rhi, hh);
+        float blo[3], bhi[3];                                  // bounding box of the warp's i-particles (periodic boxes)
+        if constexpr (BOX == 1) warp_box<Path>(S, blo, bhi);
 #pragma unroll
         for (int q = 0; q < Path::NOUT * R_I; ++q) acc[q * CTA_THREADS] = 0.0;
 
@@ -202,9 +234,18 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
             mbar_wait(&full_bar[s], (it / STAGES) & 1);
             const Tile& T = *reinterpret_cast<const Tile*>(smem_raw + s * STRIDE);
             if constexpr (BOX == 1) {
-                Path::template near_box<true>(T, S, acc, box_L, box_invL);
+                // cell-ordered input: most tile pairs share one image shift and cannot be softened (box_shift in common.cuh)
+                const BoxShift bs = box_shift(blo, bhi, hh, T.meta, (float)box_L);
+                if (bs.kind == 0) {
+                    if (pending) { Path::far_flush(F, acc); pending = 0; }
+                    Path::template near_box<true>(T, S, acc, box_L, box_invL);
+                } else {
+                    if (bs.kind == 1) Path::template far_box<false>(T, S, F, zero, bs, box_L);
+                    else Path::template far_box<true>(T, S, F, zero, bs, box_L);
+                    if (++pending >= Path::FAR_TILES_PER_FLUSH) { Path::far_flush(F, acc); pending = 0; }
+                }
             } else if constexpr (BOX == 2) {
-                Path::near_images(T, S, acc, box_L, box_invL);
+                Path::near_images(T, S, acc, box_L, box_invL, img_tab);
             } else {
             // the decision is warp-uniform by construction (warp-reduced bounds); the vote tells the compiler so
             if (__all_sync(0xffffffffu, tile_is_far(rlo, rhi, hh, T.meta))) {
@@ -287,6 +328,114 @@ __global__ void __launch_bounds__(256) forces_band_reduce_kernel(const double* _
         }
         if (to_dd) { acc_hi[(long long)c * cnt + i] = hi; acc_lo[(long long)c * cnt + i] = lo; }
         else acc_out[(long long)c * cnt + i] = hi + lo;
+    }
+}
+
+// ---- split-j driver ------------------------------------------------------------------------------------------------
+// One i-GROUP of 128 particles (4 per lane) per CTA column, the j-range SPLIT over the 16 warps of the CTA (and over
+// gridDim.y CTAs): every warp holds the same 128 particles and sums its own work units -- (tile, range of `sub` sources)
+// pairs, unit u of the CTA going to warp u mod 16 -- straight from the tile records in global memory (L1/L2: a warp reads
+// one record at a time for all its lanes).  The warps' partial accelerations meet in shared memory and are added in fixed
+// warp order (TwoSum, double-double): row a3 of the hot path as north_star words it, "reduction of split-j partial
+// accelerations", deterministic.  Used where the ring driver's 2,048-particle i-blocks are too coarse:
+//   * small N (open boundary): N = 4,096 is 2 i-blocks x 16 tiles for 148 SMs in the ring driver; here 32 groups x 64 units;
+//   * periodic boxes (BOX = 1): the far/near/shift decision is per (warp's group, tile) and its cost varies by 2x; warps
+//     that share a tile ring wait for the slowest of them at every tile, warps with their own units do not.
+// gridDim = (groups, jsplit); partials (jsplit > 1): [group][jsplit][3 or 6][128] doubles, summed by forces_splitj_reduce.
+constexpr int SPLITJ_GROUP = WARP_I;                       // 128 i-particles per CTA
+
+template <typename Path, int BOX>
+__global__ void __launch_bounds__(CTA_THREADS, 1)
+forces_splitj_kernel(const double* __restrict__ pos, const double* __restrict__ soft, long long N,
+                     const typename Path::Tile* __restrict__ tiles, int nt, int sub, long long i_begin, long long i_end,
+                     double* __restrict__ acc_out, double* __restrict__ partials, int zero, double box_L, double box_invL)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double* acc_all = reinterpret_cast<double*>(smem_raw);                 // [NOUT * R_I][CTA_THREADS]
+    double* acc = acc_all + threadIdx.x;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const long long cnt = i_end - i_begin;
+    typename Path::IState S;
+    float rlo, rhi, hh;
+    const long long i0 = i_begin + (long long)blockIdx.x * SPLITJ_GROUP + lane;      // the same particles in every warp
+    load_i_block<Path>(S, pos, soft, N, i0, i_end, rlo, rhi, hh);
+    float blo[3], bhi[3];
+    if constexpr (BOX == 1) warp_box<Path>(S, blo, bhi);
+#pragma unroll
+    for (int q = 0; q < Path::NOUT * R_I; ++q) acc[q * CTA_THREADS] = 0.0;
+
+    const int per_tile = TJ / sub;
+    const long long units = (long long)nt * per_tile;
+    const long long u0 = (long long)blockIdx.y * units / gridDim.y, u1 = ((long long)blockIdx.y + 1) * units / gridDim.y;
+    typename Path::FarSums F;
+    init_far_sums<Path>(F, acc);
+    int pending = 0;
+    for (long long u = u0 + warp; u < u1; u += CTA_THREADS / 32) {
+        const typename Path::Tile& T = tiles[u / per_tile];
+        const int j0 = (int)(u % per_tile) * sub, j1 = j0 + sub;
+        const TileMeta meta = T.meta;
+        if constexpr (BOX == 1) {
+            const BoxShift bs = box_shift(blo, bhi, hh, meta, (float)box_L);
+            if (bs.kind == 0) {
+                if (pending) { Path::far_flush(F, acc); pending = 0; }
+                Path::template near_box<true>(T, S, acc, box_L, box_invL, j0, j1);
+            } else {
+                if (bs.kind == 1) Path::template far_box<false>(T, S, F, zero, bs, box_L, j0, j1);
+                else Path::template far_box<true>(T, S, F, zero, bs, box_L, j0, j1);
+                if (++pending >= Path::FAR_TILES_PER_FLUSH) { Path::far_flush(F, acc); pending = 0; }
+            }
+        } else {
+            if (__all_sync(0xffffffffu, tile_is_far(rlo, rhi, hh, meta))) {
+                Path::far(T, S, F, zero, j0, j1);
+                if (++pending >= Path::FAR_TILES_PER_FLUSH) { Path::far_flush(F, acc); pending = 0; }
+            } else {
+                if (pending) { Path::far_flush(F, acc); pending = 0; }
+                Path::near(T, S, acc, j0, j1);
+            }
+        }
+    }
+    if (pending) Path::far_flush(F, acc);
+    __syncthreads();
+
+    // fixed-order sum over the 16 warps: thread (c, k, l) owns component c of particle l + 32 k of the group
+    if (threadIdx.x < 3 * SPLITJ_GROUP) {
+        const int c = threadIdx.x / SPLITJ_GROUP, r = threadIdx.x % SPLITJ_GROUP, k = r / 32, l = r % 32;
+        double hi = 0.0, lo = 0.0;
+        for (int w = 0; w < CTA_THREADS / 32; ++w) {
+            const double v = acc_all[(c * R_I + k) * CTA_THREADS + w * 32 + l];
+            const double s = hi + v, bb = s - hi;
+            lo += (hi - (s - bb)) + (v - bb);                              // TwoSum
+            hi = s;
+            if (Path::NOUT == 6) lo += acc_all[((3 + c) * R_I + k) * CTA_THREADS + w * 32 + l];
+        }
+        const long long i = (long long)blockIdx.x * SPLITJ_GROUP + l + 32 * k;        // within [i_begin, i_end)
+        if (gridDim.y == 1) {
+            if (i < cnt) acc_out[(long long)c * cnt + i] = hi + lo;
+        } else {
+            double* rec = partials + (((long long)blockIdx.x * gridDim.y + blockIdx.y) * 6) * SPLITJ_GROUP;
+            rec[c * SPLITJ_GROUP + r] = hi; rec[(3 + c) * SPLITJ_GROUP + r] = lo;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(128) forces_splitj_reduce(const double* __restrict__ partials, int jsplit, long long cnt,
+                                                            double* __restrict__ acc_out)
+{
+    const int r = threadIdx.x, k = r / 32, l = r % 32;
+    const long long i = (long long)blockIdx.x * SPLITJ_GROUP + l + 32 * k;
+    if (i >= cnt) return;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        double hi = 0.0, lo = 0.0;
+        for (int s = 0; s < jsplit; ++s) {
+            const double* rec = partials + (((long long)blockIdx.x * jsplit + s) * 6) * SPLITJ_GROUP;
+            const double v = rec[c * SPLITJ_GROUP + r];
+            const double t = hi + v, bb = t - hi;
+            lo += (hi - (t - bb)) + (v - bb);
+            hi = t;
+            lo += rec[(3 + c) * SPLITJ_GROUP + r];
+        }
+        acc_out[(long long)c * cnt + i] = hi + lo;
     }
 }
 

@@ -68,16 +68,17 @@ __device__ __noinline__ double spline_g_soft_f64(double r2, double h)
 }
 
 // Integer triplets n with n.n <= 12: a superset of every n with |d - nL| < 2.6 L for |d_c| <= L/2 (Eq. 5 cut).
+// Entry 0 is (0, 0, 0), the leading image.
 constexpr int EWALD_NTRIPLETS = 179;
 struct EwaldTriplets {
     double3 v[EWALD_NTRIPLETS];
     constexpr EwaldTriplets() : v{}
     {
-        int c = 0;
+        int c = 1;
         for (int a = -3; a <= 3; ++a)
             for (int b = -3; b <= 3; ++b)
                 for (int d = -3; d <= 3; ++d)
-                    if (a * a + b * b + d * d <= 12) { v[c].x = a; v[c].y = b; v[c].z = d; ++c; }
+                    if (a * a + b * b + d * d <= 12 && (a != 0 || b != 0 || d != 0)) { v[c].x = a; v[c].y = b; v[c].z = d; ++c; }
     }
 };
 __constant__ double3 ewald_triplets[EWALD_NTRIPLETS];
@@ -150,13 +151,14 @@ struct Fp64Path {
         far_zero(F);
     }
 
-    static __device__ __forceinline__ void far(const Tile& T, const IState& S, FarSums& F, int zero)
+    // [j0, j1): the sources of the tile to sum (the whole tile in the ring driver; a part of it in the split-j driver).
+    static __device__ __forceinline__ void far(const Tile& T, const IState& S, FarSums& F, int zero, int j0 = 0, int j1 = TJ)
     {
         constexpr double A = 1.4;
         constexpr double C0 = 1.0 / STEPS_FP64_FOLD - (1.0 - A) * (1.0 - A);   // (u - A)^2 + C0 = 1/1.875 at u = 1
         double (&ax)[R_I] = F.ax, (&ay)[R_I] = F.ay, (&az)[R_I] = F.az;
 #pragma unroll 1
-        for (int j = 0; j < TJ; ++j) {
+        for (int j = j0; j < j1; ++j) {
             const double2 XY = *reinterpret_cast<const double2*>(&T.far[j].X);
             const double2 ZC = *reinterpret_cast<const double2*>(&T.far[j].Z);
             const double X = XY.x, Y = XY.y, Z = ZC.x, C = ZC.y;
@@ -189,6 +191,61 @@ struct Fp64Path {
         }
     }
 
+    // Far body in a periodic box (Eq. 5, leading image) for a tile pair with a common image shift (box_shift in common.cuh):
+    // the shift goes onto the source, X' = X_j - c_j s (3 DFMA per source, shared by the 4 particles), then the body of far().
+    // WRAP: the pair's boxes straddle half the box in some component: d' -= L where d' > L/2, in scaled units
+    // (c_j L, c_j L/2 per source), the test as an integer compare of the bit patterns (ALU pipe; d' <= 0 never subtracts).
+    template <bool WRAP>
+    static __device__ __forceinline__ void far_box(const Tile& T, const IState& S, FarSums& F, int zero, const BoxShift& bs, double L,
+                                                   int j0 = 0, int j1 = TJ)
+    {
+        constexpr double A = 1.4;
+        constexpr double C0 = 1.0 / STEPS_FP64_FOLD - (1.0 - A) * (1.0 - A);
+        double (&ax)[R_I] = F.ax, (&ay)[R_I] = F.ay, (&az)[R_I] = F.az;
+        const double sx = bs.s[0], sy = bs.s[1], sz = bs.s[2];
+#pragma unroll 1
+        for (int j = j0; j < j1; ++j) {
+            const double2 XY = *reinterpret_cast<const double2*>(&T.far[j].X);
+            const double2 ZC = *reinterpret_cast<const double2*>(&T.far[j].Z);
+            const double C = ZC.y;
+            const double X = fma(-sx, C, XY.x), Y = fma(-sy, C, XY.y), Z = fma(-sz, C, ZC.x);
+            double dX[R_I], dY[R_I], dZ[R_I], r2[R_I], y0[R_I], y2[R_I], w[R_I];
+            STEPS_STAGE_FENCE(zero, 0);
+#pragma unroll
+            for (int k = 0; k < R_I; ++k) dX[k] = fma(-S.x[k], C, X);
+#pragma unroll
+            for (int k = 0; k < R_I; ++k) dY[k] = fma(-S.y[k], C, Y);
+#pragma unroll
+            for (int k = 0; k < R_I; ++k) dZ[k] = fma(-S.z[k], C, Z);
+            if (WRAP) {
+                const double ncL = -C * L;
+                const long long hb = __double_as_longlong(-0.5 * ncL);
+#pragma unroll
+                for (int k = 0; k < R_I; ++k) {
+                    sub_if_above(dX[k], hb, ncL); sub_if_above(dY[k], hb, ncL); sub_if_above(dZ[k], hb, ncL);
+                }
+            }
+            STEPS_STAGE_FENCE(zero, 1);
+#pragma unroll
+            for (int k = 0; k < R_I; ++k) r2[k] = fma(dZ[k], dZ[k], fma(dY[k], dY[k], dX[k] * dX[k]));
+#pragma unroll
+            for (int k = 0; k < R_I; ++k) y0[k] = rsqrt_seed(r2[k]);
+#pragma unroll
+            for (int k = 0; k < R_I; ++k) {
+                y2[k] = y0[k] * y0[k];
+                w[k] = fma(r2[k], y2[k], -A);
+                y2[k] = y0[k] * y2[k];
+                w[k] = fma(w[k], w[k], C0);
+                w[k] = y2[k] * w[k];
+            }
+            STEPS_STAGE_FENCE(zero, 2);
+#pragma unroll
+            for (int k = 0; k < R_I; ++k) {
+                ax[k] = fma(dX[k], w[k], ax[k]); ay[k] = fma(dY[k], w[k], ay[k]); az[k] = fma(dZ[k], w[k], az[k]);
+            }
+        }
+    }
+
     // Leading periodic image of a separation component (Eq. 5, quasi-periodic boundary): d - L rint(d/L)
     // with the round-to-nearest-even shift trick (valid for |d/L| < 2^51), 3 FP64 instructions, no conversion.
     static __device__ __forceinline__ double wrap(double d, double L, double invL)
@@ -198,56 +255,102 @@ struct Fp64Path {
         return __fma_rn(-L, n, d);
     }
 
-    static __device__ __forceinline__ void near(const Tile& T, const IState& S, double* acc) { near_box<false>(T, S, acc, 0.0, 0.0); }
+    static __device__ __forceinline__ void near(const Tile& T, const IState& S, double* acc, int j0 = 0, int j1 = TJ)
+    {
+        near_box<false>(T, S, acc, 0.0, 0.0, j0, j1);
+    }
 
     // Periodic image sum, Eq. 5 (L65-70) with the paper's cut: every image x - nL of the separation with
     // |x - nL| < 2.6 L contributes through the pair law.  Around the nearest image (|d_c| <= L/2) these are among the
-    // triplets with |n| < 2.6 + sqrt(3)/2, i.e. n.n <= 12: 179 of them (constant-memory table ewald_triplets); the loop
-    // walks these and applies the cut per image (row 8(f)-3, second part).  The 4 register-blocked i-particles run in
-    // lockstep inside the image loop.
-    static __device__ __forceinline__ void near_images(const Tile& T, const IState& S, double* acc, double L, double invL)
+    // triplets with |n| < 2.6 + sqrt(3)/2, i.e. n.n <= 12: 179 of them; `tab` holds their offsets n L (3 doubles each,
+    // entry 0 = the nearest image) in shared memory.  Every image other than the nearest is at least L/2 away, so when
+    // h_i + h_j <= L/2 (any sane softening) only the nearest image can be softened: it goes through the near body
+    // (spline test), the other 178 through a branch-free Newtonian body -- 3 DADD, 3 for r^2, the 5-instruction r^-3 of
+    // the far body, 3 DFMA = 14 FP64-pipe instructions per image -- with the cut applied as an integer compare of the
+    // bit patterns (ALU pipe, not FP64) and m_j multiplied once per pair.  Pairs with h_i + h_j > L/2 take the general loop.
+    static __device__ __forceinline__ void near_images(const Tile& T, const IState& S, double* acc, double L, double invL,
+                                                       const double* __restrict__ tab)
     {
-        const double cut2 = (2.6 * L) * (2.6 * L);
-        double ax[R_I], ay[R_I], az[R_I];
-#pragma unroll
-        for (int k = 0; k < R_I; ++k) ax[k] = ay[k] = az[k] = 0.0;
+        constexpr double A = 1.4;
+        constexpr double C0 = 1.0 / STEPS_FP64_FOLD - (1.0 - A) * (1.0 - A);
+        const double cut2 = (2.6 * L) * (2.6 * L), halfL = 0.5 * L;
+        const long long cut2_bits = __double_as_longlong(cut2);
 #pragma unroll 1
         for (int j = 0; j < TJ; ++j) {
             const double xj = T.x[j], yj = T.y[j], zj = T.z[j], mq = T.m[j], hj = T.h[j];
             if (mq == 0.0) continue;                                   // pads and massless sources (warp-uniform)
-            double dx[R_I], dy[R_I], dz[R_I], hs2[R_I], hs[R_I];
+            // px: sum over the images of s v, in units of 1 / STEPS_FP64_FOLD (the far body's r^-3 carries that factor)
+            double dx[R_I], dy[R_I], dz[R_I], px[R_I], py[R_I], pz[R_I];
+            bool newtonian = true;
 #pragma unroll
             for (int k = 0; k < R_I; ++k) {
                 dx[k] = wrap(xj - S.x[k], L, invL); dy[k] = wrap(yj - S.y[k], L, invL); dz[k] = wrap(zj - S.z[k], L, invL);
-                hs[k] = S.h[k] + hj; hs2[k] = hs[k] * hs[k];
+                const double hs = S.h[k] + hj;
+                newtonian = newtonian && hs <= halfL;
+                const double r2 = fma(dz[k], dz[k], fma(dy[k], dy[k], dx[k] * dx[k]));
+                double s0 = rcube(r2);                                // the nearest image: Eq. 4 in full (readings #2, #4)
+                if (r2 < hs * hs || r2 == 0.0) s0 = (r2 == 0.0) ? 0.0 : spline_g_soft_f64(r2, hs);
+                s0 *= 1.0 / STEPS_FP64_FOLD;
+                px[k] = dx[k] * s0; py[k] = dy[k] * s0; pz[k] = dz[k] * s0;
             }
+            if (__all_sync(0xffffffffu, newtonian)) {
 #pragma unroll 1
-            for (int c = 0; c < EWALD_NTRIPLETS; ++c) {
-                const double ox = ewald_triplets[c].x * L, oy = ewald_triplets[c].y * L, oz = ewald_triplets[c].z * L;
+                for (int c = 1; c < EWALD_NTRIPLETS; ++c) {
+                    const double ox = tab[3 * c], oy = tab[3 * c + 1], oz = tab[3 * c + 2];
+                    double vx[R_I], vy[R_I], vz[R_I], r2[R_I], y0[R_I], y2[R_I], w[R_I];
 #pragma unroll
-                for (int k = 0; k < R_I; ++k) {
-                    const double vx = dx[k] - ox, vy = dy[k] - oy, vz = dz[k] - oz;
-                    const double r2 = fma(vz, vz, fma(vy, vy, vx * vx));
-                    double s = mq * rcube(r2);
-                    if (r2 < hs2[k] || r2 == 0.0) s = (r2 == 0.0) ? 0.0 : mq * spline_g_soft_f64(r2, hs[k]);
-                    if (!(r2 < cut2)) s = 0.0;                         // "|x - nL| < 2.6 L" (strict, as printed)
-                    ax[k] = fma(vx, s, ax[k]); ay[k] = fma(vy, s, ay[k]); az[k] = fma(vz, s, az[k]);
+                    for (int k = 0; k < R_I; ++k) { vx[k] = dx[k] - ox; vy[k] = dy[k] - oy; vz[k] = dz[k] - oz; }
+#pragma unroll
+                    for (int k = 0; k < R_I; ++k) r2[k] = fma(vz[k], vz[k], fma(vy[k], vy[k], vx[k] * vx[k]));
+#pragma unroll
+                    for (int k = 0; k < R_I; ++k) y0[k] = rsqrt_seed(r2[k]);
+#pragma unroll
+                    for (int k = 0; k < R_I; ++k) {
+                        y2[k] = y0[k] * y0[k];
+                        w[k] = fma(r2[k], y2[k], -A);
+                        y2[k] = y0[k] * y2[k];
+                        w[k] = fma(w[k], w[k], C0);
+                        w[k] = y2[k] * w[k];
+                        if (!(__double_as_longlong(r2[k]) < cut2_bits)) w[k] = 0.0;   // "|x - nL| < 2.6 L", strict (r2 >= 0)
+                    }
+#pragma unroll
+                    for (int k = 0; k < R_I; ++k) {
+                        px[k] = fma(vx[k], w[k], px[k]); py[k] = fma(vy[k], w[k], py[k]); pz[k] = fma(vz[k], w[k], pz[k]);
+                    }
+                }
+            } else {                                                   // some h_i + h_j > L/2: every image through Eq. 4
+#pragma unroll 1
+                for (int c = 1; c < EWALD_NTRIPLETS; ++c) {
+                    const double ox = tab[3 * c], oy = tab[3 * c + 1], oz = tab[3 * c + 2];
+#pragma unroll
+                    for (int k = 0; k < R_I; ++k) {
+                        const double vx = dx[k] - ox, vy = dy[k] - oy, vz = dz[k] - oz;
+                        const double r2 = fma(vz, vz, fma(vy, vy, vx * vx));
+                        const double hs = S.h[k] + hj;
+                        double s = rcube(r2);
+                        if (r2 < hs * hs) s = spline_g_soft_f64(r2, hs);
+                        if (!(r2 < cut2)) s = 0.0;
+                        s *= 1.0 / STEPS_FP64_FOLD;
+                        px[k] = fma(vx, s, px[k]); py[k] = fma(vy, s, py[k]); pz[k] = fma(vz, s, pz[k]);
+                    }
                 }
             }
-        }
+            const double mf = STEPS_FP64_FOLD * mq;
 #pragma unroll
-        for (int k = 0; k < R_I; ++k) { flush(acc, 0, k, ax[k]); flush(acc, 1, k, ay[k]); flush(acc, 2, k, az[k]); }
+            for (int k = 0; k < R_I; ++k) { flush(acc, 0, k, mf * px[k]); flush(acc, 1, k, mf * py[k]); flush(acc, 2, k, mf * pz[k]); }
+        }
     }
 
     // PERIODIC: every separation is replaced by its leading image in a cubic box of side L (row 8(f)-3).
     template <bool PERIODIC>
-    static __device__ __forceinline__ void near_box(const Tile& T, const IState& S, double* acc, double L, double invL)
+    static __device__ __forceinline__ void near_box(const Tile& T, const IState& S, double* acc, double L, double invL,
+                                                    int j0 = 0, int j1 = TJ)
     {
         double ax[R_I], ay[R_I], az[R_I];
 #pragma unroll
         for (int k = 0; k < R_I; ++k) ax[k] = ay[k] = az[k] = 0.0;
 #pragma unroll 1
-        for (int j = 0; j < TJ; ++j) {
+        for (int j = j0; j < j1; ++j) {
             const double xj = T.x[j], yj = T.y[j], zj = T.z[j], mq = T.m[j], hj = T.h[j];
 #pragma unroll
             for (int k = 0; k < R_I; ++k) {

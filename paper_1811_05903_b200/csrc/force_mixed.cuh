@@ -81,7 +81,8 @@ struct MixedPath {
     static __device__ __forceinline__ void far_zero(FarSums&) {}
     static __device__ __forceinline__ void far_flush(FarSums&, double*) {}
 
-    static __device__ __forceinline__ void far(const Tile& T, const IState& S, FarSums& F, int /*zero*/)
+    // [j0, j1): the sources of the tile to sum (multiples of 4; the whole tile in the ring driver).
+    static __device__ __forceinline__ void far(const Tile& T, const IState& S, FarSums& F, int /*zero*/, int j0 = 0, int j1 = TJ)
     {
         double* acc = F.acc;
         static_assert(R_I % 2 == 0, "i-particles are packed in pairs");
@@ -95,7 +96,7 @@ struct MixedPath {
             ax[p] = ay[p] = az[p] = 0ull;
         }
 STEPS_UNROLL(STEPS_FAR_UNROLL)
-        for (int j = 0; j < TJ; j += 4) {
+        for (int j = j0; j < j1; j += 4) {
             const float4 X = *reinterpret_cast<const float4*>(&T.X[j]);
             const float4 Y = *reinterpret_cast<const float4*>(&T.Y[j]);
             const float4 Z = *reinterpret_cast<const float4*>(&T.Z[j]);
@@ -109,6 +110,70 @@ STEPS_UNROLL(STEPS_FAR_UNROLL)
 #pragma unroll
                 for (int p = 0; p < NP; ++p) {
                     const u64 dX = fma2(nx[p], cq, Xq), dY = fma2(ny[p], cq, Yq), dZ = fma2(nz[p], cq, Zq);
+                    const u64 r2 = fma2(dZ, dZ, fma2(dY, dY, mul2(dX, dX)));
+                    float a, b;
+                    unpack2(r2, a, b);
+                    const u64 y = pack2(rsqrt_approx(a), rsqrt_approx(b));
+                    const u64 y3 = mul2(mul2(y, y), y);
+                    ax[p] = fma2(dX, y3, ax[p]);
+                    ay[p] = fma2(dY, y3, ay[p]);
+                    az[p] = fma2(dZ, y3, az[p]);
+                }
+            }
+        }
+#pragma unroll
+        for (int p = 0; p < NP; ++p) {
+            float lo, hi;
+            unpack2(ax[p], lo, hi); flush(acc, 0, 2 * p, lo); flush(acc, 0, 2 * p + 1, hi);
+            unpack2(ay[p], lo, hi); flush(acc, 1, 2 * p, lo); flush(acc, 1, 2 * p + 1, hi);
+            unpack2(az[p], lo, hi); flush(acc, 2, 2 * p, lo); flush(acc, 2, 2 * p + 1, hi);
+        }
+    }
+
+    // Far body in a periodic box (Eq. 5, leading image) for a tile pair with a common image shift (box_shift in common.cuh):
+    // the shift goes onto the source, X' = X_j - c_j s, then the body of far().  WRAP: the boxes straddle half the box in some
+    // component: the scaled differences are wrapped per pair with the source's own period c_j L (3 packed instructions each).
+    template <bool WRAP>
+    static __device__ __forceinline__ void far_box(const Tile& T, const IState& S, FarSums& F, int /*zero*/, const BoxShift& bs, double Ld,
+                                                   int j0 = 0, int j1 = TJ)
+    {
+        double* acc = F.acc;
+        constexpr int NP = R_I / 2;
+        const float sx = (float)bs.s[0], sy = (float)bs.s[1], sz = (float)bs.s[2], L = (float)Ld;
+        u64 nx[NP], ny[NP], nz[NP], ax[NP], ay[NP], az[NP];
+#pragma unroll
+        for (int p = 0; p < NP; ++p) {
+            nx[p] = pack2(-S.x[2 * p], -S.x[2 * p + 1]);
+            ny[p] = pack2(-S.y[2 * p], -S.y[2 * p + 1]);
+            nz[p] = pack2(-S.z[2 * p], -S.z[2 * p + 1]);
+            ax[p] = ay[p] = az[p] = 0ull;
+        }
+        const u64 SHIFT = pack2(12582912.0f, 12582912.0f), NSHIFT = pack2(-12582912.0f, -12582912.0f);   // 1.5 * 2^23
+#pragma unroll 1
+        for (int j = j0; j < j1; j += 4) {
+            const float4 X = *reinterpret_cast<const float4*>(&T.X[j]);
+            const float4 Y = *reinterpret_cast<const float4*>(&T.Y[j]);
+            const float4 Z = *reinterpret_cast<const float4*>(&T.Z[j]);
+            const float4 Cc = *reinterpret_cast<const float4*>(&T.c[j]);
+            const float Xs[4] = {X.x, X.y, X.z, X.w}, Ys[4] = {Y.x, Y.y, Y.z, Y.w};
+            const float Zs[4] = {Z.x, Z.y, Z.z, Z.w}, Cs[4] = {Cc.x, Cc.y, Cc.z, Cc.w};
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const float c = Cs[q ^ STEPS_C_SWIZZLE];
+                const float xs = fmaf(-sx, c, Xs[q]), ys = fmaf(-sy, c, Ys[q]), zs = fmaf(-sz, c, Zs[q]);
+                const u64 cq = pack2(c, c), Xq = pack2(xs, xs), Yq = pack2(ys, ys), Zq = pack2(zs, zs);
+                // pads (c = STEPS_PAD_C32) keep their parked difference: period 0, so that dX.dX still overflows to +inf
+                const bool live = c < 1.0e17f;
+                const float cL = live ? c * L : 0.0f, icL = live ? __frcp_rn(c * L) : 0.0f;
+                const u64 ncL = pack2(-cL, -cL), icL2 = pack2(icL, icL);
+#pragma unroll
+                for (int p = 0; p < NP; ++p) {
+                    u64 dX = fma2(nx[p], cq, Xq), dY = fma2(ny[p], cq, Yq), dZ = fma2(nz[p], cq, Zq);
+                    if (WRAP) {
+                        dX = fma2(ncL, add2(fma2(dX, icL2, SHIFT), NSHIFT), dX);
+                        dY = fma2(ncL, add2(fma2(dY, icL2, SHIFT), NSHIFT), dY);
+                        dZ = fma2(ncL, add2(fma2(dZ, icL2, SHIFT), NSHIFT), dZ);
+                    }
                     const u64 r2 = fma2(dZ, dZ, fma2(dY, dY, mul2(dX, dX)));
                     float a, b;
                     unpack2(r2, a, b);
@@ -146,11 +211,15 @@ STEPS_UNROLL(STEPS_FAR_UNROLL)
         return fma2(negL, n, d);
     }
 
-    static __device__ __forceinline__ void near(const Tile& T, const IState& S, double* acc) { near_box<false>(T, S, acc, 0.0, 0.0); }
+    static __device__ __forceinline__ void near(const Tile& T, const IState& S, double* acc, int j0 = 0, int j1 = TJ)
+    {
+        near_box<false>(T, S, acc, 0.0, 0.0, j0, j1);
+    }
 
     // PERIODIC: every separation is replaced by its leading image in a cubic box of side L (row 8(f)-3).
     template <bool PERIODIC>
-    static __device__ __forceinline__ void near_box(const Tile& T, const IState& S, double* acc, double Ld, double invLd)
+    static __device__ __forceinline__ void near_box(const Tile& T, const IState& S, double* acc, double Ld, double invLd,
+                                                    int j0 = 0, int j1 = TJ)
     {
         const u64 negL = pack2(-(float)Ld, -(float)Ld), invL = pack2((float)invLd, (float)invLd);
         u64 xi[R_I], yi[R_I], zi[R_I], hi[R_I], ax[R_I], ay[R_I], az[R_I];
@@ -161,7 +230,7 @@ STEPS_UNROLL(STEPS_FAR_UNROLL)
             ax[k] = ay[k] = az[k] = 0ull;
         }
 #pragma unroll 2
-        for (int j = 0; j < TJ; j += 2) {
+        for (int j = j0; j < j1; j += 2) {
             const u64 xj = *reinterpret_cast<const u64*>(&T.x[j]), yj = *reinterpret_cast<const u64*>(&T.y[j]);
             const u64 zj = *reinterpret_cast<const u64*>(&T.z[j]), mj = *reinterpret_cast<const u64*>(&T.m[j]);
             const u64 hj = *reinterpret_cast<const u64*>(&T.h[j]);

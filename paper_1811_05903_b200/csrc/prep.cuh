@@ -79,7 +79,17 @@ __global__ void __launch_bounds__(TJ) prep_tiles(const double* __restrict__ pos,
     if (force_near) hh = __int_as_float(0x7f800000);
     block_bounds(rlo, rhi, hh);
     if (threadIdx.x == 0) {
-        T.meta.rmin = rlo; T.meta.rmax = rhi; T.meta.hmax = hh; T.meta.pad = 0.0f;
+        T.meta.rmin = rlo; T.meta.rmax = rhi; T.meta.hmax = hh; T.meta.pad = 0.0f; T.meta.pad2[0] = T.meta.pad2[1] = 0.0f;
+    }
+    // bounding box (three more rounds of the same reduction; prep is O(N) and < 0.01 % of an evaluation)
+    const float inf = __int_as_float(0x7f800000);
+    const double cs[3] = {x, y, z};
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        __syncthreads();                                     // block_bounds' shared scratch is reused
+        float lo = real ? __double2float_rd(cs[c]) : inf, hi = real ? __double2float_ru(cs[c]) : -inf, unused = 0.0f;
+        block_bounds(lo, hi, unused);
+        if (threadIdx.x == 0) { T.meta.lo[c] = lo; T.meta.hi[c] = hi; }
     }
 }
 

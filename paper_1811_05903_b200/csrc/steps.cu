@@ -37,6 +37,7 @@ constexpr int MAX_GRID = 148 * 4;
 constexpr int SYM_MIN_BLOCKS = 64;
 std::atomic<long long> g_sym_panel_items{16384};
 std::atomic<int> g_sym_enabled{1};
+std::atomic<int> g_splitj{1};           // 0 = never use the split-j driver (testing)
 
 struct Workspace {
     void* tiles = nullptr;          // max(sizeof(TileF32), sizeof(TileF64)) * ntiles (padded to whole blocks)
@@ -237,6 +238,53 @@ int launch_forces_sym(const double* pos, const double* mass, const double* soft,
     return STEPS_OK;
 }
 
+// Split-j driver (force_driver.cuh): one 128-particle group per CTA column, the j-range split over the warps and over
+// `jsplit` CTAs.  The source sub-range per work unit shrinks (256 -> 64) until there are about two units per resident warp.
+template <typename Path, int BOX>
+int launch_splitj(const double* pos, const double* soft, long long N, const typename Path::Tile* tiles, int nt,
+                  long long i_begin, long long i_end, double* acc_out, cudaStream_t st, Workspace& w, double L)
+{
+    const long long cnt = i_end - i_begin;
+    const long long groups = (cnt + SPLITJ_GROUP - 1) / SPLITJ_GROUP;
+    const long long warps = (long long)w.num_sms * (CTA_THREADS / 32);
+    int sub = TJ;
+    while (sub > 64 && groups * nt * (TJ / sub) < 4 * warps) sub /= 2;
+    const long long units = (long long)nt * (TJ / sub);                      // per group
+    // one CTA per SM is resident (512 threads, up to 96 KiB of accumulators): with fewer groups than SMs the j-range is split
+    // over floor(SMs / groups) CTAs so that the whole grid is ONE wave; with more groups than SMs there is nothing to split
+    long long jsplit = groups < w.num_sms ? w.num_sms / groups : 1;
+    jsplit = std::max(1ll, std::min(jsplit, units / (CTA_THREADS / 32)));
+    const long long rec_cap = (long long)(partial_bytes(N) / (sizeof(double) * 6 * SPLITJ_GROUP));
+    if (groups * jsplit > rec_cap) jsplit = std::max(1ll, rec_cap / groups);
+    if (groups > 0x7fffffffll || jsplit > 65535) return STEPS_EINVAL;
+    auto kern = forces_splitj_kernel<Path, BOX>;
+    constexpr int smem = Path::NOUT * R_I * CTA_THREADS * (int)sizeof(double);
+    static bool attr_set = false;                                                // per instantiation
+    if (!attr_set) { STEPS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); attr_set = true; }
+    const bool prof = g_profile.load() != 0;
+    if (prof) {
+        if (!w.ev0) { STEPS_CUDA(cudaEventCreate(&w.ev0)); STEPS_CUDA(cudaEventCreate(&w.ev1)); }
+        STEPS_CUDA(cudaEventRecord(w.ev0, st));
+    }
+    kern<<<dim3((unsigned)groups, (unsigned)jsplit), CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, sub, i_begin, i_end, acc_out,
+                                                                                w.partials, 0, L, L > 0.0 ? 1.0 / L : 0.0);
+    g_launches++;
+    if (jsplit > 1) {
+        forces_splitj_reduce<<<(unsigned)groups, SPLITJ_GROUP, 0, st>>>(w.partials, (int)jsplit, cnt, acc_out);
+        g_launches++;
+    }
+    if (prof) { STEPS_CUDA(cudaEventRecord(w.ev1, st)); w.ev_valid = true; }
+    STEPS_CUDA(cudaGetLastError());
+    return STEPS_OK;
+}
+
+// The ring driver's (i-block, j-tile) items are too few to fill the SMs below this many per SM: split-j driver instead,
+// as long as its groups fit one wave of CTAs (N <= 128 x SMs = 18,944 on B200; measured 3.7x at N = 4,096).
+inline bool use_splitj(long long cnt, long long N, const Workspace& w)
+{
+    return g_splitj.load() != 0 && (cnt + SPLITJ_GROUP - 1) / SPLITJ_GROUP <= w.num_sms && nblocks_of(cnt) * ntiles_of(N) < 8ll * w.num_sms;
+}
+
 template <typename Path>
 int launch_forces(const double* pos, const double* mass, const double* soft, long long N, long long i_begin,
                   long long i_end, double* acc_out, cudaStream_t st, Workspace& w, int& grid_cache)
@@ -251,6 +299,8 @@ int launch_forces(const double* pos, const double* mass, const double* soft, lon
     g_launches++;
     const long long cnt = i_end - i_begin;
     const int nb = (int)nblocks_of(cnt);
+    if (g_driver.load() == 0 && use_splitj(cnt, N, w))
+        return launch_splitj<Path, 0>(pos, soft, N, tiles, nt, i_begin, i_end, acc_out, st, w, 0.0);
     if (g_driver.load() == 1) {
         const int smem = stage_stride((int)sizeof(Tile)) + Path::NOUT * R_I * CTA_THREADS * (int)sizeof(double);
         STEPS_CUDA(cudaFuncSetAttribute(forces_v1_kernel<Path>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
@@ -308,6 +358,14 @@ int launch_forces_periodic(const double* pos, const double* mass, const double* 
     int rc = claim_scratch(w, st);
     if (rc != STEPS_OK) return rc;
     prep_tiles<Tile><<<nt, TJ, 0, st>>>(pos, mass, soft, N, tiles, nullptr);
+    g_launches++;
+    if constexpr (BOX == 1) {                      // leading image: per-(group, tile) decisions of uneven cost -> split-j driver
+        if (g_splitj.load() != 0) {
+            rc = launch_splitj<Path, 1>(pos, soft, N, tiles, nt, 0, N, acc_out, st, w, L);
+            if (rc != STEPS_OK) return rc;
+            return release_scratch(w, st);
+        }
+    }
     const int nb = (int)nblocks_of(N);
     constexpr int smem = persistent_smem_bytes<Path, STAGES>();
     auto kern = forces_persistent_kernel<Path, STAGES, BOX>;
@@ -316,7 +374,7 @@ int launch_forces_periodic(const double* pos, const double* mass, const double* 
     const int P = grid_cache;
     kern<<<P, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, 0, N, nb, w.partials, 0, L, 1.0 / L, nullptr);
     forces_reduce_kernel<Path::NOUT><<<(int)((N + 255) / 256), 256, 0, st>>>(w.partials, nt, nb, P, N, acc_out);
-    g_launches += 3;
+    g_launches += 2;
     STEPS_CUDA(cudaGetLastError());
     return release_scratch(w, st);
 }
@@ -638,6 +696,7 @@ int steps_set_option(const char* key, long long value)
     if (std::strcmp(key, "driver") == 0) { g_driver = (int)value; return STEPS_OK; }
     if (std::strcmp(key, "profile") == 0) { g_profile = (int)value; return STEPS_OK; }
     if (std::strcmp(key, "sym") == 0) { g_sym_enabled = (int)value; return STEPS_OK; }
+    if (std::strcmp(key, "splitj") == 0) { g_splitj = (int)value; return STEPS_OK; }
     if (std::strcmp(key, "sym_panel_items") == 0) {
         if (value < 1) return STEPS_EINVAL;
         g_sym_panel_items = value;
