@@ -16,9 +16,10 @@ mixed path (the FP32 target), `paths.fp64` carries the fp64 path.  One JSON line
     ("profile" option) for the roofline figure;
   * clocks / throttle reasons are sampled through NVML during the timed region;
   * `cpu_baseline` / `--impl reference`: the CPU oracle as it stands, on a bounded i-sample.
-  * N > 1 GPUs (torchrun): the paper's decomposition (L139) -- each rank evaluates the forces of
-    its i-range against all sources (steps_forces_range), kicks/drifts its slice, and the drifted
-    positions are all-gathered (NCCL): total work fixed => "strong" scaling.
+  * N > 1 GPUs (torchrun): the paper's decomposition (L135-139) with the i-blocks dealt round-robin
+    (shard.py) -- each rank evaluates the forces of its blocks against all sources
+    (steps_forces_blocks), kicks/drifts its particles, and the drifted positions are all-gathered
+    (NCCL): total work fixed => "strong" scaling.
 """
 from __future__ import annotations
 
@@ -261,13 +262,16 @@ def main():
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
     torch.cuda.set_device(local_rank)
     if world > 1:
+        # NCCL's communicator/topology log (NVLS, rings, ranks) to stderr: stdout carries the one JSON line
+        os.environ.setdefault("NCCL_DEBUG", "INFO")
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT,ENV")
+        os.environ.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     args.warmup = max(args.warmup, 3)
 
     n = args.n or 1048576
     ps = synth.g0(n, synth.SEED_BASE + 3)          # config 3 (identical on every rank: seeded)
-    b, e = shard.i_range(rank, world, n)
-    cnt = e - b
+    cnt = shard.owned_count(rank, world, n)        # N > 1: the rank's round-robin blocks (shard.py)
     pos = torch.from_numpy(ps.pos).cuda()           # replicated sources
     mass, soft = torch.from_numpy(ps.mass).cuda(), torch.from_numpy(ps.soft).cuda()
     S.steps_reserve(n)
@@ -301,17 +305,13 @@ def main():
                     S.steps_kdk_step(x, v, acc, mass, soft, co)
                     S.steps_momentum(v, mass, mom)
             else:
-                xl = x[:, b:e].contiguous()
-                vl, al = torch.zeros_like(xl), torch.empty(3 * cnt, dtype=torch.float64, device="cuda")
-                ml = mass[b:e].contiguous()
-                S.steps_forces_range(x, mass, soft, b, e, al, mixed=mixed)
-                state = {"x": x}
+                sh = shard.ShardedStep(S, rank, world, x, torch.zeros_like(x), mass, soft, mixed)
+                sh.forces()
 
                 def step():
-                    S.steps_kick_drift(xl, vl, al, co)
-                    state["x"] = shard.gather_soa(xl, n)
-                    S.steps_forces_range(state["x"], mass, soft, b, e, al, mixed=mixed)
-                    S.steps_momentum(vl, ml, mom)
+                    sh.step(co)
+                    if sh.cnt:
+                        S.steps_momentum(sh.v, sh.m, mom)
 
             for _ in range(args.warmup):
                 step()
@@ -395,7 +395,7 @@ def main():
         "config": {"workload": f"config3: compactified g0 set (S^3 stereographic, m~(1+r^2/4R^2)^3, eps_i=0.01(m_i/m_min)^(1/3)), N={n}, "
                                f"one steps_kdk_step (kick+drift+prep+force+reduce) + momentum per step",
                    "headline_path": head, "l2": "256 MiB flush write between timed steps (inputs 42 MB fit L2; ALU-bound)",
-                   "i_sharding": "none" if world == 1 else f"i-range per rank (PAPER L139), all-gather of positions, {world} ranks",
+                   "i_sharding": "none" if world == 1 else f"i-blocks of 2048 dealt round-robin to {world} ranks (PAPER L135-139, SURVEY 8(e)), all-gather of positions",
                    "persistent_grid": {p: S.steps_persistent_grid(p == "mixed") for p in results}},
         "roofline": r["roofline"], "paths": results, "clocks": clocks, "gpu_launches": int(launches_total),
         "e2e": e2e, "cpu_baseline": cpu, "next_rows": next_rows, "build": S.build_info(),

@@ -99,6 +99,17 @@ int steps_forces_range(const double *pos, const double *mass, const double *soft
                        long long i_begin, long long i_end, double *acc_out, int mixed,
                        steps_stream_t stream);
 
+/* The same decomposition dealt ROUND-ROBIN ("deal the radially sorted order round-robin by tile so every
+ * GPU gets the same far/near mix"): forces on the particles of the blocks first_block, first_block + block_stride, ...
+ * (blocks of steps_block_size() = 2,048 consecutive particles; rank r of P passes first_block = r, block_stride = P)
+ * against all N sources.  acc_out is SoA over the owned particles in ascending order, packed: 3 * cnt doubles with
+ * cnt = the number of owned particles (every owned block is full except possibly the last block of the set).
+ * STEPS_EINVAL for first_block outside the blocks of N or block_stride < 1. */
+int steps_forces_blocks(const double *pos, const double *mass, const double *soft, long long N,
+                        long long first_block, long long block_stride, double *acc_out, int mixed,
+                        steps_stream_t stream);
+int steps_block_size(void);
+
 /* End-to-end convenience with HOST buffers (pageable or pinned): copies pos/mass/soft to
  * the device, evaluates the forces, copies acc back and synchronises `stream` before
  * returning.  Used by bench.py's e2e figure. */

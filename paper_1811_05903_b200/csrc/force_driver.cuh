@@ -153,8 +153,10 @@ __global__ void __launch_bounds__(CTA_THREADS, 1)
 forces_persistent_kernel(const double* __restrict__ pos, const double* __restrict__ soft, long long N,
                          const typename Path::Tile* __restrict__ tiles, int nt, long long i_begin, long long i_end,
                          int nb, double* __restrict__ partials, int zero, double box_L, double box_invL,
-                         const SymPlan* __restrict__ plan)
+                         const SymPlan* __restrict__ plan, int block_stride)
 {
+    // block_stride > 1 (multi-GPU dealing, steps_forces_blocks): local i-block b is the global block
+    // i_begin / IB + b * block_stride; i_end is then N.
     static_assert(!BAND || BOX == 0, "the band split applies to the open boundary only");
     using Tile = typename Path::Tile;
     constexpr int STRIDE = stage_stride((int)sizeof(Tile));
@@ -218,7 +220,7 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
 
         typename Path::IState S;
         float rlo, rhi, hh;
-        const long long i0 = i_begin + (long long)b * IB + warp * WARP_I + lane;
+        const long long i0 = i_begin + (long long)b * block_stride * IB + warp * WARP_I + lane;
         load_i_block<Path>(S, pos, soft, N, i0, i_end, rlo, rhi, hh);
         float blo[3], bhi[3];                                  // bounding box of the warp's i-particles (periodic boxes)
         if constexpr (BOX == 1) warp_box<Path>(S, blo, bhi);

@@ -217,7 +217,7 @@ int launch_forces_sym(const double* pos, const double* mass, const double* soft,
     sym_band_width<Tile><<<nb, 128, 0, st>>>(tiles, nb, w.plan);
     sym_plan_finalize<<<1, 1024, 0, st>>>(w.plan, nb, 8 * Ps);
     if (prof) STEPS_CUDA(cudaEventRecord(w.ev0, st));
-    band<<<P, CTA_THREADS, smem_band, st>>>(pos, soft, N, tiles, ntp, 0, N, nb, w.partials, 0, 0.0, 0.0, w.plan);
+    band<<<P, CTA_THREADS, smem_band, st>>>(pos, soft, N, tiles, ntp, 0, N, nb, w.partials, 0, 0.0, 0.0, w.plan, 1);
     double* hi = w.acc_dd;
     double* lo = w.acc_dd + 3 * N;
     forces_band_reduce_kernel<Path::NOUT><<<(int)((N + 255) / 256), 256, 0, st>>>(w.partials, w.plan, P, N, acc_out, 1, hi, lo);
@@ -285,23 +285,26 @@ inline bool use_splitj(long long cnt, long long N, const Workspace& w)
     return g_splitj.load() != 0 && (cnt + SPLITJ_GROUP - 1) / SPLITJ_GROUP <= w.num_sms && nblocks_of(cnt) * ntiles_of(N) < 8ll * w.num_sms;
 }
 
+// block_stride == 1: forces on [i_begin, i_end).  block_stride > 1 (steps_forces_blocks): forces on the blocks
+// i_begin / IB + k block_stride, k = 0, 1, ...; i_end = N; `cnt` = how many particles that is; acc_out packed over them.
 template <typename Path>
 int launch_forces(const double* pos, const double* mass, const double* soft, long long N, long long i_begin,
-                  long long i_end, double* acc_out, cudaStream_t st, Workspace& w, int& grid_cache)
+                  long long i_end, double* acc_out, cudaStream_t st, Workspace& w, int& grid_cache, int block_stride = 1,
+                  long long cnt_strided = 0)
 {
     using Tile = typename Path::Tile;
-    if (i_begin == 0 && i_end == N && g_driver.load() == 0 && sym_eligible(N) && w.sym_records &&
+    if (block_stride == 1 && i_begin == 0 && i_end == N && g_driver.load() == 0 && sym_eligible(N) && w.sym_records &&
         (Path::NOUT == 6 || g_sym_enabled.load() != 2))      // "sym" = 2: fp64 path only
         return launch_forces_sym<Path>(pos, mass, soft, N, acc_out, st, w);
     const int nt = (int)ntiles_of(N);
     Tile* tiles = reinterpret_cast<Tile*>(w.tiles);
     prep_tiles<Tile><<<nt, TJ, 0, st>>>(pos, mass, soft, N, tiles, nullptr);
     g_launches++;
-    const long long cnt = i_end - i_begin;
+    const long long cnt = block_stride == 1 ? i_end - i_begin : cnt_strided;
     const int nb = (int)nblocks_of(cnt);
-    if (g_driver.load() == 0 && use_splitj(cnt, N, w))
+    if (block_stride == 1 && g_driver.load() == 0 && use_splitj(cnt, N, w))
         return launch_splitj<Path, 0>(pos, soft, N, tiles, nt, i_begin, i_end, acc_out, st, w, 0.0);
-    if (g_driver.load() == 1) {
+    if (g_driver.load() == 1 && block_stride == 1) {
         const int smem = stage_stride((int)sizeof(Tile)) + Path::NOUT * R_I * CTA_THREADS * (int)sizeof(double);
         STEPS_CUDA(cudaFuncSetAttribute(forces_v1_kernel<Path>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         forces_v1_kernel<Path><<<nb, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, i_begin, i_end, acc_out, 0);
@@ -317,7 +320,7 @@ int launch_forces(const double* pos, const double* mass, const double* soft, lon
             if (!w.ev0) { STEPS_CUDA(cudaEventCreate(&w.ev0)); STEPS_CUDA(cudaEventCreate(&w.ev1)); }
             STEPS_CUDA(cudaEventRecord(w.ev0, st));
         }
-        kern<<<P, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, i_begin, i_end, nb, w.partials, 0, 0.0, 0.0, nullptr);
+        kern<<<P, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, i_begin, i_end, nb, w.partials, 0, 0.0, 0.0, nullptr, block_stride);
         if (prof) { STEPS_CUDA(cudaEventRecord(w.ev1, st)); w.ev_valid = true; }
         forces_reduce_kernel<Path::NOUT><<<(int)((cnt + 255) / 256), 256, 0, st>>>(w.partials, nt, nb, P, cnt, acc_out);
         g_launches += 2;
@@ -372,7 +375,7 @@ int launch_forces_periodic(const double* pos, const double* mass, const double* 
     rc = persistent_grid(kern, smem, w, grid_cache);
     if (rc != STEPS_OK) return rc;
     const int P = grid_cache;
-    kern<<<P, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, 0, N, nb, w.partials, 0, L, 1.0 / L, nullptr);
+    kern<<<P, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, 0, N, nb, w.partials, 0, L, 1.0 / L, nullptr, 1);
     forces_reduce_kernel<Path::NOUT><<<(int)((N + 255) / 256), 256, 0, st>>>(w.partials, nt, nb, P, N, acc_out);
     g_launches += 2;
     STEPS_CUDA(cudaGetLastError());
@@ -432,6 +435,34 @@ int steps_forces_range(const double* pos, const double* mass, const double* soft
                        long long i_end, double* acc_out, int mixed, steps_stream_t stream)
 {
     return forces_impl(pos, mass, soft, N, i_begin, i_end, acc_out, mixed, stream);
+}
+
+int steps_block_size(void) { return IB; }
+
+int steps_forces_blocks(const double* pos, const double* mass, const double* soft, long long N, long long first_block,
+                        long long block_stride, double* acc_out, int mixed, steps_stream_t stream)
+{
+    if (!pos || !mass || !soft || !acc_out || N < 1) return STEPS_EINVAL;
+    const long long nb_all = nblocks_of(N);
+    if (first_block < 0 || first_block >= nb_all || block_stride < 1 || block_stride > 0x7fffffff) return STEPS_EINVAL;
+    if (N > (1ll << 31) - IB) return STEPS_EINVAL;
+    if (misaligned(pos) || misaligned(mass) || misaligned(soft) || misaligned(acc_out)) return STEPS_EINVAL;
+    const long long owned = (nb_all - 1 - first_block) / block_stride + 1;                     // blocks first, first + stride, ...
+    const long long last = first_block + (owned - 1) * block_stride;
+    const long long cnt = (owned - 1) * IB + std::min<long long>(IB, N - last * IB);
+    int dev;
+    int rc = current_device(&dev);
+    if (rc != STEPS_OK) return rc;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    rc = ensure_workspace(dev, N, st);
+    if (rc != STEPS_OK) return rc;
+    Workspace& w = g_ws[dev];
+    rc = claim_scratch(w, st);
+    if (rc != STEPS_OK) return rc;
+    rc = mixed ? launch_forces<MixedPath>(pos, mass, soft, N, first_block * IB, N, acc_out, st, w, w.grid_mixed, (int)block_stride, cnt)
+               : launch_forces<Fp64Path>(pos, mass, soft, N, first_block * IB, N, acc_out, st, w, w.grid_fp64, (int)block_stride, cnt);
+    if (rc != STEPS_OK) return rc;
+    return release_scratch(w, st);
 }
 
 int steps_forces_host(const double* pos_host, const double* mass_host, const double* soft_host, long long N,

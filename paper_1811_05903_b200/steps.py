@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(_HERE, "libsteps_b200.so")
 OK, EINVAL, ECUDA, EUNSUPPORTED, ENOMEM, ECAPTURE = 0, -1, -2, -3, -4, -5
 
 EXPORTS = [
-    "steps_forces", "steps_forces_mixed", "steps_forces_range", "steps_forces_host", "steps_kick_drift",
+    "steps_forces", "steps_forces_mixed", "steps_forces_range", "steps_forces_blocks", "steps_block_size", "steps_forces_host", "steps_kick_drift",
     "steps_kdk_step", "steps_hubble", "steps_scale_factor_rk4", "steps_kdk_schedule", "steps_momentum",
     "steps_timestep", "steps_timestep_coefficient", "steps_force_residual", "steps_forces_quasi_periodic", "steps_forces_periodic",
     "steps_kdk_step_adaptive", "steps_kick_close_adaptive",
@@ -66,6 +66,7 @@ def load_library(path: str) -> C.CDLL:
     L.steps_forces_mixed.argtypes = [vp, vp, vp, ll, vp, vp]
     L.steps_forces_range.argtypes = [vp, vp, vp, ll, ll, ll, vp, i32, vp]
     L.steps_forces_host.argtypes = [vp, vp, vp, ll, vp, i32, vp]
+    L.steps_forces_blocks.argtypes = [vp, vp, vp, ll, ll, ll, vp, i32, vp]
     L.steps_kick_drift.argtypes = [vp, vp, vp, ll, C.POINTER(KdkCoeffs), vp]
     L.steps_kdk_step.argtypes = [vp, vp, vp, vp, vp, ll, C.POINTER(KdkCoeffs), vp]
     L.steps_hubble.argtypes = [dbl, C.POINTER(Cosmology)]
@@ -148,6 +149,18 @@ def steps_forces_range(pos, mass, soft, i_begin: int, i_end: int, acc_out, mixed
     n = mass.numel()
     _check(lib().steps_forces_range(_dev(pos, 3 * n), _dev(mass, n), _dev(soft, n), n, i_begin, i_end,
                                     _dev(acc_out, 3 * (i_end - i_begin)), int(mixed), _stream(stream)))
+
+
+def steps_block_size() -> int:
+    return int(lib().steps_block_size())
+
+
+def steps_forces_blocks(pos, mass, soft, first_block: int, block_stride: int, acc_out, mixed: bool = False, stream=None) -> None:
+    """Forces on the particles of the blocks first_block, first_block + block_stride, ... (round-robin dealing of the
+    i-blocks over ranks); acc_out: SoA over the owned particles, packed (3 * cnt elements)."""
+    n = mass.numel()
+    _check(lib().steps_forces_blocks(_dev(pos, 3 * n), _dev(mass, n), _dev(soft, n), n, first_block, block_stride,
+                                     _dev(acc_out, acc_out.numel()), int(mixed), _stream(stream)))
 
 
 def steps_forces_host(pos_host, mass_host, soft_host, acc_host, mixed: bool = False, stream=None) -> None:

@@ -1,10 +1,10 @@
-"""-m "not gpu": the N > 1 plumbing of bench.py on CPU -- the paper's i-range decomposition
-(node k computes floor(N/N_node) force vectors against all particles, the
-main node also takes the remainder; one exchange of positions per step).  world_size 2 and 3,
-`gloo` backend, 127.0.0.1 rendezvous.  The per-rank force call is played by the oracle's
-idx-restricted sum (the CUDA path needs a GPU); what is under test is the host-side plan:
-ranges tile [0, N) exactly, the all-gather rebuilds the replicated SoA array, and the sharded
-evaluation equals the unsharded one bit for bit."""
+"""-m "not gpu": the N > 1 plumbing of bench.py on CPU -- the paper's decomposition (every node
+holds all particles, node k computes the force vectors of its share against all of them, one exchange of positions
+per step) with the i-blocks of 2,048 dealt round-robin to the ranks.  world_size 2 and 3, `gloo`
+backend, 127.0.0.1 rendezvous.  The per-rank force call is played by the oracle's idx-restricted sum (the CUDA path
+needs a GPU); what is under test is the host-side plan: the ranks' blocks partition the particles, the all-gather
+into preallocated buffers rebuilds the replicated SoA array, and the sharded evaluation equals the unsharded one bit
+for bit."""
 import os
 import socket
 
@@ -31,6 +31,17 @@ def test_i_ranges_tile_the_particles(world, n):
     assert all(e - b == base for b, e in ranges[1:])
 
 
+@pytest.mark.parametrize("world,n", [(1, 7), (2, 4096), (3, 10000), (8, 1048576), (5, 3), (3, 2048 * 7 + 5)])
+def test_round_robin_blocks_partition_the_particles(world, n):
+    seen = np.concatenate([shard.owned_indices(r, world, n) for r in range(world)])
+    assert np.array_equal(np.sort(seen), np.arange(n))
+    counts = [shard.owned_count(r, world, n) for r in range(world)]
+    assert sum(counts) == n and max(counts) - min(counts) <= shard.BLOCK
+    for r in range(world):
+        assert all(b % world == r for b in shard.owned_blocks(r, world, n))
+        assert len(shard.owned_indices(r, world, n)) == counts[r]
+
+
 def _worker(rank: int, world: int, port: int, n: int, out_dir: str) -> None:
     import torch
     import torch.distributed as dist
@@ -41,13 +52,18 @@ def _worker(rank: int, world: int, port: int, n: int, out_dir: str) -> None:
     try:
         from oracle import steps_oracle as oracle
         ps = synth.g0(n, seed=77)                              # identical on every rank (seeded)
-        b, e = shard.i_range(rank, world, n)
-        # one "step": every rank moves ITS slice (a stand-in drift), the slices are all-gathered ...
-        x_local = torch.from_numpy(ps.pos[:, b:e].copy()) * (1.0 + 1e-3 * (rank + 1))
-        x_all = shard.gather_soa(x_local, n)
-        # ... and every rank evaluates the forces of its i-range against ALL sources
+        idx = shard.owned_indices(rank, world, n)
+        gather = shard.Gather(world, n, "cpu", torch.float64)
+        x_all = torch.from_numpy(ps.pos.copy())
+        for step in range(2):                                  # twice: the buffers are reused, nothing is reallocated
+            # one "step": every rank moves ITS particles (a stand-in drift), the slices are all-gathered ...
+            x_local = x_all[:, idx] * (1.0 + 1e-3 * (rank + 1))
+            ptr = gather.recv.data_ptr()
+            gather(x_local, x_all)
+            assert gather.recv.data_ptr() == ptr
+        # ... and every rank evaluates the forces of its blocks against ALL sources
         pos = np.ascontiguousarray(x_all.numpy())
-        acc_local = oracle.forces(pos, ps.mass, ps.soft, idx=np.arange(b, e, dtype=np.int64))
+        acc_local = oracle.forces(pos, ps.mass, ps.soft, idx=idx)
         np.save(os.path.join(out_dir, f"pos_{rank}.npy"), pos)
         np.save(os.path.join(out_dir, f"acc_{rank}.npy"), acc_local)
         dist.barrier()
@@ -55,7 +71,7 @@ def _worker(rank: int, world: int, port: int, n: int, out_dir: str) -> None:
         dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("world,n", [(2, 1501), (3, 1000)])
+@pytest.mark.parametrize("world,n", [(2, 5001), (3, 9000)])
 def test_sharded_step_equals_unsharded(world, n, tmp_path, oracle):
     import torch.multiprocessing as mp
 
@@ -63,9 +79,10 @@ def test_sharded_step_equals_unsharded(world, n, tmp_path, oracle):
     mp.spawn(_worker, args=(world, port, n, str(tmp_path)), nprocs=world, join=True)
     ps = synth.g0(n, seed=77)
     expect_pos = ps.pos.copy()
-    for r, (b, e) in enumerate(shard.all_ranges(world, n)):
-        expect_pos[:, b:e] *= 1.0 + 1e-3 * (r + 1)
+    for _ in range(2):
+        for r in range(world):
+            expect_pos[:, shard.owned_indices(r, world, n)] *= 1.0 + 1e-3 * (r + 1)
     full = oracle.forces(expect_pos, ps.mass, ps.soft)
-    for r, (b, e) in enumerate(shard.all_ranges(world, n)):
+    for r in range(world):
         assert np.array_equal(np.load(tmp_path / f"pos_{r}.npy"), expect_pos), f"rank {r}: gathered positions"
-        assert np.array_equal(np.load(tmp_path / f"acc_{r}.npy"), full[:, b:e]), f"rank {r}: forces of its range"
+        assert np.array_equal(np.load(tmp_path / f"acc_{r}.npy"), full[:, shard.owned_indices(r, world, n)]), f"rank {r}: forces"
