@@ -116,6 +116,22 @@ int steps_block_size(void);
 int steps_forces_host(const double *pos_host, const double *mass_host, const double *soft_host,
                       long long N, double *acc_host, int mixed, steps_stream_t stream);
 
+/* ---- radial order --------------------------------------------- */
+
+/* perm (device, N int64, 16-byte aligned) = the particle indices in order of ascending |x| (keys |x|^2 in fp64; equal
+ * keys keep their input order).  The force calls are correct for ANY particle order; radially ordered input is what
+ * makes almost every (i-group, j-tile) pair "far" and keeps the pair-symmetric band narrow, so a long run re-sorts when
+ * steps_near_fraction has grown.  Stream-ordered; allocates its buffers on first use for a larger N (cudaMalloc). */
+int steps_sort_radial(const double *pos, long long N, long long *perm, steps_stream_t stream);
+/* dst[c][k] = src[c][perm[k]] for the ncomp components of an SoA array (ncomp = 3 for pos/vel/acc, 1 for mass/soft);
+ * src and dst must not overlap. */
+int steps_permute(const double *src, long long N, int ncomp, const long long *perm, double *dst,
+                  steps_stream_t stream);
+/* Tile-classification statistics for the given order: out2 (device, 2 doubles) = {number of (128-particle i-group,
+ * 256-source tile) pairs that are NOT far, number of all such pairs}. */
+int steps_near_fraction(const double *pos, const double *mass, const double *soft, long long N, double *out2,
+                        steps_stream_t stream);
+
 /* ---- time integration ---------------------------------- */
 
 /* Coefficients of one fused kick/drift pass.  With g_i = acc_i + B x_i the pass does

@@ -284,20 +284,35 @@ forces_sym_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__
 // every 128-source subgroup, the sources' reaction sums (two packed halves, 64 terms each) into fp64 shared memory after the
 // 32 hand-overs of a set.  Scaled sources: c_j = m_j^(-1/2) in fp32, dX = X_j - c_j x_i, y = 1/(c_j r):
 //   on i:  m_j (x_j - x_i)/r^3 = y^3 dX          on j:  -(m_i y^3 dX) c_j^2
+// THREADS x RI = 2,048: the block is held by THREADS / 32 warps with RI particles per lane.  More particles per lane means
+// more packed arithmetic per hand-over (the shuffles and the source load are per step, whatever RI is).
 __host__ __device__ constexpr int sym_mixed_stage_bytes() { return TPB * 4 * TJ * (int)sizeof(float); }     // (X, Y, Z, c) of the block's tiles
-__host__ __device__ constexpr int sym_mixed_smem_bytes() { return 2 * sym_mixed_stage_bytes() + 3 * IB * (int)sizeof(double) + 3 * R_I * CTA_THREADS * (int)sizeof(double); }
+template <int THREADS, int RI>
+__host__ __device__ constexpr int sym_mixed_smem_bytes()
+{
+    return 2 * sym_mixed_stage_bytes() + 3 * IB * (int)sizeof(double) + 3 * RI * THREADS * (int)sizeof(double);
+}
+#ifndef STEPS_SYM_MIXED_THREADS
+#define STEPS_SYM_MIXED_THREADS 256
+#endif
+constexpr int SYM_MIXED_THREADS = STEPS_SYM_MIXED_THREADS;
+constexpr int SYM_MIXED_RI = IB / SYM_MIXED_THREADS;
 
-__global__ void __launch_bounds__(CTA_THREADS, 1)
+template <int THREADS, int RI>
+__global__ void __launch_bounds__(THREADS, 1)
 forces_sym_mixed_kernel(const TileF32* __restrict__ tiles, const SymPlan* __restrict__ plan, long long k_begin, long long k_end,
                         double* __restrict__ rowrec, double* __restrict__ colrec)
 {
-    static_assert(R_I == 4, "two packed pairs per lane");
+    static_assert(THREADS * RI == IB && RI % 2 == 0, "the CTA holds one block, particles packed in pairs");
+    constexpr int NP = RI / 2;                  // packed pairs per lane
+    constexpr int WI = 32 * RI;                 // particles per warp = sources per subgroup
+    constexpr int SUBG = THREADS / 32;          // warps = subgroups per block
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ uint64_t full_bar[2];
     constexpr int STAGE = sym_mixed_stage_bytes();
     float* col = reinterpret_cast<float*>(smem_raw);                                   // [2][TPB][4][TJ]
     double* Bsm = reinterpret_cast<double*>(smem_raw + 2 * STAGE);                     // [3][IB]
-    double* Asm = Bsm + 3 * IB + threadIdx.x;                                          // [3][R_I][CTA_THREADS], this thread's column
+    double* Asm = Bsm + 3 * IB + threadIdx.x;                                          // [3][RI][THREADS], this thread's column
 
     const long long K = plan->K;
     if (k_end > K) k_end = K;
@@ -340,7 +355,6 @@ forces_sym_mixed_kernel(const TileF32* __restrict__ tiles, const SymPlan* __rest
         if (total > 1) produce(1);
     }
 
-    constexpr int NP = R_I / 2;
     u64 nx[NP], ny[NP], nz[NP], m2[NP];
     int cur_b = -1;
     const int src_lane = (lane + 31) & 31;
@@ -348,10 +362,10 @@ forces_sym_mixed_kernel(const TileF32* __restrict__ tiles, const SymPlan* __rest
     for (int it = 0; it < total; ++it) {
         if (b != cur_b) {
             cur_b = b;
-            float x[R_I], y[R_I], z[R_I], m[R_I];
+            float x[RI], y[RI], z[RI], m[RI];
 #pragma unroll
-            for (int k = 0; k < R_I; ++k) {
-                const int i = warp * WARP_I + lane + 32 * k;
+            for (int k = 0; k < RI; ++k) {
+                const int i = warp * WI + lane + 32 * k;
                 const TileF32& T = tiles[(long long)b * TPB + i / TJ];
                 x[k] = T.x[i % TJ]; y[k] = T.y[i % TJ]; z[k] = T.z[i % TJ]; m[k] = T.m[i % TJ];
             }
@@ -362,20 +376,20 @@ forces_sym_mixed_kernel(const TileF32* __restrict__ tiles, const SymPlan* __rest
             }
         }
 #pragma unroll
-        for (int q = 0; q < 3 * R_I; ++q) Asm[q * CTA_THREADS] = 0.0;
-        for (int q = threadIdx.x; q < 3 * IB; q += CTA_THREADS) Bsm[q] = 0.0;
+        for (int q = 0; q < 3 * RI; ++q) Asm[q * THREADS] = 0.0;
+        for (int q = threadIdx.x; q < 3 * IB; q += THREADS) Bsm[q] = 0.0;
         const int s = it & 1;
         mbar_wait(&full_bar[s], (it >> 1) & 1);
         __syncthreads();
         const float* cs = col + (size_t)s * (STAGE / sizeof(float));
 
-        for (int q = 0; q < SUBGROUPS; ++q) {
-            const int u = (warp + q) & (SUBGROUPS - 1);
+        for (int q = 0; q < SUBG; ++q) {
+            const int u = (warp + q) & (SUBG - 1);
             u64 ax[NP], ay[NP], az[NP];
 #pragma unroll
             for (int p = 0; p < NP; ++p) ax[p] = ay[p] = az[p] = 0ull;
-            for (int t = 0; t < WARP_I / 32; ++t) {
-                const int j0 = u * WARP_I + t * 32;                                   // first source of the set (within the block)
+            for (int t = 0; t < WI / 32; ++t) {
+                const int j0 = u * WI + t * 32;                                       // first source of the set (within the block)
                 const float* set = cs + (j0 / TJ) * (4 * TJ) + (j0 % TJ);           // X of source j0; Y, Z, c follow at + TJ each
                 u64 bx = 0ull, by = 0ull, bz = 0ull;
 #pragma unroll 2
@@ -404,29 +418,31 @@ forces_sym_mixed_kernel(const TileF32* __restrict__ tiles, const SymPlan* __rest
                     bz = __shfl_sync(0xffffffffu, bz, src_lane);
                 }
                 float lo, hi;
-                const int j = j0 + lane;
+                const int j = j0 + lane;                       // 32 steps x NP terms per packed half: <= 128
                 unpack2(bx, lo, hi); Bsm[j] += (double)lo + (double)hi;
                 unpack2(by, lo, hi); Bsm[IB + j] += (double)lo + (double)hi;
                 unpack2(bz, lo, hi); Bsm[2 * IB + j] += (double)lo + (double)hi;
-            }
+                if ((t & 3) == 3) {                            // 128 sources per particle: into the fp64 accumulators
 #pragma unroll
-            for (int p = 0; p < NP; ++p) {                   // 128 sources per particle: into the fp64 accumulators
-                float lo, hi;
-                unpack2(ax[p], lo, hi); Asm[(0 * R_I + 2 * p) * CTA_THREADS] += (double)lo; Asm[(0 * R_I + 2 * p + 1) * CTA_THREADS] += (double)hi;
-                unpack2(ay[p], lo, hi); Asm[(1 * R_I + 2 * p) * CTA_THREADS] += (double)lo; Asm[(1 * R_I + 2 * p + 1) * CTA_THREADS] += (double)hi;
-                unpack2(az[p], lo, hi); Asm[(2 * R_I + 2 * p) * CTA_THREADS] += (double)lo; Asm[(2 * R_I + 2 * p + 1) * CTA_THREADS] += (double)hi;
+                    for (int p = 0; p < NP; ++p) {
+                        unpack2(ax[p], lo, hi); Asm[(0 * RI + 2 * p) * THREADS] += (double)lo; Asm[(0 * RI + 2 * p + 1) * THREADS] += (double)hi;
+                        unpack2(ay[p], lo, hi); Asm[(1 * RI + 2 * p) * THREADS] += (double)lo; Asm[(1 * RI + 2 * p + 1) * THREADS] += (double)hi;
+                        unpack2(az[p], lo, hi); Asm[(2 * RI + 2 * p) * THREADS] += (double)lo; Asm[(2 * RI + 2 * p + 1) * THREADS] += (double)hi;
+                        ax[p] = ay[p] = az[p] = 0ull;
+                    }
+                }
             }
             __syncthreads();
         }
 
         const long long rec = (kk0 + it - k_begin) * 3 * IB;
 #pragma unroll
-        for (int k = 0; k < R_I; ++k) {
-            const int i = warp * WARP_I + lane + 32 * k;
+        for (int k = 0; k < RI; ++k) {
+            const int i = warp * WI + lane + 32 * k;
 #pragma unroll
-            for (int cc = 0; cc < 3; ++cc) rowrec[rec + cc * IB + i] = Asm[(cc * R_I + k) * CTA_THREADS];
+            for (int cc = 0; cc < 3; ++cc) rowrec[rec + cc * IB + i] = Asm[(cc * RI + k) * THREADS];
         }
-        for (int j = threadIdx.x; j < IB; j += CTA_THREADS) {
+        for (int j = threadIdx.x; j < IB; j += THREADS) {
             const double cj = (double)cs[(j / TJ) * (4 * TJ) + 3 * TJ + ((j % TJ) ^ STEPS_C_SWIZZLE)];
             const double f = -cj * cj;
             colrec[rec + j] = f * Bsm[j]; colrec[rec + IB + j] = f * Bsm[IB + j]; colrec[rec + 2 * IB + j] = f * Bsm[2 * IB + j];

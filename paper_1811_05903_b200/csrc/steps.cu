@@ -15,6 +15,7 @@
 #include "force_driver.cuh"
 #include "force_sym.cuh"
 #include "kdk.cuh"
+#include "sort.cuh"
 
 using namespace steps;
 
@@ -51,6 +52,8 @@ struct Workspace {
     int grid_mixed = 0, grid_fp64 = 0, grid_fp64_band = 0, grid_mixed_band = 0, grid_sym = 0, grid_sym_mixed = 0;   // persistent grids: SMs x resident CTAs
     int grid_mixed_periodic = 0, grid_fp64_periodic = 0, grid_fp64_images = 0;
     double* mom_partial = nullptr;  // MOM_BLOCKS * 4
+    void* sort_buf = nullptr;       // steps_sort_radial: keys in/out, index in, cub temporary storage
+    size_t sort_bytes = 0;
     // staging buffers of steps_forces_host
     double* h_pos = nullptr; double* h_mass = nullptr; double* h_soft = nullptr; double* h_acc = nullptr;
     long long h_cap = 0;
@@ -178,12 +181,12 @@ int release_scratch(Workspace& w, cudaStream_t st)
 bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
 
 template <typename Kernel>
-int persistent_grid(Kernel kern, int smem, const Workspace& w, int& grid_cache)
+int persistent_grid(Kernel kern, int smem, const Workspace& w, int& grid_cache, int threads = CTA_THREADS)
 {
     if (grid_cache == 0) {
         STEPS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         int per_sm = 0;
-        STEPS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, CTA_THREADS, smem));
+        STEPS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
         if (per_sm < 1) return STEPS_EUNSUPPORTED;
         const int g = w.num_sms * per_sm;
         grid_cache = g > MAX_GRID ? MAX_GRID : g;
@@ -207,7 +210,9 @@ int launch_forces_sym(const double* pos, const double* mass, const double* soft,
     int rc = persistent_grid(band, smem_band, w, FP64 ? w.grid_fp64_band : w.grid_mixed_band);
     if (rc != STEPS_OK) return rc;
     if constexpr (FP64) rc = persistent_grid(forces_sym_kernel, sym_smem_bytes(), w, w.grid_sym);
-    else rc = persistent_grid(forces_sym_mixed_kernel, sym_mixed_smem_bytes(), w, w.grid_sym_mixed);
+    else rc = persistent_grid(forces_sym_mixed_kernel<SYM_MIXED_THREADS, SYM_MIXED_RI>, sym_mixed_smem_bytes<SYM_MIXED_THREADS, SYM_MIXED_RI>(),
+                              w, w.grid_sym_mixed, SYM_MIXED_THREADS);
+    if (!FP64 && w.grid_sym_mixed > w.num_sms) w.grid_sym_mixed = w.num_sms;      // one CTA per SM: the item shares stay equal
     if (rc != STEPS_OK) return rc;
     const int P = FP64 ? w.grid_fp64_band : w.grid_mixed_band, Ps = FP64 ? w.grid_sym : w.grid_sym_mixed;
     const bool prof = g_profile.load() != 0;
@@ -228,7 +233,8 @@ int launch_forces_sym(const double* pos, const double* mass, const double* soft,
     for (long long k0 = 0; k0 < kmax; k0 += items) {
         const long long k1 = std::min(kmax, k0 + items);
         if constexpr (FP64) forces_sym_kernel<<<Ps, CTA_THREADS, sym_smem_bytes(), st>>>(tiles, w.plan, k0, k1, rowrec, colrec, 0);
-        else forces_sym_mixed_kernel<<<Ps, CTA_THREADS, sym_mixed_smem_bytes(), st>>>(tiles, w.plan, k0, k1, rowrec, colrec);
+        else forces_sym_mixed_kernel<SYM_MIXED_THREADS, SYM_MIXED_RI><<<Ps, SYM_MIXED_THREADS, sym_mixed_smem_bytes<SYM_MIXED_THREADS, SYM_MIXED_RI>(), st>>>(
+                tiles, w.plan, k0, k1, rowrec, colrec);
         forces_sym_reduce_kernel<<<(int)((N + 255) / 256), 256, 0, st>>>(w.plan, rowrec, colrec, k0, k1, N, hi, lo,
                                                                           k1 == kmax ? 1 : 0, acc_out);
         g_launches += 2;
@@ -666,6 +672,81 @@ int steps_force_residual(const double* pos, const double* acc, long long N, doub
     return release_scratch(g_ws[dev], st);
 }
 
+int steps_sort_radial(const double* pos, long long N, long long* perm, steps_stream_t stream)
+{
+    if (!pos || !perm || N < 1 || N > (1ll << 31) - IB) return STEPS_EINVAL;
+    if (misaligned(pos) || misaligned(perm)) return STEPS_EINVAL;
+    int dev;
+    int rc = current_device(&dev);
+    if (rc != STEPS_OK) return rc;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    rc = ensure_workspace(dev, 1, st);
+    if (rc != STEPS_OK) return rc;
+    Workspace& w = g_ws[dev];
+    size_t temp_bytes = 0;
+    STEPS_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, temp_bytes, (const double*)nullptr, (double*)nullptr, (const long long*)nullptr,
+                                               (long long*)nullptr, (int)N, 0, 64, st));
+    const size_t arr = (sizeof(double) * (size_t)N + 255) / 256 * 256;
+    const size_t need = 3 * arr + temp_bytes;
+    {
+        std::lock_guard<std::mutex> lock(g_mutex);
+        if (need > w.sort_bytes) {
+            if (stream_is_capturing(st)) return STEPS_ECAPTURE;
+            STEPS_CUDA(cudaDeviceSynchronize());
+            cudaFree(w.sort_buf); w.sort_buf = nullptr; w.sort_bytes = 0;
+            if (cudaMalloc(&w.sort_buf, need) != cudaSuccess) { cudaGetLastError(); return STEPS_ENOMEM; }
+            w.sort_bytes = need;
+        }
+    }
+    rc = claim_scratch(w, st);
+    if (rc != STEPS_OK) return rc;
+    unsigned char* base = static_cast<unsigned char*>(w.sort_buf);
+    double* keys_in = reinterpret_cast<double*>(base);
+    double* keys_out = reinterpret_cast<double*>(base + arr);
+    long long* idx_in = reinterpret_cast<long long*>(base + 2 * arr);
+    radial_keys_kernel<<<(int)((N + 255) / 256), 256, 0, st>>>(pos, N, keys_in, idx_in);
+    STEPS_CUDA(cub::DeviceRadixSort::SortPairs(base + 3 * arr, temp_bytes, keys_in, keys_out, idx_in, perm, (int)N, 0, 64, st));
+    g_launches += 1;
+    STEPS_CUDA(cudaGetLastError());
+    return release_scratch(w, st);
+}
+
+int steps_permute(const double* src, long long N, int ncomp, const long long* perm, double* dst, steps_stream_t stream)
+{
+    if (!src || !perm || !dst || N < 1 || ncomp < 1 || src == dst) return STEPS_EINVAL;
+    int dev;
+    int rc = current_device(&dev);
+    if (rc != STEPS_OK) return rc;
+    permute_kernel<<<(int)((N + 255) / 256), 256, 0, reinterpret_cast<cudaStream_t>(stream)>>>(src, N, ncomp, perm, dst);
+    g_launches++;
+    STEPS_CUDA(cudaGetLastError());
+    return STEPS_OK;
+}
+
+int steps_near_fraction(const double* pos, const double* mass, const double* soft, long long N, double* out2, steps_stream_t stream)
+{
+    if (!pos || !mass || !soft || !out2 || N < 1 || N > (1ll << 31) - IB) return STEPS_EINVAL;
+    int dev;
+    int rc = current_device(&dev);
+    if (rc != STEPS_OK) return rc;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    rc = ensure_workspace(dev, N, st);
+    if (rc != STEPS_OK) return rc;
+    Workspace& w = g_ws[dev];
+    rc = claim_scratch(w, st);
+    if (rc != STEPS_OK) return rc;
+    const int nt = (int)ntiles_of(N);
+    TileF64* tiles = reinterpret_cast<TileF64*>(w.tiles);
+    unsigned long long* counts = reinterpret_cast<unsigned long long*>(w.mom_partial);
+    STEPS_CUDA(cudaMemsetAsync(counts, 0, 2 * sizeof(unsigned long long), st));
+    prep_tiles<TileF64><<<nt, TJ, 0, st>>>(pos, mass, soft, N, tiles, nullptr);
+    near_pairs_kernel<TileF64><<<(int)((N + WARP_I - 1) / WARP_I), 128, 0, st>>>(pos, soft, N, tiles, nt, counts);
+    counts_to_double_kernel<<<1, 32, 0, st>>>(counts, out2);
+    g_launches += 3;
+    STEPS_CUDA(cudaGetLastError());
+    return release_scratch(w, st);
+}
+
 int steps_reserve(long long N)
 {
     if (N < 1) return STEPS_EINVAL;
@@ -686,7 +767,7 @@ void steps_shutdown(void)
         cudaSetDevice(d);
         cudaDeviceSynchronize();
         cudaFree(w.tiles); cudaFree(w.partials); cudaFree(w.plan); cudaFree(w.acc_dd); cudaFree(w.sym_records);
-        cudaFree(w.mom_partial);
+        cudaFree(w.mom_partial); cudaFree(w.sort_buf);
         cudaFree(w.h_pos); cudaFree(w.h_mass); cudaFree(w.h_soft); cudaFree(w.h_acc);
         if (w.ev0) { cudaEventDestroy(w.ev0); cudaEventDestroy(w.ev1); }
         if (w.scratch_done) cudaEventDestroy(w.scratch_done);

@@ -15,6 +15,7 @@ OK, EINVAL, ECUDA, EUNSUPPORTED, ENOMEM, ECAPTURE = 0, -1, -2, -3, -4, -5
 
 EXPORTS = [
     "steps_forces", "steps_forces_mixed", "steps_forces_range", "steps_forces_blocks", "steps_block_size", "steps_forces_host", "steps_kick_drift",
+    "steps_sort_radial", "steps_permute", "steps_near_fraction",
     "steps_kdk_step", "steps_hubble", "steps_scale_factor_rk4", "steps_kdk_schedule", "steps_momentum",
     "steps_timestep", "steps_timestep_coefficient", "steps_force_residual", "steps_forces_quasi_periodic", "steps_forces_periodic",
     "steps_kdk_step_adaptive", "steps_kick_close_adaptive",
@@ -67,6 +68,9 @@ def load_library(path: str) -> C.CDLL:
     L.steps_forces_range.argtypes = [vp, vp, vp, ll, ll, ll, vp, i32, vp]
     L.steps_forces_host.argtypes = [vp, vp, vp, ll, vp, i32, vp]
     L.steps_forces_blocks.argtypes = [vp, vp, vp, ll, ll, ll, vp, i32, vp]
+    L.steps_sort_radial.argtypes = [vp, ll, vp, vp]
+    L.steps_permute.argtypes = [vp, ll, i32, vp, vp, vp]
+    L.steps_near_fraction.argtypes = [vp, vp, vp, ll, vp, vp]
     L.steps_kick_drift.argtypes = [vp, vp, vp, ll, C.POINTER(KdkCoeffs), vp]
     L.steps_kdk_step.argtypes = [vp, vp, vp, vp, vp, ll, C.POINTER(KdkCoeffs), vp]
     L.steps_hubble.argtypes = [dbl, C.POINTER(Cosmology)]
@@ -161,6 +165,27 @@ def steps_forces_blocks(pos, mass, soft, first_block: int, block_stride: int, ac
     n = mass.numel()
     _check(lib().steps_forces_blocks(_dev(pos, 3 * n), _dev(mass, n), _dev(soft, n), n, first_block, block_stride,
                                      _dev(acc_out, acc_out.numel()), int(mixed), _stream(stream)))
+
+
+def steps_sort_radial(pos, perm, stream=None) -> None:
+    """perm (int64 device tensor, N) = particle indices by ascending |x|."""
+    import torch
+    n = pos.numel() // 3
+    if not (perm.is_cuda and perm.dtype == torch.int64 and perm.is_contiguous() and perm.numel() == n):
+        raise StepsError("perm must be a contiguous CUDA int64 tensor with N elements")
+    _check(lib().steps_sort_radial(_dev(pos, 3 * n), n, perm.data_ptr(), _stream(stream)))
+
+
+def steps_permute(src, perm, dst, stream=None) -> None:
+    """dst[c][k] = src[c][perm[k]] (SoA with src.numel() / N components)."""
+    n = perm.numel()
+    ncomp = src.numel() // n
+    _check(lib().steps_permute(_dev(src, ncomp * n), n, ncomp, perm.data_ptr(), _dev(dst, ncomp * n), _stream(stream)))
+
+
+def steps_near_fraction(pos, mass, soft, out2, stream=None) -> None:
+    n = mass.numel()
+    _check(lib().steps_near_fraction(_dev(pos, 3 * n), _dev(mass, n), _dev(soft, n), n, _dev(out2, 2), _stream(stream)))
 
 
 def steps_forces_host(pos_host, mass_host, soft_host, acc_host, mixed: bool = False, stream=None) -> None:

@@ -226,6 +226,78 @@ def test_forces_range_and_host_entry_points(S, oracle):
     assert L.steps_forces_range(dpos.data_ptr(), dm.data_ptr(), dh.data_ptr(), 5000, 10, 10, dpos.data_ptr(), 0, None) == S.EINVAL
 
 
+def test_radial_sort_permute_and_near_fraction(S, oracle):
+    """Row a0: steps_sort_radial orders by |x| (checked against numpy, not against itself), steps_permute applies it, the
+    forces of the re-ordered set are the permuted forces of the original one (to the oracle bar), and the share of
+    (i-group, tile) pairs that need the per-pair softening test collapses with the order (steps_near_fraction)."""
+    import torch
+    n = 30011
+    ps = synth.g0(n, seed=31, sort=False)
+    shuffle = np.random.default_rng(5).permutation(n)
+    pos, mass, soft = np.ascontiguousarray(ps.pos[:, shuffle]), ps.mass[shuffle].copy(), ps.soft[shuffle].copy()
+    dpos, dm, dh = dev(pos), dev(mass), dev(soft)
+    perm = torch.empty(n, dtype=torch.int64, device="cuda")
+    S.steps_sort_radial(dpos, perm)
+    p = perm.cpu().numpy()
+    assert np.array_equal(np.sort(p), np.arange(n))
+    r = np.linalg.norm(pos, axis=0)
+    assert np.all(np.diff(r[p]) >= -4e-16 * r[p][1:])          # ascending up to the rounding of the fp64 keys
+    spos, sm, sh = torch.empty_like(dpos), torch.empty_like(dm), torch.empty_like(dh)
+    S.steps_permute(dpos, perm, spos); S.steps_permute(dm, perm, sm); S.steps_permute(dh, perm, sh)
+    assert np.array_equal(spos.cpu().numpy(), pos[:, p]) and np.array_equal(sm.cpu().numpy(), mass[p])
+    out = torch.empty(2, dtype=torch.float64, device="cuda")
+    S.steps_near_fraction(dpos, dm, dh, out); unsorted = out.cpu().numpy().copy()
+    S.steps_near_fraction(spos, sm, sh, out); ordered = out.cpu().numpy().copy()
+    print(f"near (i-group, tile) pairs: unsorted {unsorted[0] / unsorted[1]:.3f}, radially sorted {ordered[0] / ordered[1]:.4f}")
+    assert unsorted[1] == ordered[1] == -(-n // 128) * -(-n // 256)
+    assert unsorted[0] / unsorted[1] > 0.9 and ordered[0] / ordered[1] < 0.1
+    a_un, a_so = torch.empty_like(dpos), torch.empty_like(dpos)
+    S.steps_forces(dpos, dm, dh, a_un); S.steps_forces(spos, sm, sh, a_so)
+    ref = oracle.forces(pos, mass, soft)
+    check(a_un.cpu().numpy(), ref, False, "unsorted")
+    check(a_so.cpu().numpy(), ref[:, p], False, "sorted by the library")
+
+
+@pytest.mark.parametrize("n", [1, 257, 2049, 5000, 20001])
+def test_outputs_stay_inside_their_buffers(S, n):
+    """compute-sanitizer is closed on this pool (profiles/r02_sanitizer.md), so out-of-bounds writes are looked for with
+    guard regions: every output buffer sits between two sentinel-filled pads that must come back untouched, for every
+    force entry point and the O(N) kernels, at ragged sizes (N not a multiple of the tile / group / block)."""
+    import torch
+    ps = synth.g0(n, seed=900 + n, eps0=0.05)
+    dpos, dm, dh = dev(ps.pos), dev(ps.mass), dev(ps.soft)
+    pad, sentinel = 4096, -1.2345e300
+    big = torch.full((3 * n + 2 * pad,), sentinel, dtype=torch.float64, device="cuda")
+    acc = big[pad:pad + 3 * n]
+
+    def intact():
+        torch.cuda.synchronize()
+        return bool((big[:pad] == sentinel).all()) and bool((big[pad + 3 * n:] == sentinel).all())
+
+    for call in (lambda: S.steps_forces(dpos, dm, dh, acc), lambda: S.steps_forces_mixed(dpos, dm, dh, acc),
+                 lambda: S.steps_forces_quasi_periodic(dpos, dm, dh, 50.0, acc),
+                 lambda: S.steps_forces_quasi_periodic(dpos, dm, dh, 50.0, acc, mixed=True)):
+        call()
+        assert intact() and bool(torch.isfinite(acc).all())
+    if n <= 5000:
+        S.steps_forces_periodic(dpos, dm, dh, 50.0, acc)
+        assert intact() and bool(torch.isfinite(acc).all())
+    if n > 1:                                                   # a sub-range and a block-strided set, packed outputs
+        b, e = n // 3, n - 1
+        big.fill_(sentinel)
+        S.steps_forces_range(dpos, dm, dh, b, e, big[pad:pad + 3 * (e - b)], mixed=False)
+        torch.cuda.synchronize()
+        assert bool((big[:pad] == sentinel).all()) and bool((big[pad + 3 * (e - b):] == sentinel).all())
+        from paper_1811_05903_b200 import shard
+        cnt = shard.owned_count(1, 2, n)
+        if cnt:
+            big.fill_(sentinel)
+            S.steps_forces_blocks(dpos, dm, dh, 1, 2, big[pad:pad + 3 * cnt], mixed=True)
+            torch.cuda.synchronize()
+            assert bool((big[:pad] == sentinel).all()) and bool((big[pad + 3 * cnt:] == sentinel).all())
+            assert bool(torch.isfinite(big[pad:pad + 3 * cnt]).all())
+
+
 @pytest.mark.parametrize("world", [2, 3])
 @pytest.mark.parametrize("mixed", [False, True], ids=["fp64", "mixed"])
 def test_sharded_step_on_one_gpu_equals_unsharded(S, mixed, world):
@@ -757,28 +829,56 @@ def test_config4_free_running_vs_oracle_8192(S, oracle):
 
 
 def test_config4_momentum_drift_262144(S, oracle):
-    """Config 4 at its full size: total momentum drift <= 1e-10 relative in fp64 through 200 steps."""
+    """Config 4 at its full size: total momentum drift <= 1e-10 relative in fp64 through 200 steps -- once as the
+    particles come (no re-sorting), once re-sorted radially at the start and every 20 steps (integrate.resort_radial).
+    Also the measurement VERDICT r01 asked for: the share of (i-group, tile) pairs that need the per-pair softening test
+    at steps 0 / 100 / 200, and the wall clock of the two runs (DESIGN.md section 5.2 records the numbers)."""
+    import time
     import torch
     from paper_1811_05903_b200 import integrate
     ps = _config4(oracle, 262144)
     B = 1.0 / ps.r_cut ** 3
     dts = oracle.ln_a_schedule(1 / 51, 1.0, 200, LCDM)
-    dpos, dvel, dm, dh = dev(ps.pos), dev(ps.vel), dev(ps.mass), dev(ps.soft)
-    dacc = torch.empty_like(dpos)
     out = torch.empty(4, dtype=torch.float64, device="cuda")
-    S.steps_forces(dpos, dm, dh, dacc)
-    worst = []
+    report = {}
+    for resort in (0, 20, 2):
+        dpos, dvel, dm, dh = dev(ps.pos), dev(ps.vel), dev(ps.mass), dev(ps.soft)
+        dacc = torch.empty_like(dpos)
+        ids = torch.arange(ps.n, dtype=torch.int64, device="cuda")
+        if resort:
+            integrate.resort_radial([dpos, dvel], [dm, dh], ids)
+        S.steps_forces(dpos, dm, dh, dacc)
+        worst, near = [], {}
 
-    def on_step(k, a):
-        if k % 20 == 19:
-            S.steps_momentum(dvel, dm, out)
-            o = out.cpu().numpy()
-            worst.append(np.linalg.norm(o[:3]) / o[3])
+        def near_fraction(tag):
+            S.steps_near_fraction(dpos, dm, dh, out[:2])
+            o = out[:2].cpu().numpy()
+            near[tag] = round(float(o[0] / o[1]), 4)
 
-    integrate.run_kdk(dpos, dvel, dacc, dm, dh, 1 / 51, dts, S.Cosmology(**LCDM), 1.0, B, on_step=on_step)
-    S.steps_momentum(dvel, dm, out)
-    o = out.cpu().numpy()
-    worst.append(np.linalg.norm(o[:3]) / o[3])
-    print("config4 N=262144 momentum |P|/sum m|v| per 20 steps:", ["%.2e" % w for w in worst])
-    assert np.all(np.isfinite(dpos.cpu().numpy()))
-    assert max(worst) <= 1e-10
+        near_fraction("step 0")
+
+        def on_step(k, a):
+            if k % 20 == 19:
+                S.steps_momentum(dvel, dm, out)
+                o = out.cpu().numpy()
+                worst.append(np.linalg.norm(o[:3]) / o[3])
+            if k + 1 in (100, 200):
+                near_fraction(f"step {k + 1}")
+
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        integrate.run_kdk(dpos, dvel, dacc, dm, dh, 1 / 51, dts, S.Cosmology(**LCDM), 1.0, B, on_step=on_step,
+                          resort_every=resort, ids=ids)
+        torch.cuda.synchronize()
+        wall = time.perf_counter() - t0
+        S.steps_momentum(dvel, dm, out)
+        o = out.cpu().numpy()
+        worst.append(np.linalg.norm(o[:3]) / o[3])
+        report[resort] = (near, wall, max(worst))
+        assert np.all(np.isfinite(dpos.cpu().numpy()))
+        assert max(worst) <= 1e-10
+        assert np.array_equal(np.sort(ids.cpu().numpy()), np.arange(ps.n))
+    for resort, (near, wall, w) in report.items():
+        print(f"config4 N=262144, 200 steps, re-sort every {resort or 'never'}: near (i-group, tile) share {near}, "
+              f"wall {wall:.2f} s, worst |P|/sum m|v| {w:.2e}")
+    assert report[20][0]["step 200"] < report[0][0]["step 200"] and report[20][1] < report[0][1]
