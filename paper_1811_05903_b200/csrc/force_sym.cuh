@@ -115,14 +115,23 @@ __global__ void __launch_bounds__(1024) sym_plan_finalize(SymPlan* __restrict__ 
     for (int b = b0; b < b1; ++b) { cum[b] = s; s += width(b); }
 }
 
-constexpr int sym_smem_bytes() { return 2 * IB * (int)sizeof(FarSrcF64) + 3 * IB * (int)sizeof(double); }
+__host__ __device__ constexpr int sym_smem_bytes() { return 2 * IB * (int)sizeof(FarSrcF64) + 3 * IB * (int)sizeof(double); }
+#ifndef STEPS_SYM_FP64_THREADS
+#define STEPS_SYM_FP64_THREADS 512
+#endif
+constexpr int SYM_FP64_THREADS = STEPS_SYM_FP64_THREADS;
+constexpr int SYM_FP64_RI = IB / SYM_FP64_THREADS;
 
 // Items [k_begin, k_end) of the plan's item list (one panel), shared out evenly over the grid.
-// rowrec / colrec: [k - k_begin][3][IB] doubles.
-__global__ void __launch_bounds__(CTA_THREADS, 1)
+// rowrec / colrec: [k - k_begin][3][IB] doubles.  THREADS x RI = 2,048: THREADS / 32 warps hold the block, RI particles per lane.
+template <int THREADS, int RI>
+__global__ void __launch_bounds__(THREADS, 1)
 forces_sym_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__ plan, long long k_begin, long long k_end,
                   double* __restrict__ rowrec, double* __restrict__ colrec, int zero)
 {
+    static_assert(THREADS * RI == IB, "the CTA holds one block");
+    constexpr int WI = 32 * RI;                 // particles per warp = sources per subgroup
+    constexpr int SUBG = THREADS / 32;          // warps = subgroups per block
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ uint64_t full_bar[2];
     FarSrcF64* col = reinterpret_cast<FarSrcF64*>(smem_raw);                       // [2][IB]
@@ -175,7 +184,7 @@ forces_sym_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__
 
     constexpr double A = 1.4;
     constexpr double C0 = 1.0 / STEPS_FP64_FOLD - (1.0 - A) * (1.0 - A);
-    double xi[R_I], yi[R_I], zi[R_I], mi[R_I];
+    double xi[RI], yi[RI], zi[RI], mi[RI];
     int cur_b = -1;
     const int src_lane = (lane + 31) & 31;                       // reaction sums come from lane - 1
 
@@ -183,25 +192,25 @@ forces_sym_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__
         if (b != cur_b) {                                        // the row block's particles (plain copy of the tiles; pads: m = 0)
             cur_b = b;
 #pragma unroll
-            for (int k = 0; k < R_I; ++k) {
-                const int i = warp * WARP_I + lane + 32 * k;     // within the block
+            for (int k = 0; k < RI; ++k) {
+                const int i = warp * WI + lane + 32 * k;     // within the block
                 const TileF64& T = tiles[(long long)b * TPB + i / TJ];
                 xi[k] = T.x[i % TJ]; yi[k] = T.y[i % TJ]; zi[k] = T.z[i % TJ]; mi[k] = T.m[i % TJ];
             }
         }
-        double ax[R_I], ay[R_I], az[R_I];
+        double ax[RI], ay[RI], az[RI];
 #pragma unroll
-        for (int k = 0; k < R_I; ++k) ax[k] = ay[k] = az[k] = 0.0;
-        for (int q = threadIdx.x; q < 3 * IB; q += CTA_THREADS) Bsm[q] = 0.0;
+        for (int k = 0; k < RI; ++k) ax[k] = ay[k] = az[k] = 0.0;
+        for (int q = threadIdx.x; q < 3 * IB; q += THREADS) Bsm[q] = 0.0;
         const int s = it & 1;
         mbar_wait(&full_bar[s], (it >> 1) & 1);
         __syncthreads();
         const FarSrcF64* cs = col + (size_t)s * IB;
 
-        for (int q = 0; q < SUBGROUPS; ++q) {
-            const int u = (warp + q) & (SUBGROUPS - 1);
-            for (int t = 0; t < WARP_I / 32; ++t) {
-                const FarSrcF64* set = cs + u * WARP_I + t * 32;
+        for (int q = 0; q < SUBG; ++q) {
+            const int u = (warp + q) & (SUBG - 1);
+            for (int t = 0; t < WI / 32; ++t) {
+                const FarSrcF64* set = cs + u * WI + t * 32;
                 double bx = 0.0, by = 0.0, bz = 0.0;
                 // (a 16-byte-half swizzle of the records removes the 2-way bank conflict of this 32-byte stride, but
                 // its address arithmetic costs more than the conflict: measured 85.3 % against 87.1 % of peak)
@@ -212,21 +221,21 @@ forces_sym_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__
                     const double2 XY = *reinterpret_cast<const double2*>(&src->X);
                     const double2 ZC = *reinterpret_cast<const double2*>(&src->Z);
                     const double X = XY.x, Y = XY.y, Z = ZC.x, C = ZC.y;
-                    double dX[R_I], dY[R_I], dZ[R_I], r2[R_I], y0[R_I], y2[R_I], w[R_I];
+                    double dX[RI], dY[RI], dZ[RI], r2[RI], y0[RI], y2[RI], w[RI];
                     STEPS_STAGE_FENCE(zero, 0);
 #pragma unroll
-                    for (int k = 0; k < R_I; ++k) dX[k] = fma(-xi[k], C, X);
+                    for (int k = 0; k < RI; ++k) dX[k] = fma(-xi[k], C, X);
 #pragma unroll
-                    for (int k = 0; k < R_I; ++k) dY[k] = fma(-yi[k], C, Y);
+                    for (int k = 0; k < RI; ++k) dY[k] = fma(-yi[k], C, Y);
 #pragma unroll
-                    for (int k = 0; k < R_I; ++k) dZ[k] = fma(-zi[k], C, Z);
+                    for (int k = 0; k < RI; ++k) dZ[k] = fma(-zi[k], C, Z);
                     STEPS_STAGE_FENCE(zero, 1);
 #pragma unroll
-                    for (int k = 0; k < R_I; ++k) r2[k] = fma(dZ[k], dZ[k], fma(dY[k], dY[k], dX[k] * dX[k]));
+                    for (int k = 0; k < RI; ++k) r2[k] = fma(dZ[k], dZ[k], fma(dY[k], dY[k], dX[k] * dX[k]));
 #pragma unroll
-                    for (int k = 0; k < R_I; ++k) y0[k] = rsqrt_seed(r2[k]);
+                    for (int k = 0; k < RI; ++k) y0[k] = rsqrt_seed(r2[k]);
 #pragma unroll
-                    for (int k = 0; k < R_I; ++k) {
+                    for (int k = 0; k < RI; ++k) {
                         y2[k] = y0[k] * y0[k];
                         w[k] = fma(r2[k], y2[k], -A);
                         y2[k] = y0[k] * y2[k];
@@ -235,7 +244,7 @@ forces_sym_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__
                     }
                     STEPS_STAGE_FENCE(zero, 2);
 #pragma unroll
-                    for (int k = 0; k < R_I; ++k) {
+                    for (int k = 0; k < RI; ++k) {
                         // one basic block per particle: w, then dZ, then s_i stay in the operand-reuse cache, every instruction
                         // reads at most two new operands (ptxas otherwise hoists the s_i products: 85.1 -> 87.1 % of peak)
                         if (k > 0) STEPS_STAGE_FENCE(zero, 2 + k);
@@ -252,7 +261,7 @@ forces_sym_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__
                     bz = __shfl_sync(0xffffffffu, bz, src_lane);
                 }
                 // 32 hand-overs later the sums of source `lane` of the set are back in this lane
-                const int j = u * WARP_I + t * 32 + lane;
+                const int j = u * WI + t * 32 + lane;
                 Bsm[j] += bx; Bsm[IB + j] += by; Bsm[2 * IB + j] += bz;
             }
             __syncthreads();
@@ -261,11 +270,11 @@ forces_sym_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__
         // partial records of the item
         const long long rec = (kk0 + it - k_begin) * 3 * IB;
 #pragma unroll
-        for (int k = 0; k < R_I; ++k) {
-            const int i = warp * WARP_I + lane + 32 * k;
+        for (int k = 0; k < RI; ++k) {
+            const int i = warp * WI + lane + 32 * k;
             rowrec[rec + i] = ax[k]; rowrec[rec + IB + i] = ay[k]; rowrec[rec + 2 * IB + i] = az[k];
         }
-        for (int j = threadIdx.x; j < IB; j += CTA_THREADS) {
+        for (int j = threadIdx.x; j < IB; j += THREADS) {
             const double cj = cs[j].c;
             const double f = -STEPS_FP64_FOLD * cj * cj;
             colrec[rec + j] = f * Bsm[j]; colrec[rec + IB + j] = f * Bsm[IB + j]; colrec[rec + 2 * IB + j] = f * Bsm[2 * IB + j];

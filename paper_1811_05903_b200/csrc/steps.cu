@@ -209,7 +209,8 @@ int launch_forces_sym(const double* pos, const double* mass, const double* soft,
     auto band = forces_persistent_kernel<Path, STAGES, 0, true>;
     int rc = persistent_grid(band, smem_band, w, FP64 ? w.grid_fp64_band : w.grid_mixed_band);
     if (rc != STEPS_OK) return rc;
-    if constexpr (FP64) rc = persistent_grid(forces_sym_kernel, sym_smem_bytes(), w, w.grid_sym);
+    if constexpr (FP64) rc = persistent_grid(forces_sym_kernel<SYM_FP64_THREADS, SYM_FP64_RI>, sym_smem_bytes(), w, w.grid_sym, SYM_FP64_THREADS);
+    if (FP64 && w.grid_sym > w.num_sms) w.grid_sym = w.num_sms;
     else rc = persistent_grid(forces_sym_mixed_kernel<SYM_MIXED_THREADS, SYM_MIXED_RI>, sym_mixed_smem_bytes<SYM_MIXED_THREADS, SYM_MIXED_RI>(),
                               w, w.grid_sym_mixed, SYM_MIXED_THREADS);
     if (!FP64 && w.grid_sym_mixed > w.num_sms) w.grid_sym_mixed = w.num_sms;      // one CTA per SM: the item shares stay equal
@@ -232,7 +233,7 @@ int launch_forces_sym(const double* pos, const double* mass, const double* soft,
     double* colrec = w.sym_records + (size_t)items * 3 * IB;
     for (long long k0 = 0; k0 < kmax; k0 += items) {
         const long long k1 = std::min(kmax, k0 + items);
-        if constexpr (FP64) forces_sym_kernel<<<Ps, CTA_THREADS, sym_smem_bytes(), st>>>(tiles, w.plan, k0, k1, rowrec, colrec, 0);
+        if constexpr (FP64) forces_sym_kernel<SYM_FP64_THREADS, SYM_FP64_RI><<<Ps, SYM_FP64_THREADS, sym_smem_bytes(), st>>>(tiles, w.plan, k0, k1, rowrec, colrec, 0);
         else forces_sym_mixed_kernel<SYM_MIXED_THREADS, SYM_MIXED_RI><<<Ps, SYM_MIXED_THREADS, sym_mixed_smem_bytes<SYM_MIXED_THREADS, SYM_MIXED_RI>(), st>>>(
                 tiles, w.plan, k0, k1, rowrec, colrec);
         forces_sym_reduce_kernel<<<(int)((N + 255) / 256), 256, 0, st>>>(w.plan, rowrec, colrec, k0, k1, N, hi, lo,

@@ -144,6 +144,39 @@ def test_config3_one_million_sampled(S, oracle, mixed):
     check(gpu_forces(S, ps, mixed, idx), ref, mixed, "config3")
 
 
+@pytest.mark.parametrize("mixed", [False, True], ids=["fp64", "mixed"])
+@pytest.mark.parametrize("case", ["ragged", "unsorted", "massless", "stale_order", "one_sided"])
+def test_pair_symmetric_path_and_its_fallbacks(S, oracle, mixed, case):
+    """N >= 131,072 takes the pair-symmetric route (band + every far block pair once).  Against the oracle on a sample:
+    ragged     N = 150,001: the last block holds 497 particles, the rest of its tiles are pads;
+    unsorted   a random permutation: no block pair is far, the device sets W = nb - 1 and everything runs one-sided;
+    massless   three tracer particles (m = 0): their reaction sums could not be divided by m_j, so their tiles are marked
+               and the device falls back in the same way -- the tracers still feel the others;
+    stale_order every particle moved radially by up to 3 % (an order several steps old): a wider band, W > 1;
+    one_sided  the "sym" option off: the one-sided kernels at this size, same answer to rounding."""
+    import torch
+    n = 150001 if case == "ragged" else 139264
+    ps = synth.g0(n, seed=4242)
+    pos, mass, soft = ps.pos.copy(), ps.mass.copy(), ps.soft.copy()
+    rng = np.random.default_rng(17)
+    if case == "unsorted":
+        perm = rng.permutation(n)
+        pos, mass, soft = np.ascontiguousarray(pos[:, perm]), mass[perm].copy(), soft[perm].copy()
+    elif case == "massless":
+        mass[[5, n // 2, n - 3]] = 0.0
+    elif case == "stale_order":
+        pos = np.ascontiguousarray(pos * (1.0 + 0.03 * rng.uniform(-1.0, 1.0, size=n)))
+    idx = np.unique(np.concatenate([synth.stratified_sample(n, 1536), [5, n // 2, n - 3]]))
+    ref = oracle.forces(pos, mass, soft, idx=idx)
+    if case == "one_sided":
+        S.steps_set_option("sym", 0)
+    try:
+        got = gpu_forces(S, (pos, mass, soft), mixed, idx)
+    finally:
+        S.steps_set_option("sym", 1)
+    check(got, ref, mixed, f"sym/{case}")
+
+
 def test_newtons_third_law_and_determinism_on_device(S):
     import torch
     ps = synth.config(1)
