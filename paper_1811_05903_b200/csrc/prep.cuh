@@ -71,7 +71,10 @@ __global__ void __launch_bounds__(TJ) prep_tiles(const double* __restrict__ pos,
         T.far[t].Y = scaled_ok ? y * c : STEPS_PAD_X64;
         T.far[t].Z = scaled_ok ? z * c : STEPS_PAD_X64;
     }
-    const bool force_near = real && m != 0.0 && !scaled_ok;
+    // A massless particle exerts nothing either way (its scaled copy is parked), but as a TARGET of the pair-symmetric
+    // evaluation its reaction sum could not be divided by m_j: its tile is marked like an unscalable one, which keeps every
+    // block pair of its block out of the symmetric items (W = nb - 1 on the device).
+    const bool force_near = real && !scaled_ok;
     const double r = sqrt(x * x + y * y + z * z);
     float rlo = real ? __double2float_rd(r) : __int_as_float(0x7f800000);
     float rhi = real ? __double2float_ru(r) : 0.0f;
