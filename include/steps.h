@@ -186,9 +186,13 @@ int steps_momentum(const double *vec, const double *mass, long long N, double *o
  * term of the sum in Eq. 5 is kept for each pair of particles" -- every separation x_j - x_i is replaced by its image of
  * smallest length in a cubic box of side L (component-wise d - L rint(d / L), ties to even), otherwise exactly
  * steps_forces / steps_forces_mixed (mixed != 0): same layout, same pair law with pair softening soft_i + soft_j, G = 1,
- * acc overwritten.  Positions need not lie inside [0, L).  First version: every tile pair goes through the per-pair
- * softening test (no far/near split in a periodic box) in the persistent stream-K driver.  The image sum of Eq. 5 with the
- * 2.6 L cut is steps_forces_periodic below.  STEPS_EINVAL additionally for L <= 0. */
+ * acc overwritten.  Positions need not lie inside [0, L): the fp64 path wraps separations, valid for |x_j - x_i| < 2^51 L;
+ * the mixed path casts positions to fp32 first, so it keeps its accuracy only for positions within a few L of the box
+ * (|x| / L < 2^22 is the hard limit of its wrap).  Fast path: CELL-ORDERED input (e.g. Morton order of a grid, see
+ * synth.morton_order) -- the periodic counterpart of the radial order: a (128-particle group, tile) pair whose bounding
+ * boxes are compact shares one image shift per component and runs the open-boundary far body; unordered input goes through
+ * the general wrapped body with the per-pair softening test for every tile -- slower, never wrong.  The image sum of Eq. 5
+ * with the 2.6 L cut is steps_forces_periodic below.  STEPS_EINVAL additionally for L <= 0. */
 int steps_forces_quasi_periodic(const double *pos, const double *mass, const double *soft, long long N,
                                 double L, double *acc, int mixed, steps_stream_t stream);
 
@@ -196,7 +200,10 @@ int steps_forces_quasi_periodic(const double *pos, const double *mass, const dou
  * images x - nL of every separation with the paper's cut |x - nL| < 2.6 L (strict), each image through the pair law with
  * pair softening soft_i + soft_j; fp64 path only (the images of a homogeneous box cancel to a small remainder).  Layout,
  * G = 1 and error behaviour as steps_forces_quasi_periodic; the result does not depend on which representative modulo L
- * the positions are given in.  Cost: 179 candidate images per pair (about 81 of them inside the cut). */
+ * the positions are given in (|x_j - x_i| < 2^51 L).  Cost: 179 candidate images per pair (74 of them inside the cut on
+ * average).  A particle's OWN images (j = i, n != 0) are summed like any other pair's: the triplet set is symmetric under
+ * n -> -n, so they cancel to rounding (the oracle skips j = i altogether).  Softening up to h_i + h_j <= L/2 takes the
+ * fast route (only the nearest image can then be softened); larger softening is handled image by image. */
 int steps_forces_periodic(const double *pos, const double *mass, const double *soft, long long N, double L,
                           double *acc, steps_stream_t stream);
 

@@ -7,7 +7,8 @@
 //     (b, c) is "far" when the radial intervals of the two blocks are separated by more than hmax_b + hmax_c (the same
 //     triangle-inequality test as tile_is_far, on block bounds): then no pair of it can be softened and every pair
 //     is exactly Newtonian.  W = max |c - b| over the block pairs that are NOT far (a device scalar, sym_band_width):
-//     for radially sorted input W = 1 (only neighbouring blocks touch), for unsorted input W = nb - 1.
+//     for radially sorted input W = 1 ... 7 (N = 131,072 ... 1,048,576: the softening shell spans more of the ever thinner
+//     radial blocks), for unsorted input W = nb - 1.
 //   * Block pairs with |c - b| <= W (the "band": the diagonal, all softened pairs, the self pairs) go through the
 //     asymmetric persistent kernel of force_driver.cuh, restricted to the band's tiles.
 //   * Every block pair with c - b > W is ONE work item of forces_sym_kernel: the CTA's 16 warps hold the 2048 particles of
