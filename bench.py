@@ -337,7 +337,7 @@ def main():
             kern_inter = float(cnt) * (n - 1.0)                 # this rank's launch
             achieved = FLOP_PER_INTERACTION * kern_inter / (k_ms * 1e-3) / 1e12
             traffic, traffic_source = ncu_traffic(path, n) if world == 1 else (None, "multi-GPU run")
-            symmetric = world == 1 and S.steps_pair_symmetric(n)
+            symmetric = world == 1 and S.steps_pair_symmetric(n, mixed)
             results[path] = {
                 "value": args.steps * inter_step / (total_ms * 1e-3), "unit": UNIT,
                 "ms_per_step": total_ms / args.steps, "force_kernel_ms": k_ms, "gpu_launches": int(launches),

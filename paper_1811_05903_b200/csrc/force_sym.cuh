@@ -82,7 +82,7 @@ __global__ void __launch_bounds__(128) sym_band_width(const Tile* __restrict__ t
 }
 
 // One CTA: the item count and the band's cumulative tile counts from W.
-__global__ void __launch_bounds__(1024) sym_plan_finalize(SymPlan* __restrict__ plan, int nb, int sym_min_items)
+__global__ void __launch_bounds__(1024) sym_plan_finalize(SymPlan* __restrict__ plan, int nb, int sym_min_items, int split)
 {
     long long* cum = reinterpret_cast<long long*>(plan + 1);
     __shared__ long long part[1024];
@@ -92,7 +92,7 @@ __global__ void __launch_bounds__(1024) sym_plan_finalize(SymPlan* __restrict__ 
         long long Km = nb - 1 - W;
         if (Km < 0) Km = 0;
         // too few items to balance over the SMs: everything through the band (W = nb - 1)
-        if (Km * (Km + 1) / 2 < sym_min_items) { W = nb - 1; Km = 0; }
+        if (Km * (Km + 1) / 2 * split < sym_min_items) { W = nb - 1; Km = 0; }
         plan->W = W; plan->nb = nb; plan->Km = (int)Km; plan->nt = nb * TPB; plan->K = Km * (Km + 1) / 2;
         sW = W;
     }
@@ -125,11 +125,13 @@ constexpr int SYM_FP64_RI = IB / SYM_FP64_THREADS;
 
 // Items [k_begin, k_end) of the plan's item list (one panel), shared out evenly over the grid.
 // rowrec / colrec: [k - k_begin][3][IB] doubles.  THREADS x RI = 2,048: THREADS / 32 warps hold the block, RI particles per lane.
-template <int THREADS, int RI>
+// SPLIT = false: one work unit per item (`split_arg` ignored, every loop bound a compile-time constant: the large-N kernel).
+template <int THREADS, int RI, bool SPLIT>
 __global__ void __launch_bounds__(THREADS, 1)
 forces_sym_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__ plan, long long k_begin, long long k_end,
-                  double* __restrict__ rowrec, double* __restrict__ colrec, int zero)
+                  double* __restrict__ rowrec, double* __restrict__ colrec, int zero, int split_arg)
 {
+    const int split = SPLIT ? split_arg : 1;
     static_assert(THREADS * RI == IB, "the CTA holds one block");
     constexpr int WI = 32 * RI;                 // particles per warp = sources per subgroup
     constexpr int SUBG = THREADS / 32;          // warps = subgroups per block
@@ -138,7 +140,9 @@ forces_sym_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__
     FarSrcF64* col = reinterpret_cast<FarSrcF64*>(smem_raw);                       // [2][IB]
     double* Bsm = reinterpret_cast<double*>(smem_raw + 2 * IB * sizeof(FarSrcF64));   // [3][IB]
 
-    const long long K = plan->K;
+    // `split` parts per item (the SUBG rounds of an item shared among `split` consecutive sub-items, so that a mid-size N
+    // still has enough work units for 148 SMs); [k_begin, k_end), the records and the grid's shares are in SUB-items
+    const long long K = plan->K * split;
     if (k_end > K) k_end = K;
     if (k_begin >= k_end) return;
     const int W = plan->W, nb = plan->nb, Km = plan->Km;
@@ -153,12 +157,13 @@ forces_sym_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__
     int b, c;
     {
         const double t = 2.0 * Km + 1.0;
-        int bb = (int)((t - sqrt(fmax(t * t - 8.0 * (double)kk0, 0.0))) * 0.5);
+        const long long item0 = kk0 / split;
+        int bb = (int)((t - sqrt(fmax(t * t - 8.0 * (double)item0, 0.0))) * 0.5);
         bb = max(0, min(bb, Km - 1));
-        while (bb + 1 < Km && sym_row_start(bb + 1, Km) <= kk0) ++bb;
-        while (bb > 0 && sym_row_start(bb, Km) > kk0) --bb;
+        while (bb + 1 < Km && sym_row_start(bb + 1, Km) <= item0) ++bb;
+        while (bb > 0 && sym_row_start(bb, Km) > item0) --bb;
         b = bb;
-        c = bb + W + 1 + (int)(kk0 - sym_row_start(bb, Km));
+        c = bb + W + 1 + (int)(item0 - sym_row_start(bb, Km));
     }
 
     if (threadIdx.x == 0) {
@@ -176,7 +181,7 @@ forces_sym_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__
         for (int t = 0; t < TPB; ++t)
             bulk_load(col + (size_t)s * IB + t * TJ, &tiles[(long long)pc * TPB + t].far[0], (uint32_t)(TJ * sizeof(FarSrcF64)),
                       &full_bar[s]);
-        if (++pc == nb) { ++pb; pc = pb + W + 1; }
+        if ((kk0 + it + 1) % split == 0 && ++pc == nb) { ++pb; pc = pb + W + 1; }     // the next sub-item starts a new item
     };
     if (threadIdx.x == 0) {
         produce(0);
@@ -208,7 +213,8 @@ forces_sym_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__
         __syncthreads();
         const FarSrcF64* cs = col + (size_t)s * IB;
 
-        for (int q = 0; q < SUBG; ++q) {
+        const int part = SPLIT ? (int)((kk0 + it) % split) : 0, rounds = SPLIT ? SUBG / split : SUBG;
+        for (int q = part * rounds; q < (part + 1) * rounds; ++q) {
             const int u = (warp + q) & (SUBG - 1);
             for (int t = 0; t < WI / 32; ++t) {
                 const FarSrcF64* set = cs + u * WI + t * 32;
@@ -282,7 +288,7 @@ forces_sym_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__
         }
         __syncthreads();                                          // stage s and Bsm are free again
         if (threadIdx.x == 0 && it + 2 < total) produce(it + 2);
-        if (++c == nb) { ++b; c = b + W + 1; }
+        if ((kk0 + it + 1) % split == 0 && ++c == nb) { ++b; c = b + W + 1; }
     }
 }
 
@@ -308,11 +314,12 @@ __host__ __device__ constexpr int sym_mixed_smem_bytes()
 constexpr int SYM_MIXED_THREADS = STEPS_SYM_MIXED_THREADS;
 constexpr int SYM_MIXED_RI = IB / SYM_MIXED_THREADS;
 
-template <int THREADS, int RI>
+template <int THREADS, int RI, bool SPLIT>
 __global__ void __launch_bounds__(THREADS, 1)
 forces_sym_mixed_kernel(const TileF32* __restrict__ tiles, const SymPlan* __restrict__ plan, long long k_begin, long long k_end,
-                        double* __restrict__ rowrec, double* __restrict__ colrec)
+                        double* __restrict__ rowrec, double* __restrict__ colrec, int split_arg)
 {
+    const int split = SPLIT ? split_arg : 1;
     static_assert(THREADS * RI == IB && RI % 2 == 0, "the CTA holds one block, particles packed in pairs");
     constexpr int NP = RI / 2;                  // packed pairs per lane
     constexpr int WI = 32 * RI;                 // particles per warp = sources per subgroup
@@ -324,7 +331,9 @@ forces_sym_mixed_kernel(const TileF32* __restrict__ tiles, const SymPlan* __rest
     double* Bsm = reinterpret_cast<double*>(smem_raw + 2 * STAGE);                     // [3][IB]
     double* Asm = Bsm + 3 * IB + threadIdx.x;                                          // [3][RI][THREADS], this thread's column
 
-    const long long K = plan->K;
+    // `split` parts per item (the SUBG rounds of an item shared among `split` consecutive sub-items, so that a mid-size N
+    // still has enough work units for 148 SMs); [k_begin, k_end), the records and the grid's shares are in SUB-items
+    const long long K = plan->K * split;
     if (k_end > K) k_end = K;
     if (k_begin >= k_end) return;
     const int W = plan->W, nb = plan->nb, Km = plan->Km;
@@ -338,12 +347,13 @@ forces_sym_mixed_kernel(const TileF32* __restrict__ tiles, const SymPlan* __rest
     int b, c;
     {
         const double t = 2.0 * Km + 1.0;
-        int bb = (int)((t - sqrt(fmax(t * t - 8.0 * (double)kk0, 0.0))) * 0.5);
+        const long long item0 = kk0 / split;
+        int bb = (int)((t - sqrt(fmax(t * t - 8.0 * (double)item0, 0.0))) * 0.5);
         bb = max(0, min(bb, Km - 1));
-        while (bb + 1 < Km && sym_row_start(bb + 1, Km) <= kk0) ++bb;
-        while (bb > 0 && sym_row_start(bb, Km) > kk0) --bb;
+        while (bb + 1 < Km && sym_row_start(bb + 1, Km) <= item0) ++bb;
+        while (bb > 0 && sym_row_start(bb, Km) > item0) --bb;
         b = bb;
-        c = bb + W + 1 + (int)(kk0 - sym_row_start(bb, Km));
+        c = bb + W + 1 + (int)(item0 - sym_row_start(bb, Km));
     }
     if (threadIdx.x == 0) {
         mbar_init(&full_bar[0], 1); mbar_init(&full_bar[1], 1);
@@ -358,7 +368,7 @@ forces_sym_mixed_kernel(const TileF32* __restrict__ tiles, const SymPlan* __rest
         for (int t = 0; t < TPB; ++t)          // X[], Y[], Z[], c[] are the first 4 TJ floats of a tile record
             bulk_load(reinterpret_cast<unsigned char*>(col) + (size_t)s * STAGE + t * (4 * TJ * sizeof(float)),
                       &tiles[(long long)pc * TPB + t].X[0], (uint32_t)(4 * TJ * sizeof(float)), &full_bar[s]);
-        if (++pc == nb) { ++pb; pc = pb + W + 1; }
+        if ((kk0 + it + 1) % split == 0 && ++pc == nb) { ++pb; pc = pb + W + 1; }     // the next sub-item starts a new item
     };
     if (threadIdx.x == 0) {
         produce(0);
@@ -393,7 +403,8 @@ forces_sym_mixed_kernel(const TileF32* __restrict__ tiles, const SymPlan* __rest
         __syncthreads();
         const float* cs = col + (size_t)s * (STAGE / sizeof(float));
 
-        for (int q = 0; q < SUBG; ++q) {
+        const int part = SPLIT ? (int)((kk0 + it) % split) : 0, rounds = SPLIT ? SUBG / split : SUBG;
+        for (int q = part * rounds; q < (part + 1) * rounds; ++q) {
             const int u = (warp + q) & (SUBG - 1);
             u64 ax[NP], ay[NP], az[NP];
 #pragma unroll
@@ -459,7 +470,7 @@ forces_sym_mixed_kernel(const TileF32* __restrict__ tiles, const SymPlan* __rest
         }
         __syncthreads();
         if (threadIdx.x == 0 && it + 2 < total) produce(it + 2);
-        if (++c == nb) { ++b; c = b + W + 1; }
+        if ((kk0 + it + 1) % split == 0 && ++c == nb) { ++b; c = b + W + 1; }
     }
 }
 
@@ -467,11 +478,11 @@ forces_sym_mixed_kernel(const TileF32* __restrict__ tiles, const SymPlan* __rest
 __global__ void __launch_bounds__(256)
 forces_sym_reduce_kernel(const SymPlan* __restrict__ plan, const double* __restrict__ rowrec, const double* __restrict__ colrec,
                          long long k_begin, long long k_end, long long N, double* __restrict__ acc_hi,
-                         double* __restrict__ acc_lo, int last, double* __restrict__ acc_out)
+                         double* __restrict__ acc_lo, int last, double* __restrict__ acc_out, int split)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
-    const long long K = plan->K;
+    const long long K = plan->K * split;               // sub-items (see forces_sym_kernel)
     if (k_end > K) k_end = K;
     const int W = plan->W, Km = plan->Km;
     const int b = (int)(i / IB), off = (int)(i - (long long)b * IB);
@@ -490,13 +501,13 @@ forces_sym_reduce_kernel(const SymPlan* __restrict__ plan, const double* __restr
     };
     if (k_begin < k_end) {
         if (b < Km) {                                              // this block as the row of its items
-            const long long r0 = sym_row_start(b, Km), r1 = r0 + (Km - b);
+            const long long r0 = sym_row_start(b, Km) * split, r1 = r0 + (long long)(Km - b) * split;
             for (long long k = max(r0, k_begin); k < min(r1, k_end); ++k) add(rowrec, k);
         }
         const int rows = min(Km, b - W);                           // this block as the column of item (bb, b), bb + W < b
         for (int bb = 0; bb < rows; ++bb) {
-            const long long k = sym_row_start(bb, Km) + (b - bb - W - 1);
-            if (k >= k_begin && k < k_end) add(colrec, k);
+            const long long k0 = (sym_row_start(bb, Km) + (b - bb - W - 1)) * split;
+            for (long long k = max(k0, k_begin); k < min(k0 + split, k_end); ++k) add(colrec, k);
         }
     }
 #pragma unroll

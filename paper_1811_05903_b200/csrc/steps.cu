@@ -35,7 +35,8 @@ constexpr int MAX_GRID = 148 * 4;
 
 // Pair-symmetric evaluation (force_sym.cuh) of the fp64 path: used for full evaluations of at least SYM_MIN_BLOCKS blocks;
 // its partial records are produced and consumed in panels of at most g_sym_panel_items items (96 KiB of records each).
-constexpr int SYM_MIN_BLOCKS = 64;
+constexpr int SYM_MIN_BLOCKS = 16;         // fp64: from N = 30,721, with the items split into parts while the blocks are few
+constexpr int SYM_MIN_BLOCKS_MIXED = 64;   // mixed: whole items only (its split variant is slower than the ring kernel): N >= 129,025
 std::atomic<long long> g_sym_panel_items{16384};
 std::atomic<int> g_sym_enabled{1};
 std::atomic<int> g_splitj{1};           // 0 = never use the split-j driver (testing)
@@ -60,6 +61,7 @@ struct Workspace {
     int cc_major = -1;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;   // "profile" option: around the last force kernel(s)
     bool ev_valid = false;
+    bool sym_split_ready = false, sym_split_ready_mixed = false;
     // One scratch area per device: calls on different streams are serialised through this event (see claim_scratch).
     cudaEvent_t scratch_done = nullptr;
     cudaStream_t scratch_stream = nullptr;
@@ -74,9 +76,12 @@ inline long long ntiles_padded(long long N) { return nblocks_of(N) * TPB; }     
 inline size_t partial_bytes(long long N) { return sizeof(double) * 6 * IB * (size_t)(nblocks_of(N) + MAX_GRID); }
 inline size_t tile_bytes_max() { return sizeof(TileF64) > sizeof(TileF32) ? sizeof(TileF64) : sizeof(TileF32); }
 inline long long sym_items_max(long long N) { const long long nb = nblocks_of(N); return nb * (nb - 1) / 2; }
-inline long long sym_panel_items_for(long long N) { return std::max(1ll, std::min(sym_items_max(N), g_sym_panel_items.load())); }
+inline long long sym_panel_items_for(long long N) { return std::max(1ll, std::min(16 * sym_items_max(N), g_sym_panel_items.load())); }
 inline size_t sym_record_bytes(long long items) { return sizeof(double) * 2 * 3 * IB * (size_t)items; }
-inline bool sym_eligible(long long N) { return g_sym_enabled.load() != 0 && nblocks_of(N) >= SYM_MIN_BLOCKS; }
+inline bool sym_eligible(long long N, bool mixed = false)
+{
+    return g_sym_enabled.load() != 0 && nblocks_of(N) >= (mixed ? SYM_MIN_BLOCKS_MIXED : SYM_MIN_BLOCKS);
+}
 
 int cuda_fail(cudaError_t e)
 {
@@ -209,35 +214,57 @@ int launch_forces_sym(const double* pos, const double* mass, const double* soft,
     auto band = forces_persistent_kernel<Path, STAGES, 0, true>;
     int rc = persistent_grid(band, smem_band, w, FP64 ? w.grid_fp64_band : w.grid_mixed_band);
     if (rc != STEPS_OK) return rc;
-    if constexpr (FP64) rc = persistent_grid(forces_sym_kernel<SYM_FP64_THREADS, SYM_FP64_RI>, sym_smem_bytes(), w, w.grid_sym, SYM_FP64_THREADS);
-    if (FP64 && w.grid_sym > w.num_sms) w.grid_sym = w.num_sms;
-    else rc = persistent_grid(forces_sym_mixed_kernel<SYM_MIXED_THREADS, SYM_MIXED_RI>, sym_mixed_smem_bytes<SYM_MIXED_THREADS, SYM_MIXED_RI>(),
-                              w, w.grid_sym_mixed, SYM_MIXED_THREADS);
-    if (!FP64 && w.grid_sym_mixed > w.num_sms) w.grid_sym_mixed = w.num_sms;      // one CTA per SM: the item shares stay equal
+    int unused = 0;                                  // the SPLIT variants only need their shared-memory attribute set
+    if constexpr (FP64) {
+        rc = persistent_grid(forces_sym_kernel<SYM_FP64_THREADS, SYM_FP64_RI, false>, sym_smem_bytes(), w, w.grid_sym, SYM_FP64_THREADS);
+        if (rc == STEPS_OK && !w.sym_split_ready)
+            rc = persistent_grid(forces_sym_kernel<SYM_FP64_THREADS, SYM_FP64_RI, true>, sym_smem_bytes(), w, unused, SYM_FP64_THREADS);
+        if (w.grid_sym > w.num_sms) w.grid_sym = w.num_sms;
+    } else {
+        rc = persistent_grid(forces_sym_mixed_kernel<SYM_MIXED_THREADS, SYM_MIXED_RI, false>, sym_mixed_smem_bytes<SYM_MIXED_THREADS, SYM_MIXED_RI>(),
+                             w, w.grid_sym_mixed, SYM_MIXED_THREADS);
+        if (rc == STEPS_OK && !w.sym_split_ready_mixed)
+            rc = persistent_grid(forces_sym_mixed_kernel<SYM_MIXED_THREADS, SYM_MIXED_RI, true>, sym_mixed_smem_bytes<SYM_MIXED_THREADS, SYM_MIXED_RI>(),
+                                 w, unused, SYM_MIXED_THREADS);
+        if (w.grid_sym_mixed > w.num_sms) w.grid_sym_mixed = w.num_sms;      // one CTA per SM: the item shares stay equal
+    }
     if (rc != STEPS_OK) return rc;
+    (FP64 ? w.sym_split_ready : w.sym_split_ready_mixed) = true;
     const int P = FP64 ? w.grid_fp64_band : w.grid_mixed_band, Ps = FP64 ? w.grid_sym : w.grid_sym_mixed;
     const bool prof = g_profile.load() != 0;
     if (prof && !w.ev0) { STEPS_CUDA(cudaEventCreate(&w.ev0)); STEPS_CUDA(cudaEventCreate(&w.ev1)); }
 
+    // Parts per item: with few blocks an item (0.3-0.7 ms) is too coarse a unit for 148 SMs, so its rounds are shared among
+    // `split` sub-items (a power of two, at most the warps per CTA) until there are about 24 of them per CTA.
+    int split = 1;
+    const int max_split = (FP64 ? SYM_FP64_THREADS : SYM_MIXED_THREADS) / 32;
+    if constexpr (FP64)
+        while (split < max_split && sym_items_max(N) * split < 24ll * Ps) split *= 2;
+
     prep_tiles<Tile><<<ntp, TJ, 0, st>>>(pos, mass, soft, N, tiles, &w.plan->W);
     sym_band_width<Tile><<<nb, 128, 0, st>>>(tiles, nb, w.plan);
-    sym_plan_finalize<<<1, 1024, 0, st>>>(w.plan, nb, 8 * Ps);
+    sym_plan_finalize<<<1, 1024, 0, st>>>(w.plan, nb, 8 * Ps, split);
     if (prof) STEPS_CUDA(cudaEventRecord(w.ev0, st));
     band<<<P, CTA_THREADS, smem_band, st>>>(pos, soft, N, tiles, ntp, 0, N, nb, w.partials, 0, 0.0, 0.0, w.plan, 1);
     double* hi = w.acc_dd;
     double* lo = w.acc_dd + 3 * N;
     forces_band_reduce_kernel<Path::NOUT><<<(int)((N + 255) / 256), 256, 0, st>>>(w.partials, w.plan, P, N, acc_out, 1, hi, lo);
     g_launches += 5;
-    const long long items = w.sym_panel_items, kmax = sym_items_max(N);
+    const long long items = w.sym_panel_items, kmax = sym_items_max(N) * split;          // in sub-items
     double* rowrec = w.sym_records;
     double* colrec = w.sym_records + (size_t)items * 3 * IB;
     for (long long k0 = 0; k0 < kmax; k0 += items) {
         const long long k1 = std::min(kmax, k0 + items);
-        if constexpr (FP64) forces_sym_kernel<SYM_FP64_THREADS, SYM_FP64_RI><<<Ps, SYM_FP64_THREADS, sym_smem_bytes(), st>>>(tiles, w.plan, k0, k1, rowrec, colrec, 0);
-        else forces_sym_mixed_kernel<SYM_MIXED_THREADS, SYM_MIXED_RI><<<Ps, SYM_MIXED_THREADS, sym_mixed_smem_bytes<SYM_MIXED_THREADS, SYM_MIXED_RI>(), st>>>(
-                tiles, w.plan, k0, k1, rowrec, colrec);
+        if constexpr (FP64) {
+            auto k = split == 1 ? forces_sym_kernel<SYM_FP64_THREADS, SYM_FP64_RI, false> : forces_sym_kernel<SYM_FP64_THREADS, SYM_FP64_RI, true>;
+            k<<<Ps, SYM_FP64_THREADS, sym_smem_bytes(), st>>>(tiles, w.plan, k0, k1, rowrec, colrec, 0, split);
+        } else {
+            auto k = split == 1 ? forces_sym_mixed_kernel<SYM_MIXED_THREADS, SYM_MIXED_RI, false>
+                                : forces_sym_mixed_kernel<SYM_MIXED_THREADS, SYM_MIXED_RI, true>;
+            k<<<Ps, SYM_MIXED_THREADS, sym_mixed_smem_bytes<SYM_MIXED_THREADS, SYM_MIXED_RI>(), st>>>(tiles, w.plan, k0, k1, rowrec, colrec, split);
+        }
         forces_sym_reduce_kernel<<<(int)((N + 255) / 256), 256, 0, st>>>(w.plan, rowrec, colrec, k0, k1, N, hi, lo,
-                                                                          k1 == kmax ? 1 : 0, acc_out);
+                                                                          k1 == kmax ? 1 : 0, acc_out, split);
         g_launches += 2;
     }
     if (prof) { STEPS_CUDA(cudaEventRecord(w.ev1, st)); w.ev_valid = true; }
@@ -300,7 +327,7 @@ int launch_forces(const double* pos, const double* mass, const double* soft, lon
                   long long cnt_strided = 0)
 {
     using Tile = typename Path::Tile;
-    if (block_stride == 1 && i_begin == 0 && i_end == N && g_driver.load() == 0 && sym_eligible(N) && w.sym_records &&
+    if (block_stride == 1 && i_begin == 0 && i_end == N && g_driver.load() == 0 && sym_eligible(N, Path::NOUT == 3) && w.sym_records &&
         (Path::NOUT == 6 || g_sym_enabled.load() != 2))      // "sym" = 2: fp64 path only
         return launch_forces_sym<Path>(pos, mass, soft, N, acc_out, st, w);
     const int nt = (int)ntiles_of(N);
@@ -829,7 +856,7 @@ double steps_last_force_kernel_ms(void)
     return (double)ms;
 }
 
-int steps_pair_symmetric(long long N) { return N >= 1 && sym_eligible(N) && g_driver.load() == 0 ? 1 : 0; }
+int steps_pair_symmetric(long long N, int mixed) { return N >= 1 && sym_eligible(N, mixed != 0) && g_driver.load() == 0 ? 1 : 0; }
 
 int steps_persistent_grid(int mixed)
 {

@@ -97,7 +97,7 @@ def load_library(path: str) -> C.CDLL:
     L.steps_set_option.argtypes = [C.c_char_p, ll]
     L.steps_last_force_kernel_ms.restype = dbl
     L.steps_persistent_grid.argtypes = [i32]
-    L.steps_pair_symmetric.argtypes = [ll]
+    L.steps_pair_symmetric.argtypes = [ll, i32]
     return L
 
 
@@ -304,5 +304,5 @@ def steps_persistent_grid(mixed: bool) -> int:
     return int(lib().steps_persistent_grid(int(mixed)))
 
 
-def steps_pair_symmetric(n: int) -> bool:
-    return bool(lib().steps_pair_symmetric(n))
+def steps_pair_symmetric(n: int, mixed: bool = False) -> bool:
+    return bool(lib().steps_pair_symmetric(n, int(mixed)))
