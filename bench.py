@@ -245,6 +245,8 @@ def main():
     ap.add_argument("--ref-pairs", type=float, default=4e9, help="--impl reference: pair budget per step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-next-rows", action="store_true", help="skip the periodic / adaptive-step rows (SURVEY 8(f))")
+    ap.add_argument("--sharded-step", action="store_true",
+                    help="time the N > 1 step (shard.ShardedStep: steps_forces_blocks + exchange) even with one rank")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -297,7 +299,7 @@ def main():
             mixed = path == "mixed"
             x = pos.clone()
             co = S.KdkCoeffs(1.0, 0.0, sched["alpha_open"], sched["beta_open"], sched["gamma"], B, int(mixed))
-            if world == 1:
+            if world == 1 and not args.sharded_step:
                 v, acc = torch.zeros_like(x), torch.empty_like(x)
                 (S.steps_forces_mixed if mixed else S.steps_forces)(x, mass, soft, acc)
 
@@ -336,8 +338,9 @@ def main():
             peak = PEAK_FP32_TFLOPS if mixed else PEAK_FP64_TFLOPS
             kern_inter = float(cnt) * (n - 1.0)                 # this rank's launch
             achieved = FLOP_PER_INTERACTION * kern_inter / (k_ms * 1e-3) / 1e12
-            traffic, traffic_source = ncu_traffic(path, n) if world == 1 else (None, "multi-GPU run")
-            symmetric = world == 1 and S.steps_pair_symmetric(n, mixed)
+            sharded = world > 1 or args.sharded_step
+            traffic, traffic_source = ncu_traffic(path, n) if not sharded else (None, "sharded step (one-sided kernel)")
+            symmetric = not sharded and S.steps_pair_symmetric(n, mixed)
             results[path] = {
                 "value": args.steps * inter_step / (total_ms * 1e-3), "unit": UNIT,
                 "ms_per_step": total_ms / args.steps, "force_kernel_ms": k_ms, "gpu_launches": int(launches),
@@ -395,7 +398,7 @@ def main():
         "config": {"workload": f"config3: compactified g0 set (S^3 stereographic, m~(1+r^2/4R^2)^3, eps_i=0.01(m_i/m_min)^(1/3)), N={n}, "
                                f"one steps_kdk_step (kick+drift+prep+force+reduce) + momentum per step",
                    "headline_path": head, "l2": "256 MiB flush write between timed steps (inputs 42 MB fit L2; ALU-bound)",
-                   "i_sharding": "none" if world == 1 else f"i-blocks of 2048 dealt round-robin to {world} ranks (PAPER L135-139, SURVEY 8(e)), all-gather of positions",
+                   "i_sharding": "none" if world == 1 and not args.sharded_step else f"i-blocks of 2048 dealt round-robin to {world} ranks (PAPER L135-139, SURVEY 8(e)), all-gather of positions",
                    "persistent_grid": {p: S.steps_persistent_grid(p == "mixed") for p in results}},
         "roofline": r["roofline"], "paths": results, "clocks": clocks, "gpu_launches": int(launches_total),
         "e2e": e2e, "cpu_baseline": cpu, "next_rows": next_rows, "build": S.build_info(),

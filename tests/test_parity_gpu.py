@@ -672,12 +672,15 @@ def test_device_resident_adaptive_run_matches_oracle(S, oracle, mode):
 
 
 @pytest.mark.gpu
-def test_device_resident_steps_replay_from_a_cuda_graph(S, oracle):
+@pytest.mark.parametrize("n,mixed", [(4096, False), (40000, False), (140000, True)])
+def test_device_resident_steps_replay_from_a_cuda_graph(S, oracle, n, mixed):
     """Five adaptive steps captured ONCE in a CUDA graph and replayed four times give bit for bit the state of twenty
     eager calls: the whole step (time-step criterion, coefficients, kick/drift, tile prep, forces, reduce) is
-    stream-ordered device work with no host dependence."""
+    stream-ordered device work with no host dependence.  N = 4,096: split-j driver; 40,000: fp64 band + pair-symmetric
+    sub-items; 140,000 mixed: band + pair-symmetric items -- their plan (band width, item count) is computed on the device
+    inside the captured sequence.  Also: a call that would have to allocate workspace under capture is refused."""
     import torch
-    ps = _config4(oracle, 4096)
+    ps = _config4(oracle, n)
     B, G, eps, dt_max, a0 = 1.0 / ps.r_cut ** 3, 1.0, 0.025, 0.5, 1 / 51
     c = S.Cosmology(**LCDM)
     dm, dh = dev(ps.mass), dev(ps.soft)
@@ -685,12 +688,12 @@ def test_device_resident_steps_replay_from_a_cuda_graph(S, oracle):
     def fresh():
         dpos, dvel = dev(ps.pos), dev(ps.vel)
         dacc = torch.empty_like(dpos)
-        S.steps_forces(dpos, dm, dh, dacc)
+        (S.steps_forces_mixed if mixed else S.steps_forces)(dpos, dm, dh, dacc)
         return dpos, dvel, dacc, torch.tensor([a0, 0.0, 1.0, 0.0, 0.0], dtype=torch.float64, device="cuda")
 
     pos_e, vel_e, acc_e, st_e = fresh()
     for _ in range(20):
-        S.steps_kdk_step_adaptive(pos_e, vel_e, acc_e, dm, dh, st_e, c, G, B, eps, dt_max)
+        S.steps_kdk_step_adaptive(pos_e, vel_e, acc_e, dm, dh, st_e, c, G, B, eps, dt_max, mixed=mixed)
     torch.cuda.synchronize()
 
     pos_g, vel_g, acc_g, st_g = fresh()
@@ -700,7 +703,12 @@ def test_device_resident_steps_replay_from_a_cuda_graph(S, oracle):
     with torch.cuda.stream(side):
         with torch.cuda.graph(g, stream=side):
             for _ in range(5):
-                S.steps_kdk_step_adaptive(pos_g, vel_g, acc_g, dm, dh, st_g, c, G, B, eps, dt_max)
+                S.steps_kdk_step_adaptive(pos_g, vel_g, acc_g, dm, dh, st_g, c, G, B, eps, dt_max, mixed=mixed)
+            if n == 4096:                         # a larger N than any reserved so far would need cudaMalloc: refused
+                big = 3 * 1024 * 1024 + 77
+                z = torch.empty(0)                # never dereferenced: the call returns before any launch
+                rc = S.lib().steps_forces(pos_g.data_ptr(), dm.data_ptr(), dh.data_ptr(), big, acc_g.data_ptr(), side.cuda_stream)
+                assert rc == S.ECAPTURE, rc
     torch.cuda.current_stream().wait_stream(side)
     for _ in range(4):
         g.replay()
