@@ -227,7 +227,13 @@ double steps_timestep_coefficient(double G, double a);
  * step + opening kick + drift; force evaluation at the new positions into acc; state advanced to a_{n+1}.  acc must hold
  * the forces at the current positions on entry (steps_forces before the first call).  steps_kick_close_adaptive applies
  * the pending closing half kick (end of a run, or before velocities are read) and resets it to the identity.
- * G < 0 = reversed gravity (glass generation).  cosmo is read on the host at call time. */
+ * G < 0 = reversed gravity (glass generation).  cosmo is read on the host at call time.
+ * Eq. 12's minimum is FUSED into the last kernel of the call's force evaluation (it writes every acc_i anyway) and used by
+ * the next call when that call follows directly -- same pos/acc/soft/state5 pointers, N, |G|, B, eps and no other call of
+ * this library in between; otherwise the next call forms the minimum with a separate O(N) pass (always on the first step).
+ * Consequence for the caller: between two consecutive calls, change pos, acc, soft or state5 only through this library
+ * (as the contract above already demands of acc), or switch the shortcut off with steps_set_option("fuse_eq12", 0).
+ * Both ways give bit-identical steps. */
 int steps_kdk_step_adaptive(double *pos, double *vel, double *acc, const double *mass, const double *soft,
                             long long N, double *state5, const steps_cosmology *cosmo, double G, double B,
                             double eps, double dt_max, int mixed, steps_stream_t stream);
@@ -257,7 +263,8 @@ long long steps_kernel_launch_count(void);
  * the force kernel(s) of every later call with CUDA events recorded on the call's stream.
  * "sym": 0 = never use the pair-symmetric evaluation (default 1).  "sym_panel_items": how many
  * block-pair items (96 KiB of partial records each) the symmetric evaluation keeps in flight
- * (default 16384 = 1.5 GiB; the items are run in panels of this size).  Unknown key: STEPS_EINVAL. */
+ * (default 16384 = 1.5 GiB; the items are run in panels of this size).  "splitj": 0 = never use the split-j driver.
+ * "fuse_eq12": 0 = steps_kdk_step_adaptive always forms Eq. 12's minimum in its own pass.  Unknown key: STEPS_EINVAL. */
 int steps_set_option(const char *key, long long value);
 /* With "profile" on: device time in ms of the most recent force kernel launched on the current
  * device (waits for it to finish); -1 if none was recorded.  For a pair-symmetric evaluation: from the

@@ -153,6 +153,38 @@ __device__ __forceinline__ void sub_if_above(double& d, long long half_bits, dou
         : "+d"(d) : "l"(__double_as_longlong(d)), "l"(half_bits), "d"(neg_period));
 }
 
+// ---- Eq. 12 fused into the force evaluation's last kernel ------------------------------------------
+// When `out_bits` is set, the kernel that writes the final accelerations of a FULL evaluation also forms every particle's
+// step-length candidate sqrt(2 (2.8 h_i) eps / |A_i|), A_i = |G| a^-3 (acc_i + B x_i) (Eq. 12, DESIGN.md
+// reading #11; a read from the device-resident run state) and folds the minimum into *out_bits with an atomicMin on the bit
+// pattern (positive doubles order like their bit patterns; the minimum is exact, so the order of the atomics is immaterial).
+// steps_kdk_step_adaptive uses it to skip the separate O(N) pass over (pos, acc, soft) at the start of the NEXT step.
+struct Eq12Fuse {
+    const double* pos;
+    const double* soft;
+    const double* a_state;            // &RunState::a
+    double absG, B, eps;
+    unsigned long long* out_bits;     // nullptr: off
+};
+// The candidate of one particle, exactly the arithmetic of the unfused pass (timestep_state_stage1 calls this too).
+__device__ __forceinline__ double eq12_candidate(double ax, double ay, double az, double x, double y, double z, double h,
+                                                 double coef, double B, double eps, double dt)
+{
+    const double Ax = coef * (ax + B * x);
+    const double Ay = coef * (ay + B * y);
+    const double Az = coef * (az + B * z);
+    const double A = sqrt(Ax * Ax + Ay * Ay + Az * Az);
+    if (A > 0.0) dt = fmin(dt, sqrt(2.0 * (2.8 * h) * eps / A));
+    return dt;
+}
+__device__ __forceinline__ void eq12_fold(const Eq12Fuse& f, double dt)       // every thread of the warp calls it
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) dt = fmin(dt, __shfl_xor_sync(0xffffffffu, dt, o));
+    if ((threadIdx.x & 31) == 0) atomicMin(f.out_bits, (unsigned long long)__double_as_longlong(dt));
+}
+#define STEPS_DT_INF_BITS 0x7ff0000000000000ull
+
 // Never-taken branch on bit n of `zero` (always 0, unknown to the compiler): ends a basic block, which
 // is the only ordering ptxas respects.  One uniform-datapath branch per use, no FP64-pipe work.
 #define STEPS_STAGE_FENCE(zero, n)                                                              \

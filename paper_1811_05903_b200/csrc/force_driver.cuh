@@ -275,10 +275,12 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
 // Fixed-order sum of the partial records of each i-block -> acc_out (SoA over [i_begin, i_end)).
 template <int NOUT>
 __global__ void __launch_bounds__(256) forces_reduce_kernel(const double* __restrict__ partials, int nt, int nb, int P,
-                                                            long long cnt, double* __restrict__ acc_out)
+                                                            long long cnt, double* __restrict__ acc_out, Eq12Fuse fuse)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= cnt) return;
+    double dt = __longlong_as_double((long long)STEPS_DT_INF_BITS);
+    if (i < cnt) {
+    double a3[3];
     const int b = (int)(i / IB), off = (int)(i - (long long)b * IB);
     const long long W = (long long)nb * nt;
     // CTA p owns w in [floor(p W / P), floor((p+1) W / P));  the CTA that owns w is floor(((w+1) P - 1) / W)
@@ -297,8 +299,16 @@ __global__ void __launch_bounds__(256) forces_reduce_kernel(const double* __rest
             hi = s;
             if (NOUT == 6) lo += rec[(long long)(3 + c) * IB];
         }
-        acc_out[(long long)c * cnt + i] = hi + lo;
+        a3[c] = hi + lo;
+        acc_out[(long long)c * cnt + i] = a3[c];
     }
+    if (fuse.out_bits) {                                    // full evaluations only: i is the particle index, cnt = N
+        const double a = *fuse.a_state, coef = fuse.absG / (a * a * a);
+        dt = eq12_candidate(a3[0], a3[1], a3[2], fuse.pos[i], fuse.pos[cnt + i], fuse.pos[2 * cnt + i], fuse.soft[i], coef, fuse.B,
+                            fuse.eps, dt);
+    }
+    }
+    if (fuse.out_bits) eq12_fold(fuse, dt);                 // all 32 lanes of every warp, valid particle or not
 }
 
 // The same for the BAND mode (rows of different lengths: the owners of a row come from the plan's cumulative counts).
@@ -350,9 +360,11 @@ template <typename Path, int BOX>
 __global__ void __launch_bounds__(CTA_THREADS, 1)
 forces_splitj_kernel(const double* __restrict__ pos, const double* __restrict__ soft, long long N,
                      const typename Path::Tile* __restrict__ tiles, int nt, int sub, long long i_begin, long long i_end,
-                     double* __restrict__ acc_out, double* __restrict__ partials, int zero, double box_L, double box_invL)
+                     double* __restrict__ acc_out, double* __restrict__ partials, int zero, double box_L, double box_invL,
+                     Eq12Fuse fuse)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ double res[3][SPLITJ_GROUP];                                // the group's final accelerations (Eq. 12 fusion)
     double* acc_all = reinterpret_cast<double*>(smem_raw);                 // [NOUT * R_I][CTA_THREADS]
     double* acc = acc_all + threadIdx.x;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -413,19 +425,36 @@ forces_splitj_kernel(const double* __restrict__ pos, const double* __restrict__ 
         const long long i = (long long)blockIdx.x * SPLITJ_GROUP + l + 32 * k;        // within [i_begin, i_end)
         if (gridDim.y == 1) {
             if (i < cnt) acc_out[(long long)c * cnt + i] = hi + lo;
+            res[c][r] = hi + lo;
         } else {
             double* rec = partials + (((long long)blockIdx.x * gridDim.y + blockIdx.y) * 6) * SPLITJ_GROUP;
             rec[c * SPLITJ_GROUP + r] = hi; rec[(3 + c) * SPLITJ_GROUP + r] = lo;
         }
     }
+    if (fuse.out_bits != nullptr && gridDim.y == 1) {                       // full evaluations only (i_begin = 0, cnt = N)
+        __syncthreads();
+        if (threadIdx.x < SPLITJ_GROUP) {
+            const int r = threadIdx.x, k = r / 32, l = r % 32;
+            const long long i = (long long)blockIdx.x * SPLITJ_GROUP + l + 32 * k;
+            double dt = __longlong_as_double((long long)STEPS_DT_INF_BITS);
+            if (i < cnt) {
+                const double a = *fuse.a_state, coef = fuse.absG / (a * a * a);
+                dt = eq12_candidate(res[0][r], res[1][r], res[2][r], fuse.pos[i], fuse.pos[cnt + i], fuse.pos[2 * cnt + i], fuse.soft[i],
+                                    coef, fuse.B, fuse.eps, dt);
+            }
+            eq12_fold(fuse, dt);
+        }
+    }
 }
 
 __global__ void __launch_bounds__(128) forces_splitj_reduce(const double* __restrict__ partials, int jsplit, long long cnt,
-                                                            double* __restrict__ acc_out)
+                                                            double* __restrict__ acc_out, Eq12Fuse fuse)
 {
     const int r = threadIdx.x, k = r / 32, l = r % 32;
     const long long i = (long long)blockIdx.x * SPLITJ_GROUP + l + 32 * k;
-    if (i >= cnt) return;
+    double dt = __longlong_as_double((long long)STEPS_DT_INF_BITS);
+    if (i < cnt) {
+    double a3[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         double hi = 0.0, lo = 0.0;
@@ -437,8 +466,16 @@ __global__ void __launch_bounds__(128) forces_splitj_reduce(const double* __rest
             hi = t;
             lo += rec[(3 + c) * SPLITJ_GROUP + r];
         }
-        acc_out[(long long)c * cnt + i] = hi + lo;
+        a3[c] = hi + lo;
+        acc_out[(long long)c * cnt + i] = a3[c];
     }
+    if (fuse.out_bits) {
+        const double a = *fuse.a_state, coef = fuse.absG / (a * a * a);
+        dt = eq12_candidate(a3[0], a3[1], a3[2], fuse.pos[i], fuse.pos[cnt + i], fuse.pos[2 * cnt + i], fuse.soft[i], coef, fuse.B,
+                            fuse.eps, dt);
+    }
+    }
+    if (fuse.out_bits) eq12_fold(fuse, dt);
 }
 
 // ---- simple driver (cross-check) -----------------------------------------------------------------

@@ -478,10 +478,11 @@ forces_sym_mixed_kernel(const TileF32* __restrict__ tiles, const SymPlan* __rest
 __global__ void __launch_bounds__(256)
 forces_sym_reduce_kernel(const SymPlan* __restrict__ plan, const double* __restrict__ rowrec, const double* __restrict__ colrec,
                          long long k_begin, long long k_end, long long N, double* __restrict__ acc_hi,
-                         double* __restrict__ acc_lo, int last, double* __restrict__ acc_out, int split)
+                         double* __restrict__ acc_lo, int last, double* __restrict__ acc_out, int split, Eq12Fuse fuse)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
+    double dt = __longlong_as_double((long long)STEPS_DT_INF_BITS);
+    if (i < N) {
     const long long K = plan->K * split;               // sub-items (see forces_sym_kernel)
     if (k_end > K) k_end = K;
     const int W = plan->W, Km = plan->Km;
@@ -515,6 +516,13 @@ forces_sym_reduce_kernel(const SymPlan* __restrict__ plan, const double* __restr
         if (last) acc_out[cc * N + i] = hi[cc] + lo[cc];
         else { acc_hi[cc * N + i] = hi[cc]; acc_lo[cc * N + i] = lo[cc]; }
     }
+    if (last && fuse.out_bits) {
+        const double a = *fuse.a_state, coef = fuse.absG / (a * a * a);
+        dt = eq12_candidate(hi[0] + lo[0], hi[1] + lo[1], hi[2] + lo[2], fuse.pos[i], fuse.pos[N + i], fuse.pos[2 * N + i], fuse.soft[i],
+                            coef, fuse.B, fuse.eps, dt);
+    }
+    }
+    if (last && fuse.out_bits) eq12_fold(fuse, dt);
 }
 
 }  // namespace steps

@@ -72,13 +72,8 @@ __global__ void __launch_bounds__(256) timestep_stage1(const double* __restrict_
 {
     double dt = dt_max;
     const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
-        const double Ax = coef * (acc[i] + B * pos[i]);
-        const double Ay = coef * (acc[N + i] + B * pos[N + i]);
-        const double Az = coef * (acc[2 * N + i] + B * pos[2 * N + i]);
-        const double A = sqrt(Ax * Ax + Ay * Ay + Az * Az);
-        if (A > 0.0) dt = fmin(dt, sqrt(2.0 * (2.8 * soft[i]) * eps / A));
-    }
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride)
+        dt = eq12_candidate(acc[i], acc[N + i], acc[2 * N + i], pos[i], pos[N + i], pos[2 * N + i], soft[i], coef, B, eps, dt);
     __shared__ double sh[8];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) dt = fmin(dt, __shfl_down_sync(0xffffffffu, dt, o));
@@ -158,13 +153,8 @@ __global__ void __launch_bounds__(256) timestep_state_stage1(const double* __res
     const double coef = absG / (a * a * a);
     double dt = dt_max;
     const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
-        const double Ax = coef * (acc[i] + B * pos[i]);
-        const double Ay = coef * (acc[N + i] + B * pos[N + i]);
-        const double Az = coef * (acc[2 * N + i] + B * pos[2 * N + i]);
-        const double A = sqrt(Ax * Ax + Ay * Ay + Az * Az);
-        if (A > 0.0) dt = fmin(dt, sqrt(2.0 * (2.8 * soft[i]) * eps / A));
-    }
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride)
+        dt = eq12_candidate(acc[i], acc[N + i], acc[2 * N + i], pos[i], pos[N + i], pos[2 * N + i], soft[i], coef, B, eps, dt);
     __shared__ double sh[8];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) dt = fmin(dt, __shfl_down_sync(0xffffffffu, dt, o));
@@ -179,12 +169,20 @@ __global__ void __launch_bounds__(256) timestep_state_stage1(const double* __res
 // Stage 2 + the step's coefficients (the arithmetic of steps_kdk_schedule, on the device): writes the six kick/drift
 // scalars of THIS step to coef6 = {alpha_close(prev), beta_close(prev), alpha_open, beta_open, gamma, B} and advances
 // the state to a_{n+1} with the new closing coefficients.
+// fused_bits != nullptr: the minimum over the particles was folded into *fused_bits by the previous force evaluation
+// (Eq12Fuse in common.cuh) instead of into `partial` (all bits set = no particle put a limit: NaN, which fmin ignores).
 __global__ void step_coefficients_kernel(const double* __restrict__ partial, int nblocks, RunState* __restrict__ st,
-                                         CosmoScalars c, double G, double B, double* __restrict__ coef6)
+                                         CosmoScalars c, double G, double B, double* __restrict__ coef6,
+                                         unsigned long long* __restrict__ fused_bits, double dt_max)
 {
     if (threadIdx.x != 0) return;
-    double dt = partial[0];
-    for (int b = 1; b < nblocks; ++b) dt = fmin(dt, partial[b]);
+    double dt;
+    if (fused_bits != nullptr) {
+        dt = fmin(dt_max, __longlong_as_double((long long)*fused_bits));
+    } else {
+        dt = partial[0];
+        for (int b = 1; b < nblocks; ++b) dt = fmin(dt, partial[b]);
+    }
     const double a_n = st->a;
     const bool is_static = (c.H0 == 0.0);
     const double H_n = is_static ? 0.0 : hubble_dev(a_n, c);

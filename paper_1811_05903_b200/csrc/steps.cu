@@ -22,6 +22,10 @@ using namespace steps;
 namespace {
 
 std::atomic<long long> g_launches{0};
+// Eq. 12 fused into the last kernel of the force evaluation that steps_kdk_step_adaptive launches (Eq12Fuse, common.cuh):
+// set by that call around its forces_impl, read by the launchers of the final-writer kernels of FULL evaluations.
+thread_local Eq12Fuse t_fuse = {nullptr, nullptr, nullptr, 0.0, 0.0, 0.0, nullptr};
+const Eq12Fuse NO_FUSE = {nullptr, nullptr, nullptr, 0.0, 0.0, 0.0, nullptr};
 thread_local int g_last_cuda_error = 0;
 std::atomic<int> g_driver{0};   // 0 = default, 1 = simple v1 driver (cross-check)
 std::atomic<int> g_profile{0};  // 1 = bracket the force kernel with CUDA events on its stream
@@ -40,6 +44,20 @@ constexpr int SYM_MIN_BLOCKS_MIXED = 64;   // mixed: whole items only (its split
 std::atomic<long long> g_sym_panel_items{16384};
 std::atomic<int> g_sym_enabled{1};
 std::atomic<int> g_splitj{1};           // 0 = never use the split-j driver (testing)
+
+// What the fused Eq. 12 minimum of the last steps_kdk_step_adaptive call was computed from (see that function).
+struct FuseToken {
+    const void *pos, *acc, *soft, *state;
+    long long N;
+    double absG, B, eps;
+    long long launches;
+    bool operator==(const FuseToken& o) const
+    {
+        return pos == o.pos && acc == o.acc && soft == o.soft && state == o.state && N == o.N && absG == o.absG && B == o.B &&
+               eps == o.eps && launches == o.launches;
+    }
+};
+std::atomic<int> g_fuse_eq12{1};        // 0 = always the separate Eq. 12 pass (testing)
 
 struct Workspace {
     void* tiles = nullptr;          // max(sizeof(TileF32), sizeof(TileF64)) * ntiles (padded to whole blocks)
@@ -62,6 +80,8 @@ struct Workspace {
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;   // "profile" option: around the last force kernel(s)
     bool ev_valid = false;
     bool sym_split_ready = false, sym_split_ready_mixed = false;
+    FuseToken fuse_token{};
+    bool fuse_valid = false;
     // One scratch area per device: calls on different streams are serialised through this event (see claim_scratch).
     cudaEvent_t scratch_done = nullptr;
     cudaStream_t scratch_stream = nullptr;
@@ -264,7 +284,7 @@ int launch_forces_sym(const double* pos, const double* mass, const double* soft,
             k<<<Ps, SYM_MIXED_THREADS, sym_mixed_smem_bytes<SYM_MIXED_THREADS, SYM_MIXED_RI>(), st>>>(tiles, w.plan, k0, k1, rowrec, colrec, split);
         }
         forces_sym_reduce_kernel<<<(int)((N + 255) / 256), 256, 0, st>>>(w.plan, rowrec, colrec, k0, k1, N, hi, lo,
-                                                                          k1 == kmax ? 1 : 0, acc_out, split);
+                                                                          k1 == kmax ? 1 : 0, acc_out, split, t_fuse);
         g_launches += 2;
     }
     if (prof) { STEPS_CUDA(cudaEventRecord(w.ev1, st)); w.ev_valid = true; }
@@ -300,11 +320,12 @@ int launch_splitj(const double* pos, const double* soft, long long N, const type
         if (!w.ev0) { STEPS_CUDA(cudaEventCreate(&w.ev0)); STEPS_CUDA(cudaEventCreate(&w.ev1)); }
         STEPS_CUDA(cudaEventRecord(w.ev0, st));
     }
+    const Eq12Fuse fuse = (BOX == 0 && i_begin == 0 && i_end == N) ? t_fuse : NO_FUSE;
     kern<<<dim3((unsigned)groups, (unsigned)jsplit), CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, sub, i_begin, i_end, acc_out,
-                                                                                w.partials, 0, L, L > 0.0 ? 1.0 / L : 0.0);
+                                                                                w.partials, 0, L, L > 0.0 ? 1.0 / L : 0.0, fuse);
     g_launches++;
     if (jsplit > 1) {
-        forces_splitj_reduce<<<(unsigned)groups, SPLITJ_GROUP, 0, st>>>(w.partials, (int)jsplit, cnt, acc_out);
+        forces_splitj_reduce<<<(unsigned)groups, SPLITJ_GROUP, 0, st>>>(w.partials, (int)jsplit, cnt, acc_out, fuse);
         g_launches++;
     }
     if (prof) { STEPS_CUDA(cudaEventRecord(w.ev1, st)); w.ev_valid = true; }
@@ -356,7 +377,8 @@ int launch_forces(const double* pos, const double* mass, const double* soft, lon
         }
         kern<<<P, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, i_begin, i_end, nb, w.partials, 0, 0.0, 0.0, nullptr, block_stride);
         if (prof) { STEPS_CUDA(cudaEventRecord(w.ev1, st)); w.ev_valid = true; }
-        forces_reduce_kernel<Path::NOUT><<<(int)((cnt + 255) / 256), 256, 0, st>>>(w.partials, nt, nb, P, cnt, acc_out);
+        forces_reduce_kernel<Path::NOUT><<<(int)((cnt + 255) / 256), 256, 0, st>>>(
+            w.partials, nt, nb, P, cnt, acc_out, (block_stride == 1 && i_begin == 0 && i_end == N) ? t_fuse : NO_FUSE);
         g_launches += 2;
     }
     STEPS_CUDA(cudaGetLastError());
@@ -410,7 +432,7 @@ int launch_forces_periodic(const double* pos, const double* mass, const double* 
     if (rc != STEPS_OK) return rc;
     const int P = grid_cache;
     kern<<<P, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, 0, N, nb, w.partials, 0, L, 1.0 / L, nullptr, 1);
-    forces_reduce_kernel<Path::NOUT><<<(int)((N + 255) / 256), 256, 0, st>>>(w.partials, nt, nb, P, N, acc_out);
+    forces_reduce_kernel<Path::NOUT><<<(int)((N + 255) / 256), 256, 0, st>>>(w.partials, nt, nb, P, N, acc_out, NO_FUSE);
     g_launches += 2;
     STEPS_CUDA(cudaGetLastError());
     return release_scratch(w, st);
@@ -575,19 +597,42 @@ int steps_kdk_step_adaptive(double* pos, double* vel, double* acc, const double*
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     rc = claim_scratch(g_ws[dev], st);                      // released by the force evaluation at the end of this call
     if (rc != STEPS_OK) return rc;
-    double* partial = g_ws[dev].mom_partial;
+    Workspace& w = g_ws[dev];
+    double* partial = w.mom_partial;
     double* coef6 = partial + 2 * MOM_BLOCKS;
+    unsigned long long* fused_bits = reinterpret_cast<unsigned long long*>(partial + 2 * MOM_BLOCKS + 8);
     RunState* rs = reinterpret_cast<RunState*>(state5);
     const CosmoScalars cs{c->H0, c->Omega_m, c->Omega_r, c->Omega_L, c->Omega_k};
-    timestep_state_stage1<<<MOM_BLOCKS, 256, 0, st>>>(pos, acc, soft, N, rs, std::fabs(G), B, eps, dt_max, partial);
-    step_coefficients_kernel<<<1, 32, 0, st>>>(partial, MOM_BLOCKS, rs, cs, G, B, coef6);
+    // Eq. 12: the minimum over the particles was folded into `fused_bits` by the force evaluation of the PREVIOUS call of this
+    // function when that call was the last thing this library launched and it was for the same arrays and parameters (the
+    // candidates depend on pos, acc, soft, |G|, B, eps and on the run state's a); otherwise the O(N) pass forms it now.
+    const FuseToken now{pos, acc, soft, state5, N, std::fabs(G), B, eps, g_launches.load()};
+    const bool fused = w.fuse_valid && w.fuse_token == now;
+    if (!fused) {
+        timestep_state_stage1<<<MOM_BLOCKS, 256, 0, st>>>(pos, acc, soft, N, rs, std::fabs(G), B, eps, dt_max, partial);
+        g_launches++;
+    }
+    step_coefficients_kernel<<<1, 32, 0, st>>>(partial, MOM_BLOCKS, rs, cs, G, B, coef6, fused ? fused_bits : nullptr, dt_max);
     const long long M = 3 * N;
     long long blocks = (M + 255) / 256;
     if (blocks > 148 * 16) blocks = 148 * 16;
     kick_drift_dev_kernel<<<(int)blocks, 256, 0, st>>>(pos, vel, acc, M, coef6);
-    g_launches += 3;
+    g_launches += 2;
     STEPS_CUDA(cudaGetLastError());
-    return forces_impl(pos, mass, soft, N, 0, N, acc, mixed, stream);
+    w.fuse_valid = false;
+    if (g_fuse_eq12.load() != 0) {
+        STEPS_CUDA(cudaMemsetAsync(fused_bits, 0xff, sizeof(unsigned long long), st));      // any bit pattern >= +inf: no limit yet
+        t_fuse = Eq12Fuse{pos, soft, state5, std::fabs(G), B, eps, fused_bits};
+    }
+    rc = forces_impl(pos, mass, soft, N, 0, N, acc, mixed, stream);
+    const bool was_on = t_fuse.out_bits != nullptr;
+    t_fuse = NO_FUSE;
+    if (rc != STEPS_OK) return rc;
+    if (was_on) {
+        w.fuse_token = FuseToken{pos, acc, soft, state5, N, std::fabs(G), B, eps, g_launches.load()};
+        w.fuse_valid = true;
+    }
+    return STEPS_OK;
 }
 
 int steps_kick_close_adaptive(double* pos, double* vel, const double* acc, long long N, double* state5, double B,
@@ -837,6 +882,7 @@ int steps_set_option(const char* key, long long value)
     if (std::strcmp(key, "profile") == 0) { g_profile = (int)value; return STEPS_OK; }
     if (std::strcmp(key, "sym") == 0) { g_sym_enabled = (int)value; return STEPS_OK; }
     if (std::strcmp(key, "splitj") == 0) { g_splitj = (int)value; return STEPS_OK; }
+    if (std::strcmp(key, "fuse_eq12") == 0) { g_fuse_eq12 = (int)value; return STEPS_OK; }
     if (std::strcmp(key, "sym_panel_items") == 0) {
         if (value < 1) return STEPS_EINVAL;
         g_sym_panel_items = value;

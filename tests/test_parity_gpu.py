@@ -717,6 +717,40 @@ def test_device_resident_steps_replay_from_a_cuda_graph(S, oracle, n, mixed):
     assert torch.equal(pos_g, pos_e) and torch.equal(vel_g, vel_e) and torch.equal(acc_g, acc_e)
 
 
+@pytest.mark.gpu
+@pytest.mark.parametrize("n", [4096, 20000, 40000, 140000])
+def test_fused_timestep_minimum_equals_the_separate_pass(S, oracle, n):
+    """Eq. 12's minimum fused into the force evaluation's last kernel (split-j epilogue at 4,096, ring reduce at 20,000,
+    pair-symmetric panel reduce at 40,000 / 140,000) against the separate O(N) pass: twelve adaptive steps, bit-identical
+    state either way; and the shortcut is dropped when another library call comes between two steps."""
+    import torch
+    ps = _config4(oracle, n)
+    B, G, eps, dt_max, a0 = 1.0 / ps.r_cut ** 3, 1.0, 0.025, 0.5, 1 / 51
+    c = S.Cosmology(**LCDM)
+    dm, dh = dev(ps.mass), dev(ps.soft)
+    out = torch.empty(4, dtype=torch.float64, device="cuda")
+    runs = {}
+    for fuse in (1, 0):
+        S.steps_set_option("fuse_eq12", fuse)
+        try:
+            dpos, dvel = dev(ps.pos), dev(ps.vel)
+            dacc = torch.empty_like(dpos)
+            S.steps_forces(dpos, dm, dh, dacc)
+            st = torch.tensor([a0, 0.0, 1.0, 0.0, 0.0], dtype=torch.float64, device="cuda")
+            l0 = S.steps_kernel_launch_count()
+            for k in range(12):
+                S.steps_kdk_step_adaptive(dpos, dvel, dacc, dm, dh, st, c, G, B, eps, dt_max)
+                if k == 5:
+                    S.steps_momentum(dvel, dm, out)          # a foreign call: the next step must not use the shortcut
+            torch.cuda.synchronize()
+            runs[fuse] = (dpos.clone(), dvel.clone(), dacc.clone(), st.clone(), S.steps_kernel_launch_count() - l0)
+        finally:
+            S.steps_set_option("fuse_eq12", 1)
+    for a, b in zip(runs[1][:4], runs[0][:4]):
+        assert torch.equal(a, b)
+    assert runs[0][4] - runs[1][4] == 10                     # 12 steps: the first and the one after the foreign call keep the pass
+
+
 # ---- Eq. 5 (L65-70) with the cut |x - nL| < 2.6 L: periodic image sum (fp64) ------------------------------------------
 @pytest.mark.gpu
 @pytest.mark.parametrize("n", [2, 27, 300, 1500])
