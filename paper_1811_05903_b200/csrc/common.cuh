@@ -107,50 +107,66 @@ __device__ __forceinline__ bool tile_is_far(float rminI, float rmaxI, float hmax
     return gap > need;
 }
 
-// ---- periodic boxes (Eq. 5, leading image): one image shift per (i-group, j-tile) pair -----------------
-// With cell-ordered input (each tile a compact cell) the separations x_j - x_i of a tile pair span, per component, an
-// interval [dmin, dmax] much shorter than L.  With n = floor(dmin / L) every d' = d - n L lies in [lo, hi], lo in [0, L):
-//   hi <= L/2           all pairs take image n          (shift n L, no per-pair wrap)
-//   lo >= L/2           all pairs take image n + 1      (shift (n + 1) L, no per-pair wrap; needs hi <= 3L/2)
-//   otherwise           the interval straddles L/2: shift n L and, per pair, d' -= L where d' > L/2 (needs hi < 3L/2)
-// gmin = the smallest |leading-image separation| any pair of the two boxes can have in this component.
-// kind: 0 = no common shift possible (boxes too wide: unsorted input) or a softened pair is possible -> general body;
-//       1 = far, uniform shift;  2 = far, per-pair conditional subtraction.
+// ---- periodic boxes (Eq. 5, leading image): one image decision per (i-group, j-unit) pair ---------------
+// With cell-ordered input the separations d = x_j - x_i of a (group, unit) pair span, per component, an interval
+// [dmin, dmax] shorter than L (from the two bounding boxes).  With k = the leading-image index of dmin, i.e.
+// dmin in [(k - 1/2) L, (k + 1/2) L), and top = (k + 1/2) L:
+//   dmax < top    every pair takes image k:  d' = d - k L                                   (uniform shift k L)
+//   otherwise     the interval holds the half-box point `top` (and, being shorter than L, no other): with e = d - top,
+//                 |e| <= L, the leading image is  d' = e - copysign(L/2, e)  (image k below the point, k + 1 above it) --
+//                 a FOLD: one addition and one bit operation per pair and component, no rounding to the lattice, no compare.
+// The shift (k L or top) goes onto the i-particles once per (group, unit) pair (x_i' = x_i + s), so the pair arithmetic
+// is the open-boundary far body plus the fold of the components in `mask`.
+// gmin = the smallest |d'| any pair of the two boxes can have in this component; the pair is FAR when no separation
+// can be below the largest pair softening.
+// kind: 0 = a softened pair is possible, or a box pair spans a whole period (unsorted input) -> general wrapped body;
+//       1 = far: shift s, fold the components in mask.
 struct BoxShift {
-    int kind;
+    int kind, mask;
     double s[3];
 };
-__device__ __forceinline__ BoxShift box_shift(const float (&loI)[3], const float (&hiI)[3], float hmaxI, const TileMeta& J, float L)
+__device__ __forceinline__ BoxShift box_shift(const float (&loI)[3], const float (&hiI)[3], float hmaxI, const float (&loJ)[3],
+                                              const float (&hiJ)[3], float hmaxJ, double L, double invL)
 {
     BoxShift d;
-    d.kind = 1;
-    float g2 = 0.0f;
-    const float half = 0.5f * L, eps = 1.0e-5f * L;
+    d.kind = 1; d.mask = 0;
+    double g2 = 0.0;
+    const double eps = 1.0e-5 * L;                               // outward: fp32 rounding of the bounds and of the mixed path's coordinates
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        const float dmin = (J.lo[c] - hiI[c]) - eps, dmax = (J.hi[c] - loI[c]) + eps;   // outward (fp32 rounding of the bounds)
-        const float n = floorf(dmin / L);
-        const float lo = dmin - n * L, hi = dmax - n * L;
-        float gmin;
-        if (!(dmax - dmin < 0.45f * L)) { d.kind = 0; d.s[c] = 0.0; continue; }       // also catches NaN / inf bounds
-        if (hi <= half - eps) { d.s[c] = (double)n * (double)L; gmin = lo; }
-        else if (lo >= half + eps) { d.s[c] = ((double)n + 1.0) * (double)L; gmin = fmaxf(L - hi, 0.0f); }
-        else { d.s[c] = (double)n * (double)L; gmin = fmaxf(fminf(lo, L - hi), 0.0f); if (d.kind == 1) d.kind = 2; }
-        g2 = fmaf(gmin, gmin, g2);
+        const double dmin = ((double)loJ[c] - (double)hiI[c]) - eps, dmax = ((double)hiJ[c] - (double)loI[c]) + eps;
+        if (!(dmax - dmin < 0.999 * L) || !(dmax >= dmin)) { d.kind = 0; d.s[c] = 0.0; continue; }   // also NaN / inf / empty boxes
+        const double k = floor(fma(dmin, invL, 0.5));
+        const double top = (k + 0.5) * L;
+        double gmin;
+        if (dmax < top) {
+            d.s[c] = k * L;
+            const double lo = dmin - d.s[c], hi = dmax - d.s[c];
+            gmin = lo > 0.0 ? lo : (hi < 0.0 ? -hi : 0.0);
+        } else {
+            d.s[c] = top; d.mask |= 1 << c;
+            gmin = fmax(0.0, 0.5 * L - fmax(top - dmin, dmax - top));
+        }
+        g2 = fma(gmin, gmin, g2);
     }
     if (d.kind != 0) {
-        const float need = (hmaxI + J.hmax) * 1.0001f + 1.0e-5f * L;
+        const double need = ((double)hmaxI + (double)hmaxJ) * 1.0001 + eps;
         if (!(g2 > need * need)) d.kind = 0;
     }
     return d;
 }
-
-// d -= period where d > half, both as bit patterns (valid for half > 0; d <= 0 never subtracts): one 64-bit integer compare
-// on the ALU pipe and ONE predicated DADD, instead of the compare + add + two selects the compiler makes of the C form.
-__device__ __forceinline__ void sub_if_above(double& d, long long half_bits, double neg_period)
+__device__ __forceinline__ BoxShift box_shift(const float (&loI)[3], const float (&hiI)[3], float hmaxI, const TileMeta& J, double L,
+                                              double invL)
 {
-    asm("{\n.reg .pred p;\nsetp.gt.s64 p, %1, %2;\n@p add.f64 %0, %0, %3;\n}"
-        : "+d"(d) : "l"(__double_as_longlong(d)), "l"(half_bits), "d"(neg_period));
+    return box_shift(loI, hiI, hmaxI, J.lo, J.hi, J.hmax, L, invL);
+}
+
+// The fold of one separation component: e - copysign(h, e) as (|e| - h) with the sign of e (h = half the period, in the
+// units of e).  One DADD (|e| is an operand modifier) and one LOP3 on the high word.
+__device__ __forceinline__ double fold_f64(double e, double h)
+{
+    const double u = fabs(e) - h;
+    return __hiloint2double(__double2hiint(u) ^ (__double2hiint(e) & 0x80000000), __double2loint(u));
 }
 
 // ---- Eq. 12 fused into the force evaluation's last kernel ------------------------------------------

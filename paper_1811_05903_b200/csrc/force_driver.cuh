@@ -109,6 +109,48 @@ __device__ __forceinline__ void init_far_sums(typename Path::FarSums& F, double*
     else Path::far_zero(F);
 }
 
+// Periodic far body of a (group, tile) pair; Q = the group with the pair's image shift on it, the fold mask picks the body.
+template <typename Path>
+__device__ __forceinline__ void far_fold_dispatch(const typename Path::Tile& T, const typename Path::IState& Q, typename Path::FarSums& F,
+                                                  int zero, int mask, double halfL, int j0, int j1)
+{
+    switch (mask) {
+        case 0: Path::template far_fold<0>(T, Q, F, zero, halfL, j0, j1); break;
+        case 1: Path::template far_fold<1>(T, Q, F, zero, halfL, j0, j1); break;
+        case 2: Path::template far_fold<2>(T, Q, F, zero, halfL, j0, j1); break;
+        case 3: Path::template far_fold<3>(T, Q, F, zero, halfL, j0, j1); break;
+        case 4: Path::template far_fold<4>(T, Q, F, zero, halfL, j0, j1); break;
+        case 5: Path::template far_fold<5>(T, Q, F, zero, halfL, j0, j1); break;
+        case 6: Path::template far_fold<6>(T, Q, F, zero, halfL, j0, j1); break;
+        default: Path::template far_fold<7>(T, Q, F, zero, halfL, j0, j1); break;
+    }
+}
+
+// The decision of box_shift packed into one word (forces_boxring_kernel keeps one per tile in shared memory):
+// bits 0-2 fold mask, bit 3 general body, bits 8-15 / 16-23 / 24-31 the shifts in units of L/2 (signed bytes).
+constexpr uint32_t BOXCODE_GENERAL = 8u;
+__device__ __forceinline__ uint32_t boxcode_pack(const BoxShift& bs, double invL)
+{
+    if (bs.kind == 0) return BOXCODE_GENERAL;
+    uint32_t code = (uint32_t)bs.mask;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const double k2 = rint(2.0 * bs.s[c] * invL);           // an integer by construction (k L or (k + 1/2) L)
+        if (!(fabs(k2) <= 127.0)) return BOXCODE_GENERAL;       // particles many periods apart: the general body wraps them
+        code |= ((uint32_t)(int)k2 & 0xffu) << (8 + 8 * c);
+    }
+    return code;
+}
+__device__ __forceinline__ BoxShift boxcode_unpack(uint32_t code, double L)
+{
+    BoxShift bs;
+    bs.kind = (code & BOXCODE_GENERAL) ? 0 : 1;
+    bs.mask = (int)(code & 7u);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) bs.s[c] = (double)(int)(signed char)((code >> (8 + 8 * c)) & 0xffu) * (0.5 * L);   // exact: see box_shift
+    return bs;
+}
+
 __host__ __device__ constexpr int stage_stride(int tile_bytes) { return (tile_bytes + 127) / 128 * 128; }
 
 template <typename Path, int STAGES>
@@ -144,11 +186,11 @@ __device__ __forceinline__ int band_row_of(const long long* __restrict__ cum, in
 
 // ---- persistent stream-K driver ------------------------------------------------------------------
 // partials: [nb + gridDim.x slots][Path::NOUT][IB] doubles; CTA p's record for i-block b is slot b + p.
-// BOX != 0 (periodic boundaries, Eq. 5): every tile goes through the near body with
-// leading-image separations (BOX = 1, quasi-periodic) or the image sum (BOX = 2) in a cubic box of side box_L -- the radial far/near classification of the compactified
-// sets does not apply in a periodic box.
+// BOX = 2 (periodic boundaries, Eq. 5): every tile goes through the image sum in a cubic
+// box of side box_L -- the radial far/near classification of the compactified sets does not apply in a periodic box.
+// (The leading-image box, BOX = 1, has its own driver: forces_boxring_kernel below.)
 // BAND (open boundary only): the iteration space is the band of `plan` instead of all nb x nt (i-block, tile) pairs.
-template <typename Path, int STAGES, int BOX = 0, bool BAND = false>   // BOX: 0 open boundary, 1 nearest image, 2 image sum with the 2.6 L cut
+template <typename Path, int STAGES, int BOX = 0, bool BAND = false>   // BOX: 0 open boundary, 2 image sum with the 2.6 L cut
 __global__ void __launch_bounds__(CTA_THREADS, 1)
 forces_persistent_kernel(const double* __restrict__ pos, const double* __restrict__ soft, long long N,
                          const typename Path::Tile* __restrict__ tiles, int nt, long long i_begin, long long i_end,
@@ -158,6 +200,7 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
     // block_stride > 1 (multi-GPU dealing, steps_forces_blocks): local i-block b is the global block
     // i_begin / IB + b * block_stride; i_end is then N.
     static_assert(!BAND || BOX == 0, "the band split applies to the open boundary only");
+    static_assert(BOX != 1, "the leading-image box runs on forces_boxring_kernel");
     using Tile = typename Path::Tile;
     constexpr int STRIDE = stage_stride((int)sizeof(Tile));
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -222,8 +265,6 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
         float rlo, rhi, hh;
         const long long i0 = i_begin + (long long)b * block_stride * IB + warp * WARP_I + lane;
         load_i_block<Path>(S, pos, soft, N, i0, i_end, rlo, rhi, hh);
-        float blo[3], bhi[3];                                  // bounding box of the warp's i-particles (periodic boxes)
-        if constexpr (BOX == 1) warp_box<Path>(S, blo, bhi);
 #pragma unroll
         for (int q = 0; q < Path::NOUT * R_I; ++q) acc[q * CTA_THREADS] = 0.0;
 
@@ -235,18 +276,7 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
             const int s = it % STAGES;
             mbar_wait(&full_bar[s], (it / STAGES) & 1);
             const Tile& T = *reinterpret_cast<const Tile*>(smem_raw + s * STRIDE);
-            if constexpr (BOX == 1) {
-                // cell-ordered input: most tile pairs share one image shift and cannot be softened (box_shift in common.cuh)
-                const BoxShift bs = box_shift(blo, bhi, hh, T.meta, (float)box_L);
-                if (bs.kind == 0) {
-                    if (pending) { Path::far_flush(F, acc); pending = 0; }
-                    Path::template near_box<true>(T, S, acc, box_L, box_invL);
-                } else {
-                    if (bs.kind == 1) Path::template far_box<false>(T, S, F, zero, bs, box_L);
-                    else Path::template far_box<true>(T, S, F, zero, bs, box_L);
-                    if (++pending >= Path::FAR_TILES_PER_FLUSH) { Path::far_flush(F, acc); pending = 0; }
-                }
-            } else if constexpr (BOX == 2) {
+            if constexpr (BOX == 2) {
                 Path::near_images(T, S, acc, box_L, box_invL, img_tab);
             } else {
             // the decision is warp-uniform by construction (warp-reduced bounds); the vote tells the compiler so
@@ -373,8 +403,7 @@ forces_splitj_kernel(const double* __restrict__ pos, const double* __restrict__ 
     float rlo, rhi, hh;
     const long long i0 = i_begin + (long long)blockIdx.x * SPLITJ_GROUP + lane;      // the same particles in every warp
     load_i_block<Path>(S, pos, soft, N, i0, i_end, rlo, rhi, hh);
-    float blo[3], bhi[3];
-    if constexpr (BOX == 1) warp_box<Path>(S, blo, bhi);
+    static_assert(BOX == 0, "periodic boxes run on forces_boxring_kernel / the persistent driver");
 #pragma unroll
     for (int q = 0; q < Path::NOUT * R_I; ++q) acc[q * CTA_THREADS] = 0.0;
 
@@ -388,17 +417,7 @@ forces_splitj_kernel(const double* __restrict__ pos, const double* __restrict__ 
         const typename Path::Tile& T = tiles[u / per_tile];
         const int j0 = (int)(u % per_tile) * sub, j1 = j0 + sub;
         const TileMeta meta = T.meta;
-        if constexpr (BOX == 1) {
-            const BoxShift bs = box_shift(blo, bhi, hh, meta, (float)box_L);
-            if (bs.kind == 0) {
-                if (pending) { Path::far_flush(F, acc); pending = 0; }
-                Path::template near_box<true>(T, S, acc, box_L, box_invL, j0, j1);
-            } else {
-                if (bs.kind == 1) Path::template far_box<false>(T, S, F, zero, bs, box_L, j0, j1);
-                else Path::template far_box<true>(T, S, F, zero, bs, box_L, j0, j1);
-                if (++pending >= Path::FAR_TILES_PER_FLUSH) { Path::far_flush(F, acc); pending = 0; }
-            }
-        } else {
+        {
             if (__all_sync(0xffffffffu, tile_is_far(rlo, rhi, hh, meta))) {
                 Path::far(T, S, F, zero, j0, j1);
                 if (++pending >= Path::FAR_TILES_PER_FLUSH) { Path::far_flush(F, acc); pending = 0; }
@@ -476,6 +495,170 @@ __global__ void __launch_bounds__(128) forces_splitj_reduce(const double* __rest
     }
     }
     if (fuse.out_bits) eq12_fold(fuse, dt);
+}
+
+// ---- group-ring driver: the leading-image periodic box (Eq. 5) -----------------------
+// One i-GROUP of 128 particles (4 per lane) per CTA column, held by ALL 16 warps of the CTA.  The warps form BOXRING_G
+// sub-rings of 4 warps; each sub-ring streams every fourth tile of the range through its own bulk-copy ring (its first
+// lane is the producer) and each of its warps takes a quarter (64 sources) of every tile.
+// Why this shape: in a periodic box the image decision (box_shift: far or possibly softened, the shift, which components
+// fold) is per (group, tile) pair and its cost differs by up to 2x.  Warps that hold DIFFERENT groups and share a tile
+// ring wait for the slowest decision at every tile; warps that hold the SAME group all run the same body on a tile, so a
+// ring stays in step and every load is a shared-memory broadcast.  The decisions -- one word per tile -- are computed by
+// the whole CTA ahead of the rings, DEC_CHUNK tiles at a time, so they cost nothing in the loop, and the producers know
+// them: only the FAR part of a tile record (the scaled sources, 8 KiB fp64 / 4 KiB fp32) is copied, and only for tiles
+// that take the far body; the rare tile that may hold a softened pair is read by the general wrapped body straight from
+// global memory.
+// The 16 partial accelerations meet in shared memory and are added in fixed warp order (TwoSum), as in the split-j
+// driver; gridDim.y > 1 splits the tile range over CTAs (records summed by forces_splitj_reduce).
+constexpr int BOXRING_G = 4;                               // sub-rings per CTA
+constexpr int BOXRING_STAGES = 3;                          // stages per sub-ring
+constexpr int DEC_CHUNK = 512;                             // decisions per sub-ring kept in shared memory at a time
+template <typename Path>
+__host__ __device__ constexpr int far_part_bytes()         // the scaled sources lead the tile record (common.cuh)
+{
+    return Path::NOUT == 6 ? TJ * (int)sizeof(FarSrcF64) : 4 * TJ * (int)sizeof(float);
+}
+template <typename Path>
+constexpr int boxring_smem_bytes()
+{
+    return BOXRING_G * BOXRING_STAGES * far_part_bytes<Path>() + Path::NOUT * R_I * CTA_THREADS * (int)sizeof(double) +
+           BOXRING_G * DEC_CHUNK * (int)sizeof(uint32_t);
+}
+
+template <typename Path>
+__global__ void __launch_bounds__(CTA_THREADS, 1)
+forces_boxring_kernel(const double* __restrict__ pos, const double* __restrict__ soft, long long N,
+                      const typename Path::Tile* __restrict__ tiles, int nt, double* __restrict__ acc_out,
+                      double* __restrict__ partials, int zero, double box_L, double box_invL)
+{
+    using Tile = typename Path::Tile;
+    using IState = typename Path::IState;
+    using Elem = decltype(IState::x[0] + 0);               // double or float
+    constexpr int G = BOXRING_G, STAGES = BOXRING_STAGES, FAR_BYTES = far_part_bytes<Path>();
+    constexpr int WARPS = CTA_THREADS / 32, WG = WARPS / G, PER_WARP = TJ / WG;   // 4 warps per sub-ring, 64 sources per warp and tile
+    static_assert(WARPS % G == 0 && TJ % WG == 0 && PER_WARP % 4 == 0, "every warp takes whole float4 groups of each tile");
+    static_assert(FAR_BYTES % 128 == 0, "stage alignment");
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ uint64_t full_bar[G][STAGES], empty_bar[G][STAGES];
+    __shared__ Elem gs[4 * R_I][32];                        // the group's particles (x, y, z, h), unshifted: read back when a
+                                                            // tile needs another image shift or the general body
+    double* acc_all = reinterpret_cast<double*>(smem_raw + G * STAGES * FAR_BYTES);   // [NOUT * R_I][CTA_THREADS]
+    double* acc = acc_all + threadIdx.x;
+    uint32_t* codes_all = reinterpret_cast<uint32_t*>(acc_all + Path::NOUT * R_I * CTA_THREADS);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int g = warp / WG, wg = warp % WG;                 // sub-ring, warp within it
+    unsigned char* ring = smem_raw + g * STAGES * FAR_BYTES;
+    const uint32_t* codes = codes_all + g * DEC_CHUNK;
+    const bool producer = wg == 0 && lane == 0;
+
+    float blo[3], bhi[3], hh;
+    {
+        IState S;
+        float rlo, rhi;
+        const long long i0 = (long long)blockIdx.x * SPLITJ_GROUP + lane;     // the same particles in every warp
+        load_i_block<Path>(S, pos, soft, N, i0, N, rlo, rhi, hh);
+        warp_box<Path>(S, blo, bhi);
+        if (warp == 0) {
+#pragma unroll
+            for (int k = 0; k < R_I; ++k) { gs[k][lane] = S.x[k]; gs[R_I + k][lane] = S.y[k]; gs[2 * R_I + k][lane] = S.z[k]; gs[3 * R_I + k][lane] = S.h[k]; }
+        }
+    }
+    auto group_state = [&]() {
+        IState S;
+#pragma unroll
+        for (int k = 0; k < R_I; ++k) { S.x[k] = gs[k][lane]; S.y[k] = gs[R_I + k][lane]; S.z[k] = gs[2 * R_I + k][lane]; S.h[k] = gs[3 * R_I + k][lane]; }
+        return S;
+    };
+#pragma unroll
+    for (int q = 0; q < Path::NOUT * R_I; ++q) acc[q * CTA_THREADS] = 0.0;
+
+    // tile range of this CTA; sub-ring g takes the tiles t0 + g, t0 + g + G, ... (interleaved: every sub-ring meets the same
+    // mix of decisions, so the four finish together)
+    const int t0 = (int)((long long)blockIdx.y * nt / gridDim.y), t1 = (int)(((long long)blockIdx.y + 1) * nt / gridDim.y);
+    const int mine = (t1 - t0 - g + G - 1) / G;              // tiles of this sub-ring
+    const int chunks = ((t1 - t0 + G - 1) / G + DEC_CHUNK - 1) / DEC_CHUNK;   // the same for every sub-ring (CTA-wide barriers)
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int r = 0; r < G; ++r)
+#pragma unroll
+            for (int s = 0; s < STAGES; ++s) { mbar_init(&full_bar[r][s], 1); mbar_init(&empty_bar[r][s], WG); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+
+    typename Path::FarSums F;
+    init_far_sums<Path>(F, acc);
+    Path::far_zero(F);
+    IState Q;                                               // the group with the current image shift on it
+    uint32_t q_key = 0xffffffffu;                           // the shift bytes Q was built for (none yet)
+    int pending = 0;                                        // sources summed in F since its last flush
+    int produced = 0, consumed = 0;                         // far tiles of this sub-ring so far
+    const int j0 = wg * PER_WARP, j1 = j0 + PER_WARP;
+    for (int ch = 0; ch < chunks; ++ch) {
+        const int k0 = ch * DEC_CHUNK, cnt = max(0, min(DEC_CHUNK, mine - k0));   // this sub-ring's tiles k0 .. k0 + cnt of its list
+        __syncthreads();                                    // the previous chunk's decisions are no longer read (and: gs, barrier init)
+        for (int q = threadIdx.x; q < G * DEC_CHUNK; q += CTA_THREADS) {       // all threads compute the decisions of all sub-rings
+            const int r = q / DEC_CHUNK, tile = t0 + r + G * (k0 + q % DEC_CHUNK);
+            if (tile < t1) codes_all[q] = boxcode_pack(box_shift(blo, bhi, hh, tiles[tile].meta, box_L, box_invL), box_invL);
+        }
+        __syncthreads();
+        int pq = 0;                                         // producer cursor within the chunk
+        auto produce_next = [&]() {                         // the next far tile of the chunk, if any
+            while (pq < cnt && (codes[pq] & BOXCODE_GENERAL)) ++pq;
+            if (pq >= cnt) return;
+            const int s = produced % STAGES;
+            if (produced >= STAGES) mbar_wait(&empty_bar[g][s], ((produced / STAGES) - 1) & 1);
+            mbar_expect_tx(&full_bar[g][s], (uint32_t)FAR_BYTES);
+            bulk_load(ring + s * FAR_BYTES, tiles + (t0 + g + G * (k0 + pq)), (uint32_t)FAR_BYTES, &full_bar[g][s]);
+            ++produced; ++pq;
+        };
+        if (producer)
+            for (int k = 0; k < STAGES - 1; ++k) produce_next();
+        for (int q = 0; q < cnt; ++q) {
+            const uint32_t code = codes[q];
+            if (code & BOXCODE_GENERAL) {
+                if (pending) { Path::fold_flush(F, acc); pending = 0; }
+                Path::template near_box<true>(tiles[t0 + g + G * (k0 + q)], group_state(), acc, box_L, box_invL, j0, j1);
+                continue;
+            }
+            if (producer) produce_next();
+            const int s = consumed % STAGES;
+            mbar_wait(&full_bar[g][s], (consumed / STAGES) & 1);
+            const Tile& T = *reinterpret_cast<const Tile*>(ring + s * FAR_BYTES);    // only its far part is there
+            if ((code >> 8) != q_key) {
+                q_key = code >> 8;
+                Q = Path::shifted(group_state(), boxcode_unpack(code, box_L).s);
+            }
+            far_fold_dispatch<Path>(T, Q, F, zero, (int)(code & 7u), 0.5 * box_L, j0, j1);
+            pending += PER_WARP;
+            if (pending >= Path::FAR_SOURCES_PER_FLUSH) { Path::fold_flush(F, acc); pending = 0; }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty_bar[g][s]);
+            ++consumed;
+        }
+    }
+    if (pending) Path::fold_flush(F, acc);
+    __syncthreads();
+
+    // fixed-order sum over the 16 warps: thread (c, k, l) owns component c of particle l + 32 k of the group
+    if (threadIdx.x < 3 * SPLITJ_GROUP) {
+        const int c = threadIdx.x / SPLITJ_GROUP, r = threadIdx.x % SPLITJ_GROUP, k = r / 32, l = r % 32;
+        double hi = 0.0, lo = 0.0;
+        for (int w = 0; w < WARPS; ++w) {
+            const double v = acc_all[(c * R_I + k) * CTA_THREADS + w * 32 + l];
+            const double s = hi + v, bb = s - hi;
+            lo += (hi - (s - bb)) + (v - bb);                              // TwoSum
+            hi = s;
+            if (Path::NOUT == 6) lo += acc_all[((3 + c) * R_I + k) * CTA_THREADS + w * 32 + l];
+        }
+        const long long i = (long long)blockIdx.x * SPLITJ_GROUP + l + 32 * k;
+        if (gridDim.y == 1) {
+            if (i < N) acc_out[(long long)c * N + i] = hi + lo;
+        } else {
+            double* rec = partials + (((long long)blockIdx.x * gridDim.y + blockIdx.y) * 6) * SPLITJ_GROUP;
+            rec[c * SPLITJ_GROUP + r] = hi; rec[(3 + c) * SPLITJ_GROUP + r] = lo;
+        }
+    }
 }
 
 // ---- simple driver (cross-check) -----------------------------------------------------------------

@@ -139,6 +139,7 @@ struct Fp64Path {
         double ax[R_I], ay[R_I], az[R_I];
     };
     static constexpr int FAR_TILES_PER_FLUSH = STEPS_FP64_FAR_TILES_PER_FLUSH;
+    static constexpr int FAR_SOURCES_PER_FLUSH = FAR_TILES_PER_FLUSH * TJ;      // the same, for drivers that sum parts of tiles
     static __device__ __forceinline__ void far_zero(FarSums& F)
     {
 #pragma unroll
@@ -150,6 +151,8 @@ struct Fp64Path {
         for (int k = 0; k < R_I; ++k) { flush(acc, 0, k, F.ax[k]); flush(acc, 1, k, F.ay[k]); flush(acc, 2, k, F.az[k]); }
         far_zero(F);
     }
+
+    static __device__ __forceinline__ void fold_flush(FarSums& F, double* acc) { far_flush(F, acc); }   // far_fold() sums into F like far()
 
     // [j0, j1): the sources of the tile to sum (the whole tile in the ring driver; a part of it in the split-j driver).
     static __device__ __forceinline__ void far(const Tile& T, const IState& S, FarSums& F, int zero, int j0 = 0, int j1 = TJ)
@@ -191,24 +194,30 @@ struct Fp64Path {
         }
     }
 
-    // Far body in a periodic box (Eq. 5, leading image) for a tile pair with a common image shift (box_shift in common.cuh):
-    // the shift goes onto the source, X' = X_j - c_j s (3 DFMA per source, shared by the 4 particles), then the body of far().
-    // WRAP: the pair's boxes straddle half the box in some component: d' -= L where d' > L/2, in scaled units
-    // (c_j L, c_j L/2 per source), the test as an integer compare of the bit patterns (ALU pipe; d' <= 0 never subtracts).
-    template <bool WRAP>
-    static __device__ __forceinline__ void far_box(const Tile& T, const IState& S, FarSums& F, int zero, const BoxShift& bs, double L,
-                                                   int j0 = 0, int j1 = TJ)
+    // Far body in a periodic box (Eq. 5, leading image) for a (group, unit) pair that cannot be softened (box_shift in
+    // common.cuh).  The image shift is already on the i-particles (`shifted`), so the pair arithmetic is the body of far()
+    // plus, for the components in MASK -- those whose separations straddle half the box -- the fold d' = e - copysign(L/2, e)
+    // in scaled units (h = c_j L/2, one DMUL per source): 14 + popcount(MASK) FP64-pipe instructions per interaction.
+    static __device__ __forceinline__ IState shifted(const IState& S, const double (&s)[3])
+    {
+        IState Q;
+#pragma unroll
+        for (int k = 0; k < R_I; ++k) { Q.x[k] = S.x[k] + s[0]; Q.y[k] = S.y[k] + s[1]; Q.z[k] = S.z[k] + s[2]; Q.h[k] = S.h[k]; }
+        return Q;
+    }
+    template <int MASK>
+    static __device__ __forceinline__ void far_fold(const Tile& T, const IState& S, FarSums& F, int zero, double halfL,
+                                                    int j0 = 0, int j1 = TJ)
     {
         constexpr double A = 1.4;
         constexpr double C0 = 1.0 / STEPS_FP64_FOLD - (1.0 - A) * (1.0 - A);
         double (&ax)[R_I] = F.ax, (&ay)[R_I] = F.ay, (&az)[R_I] = F.az;
-        const double sx = bs.s[0], sy = bs.s[1], sz = bs.s[2];
 #pragma unroll 1
         for (int j = j0; j < j1; ++j) {
             const double2 XY = *reinterpret_cast<const double2*>(&T.far[j].X);
             const double2 ZC = *reinterpret_cast<const double2*>(&T.far[j].Z);
-            const double C = ZC.y;
-            const double X = fma(-sx, C, XY.x), Y = fma(-sy, C, XY.y), Z = fma(-sz, C, ZC.x);
+            const double X = XY.x, Y = XY.y, Z = ZC.x, C = ZC.y;
+            const double hc = C * halfL;
             double dX[R_I], dY[R_I], dZ[R_I], r2[R_I], y0[R_I], y2[R_I], w[R_I];
             STEPS_STAGE_FENCE(zero, 0);
 #pragma unroll
@@ -217,13 +226,17 @@ struct Fp64Path {
             for (int k = 0; k < R_I; ++k) dY[k] = fma(-S.y[k], C, Y);
 #pragma unroll
             for (int k = 0; k < R_I; ++k) dZ[k] = fma(-S.z[k], C, Z);
-            if (WRAP) {
-                const double ncL = -C * L;
-                const long long hb = __double_as_longlong(-0.5 * ncL);
+            if (MASK & 1) {
 #pragma unroll
-                for (int k = 0; k < R_I; ++k) {
-                    sub_if_above(dX[k], hb, ncL); sub_if_above(dY[k], hb, ncL); sub_if_above(dZ[k], hb, ncL);
-                }
+                for (int k = 0; k < R_I; ++k) dX[k] = fold_f64(dX[k], hc);
+            }
+            if (MASK & 2) {
+#pragma unroll
+                for (int k = 0; k < R_I; ++k) dY[k] = fold_f64(dY[k], hc);
+            }
+            if (MASK & 4) {
+#pragma unroll
+                for (int k = 0; k < R_I; ++k) dZ[k] = fold_f64(dZ[k], hc);
             }
             STEPS_STAGE_FENCE(zero, 1);
 #pragma unroll

@@ -74,12 +74,31 @@ struct MixedPath {
     // 2 words/clk/lane), see DESIGN.md "what limits the mixed far body".
     // The mixed path flushes its fp32 partial sums inside far() at every tile (<= 128 terms per packed half), so it
     // carries nothing across tiles: FarSums only holds the accumulator pointer.
+    // far_fold() (periodic boxes, where a warp sums only a sixteenth of a tile per call) keeps packed fp32 sums in
+    // ax/ay/az across calls; its driver flushes them every FAR_SOURCES_PER_FLUSH sources (<= 128 terms per packed half).
     struct FarSums {
         double* acc;
+        u64 ax[R_I / 2], ay[R_I / 2], az[R_I / 2];
     };
     static constexpr int FAR_TILES_PER_FLUSH = 1 << 30;
-    static __device__ __forceinline__ void far_zero(FarSums&) {}
-    static __device__ __forceinline__ void far_flush(FarSums&, double*) {}
+    static constexpr int FAR_SOURCES_PER_FLUSH = 128;
+    static __device__ __forceinline__ void far_zero(FarSums& F)
+    {
+#pragma unroll
+        for (int p = 0; p < R_I / 2; ++p) F.ax[p] = F.ay[p] = F.az[p] = 0ull;
+    }
+    static __device__ __forceinline__ void far_flush(FarSums&, double*) {}      // far() flushes at every tile itself
+    static __device__ __forceinline__ void fold_flush(FarSums& F, double* acc)  // the sums far_fold() carries
+    {
+#pragma unroll
+        for (int p = 0; p < R_I / 2; ++p) {
+            float lo, hi;
+            unpack2(F.ax[p], lo, hi); flush(acc, 0, 2 * p, lo); flush(acc, 0, 2 * p + 1, hi);
+            unpack2(F.ay[p], lo, hi); flush(acc, 1, 2 * p, lo); flush(acc, 1, 2 * p + 1, hi);
+            unpack2(F.az[p], lo, hi); flush(acc, 2, 2 * p, lo); flush(acc, 2, 2 * p + 1, hi);
+        }
+        far_zero(F);
+    }
 
     // [j0, j1): the sources of the tile to sum (multiples of 4; the whole tile in the ring driver).
     static __device__ __forceinline__ void far(const Tile& T, const IState& S, FarSums& F, int /*zero*/, int j0 = 0, int j1 = TJ)
@@ -130,26 +149,40 @@ STEPS_UNROLL(STEPS_FAR_UNROLL)
         }
     }
 
-    // Far body in a periodic box (Eq. 5, leading image) for a tile pair with a common image shift (box_shift in common.cuh):
-    // the shift goes onto the source, X' = X_j - c_j s, then the body of far().  WRAP: the boxes straddle half the box in some
-    // component: the scaled differences are wrapped per pair with the source's own period c_j L (3 packed instructions each).
-    template <bool WRAP>
-    static __device__ __forceinline__ void far_box(const Tile& T, const IState& S, FarSums& F, int /*zero*/, const BoxShift& bs, double Ld,
-                                                   int j0 = 0, int j1 = TJ)
+    // Far body in a periodic box (Eq. 5, leading image) for a (group, unit) pair that cannot be softened (box_shift in
+    // common.cuh).  The image shift is already on the i-particles (`shifted`), so the pair arithmetic is the body of far()
+    // plus, for the components in MASK -- those whose separations straddle half the box -- the fold d' = e - copysign(h, e),
+    // h = c_j L/2 per source: one packed subtraction and two LOP3 (the sign transfer, ALU pipe) per two interactions.
+    // The packed sums stay in F across calls (see FarSums).
+    static __device__ __forceinline__ IState shifted(const IState& S, const double (&s)[3])
     {
-        double* acc = F.acc;
+        IState Q;
+#pragma unroll
+        for (int k = 0; k < R_I; ++k) {
+            Q.x[k] = (float)((double)S.x[k] + s[0]); Q.y[k] = (float)((double)S.y[k] + s[1]); Q.z[k] = (float)((double)S.z[k] + s[2]);
+            Q.h[k] = S.h[k];
+        }
+        return Q;
+    }
+    static __device__ __forceinline__ u64 fold2(u64 e, u64 h2)
+    {
+        return sub2(e, h2 | (e & 0x8000000080000000ull));
+    }
+    template <int MASK>
+    static __device__ __forceinline__ void far_fold(const Tile& T, const IState& S, FarSums& F, int /*zero*/, double halfLd,
+                                                    int j0 = 0, int j1 = TJ)
+    {
         constexpr int NP = R_I / 2;
-        const float sx = (float)bs.s[0], sy = (float)bs.s[1], sz = (float)bs.s[2], L = (float)Ld;
-        u64 nx[NP], ny[NP], nz[NP], ax[NP], ay[NP], az[NP];
+        const float halfL = (float)halfLd;
+        u64 nx[NP], ny[NP], nz[NP];
+        u64 (&ax)[NP] = F.ax, (&ay)[NP] = F.ay, (&az)[NP] = F.az;
 #pragma unroll
         for (int p = 0; p < NP; ++p) {
             nx[p] = pack2(-S.x[2 * p], -S.x[2 * p + 1]);
             ny[p] = pack2(-S.y[2 * p], -S.y[2 * p + 1]);
             nz[p] = pack2(-S.z[2 * p], -S.z[2 * p + 1]);
-            ax[p] = ay[p] = az[p] = 0ull;
         }
-        const u64 SHIFT = pack2(12582912.0f, 12582912.0f), NSHIFT = pack2(-12582912.0f, -12582912.0f);   // 1.5 * 2^23
-#pragma unroll 1
+STEPS_UNROLL(STEPS_FAR_UNROLL)
         for (int j = j0; j < j1; j += 4) {
             const float4 X = *reinterpret_cast<const float4*>(&T.X[j]);
             const float4 Y = *reinterpret_cast<const float4*>(&T.Y[j]);
@@ -160,20 +193,15 @@ STEPS_UNROLL(STEPS_FAR_UNROLL)
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 const float c = Cs[q ^ STEPS_C_SWIZZLE];
-                const float xs = fmaf(-sx, c, Xs[q]), ys = fmaf(-sy, c, Ys[q]), zs = fmaf(-sz, c, Zs[q]);
-                const u64 cq = pack2(c, c), Xq = pack2(xs, xs), Yq = pack2(ys, ys), Zq = pack2(zs, zs);
-                // pads (c = STEPS_PAD_C32) keep their parked difference: period 0, so that dX.dX still overflows to +inf
-                const bool live = c < 1.0e17f;
-                const float cL = live ? c * L : 0.0f, icL = live ? __frcp_rn(c * L) : 0.0f;
-                const u64 ncL = pack2(-cL, -cL), icL2 = pack2(icL, icL);
+                const u64 cq = pack2(c, c), Xq = pack2(Xs[q], Xs[q]), Yq = pack2(Ys[q], Ys[q]), Zq = pack2(Zs[q], Zs[q]);
+                const float hc = c * halfL;          // pads: 5e17 L against a parked difference of 1e30, which stays parked
+                const u64 h2 = pack2(hc, hc);
 #pragma unroll
                 for (int p = 0; p < NP; ++p) {
                     u64 dX = fma2(nx[p], cq, Xq), dY = fma2(ny[p], cq, Yq), dZ = fma2(nz[p], cq, Zq);
-                    if (WRAP) {
-                        dX = fma2(ncL, add2(fma2(dX, icL2, SHIFT), NSHIFT), dX);
-                        dY = fma2(ncL, add2(fma2(dY, icL2, SHIFT), NSHIFT), dY);
-                        dZ = fma2(ncL, add2(fma2(dZ, icL2, SHIFT), NSHIFT), dZ);
-                    }
+                    if (MASK & 1) dX = fold2(dX, h2);
+                    if (MASK & 2) dY = fold2(dY, h2);
+                    if (MASK & 4) dZ = fold2(dZ, h2);
                     const u64 r2 = fma2(dZ, dZ, fma2(dY, dY, mul2(dX, dX)));
                     float a, b;
                     unpack2(r2, a, b);
@@ -184,13 +212,6 @@ STEPS_UNROLL(STEPS_FAR_UNROLL)
                     az[p] = fma2(dZ, y3, az[p]);
                 }
             }
-        }
-#pragma unroll
-        for (int p = 0; p < NP; ++p) {
-            float lo, hi;
-            unpack2(ax[p], lo, hi); flush(acc, 0, 2 * p, lo); flush(acc, 0, 2 * p + 1, hi);
-            unpack2(ay[p], lo, hi); flush(acc, 1, 2 * p, lo); flush(acc, 1, 2 * p + 1, hi);
-            unpack2(az[p], lo, hi); flush(acc, 2, 2 * p, lo); flush(acc, 2, 2 * p + 1, hi);
         }
     }
 

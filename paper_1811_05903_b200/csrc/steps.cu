@@ -418,13 +418,27 @@ int launch_forces_periodic(const double* pos, const double* mass, const double* 
     if (rc != STEPS_OK) return rc;
     prep_tiles<Tile><<<nt, TJ, 0, st>>>(pos, mass, soft, N, tiles, nullptr);
     g_launches++;
-    if constexpr (BOX == 1) {                      // leading image: per-(group, tile) decisions of uneven cost -> split-j driver
-        if (g_splitj.load() != 0) {
-            rc = launch_splitj<Path, 1>(pos, soft, N, tiles, nt, 0, N, acc_out, st, w, L);
-            if (rc != STEPS_OK) return rc;
-            return release_scratch(w, st);
+    if constexpr (BOX == 1) {                      // leading image: one 128-particle group per CTA column (forces_boxring_kernel)
+        const long long groups = (N + SPLITJ_GROUP - 1) / SPLITJ_GROUP;
+        // with fewer groups than SMs the tile range is split over floor(SMs / groups) CTAs so that the grid is one wave
+        long long jsplit = groups < w.num_sms ? w.num_sms / groups : 1;
+        jsplit = std::max(1ll, std::min<long long>(jsplit, nt));
+        const long long rec_cap = (long long)(partial_bytes(N) / (sizeof(double) * 6 * SPLITJ_GROUP));
+        if (groups * jsplit > rec_cap) jsplit = std::max(1ll, rec_cap / groups);
+        if (groups > 0x7fffffffll || jsplit > 65535) return STEPS_EINVAL;
+        auto kern = forces_boxring_kernel<Path>;
+        constexpr int smem = boxring_smem_bytes<Path>();
+        static bool attr_set = false;                                              // per instantiation
+        if (!attr_set) { STEPS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); attr_set = true; }
+        kern<<<dim3((unsigned)groups, (unsigned)jsplit), CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, acc_out, w.partials, 0, L, 1.0 / L);
+        g_launches++;
+        if (jsplit > 1) {
+            forces_splitj_reduce<<<(unsigned)groups, SPLITJ_GROUP, 0, st>>>(w.partials, (int)jsplit, N, acc_out, NO_FUSE);
+            g_launches++;
         }
-    }
+        STEPS_CUDA(cudaGetLastError());
+        return release_scratch(w, st);
+    } else {
     const int nb = (int)nblocks_of(N);
     constexpr int smem = persistent_smem_bytes<Path, STAGES>();
     auto kern = forces_persistent_kernel<Path, STAGES, BOX>;
@@ -436,6 +450,7 @@ int launch_forces_periodic(const double* pos, const double* mass, const double* 
     g_launches += 2;
     STEPS_CUDA(cudaGetLastError());
     return release_scratch(w, st);
+    }
 }
 
 }  // namespace
