@@ -161,6 +161,41 @@ __device__ __forceinline__ BoxShift box_shift(const float (&loI)[3], const float
     return box_shift(loI, hiI, hmaxI, J.lo, J.hi, J.hmax, L, invL);
 }
 
+// Bounding box and largest softening of 128 consecutive particles (one i-group of the drivers; built by group_meta_kernel
+// in prep.cuh), the unit of the image decisions of the pair-symmetric periodic evaluation.  An empty group (beyond N) has
+// lo = +inf, hi = -inf; a group with a massless or unscalable particle has hmax = +inf (never "far").
+struct alignas(16) GroupMeta {
+    float lo[3], hi[3], hmax, pad;
+};
+static_assert(sizeof(GroupMeta) == 32, "GroupMeta layout");
+// The box of GRAN consecutive groups (GRAN = 1: 128 particles, the fp64 kernels' unit; 2: 256, the mixed kernels').
+template <int GRAN>
+__device__ __forceinline__ GroupMeta group_box(const GroupMeta* __restrict__ gm, int idx)
+{
+    GroupMeta m = gm[idx * GRAN];
+#pragma unroll
+    for (int q = 1; q < GRAN; ++q) {
+        const GroupMeta o = gm[idx * GRAN + q];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { m.lo[c] = fminf(m.lo[c], o.lo[c]); m.hi[c] = fmaxf(m.hi[c], o.hi[c]); }
+        m.hmax = fmaxf(m.hmax, o.hmax);
+    }
+    return m;
+}
+// The image decision of the pair of groups (a, b), a != b, for separations x_j - x_i with i in a and j in b.  The boxes are
+// always passed to box_shift in index order, and the decision of (b, a) is the mirror image of that of (a, b) (shift
+// negated, same fold mask, same kind): the one-sided kernel (which meets every pair from both ends) and the pair-symmetric
+// kernel (which meets it once) therefore agree bit for bit on which pairs "may be softened" -- each pair is evaluated by
+// exactly one of them.
+template <int GRAN>
+__device__ __forceinline__ BoxShift pair_decision(const GroupMeta* __restrict__ gm, int a, int b, double L, double invL)
+{
+    const GroupMeta A = group_box<GRAN>(gm, a < b ? a : b), B = group_box<GRAN>(gm, a < b ? b : a);
+    BoxShift d = box_shift(A.lo, A.hi, A.hmax, B.lo, B.hi, B.hmax, L, invL);
+    if (a > b) { d.s[0] = -d.s[0]; d.s[1] = -d.s[1]; d.s[2] = -d.s[2]; }
+    return d;
+}
+
 // The fold of one separation component: e - copysign(h, e) as (|e| - h) with the sign of e (h = half the period, in the
 // units of e).  One DADD (|e| is an operand modifier) and one LOP3 on the high word.
 __device__ __forceinline__ double fold_f64(double e, double h)

@@ -466,8 +466,10 @@ forces_splitj_kernel(const double* __restrict__ pos, const double* __restrict__ 
     }
 }
 
+// acc_lo_out != nullptr: the result stays double-double (acc_out = hi, acc_lo_out = lo) for forces_sym_reduce_kernel.
 __global__ void __launch_bounds__(128) forces_splitj_reduce(const double* __restrict__ partials, int jsplit, long long cnt,
-                                                            double* __restrict__ acc_out, Eq12Fuse fuse)
+                                                            double* __restrict__ acc_out, Eq12Fuse fuse,
+                                                            double* __restrict__ acc_lo_out = nullptr)
 {
     const int r = threadIdx.x, k = r / 32, l = r % 32;
     const long long i = (long long)blockIdx.x * SPLITJ_GROUP + l + 32 * k;
@@ -486,7 +488,8 @@ __global__ void __launch_bounds__(128) forces_splitj_reduce(const double* __rest
             lo += rec[(3 + c) * SPLITJ_GROUP + r];
         }
         a3[c] = hi + lo;
-        acc_out[(long long)c * cnt + i] = a3[c];
+        if (acc_lo_out) { acc_out[(long long)c * cnt + i] = hi; acc_lo_out[(long long)c * cnt + i] = lo; }
+        else acc_out[(long long)c * cnt + i] = a3[c];
     }
     if (fuse.out_bits) {
         const double a = *fuse.a_state, coef = fuse.absG / (a * a * a);
@@ -511,6 +514,10 @@ __global__ void __launch_bounds__(128) forces_splitj_reduce(const double* __rest
 // global memory.
 // The 16 partial accelerations meet in shared memory and are added in fixed warp order (TwoSum), as in the split-j
 // driver; gridDim.y > 1 splits the tile range over CTAs (records summed by forces_splitj_reduce).
+// RESTRICTED mode (plan != nullptr and the plan kept its items, W < nb - 1): the pairs of two DIFFERENT blocks of 2,048
+// particles belong to the pair-symmetric kernel (forces_sym_box_kernel, force_sym.cuh) and to forces_boxgen_kernel below
+// (the units that may hold a softened pair); this kernel then evaluates the group's own block only and ADDS its result to
+// the double-double (acc_out = hi, acc_lo_out = lo) that forces_boxgen_kernel wrote.
 constexpr int BOXRING_G = 4;                               // sub-rings per CTA
 constexpr int BOXRING_STAGES = 3;                          // stages per sub-ring
 constexpr int DEC_CHUNK = 512;                             // decisions per sub-ring kept in shared memory at a time
@@ -530,8 +537,11 @@ template <typename Path>
 __global__ void __launch_bounds__(CTA_THREADS, 1)
 forces_boxring_kernel(const double* __restrict__ pos, const double* __restrict__ soft, long long N,
                       const typename Path::Tile* __restrict__ tiles, int nt, double* __restrict__ acc_out,
-                      double* __restrict__ partials, int zero, double box_L, double box_invL)
+                      double* __restrict__ partials, int zero, double box_L, double box_invL,
+                      const GroupMeta* __restrict__ gm, const SymPlan* __restrict__ plan, double* __restrict__ acc_lo_out)
 {
+    const bool restricted = plan != nullptr && plan->W < plan->nb - 1;
+    const int my_block = (int)(((long long)blockIdx.x * SPLITJ_GROUP) / IB);
     using Tile = typename Path::Tile;
     using IState = typename Path::IState;
     using Elem = decltype(IState::x[0] + 0);               // double or float
@@ -575,7 +585,9 @@ forces_boxring_kernel(const double* __restrict__ pos, const double* __restrict__
 
     // tile range of this CTA; sub-ring g takes the tiles t0 + g, t0 + g + G, ... (interleaved: every sub-ring meets the same
     // mix of decisions, so the four finish together)
-    const int t0 = (int)((long long)blockIdx.y * nt / gridDim.y), t1 = (int)(((long long)blockIdx.y + 1) * nt / gridDim.y);
+    // (restricted mode: only the tiles of the group's own block; the launcher then uses gridDim.y = 1)
+    const int t0 = restricted ? min(nt, my_block * (IB / TJ)) : (int)((long long)blockIdx.y * nt / gridDim.y);
+    const int t1 = restricted ? min(nt, (my_block + 1) * (IB / TJ)) : (int)(((long long)blockIdx.y + 1) * nt / gridDim.y);
     const int mine = (t1 - t0 - g + G - 1) / G;              // tiles of this sub-ring
     const int chunks = ((t1 - t0 + G - 1) / G + DEC_CHUNK - 1) / DEC_CHUNK;   // the same for every sub-ring (CTA-wide barriers)
     if (threadIdx.x == 0) {
@@ -653,9 +665,135 @@ forces_boxring_kernel(const double* __restrict__ pos, const double* __restrict__
         }
         const long long i = (long long)blockIdx.x * SPLITJ_GROUP + l + 32 * k;
         if (gridDim.y == 1) {
-            if (i < N) acc_out[(long long)c * N + i] = hi + lo;
+            if (i < N) {
+                if (acc_lo_out) {
+                    if (restricted) {                                        // += what forces_boxgen_kernel left there
+                        const double v = acc_out[(long long)c * N + i];
+                        const double s = hi + v, bb = s - hi;
+                        lo += (hi - (s - bb)) + (v - bb) + acc_lo_out[(long long)c * N + i];
+                        hi = s;
+                    }
+                    acc_out[(long long)c * N + i] = hi; acc_lo_out[(long long)c * N + i] = lo;
+                } else acc_out[(long long)c * N + i] = hi + lo;
+            }
         } else {
             double* rec = partials + (((long long)blockIdx.x * gridDim.y + blockIdx.y) * 6) * SPLITJ_GROUP;
+            rec[c * SPLITJ_GROUP + r] = hi; rec[(3 + c) * SPLITJ_GROUP + r] = lo;
+        }
+    }
+}
+
+// ---- the possibly-softened units of other blocks (periodic pair-symmetric evaluation) -----------------------------------
+// One 128-particle group per CTA.  pair_decision (common.cuh) is taken for the group (fp64) / its 256-particle parent
+// (mixed) against every 128- / 256-source unit of the OTHER blocks -- the very call by which forces_sym_box_kernel skips
+// a meeting; the units it calls "general" are gathered into a list in a fixed order (warp w scans its slice of the units,
+// the offsets come from the warps' counts); the listed units' plain sources are staged in shared memory eight at a time
+// and each is shared by four warps (a quarter of its sources each) through the general wrapped body.  Writes the group's
+// result double-double (zero when the plan has no items: then forces_boxring_kernel evaluates everything).
+// gridDim.y > 1 splits the unit range over CTAs (records [group][y][6][128] in `records`, summed by forces_splitj_reduce):
+// a group whose bounding box spans the whole box -- its 128 particles straddle a top-level jump of the cell order, a few
+// groups of any set -- has EVERY unit on its list, and one CTA would work on it long after all others are done.
+constexpr int BOXGEN_CHUNK = 4096;                         // units decided and listed at a time (16 KiB of list)
+constexpr int BOXGEN_BATCH = 8;                            // listed units staged in shared memory at a time (5 KiB each)
+template <typename Path>
+constexpr int boxgen_smem_bytes()
+{
+    return Path::NOUT * R_I * CTA_THREADS * (int)sizeof(double) + BOXGEN_CHUNK * (int)sizeof(uint32_t) +
+           BOXGEN_BATCH * 5 * (Path::NOUT == 6 ? 1 : 2) * SPLITJ_GROUP * (Path::NOUT == 6 ? 8 : 4);
+}
+
+template <typename Path>
+__global__ void __launch_bounds__(CTA_THREADS, 1)
+forces_boxgen_kernel(const double* __restrict__ pos, const double* __restrict__ soft, long long N,
+                     const typename Path::Tile* __restrict__ tiles, int nt, double* __restrict__ acc_hi, double* __restrict__ acc_lo,
+                     double* __restrict__ records, double box_L, double box_invL, const GroupMeta* __restrict__ gm,
+                     const SymPlan* __restrict__ plan)
+{
+    using IState = typename Path::IState;
+    constexpr int GRAN = Path::NOUT == 6 ? 1 : 2;           // groups per unit (the symmetric kernels' subgroups)
+    using Elem = decltype(IState::x[0] + 0);                // double or float
+    constexpr int UNIT = GRAN * SPLITJ_GROUP, WARPS = CTA_THREADS / 32, WPU = 4, SLICE = UNIT / WPU;   // 4 warps per unit
+    static_assert(TJ == 2 * SPLITJ_GROUP && SLICE % 2 == 0, "a tile is two groups; the mixed general body takes sources in pairs");
+    static_assert(BOXGEN_BATCH % (WARPS / WPU) == 0, "whole rounds of WARPS / WPU units per batch");
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ int gcount[WARPS];
+    double* acc_all = reinterpret_cast<double*>(smem_raw);
+    double* acc = acc_all + threadIdx.x;
+    uint32_t* glist = reinterpret_cast<uint32_t*>(acc_all + Path::NOUT * R_I * CTA_THREADS);
+    Elem* stage = reinterpret_cast<Elem*>(glist + BOXGEN_CHUNK);             // [BOXGEN_BATCH][5 (x, y, z, m, h)][UNIT]
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const bool active = plan->W < plan->nb - 1;
+    const int my_block = (int)(((long long)blockIdx.x * SPLITJ_GROUP) / IB);
+    const int me = (int)blockIdx.x / GRAN;                  // this group's unit index
+    const int units_all = (int)((N + UNIT - 1) / UNIT);
+    const int u_lo = (int)((long long)blockIdx.y * units_all / gridDim.y), units = (int)(((long long)blockIdx.y + 1) * units_all / gridDim.y);
+
+    IState S;
+    {
+        float rlo, rhi, hh;
+        const long long i0 = (long long)blockIdx.x * SPLITJ_GROUP + lane;
+        load_i_block<Path>(S, pos, soft, N, i0, N, rlo, rhi, hh);
+    }
+#pragma unroll
+    for (int q = 0; q < Path::NOUT * R_I; ++q) acc[q * CTA_THREADS] = 0.0;
+
+    for (int u0 = u_lo; active && u0 < units; u0 += BOXGEN_CHUNK) {
+        const int cnt = min(BOXGEN_CHUNK, units - u0);
+        constexpr int PER = BOXGEN_CHUNK / WARPS;           // units scanned per warp
+        auto wanted = [&](int q) {
+            if (q >= cnt) return false;
+            const int u = u0 + q;
+            if ((int)(((long long)u * UNIT) / IB) == my_block) return false;       // own block: forces_boxring_kernel
+            return (boxcode_pack(pair_decision<GRAN>(gm, me, u, box_L, box_invL), box_invL) & BOXCODE_GENERAL) != 0;
+        };
+        unsigned flags[PER / 32];
+        int mine_cnt = 0;
+#pragma unroll
+        for (int r = 0; r < PER / 32; ++r) { flags[r] = __ballot_sync(0xffffffffu, wanted(warp * PER + r * 32 + lane)); mine_cnt += __popc(flags[r]); }
+        __syncthreads();                                    // the previous chunk's list is no longer read
+        if (lane == 0) gcount[warp] = mine_cnt;
+        __syncthreads();
+        int at = 0, total_cnt = 0;
+        for (int w = 0; w < WARPS; ++w) { if (w < warp) at += gcount[w]; total_cnt += gcount[w]; }
+#pragma unroll
+        for (int r = 0; r < PER / 32; ++r) {
+            if (flags[r] >> lane & 1u) glist[at + __popc(flags[r] & ((1u << lane) - 1u))] = (uint32_t)(u0 + warp * PER + r * 32 + lane);
+            at += __popc(flags[r]);
+        }
+        __syncthreads();
+        for (int e0 = 0; e0 < total_cnt; e0 += BOXGEN_BATCH) {
+            const int nbatch = min(BOXGEN_BATCH, total_cnt - e0);
+            if (e0 > 0) __syncthreads();                    // the previous batch is no longer read
+            for (int q = threadIdx.x; q < nbatch * 5 * UNIT; q += CTA_THREADS) {
+                const int e = q / (5 * UNIT), a = (q / UNIT) % 5, j = q % UNIT;
+                const long long src = (long long)glist[e0 + e] * UNIT;            // first source of the unit
+                // x[], y[], z[], m[], h[] follow one another in the tile record (common.cuh)
+                stage[q] = (&tiles[src / TJ].x[0])[a * TJ + (int)(src % TJ) + j];
+            }
+            __syncthreads();
+            for (int e = warp / WPU; e < nbatch; e += WARPS / WPU) {
+                const Elem* u = stage + e * 5 * UNIT;
+                const int j0 = (warp % WPU) * SLICE;
+                Path::template near_view<true>(u, u + UNIT, u + 2 * UNIT, u + 3 * UNIT, u + 4 * UNIT, S, acc, box_L, box_invL, j0, j0 + SLICE);
+            }
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x < 3 * SPLITJ_GROUP) {                   // fixed-order sum over the 16 warps, as in the split-j driver
+        const int c = threadIdx.x / SPLITJ_GROUP, r = threadIdx.x % SPLITJ_GROUP, k = r / 32, l = r % 32;
+        double hi = 0.0, lo = 0.0;
+        for (int w = 0; w < WARPS; ++w) {
+            const double v = acc_all[(c * R_I + k) * CTA_THREADS + w * 32 + l];
+            const double s = hi + v, bb = s - hi;
+            lo += (hi - (s - bb)) + (v - bb);                              // TwoSum
+            hi = s;
+            if (Path::NOUT == 6) lo += acc_all[((3 + c) * R_I + k) * CTA_THREADS + w * 32 + l];
+        }
+        const long long i = (long long)blockIdx.x * SPLITJ_GROUP + l + 32 * k;
+        if (gridDim.y == 1) {
+            if (i < N) { acc_hi[(long long)c * N + i] = hi; acc_lo[(long long)c * N + i] = lo; }
+        } else {
+            double* rec = records + (((long long)blockIdx.x * gridDim.y + blockIdx.y) * 6) * SPLITJ_GROUP;
             rec[c * SPLITJ_GROUP + r] = hi; rec[(3 + c) * SPLITJ_GROUP + r] = lo;
         }
     }

@@ -359,12 +359,21 @@ struct Fp64Path {
     static __device__ __forceinline__ void near_box(const Tile& T, const IState& S, double* acc, double L, double invL,
                                                     int j0 = 0, int j1 = TJ)
     {
+        near_view<PERIODIC>(T.x, T.y, T.z, T.m, T.h, S, acc, L, invL, j0, j1);
+    }
+    // The same on any copy of the plain sources (x, y, z, m, h), e.g. one staged in shared memory.
+    template <bool PERIODIC>
+    static __device__ __forceinline__ void near_view(const double* __restrict__ Tx, const double* __restrict__ Ty,
+                                                     const double* __restrict__ Tz, const double* __restrict__ Tm,
+                                                     const double* __restrict__ Th, const IState& S, double* acc, double L,
+                                                     double invL, int j0, int j1)
+    {
         double ax[R_I], ay[R_I], az[R_I];
 #pragma unroll
         for (int k = 0; k < R_I; ++k) ax[k] = ay[k] = az[k] = 0.0;
 #pragma unroll 1
         for (int j = j0; j < j1; ++j) {
-            const double xj = T.x[j], yj = T.y[j], zj = T.z[j], mq = T.m[j], hj = T.h[j];
+            const double xj = Tx[j], yj = Ty[j], zj = Tz[j], mq = Tm[j], hj = Th[j];
 #pragma unroll
             for (int k = 0; k < R_I; ++k) {
                 double dx = xj - S.x[k], dy = yj - S.y[k], dz = zj - S.z[k];

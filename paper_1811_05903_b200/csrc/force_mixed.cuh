@@ -242,6 +242,15 @@ STEPS_UNROLL(STEPS_FAR_UNROLL)
     static __device__ __forceinline__ void near_box(const Tile& T, const IState& S, double* acc, double Ld, double invLd,
                                                     int j0 = 0, int j1 = TJ)
     {
+        near_view<PERIODIC>(T.x, T.y, T.z, T.m, T.h, S, acc, Ld, invLd, j0, j1);
+    }
+    // The same on any copy of the plain sources (x, y, z, m, h), e.g. one staged in shared memory (8-byte aligned, j0 even).
+    template <bool PERIODIC>
+    static __device__ __forceinline__ void near_view(const float* __restrict__ Tx, const float* __restrict__ Ty,
+                                                     const float* __restrict__ Tz, const float* __restrict__ Tm,
+                                                     const float* __restrict__ Th, const IState& S, double* acc, double Ld,
+                                                     double invLd, int j0, int j1)
+    {
         const u64 negL = pack2(-(float)Ld, -(float)Ld), invL = pack2((float)invLd, (float)invLd);
         u64 xi[R_I], yi[R_I], zi[R_I], hi[R_I], ax[R_I], ay[R_I], az[R_I];
 #pragma unroll
@@ -252,9 +261,9 @@ STEPS_UNROLL(STEPS_FAR_UNROLL)
         }
 #pragma unroll 2
         for (int j = j0; j < j1; j += 2) {
-            const u64 xj = *reinterpret_cast<const u64*>(&T.x[j]), yj = *reinterpret_cast<const u64*>(&T.y[j]);
-            const u64 zj = *reinterpret_cast<const u64*>(&T.z[j]), mj = *reinterpret_cast<const u64*>(&T.m[j]);
-            const u64 hj = *reinterpret_cast<const u64*>(&T.h[j]);
+            const u64 xj = *reinterpret_cast<const u64*>(&Tx[j]), yj = *reinterpret_cast<const u64*>(&Ty[j]);
+            const u64 zj = *reinterpret_cast<const u64*>(&Tz[j]), mj = *reinterpret_cast<const u64*>(&Tm[j]);
+            const u64 hj = *reinterpret_cast<const u64*>(&Th[j]);
 #pragma unroll
             for (int k = 0; k < R_I; ++k) {
                 u64 dx = sub2(xj, xi[k]), dy = sub2(yj, yi[k]), dz = sub2(zj, zi[k]);

@@ -474,6 +474,415 @@ forces_sym_mixed_kernel(const TileF32* __restrict__ tiles, const SymPlan* __rest
     }
 }
 
+// ---- the pair-symmetric evaluation in a periodic box (leading image, Eq. 5) -------------
+// The same items, rounds, hand-over and records as above, with three differences:
+//   * every block pair (b, c), c > b, is an item (W = 0): in a periodic box closeness is not a matter of |c - b|.  Which
+//     pairs may be softened is decided per MEETING of a warp's group (128 particles fp64 / 256 mixed) with a subgroup of
+//     the column block, by pair_decision (common.cuh) on the groups' bounding boxes: a meeting that may hold a softened pair
+//     is skipped here and evaluated by forces_boxring_kernel in restricted mode (force_driver.cuh), which takes the very
+//     same decision from the very same call;
+//   * the image shift of the meeting goes onto the warp's particles (a copy of the row block's positions stays in shared
+//     memory, each thread's own four/eight), and the components whose separations straddle half the box are folded
+//     (fold_f64 / fold2: one addition + one bit operation per pair and component), the body chosen by the fold mask;
+//   * the reaction on j uses the folded separation as well -- the leading image of x_i - x_j is minus that of x_j - x_i.
+template <int RI, int MASK>
+__device__ __forceinline__ void sym_box_steps(const FarSrcF64* __restrict__ set, int lane, int src_lane, const double (&xi)[RI],
+                                              const double (&yi)[RI], const double (&zi)[RI], const double (&mi)[RI], double (&ax)[RI],
+                                              double (&ay)[RI], double (&az)[RI], double& bx, double& by, double& bz, int zero, double halfL)
+{
+    constexpr double A = 1.4;
+    constexpr double C0 = 1.0 / STEPS_FP64_FOLD - (1.0 - A) * (1.0 - A);
+#pragma unroll 1
+    for (int st = 0; st < 32; ++st) {
+        const FarSrcF64* src = set + ((lane - st) & 31);
+        const double2 XY = *reinterpret_cast<const double2*>(&src->X);
+        const double2 ZC = *reinterpret_cast<const double2*>(&src->Z);
+        const double X = XY.x, Y = XY.y, Z = ZC.x, C = ZC.y;
+        const double hc = C * halfL;
+        double dX[RI], dY[RI], dZ[RI], r2[RI], y0[RI], y2[RI], w[RI];
+        STEPS_STAGE_FENCE(zero, 0);
+#pragma unroll
+        for (int k = 0; k < RI; ++k) dX[k] = fma(-xi[k], C, X);
+#pragma unroll
+        for (int k = 0; k < RI; ++k) dY[k] = fma(-yi[k], C, Y);
+#pragma unroll
+        for (int k = 0; k < RI; ++k) dZ[k] = fma(-zi[k], C, Z);
+        if (MASK & 1) {
+#pragma unroll
+            for (int k = 0; k < RI; ++k) dX[k] = fold_f64(dX[k], hc);
+        }
+        if (MASK & 2) {
+#pragma unroll
+            for (int k = 0; k < RI; ++k) dY[k] = fold_f64(dY[k], hc);
+        }
+        if (MASK & 4) {
+#pragma unroll
+            for (int k = 0; k < RI; ++k) dZ[k] = fold_f64(dZ[k], hc);
+        }
+        STEPS_STAGE_FENCE(zero, 1);
+#pragma unroll
+        for (int k = 0; k < RI; ++k) r2[k] = fma(dZ[k], dZ[k], fma(dY[k], dY[k], dX[k] * dX[k]));
+#pragma unroll
+        for (int k = 0; k < RI; ++k) y0[k] = rsqrt_seed(r2[k]);
+#pragma unroll
+        for (int k = 0; k < RI; ++k) {
+            y2[k] = y0[k] * y0[k];
+            w[k] = fma(r2[k], y2[k], -A);
+            y2[k] = y0[k] * y2[k];
+            w[k] = fma(w[k], w[k], C0);
+            w[k] = y2[k] * w[k];
+        }
+        STEPS_STAGE_FENCE(zero, 2);
+#pragma unroll
+        for (int k = 0; k < RI; ++k) {
+            if (k > 0) STEPS_STAGE_FENCE(zero, 2 + k);
+            const double si = mi[k] * w[k];
+            ax[k] = fma(dX[k], w[k], ax[k]);
+            ay[k] = fma(dY[k], w[k], ay[k]);
+            az[k] = fma(dZ[k], w[k], az[k]);
+            bz = fma(dZ[k], si, bz);
+            by = fma(dY[k], si, by);
+            bx = fma(dX[k], si, bx);
+        }
+        bx = __shfl_sync(0xffffffffu, bx, src_lane);
+        by = __shfl_sync(0xffffffffu, by, src_lane);
+        bz = __shfl_sync(0xffffffffu, bz, src_lane);
+    }
+}
+
+__host__ __device__ constexpr int sym_box_smem_bytes() { return sym_smem_bytes() + 3 * IB * (int)sizeof(double); }
+
+template <int THREADS, int RI, bool SPLIT>
+__global__ void __launch_bounds__(THREADS, 1)
+forces_sym_box_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__ plan, const GroupMeta* __restrict__ gm,
+                      long long k_begin, long long k_end, double* __restrict__ rowrec, double* __restrict__ colrec, int zero,
+                      int split_arg, double box_L, double box_invL)
+{
+    const int split = SPLIT ? split_arg : 1;
+    static_assert(THREADS * RI == IB, "the CTA holds one block");
+    constexpr int WI = 32 * RI;                 // particles per warp = sources per subgroup
+    constexpr int SUBG = THREADS / 32;          // warps = subgroups per block
+    static_assert(WI == WARP_I, "a warp's particles are one group of GroupMeta");
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ uint64_t full_bar[2];
+    FarSrcF64* col = reinterpret_cast<FarSrcF64*>(smem_raw);                       // [2][IB]
+    double* Bsm = reinterpret_cast<double*>(smem_raw + 2 * IB * sizeof(FarSrcF64));   // [3][IB]
+    double* Xsm = Bsm + 3 * IB + threadIdx.x;                                      // [3][RI][THREADS]: the row block, unshifted
+
+    const long long K = plan->K * split;
+    if (k_end > K) k_end = K;
+    if (k_begin >= k_end) return;
+    const int nb = plan->nb, Km = plan->Km;     // W = 0: item (b, c) for every c > b
+    const long long n_items = k_end - k_begin;
+    const long long kk0 = k_begin + (long long)blockIdx.x * n_items / gridDim.x;
+    const long long kk1 = k_begin + ((long long)blockIdx.x + 1) * n_items / gridDim.x;
+    const int total = (int)(kk1 - kk0);
+    if (total <= 0) return;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    int b, c;
+    {
+        const double t = 2.0 * Km + 1.0;
+        const long long item0 = kk0 / split;
+        int bb = (int)((t - sqrt(fmax(t * t - 8.0 * (double)item0, 0.0))) * 0.5);
+        bb = max(0, min(bb, Km - 1));
+        while (bb + 1 < Km && sym_row_start(bb + 1, Km) <= item0) ++bb;
+        while (bb > 0 && sym_row_start(bb, Km) > item0) --bb;
+        b = bb;
+        c = bb + 1 + (int)(item0 - sym_row_start(bb, Km));
+    }
+
+    if (threadIdx.x == 0) {
+        mbar_init(&full_bar[0], 1); mbar_init(&full_bar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    int pb = b, pc = c;
+    auto produce = [&](int it) {
+        const int s = it & 1;
+        mbar_expect_tx(&full_bar[s], (uint32_t)(IB * sizeof(FarSrcF64)));
+#pragma unroll
+        for (int t = 0; t < TPB; ++t)
+            bulk_load(col + (size_t)s * IB + t * TJ, &tiles[(long long)pc * TPB + t].far[0], (uint32_t)(TJ * sizeof(FarSrcF64)),
+                      &full_bar[s]);
+        if ((kk0 + it + 1) % split == 0 && ++pc == nb) { ++pb; pc = pb + 1; }
+    };
+    if (threadIdx.x == 0) {
+        produce(0);
+        if (total > 1) produce(1);
+    }
+
+    double mi[RI];
+    int cur_b = -1;
+    const int src_lane = (lane + 31) & 31;
+    const double halfL = 0.5 * box_L;
+
+    for (int it = 0; it < total; ++it) {
+        if (b != cur_b) {
+            cur_b = b;
+#pragma unroll
+            for (int k = 0; k < RI; ++k) {
+                const int i = warp * WI + lane + 32 * k;
+                const TileF64& T = tiles[(long long)b * TPB + i / TJ];
+                Xsm[(0 * RI + k) * THREADS] = T.x[i % TJ]; Xsm[(1 * RI + k) * THREADS] = T.y[i % TJ];
+                Xsm[(2 * RI + k) * THREADS] = T.z[i % TJ]; mi[k] = T.m[i % TJ];
+            }
+        }
+        double ax[RI], ay[RI], az[RI];
+#pragma unroll
+        for (int k = 0; k < RI; ++k) ax[k] = ay[k] = az[k] = 0.0;
+        for (int q = threadIdx.x; q < 3 * IB; q += THREADS) Bsm[q] = 0.0;
+        const int s = it & 1;
+        mbar_wait(&full_bar[s], (it >> 1) & 1);
+        __syncthreads();
+        const FarSrcF64* cs = col + (size_t)s * IB;
+
+        // the image decisions of this warp's SUBG meetings of the item, one per lane (boxcode_pack, force_driver.cuh)
+        const uint32_t my_code = boxcode_pack(pair_decision<1>(gm, b * SUBG + warp, c * SUBG + (lane & (SUBG - 1)), box_L, box_invL), box_invL);
+        const int part = SPLIT ? (int)((kk0 + it) % split) : 0, rounds = SPLIT ? SUBG / split : SUBG;
+        for (int q = part * rounds; q < (part + 1) * rounds; ++q) {
+            const int u = (warp + q) & (SUBG - 1);
+            const BoxShift dec = boxcode_unpack(__shfl_sync(0xffffffffu, my_code, u), box_L);
+            if (dec.kind != 0) {                              // else: forces_boxring_kernel evaluates this meeting
+                double xi[RI], yi[RI], zi[RI];
+#pragma unroll
+                for (int k = 0; k < RI; ++k) {
+                    xi[k] = Xsm[(0 * RI + k) * THREADS] + dec.s[0]; yi[k] = Xsm[(1 * RI + k) * THREADS] + dec.s[1];
+                    zi[k] = Xsm[(2 * RI + k) * THREADS] + dec.s[2];
+                }
+                for (int t = 0; t < WI / 32; ++t) {
+                    const FarSrcF64* set = cs + u * WI + t * 32;
+                    double bx = 0.0, by = 0.0, bz = 0.0;
+                    switch (dec.mask) {
+                        case 0: sym_box_steps<RI, 0>(set, lane, src_lane, xi, yi, zi, mi, ax, ay, az, bx, by, bz, zero, halfL); break;
+                        case 1: sym_box_steps<RI, 1>(set, lane, src_lane, xi, yi, zi, mi, ax, ay, az, bx, by, bz, zero, halfL); break;
+                        case 2: sym_box_steps<RI, 2>(set, lane, src_lane, xi, yi, zi, mi, ax, ay, az, bx, by, bz, zero, halfL); break;
+                        case 3: sym_box_steps<RI, 3>(set, lane, src_lane, xi, yi, zi, mi, ax, ay, az, bx, by, bz, zero, halfL); break;
+                        case 4: sym_box_steps<RI, 4>(set, lane, src_lane, xi, yi, zi, mi, ax, ay, az, bx, by, bz, zero, halfL); break;
+                        case 5: sym_box_steps<RI, 5>(set, lane, src_lane, xi, yi, zi, mi, ax, ay, az, bx, by, bz, zero, halfL); break;
+                        case 6: sym_box_steps<RI, 6>(set, lane, src_lane, xi, yi, zi, mi, ax, ay, az, bx, by, bz, zero, halfL); break;
+                        default: sym_box_steps<RI, 7>(set, lane, src_lane, xi, yi, zi, mi, ax, ay, az, bx, by, bz, zero, halfL); break;
+                    }
+                    const int j = u * WI + t * 32 + lane;
+                    Bsm[j] += bx; Bsm[IB + j] += by; Bsm[2 * IB + j] += bz;
+                }
+            }
+            __syncthreads();
+        }
+
+        const long long rec = (kk0 + it - k_begin) * 3 * IB;
+#pragma unroll
+        for (int k = 0; k < RI; ++k) {
+            const int i = warp * WI + lane + 32 * k;
+            rowrec[rec + i] = ax[k]; rowrec[rec + IB + i] = ay[k]; rowrec[rec + 2 * IB + i] = az[k];
+        }
+        for (int j = threadIdx.x; j < IB; j += THREADS) {
+            const double cj = cs[j].c;
+            const double f = -STEPS_FP64_FOLD * cj * cj;
+            colrec[rec + j] = f * Bsm[j]; colrec[rec + IB + j] = f * Bsm[IB + j]; colrec[rec + 2 * IB + j] = f * Bsm[2 * IB + j];
+        }
+        __syncthreads();
+        if (threadIdx.x == 0 && it + 2 < total) produce(it + 2);
+        if ((kk0 + it + 1) % split == 0 && ++c == nb) { ++b; c = b + 1; }
+    }
+}
+
+// The mixed path of the same: the warp's 256 particles are two groups of GroupMeta (pair_decision<2>), a subgroup is one tile.
+template <int THREADS, int RI>
+__host__ __device__ constexpr int sym_mixed_box_smem_bytes() { return sym_mixed_smem_bytes<THREADS, RI>() + 3 * IB * (int)sizeof(float); }
+
+template <int NP, int MASK>
+__device__ __forceinline__ void sym_mixed_box_steps(const float* __restrict__ set, int lane, int src_lane, const u64 (&nx)[NP],
+                                                    const u64 (&ny)[NP], const u64 (&nz)[NP], const u64 (&m2)[NP], u64 (&ax)[NP],
+                                                    u64 (&ay)[NP], u64 (&az)[NP], u64& bx, u64& by, u64& bz, float halfL)
+{
+#pragma unroll 2
+    for (int st = 0; st < 32; ++st) {
+        const int r = (lane - st) & 31;
+        const float X = set[r], Y = set[TJ + r], Z = set[2 * TJ + r], C = set[3 * TJ + (r ^ STEPS_C_SWIZZLE)];
+        const u64 cq = pack2(C, C), Xq = pack2(X, X), Yq = pack2(Y, Y), Zq = pack2(Z, Z);
+        const float hc = C * halfL;
+        const u64 h2 = pack2(hc, hc);
+#pragma unroll
+        for (int p = 0; p < NP; ++p) {
+            u64 dX = fma2(nx[p], cq, Xq), dY = fma2(ny[p], cq, Yq), dZ = fma2(nz[p], cq, Zq);
+            if (MASK & 1) dX = MixedPath::fold2(dX, h2);
+            if (MASK & 2) dY = MixedPath::fold2(dY, h2);
+            if (MASK & 4) dZ = MixedPath::fold2(dZ, h2);
+            const u64 r2 = fma2(dZ, dZ, fma2(dY, dY, mul2(dX, dX)));
+            float ra, rb;
+            unpack2(r2, ra, rb);
+            const u64 y = pack2(rsqrt_approx(ra), rsqrt_approx(rb));
+            const u64 y3 = mul2(mul2(y, y), y);
+            const u64 si = mul2(y3, m2[p]);
+            ax[p] = fma2(dX, y3, ax[p]);
+            ay[p] = fma2(dY, y3, ay[p]);
+            az[p] = fma2(dZ, y3, az[p]);
+            bz = fma2(dZ, si, bz);
+            by = fma2(dY, si, by);
+            bx = fma2(dX, si, bx);
+        }
+        bx = __shfl_sync(0xffffffffu, bx, src_lane);
+        by = __shfl_sync(0xffffffffu, by, src_lane);
+        bz = __shfl_sync(0xffffffffu, bz, src_lane);
+    }
+}
+
+template <int THREADS, int RI, bool SPLIT>
+__global__ void __launch_bounds__(THREADS, 1)
+forces_sym_mixed_box_kernel(const TileF32* __restrict__ tiles, const SymPlan* __restrict__ plan, const GroupMeta* __restrict__ gm,
+                            long long k_begin, long long k_end, double* __restrict__ rowrec, double* __restrict__ colrec,
+                            int split_arg, double box_L, double box_invL)
+{
+    const int split = SPLIT ? split_arg : 1;
+    static_assert(THREADS * RI == IB && RI % 2 == 0, "the CTA holds one block, particles packed in pairs");
+    constexpr int NP = RI / 2;                  // packed pairs per lane
+    constexpr int WI = 32 * RI;                 // particles per warp = sources per subgroup
+    constexpr int SUBG = THREADS / 32;          // warps = subgroups per block
+    static_assert(WI == 2 * WARP_I && WI == TJ, "a warp's particles are two groups of GroupMeta, a subgroup is one tile");
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ uint64_t full_bar[2];
+    constexpr int STAGE = sym_mixed_stage_bytes();
+    float* col = reinterpret_cast<float*>(smem_raw);                                   // [2][TPB][4][TJ]
+    double* Bsm = reinterpret_cast<double*>(smem_raw + 2 * STAGE);                     // [3][IB]
+    double* Asm = Bsm + 3 * IB + threadIdx.x;                                          // [3][RI][THREADS], this thread's column
+    float* Xsm = reinterpret_cast<float*>(Bsm + 3 * IB + 3 * RI * THREADS) + threadIdx.x;   // [3][RI][THREADS]: the row block, unshifted
+
+    const long long K = plan->K * split;
+    if (k_end > K) k_end = K;
+    if (k_begin >= k_end) return;
+    const int nb = plan->nb, Km = plan->Km;
+    const long long n_items = k_end - k_begin;
+    const long long kk0 = k_begin + (long long)blockIdx.x * n_items / gridDim.x;
+    const long long kk1 = k_begin + ((long long)blockIdx.x + 1) * n_items / gridDim.x;
+    const int total = (int)(kk1 - kk0);
+    if (total <= 0) return;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    int b, c;
+    {
+        const double t = 2.0 * Km + 1.0;
+        const long long item0 = kk0 / split;
+        int bb = (int)((t - sqrt(fmax(t * t - 8.0 * (double)item0, 0.0))) * 0.5);
+        bb = max(0, min(bb, Km - 1));
+        while (bb + 1 < Km && sym_row_start(bb + 1, Km) <= item0) ++bb;
+        while (bb > 0 && sym_row_start(bb, Km) > item0) --bb;
+        b = bb;
+        c = bb + 1 + (int)(item0 - sym_row_start(bb, Km));
+    }
+    if (threadIdx.x == 0) {
+        mbar_init(&full_bar[0], 1); mbar_init(&full_bar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    int pb = b, pc = c;
+    auto produce = [&](int it) {
+        const int s = it & 1;
+        mbar_expect_tx(&full_bar[s], (uint32_t)STAGE);
+#pragma unroll
+        for (int t = 0; t < TPB; ++t)
+            bulk_load(reinterpret_cast<unsigned char*>(col) + (size_t)s * STAGE + t * (4 * TJ * sizeof(float)),
+                      &tiles[(long long)pc * TPB + t].X[0], (uint32_t)(4 * TJ * sizeof(float)), &full_bar[s]);
+        if ((kk0 + it + 1) % split == 0 && ++pc == nb) { ++pb; pc = pb + 1; }
+    };
+    if (threadIdx.x == 0) {
+        produce(0);
+        if (total > 1) produce(1);
+    }
+
+    u64 m2[NP];
+    int cur_b = -1;
+    const int src_lane = (lane + 31) & 31;
+    const float halfL = (float)(0.5 * box_L);
+
+    for (int it = 0; it < total; ++it) {
+        if (b != cur_b) {
+            cur_b = b;
+            float m[RI];
+#pragma unroll
+            for (int k = 0; k < RI; ++k) {
+                const int i = warp * WI + lane + 32 * k;
+                const TileF32& T = tiles[(long long)b * TPB + i / TJ];
+                Xsm[(0 * RI + k) * THREADS] = T.x[i % TJ]; Xsm[(1 * RI + k) * THREADS] = T.y[i % TJ];
+                Xsm[(2 * RI + k) * THREADS] = T.z[i % TJ]; m[k] = T.m[i % TJ];
+            }
+#pragma unroll
+            for (int p = 0; p < NP; ++p) m2[p] = pack2(m[2 * p], m[2 * p + 1]);
+        }
+#pragma unroll
+        for (int q = 0; q < 3 * RI; ++q) Asm[q * THREADS] = 0.0;
+        for (int q = threadIdx.x; q < 3 * IB; q += THREADS) Bsm[q] = 0.0;
+        const int s = it & 1;
+        mbar_wait(&full_bar[s], (it >> 1) & 1);
+        __syncthreads();
+        const float* cs = col + (size_t)s * (STAGE / sizeof(float));
+
+        const uint32_t my_code = boxcode_pack(pair_decision<2>(gm, b * SUBG + warp, c * SUBG + (lane & (SUBG - 1)), box_L, box_invL), box_invL);
+        const int part = SPLIT ? (int)((kk0 + it) % split) : 0, rounds = SPLIT ? SUBG / split : SUBG;
+        for (int q = part * rounds; q < (part + 1) * rounds; ++q) {
+            const int u = (warp + q) & (SUBG - 1);
+            const BoxShift dec = boxcode_unpack(__shfl_sync(0xffffffffu, my_code, u), box_L);
+            if (dec.kind != 0) {                              // else: forces_boxring_kernel evaluates this meeting
+                u64 nx[NP], ny[NP], nz[NP], ax[NP], ay[NP], az[NP];
+#pragma unroll
+                for (int p = 0; p < NP; ++p) {
+                    nx[p] = pack2(-(float)((double)Xsm[(0 * RI + 2 * p) * THREADS] + dec.s[0]), -(float)((double)Xsm[(0 * RI + 2 * p + 1) * THREADS] + dec.s[0]));
+                    ny[p] = pack2(-(float)((double)Xsm[(1 * RI + 2 * p) * THREADS] + dec.s[1]), -(float)((double)Xsm[(1 * RI + 2 * p + 1) * THREADS] + dec.s[1]));
+                    nz[p] = pack2(-(float)((double)Xsm[(2 * RI + 2 * p) * THREADS] + dec.s[2]), -(float)((double)Xsm[(2 * RI + 2 * p + 1) * THREADS] + dec.s[2]));
+                    ax[p] = ay[p] = az[p] = 0ull;
+                }
+                for (int t = 0; t < WI / 32; ++t) {
+                    const int j0 = u * WI + t * 32;
+                    const float* set = cs + (j0 / TJ) * (4 * TJ) + (j0 % TJ);
+                    u64 bx = 0ull, by = 0ull, bz = 0ull;
+                    switch (dec.mask) {
+                        case 0: sym_mixed_box_steps<NP, 0>(set, lane, src_lane, nx, ny, nz, m2, ax, ay, az, bx, by, bz, halfL); break;
+                        case 1: sym_mixed_box_steps<NP, 1>(set, lane, src_lane, nx, ny, nz, m2, ax, ay, az, bx, by, bz, halfL); break;
+                        case 2: sym_mixed_box_steps<NP, 2>(set, lane, src_lane, nx, ny, nz, m2, ax, ay, az, bx, by, bz, halfL); break;
+                        case 3: sym_mixed_box_steps<NP, 3>(set, lane, src_lane, nx, ny, nz, m2, ax, ay, az, bx, by, bz, halfL); break;
+                        case 4: sym_mixed_box_steps<NP, 4>(set, lane, src_lane, nx, ny, nz, m2, ax, ay, az, bx, by, bz, halfL); break;
+                        case 5: sym_mixed_box_steps<NP, 5>(set, lane, src_lane, nx, ny, nz, m2, ax, ay, az, bx, by, bz, halfL); break;
+                        case 6: sym_mixed_box_steps<NP, 6>(set, lane, src_lane, nx, ny, nz, m2, ax, ay, az, bx, by, bz, halfL); break;
+                        default: sym_mixed_box_steps<NP, 7>(set, lane, src_lane, nx, ny, nz, m2, ax, ay, az, bx, by, bz, halfL); break;
+                    }
+                    float lo, hi;
+                    const int j = j0 + lane;
+                    unpack2(bx, lo, hi); Bsm[j] += (double)lo + (double)hi;
+                    unpack2(by, lo, hi); Bsm[IB + j] += (double)lo + (double)hi;
+                    unpack2(bz, lo, hi); Bsm[2 * IB + j] += (double)lo + (double)hi;
+                    if ((t & 3) == 3) {
+#pragma unroll
+                        for (int p = 0; p < NP; ++p) {
+                            unpack2(ax[p], lo, hi); Asm[(0 * RI + 2 * p) * THREADS] += (double)lo; Asm[(0 * RI + 2 * p + 1) * THREADS] += (double)hi;
+                            unpack2(ay[p], lo, hi); Asm[(1 * RI + 2 * p) * THREADS] += (double)lo; Asm[(1 * RI + 2 * p + 1) * THREADS] += (double)hi;
+                            unpack2(az[p], lo, hi); Asm[(2 * RI + 2 * p) * THREADS] += (double)lo; Asm[(2 * RI + 2 * p + 1) * THREADS] += (double)hi;
+                            ax[p] = ay[p] = az[p] = 0ull;
+                        }
+                    }
+                }
+            }
+            __syncthreads();
+        }
+
+        const long long rec = (kk0 + it - k_begin) * 3 * IB;
+#pragma unroll
+        for (int k = 0; k < RI; ++k) {
+            const int i = warp * WI + lane + 32 * k;
+#pragma unroll
+            for (int cc = 0; cc < 3; ++cc) rowrec[rec + cc * IB + i] = Asm[(cc * RI + k) * THREADS];
+        }
+        for (int j = threadIdx.x; j < IB; j += THREADS) {
+            const double cj = (double)cs[(j / TJ) * (4 * TJ) + 3 * TJ + ((j % TJ) ^ STEPS_C_SWIZZLE)];
+            const double f = -cj * cj;
+            colrec[rec + j] = f * Bsm[j]; colrec[rec + IB + j] = f * Bsm[IB + j]; colrec[rec + 2 * IB + j] = f * Bsm[2 * IB + j];
+        }
+        __syncthreads();
+        if (threadIdx.x == 0 && it + 2 < total) produce(it + 2);
+        if ((kk0 + it + 1) % split == 0 && ++c == nb) { ++b; c = b + 1; }
+    }
+}
+
 // acc (double-double, SoA over all N particles) += the records of one panel, in fixed order; `last` writes acc_out = hi + lo.
 __global__ void __launch_bounds__(256)
 forces_sym_reduce_kernel(const SymPlan* __restrict__ plan, const double* __restrict__ rowrec, const double* __restrict__ colrec,

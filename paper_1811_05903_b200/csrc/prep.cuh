@@ -96,4 +96,45 @@ __global__ void __launch_bounds__(TJ) prep_tiles(const double* __restrict__ pos,
     }
 }
 
+// Bounding box and largest softening of every group of 128 consecutive particles (GroupMeta, common.cuh); one warp per
+// group, `ngroups` >= ceil(N / 128) (the groups beyond N are written empty).  Runs after prep_tiles: a tile that prep
+// marked hmax = +inf (a massless or unscalable particle) passes the mark on to its two groups.
+template <typename Tile>
+__global__ void __launch_bounds__(128) group_meta_kernel(const double* __restrict__ pos, const double* __restrict__ soft, long long N,
+                                                         const Tile* __restrict__ tiles, GroupMeta* __restrict__ gm, int ngroups)
+{
+    const int g = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (g >= ngroups) return;
+    const float inf = __int_as_float(0x7f800000);
+    float lo[3] = {inf, inf, inf}, hi[3] = {-inf, -inf, -inf}, hh = 0.0f;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const long long i = (long long)g * 128 + lane + 32 * k;
+        if (i < N) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const double v = pos[c * N + i];
+                lo[c] = fminf(lo[c], __double2float_rd(v)); hi[c] = fmaxf(hi[c], __double2float_ru(v));
+            }
+            hh = fmaxf(hh, __double2float_ru(soft[i]));
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            lo[c] = fminf(lo[c], __shfl_xor_sync(0xffffffffu, lo[c], o)); hi[c] = fmaxf(hi[c], __shfl_xor_sync(0xffffffffu, hi[c], o));
+        }
+        hh = fmaxf(hh, __shfl_xor_sync(0xffffffffu, hh, o));
+    }
+    if (lane == 0) {
+        if ((long long)g * 128 < N) hh = fmaxf(hh, tiles[g / 2].meta.hmax >= inf ? inf : 0.0f);
+        GroupMeta m;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { m.lo[c] = lo[c]; m.hi[c] = hi[c]; }
+        m.hmax = hh; m.pad = 0.0f;
+        gm[g] = m;
+    }
+}
+
 }  // namespace steps

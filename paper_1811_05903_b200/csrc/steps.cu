@@ -64,6 +64,7 @@ struct Workspace {
     double* partials = nullptr;     // (nb + grid) * 6 * IB doubles (persistent driver's split-j records)
     long long cap_particles = 0;
     SymPlan* plan = nullptr;        // SymPlan + cum[nb + 1]
+    GroupMeta* gm = nullptr;        // one per 128 particles, padded to whole blocks (periodic pair-symmetric evaluation)
     double* acc_dd = nullptr;       // 6 N doubles: (hi, lo) of the band result, the symmetric records are added to it
     double* sym_records = nullptr;  // 2 * panel_items * 3 * IB doubles (row records, then column records)
     long long sym_cap_particles = 0, sym_panel_items = 0;
@@ -156,13 +157,14 @@ int ensure_workspace(int dev, long long N, cudaStream_t st)
     }
     if (need_tiles || need_sym) STEPS_CUDA(cudaDeviceSynchronize());      // nothing in flight may still use the old scratch
     if (need_tiles) {
-        cudaFree(w.tiles); cudaFree(w.partials); cudaFree(w.plan);
-        w.tiles = nullptr; w.partials = nullptr; w.plan = nullptr; w.cap_particles = 0;
+        cudaFree(w.tiles); cudaFree(w.partials); cudaFree(w.plan); cudaFree(w.gm);
+        w.tiles = nullptr; w.partials = nullptr; w.plan = nullptr; w.gm = nullptr; w.cap_particles = 0;
         if (cudaMalloc(&w.tiles, tile_bytes_max() * (size_t)ntiles_padded(N)) != cudaSuccess ||
             cudaMalloc(&w.partials, partial_bytes(N)) != cudaSuccess ||
-            cudaMalloc(&w.plan, sizeof(SymPlan) + sizeof(long long) * (size_t)(nblocks_of(N) + 1)) != cudaSuccess) {
+            cudaMalloc(&w.plan, sizeof(SymPlan) + sizeof(long long) * (size_t)(nblocks_of(N) + 1)) != cudaSuccess ||
+            cudaMalloc(&w.gm, sizeof(GroupMeta) * (size_t)nblocks_of(N) * (IB / SPLITJ_GROUP)) != cudaSuccess) {
             cudaGetLastError();
-            cudaFree(w.tiles); cudaFree(w.partials); w.tiles = nullptr; w.partials = nullptr;
+            cudaFree(w.tiles); cudaFree(w.partials); cudaFree(w.plan); w.tiles = nullptr; w.partials = nullptr; w.plan = nullptr;
             return STEPS_ENOMEM;
         }
         w.cap_particles = nblocks_of(N) * IB;
@@ -407,6 +409,113 @@ int forces_impl(const double* pos, const double* mass, const double* soft, long 
     return release_scratch(w, st);
 }
 
+// Leading-image periodic box (steps_forces_quasi_periodic).  One 128-particle group per CTA column (forces_boxring_kernel);
+// from 16 (fp64) / 64 (mixed) blocks the far pairs of DIFFERENT blocks go through the pair-symmetric kernels
+// (forces_sym_box_kernel / forces_sym_mixed_box_kernel), each evaluated once, and the group-ring kernel runs in restricted
+// mode (the groups' own blocks + the units that may hold a softened pair).  All decisions that depend on the data are taken
+// on the device (pair_decision on the group boxes; the plan falls back to "everything one-sided" when the items are too few).
+template <typename Path>
+int launch_forces_box(const double* pos, const double* mass, const double* soft, long long N, double L, double* acc_out,
+                      cudaStream_t st, Workspace& w)
+{
+    using Tile = typename Path::Tile;
+    constexpr bool FP64 = Path::NOUT == 6;
+    const int nb = (int)nblocks_of(N);
+    const int nt = (int)ntiles_of(N);
+    Tile* tiles = reinterpret_cast<Tile*>(w.tiles);
+    const bool sym = g_driver.load() == 0 && sym_eligible(N, !FP64) && w.sym_records && (FP64 || g_sym_enabled.load() != 2);
+    const long long groups = (N + SPLITJ_GROUP - 1) / SPLITJ_GROUP;
+    // with fewer groups than SMs the tile range is split over floor(SMs / groups) CTAs so that the grid is one wave
+    long long jsplit = groups < w.num_sms ? w.num_sms / groups : 1;
+    jsplit = std::max(1ll, std::min<long long>(jsplit, nt));
+    const long long rec_cap = (long long)(partial_bytes(N) / (sizeof(double) * 6 * SPLITJ_GROUP));
+    if (groups * jsplit > rec_cap) jsplit = std::max(1ll, rec_cap / groups);
+    if (groups > 0x7fffffffll || jsplit > 65535) return STEPS_EINVAL;
+    auto ring = forces_boxring_kernel<Path>;
+    constexpr int smem = boxring_smem_bytes<Path>();
+    static bool attr_set = false;                                              // per instantiation
+    if (!attr_set) { STEPS_CUDA(cudaFuncSetAttribute(ring, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); attr_set = true; }
+    const bool prof = g_profile.load() != 0;
+    if (prof && !w.ev0) { STEPS_CUDA(cudaEventCreate(&w.ev0)); STEPS_CUDA(cudaEventCreate(&w.ev1)); }
+    const dim3 grid((unsigned)groups, (unsigned)jsplit);
+
+    if (!sym) {
+        prep_tiles<Tile><<<nt, TJ, 0, st>>>(pos, mass, soft, N, tiles, nullptr);
+        if (prof) STEPS_CUDA(cudaEventRecord(w.ev0, st));
+        ring<<<grid, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, acc_out, w.partials, 0, L, 1.0 / L, nullptr, nullptr, nullptr);
+        g_launches += 2;
+        if (jsplit > 1) {
+            forces_splitj_reduce<<<(unsigned)groups, SPLITJ_GROUP, 0, st>>>(w.partials, (int)jsplit, N, acc_out, NO_FUSE);
+            g_launches++;
+        }
+        if (prof) { STEPS_CUDA(cudaEventRecord(w.ev1, st)); w.ev_valid = true; }
+        STEPS_CUDA(cudaGetLastError());
+        return STEPS_OK;
+    }
+
+    const int ntp = nb * TPB, ngm = nb * (IB / SPLITJ_GROUP);
+    int Ps = 0;
+    int split = 1;
+    if constexpr (FP64) {
+        static int grid_box = 0, unused = 0;
+        int rc = persistent_grid(forces_sym_box_kernel<SYM_FP64_THREADS, SYM_FP64_RI, false>, sym_box_smem_bytes(), w, grid_box, SYM_FP64_THREADS);
+        if (rc == STEPS_OK && unused == 0)
+            rc = persistent_grid(forces_sym_box_kernel<SYM_FP64_THREADS, SYM_FP64_RI, true>, sym_box_smem_bytes(), w, unused, SYM_FP64_THREADS);
+        if (rc != STEPS_OK) return rc;
+        Ps = std::min(grid_box, w.num_sms);
+        while (split < SYM_FP64_THREADS / 32 && sym_items_max(N) * split < 24ll * Ps) split *= 2;
+    } else {
+        static int grid_box = 0;
+        const int rc = persistent_grid(forces_sym_mixed_box_kernel<SYM_MIXED_THREADS, SYM_MIXED_RI, false>,
+                                       sym_mixed_box_smem_bytes<SYM_MIXED_THREADS, SYM_MIXED_RI>(), w, grid_box, SYM_MIXED_THREADS);
+        if (rc != STEPS_OK) return rc;
+        Ps = std::min(grid_box, w.num_sms);
+    }
+    prep_tiles<Tile><<<ntp, TJ, 0, st>>>(pos, mass, soft, N, tiles, &w.plan->W);          // W = 0: every block pair is an item
+    group_meta_kernel<Tile><<<(ngm + 3) / 4, 128, 0, st>>>(pos, soft, N, tiles, w.gm, ngm);
+    sym_plan_finalize<<<1, 1024, 0, st>>>(w.plan, nb, 8 * Ps, split);
+    if (prof) STEPS_CUDA(cudaEventRecord(w.ev0, st));
+    double* hi = w.acc_dd;
+    double* lo = w.acc_dd + 3 * N;
+    // one-sided part: the possibly-softened units of other blocks (zero if the plan kept no items), then the groups' own
+    // blocks (everything if the plan kept no items) added to it; groups >= SMs here, so the tile range is never split
+    auto gen = forces_boxgen_kernel<Path>;
+    static bool gen_attr_set = false;
+    if (!gen_attr_set) { STEPS_CUDA(cudaFuncSetAttribute(gen, cudaFuncAttributeMaxDynamicSharedMemorySize, boxgen_smem_bytes<Path>())); gen_attr_set = true; }
+    // (the unit range of a group is split over up to 8 CTAs, see forces_boxgen_kernel; their records use the symmetric
+    // kernels' record buffer, which is free until the first panel)
+    long long gsplit = 8;
+    while (gsplit > 1 && (size_t)groups * gsplit * 6 * SPLITJ_GROUP * sizeof(double) > sym_record_bytes(w.sym_panel_items)) gsplit /= 2;
+    gen<<<dim3((unsigned)groups, (unsigned)gsplit), CTA_THREADS, boxgen_smem_bytes<Path>(), st>>>(pos, soft, N, tiles, nt, hi, lo, w.sym_records,
+                                                                                                   L, 1.0 / L, w.gm, w.plan);
+    if (gsplit > 1) {
+        forces_splitj_reduce<<<(unsigned)groups, SPLITJ_GROUP, 0, st>>>(w.sym_records, (int)gsplit, N, hi, NO_FUSE, lo);
+        g_launches++;
+    }
+    ring<<<(unsigned)groups, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, hi, w.partials, 0, L, 1.0 / L, w.gm, w.plan, lo);
+    g_launches += 5;
+    const long long items = w.sym_panel_items, kmax = sym_items_max(N) * split;          // in sub-items
+    double* rowrec = w.sym_records;
+    double* colrec = w.sym_records + (size_t)items * 3 * IB;
+    for (long long k0 = 0; k0 < kmax; k0 += items) {
+        const long long k1 = std::min(kmax, k0 + items);
+        if constexpr (FP64) {
+            auto k = split == 1 ? forces_sym_box_kernel<SYM_FP64_THREADS, SYM_FP64_RI, false> : forces_sym_box_kernel<SYM_FP64_THREADS, SYM_FP64_RI, true>;
+            k<<<Ps, SYM_FP64_THREADS, sym_box_smem_bytes(), st>>>(tiles, w.plan, w.gm, k0, k1, rowrec, colrec, 0, split, L, 1.0 / L);
+        } else {
+            forces_sym_mixed_box_kernel<SYM_MIXED_THREADS, SYM_MIXED_RI, false>
+                <<<Ps, SYM_MIXED_THREADS, sym_mixed_box_smem_bytes<SYM_MIXED_THREADS, SYM_MIXED_RI>(), st>>>(tiles, w.plan, w.gm, k0, k1, rowrec,
+                                                                                                               colrec, split, L, 1.0 / L);
+        }
+        forces_sym_reduce_kernel<<<(int)((N + 255) / 256), 256, 0, st>>>(w.plan, rowrec, colrec, k0, k1, N, hi, lo,
+                                                                          k1 == kmax ? 1 : 0, acc_out, split, NO_FUSE);
+        g_launches += 2;
+    }
+    if (prof) { STEPS_CUDA(cudaEventRecord(w.ev1, st)); w.ev_valid = true; }
+    STEPS_CUDA(cudaGetLastError());
+    return STEPS_OK;
+}
+
 template <typename Path, int BOX>
 int launch_forces_periodic(const double* pos, const double* mass, const double* soft, long long N, double L, double* acc_out,
                            cudaStream_t st, Workspace& w, int& grid_cache)
@@ -416,27 +525,13 @@ int launch_forces_periodic(const double* pos, const double* mass, const double* 
     Tile* tiles = reinterpret_cast<Tile*>(w.tiles);
     int rc = claim_scratch(w, st);
     if (rc != STEPS_OK) return rc;
-    prep_tiles<Tile><<<nt, TJ, 0, st>>>(pos, mass, soft, N, tiles, nullptr);
-    g_launches++;
-    if constexpr (BOX == 1) {                      // leading image: one 128-particle group per CTA column (forces_boxring_kernel)
-        const long long groups = (N + SPLITJ_GROUP - 1) / SPLITJ_GROUP;
-        // with fewer groups than SMs the tile range is split over floor(SMs / groups) CTAs so that the grid is one wave
-        long long jsplit = groups < w.num_sms ? w.num_sms / groups : 1;
-        jsplit = std::max(1ll, std::min<long long>(jsplit, nt));
-        const long long rec_cap = (long long)(partial_bytes(N) / (sizeof(double) * 6 * SPLITJ_GROUP));
-        if (groups * jsplit > rec_cap) jsplit = std::max(1ll, rec_cap / groups);
-        if (groups > 0x7fffffffll || jsplit > 65535) return STEPS_EINVAL;
-        auto kern = forces_boxring_kernel<Path>;
-        constexpr int smem = boxring_smem_bytes<Path>();
-        static bool attr_set = false;                                              // per instantiation
-        if (!attr_set) { STEPS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); attr_set = true; }
-        kern<<<dim3((unsigned)groups, (unsigned)jsplit), CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, acc_out, w.partials, 0, L, 1.0 / L);
+    if constexpr (BOX != 1) {
+        prep_tiles<Tile><<<nt, TJ, 0, st>>>(pos, mass, soft, N, tiles, nullptr);
         g_launches++;
-        if (jsplit > 1) {
-            forces_splitj_reduce<<<(unsigned)groups, SPLITJ_GROUP, 0, st>>>(w.partials, (int)jsplit, N, acc_out, NO_FUSE);
-            g_launches++;
-        }
-        STEPS_CUDA(cudaGetLastError());
+    }
+    if constexpr (BOX == 1) {
+        rc = launch_forces_box<Path>(pos, mass, soft, N, L, acc_out, st, w);
+        if (rc != STEPS_OK) return rc;
         return release_scratch(w, st);
     } else {
     const int nb = (int)nblocks_of(N);
@@ -854,7 +949,7 @@ void steps_shutdown(void)
         if (!w.tiles && !w.mom_partial && !w.h_pos) continue;
         cudaSetDevice(d);
         cudaDeviceSynchronize();
-        cudaFree(w.tiles); cudaFree(w.partials); cudaFree(w.plan); cudaFree(w.acc_dd); cudaFree(w.sym_records);
+        cudaFree(w.tiles); cudaFree(w.partials); cudaFree(w.plan); cudaFree(w.gm); cudaFree(w.acc_dd); cudaFree(w.sym_records);
         cudaFree(w.mom_partial); cudaFree(w.sort_buf);
         cudaFree(w.h_pos); cudaFree(w.h_mass); cudaFree(w.h_soft); cudaFree(w.h_acc);
         if (w.ev0) { cudaEventDestroy(w.ev0); cudaEventDestroy(w.ev1); }
@@ -868,7 +963,8 @@ long long steps_workspace_bytes(long long N)
 {
     if (N < 1) return 0;
     size_t bytes = tile_bytes_max() * (size_t)ntiles_padded(N) + partial_bytes(N) + sizeof(double) * MOM_BLOCKS * 4 +
-                   sizeof(SymPlan) + sizeof(long long) * (size_t)(nblocks_of(N) + 1);
+                   sizeof(SymPlan) + sizeof(long long) * (size_t)(nblocks_of(N) + 1) +
+                   sizeof(GroupMeta) * (size_t)nblocks_of(N) * (IB / SPLITJ_GROUP);
     if (sym_eligible(N)) bytes += sizeof(double) * 6 * (size_t)N + sym_record_bytes(sym_panel_items_for(N));
     return (long long)bytes;
 }

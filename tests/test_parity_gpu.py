@@ -536,7 +536,7 @@ def _periodic_box(n, L, seed):
 @pytest.mark.gpu
 @pytest.mark.parametrize("mixed", [False, True], ids=["fp64", "mixed"])
 @pytest.mark.parametrize("n,ordered", [(2, False), (257, False), (5000, False), (32768, False), (5000, True), (32768, True),
-                                       (100003, True)])
+                                       (100003, True), (150001, True), (262144, True)])
 def test_quasi_periodic_forces_match_oracle(S, oracle, mixed, n, ordered):
     """ordered: Morton (cell) order -- tile pairs share one image shift and most take the periodic far bodies (uniform
     shift / per-pair conditional wrap); unordered input goes through the general wrapped body for every tile."""
