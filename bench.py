@@ -170,26 +170,27 @@ def bench_next_rows(S, synth, torch, stream, reps: int = 3):
         return pos, mass, soft, torch.empty_like(pos)
 
     rows = {}
-    n = 262144
-    pos, mass, soft, acc = box(n, 9001)
-    for mixed in (False, True):
-        ms = timed(lambda: S.steps_forces_quasi_periodic(pos, mass, soft, 1.0, acc, mixed=mixed))
-        rate = n * (n - 1.0) / (ms * 1e-3)
-        peak = PEAK_FP32_TFLOPS if mixed else PEAK_FP64_TFLOPS
-        rows["quasi_periodic_" + ("mixed" if mixed else "fp64")] = {
-            "value": rate, "unit": UNIT, "ms": ms, "N": n, "workload": "uniform periodic box in Morton order, leading image (Eq. 5)",
-            "roofline": {"bound": "alu", "achieved": FLOP_PER_INTERACTION * rate / 1e12, "peak": peak, "unit": "TFLOP/s",
-                         "frac": FLOP_PER_INTERACTION * rate / 1e12 / peak}}
-    n = 32768
-    pos, mass, soft, acc = box(n, 9002)
-    ms = timed(lambda: S.steps_forces_periodic(pos, mass, soft, 1.0, acc))
+    for n, tag in ((262144, ""), (1048576, "_1M")):
+        pos, mass, soft, acc = box(n, 9001)
+        for mixed in (False, True):
+            ms = timed(lambda: S.steps_forces_quasi_periodic(pos, mass, soft, 1.0, acc, mixed=mixed))
+            rate = n * (n - 1.0) / (ms * 1e-3)
+            peak = PEAK_FP32_TFLOPS if mixed else PEAK_FP64_TFLOPS
+            rows["quasi_periodic_" + ("mixed" if mixed else "fp64") + tag] = {
+                "value": rate, "unit": UNIT, "ms": ms, "N": n, "workload": "uniform periodic box in Morton order, leading image (Eq. 5)",
+                "roofline": {"bound": "alu", "achieved": FLOP_PER_INTERACTION * rate / 1e12, "peak": peak, "unit": "TFLOP/s",
+                             "frac": FLOP_PER_INTERACTION * rate / 1e12 / peak}}
+        del pos, mass, soft, acc
     images = 4.0 / 3.0 * math.pi * 2.6 ** 3                        # mean number of images inside the 2.6 L cut per pair
-    rate = n * (n - 1.0) / (ms * 1e-3)
-    rows["periodic_images"] = {
-        "value": rate, "unit": "pairs/s (each summed over its images inside |x - nL| < 2.6 L)", "ms": ms, "N": n,
-        "images_per_pair_in_cut": images, "image_terms_per_s": rate * images,
-        "roofline": {"bound": "alu", "achieved": FLOP_PER_INTERACTION * rate * images / 1e12, "peak": PEAK_FP64_TFLOPS,
-                     "unit": "TFLOP/s", "frac": FLOP_PER_INTERACTION * rate * images / 1e12 / PEAK_FP64_TFLOPS}}
+    for n, tag in ((32768, ""), (131072, "_131072")):
+        pos, mass, soft, acc = box(n, 9002)
+        ms = timed(lambda: S.steps_forces_periodic(pos, mass, soft, 1.0, acc))
+        rate = n * (n - 1.0) / (ms * 1e-3)
+        rows["periodic_images" + tag] = {
+            "value": rate, "unit": "pairs/s (each summed over its images inside |x - nL| < 2.6 L)", "ms": ms, "N": n,
+            "images_per_pair_in_cut": images, "image_terms_per_s": rate * images,
+            "roofline": {"bound": "alu", "achieved": FLOP_PER_INTERACTION * rate * images / 1e12, "peak": PEAK_FP64_TFLOPS,
+                         "unit": "TFLOP/s", "frac": FLOP_PER_INTERACTION * rate * images / 1e12 / PEAK_FP64_TFLOPS}}
     # device-resident adaptive step (Eq. 12 + KDK + force evaluation), config 0 size and 32,768
     for n in (4096, 32768):
         ps = synth.g0(n, synth.SEED_BASE)

@@ -189,10 +189,14 @@ int steps_momentum(const double *vec, const double *mass, long long N, double *o
  * acc overwritten.  Positions need not lie inside [0, L): the fp64 path wraps separations, valid for |x_j - x_i| < 2^51 L;
  * the mixed path casts positions to fp32 first, so it keeps its accuracy only for positions within a few L of the box
  * (|x| / L < 2^22 is the hard limit of its wrap).  Fast path: CELL-ORDERED input (e.g. Morton order of a grid, see
- * synth.morton_order) -- the periodic counterpart of the radial order: a (128-particle group, tile) pair whose bounding
- * boxes are compact shares one image shift per component and runs the open-boundary far body; unordered input goes through
- * the general wrapped body with the per-pair softening test for every tile -- slower, never wrong.  The image sum of Eq. 5
- * with the 2.6 L cut is steps_forces_periodic below.  STEPS_EINVAL additionally for L <= 0. */
+ * synth.morton_order) -- the periodic counterpart of the radial order: groups of consecutive particles whose bounding
+ * boxes are compact and cannot hold a softened pair share one image decision -- a lattice shift per component, plus a
+ * FOLD (d' = e - copysign(L/2, e), one addition and one bit operation) of the components whose separations straddle half
+ * the box -- and run the open-boundary far body; from N = 30,721 (fp64) / 129,025 (mixed) such pairs of groups of two
+ * different blocks of 2,048 particles are evaluated ONCE and applied to both groups (Newton III, as steps_forces does).
+ * Unordered input, or particles given many periods apart, go through the general wrapped body with the per-pair softening
+ * test -- slower, never wrong.  Ties (a separation component of exactly L/2, measure zero) may pick either image.  The
+ * image sum of Eq. 5 with the 2.6 L cut is steps_forces_periodic below.  STEPS_EINVAL additionally for L <= 0. */
 int steps_forces_quasi_periodic(const double *pos, const double *mass, const double *soft, long long N,
                                 double L, double *acc, int mixed, steps_stream_t stream);
 
@@ -200,8 +204,10 @@ int steps_forces_quasi_periodic(const double *pos, const double *mass, const dou
  * images x - nL of every separation with the paper's cut |x - nL| < 2.6 L (strict), each image through the pair law with
  * pair softening soft_i + soft_j; fp64 path only (the images of a homogeneous box cancel to a small remainder).  Layout,
  * G = 1 and error behaviour as steps_forces_quasi_periodic; the result does not depend on which representative modulo L
- * the positions are given in (|x_j - x_i| < 2^51 L).  Cost: 179 candidate images per pair (74 of them inside the cut on
- * average).  A particle's OWN images (j = i, n != 0) are summed like any other pair's: the triplet set is symmetric under
+ * the positions are given in (|x_j - x_i| < 2^51 L).  Cost: 74 images per pair inside the cut on average; a pair on its
+ * own needs 179 candidates (all n.n <= 12 around its leading image), a (128-particle group, tile) pair of cell-ordered
+ * input whose bounding boxes are compact and cannot hold a softened pair is pruned to the ~90-110 candidates that come
+ * within the cut for some pair of the two boxes.  A particle's OWN images (j = i, n != 0) are summed like any other pair's: the triplet set is symmetric under
  * n -> -n, so they cancel to rounding (the oracle skips j = i altogether).  Softening up to h_i + h_j <= L/2 takes the
  * fast route (only the nearest image can then be softened); larger softening is handled image by image. */
 int steps_forces_periodic(const double *pos, const double *mass, const double *soft, long long N, double L,

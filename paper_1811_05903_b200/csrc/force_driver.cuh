@@ -186,11 +186,10 @@ __device__ __forceinline__ int band_row_of(const long long* __restrict__ cum, in
 
 // ---- persistent stream-K driver ------------------------------------------------------------------
 // partials: [nb + gridDim.x slots][Path::NOUT][IB] doubles; CTA p's record for i-block b is slot b + p.
-// BOX = 2 (periodic boundaries, Eq. 5): every tile goes through the image sum in a cubic
-// box of side box_L -- the radial far/near classification of the compactified sets does not apply in a periodic box.
-// (The leading-image box, BOX = 1, has its own driver: forces_boxring_kernel below.)
+// (Periodic boxes, have their own driver: forces_boxring_kernel below.  BOX stays a parameter of the
+// launchers; here it is always 0.)
 // BAND (open boundary only): the iteration space is the band of `plan` instead of all nb x nt (i-block, tile) pairs.
-template <typename Path, int STAGES, int BOX = 0, bool BAND = false>   // BOX: 0 open boundary, 2 image sum with the 2.6 L cut
+template <typename Path, int STAGES, int BOX = 0, bool BAND = false>
 __global__ void __launch_bounds__(CTA_THREADS, 1)
 forces_persistent_kernel(const double* __restrict__ pos, const double* __restrict__ soft, long long N,
                          const typename Path::Tile* __restrict__ tiles, int nt, long long i_begin, long long i_end,
@@ -200,20 +199,12 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
     // block_stride > 1 (multi-GPU dealing, steps_forces_blocks): local i-block b is the global block
     // i_begin / IB + b * block_stride; i_end is then N.
     static_assert(!BAND || BOX == 0, "the band split applies to the open boundary only");
-    static_assert(BOX != 1, "the leading-image box runs on forces_boxring_kernel");
+    static_assert(BOX == 0, "periodic boxes run on forces_boxring_kernel");
     using Tile = typename Path::Tile;
     constexpr int STRIDE = stage_stride((int)sizeof(Tile));
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ uint64_t full_bar[STAGES], empty_bar[STAGES];
     double* acc = reinterpret_cast<double*>(smem_raw + STAGES * STRIDE) + threadIdx.x;
-    __shared__ double img_tab[BOX == 2 ? 3 * EWALD_NTRIPLETS : 1];     // image offsets n L of Eq. 5 (BOX = 2 only)
-    if constexpr (BOX == 2) {
-        for (int q = threadIdx.x; q < EWALD_NTRIPLETS; q += CTA_THREADS) {
-            img_tab[3 * q] = ewald_triplets[q].x * box_L; img_tab[3 * q + 1] = ewald_triplets[q].y * box_L;
-            img_tab[3 * q + 2] = ewald_triplets[q].z * box_L;
-        }
-    }
-
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const long long* cum = BAND ? plan_cum(plan) : nullptr;
     const int bandW = BAND ? plan->W : 0;
@@ -276,9 +267,7 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
             const int s = it % STAGES;
             mbar_wait(&full_bar[s], (it / STAGES) & 1);
             const Tile& T = *reinterpret_cast<const Tile*>(smem_raw + s * STRIDE);
-            if constexpr (BOX == 2) {
-                Path::near_images(T, S, acc, box_L, box_invL, img_tab);
-            } else {
+            {
             // the decision is warp-uniform by construction (warp-reduced bounds); the vote tells the compiler so
             if (__all_sync(0xffffffffu, tile_is_far(rlo, rhi, hh, T.meta))) {
                 Path::far(T, S, F, zero);
@@ -500,7 +489,7 @@ __global__ void __launch_bounds__(128) forces_splitj_reduce(const double* __rest
     if (fuse.out_bits) eq12_fold(fuse, dt);
 }
 
-// ---- group-ring driver: the leading-image periodic box (Eq. 5) -----------------------
+// ---- group-ring driver: periodic boxes (Eq. 5); BOX = 1 leading image, 2 image sum --------
 // One i-GROUP of 128 particles (4 per lane) per CTA column, held by ALL 16 warps of the CTA.  The warps form BOXRING_G
 // sub-rings of 4 warps; each sub-ring streams every fourth tile of the range through its own bulk-copy ring (its first
 // lane is the producer) and each of its warps takes a quarter (64 sources) of every tile.
@@ -518,22 +507,32 @@ __global__ void __launch_bounds__(128) forces_splitj_reduce(const double* __rest
 // particles belong to the pair-symmetric kernel (forces_sym_box_kernel, force_sym.cuh) and to forces_boxgen_kernel below
 // (the units that may hold a softened pair); this kernel then evaluates the group's own block only and ADDS its result to
 // the double-double (acc_out = hi, acc_lo_out = lo) that forces_boxgen_kernel wrote.
+// BOX = 2: the image sum of Eq. 5 with the 2.6 L cut (fp64) on the same driver.  A far (group, tile) pair -- no image of
+// any of its pairs can be softened -- has its candidate images PRUNED from the two bounding boxes: with the lattice shift
+// that centres the box difference every separation of the pair lies in [a, b] per component, and image n can come
+// within the cut only if the distance from n L to that box is below 2.6 L (about 90-110 of the 343 n in [-3, 3]^3 for
+// compact cells; a pair on its own needs 179).  The ring then carries the tile's PLAIN sources; the other tiles go
+// through Fp64Path::near_images from global memory.  All warps of the CTA hold the same group, so they all have the same
+// candidate list for a tile (each warp builds its own copy) and the same cost: warps holding different groups would wait
+// at every tile for the one whose pair is not far (179 candidates + the softening tests).
 constexpr int BOXRING_G = 4;                               // sub-rings per CTA
-constexpr int BOXRING_STAGES = 3;                          // stages per sub-ring
 constexpr int DEC_CHUNK = 512;                             // decisions per sub-ring kept in shared memory at a time
-template <typename Path>
-__host__ __device__ constexpr int far_part_bytes()         // the scaled sources lead the tile record (common.cuh)
+template <typename Path, int BOX>
+__host__ __device__ constexpr int boxring_stages() { return BOX == 2 ? 2 : 3; }     // stages per sub-ring
+template <typename Path, int BOX>
+__host__ __device__ constexpr int boxring_part_bytes()     // what the ring carries of a tile record (common.cuh)
 {
-    return Path::NOUT == 6 ? TJ * (int)sizeof(FarSrcF64) : 4 * TJ * (int)sizeof(float);
+    // BOX = 1: the scaled sources, which lead the record; BOX = 2: the plain sources x[], y[], z[], m[], h[] that follow them
+    return BOX == 2 ? 5 * TJ * (int)sizeof(double) : (Path::NOUT == 6 ? TJ * (int)sizeof(FarSrcF64) : 4 * TJ * (int)sizeof(float));
 }
-template <typename Path>
+template <typename Path, int BOX>
 constexpr int boxring_smem_bytes()
 {
-    return BOXRING_G * BOXRING_STAGES * far_part_bytes<Path>() + Path::NOUT * R_I * CTA_THREADS * (int)sizeof(double) +
-           BOXRING_G * DEC_CHUNK * (int)sizeof(uint32_t);
+    return BOXRING_G * boxring_stages<Path, BOX>() * boxring_part_bytes<Path, BOX>() +
+           Path::NOUT * R_I * CTA_THREADS * (int)sizeof(double) + BOXRING_G * DEC_CHUNK * (int)sizeof(uint32_t);
 }
 
-template <typename Path>
+template <typename Path, int BOX>
 __global__ void __launch_bounds__(CTA_THREADS, 1)
 forces_boxring_kernel(const double* __restrict__ pos, const double* __restrict__ soft, long long N,
                       const typename Path::Tile* __restrict__ tiles, int nt, double* __restrict__ acc_out,
@@ -545,14 +544,32 @@ forces_boxring_kernel(const double* __restrict__ pos, const double* __restrict__
     using Tile = typename Path::Tile;
     using IState = typename Path::IState;
     using Elem = decltype(IState::x[0] + 0);               // double or float
-    constexpr int G = BOXRING_G, STAGES = BOXRING_STAGES, FAR_BYTES = far_part_bytes<Path>();
+    static_assert(BOX == 1 || (BOX == 2 && Path::NOUT == 6), "leading image (both paths) or image sum (fp64)");
+    constexpr int G = BOXRING_G, STAGES = boxring_stages<Path, BOX>(), FAR_BYTES = boxring_part_bytes<Path, BOX>();
+    constexpr size_t PART_OFFSET = BOX == 2 ? TJ * sizeof(FarSrcF64) : 0;      // of the carried part within the tile record
     constexpr int WARPS = CTA_THREADS / 32, WG = WARPS / G, PER_WARP = TJ / WG;   // 4 warps per sub-ring, 64 sources per warp and tile
     static_assert(WARPS % G == 0 && TJ % WG == 0 && PER_WARP % 4 == 0, "every warp takes whole float4 groups of each tile");
-    static_assert(FAR_BYTES % 128 == 0, "stage alignment");
+    static_assert(FAR_BYTES % 128 == 0 && PART_OFFSET % 16 == 0, "stage alignment");
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ uint64_t full_bar[G][STAGES], empty_bar[G][STAGES];
     __shared__ Elem gs[4 * R_I][32];                        // the group's particles (x, y, z, h), unshifted: read back when a
                                                             // tile needs another image shift or the general body
+    // BOX = 2: image offsets n L of the unpruned route (near_images), of all n in [-3, 3]^3 (pruned route), and per warp the
+    // candidates of its current tile
+    constexpr int NCUBE = 343, CAND_STRIDE = 352;
+    __shared__ double img_tab[BOX == 2 ? 3 * EWALD_NTRIPLETS : 1];
+    __shared__ double cube_tab[BOX == 2 ? 3 * NCUBE : 1];
+    __shared__ unsigned short cand_all[BOX == 2 ? WARPS * CAND_STRIDE : 1];
+    if constexpr (BOX == 2) {
+        for (int q = threadIdx.x; q < EWALD_NTRIPLETS; q += CTA_THREADS) {
+            img_tab[3 * q] = ewald_triplets[q].x * box_L; img_tab[3 * q + 1] = ewald_triplets[q].y * box_L;
+            img_tab[3 * q + 2] = ewald_triplets[q].z * box_L;
+        }
+        for (int q = threadIdx.x; q < NCUBE; q += CTA_THREADS) {
+            cube_tab[3 * q] = (double)(q % 7 - 3) * box_L; cube_tab[3 * q + 1] = (double)((q / 7) % 7 - 3) * box_L;
+            cube_tab[3 * q + 2] = (double)(q / 49 - 3) * box_L;
+        }
+    }
     double* acc_all = reinterpret_cast<double*>(smem_raw + G * STAGES * FAR_BYTES);   // [NOUT * R_I][CTA_THREADS]
     double* acc = acc_all + threadIdx.x;
     uint32_t* codes_all = reinterpret_cast<uint32_t*>(acc_all + Path::NOUT * R_I * CTA_THREADS);
@@ -583,13 +600,15 @@ forces_boxring_kernel(const double* __restrict__ pos, const double* __restrict__
 #pragma unroll
     for (int q = 0; q < Path::NOUT * R_I; ++q) acc[q * CTA_THREADS] = 0.0;
 
-    // tile range of this CTA; sub-ring g takes the tiles t0 + g, t0 + g + G, ... (interleaved: every sub-ring meets the same
-    // mix of decisions, so the four finish together)
-    // (restricted mode: only the tiles of the group's own block; the launcher then uses gridDim.y = 1)
-    const int t0 = restricted ? min(nt, my_block * (IB / TJ)) : (int)((long long)blockIdx.y * nt / gridDim.y);
-    const int t1 = restricted ? min(nt, (my_block + 1) * (IB / TJ)) : (int)(((long long)blockIdx.y + 1) * nt / gridDim.y);
-    const int mine = (t1 - t0 - g + G - 1) / G;              // tiles of this sub-ring
-    const int chunks = ((t1 - t0 + G - 1) / G + DEC_CHUNK - 1) / DEC_CHUNK;   // the same for every sub-ring (CTA-wide barriers)
+    // The tiles of this CTA: first, first + step, ... (`ntiles` of them) -- every gridDim.y-th tile, so that the CTAs that
+    // share a group meet the same mix of decisions; restricted mode: the tiles of the group's own block (gridDim.y = 1).
+    // Sub-ring g takes every G-th of those, for the same reason: the four finish together.
+    const int first = restricted ? min(nt, my_block * (IB / TJ)) : (int)blockIdx.y;
+    const int step = restricted ? 1 : (int)gridDim.y;
+    const int ntiles = restricted ? min(nt, (my_block + 1) * (IB / TJ)) - first : (nt - first + step - 1) / step;
+    auto tile_of = [&](int r, int k) { return first + step * (r + G * k); };      // tile k of sub-ring r
+    const int mine = (ntiles - g + G - 1) / G;               // tiles of this sub-ring
+    const int chunks = ((ntiles + G - 1) / G + DEC_CHUNK - 1) / DEC_CHUNK;    // the same for every sub-ring (CTA-wide barriers)
     if (threadIdx.x == 0) {
 #pragma unroll
         for (int r = 0; r < G; ++r)
@@ -610,8 +629,9 @@ forces_boxring_kernel(const double* __restrict__ pos, const double* __restrict__
         const int k0 = ch * DEC_CHUNK, cnt = max(0, min(DEC_CHUNK, mine - k0));   // this sub-ring's tiles k0 .. k0 + cnt of its list
         __syncthreads();                                    // the previous chunk's decisions are no longer read (and: gs, barrier init)
         for (int q = threadIdx.x; q < G * DEC_CHUNK; q += CTA_THREADS) {       // all threads compute the decisions of all sub-rings
-            const int r = q / DEC_CHUNK, tile = t0 + r + G * (k0 + q % DEC_CHUNK);
-            if (tile < t1) codes_all[q] = boxcode_pack(box_shift(blo, bhi, hh, tiles[tile].meta, box_L, box_invL), box_invL);
+            const int r = q / DEC_CHUNK, k = k0 + q % DEC_CHUNK;
+            if (r + G * k < ntiles)
+                codes_all[q] = boxcode_pack(box_shift(blo, bhi, hh, tiles[tile_of(r, k)].meta, box_L, box_invL), box_invL);
         }
         __syncthreads();
         int pq = 0;                                         // producer cursor within the chunk
@@ -621,7 +641,8 @@ forces_boxring_kernel(const double* __restrict__ pos, const double* __restrict__
             const int s = produced % STAGES;
             if (produced >= STAGES) mbar_wait(&empty_bar[g][s], ((produced / STAGES) - 1) & 1);
             mbar_expect_tx(&full_bar[g][s], (uint32_t)FAR_BYTES);
-            bulk_load(ring + s * FAR_BYTES, tiles + (t0 + g + G * (k0 + pq)), (uint32_t)FAR_BYTES, &full_bar[g][s]);
+            bulk_load(ring + s * FAR_BYTES, reinterpret_cast<const unsigned char*>(tiles + tile_of(g, k0 + pq)) + PART_OFFSET,
+                      (uint32_t)FAR_BYTES, &full_bar[g][s]);
             ++produced; ++pq;
         };
         if (producer)
@@ -629,21 +650,64 @@ forces_boxring_kernel(const double* __restrict__ pos, const double* __restrict__
         for (int q = 0; q < cnt; ++q) {
             const uint32_t code = codes[q];
             if (code & BOXCODE_GENERAL) {
-                if (pending) { Path::fold_flush(F, acc); pending = 0; }
-                Path::template near_box<true>(tiles[t0 + g + G * (k0 + q)], group_state(), acc, box_L, box_invL, j0, j1);
+                if constexpr (BOX == 2) {
+                    Path::near_images(tiles[tile_of(g, k0 + q)], group_state(), acc, box_L, box_invL, img_tab, j0, j1);
+                } else {
+                    if (pending) { Path::fold_flush(F, acc); pending = 0; }
+                    Path::template near_box<true>(tiles[tile_of(g, k0 + q)], group_state(), acc, box_L, box_invL, j0, j1);
+                }
                 continue;
             }
             if (producer) produce_next();
             const int s = consumed % STAGES;
             mbar_wait(&full_bar[g][s], (consumed / STAGES) & 1);
-            const Tile& T = *reinterpret_cast<const Tile*>(ring + s * FAR_BYTES);    // only its far part is there
-            if ((code >> 8) != q_key) {
-                q_key = code >> 8;
-                Q = Path::shifted(group_state(), boxcode_unpack(code, box_L).s);
+            if constexpr (BOX == 2) {
+                // the candidate images of this (group, tile) pair, pruned from the two bounding boxes (see the header comment)
+                const TileMeta meta = tiles[tile_of(g, k0 + q)].meta;
+                double sh[3], a[3], b[3];
+                const double eps = 1.0e-5 * box_L;
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const double dmin = ((double)meta.lo[c] - (double)bhi[c]) - eps, dmax = ((double)meta.hi[c] - (double)blo[c]) + eps;
+                    sh[c] = box_L * rint(0.5 * (dmin + dmax) * box_invL);
+                    a[c] = dmin - sh[c]; b[c] = dmax - sh[c];
+                }
+                unsigned short* cand = cand_all + warp * CAND_STRIDE;
+                const double cut2 = (2.6 * box_L) * (2.6 * box_L);
+                int ncand = 0;
+                for (int q0 = 0; q0 < NCUBE; q0 += 32) {
+                    const int t = q0 + lane;
+                    bool keep = false;
+                    if (t < NCUBE) {
+                        double g2 = 0.0;
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) {
+                            const double o = cube_tab[3 * t + c];
+                            const double gap = fmax(0.0, fmax(a[c] - o, o - b[c]));
+                            g2 = fma(gap, gap, g2);
+                        }
+                        keep = g2 < cut2;
+                    }
+                    const unsigned m = __ballot_sync(0xffffffffu, keep);
+                    if (keep) cand[ncand + __popc(m & ((1u << lane) - 1u))] = (unsigned short)t;
+                    ncand += __popc(m);
+                }
+                __syncwarp();
+                Q = group_state();
+#pragma unroll
+                for (int k = 0; k < R_I; ++k) { Q.x[k] += sh[0]; Q.y[k] += sh[1]; Q.z[k] += sh[2]; }
+                const double* P = reinterpret_cast<const double*>(ring + s * FAR_BYTES);      // x[], y[], z[], m[], h[]
+                Path::far_images(P, P + TJ, P + 2 * TJ, P + 3 * TJ, Q, acc, box_L, cube_tab, cand, ncand, j0, j1);
+            } else {
+                const Tile& T = *reinterpret_cast<const Tile*>(ring + s * FAR_BYTES);    // only its far part is there
+                if ((code >> 8) != q_key) {
+                    q_key = code >> 8;
+                    Q = Path::shifted(group_state(), boxcode_unpack(code, box_L).s);
+                }
+                far_fold_dispatch<Path>(T, Q, F, zero, (int)(code & 7u), 0.5 * box_L, j0, j1);
+                pending += PER_WARP;
+                if (pending >= Path::FAR_SOURCES_PER_FLUSH) { Path::fold_flush(F, acc); pending = 0; }
             }
-            far_fold_dispatch<Path>(T, Q, F, zero, (int)(code & 7u), 0.5 * box_L, j0, j1);
-            pending += PER_WARP;
-            if (pending >= Path::FAR_SOURCES_PER_FLUSH) { Path::fold_flush(F, acc); pending = 0; }
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty_bar[g][s]);
             ++consumed;

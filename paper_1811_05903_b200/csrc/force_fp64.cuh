@@ -282,14 +282,14 @@ struct Fp64Path {
     // the far body, 3 DFMA = 14 FP64-pipe instructions per image -- with the cut applied as an integer compare of the
     // bit patterns (ALU pipe, not FP64) and m_j multiplied once per pair.  Pairs with h_i + h_j > L/2 take the general loop.
     static __device__ __forceinline__ void near_images(const Tile& T, const IState& S, double* acc, double L, double invL,
-                                                       const double* __restrict__ tab)
+                                                       const double* __restrict__ tab, int j0 = 0, int j1 = TJ)
     {
         constexpr double A = 1.4;
         constexpr double C0 = 1.0 / STEPS_FP64_FOLD - (1.0 - A) * (1.0 - A);
         const double cut2 = (2.6 * L) * (2.6 * L), halfL = 0.5 * L;
         const long long cut2_bits = __double_as_longlong(cut2);
 #pragma unroll 1
-        for (int j = 0; j < TJ; ++j) {
+        for (int j = j0; j < j1; ++j) {
             const double xj = T.x[j], yj = T.y[j], zj = T.z[j], mq = T.m[j], hj = T.h[j];
             if (mq == 0.0) continue;                                   // pads and massless sources (warp-uniform)
             // px: sum over the images of s v, in units of 1 / STEPS_FP64_FOLD (the far body's r^-3 carries that factor)
@@ -351,6 +351,71 @@ struct Fp64Path {
             const double mf = STEPS_FP64_FOLD * mq;
 #pragma unroll
             for (int k = 0; k < R_I; ++k) { flush(acc, 0, k, mf * px[k]); flush(acc, 1, k, mf * py[k]); flush(acc, 2, k, mf * pz[k]); }
+        }
+    }
+
+    // The image sum for a (group, tile) pair NO image of which can be softened (the driver's box test), with the candidate
+    // images pruned from the two bounding boxes: `Q` carries the pair's common lattice shift (so every separation
+    // d = x_j - x_i' lies in the box-difference interval the driver pruned against -- no per-pair wrap: the image SET
+    // {d - nL : |d - nL| < 2.6 L} does not depend on the representative, reading #17), `cand[0..ncand)` are the indices
+    // into `tab` (offsets n L, n in [-3, 3]^3) of the images that come within the cut for SOME pair of the two boxes --
+    // about 90 for compact cells instead of the 179 a single pair needs in the worst case.  Every image runs the
+    // branch-free 14-instruction Newtonian body, the cut as an integer compare.
+    // (Tx, Ty, Tz, Tm: the tile's plain sources, e.g. staged in shared memory; [j0, j1): the sources to sum.)
+    // The candidates are walked twice per source, for two of the thread's four particles at a time: with all four in one
+    // pass the live values (separations, sums, temporaries) exceed the register file and ptxas runs the four dependent
+    // 12-instruction chains one after the other (FP64 pipe 66 % active, measured); two at a time they interleave.
+    static __device__ __forceinline__ void far_images(const double* __restrict__ Tx, const double* __restrict__ Ty,
+                                                      const double* __restrict__ Tz, const double* __restrict__ Tm, const IState& Q,
+                                                      double* acc, double L, const double* __restrict__ tab,
+                                                      const unsigned short* __restrict__ cand, int ncand, int j0, int j1)
+    {
+        constexpr double A = 1.4;
+        constexpr double C0 = 1.0 / STEPS_FP64_FOLD - (1.0 - A) * (1.0 - A);
+        constexpr int H = 2;                                           // particles per pass
+        static_assert(R_I % H == 0, "whole passes");
+        const long long cut2_bits = __double_as_longlong((2.6 * L) * (2.6 * L));
+#pragma unroll 1
+        for (int j = j0; j < j1; ++j) {
+            const double xj = Tx[j], yj = Ty[j], zj = Tz[j], mq = Tm[j];
+            if (mq == 0.0) continue;                                   // pads and massless sources (warp-uniform)
+            const double mf = STEPS_FP64_FOLD * mq;
+#pragma unroll
+            for (int k0 = 0; k0 < R_I; k0 += H) {
+                double dx[H], dy[H], dz[H], px[H], py[H], pz[H];
+#pragma unroll
+                for (int k = 0; k < H; ++k) {
+                    dx[k] = xj - Q.x[k0 + k]; dy[k] = yj - Q.y[k0 + k]; dz[k] = zj - Q.z[k0 + k];
+                    px[k] = py[k] = pz[k] = 0.0;
+                }
+#pragma unroll 2
+                for (int c = 0; c < ncand; ++c) {
+                    const int t3 = 3 * cand[c];
+                    const double ox = tab[t3], oy = tab[t3 + 1], oz = tab[t3 + 2];
+                    double vx[H], vy[H], vz[H], r2[H], y0[H], y2[H], w[H];
+#pragma unroll
+                    for (int k = 0; k < H; ++k) { vx[k] = dx[k] - ox; vy[k] = dy[k] - oy; vz[k] = dz[k] - oz; }
+#pragma unroll
+                    for (int k = 0; k < H; ++k) r2[k] = fma(vz[k], vz[k], fma(vy[k], vy[k], vx[k] * vx[k]));
+#pragma unroll
+                    for (int k = 0; k < H; ++k) y0[k] = rsqrt_seed(r2[k]);
+#pragma unroll
+                    for (int k = 0; k < H; ++k) {
+                        y2[k] = y0[k] * y0[k];
+                        w[k] = fma(r2[k], y2[k], -A);
+                        y2[k] = y0[k] * y2[k];
+                        w[k] = fma(w[k], w[k], C0);
+                        w[k] = y2[k] * w[k];
+                        if (!(__double_as_longlong(r2[k]) < cut2_bits)) w[k] = 0.0;   // "|x - nL| < 2.6 L", strict (r2 >= 0)
+                    }
+#pragma unroll
+                    for (int k = 0; k < H; ++k) {
+                        px[k] = fma(vx[k], w[k], px[k]); py[k] = fma(vy[k], w[k], py[k]); pz[k] = fma(vz[k], w[k], pz[k]);
+                    }
+                }
+#pragma unroll
+                for (int k = 0; k < H; ++k) { flush(acc, 0, k0 + k, mf * px[k]); flush(acc, 1, k0 + k, mf * py[k]); flush(acc, 2, k0 + k, mf * pz[k]); }
+            }
         }
     }
 

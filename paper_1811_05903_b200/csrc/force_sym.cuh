@@ -692,12 +692,15 @@ forces_sym_box_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restri
 template <int THREADS, int RI>
 __host__ __device__ constexpr int sym_mixed_box_smem_bytes() { return sym_mixed_smem_bytes<THREADS, RI>() + 3 * IB * (int)sizeof(float); }
 
+#ifndef STEPS_SYMBOX_UNROLL
+#define STEPS_SYMBOX_UNROLL 1
+#endif
 template <int NP, int MASK>
 __device__ __forceinline__ void sym_mixed_box_steps(const float* __restrict__ set, int lane, int src_lane, const u64 (&nx)[NP],
                                                     const u64 (&ny)[NP], const u64 (&nz)[NP], const u64 (&m2)[NP], u64 (&ax)[NP],
                                                     u64 (&ay)[NP], u64 (&az)[NP], u64& bx, u64& by, u64& bz, float halfL)
 {
-#pragma unroll 2
+STEPS_UNROLL(STEPS_SYMBOX_UNROLL)
     for (int st = 0; st < 32; ++st) {
         const int r = (lane - st) & 31;
         const float X = set[r], Y = set[TJ + r], Z = set[2 * TJ + r], C = set[3 * TJ + (r ^ STEPS_C_SWIZZLE)];

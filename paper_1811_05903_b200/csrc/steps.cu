@@ -431,8 +431,8 @@ int launch_forces_box(const double* pos, const double* mass, const double* soft,
     const long long rec_cap = (long long)(partial_bytes(N) / (sizeof(double) * 6 * SPLITJ_GROUP));
     if (groups * jsplit > rec_cap) jsplit = std::max(1ll, rec_cap / groups);
     if (groups > 0x7fffffffll || jsplit > 65535) return STEPS_EINVAL;
-    auto ring = forces_boxring_kernel<Path>;
-    constexpr int smem = boxring_smem_bytes<Path>();
+    auto ring = forces_boxring_kernel<Path, 1>;
+    constexpr int smem = boxring_smem_bytes<Path, 1>();
     static bool attr_set = false;                                              // per instantiation
     if (!attr_set) { STEPS_CUDA(cudaFuncSetAttribute(ring, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); attr_set = true; }
     const bool prof = g_profile.load() != 0;
@@ -534,17 +534,32 @@ int launch_forces_periodic(const double* pos, const double* mass, const double* 
         if (rc != STEPS_OK) return rc;
         return release_scratch(w, st);
     } else {
-    const int nb = (int)nblocks_of(N);
-    constexpr int smem = persistent_smem_bytes<Path, STAGES>();
-    auto kern = forces_persistent_kernel<Path, STAGES, BOX>;
-    rc = persistent_grid(kern, smem, w, grid_cache);
-    if (rc != STEPS_OK) return rc;
-    const int P = grid_cache;
-    kern<<<P, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, 0, N, nb, w.partials, 0, L, 1.0 / L, nullptr, 1);
-    forces_reduce_kernel<Path::NOUT><<<(int)((N + 255) / 256), 256, 0, st>>>(w.partials, nt, nb, P, N, acc_out, NO_FUSE);
-    g_launches += 2;
-    STEPS_CUDA(cudaGetLastError());
-    return release_scratch(w, st);
+        // Image sum: the group-ring driver with BOX = 2.  The tile range is split over `jsplit` CTAs so that the grid is
+        // (close to) whole waves of one CTA per SM -- an image-sum CTA runs for milliseconds, a ragged last wave shows.
+        const long long groups = (N + SPLITJ_GROUP - 1) / SPLITJ_GROUP;
+        long long jsplit = 1;
+        double best = 0.0;
+        for (long long j = 1; j <= 8 && j <= nt; ++j) {
+            const double waves = (double)(groups * j) / w.num_sms;
+            const double eff = waves / std::ceil(waves);
+            if (eff > best + 0.02) { best = eff; jsplit = j; }
+        }
+        const long long rec_cap = (long long)(partial_bytes(N) / (sizeof(double) * 6 * SPLITJ_GROUP));
+        if (groups * jsplit > rec_cap) jsplit = std::max(1ll, rec_cap / groups);
+        if (groups > 0x7fffffffll) return STEPS_EINVAL;
+        auto kern = forces_boxring_kernel<Path, 2>;
+        constexpr int smem = boxring_smem_bytes<Path, 2>();
+        static bool attr_set = false;
+        if (!attr_set) { STEPS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); attr_set = true; }
+        kern<<<dim3((unsigned)groups, (unsigned)jsplit), CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, acc_out, w.partials, 0, L, 1.0 / L,
+                                                                                    nullptr, nullptr, nullptr);
+        g_launches++;
+        if (jsplit > 1) {
+            forces_splitj_reduce<<<(unsigned)groups, SPLITJ_GROUP, 0, st>>>(w.partials, (int)jsplit, N, acc_out, NO_FUSE);
+            g_launches++;
+        }
+        STEPS_CUDA(cudaGetLastError());
+        return release_scratch(w, st);
     }
 }
 
