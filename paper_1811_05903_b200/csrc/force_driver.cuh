@@ -532,6 +532,24 @@ constexpr int boxring_smem_bytes()
            Path::NOUT * R_I * CTA_THREADS * (int)sizeof(double) + BOXRING_G * DEC_CHUNK * (int)sizeof(uint32_t);
 }
 
+// The general body of the group-ring driver as a CALL: it is the rare path (a tile that may hold a softened pair), and
+// inlined next to the far loops it costs them registers -- ptxas then spills the i-particles inside the far loop (measured:
+// 12 local loads per source).  The group's particles come from the shared-memory copy `gs` ([x, y, z, h][R_I][32 lanes]).
+template <typename Path, int BOX>
+__device__ __noinline__ void boxring_general(const typename Path::Tile* __restrict__ T, const void* __restrict__ gs_raw, double* acc,
+                                             double L, double invL, const double* __restrict__ img_tab, int j0, int j1)
+{
+    using IState = typename Path::IState;
+    using Elem = decltype(IState::x[0] + 0);
+    const Elem (*gs)[32] = reinterpret_cast<const Elem (*)[32]>(gs_raw);
+    const int lane = threadIdx.x & 31;
+    IState S;
+#pragma unroll
+    for (int k = 0; k < R_I; ++k) { S.x[k] = gs[k][lane]; S.y[k] = gs[R_I + k][lane]; S.z[k] = gs[2 * R_I + k][lane]; S.h[k] = gs[3 * R_I + k][lane]; }
+    if constexpr (BOX == 2) Path::near_images(*T, S, acc, L, invL, img_tab, j0, j1);
+    else Path::template near_global<BOX == 1>(*T, S, acc, L, invL, j0, j1);
+}
+
 template <typename Path, int BOX>
 __global__ void __launch_bounds__(CTA_THREADS, 1)
 forces_boxring_kernel(const double* __restrict__ pos, const double* __restrict__ soft, long long N,
@@ -579,16 +597,23 @@ forces_boxring_kernel(const double* __restrict__ pos, const double* __restrict__
     const uint32_t* codes = codes_all + g * DEC_CHUNK;
     const bool producer = wg == 0 && lane == 0;
 
-    float blo[3], bhi[3], hh;
+    // the group's bounds (bounding box, largest softening) live in shared memory, not in registers: they
+    // are needed once per chunk (and per tile in the image sum), and the far loops need every register
+    __shared__ float gbox[8];                               // lo[3], hi[3], hmax
     {
         IState S;
-        float rlo, rhi;
+        float blo[3], bhi[3], hh, rlo, rhi;
         const long long i0 = (long long)blockIdx.x * SPLITJ_GROUP + lane;     // the same particles in every warp
         load_i_block<Path>(S, pos, soft, N, i0, N, rlo, rhi, hh);
         warp_box<Path>(S, blo, bhi);
         if (warp == 0) {
 #pragma unroll
             for (int k = 0; k < R_I; ++k) { gs[k][lane] = S.x[k]; gs[R_I + k][lane] = S.y[k]; gs[2 * R_I + k][lane] = S.z[k]; gs[3 * R_I + k][lane] = S.h[k]; }
+            if (lane == 0) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) { gbox[c] = blo[c]; gbox[3 + c] = bhi[c]; }
+                gbox[6] = hh;
+            }
         }
     }
     auto group_state = [&]() {
@@ -628,6 +653,8 @@ forces_boxring_kernel(const double* __restrict__ pos, const double* __restrict__
     for (int ch = 0; ch < chunks; ++ch) {
         const int k0 = ch * DEC_CHUNK, cnt = max(0, min(DEC_CHUNK, mine - k0));   // this sub-ring's tiles k0 .. k0 + cnt of its list
         __syncthreads();                                    // the previous chunk's decisions are no longer read (and: gs, barrier init)
+        const float blo[3] = {gbox[0], gbox[1], gbox[2]}, bhi[3] = {gbox[3], gbox[4], gbox[5]};
+        const float hh = gbox[6];
         for (int q = threadIdx.x; q < G * DEC_CHUNK; q += CTA_THREADS) {       // all threads compute the decisions of all sub-rings
             const int r = q / DEC_CHUNK, k = k0 + q % DEC_CHUNK;
             if (r + G * k < ntiles)
@@ -650,12 +677,8 @@ forces_boxring_kernel(const double* __restrict__ pos, const double* __restrict__
         for (int q = 0; q < cnt; ++q) {
             const uint32_t code = codes[q];
             if (code & BOXCODE_GENERAL) {
-                if constexpr (BOX == 2) {
-                    Path::near_images(tiles[tile_of(g, k0 + q)], group_state(), acc, box_L, box_invL, img_tab, j0, j1);
-                } else {
-                    if (pending) { Path::fold_flush(F, acc); pending = 0; }
-                    Path::template near_box<true>(tiles[tile_of(g, k0 + q)], group_state(), acc, box_L, box_invL, j0, j1);
-                }
+                if constexpr (BOX != 2) { if (pending) { Path::fold_flush(F, acc); pending = 0; } }
+                boxring_general<Path, BOX>(&tiles[tile_of(g, k0 + q)], &gs[0][0], acc, box_L, box_invL, img_tab, j0, j1);
                 continue;
             }
             if (producer) produce_next();
@@ -668,7 +691,7 @@ forces_boxring_kernel(const double* __restrict__ pos, const double* __restrict__
                 const double eps = 1.0e-5 * box_L;
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
-                    const double dmin = ((double)meta.lo[c] - (double)bhi[c]) - eps, dmax = ((double)meta.hi[c] - (double)blo[c]) + eps;
+                    const double dmin = ((double)meta.lo[c] - (double)gbox[3 + c]) - eps, dmax = ((double)meta.hi[c] - (double)gbox[c]) + eps;
                     sh[c] = box_L * rint(0.5 * (dmin + dmax) * box_invL);
                     a[c] = dmin - sh[c]; b[c] = dmax - sh[c];
                 }

@@ -426,6 +426,23 @@ struct Fp64Path {
     {
         near_view<PERIODIC>(T.x, T.y, T.z, T.m, T.h, S, acc, L, invL, j0, j1);
     }
+    // One source against the thread's R_I particles through all three branches of Eq. 4.
+    template <bool PERIODIC>
+    static __device__ __forceinline__ void near_one(double xj, double yj, double zj, double mq, double hj, const IState& S,
+                                                    double (&ax)[R_I], double (&ay)[R_I], double (&az)[R_I], double L, double invL)
+    {
+#pragma unroll
+        for (int k = 0; k < R_I; ++k) {
+            double dx = xj - S.x[k], dy = yj - S.y[k], dz = zj - S.z[k];
+            if (PERIODIC) { dx = wrap(dx, L, invL); dy = wrap(dy, L, invL); dz = wrap(dz, L, invL); }
+            const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+            const double hs = S.h[k] + hj;
+            double s = mq * rcube(r2);
+            if (r2 < hs * hs || r2 == 0.0)                        // Eq. 4 branches 1-2; readings #2, #4
+                s = (r2 == 0.0) ? 0.0 : mq * spline_g_soft_f64(r2, hs);
+            ax[k] = fma(dx, s, ax[k]); ay[k] = fma(dy, s, ay[k]); az[k] = fma(dz, s, az[k]);
+        }
+    }
     // The same on any copy of the plain sources (x, y, z, m, h), e.g. one staged in shared memory.
     template <bool PERIODIC>
     static __device__ __forceinline__ void near_view(const double* __restrict__ Tx, const double* __restrict__ Ty,
@@ -437,19 +454,27 @@ struct Fp64Path {
 #pragma unroll
         for (int k = 0; k < R_I; ++k) ax[k] = ay[k] = az[k] = 0.0;
 #pragma unroll 1
-        for (int j = j0; j < j1; ++j) {
-            const double xj = Tx[j], yj = Ty[j], zj = Tz[j], mq = Tm[j], hj = Th[j];
+        for (int j = j0; j < j1; ++j) near_one<PERIODIC>(Tx[j], Ty[j], Tz[j], Tm[j], Th[j], S, ax, ay, az, L, invL);
 #pragma unroll
-            for (int k = 0; k < R_I; ++k) {
-                double dx = xj - S.x[k], dy = yj - S.y[k], dz = zj - S.z[k];
-                if (PERIODIC) { dx = wrap(dx, L, invL); dy = wrap(dy, L, invL); dz = wrap(dz, L, invL); }
-                const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-                const double hs = S.h[k] + hj;
-                double s = mq * rcube(r2);
-                if (r2 < hs * hs || r2 == 0.0)                        // Eq. 4 branches 1-2; readings #2, #4
-                    s = (r2 == 0.0) ? 0.0 : mq * spline_g_soft_f64(r2, hs);
-                ax[k] = fma(dx, s, ax[k]); ay[k] = fma(dy, s, ay[k]); az[k] = fma(dz, s, az[k]);
-            }
+        for (int k = 0; k < R_I; ++k) { flush(acc, 0, k, ax[k]); flush(acc, 1, k, ay[k]); flush(acc, 2, k, az[k]); }
+    }
+    // The same for a tile record in GLOBAL memory (the group-ring driver's general tiles): a warp-uniform load per source
+    // would pay the L2 latency at every source; instead every lane loads one source of 32 (coalesced) and the warp hands
+    // them round by shuffle.  [j0, j1) must be whole sets of 32.
+    template <bool PERIODIC>
+    static __device__ __forceinline__ void near_global(const Tile& T, const IState& S, double* acc, double L, double invL, int j0, int j1)
+    {
+        const int lane = threadIdx.x & 31;
+        double ax[R_I], ay[R_I], az[R_I];
+#pragma unroll
+        for (int k = 0; k < R_I; ++k) ax[k] = ay[k] = az[k] = 0.0;
+#pragma unroll 1
+        for (int jb = j0; jb < j1; jb += 32) {
+            const double lx = T.x[jb + lane], ly = T.y[jb + lane], lz = T.z[jb + lane], lm = T.m[jb + lane], lh = T.h[jb + lane];
+#pragma unroll 1
+            for (int s = 0; s < 32; ++s)
+                near_one<PERIODIC>(__shfl_sync(0xffffffffu, lx, s), __shfl_sync(0xffffffffu, ly, s), __shfl_sync(0xffffffffu, lz, s),
+                                   __shfl_sync(0xffffffffu, lm, s), __shfl_sync(0xffffffffu, lh, s), S, ax, ay, az, L, invL);
         }
 #pragma unroll
         for (int k = 0; k < R_I; ++k) { flush(acc, 0, k, ax[k]); flush(acc, 1, k, ay[k]); flush(acc, 2, k, az[k]); }

@@ -244,6 +244,34 @@ STEPS_UNROLL(STEPS_FAR_UNROLL)
     {
         near_view<PERIODIC>(T.x, T.y, T.z, T.m, T.h, S, acc, Ld, invLd, j0, j1);
     }
+    // Two sources (packed) against the thread's R_I particles through all three branches of Eq. 4.
+    template <bool PERIODIC>
+    static __device__ __forceinline__ void near_two(u64 xj, u64 yj, u64 zj, u64 mj, u64 hj, const u64 (&xi)[R_I], const u64 (&yi)[R_I],
+                                                    const u64 (&zi)[R_I], const u64 (&hi)[R_I], u64 (&ax)[R_I], u64 (&ay)[R_I],
+                                                    u64 (&az)[R_I], u64 negL, u64 invL)
+    {
+#pragma unroll
+        for (int k = 0; k < R_I; ++k) {
+            u64 dx = sub2(xj, xi[k]), dy = sub2(yj, yi[k]), dz = sub2(zj, zi[k]);
+            if (PERIODIC) { dx = wrap2(dx, negL, invL); dy = wrap2(dy, negL, invL); dz = wrap2(dz, negL, invL); }
+            const u64 r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+            const u64 hs = add2(hj, hi[k]);
+            const u64 hs2 = mul2(hs, hs);
+            float ra, rb, ha, hb;
+            unpack2(r2, ra, rb);
+            unpack2(hs2, ha, hb);
+            const u64 rinv = pack2(rsqrt_approx(ra), rsqrt_approx(rb));
+            u64 s = mul2(mul2(mj, rinv), mul2(rinv, rinv));
+            if (!(ra >= ha && rb >= hb && fminf(ra, rb) > 0.0f)) {   // some half is softened, coincident or NaN
+                float sa, sb, ma, mb, hsa, hsb;
+                unpack2(s, sa, sb); unpack2(mj, ma, mb); unpack2(hs, hsa, hsb);
+                s = pack2(patch(ra, ha, hsa, ma, sa), patch(rb, hb, hsb, mb, sb));
+            }
+            ax[k] = fma2(dx, s, ax[k]);
+            ay[k] = fma2(dy, s, ay[k]);
+            az[k] = fma2(dz, s, az[k]);
+        }
+    }
     // The same on any copy of the plain sources (x, y, z, m, h), e.g. one staged in shared memory (8-byte aligned, j0 even).
     template <bool PERIODIC>
     static __device__ __forceinline__ void near_view(const float* __restrict__ Tx, const float* __restrict__ Ty,
@@ -260,31 +288,42 @@ STEPS_UNROLL(STEPS_FAR_UNROLL)
             ax[k] = ay[k] = az[k] = 0ull;
         }
 #pragma unroll 2
-        for (int j = j0; j < j1; j += 2) {
-            const u64 xj = *reinterpret_cast<const u64*>(&Tx[j]), yj = *reinterpret_cast<const u64*>(&Ty[j]);
-            const u64 zj = *reinterpret_cast<const u64*>(&Tz[j]), mj = *reinterpret_cast<const u64*>(&Tm[j]);
-            const u64 hj = *reinterpret_cast<const u64*>(&Th[j]);
+        for (int j = j0; j < j1; j += 2)
+            near_two<PERIODIC>(*reinterpret_cast<const u64*>(&Tx[j]), *reinterpret_cast<const u64*>(&Ty[j]), *reinterpret_cast<const u64*>(&Tz[j]),
+                               *reinterpret_cast<const u64*>(&Tm[j]), *reinterpret_cast<const u64*>(&Th[j]), xi, yi, zi, hi, ax, ay, az, negL, invL);
 #pragma unroll
-            for (int k = 0; k < R_I; ++k) {
-                u64 dx = sub2(xj, xi[k]), dy = sub2(yj, yi[k]), dz = sub2(zj, zi[k]);
-                if (PERIODIC) { dx = wrap2(dx, negL, invL); dy = wrap2(dy, negL, invL); dz = wrap2(dz, negL, invL); }
-                const u64 r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
-                const u64 hs = add2(hj, hi[k]);
-                const u64 hs2 = mul2(hs, hs);
-                float ra, rb, ha, hb;
-                unpack2(r2, ra, rb);
-                unpack2(hs2, ha, hb);
-                const u64 rinv = pack2(rsqrt_approx(ra), rsqrt_approx(rb));
-                u64 s = mul2(mul2(mj, rinv), mul2(rinv, rinv));
-                if (!(ra >= ha && rb >= hb && fminf(ra, rb) > 0.0f)) {   // some half is softened, coincident or NaN
-                    float sa, sb, ma, mb, hsa, hsb;
-                    unpack2(s, sa, sb); unpack2(mj, ma, mb); unpack2(hs, hsa, hsb);
-                    s = pack2(patch(ra, ha, hsa, ma, sa), patch(rb, hb, hsb, mb, sb));
-                }
-                ax[k] = fma2(dx, s, ax[k]);
-                ay[k] = fma2(dy, s, ay[k]);
-                az[k] = fma2(dz, s, az[k]);
-            }
+        for (int k = 0; k < R_I; ++k) {
+            float lo, hi2;
+            unpack2(ax[k], lo, hi2); flush(acc, 0, k, lo + hi2);
+            unpack2(ay[k], lo, hi2); flush(acc, 1, k, lo + hi2);
+            unpack2(az[k], lo, hi2); flush(acc, 2, k, lo + hi2);
+        }
+    }
+    // The same for a tile record in GLOBAL memory (the group-ring driver's general tiles): every lane loads one packed pair of
+    // sources out of 64 (coalesced) and the warp hands them round by shuffle, instead of a warp-uniform load -- and the L2
+    // latency -- per pair.  [j0, j1) must be whole sets of 64.
+    template <bool PERIODIC>
+    static __device__ __forceinline__ void near_global(const Tile& T, const IState& S, double* acc, double Ld, double invLd, int j0, int j1)
+    {
+        const int lane = threadIdx.x & 31;
+        const u64 negL = pack2(-(float)Ld, -(float)Ld), invL = pack2((float)invLd, (float)invLd);
+        u64 xi[R_I], yi[R_I], zi[R_I], hi[R_I], ax[R_I], ay[R_I], az[R_I];
+#pragma unroll
+        for (int k = 0; k < R_I; ++k) {
+            xi[k] = pack2(S.x[k], S.x[k]); yi[k] = pack2(S.y[k], S.y[k]); zi[k] = pack2(S.z[k], S.z[k]);
+            hi[k] = pack2(S.h[k], S.h[k]);
+            ax[k] = ay[k] = az[k] = 0ull;
+        }
+#pragma unroll 1
+        for (int jb = j0; jb < j1; jb += 64) {
+            const int j = jb + 2 * lane;
+            const u64 lx = *reinterpret_cast<const u64*>(&T.x[j]), ly = *reinterpret_cast<const u64*>(&T.y[j]);
+            const u64 lz = *reinterpret_cast<const u64*>(&T.z[j]), lm = *reinterpret_cast<const u64*>(&T.m[j]);
+            const u64 lh = *reinterpret_cast<const u64*>(&T.h[j]);
+#pragma unroll 1
+            for (int s = 0; s < 32; ++s)
+                near_two<PERIODIC>(__shfl_sync(0xffffffffu, lx, s), __shfl_sync(0xffffffffu, ly, s), __shfl_sync(0xffffffffu, lz, s),
+                                   __shfl_sync(0xffffffffu, lm, s), __shfl_sync(0xffffffffu, lh, s), xi, yi, zi, hi, ax, ay, az, negL, invL);
         }
 #pragma unroll
         for (int k = 0; k < R_I; ++k) {

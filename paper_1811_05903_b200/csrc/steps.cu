@@ -294,6 +294,28 @@ int launch_forces_sym(const double* pos, const double* mass, const double* soft,
     return STEPS_OK;
 }
 
+// The group-ring driver has one CTA per (group, part of the tile range) and one resident CTA per SM: with fewer groups than
+// SMs the tile range is split so that the grid is one wave; otherwise over 1...8 parts, whichever makes the grid closest
+// to whole waves (a CTA runs for a long time -- milliseconds in the image sum -- and a ragged last wave shows).
+long long boxring_jsplit(long long groups, long long nt, long long N, const Workspace& w)
+{
+    long long jsplit = 1;
+    if (groups < w.num_sms) {
+        jsplit = w.num_sms / groups;
+    } else {
+        double best = 0.0;
+        for (long long j = 1; j <= 8; ++j) {
+            const double waves = (double)(groups * j) / w.num_sms;
+            const double eff = waves / std::ceil(waves);
+            if (eff > best + 0.02) { best = eff; jsplit = j; }
+        }
+    }
+    jsplit = std::max(1ll, std::min(jsplit, nt / BOXRING_G));                 // at least one tile per sub-ring
+    const long long rec_cap = (long long)(partial_bytes(N) / (sizeof(double) * 6 * SPLITJ_GROUP));
+    if (groups * jsplit > rec_cap) jsplit = std::max(1ll, rec_cap / groups);
+    return jsplit;
+}
+
 // Split-j driver (force_driver.cuh): one 128-particle group per CTA column, the j-range split over the warps and over
 // `jsplit` CTAs.  The source sub-range per work unit shrinks (256 -> 64) until there are about two units per resident warp.
 template <typename Path, int BOX>
@@ -425,11 +447,7 @@ int launch_forces_box(const double* pos, const double* mass, const double* soft,
     Tile* tiles = reinterpret_cast<Tile*>(w.tiles);
     const bool sym = g_driver.load() == 0 && sym_eligible(N, !FP64) && w.sym_records && (FP64 || g_sym_enabled.load() != 2);
     const long long groups = (N + SPLITJ_GROUP - 1) / SPLITJ_GROUP;
-    // with fewer groups than SMs the tile range is split over floor(SMs / groups) CTAs so that the grid is one wave
-    long long jsplit = groups < w.num_sms ? w.num_sms / groups : 1;
-    jsplit = std::max(1ll, std::min<long long>(jsplit, nt));
-    const long long rec_cap = (long long)(partial_bytes(N) / (sizeof(double) * 6 * SPLITJ_GROUP));
-    if (groups * jsplit > rec_cap) jsplit = std::max(1ll, rec_cap / groups);
+    const long long jsplit = boxring_jsplit(groups, nt, N, w);
     if (groups > 0x7fffffffll || jsplit > 65535) return STEPS_EINVAL;
     auto ring = forces_boxring_kernel<Path, 1>;
     constexpr int smem = boxring_smem_bytes<Path, 1>();
@@ -537,15 +555,7 @@ int launch_forces_periodic(const double* pos, const double* mass, const double* 
         // Image sum: the group-ring driver with BOX = 2.  The tile range is split over `jsplit` CTAs so that the grid is
         // (close to) whole waves of one CTA per SM -- an image-sum CTA runs for milliseconds, a ragged last wave shows.
         const long long groups = (N + SPLITJ_GROUP - 1) / SPLITJ_GROUP;
-        long long jsplit = 1;
-        double best = 0.0;
-        for (long long j = 1; j <= 8 && j <= nt; ++j) {
-            const double waves = (double)(groups * j) / w.num_sms;
-            const double eff = waves / std::ceil(waves);
-            if (eff > best + 0.02) { best = eff; jsplit = j; }
-        }
-        const long long rec_cap = (long long)(partial_bytes(N) / (sizeof(double) * 6 * SPLITJ_GROUP));
-        if (groups * jsplit > rec_cap) jsplit = std::max(1ll, rec_cap / groups);
+        const long long jsplit = boxring_jsplit(groups, nt, N, w);
         if (groups > 0x7fffffffll) return STEPS_EINVAL;
         auto kern = forces_boxring_kernel<Path, 2>;
         constexpr int smem = boxring_smem_bytes<Path, 2>();
