@@ -408,7 +408,7 @@ forces_splitj_kernel(const double* __restrict__ pos, const double* __restrict__ 
         const TileMeta meta = T.meta;
         {
             if (__all_sync(0xffffffffu, tile_is_far(rlo, rhi, hh, meta))) {
-                Path::far(T, S, F, zero, j0, j1);
+                Path::template far<true>(T, S, F, zero, j0, j1);
                 if (++pending >= Path::FAR_TILES_PER_FLUSH) { Path::far_flush(F, acc); pending = 0; }
             } else {
                 if (pending) { Path::far_flush(F, acc); pending = 0; }

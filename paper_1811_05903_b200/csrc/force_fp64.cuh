@@ -155,15 +155,26 @@ struct Fp64Path {
     static __device__ __forceinline__ void fold_flush(FarSums& F, double* acc) { far_flush(F, acc); }   // far_fold() sums into F like far()
 
     // [j0, j1): the sources of the tile to sum (the whole tile in the ring driver; a part of it in the split-j driver).
+    // PREFETCH (tile record in GLOBAL memory, split-j driver): the next source is loaded one pass ahead, so that its L2
+    // latency is behind the arithmetic of this pass (in shared memory the load is cheap and the registers are worth more).
+    template <bool PREFETCH = false>
     static __device__ __forceinline__ void far(const Tile& T, const IState& S, FarSums& F, int zero, int j0 = 0, int j1 = TJ)
     {
         constexpr double A = 1.4;
         constexpr double C0 = 1.0 / STEPS_FP64_FOLD - (1.0 - A) * (1.0 - A);   // (u - A)^2 + C0 = 1/1.875 at u = 1
         double (&ax)[R_I] = F.ax, (&ay)[R_I] = F.ay, (&az)[R_I] = F.az;
+        double2 nXY, nZC;
+        if (PREFETCH) { nXY = *reinterpret_cast<const double2*>(&T.far[j0].X); nZC = *reinterpret_cast<const double2*>(&T.far[j0].Z); }
 #pragma unroll 1
         for (int j = j0; j < j1; ++j) {
-            const double2 XY = *reinterpret_cast<const double2*>(&T.far[j].X);
-            const double2 ZC = *reinterpret_cast<const double2*>(&T.far[j].Z);
+            double2 XY, ZC;
+            if (PREFETCH) {
+                XY = nXY; ZC = nZC;
+                const int jn = min(j + 1, j1 - 1);
+                nXY = *reinterpret_cast<const double2*>(&T.far[jn].X); nZC = *reinterpret_cast<const double2*>(&T.far[jn].Z);
+            } else {
+                XY = *reinterpret_cast<const double2*>(&T.far[j].X); ZC = *reinterpret_cast<const double2*>(&T.far[j].Z);
+            }
             const double X = XY.x, Y = XY.y, Z = ZC.x, C = ZC.y;
             double dX[R_I], dY[R_I], dZ[R_I], r2[R_I], y0[R_I], y2[R_I], w[R_I];
             STEPS_STAGE_FENCE(zero, 0);

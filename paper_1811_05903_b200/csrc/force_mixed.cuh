@@ -101,6 +101,7 @@ struct MixedPath {
     }
 
     // [j0, j1): the sources of the tile to sum (multiples of 4; the whole tile in the ring driver).
+    template <bool PREFETCH = false>          // (the fp64 path's option; here the four-source loads already overlap)
     static __device__ __forceinline__ void far(const Tile& T, const IState& S, FarSums& F, int /*zero*/, int j0 = 0, int j1 = TJ)
     {
         double* acc = F.acc;

@@ -331,6 +331,16 @@ int launch_splitj(const double* pos, const double* soft, long long N, const type
     // one CTA per SM is resident (512 threads, up to 96 KiB of accumulators): with fewer groups than SMs the j-range is split
     // over floor(SMs / groups) CTAs so that the whole grid is ONE wave; with more groups than SMs there is nothing to split
     long long jsplit = groups < w.num_sms ? w.num_sms / groups : 1;
+    // ... or over up to 8 CTAs in several waves, when that fills the SMs better and leaves each CTA >= 2^24 pairs (~20 us)
+    {
+        const double one = (double)(groups * jsplit) / w.num_sms;
+        double best = one / std::ceil(one);
+        for (long long j = jsplit + 1; j <= 8; ++j) {
+            if ((double)SPLITJ_GROUP * (double)N / (double)j < 16777216.0) break;
+            const double waves = (double)(groups * j) / w.num_sms, eff = waves / std::ceil(waves);
+            if (eff > best + 0.05) { best = eff; jsplit = j; }
+        }
+    }
     jsplit = std::max(1ll, std::min(jsplit, units / (CTA_THREADS / 32)));
     const long long rec_cap = (long long)(partial_bytes(N) / (sizeof(double) * 6 * SPLITJ_GROUP));
     if (groups * jsplit > rec_cap) jsplit = std::max(1ll, rec_cap / groups);
