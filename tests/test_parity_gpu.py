@@ -291,7 +291,7 @@ def test_radial_sort_permute_and_near_fraction(S, oracle):
     check(a_so.cpu().numpy(), ref[:, p], False, "sorted by the library")
 
 
-@pytest.mark.parametrize("n", [1, 257, 2049, 5000, 20001])
+@pytest.mark.parametrize("n", [1, 257, 2049, 5000, 20001, 40001, 140001])
 def test_outputs_stay_inside_their_buffers(S, n):
     """compute-sanitizer is closed on this pool (profiles/r02_sanitizer.md), so out-of-bounds writes are looked for with
     guard regions: every output buffer sits between two sentinel-filled pads that must come back untouched, for every
@@ -606,6 +606,43 @@ def _pair_force_abs_sum(pos, mass, soft, L, idx=None):
         r2[r2 == 0] = np.inf
         out[i0:i0 + 256] = np.sum(mass[None, :] / np.maximum(r2, (2 * soft[0]) ** 2), axis=1)
     return out
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("mixed,n", [(False, 40001), (False, 150001), (True, 150001)], ids=["fp64-40001", "fp64-150001", "mixed-150001"])
+def test_quasi_periodic_pair_symmetric_route(S, mixed, n):
+    """From 16 (fp64) / 64 (mixed) blocks the far meetings of two different blocks are evaluated once and applied to both
+    groups (forces_sym_box_kernel), the possibly-softened units by forces_boxgen_kernel, the own blocks by the group-ring
+    kernel.  Every pair must be evaluated by exactly one of them: the result equals the one-sided evaluation (option
+    "sym" = 0: group-ring kernel alone) to rounding, is bit-identical run to run, and obeys Newton's third law."""
+    import torch
+    L = 1.3
+    pos, mass, soft = _periodic_box(n, L, 7700 + n)
+    rng = np.random.default_rng(n)
+    mass = mass * rng.uniform(0.5, 2.0, size=n)                 # unequal masses: a swapped m_i / m_j would show
+    mass /= mass.sum()
+    soft = soft * rng.uniform(0.5, 3.0, size=n)                 # some groups with larger softening: more general units
+    pos = np.ascontiguousarray(pos[:, synth.morton_order(pos, L)])
+    dpos, dm, dh = dev(pos), dev(mass), dev(soft)
+    a_sym, a_again, a_one = (torch.empty(3, n, dtype=torch.float64, device="cuda") for _ in range(3))
+    assert S.steps_pair_symmetric(n, mixed) == 1
+    S.steps_forces_quasi_periodic(dpos, dm, dh, L, a_sym, mixed=mixed)
+    S.steps_forces_quasi_periodic(dpos, dm, dh, L, a_again, mixed=mixed)
+    assert torch.equal(a_sym, a_again)
+    try:
+        S.steps_set_option("sym", 0)
+        S.steps_forces_quasi_periodic(dpos, dm, dh, L, a_one, mixed=mixed)
+    finally:
+        S.steps_set_option("sym", 1)
+    idx = synth.stratified_sample(n, 1024)
+    fsum = _pair_force_abs_sum(pos, mass, np.full(n, soft.min()), L, idx)
+    d = np.linalg.norm((a_sym - a_one).cpu().numpy()[:, idx], axis=0) / fsum
+    print(f"[quasi-periodic sym vs one-sided n={n} {'mixed' if mixed else 'fp64'}] relative to sum_j|f_ij|: rms "
+          f"{math.sqrt(np.mean(d ** 2)):.3e} max {d.max():.3e}")
+    assert d.max() <= (2e-5 if mixed else 1e-13)
+    dmass = torch.from_numpy(mass).cuda()
+    p = (dmass * a_sym).sum(dim=1)
+    assert float(p.norm()) < (1e-7 if mixed else 1e-13) * float((dmass * a_sym.norm(dim=0)).sum())
 
 
 @pytest.mark.gpu
