@@ -247,7 +247,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-next-rows", action="store_true", help="skip the periodic / adaptive-step rows (SURVEY 8(f))")
     ap.add_argument("--sharded-step", action="store_true",
-                    help="time the N > 1 step (shard.ShardedStep: steps_forces_blocks + exchange) even with one rank")
+                    help="time the N > 1 step (shard.WorkSharedStep / shard.ShardedStep: share of the work + exchange) even with one rank")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -293,7 +293,7 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    results, launches_total = {}, 0
+    results, launches_total, plans = {}, 0, {}
     sampler = ClockSampler(local_rank)
     with sampler:
         for path in paths:
@@ -307,6 +307,16 @@ def main():
                 def step():
                     S.steps_kdk_step(x, v, acc, mass, soft, co)
                     S.steps_momentum(v, mass, mom)
+            elif S.steps_pair_symmetric(n, mixed):
+                # N > 1: the force evaluation shared by WORK (steps_forces_share: each rank an equal part of the band visits
+                # and of the pair-symmetric items, at the single-GPU kernels' rate), one all-reduce of the partial
+                # accelerations per step, every rank advances all particles
+                sh = shard.WorkSharedStep(S, rank, world, x, torch.zeros_like(x), mass, soft, mixed)
+                sh.forces()
+
+                def step():
+                    sh.step(co)
+                    S.steps_momentum(sh.v, sh.m, mom)
             else:
                 sh = shard.ShardedStep(S, rank, world, x, torch.zeros_like(x), mass, soft, mixed)
                 sh.forces()
@@ -337,11 +347,15 @@ def main():
             total_ms = float(t_ms.item())
             k_ms = sum(kernel_ms) / len(kernel_ms)
             peak = PEAK_FP32_TFLOPS if mixed else PEAK_FP64_TFLOPS
-            kern_inter = float(cnt) * (n - 1.0)                 # this rank's launch
-            achieved = FLOP_PER_INTERACTION * kern_inter / (k_ms * 1e-3) / 1e12
             sharded = world > 1 or args.sharded_step
-            traffic, traffic_source = ncu_traffic(path, n) if not sharded else (None, "sharded step (one-sided kernel)")
-            symmetric = not sharded and S.steps_pair_symmetric(n, mixed)
+            symmetric = bool(S.steps_pair_symmetric(n, mixed))
+            # this rank's launches: its blocks against all sources (one-sided plan) or 1 / world of the pair evaluations
+            kern_inter = inter_step / world if (sharded and symmetric) else float(cnt) * (n - 1.0)
+            achieved = FLOP_PER_INTERACTION * kern_inter / (k_ms * 1e-3) / 1e12
+            traffic, traffic_source = ncu_traffic(path, n) if not sharded else (None, "sharded step")
+            plans[path] = ("none" if not sharded else
+                           f"pair evaluations shared equally among {world} ranks (steps_forces_share), all-reduce of 3N partial accelerations" if symmetric
+                           else f"i-blocks of 2048 dealt round-robin to {world} ranks (PAPER L135-139, SURVEY 8(e)), all-gather of positions")
             results[path] = {
                 "value": args.steps * inter_step / (total_ms * 1e-3), "unit": UNIT,
                 "ms_per_step": total_ms / args.steps, "force_kernel_ms": k_ms, "gpu_launches": int(launches),
@@ -399,7 +413,7 @@ def main():
         "config": {"workload": f"config3: compactified g0 set (S^3 stereographic, m~(1+r^2/4R^2)^3, eps_i=0.01(m_i/m_min)^(1/3)), N={n}, "
                                f"one steps_kdk_step (kick+drift+prep+force+reduce) + momentum per step",
                    "headline_path": head, "l2": "256 MiB flush write between timed steps (inputs 42 MB fit L2; ALU-bound)",
-                   "i_sharding": "none" if world == 1 and not args.sharded_step else f"i-blocks of 2048 dealt round-robin to {world} ranks (PAPER L135-139, SURVEY 8(e)), all-gather of positions",
+                   "i_sharding": plans[head],
                    "persistent_grid": {p: S.steps_persistent_grid(p == "mixed") for p in results}},
         "roofline": r["roofline"], "paths": results, "clocks": clocks, "gpu_launches": int(launches_total),
         "e2e": e2e, "cpu_baseline": cpu, "next_rows": next_rows, "build": S.build_info(),

@@ -108,6 +108,19 @@ int steps_forces_range(const double *pos, const double *mass, const double *soft
 int steps_forces_blocks(const double *pos, const double *mass, const double *soft, long long N,
                         long long first_block, long long block_stride, double *acc_out, int mixed,
                         steps_stream_t stream);
+
+/* The force evaluation shared among `world` ranks by WORK instead of by particles (PAPER.md L135-139 partitions the force
+ * vectors; L131 counts the work as N(N-1)/2 pair evaluations -- this call partitions those): acc_part (3N doubles, SoA over
+ * ALL particles) receives the contribution of the rank-th of `world` equal parts of the pair evaluations of steps_forces /
+ * steps_forces_mixed -- of the band's tile visits and of the pair-symmetric block-pair items, each applied to both of its
+ * blocks -- so that the SUM over the ranks of acc_part is the full result to rounding (each part is rounded to fp64 once).
+ * Every rank holds all particles; the one exchange per step is a sum-reduction of 3N doubles (NCCL all-reduce, 25 MB at
+ * N = 1M) instead of the all-gather of positions, and every rank then advances ALL particles (O(N), bit-identical on every
+ * rank).  Each rank runs the pair-symmetric kernels at their single-GPU rate (steps_forces_blocks is one-sided).  Below the
+ * pair-symmetric size (N < 30,721 fp64 / 129,025 mixed: under a millisecond of work) rank 0 evaluates everything and the
+ * other ranks return zeros.  STEPS_EINVAL for rank outside [0, world). */
+int steps_forces_share(const double *pos, const double *mass, const double *soft, long long N, int rank,
+                       int world, double *acc_part, int mixed, steps_stream_t stream);
 int steps_block_size(void);
 
 /* End-to-end convenience with HOST buffers (pageable or pinned): copies pos/mass/soft to

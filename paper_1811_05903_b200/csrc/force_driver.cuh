@@ -194,8 +194,10 @@ __global__ void __launch_bounds__(CTA_THREADS, 1)
 forces_persistent_kernel(const double* __restrict__ pos, const double* __restrict__ soft, long long N,
                          const typename Path::Tile* __restrict__ tiles, int nt, long long i_begin, long long i_end,
                          int nb, double* __restrict__ partials, int zero, double box_L, double box_invL,
-                         const SymPlan* __restrict__ plan, int block_stride)
+                         const SymPlan* __restrict__ plan, int block_stride, int share_rank = 0, int share_world = 1)
 {
+    // BAND mode, share_world > 1 (steps_forces_share): only the share_rank-th of share_world equal parts of the band's
+    // (i-block, tile) visits; forces_band_reduce_kernel gets the same two numbers.
     // block_stride > 1 (multi-GPU dealing, steps_forces_blocks): local i-block b is the global block
     // i_begin / IB + b * block_stride; i_end is then N.
     static_assert(!BAND || BOX == 0, "the band split applies to the open boundary only");
@@ -208,9 +210,11 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const long long* cum = BAND ? plan_cum(plan) : nullptr;
     const int bandW = BAND ? plan->W : 0;
-    const long long W = BAND ? plan->T : (long long)nb * nt;
-    const long long w0 = (long long)blockIdx.x * W / gridDim.x;
-    const long long w1 = ((long long)blockIdx.x + 1) * W / gridDim.x;
+    const long long Wall = BAND ? plan->T : (long long)nb * nt;
+    const long long R0 = BAND ? Wall * share_rank / share_world : 0, R1 = BAND ? Wall * (share_rank + 1) / share_world : Wall;
+    const long long W = R1 - R0;
+    const long long w0 = R0 + (long long)blockIdx.x * W / gridDim.x;
+    const long long w1 = R0 + ((long long)blockIdx.x + 1) * W / gridDim.x;
     const int total = (int)(w1 - w0);                       // tiles this CTA streams
     if (total <= 0) return;
 
@@ -335,15 +339,19 @@ __global__ void __launch_bounds__(256) forces_reduce_kernel(const double* __rest
 template <int NOUT>
 __global__ void __launch_bounds__(256) forces_band_reduce_kernel(const double* __restrict__ partials, const SymPlan* __restrict__ plan,
                                                                  int P, long long cnt, double* __restrict__ acc_out,
-                                                                 int to_dd, double* __restrict__ acc_hi, double* __restrict__ acc_lo)
+                                                                 int to_dd, double* __restrict__ acc_hi, double* __restrict__ acc_lo,
+                                                                 int share_rank = 0, int share_world = 1)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= cnt) return;
     const long long* cum = plan_cum(plan);
-    const long long W = plan->T;
+    // the share [R0, R1) of the band's visits that the kernel ran; CTA p owns the local visits [floor(p W / P), floor((p+1) W / P))
+    const long long R0 = plan->T * share_rank / share_world, R1 = plan->T * (share_rank + 1) / share_world;
+    const long long W = R1 - R0;
     const int b = (int)(i / IB), off = (int)(i - (long long)b * IB);
-    const int p_lo = (int)(((cum[b] + 1) * P - 1) / W);
-    const int p_hi = (int)((cum[b + 1] * P - 1) / W);
+    const long long v0 = max(cum[b], R0) - R0, v1 = min(cum[b + 1], R1) - R0;      // this block's visits inside the share
+    const int p_lo = v0 < v1 ? (int)(((v0 + 1) * P - 1) / W) : 1;
+    const int p_hi = v0 < v1 ? (int)((v1 * P - 1) / W) : 0;
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         double hi = 0.0, lo = 0.0;

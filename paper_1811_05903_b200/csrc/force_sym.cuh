@@ -129,7 +129,8 @@ constexpr int SYM_FP64_RI = IB / SYM_FP64_THREADS;
 template <int THREADS, int RI, bool SPLIT>
 __global__ void __launch_bounds__(THREADS, 1)
 forces_sym_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__ plan, long long k_begin, long long k_end,
-                  double* __restrict__ rowrec, double* __restrict__ colrec, int zero, int split_arg)
+                  double* __restrict__ rowrec, double* __restrict__ colrec, int zero, int split_arg, int share_rank = 0,
+                  int share_world = 1)
 {
     const int split = SPLIT ? split_arg : 1;
     static_assert(THREADS * RI == IB, "the CTA holds one block");
@@ -142,7 +143,9 @@ forces_sym_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__
 
     // `split` parts per item (the SUBG rounds of an item shared among `split` consecutive sub-items, so that a mid-size N
     // still has enough work units for 148 SMs); [k_begin, k_end), the records and the grid's shares are in SUB-items
-    const long long K = plan->K * split;
+    // share_world > 1 (steps_forces_share): [k_begin, k_end) counts from the start of this rank's share of the sub-items
+    const long long Kall = plan->K * split, S0 = Kall * share_rank / share_world, K = Kall * (share_rank + 1) / share_world;
+    k_begin += S0; k_end += S0;
     if (k_end > K) k_end = K;
     if (k_begin >= k_end) return;
     const int W = plan->W, nb = plan->nb, Km = plan->Km;
@@ -317,7 +320,7 @@ constexpr int SYM_MIXED_RI = IB / SYM_MIXED_THREADS;
 template <int THREADS, int RI, bool SPLIT>
 __global__ void __launch_bounds__(THREADS, 1)
 forces_sym_mixed_kernel(const TileF32* __restrict__ tiles, const SymPlan* __restrict__ plan, long long k_begin, long long k_end,
-                        double* __restrict__ rowrec, double* __restrict__ colrec, int split_arg)
+                        double* __restrict__ rowrec, double* __restrict__ colrec, int split_arg, int share_rank = 0, int share_world = 1)
 {
     const int split = SPLIT ? split_arg : 1;
     static_assert(THREADS * RI == IB && RI % 2 == 0, "the CTA holds one block, particles packed in pairs");
@@ -333,7 +336,9 @@ forces_sym_mixed_kernel(const TileF32* __restrict__ tiles, const SymPlan* __rest
 
     // `split` parts per item (the SUBG rounds of an item shared among `split` consecutive sub-items, so that a mid-size N
     // still has enough work units for 148 SMs); [k_begin, k_end), the records and the grid's shares are in SUB-items
-    const long long K = plan->K * split;
+    // share_world > 1 (steps_forces_share): [k_begin, k_end) counts from the start of this rank's share of the sub-items
+    const long long Kall = plan->K * split, S0 = Kall * share_rank / share_world, K = Kall * (share_rank + 1) / share_world;
+    k_begin += S0; k_end += S0;
     if (k_end > K) k_end = K;
     if (k_begin >= k_end) return;
     const int W = plan->W, nb = plan->nb, Km = plan->Km;
@@ -890,12 +895,15 @@ forces_sym_mixed_box_kernel(const TileF32* __restrict__ tiles, const SymPlan* __
 __global__ void __launch_bounds__(256)
 forces_sym_reduce_kernel(const SymPlan* __restrict__ plan, const double* __restrict__ rowrec, const double* __restrict__ colrec,
                          long long k_begin, long long k_end, long long N, double* __restrict__ acc_hi,
-                         double* __restrict__ acc_lo, int last, double* __restrict__ acc_out, int split, Eq12Fuse fuse)
+                         double* __restrict__ acc_lo, int last, double* __restrict__ acc_out, int split, Eq12Fuse fuse,
+                         int share_rank = 0, int share_world = 1)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     double dt = __longlong_as_double((long long)STEPS_DT_INF_BITS);
     if (i < N) {
-    const long long K = plan->K * split;               // sub-items (see forces_sym_kernel)
+    const long long Kall = plan->K * split;            // sub-items (see forces_sym_kernel); the rank's share of them
+    const long long S0 = Kall * share_rank / share_world, K = Kall * (share_rank + 1) / share_world;
+    k_begin += S0; k_end += S0;
     if (k_end > K) k_end = K;
     const int W = plan->W, Km = plan->Km;
     const int b = (int)(i / IB), off = (int)(i - (long long)b * IB);

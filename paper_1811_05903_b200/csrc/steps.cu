@@ -225,8 +225,11 @@ int persistent_grid(Kernel kern, int smem, const Workspace& w, int& grid_cache, 
 // through the symmetric kernel, panel by panel; all decisions that depend on the data (W) are taken on the device.
 template <typename Path>
 int launch_forces_sym(const double* pos, const double* mass, const double* soft, long long N, double* acc_out,
-                      cudaStream_t st, Workspace& w)
+                      cudaStream_t st, Workspace& w, int share_rank = 0, int share_world = 1)
 {
+    // share_world > 1 (steps_forces_share): the share_rank-th of share_world equal parts of the WORK -- of the band's tile
+    // visits and of the symmetric (sub-)items, both counted on the device -- with acc_out = this part's contribution to
+    // every particle's acceleration.
     using Tile = typename Path::Tile;
     constexpr bool FP64 = Path::NOUT == 6;
     const int nb = (int)nblocks_of(N);
@@ -267,26 +270,30 @@ int launch_forces_sym(const double* pos, const double* mass, const double* soft,
     sym_band_width<Tile><<<nb, 128, 0, st>>>(tiles, nb, w.plan);
     sym_plan_finalize<<<1, 1024, 0, st>>>(w.plan, nb, 8 * Ps, split);
     if (prof) STEPS_CUDA(cudaEventRecord(w.ev0, st));
-    band<<<P, CTA_THREADS, smem_band, st>>>(pos, soft, N, tiles, ntp, 0, N, nb, w.partials, 0, 0.0, 0.0, w.plan, 1);
+    band<<<P, CTA_THREADS, smem_band, st>>>(pos, soft, N, tiles, ntp, 0, N, nb, w.partials, 0, 0.0, 0.0, w.plan, 1, share_rank, share_world);
     double* hi = w.acc_dd;
     double* lo = w.acc_dd + 3 * N;
-    forces_band_reduce_kernel<Path::NOUT><<<(int)((N + 255) / 256), 256, 0, st>>>(w.partials, w.plan, P, N, acc_out, 1, hi, lo);
+    forces_band_reduce_kernel<Path::NOUT><<<(int)((N + 255) / 256), 256, 0, st>>>(w.partials, w.plan, P, N, acc_out, 1, hi, lo, share_rank,
+                                                                                   share_world);
     g_launches += 5;
-    const long long items = w.sym_panel_items, kmax = sym_items_max(N) * split;          // in sub-items
+    // in sub-items; a share has at most ceil(all / share_world) of them (the kernels clamp to the share's actual end)
+    const long long items = w.sym_panel_items, kmax = (sym_items_max(N) * split + share_world - 1) / share_world;
     double* rowrec = w.sym_records;
     double* colrec = w.sym_records + (size_t)items * 3 * IB;
     for (long long k0 = 0; k0 < kmax; k0 += items) {
         const long long k1 = std::min(kmax, k0 + items);
         if constexpr (FP64) {
             auto k = split == 1 ? forces_sym_kernel<SYM_FP64_THREADS, SYM_FP64_RI, false> : forces_sym_kernel<SYM_FP64_THREADS, SYM_FP64_RI, true>;
-            k<<<Ps, SYM_FP64_THREADS, sym_smem_bytes(), st>>>(tiles, w.plan, k0, k1, rowrec, colrec, 0, split);
+            k<<<Ps, SYM_FP64_THREADS, sym_smem_bytes(), st>>>(tiles, w.plan, k0, k1, rowrec, colrec, 0, split, share_rank, share_world);
         } else {
             auto k = split == 1 ? forces_sym_mixed_kernel<SYM_MIXED_THREADS, SYM_MIXED_RI, false>
                                 : forces_sym_mixed_kernel<SYM_MIXED_THREADS, SYM_MIXED_RI, true>;
-            k<<<Ps, SYM_MIXED_THREADS, sym_mixed_smem_bytes<SYM_MIXED_THREADS, SYM_MIXED_RI>(), st>>>(tiles, w.plan, k0, k1, rowrec, colrec, split);
+            k<<<Ps, SYM_MIXED_THREADS, sym_mixed_smem_bytes<SYM_MIXED_THREADS, SYM_MIXED_RI>(), st>>>(tiles, w.plan, k0, k1, rowrec, colrec, split,
+                                                                                                       share_rank, share_world);
         }
         forces_sym_reduce_kernel<<<(int)((N + 255) / 256), 256, 0, st>>>(w.plan, rowrec, colrec, k0, k1, N, hi, lo,
-                                                                          k1 == kmax ? 1 : 0, acc_out, split, t_fuse);
+                                                                          k1 == kmax ? 1 : 0, acc_out, split,
+                                                                          share_world == 1 ? t_fuse : NO_FUSE, share_rank, share_world);
         g_launches += 2;
     }
     if (prof) { STEPS_CUDA(cudaEventRecord(w.ev1, st)); w.ev_valid = true; }
@@ -409,7 +416,7 @@ int launch_forces(const double* pos, const double* mass, const double* soft, lon
             if (!w.ev0) { STEPS_CUDA(cudaEventCreate(&w.ev0)); STEPS_CUDA(cudaEventCreate(&w.ev1)); }
             STEPS_CUDA(cudaEventRecord(w.ev0, st));
         }
-        kern<<<P, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, i_begin, i_end, nb, w.partials, 0, 0.0, 0.0, nullptr, block_stride);
+        kern<<<P, CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, i_begin, i_end, nb, w.partials, 0, 0.0, 0.0, nullptr, block_stride, 0, 1);
         if (prof) { STEPS_CUDA(cudaEventRecord(w.ev1, st)); w.ev_valid = true; }
         forces_reduce_kernel<Path::NOUT><<<(int)((cnt + 255) / 256), 256, 0, st>>>(
             w.partials, nt, nb, P, cnt, acc_out, (block_stride == 1 && i_begin == 0 && i_end == N) ? t_fuse : NO_FUSE);
@@ -662,6 +669,33 @@ int steps_forces_blocks(const double* pos, const double* mass, const double* sof
     if (rc != STEPS_OK) return rc;
     rc = mixed ? launch_forces<MixedPath>(pos, mass, soft, N, first_block * IB, N, acc_out, st, w, w.grid_mixed, (int)block_stride, cnt)
                : launch_forces<Fp64Path>(pos, mass, soft, N, first_block * IB, N, acc_out, st, w, w.grid_fp64, (int)block_stride, cnt);
+    if (rc != STEPS_OK) return rc;
+    return release_scratch(w, st);
+}
+
+int steps_forces_share(const double* pos, const double* mass, const double* soft, long long N, int rank, int world,
+                       double* acc_part, int mixed, steps_stream_t stream)
+{
+    if (!pos || !mass || !soft || !acc_part || N < 1 || world < 1 || rank < 0 || rank >= world) return STEPS_EINVAL;
+    if (N > (1ll << 31) - IB) return STEPS_EINVAL;
+    if (misaligned(pos) || misaligned(mass) || misaligned(soft) || misaligned(acc_part)) return STEPS_EINVAL;
+    int dev;
+    int rc = current_device(&dev);
+    if (rc != STEPS_OK) return rc;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    rc = ensure_workspace(dev, N, st);
+    if (rc != STEPS_OK) return rc;
+    Workspace& w = g_ws[dev];
+    const bool sym = g_driver.load() == 0 && sym_eligible(N, mixed != 0) && w.sym_records && (!mixed || g_sym_enabled.load() != 2);
+    if (!sym) {                                       // too small to share (under a millisecond): rank 0 evaluates it all
+        if (rank == 0) return forces_impl(pos, mass, soft, N, 0, N, acc_part, mixed, stream);
+        STEPS_CUDA(cudaMemsetAsync(acc_part, 0, sizeof(double) * 3 * (size_t)N, st));
+        return STEPS_OK;
+    }
+    rc = claim_scratch(w, st);
+    if (rc != STEPS_OK) return rc;
+    rc = mixed ? launch_forces_sym<MixedPath>(pos, mass, soft, N, acc_part, st, w, rank, world)
+               : launch_forces_sym<Fp64Path>(pos, mass, soft, N, acc_part, st, w, rank, world);
     if (rc != STEPS_OK) return rc;
     return release_scratch(w, st);
 }

@@ -27,7 +27,8 @@ import subprocess
 import sys
 
 KERNEL_PATTERNS = ("forces_persistent_kernelINS_8Fp64Path", "forces_v1_kernelINS_8Fp64Path", "forces_sym_kernel", "forces_sym_mixed_kernel",
-                   "forces_persistent_kernelINS_9MixedPath", "forces_v1_kernelINS_9MixedPath")
+                   "forces_persistent_kernelINS_9MixedPath", "forces_v1_kernelINS_9MixedPath",
+                   "forces_sym_box_kernel", "forces_sym_mixed_box_kernel", "forces_boxring_kernel")
 # the 2-clk-per-warp arithmetic instructions with 64-bit register operands: FP64 and packed fp32x2
 FP64_OPS = ("DFMA", "DMUL", "FFMA2", "FMUL2")
 # instructions that may sit between the two instructions of a pair (ptxas itself keeps `.reuse` across these)

@@ -104,3 +104,39 @@ class ShardedStep:
         self.kick_drift(coeffs)
         self.exchange(group)
         self.forces()
+
+
+class WorkSharedStep:
+    """One rank's side of the KDK step with the force evaluation shared by WORK (steps_forces_share): every rank holds and
+    advances ALL particles (the O(N) kick/drift is repeated on every rank, bit-identically), evaluates its share of the pair
+    evaluations -- the pair-symmetric kernels at their single-GPU rate -- into a partial acceleration of every particle, and
+    the one exchange per step is a sum-reduction of those partials (3N doubles).  The phases are separate calls so that a
+    single-GPU test can play several ranks one after the other."""
+
+    def __init__(self, S, rank: int, world: int, pos, vel, mass, soft, mixed: bool):
+        import torch
+        self.S, self.rank, self.world, self.mixed = S, rank, world, mixed
+        self.n = mass.numel()
+        self.cnt = self.n                                               # every rank advances every particle
+        self.mass, self.soft = mass, soft
+        self.x, self.v, self.m = pos.clone(), vel.clone(), mass
+        self.a = torch.empty_like(self.x)                               # this rank's partial, then the reduced sum
+
+    def forces_part(self):
+        self.S.steps_forces_share(self.x, self.mass, self.soft, self.rank, self.world, self.a, mixed=self.mixed)
+
+    def reduce(self, group=None):
+        if self.world > 1:
+            import torch.distributed as dist
+            dist.all_reduce(self.a, op=dist.ReduceOp.SUM, group=group)
+
+    def forces(self, group=None):
+        self.forces_part()
+        self.reduce(group)
+
+    def kick_drift(self, coeffs):
+        self.S.steps_kick_drift(self.x, self.v, self.a, coeffs)
+
+    def step(self, coeffs, group=None):
+        self.kick_drift(coeffs)
+        self.forces(group)

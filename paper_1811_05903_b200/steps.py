@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(_HERE, "libsteps_b200.so")
 OK, EINVAL, ECUDA, EUNSUPPORTED, ENOMEM, ECAPTURE = 0, -1, -2, -3, -4, -5
 
 EXPORTS = [
-    "steps_forces", "steps_forces_mixed", "steps_forces_range", "steps_forces_blocks", "steps_block_size", "steps_forces_host", "steps_kick_drift",
+    "steps_forces", "steps_forces_mixed", "steps_forces_range", "steps_forces_blocks", "steps_forces_share", "steps_block_size", "steps_forces_host", "steps_kick_drift",
     "steps_sort_radial", "steps_permute", "steps_near_fraction",
     "steps_kdk_step", "steps_hubble", "steps_scale_factor_rk4", "steps_kdk_schedule", "steps_momentum",
     "steps_timestep", "steps_timestep_coefficient", "steps_force_residual", "steps_forces_quasi_periodic", "steps_forces_periodic",
@@ -68,6 +68,7 @@ def load_library(path: str) -> C.CDLL:
     L.steps_forces_range.argtypes = [vp, vp, vp, ll, ll, ll, vp, i32, vp]
     L.steps_forces_host.argtypes = [vp, vp, vp, ll, vp, i32, vp]
     L.steps_forces_blocks.argtypes = [vp, vp, vp, ll, ll, ll, vp, i32, vp]
+    L.steps_forces_share.argtypes = [vp, vp, vp, ll, i32, i32, vp, i32, vp]
     L.steps_sort_radial.argtypes = [vp, ll, vp, vp]
     L.steps_permute.argtypes = [vp, ll, i32, vp, vp, vp]
     L.steps_near_fraction.argtypes = [vp, vp, vp, ll, vp, vp]
@@ -165,6 +166,14 @@ def steps_forces_blocks(pos, mass, soft, first_block: int, block_stride: int, ac
     n = mass.numel()
     _check(lib().steps_forces_blocks(_dev(pos, 3 * n), _dev(mass, n), _dev(soft, n), n, first_block, block_stride,
                                      _dev(acc_out, acc_out.numel()), int(mixed), _stream(stream)))
+
+
+def steps_forces_share(pos, mass, soft, rank: int, world: int, acc_part, mixed: bool = False, stream=None) -> None:
+    """acc_part (3N) = the contribution of the rank-th of `world` equal parts of the pair evaluations to every particle's
+    acceleration; the sum over the ranks is the result of steps_forces / steps_forces_mixed to rounding."""
+    n = mass.numel()
+    _check(lib().steps_forces_share(_dev(pos, 3 * n), _dev(mass, n), _dev(soft, n), n, int(rank), int(world),
+                                    _dev(acc_part, 3 * n), int(mixed), _stream(stream)))
 
 
 def steps_sort_radial(pos, perm, stream=None) -> None:

@@ -209,6 +209,18 @@ def test_sass_reuse_patch_is_bit_identical(S):
             assert fn(dpos.data_ptr(), dm.data_ptr(), dh.data_ptr(), n, b.data_ptr(), st) == 0
             torch.cuda.synchronize()
             assert torch.equal(a, b), f"N={n} mixed={mixed}: patched and unpatched libraries differ"
+    # the periodic kernels get the hints too: group ring (N = 20,000), pair-symmetric route (40,001 fp64 / 150,001 mixed)
+    L = 1.0
+    for n, paths in ((20000, (False, True)), (40001, (False,)), (150001, (True,))):
+        pos, mass, soft = synth.periodic_box(n, L, 4400 + n)
+        dpos, dm, dh = dev(pos), dev(mass), dev(soft)
+        st = torch.cuda.current_stream().cuda_stream
+        for mixed in paths:
+            a, b = torch.empty_like(dpos), torch.empty_like(dpos)
+            S.steps_forces_quasi_periodic(dpos, dm, dh, L, a, mixed=mixed)
+            assert U.steps_forces_quasi_periodic(dpos.data_ptr(), dm.data_ptr(), dh.data_ptr(), n, L, b.data_ptr(), int(mixed), st) == 0
+            torch.cuda.synchronize()
+            assert torch.equal(a, b), f"quasi-periodic N={n} mixed={mixed}: patched and unpatched libraries differ"
     U.steps_shutdown()
 
 
@@ -329,6 +341,76 @@ def test_outputs_stay_inside_their_buffers(S, n):
             torch.cuda.synchronize()
             assert bool((big[:pad] == sentinel).all()) and bool((big[pad + 3 * cnt:] == sentinel).all())
             assert bool(torch.isfinite(big[pad:pad + 3 * cnt]).all())
+
+
+@pytest.mark.parametrize("world", [2, 3, 8])
+@pytest.mark.parametrize("mixed,n", [(False, 65536), (False, 4096), (True, 150001)], ids=["fp64-65536", "fp64-4096", "mixed-150001"])
+def test_work_shares_sum_to_the_full_evaluation(S, oracle, mixed, n, world):
+    """steps_forces_share: the pair evaluations of one force evaluation cut into `world` equal parts (band visits and
+    pair-symmetric items); the sum of the parts' partial accelerations is the full result to rounding (each part is
+    rounded to fp64 once; the parts of a particle's acceleration can be much larger than their sum, hence the bound
+    relative to sum_j |f_ij|), each part is bit-reproducible, and the sum matches the oracle on a sample."""
+    import torch
+    ps = synth.g0(n, seed=3100 + n)
+    dpos, dm, dh = dev(ps.pos), dev(ps.mass), dev(ps.soft)
+    full = torch.empty(3, n, dtype=torch.float64, device="cuda")
+    (S.steps_forces_mixed if mixed else S.steps_forces)(dpos, dm, dh, full)
+    total = torch.zeros_like(full)
+    part, again = torch.empty_like(full), torch.empty_like(full)
+    norms = []
+    for r in range(world):
+        S.steps_forces_share(dpos, dm, dh, r, world, part, mixed=mixed)
+        if r == world - 1:
+            S.steps_forces_share(dpos, dm, dh, r, world, again, mixed=mixed)
+            assert torch.equal(part, again)
+        norms.append(float(part.norm()))
+        total += part
+    scale = full.norm(dim=0)
+    d = ((total - full).norm(dim=0) / scale).cpu().numpy()
+    print(f"[work shares n={n} world={world} {'mixed' if mixed else 'fp64'}] sum vs full: rms {math.sqrt(np.mean(d ** 2)):.3e} "
+          f"max {d.max():.3e}; |part| {['%.3e' % v for v in norms]}")
+    assert d.max() <= (2e-6 if mixed else 2e-13)
+    if S.steps_pair_symmetric(n, mixed):
+        assert min(norms) > 0.0                                   # every rank has work
+    idx = synth.stratified_sample(n, 256)
+    ref = oracle.forces(ps.pos, ps.mass, ps.soft, idx=idx)
+    e = rel_err(total.cpu().numpy()[:, idx], ref)
+    assert e.max() <= (1e-4 if mixed else 1e-12)
+
+
+@pytest.mark.parametrize("mixed", [False, True], ids=["fp64", "mixed"])
+def test_work_shared_step_on_one_gpu_equals_unsharded(S, mixed):
+    """bench.py's N > 1 step with the work-shared force evaluation (shard.WorkSharedStep) played on ONE GPU, rank after
+    rank, the all-reduce replaced by adding the ranks' partials: two steps reproduce steps_kdk_step."""
+    import torch
+    from paper_1811_05903_b200 import shard
+    n, world = (150001 if mixed else 40001), 3
+    ps = synth.g0(n, seed=3300 + n)
+    dpos, dm, dh = dev(ps.pos), dev(ps.mass), dev(ps.soft)
+    co = S.KdkCoeffs(1.0, 0.0, 0.98, 1.0e-3, 2.0e-3, 1.0 / ps.r_cut ** 3, int(mixed))
+    x, v, a = dpos.clone(), torch.zeros_like(dpos), torch.empty_like(dpos)
+    (S.steps_forces_mixed if mixed else S.steps_forces)(x, dm, dh, a)
+    ranks = [shard.WorkSharedStep(S, r, world, dpos, torch.zeros_like(dpos), dm, dh, mixed) for r in range(world)]
+
+    def all_forces():
+        for sh in ranks:
+            sh.forces_part()
+        total = sum(sh.a for sh in ranks)
+        for sh in ranks:
+            sh.a.copy_(total)
+
+    all_forces()
+    for _ in range(2):
+        S.steps_kdk_step(x, v, a, dm, dh, co)
+        for sh in ranks:
+            sh.kick_drift(co)
+        all_forces()
+    for sh in ranks[1:]:
+        assert torch.equal(sh.x, ranks[0].x) and torch.equal(sh.v, ranks[0].v)
+    da = float(((ranks[0].a - a).norm(dim=0) / a.norm(dim=0)).max())
+    dx = float((ranks[0].x - x).abs().max())
+    print(f"[work-shared step {'mixed' if mixed else 'fp64'}] acc {da:.3e} x {dx:.3e}")
+    assert da <= (5e-6 if mixed else 5e-13) and dx <= 1e-12
 
 
 @pytest.mark.parametrize("world", [2, 3])

@@ -86,3 +86,69 @@ def test_sharded_step_equals_unsharded(world, n, tmp_path, oracle):
     for r in range(world):
         assert np.array_equal(np.load(tmp_path / f"pos_{r}.npy"), expect_pos), f"rank {r}: gathered positions"
         assert np.array_equal(np.load(tmp_path / f"acc_{r}.npy"), full[:, shard.owned_indices(r, world, n)]), f"rank {r}: forces"
+
+
+class _FakeSteps:
+    """Stand-in for the ctypes binding on CPU: the rank's share of the work is played by the oracle's sum over the
+    sources j = rank (mod world) (the other sources' masses set to zero) -- a partition of the pair evaluations whose
+    parts add up to the full sum, like steps_forces_share's; the kick/drift is a plain linear update."""
+
+    def __init__(self, oracle):
+        self.oracle = oracle
+
+    def steps_forces_share(self, pos, mass, soft, rank, world, acc_part, mixed=False):
+        import torch
+        m = mass.numpy().copy()
+        m[np.arange(m.size) % world != rank] = 0.0
+        acc_part.copy_(torch.from_numpy(self.oracle.forces(np.ascontiguousarray(pos.numpy()), m, soft.numpy())))
+
+    def steps_kick_drift(self, x, v, a, coeffs):
+        v.add_(a, alpha=coeffs)
+        x.add_(v, alpha=coeffs)
+
+
+def _share_worker(rank: int, world: int, port: int, n: int, out_dir: str) -> None:
+    import torch
+    import torch.distributed as dist
+
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        from oracle import steps_oracle as oracle
+        ps = synth.g0(n, seed=78)
+        pos, mass, soft = (torch.from_numpy(a.copy()) for a in (ps.pos, ps.mass, ps.soft))
+        sh = shard.WorkSharedStep(_FakeSteps(oracle), rank, world, pos, torch.zeros_like(pos), mass, soft, False)
+        sh.forces()
+        ptr = sh.a.data_ptr()
+        for _ in range(2):
+            sh.step(1.0e-2)
+        assert sh.a.data_ptr() == ptr                          # reduced in place, nothing reallocated
+        np.save(os.path.join(out_dir, f"x_{rank}.npy"), sh.x.numpy())
+        np.save(os.path.join(out_dir, f"a_{rank}.npy"), sh.a.numpy())
+        dist.barrier()
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world,n", [(2, 3001), (3, 2500)])
+def test_work_shared_step_equals_unsharded(world, n, tmp_path, oracle):
+    """shard.WorkSharedStep over gloo: every rank advances all particles, evaluates its share of the pair evaluations and
+    the partial accelerations are summed by one all-reduce; all ranks end bit-identical, and equal to the unsharded run to
+    the rounding of the sum of the parts."""
+    import torch.multiprocessing as mp
+
+    port = _free_port()
+    mp.spawn(_share_worker, args=(world, port, n, str(tmp_path)), nprocs=world, join=True)
+    ps = synth.g0(n, seed=78)
+    x, v = ps.pos.copy(), np.zeros_like(ps.pos)
+    a = oracle.forces(x, ps.mass, ps.soft)
+    for _ in range(2):
+        v += 1.0e-2 * a
+        x += 1.0e-2 * v
+        a = oracle.forces(x, ps.mass, ps.soft)
+    x0, a0 = np.load(tmp_path / "x_0.npy"), np.load(tmp_path / "a_0.npy")
+    for r in range(1, world):
+        assert np.array_equal(np.load(tmp_path / f"x_{r}.npy"), x0) and np.array_equal(np.load(tmp_path / f"a_{r}.npy"), a0)
+    assert np.max(np.abs(x0 - x)) <= 1e-12 * np.max(np.abs(x))
+    assert np.max(np.linalg.norm(a0 - a, axis=0) / np.linalg.norm(a, axis=0)) <= 1e-11
