@@ -70,7 +70,6 @@ struct Workspace {
     long long sym_cap_particles = 0, sym_panel_items = 0;
     int num_sms = 0;
     int grid_mixed = 0, grid_fp64 = 0, grid_fp64_band = 0, grid_mixed_band = 0, grid_sym = 0, grid_sym_mixed = 0;   // persistent grids: SMs x resident CTAs
-    int grid_mixed_periodic = 0, grid_fp64_periodic = 0, grid_fp64_images = 0;
     double* mom_partial = nullptr;  // MOM_BLOCKS * 4
     void* sort_buf = nullptr;       // steps_sort_radial: keys in/out, index in, cub temporary storage
     size_t sort_bytes = 0;
@@ -553,7 +552,7 @@ int launch_forces_box(const double* pos, const double* mass, const double* soft,
 
 template <typename Path, int BOX>
 int launch_forces_periodic(const double* pos, const double* mass, const double* soft, long long N, double L, double* acc_out,
-                           cudaStream_t st, Workspace& w, int& grid_cache)
+                           cudaStream_t st, Workspace& w)
 {
     using Tile = typename Path::Tile;
     const int nt = (int)ntiles_of(N);
@@ -607,8 +606,8 @@ int steps_forces_quasi_periodic(const double* pos, const double* mass, const dou
     if (rc != STEPS_OK) return rc;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     Workspace& w = g_ws[dev];
-    return mixed ? launch_forces_periodic<MixedPath, 1>(pos, mass, soft, N, L, acc, st, w, w.grid_mixed_periodic)
-                 : launch_forces_periodic<Fp64Path, 1>(pos, mass, soft, N, L, acc, st, w, w.grid_fp64_periodic);
+    return mixed ? launch_forces_periodic<MixedPath, 1>(pos, mass, soft, N, L, acc, st, w)
+                 : launch_forces_periodic<Fp64Path, 1>(pos, mass, soft, N, L, acc, st, w);
 }
 
 int steps_forces_periodic(const double* pos, const double* mass, const double* soft, long long N, double L, double* acc,
@@ -623,8 +622,7 @@ int steps_forces_periodic(const double* pos, const double* mass, const double* s
     rc = ensure_workspace(dev, N, reinterpret_cast<cudaStream_t>(stream));
     if (rc != STEPS_OK) return rc;
     Workspace& w = g_ws[dev];
-    return launch_forces_periodic<Fp64Path, 2>(pos, mass, soft, N, L, acc, reinterpret_cast<cudaStream_t>(stream), w,
-                                               w.grid_fp64_images);
+    return launch_forces_periodic<Fp64Path, 2>(pos, mass, soft, N, L, acc, reinterpret_cast<cudaStream_t>(stream), w);
 }
 
 int steps_forces(const double* pos, const double* mass, const double* soft, long long N, double* acc,

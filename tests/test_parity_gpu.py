@@ -728,6 +728,39 @@ def test_quasi_periodic_pair_symmetric_route(S, mixed, n):
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("mixed", [False, True], ids=["fp64", "mixed"])
+def test_quasi_periodic_pair_symmetric_route_with_tracers_and_a_heavy_softened_group(S, oracle, mixed):
+    """Edge cases of the periodic pair-symmetric route against the oracle: massless tracer particles (they feel forces but
+    their reaction sums cannot be divided by m_j: their groups must stay out of the symmetric meetings), a block whose
+    particles carry a softening of a tenth of the box (softened pairs far beyond the neighbouring cells), particles given
+    outside [0, L) by whole periods (fp64), and N not a multiple of the group / tile / block."""
+    import torch
+    n = 150001 if mixed else 40001
+    L = 2.5
+    pos, mass, soft = _periodic_box(n, L, 8800 + n)
+    pos = np.ascontiguousarray(pos[:, synth.morton_order(pos, L)])
+    mass[[5, 2048 * 3 + 17, n - 1]] = 0.0                       # tracers
+    soft[2048 * 5: 2048 * 5 + 300] = 0.05 * L                   # pair softening 0.1 L for 300 particles of block 5
+    if not mixed:
+        pos[:, 2048 * 7: 2048 * 7 + 40] += np.array([[2 * L], [-L], [0.0]])
+    acc = torch.empty(3, n, dtype=torch.float64, device="cuda")
+    assert S.steps_pair_symmetric(n, mixed) == 1
+    S.steps_forces_quasi_periodic(dev(pos), dev(mass), dev(soft), L, acc, mixed=mixed)
+    idx = np.unique(np.concatenate([synth.stratified_sample(n, 512), [5, 2048 * 3 + 17, n - 1], np.arange(2048 * 5, 2048 * 5 + 300, 7),
+                                    np.arange(2048 * 7, 2048 * 7 + 40, 3)]))
+    ref = oracle.forces_quasi_periodic(pos, mass, soft, L, idx=idx)
+    got = acc.cpu().numpy()[:, idx]
+    fsum = _pair_force_abs_sum(pos, mass, np.full(n, soft.min()), L, idx)
+    e_abs = np.linalg.norm(got - ref, axis=0) / fsum
+    print(f"[quasi-periodic edge cases n={n} {'mixed' if mixed else 'fp64'}] to sum_j|f_ij|: rms {math.sqrt(np.mean(e_abs ** 2)):.3e} max {e_abs.max():.3e}")
+    assert np.isfinite(got).all()
+    if mixed:
+        assert math.sqrt(np.mean(e_abs ** 2)) <= 2e-6 and e_abs.max() <= 1e-4
+    else:
+        assert e_abs.max() <= 1e-13 and rel_err(got, ref).max() <= 1e-12
+
+
+@pytest.mark.gpu
 def test_quasi_periodic_translation_invariance_and_unwrapped_positions_on_device(S):
     """Shifting every particle by an arbitrary vector, without wrapping the positions back into [0, L), must leave the
     fp64 forces unchanged to rounding (the wrap acts on separations, not on positions)."""
