@@ -490,6 +490,24 @@ forces_sym_mixed_kernel(const TileF32* __restrict__ tiles, const SymPlan* __rest
 //     memory, each thread's own four/eight), and the components whose separations straddle half the box are folded
 //     (fold_f64 / fold2: one addition + one bit operation per pair and component), the body chosen by the fold mask;
 //   * the reaction on j uses the folded separation as well -- the leading image of x_i - x_j is minus that of x_j - x_i.
+// Hand-over of a column subgroup between the warps of the periodic symmetric kernels.  Warp w meets subgroup (w + q) mod SUBG
+// in round q, so the subgroup it needs next was last used -- one round earlier -- by warp w + 1, and by nobody else: instead
+// of a CTA-wide barrier per round (every round then costs what its most-folded meeting costs) a warp only waits for its
+// neighbour's count of finished rounds.  The warps drift apart by a few rounds and the meetings' costs average out.
+__device__ __forceinline__ void round_publish(int* counter, int value)      // one lane, after __syncwarp
+{
+    asm volatile("st.release.cta.shared.s32 [%0], %1;" ::"r"(smem_u32(counter)), "r"(value) : "memory");
+}
+__device__ __forceinline__ void round_wait(const int* counter, int value)   // one lane, followed by __syncwarp
+{
+    int seen;
+    for (;;) {
+        asm volatile("ld.acquire.cta.shared.s32 %0, [%1];" : "=r"(seen) : "r"(smem_u32(counter)) : "memory");
+        if (seen >= value) break;
+        __nanosleep(200);                                    // a spinning warp would take issue slots from the working ones
+    }
+}
+
 template <int RI, int MASK>
 __device__ __forceinline__ void sym_box_steps(const FarSrcF64* __restrict__ set, int lane, int src_lane, const double (&xi)[RI],
                                               const double (&yi)[RI], const double (&zi)[RI], const double (&mi)[RI], double (&ax)[RI],
@@ -573,6 +591,8 @@ forces_sym_box_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restri
     FarSrcF64* col = reinterpret_cast<FarSrcF64*>(smem_raw);                       // [2][IB]
     double* Bsm = reinterpret_cast<double*>(smem_raw + 2 * IB * sizeof(FarSrcF64));   // [3][IB]
     double* Xsm = Bsm + 3 * IB + threadIdx.x;                                      // [3][RI][THREADS]: the row block, unshifted
+    __shared__ int round_done[SUBG];                                               // rounds finished per warp (round_wait)
+    if (threadIdx.x < SUBG) round_done[threadIdx.x] = 0;
 
     const long long K = plan->K * split;
     if (k_end > K) k_end = K;
@@ -646,8 +666,13 @@ forces_sym_box_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restri
         // the image decisions of this warp's SUBG meetings of the item, one per lane (boxcode_pack, force_driver.cuh)
         const uint32_t my_code = boxcode_pack(pair_decision<1>(gm, b * SUBG + warp, c * SUBG + (lane & (SUBG - 1)), box_L, box_invL), box_invL);
         const int part = SPLIT ? (int)((kk0 + it) % split) : 0, rounds = SPLIT ? SUBG / split : SUBG;
+        const int base = it * rounds;                         // rounds every warp had finished when this item started
         for (int q = part * rounds; q < (part + 1) * rounds; ++q) {
             const int u = (warp + q) & (SUBG - 1);
+            if (q > part * rounds) {                          // subgroup u was warp + 1's in the round before (round_wait above)
+                if (lane == 0) round_wait(&round_done[(warp + 1) & (SUBG - 1)], base + (q - part * rounds));
+                __syncwarp();
+            }
             const BoxShift dec = boxcode_unpack(__shfl_sync(0xffffffffu, my_code, u), box_L);
             if (dec.kind != 0) {                              // else: forces_boxring_kernel evaluates this meeting
                 double xi[RI], yi[RI], zi[RI];
@@ -673,8 +698,10 @@ forces_sym_box_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restri
                     Bsm[j] += bx; Bsm[IB + j] += by; Bsm[2 * IB + j] += bz;
                 }
             }
-            __syncthreads();
+            __syncwarp();
+            if (lane == 0) round_publish(&round_done[warp], base + (q - part * rounds) + 1);
         }
+        __syncthreads();                                      // every subgroup's reaction sums are complete
 
         const long long rec = (kk0 + it - k_begin) * 3 * IB;
 #pragma unroll
@@ -870,6 +897,8 @@ forces_sym_mixed_box_kernel(const TileF32* __restrict__ tiles, const SymPlan* __
                     }
                 }
             }
+            // (a CTA-wide barrier per round here: the neighbour hand-over of the fp64 kernel, round_wait, measured SLOWER with
+            // this kernel's two warps per scheduler -- 30.5 against 28.1 ms at N = 262,144)
             __syncthreads();
         }
 
