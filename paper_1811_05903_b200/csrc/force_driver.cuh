@@ -693,13 +693,23 @@ forces_boxring_kernel(const double* __restrict__ pos, const double* __restrict__
             const int s = consumed % STAGES;
             mbar_wait(&full_bar[g][s], (consumed / STAGES) & 1);
             if constexpr (BOX == 2) {
-                // the candidate images of this (group, tile) pair, pruned from the two bounding boxes (see the header comment)
-                const TileMeta meta = tiles[tile_of(g, k0 + q)].meta;
+                // the candidate images of this warp's 64 sources of the tile against the group, pruned from the two bounding
+                // boxes (see the header comment); the sources' box is taken from the staged copy itself -- a quarter of a
+                // cell-ordered tile is more compact than the tile, and every candidate less is 1 % of the work
+                const double* P = reinterpret_cast<const double*>(ring + s * FAR_BYTES);      // x[], y[], z[], m[], h[]
                 double sh[3], a[3], b[3];
                 const double eps = 1.0e-5 * box_L;
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
-                    const double dmin = ((double)meta.lo[c] - (double)gbox[3 + c]) - eps, dmax = ((double)meta.hi[c] - (double)gbox[c]) + eps;
+                    double lo = __longlong_as_double(0x7ff0000000000000ll), hi = -lo;
+#pragma unroll
+                    for (int r = 0; r < PER_WARP / 32; ++r) {
+                        const int j = j0 + 32 * r + lane;
+                        if (P[3 * TJ + j] != 0.0) { lo = fmin(lo, P[c * TJ + j]); hi = fmax(hi, P[c * TJ + j]); }    // pads (m = 0) are parked
+                    }
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) { lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o)); hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, o)); }
+                    const double dmin = (lo - (double)gbox[3 + c]) - eps, dmax = (hi - (double)gbox[c]) + eps;
                     sh[c] = box_L * rint(0.5 * (dmin + dmax) * box_invL);
                     a[c] = dmin - sh[c]; b[c] = dmax - sh[c];
                 }
@@ -727,7 +737,6 @@ forces_boxring_kernel(const double* __restrict__ pos, const double* __restrict__
                 Q = group_state();
 #pragma unroll
                 for (int k = 0; k < R_I; ++k) { Q.x[k] += sh[0]; Q.y[k] += sh[1]; Q.z[k] += sh[2]; }
-                const double* P = reinterpret_cast<const double*>(ring + s * FAR_BYTES);      // x[], y[], z[], m[], h[]
                 Path::far_images(P, P + TJ, P + 2 * TJ, P + 3 * TJ, Q, acc, box_L, cube_tab, cand, ncand, j0, j1);
             } else {
                 const Tile& T = *reinterpret_cast<const Tile*>(ring + s * FAR_BYTES);    // only its far part is there

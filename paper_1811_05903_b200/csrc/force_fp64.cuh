@@ -386,6 +386,7 @@ struct Fp64Path {
         constexpr int H = 2;                                           // particles per pass
         static_assert(R_I % H == 0, "whole passes");
         const long long cut2_bits = __double_as_longlong((2.6 * L) * (2.6 * L));
+        if (ncand <= 0) return;                                        // (only a slice of pads has no candidate)
 #pragma unroll 1
         for (int j = j0; j < j1; ++j) {
             const double xj = Tx[j], yj = Ty[j], zj = Tz[j], mq = Tm[j];
@@ -399,10 +400,14 @@ struct Fp64Path {
                     dx[k] = xj - Q.x[k0 + k]; dy[k] = yj - Q.y[k0 + k]; dz[k] = zj - Q.z[k0 + k];
                     px[k] = py[k] = pz[k] = 0.0;
                 }
+                // (the next candidate's offsets are fetched one pass ahead: index -> address -> three loads is a dependent
+                // chain of two shared-memory latencies that would otherwise open every pass)
+                double nox, noy, noz;
+                { const int t3 = 3 * cand[0]; nox = tab[t3]; noy = tab[t3 + 1]; noz = tab[t3 + 2]; }
 #pragma unroll 2
                 for (int c = 0; c < ncand; ++c) {
-                    const int t3 = 3 * cand[c];
-                    const double ox = tab[t3], oy = tab[t3 + 1], oz = tab[t3 + 2];
+                    const double ox = nox, oy = noy, oz = noz;
+                    { const int t3 = 3 * cand[min(c + 1, ncand - 1)]; nox = tab[t3]; noy = tab[t3 + 1]; noz = tab[t3 + 2]; }
                     double vx[H], vy[H], vz[H], r2[H], y0[H], y2[H], w[H];
 #pragma unroll
                     for (int k = 0; k < H; ++k) { vx[k] = dx[k] - ox; vy[k] = dy[k] - oy; vz[k] = dz[k] - oz; }
