@@ -246,6 +246,8 @@ def main():
     ap.add_argument("--ref-pairs", type=float, default=4e9, help="--impl reference: pair budget per step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-next-rows", action="store_true", help="skip the periodic / adaptive-step rows (SURVEY 8(f))")
+    ap.add_argument("--next-rows-only", action="store_true",
+                    help="only the periodic / adaptive-step rows (one JSON line with `next_rows`; for profiling them)")
     ap.add_argument("--sharded-step", action="store_true",
                     help="time the N > 1 step (shard.WorkSharedStep / shard.ShardedStep: share of the work + exchange) even with one rank")
     args = ap.parse_args()
@@ -271,6 +273,11 @@ def main():
         os.environ.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     args.warmup = max(args.warmup, 3)
+
+    if args.next_rows_only:
+        S.steps_set_option("profile", 0)
+        print(json.dumps({"next_rows": bench_next_rows(S, synth, torch, torch.cuda.current_stream(), reps=args.steps), "build": S.build_info()}))
+        return
 
     n = args.n or 1048576
     ps = synth.g0(n, synth.SEED_BASE + 3)          # config 3 (identical on every rank: seeded)

@@ -820,7 +820,7 @@ forces_boxgen_kernel(const double* __restrict__ pos, const double* __restrict__ 
     static_assert(TJ == 2 * SPLITJ_GROUP && SLICE % 2 == 0, "a tile is two groups; the mixed general body takes sources in pairs");
     static_assert(BOXGEN_BATCH % (WARPS / WPU) == 0, "whole rounds of WARPS / WPU units per batch");
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    __shared__ int gcount[WARPS];
+    __shared__ int gcount[(BOXGEN_CHUNK / CTA_THREADS) * WARPS];
     double* acc_all = reinterpret_cast<double*>(smem_raw);
     double* acc = acc_all + threadIdx.x;
     uint32_t* glist = reinterpret_cast<uint32_t*>(acc_all + Path::NOUT * R_I * CTA_THREADS);
@@ -843,26 +843,33 @@ forces_boxgen_kernel(const double* __restrict__ pos, const double* __restrict__ 
 
     for (int u0 = u_lo; active && u0 < units; u0 += BOXGEN_CHUNK) {
         const int cnt = min(BOXGEN_CHUNK, units - u0);
-        constexpr int PER = BOXGEN_CHUNK / WARPS;           // units scanned per warp
+        constexpr int ROUNDS = BOXGEN_CHUNK / CTA_THREADS;  // decisions per thread: unit q = r * CTA_THREADS + thread
         auto wanted = [&](int q) {
             if (q >= cnt) return false;
             const int u = u0 + q;
             if ((int)(((long long)u * UNIT) / IB) == my_block) return false;       // own block: forces_boxring_kernel
             return (boxcode_pack(pair_decision<GRAN>(gm, me, u, box_L, box_invL), box_invL) & BOXCODE_GENERAL) != 0;
         };
-        unsigned flags[PER / 32];
-        int mine_cnt = 0;
+        // (thread-interleaved: a CTA's share of a group is usually a few hundred units, one decision per thread; the list
+        // is in unit order: the offsets come from the (round, warp) counts)
+        unsigned flags[ROUNDS];
+        __syncthreads();                                    // the previous chunk's list and counts are no longer read
 #pragma unroll
-        for (int r = 0; r < PER / 32; ++r) { flags[r] = __ballot_sync(0xffffffffu, wanted(warp * PER + r * 32 + lane)); mine_cnt += __popc(flags[r]); }
-        __syncthreads();                                    // the previous chunk's list is no longer read
-        if (lane == 0) gcount[warp] = mine_cnt;
+        for (int r = 0; r < ROUNDS; ++r) {
+            flags[r] = r * CTA_THREADS < cnt ? __ballot_sync(0xffffffffu, wanted(r * CTA_THREADS + threadIdx.x)) : 0u;
+            if (lane == 0) gcount[r * WARPS + warp] = __popc(flags[r]);
+        }
         __syncthreads();
-        int at = 0, total_cnt = 0;
-        for (int w = 0; w < WARPS; ++w) { if (w < warp) at += gcount[w]; total_cnt += gcount[w]; }
+        int total_cnt = 0;
+        {
+            int at = 0;
 #pragma unroll
-        for (int r = 0; r < PER / 32; ++r) {
-            if (flags[r] >> lane & 1u) glist[at + __popc(flags[r] & ((1u << lane) - 1u))] = (uint32_t)(u0 + warp * PER + r * 32 + lane);
-            at += __popc(flags[r]);
+            for (int r = 0; r < ROUNDS; ++r) {
+                int before = 0;
+                for (int w = 0; w < WARPS; ++w) { const int c = gcount[r * WARPS + w]; if (w < warp) before += c; total_cnt += c; }
+                if (flags[r] >> lane & 1u) glist[at + before + __popc(flags[r] & ((1u << lane) - 1u))] = (uint32_t)(u0 + r * CTA_THREADS + threadIdx.x);
+                for (int w = 0; w < WARPS; ++w) at += gcount[r * WARPS + w];
+            }
         }
         __syncthreads();
         for (int e0 = 0; e0 < total_cnt; e0 += BOXGEN_BATCH) {

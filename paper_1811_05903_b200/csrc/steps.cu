@@ -44,6 +44,7 @@ constexpr int SYM_MIN_BLOCKS_MIXED = 64;   // mixed: whole items only (its split
 std::atomic<long long> g_sym_panel_items{16384};
 std::atomic<int> g_sym_enabled{1};
 std::atomic<int> g_splitj{1};           // 0 = never use the split-j driver (testing)
+std::atomic<int> g_box_gsplit{8};       // CTAs per group in forces_boxgen_kernel (option "box_gsplit", tuning)
 
 // What the fused Eq. 12 minimum of the last steps_kdk_step_adaptive call was computed from (see that function).
 struct FuseToken {
@@ -518,7 +519,7 @@ int launch_forces_box(const double* pos, const double* mass, const double* soft,
     if (!gen_attr_set) { STEPS_CUDA(cudaFuncSetAttribute(gen, cudaFuncAttributeMaxDynamicSharedMemorySize, boxgen_smem_bytes<Path>())); gen_attr_set = true; }
     // (the unit range of a group is split over up to 8 CTAs, see forces_boxgen_kernel; their records use the symmetric
     // kernels' record buffer, which is free until the first panel)
-    long long gsplit = 8;
+    long long gsplit = std::max(1, g_box_gsplit.load());
     while (gsplit > 1 && (size_t)groups * gsplit * 6 * SPLITJ_GROUP * sizeof(double) > sym_record_bytes(w.sym_panel_items)) gsplit /= 2;
     gen<<<dim3((unsigned)groups, (unsigned)gsplit), CTA_THREADS, boxgen_smem_bytes<Path>(), st>>>(pos, soft, N, tiles, nt, hi, lo, w.sym_records,
                                                                                                    L, 1.0 / L, w.gm, w.plan);
@@ -1060,6 +1061,7 @@ int steps_set_option(const char* key, long long value)
     if (std::strcmp(key, "profile") == 0) { g_profile = (int)value; return STEPS_OK; }
     if (std::strcmp(key, "sym") == 0) { g_sym_enabled = (int)value; return STEPS_OK; }
     if (std::strcmp(key, "splitj") == 0) { g_splitj = (int)value; return STEPS_OK; }
+    if (std::strcmp(key, "box_gsplit") == 0) { g_box_gsplit = (int)value; return STEPS_OK; }
     if (std::strcmp(key, "fuse_eq12") == 0) { g_fuse_eq12 = (int)value; return STEPS_OK; }
     if (std::strcmp(key, "sym_panel_items") == 0) {
         if (value < 1) return STEPS_EINVAL;
