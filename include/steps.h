@@ -283,7 +283,8 @@ long long steps_kernel_launch_count(void);
  * "sym": 0 = never use the pair-symmetric evaluation (default 1).  "sym_panel_items": how many
  * block-pair items (96 KiB of partial records each) the symmetric evaluation keeps in flight
  * (default 16384 = 1.5 GiB; the items are run in panels of this size).  "splitj": 0 = never use the split-j driver.
- * "fuse_eq12": 0 = steps_kdk_step_adaptive always forms Eq. 12's minimum in its own pass.  Unknown key: STEPS_EINVAL. */
+ * "fuse_eq12": 0 = steps_kdk_step_adaptive always forms Eq. 12's minimum in its own pass.  "box_gsplit": CTAs that share
+ * one group's possibly-softened units in the periodic pair-symmetric evaluation (default 8).  Unknown key: STEPS_EINVAL. */
 int steps_set_option(const char *key, long long value);
 /* With "profile" on: device time in ms of the most recent force kernel launched on the current
  * device (waits for it to finish); -1 if none was recorded.  For a pair-symmetric evaluation: from the
