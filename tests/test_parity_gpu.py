@@ -321,7 +321,8 @@ def test_outputs_stay_inside_their_buffers(S, n):
 
     for call in (lambda: S.steps_forces(dpos, dm, dh, acc), lambda: S.steps_forces_mixed(dpos, dm, dh, acc),
                  lambda: S.steps_forces_quasi_periodic(dpos, dm, dh, 50.0, acc),
-                 lambda: S.steps_forces_quasi_periodic(dpos, dm, dh, 50.0, acc, mixed=True)):
+                 lambda: S.steps_forces_quasi_periodic(dpos, dm, dh, 50.0, acc, mixed=True),
+                 lambda: S.steps_forces_share(dpos, dm, dh, 1, 3, acc), lambda: S.steps_forces_share(dpos, dm, dh, 0, 2, acc, mixed=True)):
         call()
         assert intact() and bool(torch.isfinite(acc).all())
     if n <= 5000:
