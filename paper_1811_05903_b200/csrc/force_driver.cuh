@@ -388,8 +388,11 @@ __global__ void __launch_bounds__(CTA_THREADS, 1)
 forces_splitj_kernel(const double* __restrict__ pos, const double* __restrict__ soft, long long N,
                      const typename Path::Tile* __restrict__ tiles, int nt, int sub, long long i_begin, long long i_end,
                      double* __restrict__ acc_out, double* __restrict__ partials, int zero, double box_L, double box_invL,
-                     Eq12Fuse fuse)
+                     Eq12Fuse fuse, const SymPlan* __restrict__ plan, double* __restrict__ acc_lo_out)
 {
+    // plan != nullptr: BAND mode of a pair-symmetric evaluation with few blocks (the ring driver's (i-block, tile) items are
+    // then too few for 148 SMs: N = 32,768 is 384 visits): the group only meets the tiles of the blocks within the plan's
+    // band half-width of its own block, and the result stays double-double (acc_out = hi, acc_lo_out = lo).
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ double res[3][SPLITJ_GROUP];                                // the group's final accelerations (Eq. 12 fusion)
     double* acc_all = reinterpret_cast<double*>(smem_raw);                 // [NOUT * R_I][CTA_THREADS]
@@ -405,13 +408,19 @@ forces_splitj_kernel(const double* __restrict__ pos, const double* __restrict__ 
     for (int q = 0; q < Path::NOUT * R_I; ++q) acc[q * CTA_THREADS] = 0.0;
 
     const int per_tile = TJ / sub;
-    const long long units = (long long)nt * per_tile;
+    int t_lo = 0, t_hi = nt;                                                // the tiles this group meets
+    if (plan != nullptr) {
+        const int b = (int)(((long long)blockIdx.x * SPLITJ_GROUP) / IB), W = plan->W;
+        t_lo = max(0, b - W) * (IB / TJ);
+        t_hi = min(nt, (int)min((long long)plan->nb, (long long)b + W + 1) * (IB / TJ));
+    }
+    const long long units = (long long)(t_hi - t_lo) * per_tile;
     const long long u0 = (long long)blockIdx.y * units / gridDim.y, u1 = ((long long)blockIdx.y + 1) * units / gridDim.y;
     typename Path::FarSums F;
     init_far_sums<Path>(F, acc);
     int pending = 0;
     for (long long u = u0 + warp; u < u1; u += CTA_THREADS / 32) {
-        const typename Path::Tile& T = tiles[u / per_tile];
+        const typename Path::Tile& T = tiles[t_lo + u / per_tile];
         const int j0 = (int)(u % per_tile) * sub, j1 = j0 + sub;
         const TileMeta meta = T.meta;
         {
@@ -440,7 +449,10 @@ forces_splitj_kernel(const double* __restrict__ pos, const double* __restrict__ 
         }
         const long long i = (long long)blockIdx.x * SPLITJ_GROUP + l + 32 * k;        // within [i_begin, i_end)
         if (gridDim.y == 1) {
-            if (i < cnt) acc_out[(long long)c * cnt + i] = hi + lo;
+            if (i < cnt) {
+                if (acc_lo_out) { acc_out[(long long)c * cnt + i] = hi; acc_lo_out[(long long)c * cnt + i] = lo; }
+                else acc_out[(long long)c * cnt + i] = hi + lo;
+            }
             res[c][r] = hi + lo;
         } else {
             double* rec = partials + (((long long)blockIdx.x * gridDim.y + blockIdx.y) * 6) * SPLITJ_GROUP;

@@ -40,6 +40,7 @@ constexpr int MAX_GRID = 148 * 4;
 // Pair-symmetric evaluation (force_sym.cuh) of the fp64 path: used for full evaluations of at least SYM_MIN_BLOCKS blocks;
 // its partial records are produced and consumed in panels of at most g_sym_panel_items items (96 KiB of records each).
 constexpr int SYM_MIN_BLOCKS = 16;         // fp64: from N = 30,721, with the items split into parts while the blocks are few
+constexpr int SYM_SPLITJ_BAND_MAX_BLOCKS = 64;   // up to here the band of a pair-symmetric evaluation runs on the split-j driver
 constexpr int SYM_MIN_BLOCKS_MIXED = 64;   // mixed: whole items only (its split variant is slower than the ring kernel): N >= 129,025
 std::atomic<long long> g_sym_panel_items{16384};
 std::atomic<int> g_sym_enabled{1};
@@ -270,12 +271,39 @@ int launch_forces_sym(const double* pos, const double* mass, const double* soft,
     sym_band_width<Tile><<<nb, 128, 0, st>>>(tiles, nb, w.plan);
     sym_plan_finalize<<<1, 1024, 0, st>>>(w.plan, nb, 8 * Ps, split);
     if (prof) STEPS_CUDA(cudaEventRecord(w.ev0, st));
-    band<<<P, CTA_THREADS, smem_band, st>>>(pos, soft, N, tiles, ntp, 0, N, nb, w.partials, 0, 0.0, 0.0, w.plan, 1, share_rank, share_world);
     double* hi = w.acc_dd;
     double* lo = w.acc_dd + 3 * N;
-    forces_band_reduce_kernel<Path::NOUT><<<(int)((N + 255) / 256), 256, 0, st>>>(w.partials, w.plan, P, N, acc_out, 1, hi, lo, share_rank,
-                                                                                   share_world);
-    g_launches += 5;
+    if (nb <= SYM_SPLITJ_BAND_MAX_BLOCKS && share_world == 1 && g_splitj.load() != 0) {
+        // few blocks: the band's (i-block, tile) visits are too few for the ring driver (N = 32,768: 384 visits for 148 CTAs,
+        // 0.28 of peak); the split-j driver takes the band instead, one 128-particle group per CTA, 64-source units
+        auto sj = forces_splitj_kernel<Path, 0>;
+        constexpr int smem_sj = Path::NOUT * R_I * CTA_THREADS * (int)sizeof(double);
+        static bool sj_attr_set = false;
+        if (!sj_attr_set) { STEPS_CUDA(cudaFuncSetAttribute(sj, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_sj)); sj_attr_set = true; }
+        const long long groups = (N + SPLITJ_GROUP - 1) / SPLITJ_GROUP;
+        // the band's units of a group split over 1 or 2 CTAs, whichever makes the grid closest to whole waves (one CTA per SM;
+        // more parts leave a warp less than three units: measured slower at N = 32,768)
+        long long jsplit = 1;
+        double best = 0.0;
+        for (long long j = 1; j <= 4 && 96 / j >= 48; ++j) {       // (a band of half-width 1 is 96 units of 64 sources per group)
+            const double waves = (double)(groups * j) / w.num_sms, eff = waves / std::ceil(waves);
+            if (eff > best + 0.03) { best = eff; jsplit = j; }
+        }
+        const long long rec_cap = (long long)(partial_bytes(N) / (sizeof(double) * 6 * SPLITJ_GROUP));
+        if (groups * jsplit > rec_cap) jsplit = 1;
+        sj<<<dim3((unsigned)groups, (unsigned)jsplit), CTA_THREADS, smem_sj, st>>>(pos, soft, N, tiles, (int)ntiles_of(N), 64, 0, N, hi, w.partials, 0,
+                                                                                     0.0, 0.0, NO_FUSE, w.plan, lo);
+        g_launches += 4;
+        if (jsplit > 1) {
+            forces_splitj_reduce<<<(unsigned)groups, SPLITJ_GROUP, 0, st>>>(w.partials, (int)jsplit, N, hi, NO_FUSE, lo);
+            g_launches++;
+        }
+    } else {
+        band<<<P, CTA_THREADS, smem_band, st>>>(pos, soft, N, tiles, ntp, 0, N, nb, w.partials, 0, 0.0, 0.0, w.plan, 1, share_rank, share_world);
+        forces_band_reduce_kernel<Path::NOUT><<<(int)((N + 255) / 256), 256, 0, st>>>(w.partials, w.plan, P, N, acc_out, 1, hi, lo, share_rank,
+                                                                                       share_world);
+        g_launches += 5;
+    }
     // in sub-items; a share has at most ceil(all / share_world) of them (the kernels clamp to the share's actual end)
     const long long items = w.sym_panel_items, kmax = (sym_items_max(N) * split + share_world - 1) / share_world;
     double* rowrec = w.sym_records;
@@ -363,7 +391,7 @@ int launch_splitj(const double* pos, const double* soft, long long N, const type
     }
     const Eq12Fuse fuse = (BOX == 0 && i_begin == 0 && i_end == N) ? t_fuse : NO_FUSE;
     kern<<<dim3((unsigned)groups, (unsigned)jsplit), CTA_THREADS, smem, st>>>(pos, soft, N, tiles, nt, sub, i_begin, i_end, acc_out,
-                                                                                w.partials, 0, L, L > 0.0 ? 1.0 / L : 0.0, fuse);
+                                                                                w.partials, 0, L, L > 0.0 ? 1.0 / L : 0.0, fuse, nullptr, nullptr);
     g_launches++;
     if (jsplit > 1) {
         forces_splitj_reduce<<<(unsigned)groups, SPLITJ_GROUP, 0, st>>>(w.partials, (int)jsplit, cnt, acc_out, fuse);
