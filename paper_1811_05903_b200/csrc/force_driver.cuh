@@ -818,7 +818,8 @@ constexpr int boxgen_smem_bytes()
            BOXGEN_BATCH * 5 * (Path::NOUT == 6 ? 1 : 2) * SPLITJ_GROUP * (Path::NOUT == 6 ? 8 : 4);
 }
 
-template <typename Path>
+// BOX = 2: the same for the image sum (the listed units through Fp64Path::near_images_view, all 179 candidates).
+template <typename Path, int BOX = 1>
 __global__ void __launch_bounds__(CTA_THREADS, 1)
 forces_boxgen_kernel(const double* __restrict__ pos, const double* __restrict__ soft, long long N,
                      const typename Path::Tile* __restrict__ tiles, int nt, double* __restrict__ acc_hi, double* __restrict__ acc_lo,
@@ -826,6 +827,13 @@ forces_boxgen_kernel(const double* __restrict__ pos, const double* __restrict__ 
                      const SymPlan* __restrict__ plan)
 {
     using IState = typename Path::IState;
+    __shared__ double img_tab[BOX == 2 ? 3 * EWALD_NTRIPLETS : 1];
+    if constexpr (BOX == 2) {
+        for (int q = threadIdx.x; q < EWALD_NTRIPLETS; q += CTA_THREADS) {
+            img_tab[3 * q] = ewald_triplets[q].x * box_L; img_tab[3 * q + 1] = ewald_triplets[q].y * box_L;
+            img_tab[3 * q + 2] = ewald_triplets[q].z * box_L;
+        }
+    }
     constexpr int GRAN = Path::NOUT == 6 ? 1 : 2;           // groups per unit (the symmetric kernels' subgroups)
     using Elem = decltype(IState::x[0] + 0);                // double or float
     constexpr int UNIT = GRAN * SPLITJ_GROUP, WARPS = CTA_THREADS / 32, WPU = 4, SLICE = UNIT / WPU;   // 4 warps per unit
@@ -897,7 +905,10 @@ forces_boxgen_kernel(const double* __restrict__ pos, const double* __restrict__ 
             for (int e = warp / WPU; e < nbatch; e += WARPS / WPU) {
                 const Elem* u = stage + e * 5 * UNIT;
                 const int j0 = (warp % WPU) * SLICE;
-                Path::template near_view<true>(u, u + UNIT, u + 2 * UNIT, u + 3 * UNIT, u + 4 * UNIT, S, acc, box_L, box_invL, j0, j0 + SLICE);
+                if constexpr (BOX == 2)
+                    Path::near_images_view(u, u + UNIT, u + 2 * UNIT, u + 3 * UNIT, u + 4 * UNIT, S, acc, box_L, box_invL, img_tab, j0, j0 + SLICE);
+                else
+                    Path::template near_view<true>(u, u + UNIT, u + 2 * UNIT, u + 3 * UNIT, u + 4 * UNIT, S, acc, box_L, box_invL, j0, j0 + SLICE);
             }
         }
     }

@@ -295,13 +295,21 @@ struct Fp64Path {
     static __device__ __forceinline__ void near_images(const Tile& T, const IState& S, double* acc, double L, double invL,
                                                        const double* __restrict__ tab, int j0 = 0, int j1 = TJ)
     {
+        near_images_view(T.x, T.y, T.z, T.m, T.h, S, acc, L, invL, tab, j0, j1);
+    }
+    // The same on any copy of the plain sources (x, y, z, m, h), e.g. one staged in shared memory.
+    static __device__ __forceinline__ void near_images_view(const double* __restrict__ Tx, const double* __restrict__ Ty,
+                                                            const double* __restrict__ Tz, const double* __restrict__ Tm,
+                                                            const double* __restrict__ Th, const IState& S, double* acc, double L,
+                                                            double invL, const double* __restrict__ tab, int j0, int j1)
+    {
         constexpr double A = 1.4;
         constexpr double C0 = 1.0 / STEPS_FP64_FOLD - (1.0 - A) * (1.0 - A);
         const double cut2 = (2.6 * L) * (2.6 * L), halfL = 0.5 * L;
         const long long cut2_bits = __double_as_longlong(cut2);
 #pragma unroll 1
         for (int j = j0; j < j1; ++j) {
-            const double xj = T.x[j], yj = T.y[j], zj = T.z[j], mq = T.m[j], hj = T.h[j];
+            const double xj = Tx[j], yj = Ty[j], zj = Tz[j], mq = Tm[j], hj = Th[j];
             if (mq == 0.0) continue;                                   // pads and massless sources (warp-uniform)
             // px: sum over the images of s v, in units of 1 / STEPS_FP64_FOLD (the far body's r^-3 carries that factor)
             double dx[R_I], dy[R_I], dz[R_I], px[R_I], py[R_I], pz[R_I];

@@ -920,6 +920,221 @@ forces_sym_mixed_box_kernel(const TileF32* __restrict__ tiles, const SymPlan* __
     }
 }
 
+// ---- the pair-symmetric IMAGE SUM (Eq. 5 L65-70 with the 2.6 L cut, second part) ---------------
+// The image sum of a pair is antisymmetric like the pair force itself (the image set is symmetric under n -> -n), so every
+// far meeting of a warp's 128-particle group with a 128-source subgroup of another block is evaluated ONCE:
+// P_ij = sum over the images of (v w), v = (x_j - x_i) - n L, w = |v|^-3 inside the cut, and a_i += m_j P_ij, a_j -= m_i P_ij
+// -- one pass over the ~100 candidate images per unordered pair instead of two.  Items, rounds, hand-over of the
+// reaction sums round the warp, neighbour hand-over of the subgroups and records as in forces_sym_box_kernel; the
+// candidates of a meeting are pruned from the two groups' bounding boxes as in forces_boxring_kernel<Fp64Path, 2> (no
+// per-pair wrap: one lattice shift centres the box difference).  Meetings that may hold a softened pair (pair_decision)
+// are skipped and evaluated by forces_boxgen_kernel<Fp64Path, 2>, the groups' own blocks by the group-ring kernel.
+// The column block arrives as its tiles' PLAIN sources (x, y, z, m); the particles' sums live in shared memory.
+constexpr int SYM_IMG_NCUBE = 343, SYM_IMG_CAND_STRIDE = 352;
+__host__ __device__ constexpr int sym_img_smem_bytes() { return 4 * IB * (int)sizeof(double) + 2 * 3 * IB * (int)sizeof(double); }
+
+template <int THREADS, int RI, bool SPLIT>
+__global__ void __launch_bounds__(THREADS, 1)
+forces_sym_img_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__ plan, const GroupMeta* __restrict__ gm,
+                      long long k_begin, long long k_end, double* __restrict__ rowrec, double* __restrict__ colrec, int split_arg,
+                      double box_L, double box_invL)
+{
+    const int split = SPLIT ? split_arg : 1;
+    static_assert(THREADS * RI == IB && RI % 2 == 0, "the CTA holds one block; the particles are taken two at a time");
+    constexpr int WI = 32 * RI, SUBG = THREADS / 32;
+    static_assert(WI == WARP_I && WI * 2 == TJ, "a warp's particles are one group of GroupMeta = half a tile");
+    constexpr double A = 1.4;
+    constexpr double C0 = 1.0 / STEPS_FP64_FOLD - (1.0 - A) * (1.0 - A);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ uint64_t full_bar;
+    __shared__ double cube_tab[3 * SYM_IMG_NCUBE];                                 // offsets n L, n in [-3, 3]^3
+    __shared__ unsigned short cand_all[SUBG * SYM_IMG_CAND_STRIDE];                // per warp: the candidates of its meeting
+    __shared__ int round_done[SUBG];
+    double* col = reinterpret_cast<double*>(smem_raw);                             // [TPB][x, y, z, m][TJ]
+    double* Bsm = col + 4 * IB;                                                    // [3][IB]
+    double* Asm = Bsm + 3 * IB + threadIdx.x;                                      // [3][RI][THREADS], this thread's column
+    for (int q = threadIdx.x; q < SYM_IMG_NCUBE; q += THREADS) {
+        cube_tab[3 * q] = (double)(q % 7 - 3) * box_L; cube_tab[3 * q + 1] = (double)((q / 7) % 7 - 3) * box_L;
+        cube_tab[3 * q + 2] = (double)(q / 49 - 3) * box_L;
+    }
+    if (threadIdx.x < SUBG) round_done[threadIdx.x] = 0;
+
+    const long long K = plan->K * split;
+    if (k_end > K) k_end = K;
+    if (k_begin >= k_end) return;
+    const int nb = plan->nb, Km = plan->Km;     // W = 0: item (b, c) for every c > b
+    const long long n_items = k_end - k_begin;
+    const long long kk0 = k_begin + (long long)blockIdx.x * n_items / gridDim.x;
+    const long long kk1 = k_begin + ((long long)blockIdx.x + 1) * n_items / gridDim.x;
+    const int total = (int)(kk1 - kk0);
+    if (total <= 0) return;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    int b, c;
+    {
+        const double t = 2.0 * Km + 1.0;
+        const long long item0 = kk0 / split;
+        int bb = (int)((t - sqrt(fmax(t * t - 8.0 * (double)item0, 0.0))) * 0.5);
+        bb = max(0, min(bb, Km - 1));
+        while (bb + 1 < Km && sym_row_start(bb + 1, Km) <= item0) ++bb;
+        while (bb > 0 && sym_row_start(bb, Km) > item0) --bb;
+        b = bb;
+        c = bb + 1 + (int)(item0 - sym_row_start(bb, Km));
+    }
+    if (threadIdx.x == 0) {
+        mbar_init(&full_bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    const int src_lane = (lane + 31) & 31;
+    const long long cut2_bits = __double_as_longlong((2.6 * box_L) * (2.6 * box_L));
+    const double cut2 = (2.6 * box_L) * (2.6 * box_L), eps = 1.0e-5 * box_L;
+    unsigned short* cand = cand_all + warp * SYM_IMG_CAND_STRIDE;
+
+    for (int it = 0; it < total; ++it) {
+        // the column block's plain sources: one stage (an item runs for milliseconds; the previous item's readers are past
+        // the barrier at its end)
+        if (threadIdx.x == 0) {
+            mbar_expect_tx(&full_bar, (uint32_t)(4 * IB * sizeof(double)));
+#pragma unroll
+            for (int t = 0; t < TPB; ++t)
+                bulk_load(col + t * 4 * TJ, &tiles[(long long)c * TPB + t].x[0], (uint32_t)(4 * TJ * sizeof(double)), &full_bar);
+        }
+#pragma unroll
+        for (int q = 0; q < 3 * RI; ++q) Asm[q * THREADS] = 0.0;
+        for (int q = threadIdx.x; q < 3 * IB; q += THREADS) Bsm[q] = 0.0;
+        mbar_wait(&full_bar, it & 1);
+        __syncthreads();
+
+        const uint32_t my_code = boxcode_pack(pair_decision<1>(gm, b * SUBG + warp, c * SUBG + (lane & (SUBG - 1)), box_L, box_invL), box_invL);
+        const int part = SPLIT ? (int)((kk0 + it) % split) : 0, rounds = SPLIT ? SUBG / split : SUBG;
+        const int base = it * rounds;
+        for (int q = part * rounds; q < (part + 1) * rounds; ++q) {
+            const int u = (warp + q) & (SUBG - 1);
+            if (q > part * rounds) {                          // subgroup u was warp + 1's in the round before (round_wait)
+                if (lane == 0) round_wait(&round_done[(warp + 1) & (SUBG - 1)], base + (q - part * rounds));
+                __syncwarp();
+            }
+            if (!(__shfl_sync(0xffffffffu, my_code, u) & BOXCODE_GENERAL)) {       // else: forces_boxgen_kernel<., 2> evaluates it
+                // the lattice shift that centres the box difference, and the candidates that come within the cut
+                const GroupMeta GI = gm[b * SUBG + warp], GJ = gm[c * SUBG + u];
+                double sh[3], lo3[3], hi3[3];
+#pragma unroll
+                for (int cc = 0; cc < 3; ++cc) {
+                    const double dmin = ((double)GJ.lo[cc] - (double)GI.hi[cc]) - eps, dmax = ((double)GJ.hi[cc] - (double)GI.lo[cc]) + eps;
+                    sh[cc] = box_L * rint(0.5 * (dmin + dmax) * box_invL);
+                    lo3[cc] = dmin - sh[cc]; hi3[cc] = dmax - sh[cc];
+                }
+                int ncand = 0;
+                for (int q0 = 0; q0 < SYM_IMG_NCUBE; q0 += 32) {
+                    const int tq = q0 + lane;
+                    bool keep = false;
+                    if (tq < SYM_IMG_NCUBE) {
+                        double g2 = 0.0;
+#pragma unroll
+                        for (int cc = 0; cc < 3; ++cc) {
+                            const double o = cube_tab[3 * tq + cc];
+                            const double gap = fmax(0.0, fmax(lo3[cc] - o, o - hi3[cc]));
+                            g2 = fma(gap, gap, g2);
+                        }
+                        keep = g2 < cut2;
+                    }
+                    const unsigned m = __ballot_sync(0xffffffffu, keep);
+                    if (keep) cand[ncand + __popc(m & ((1u << lane) - 1u))] = (unsigned short)tq;
+                    ncand += __popc(m);
+                }
+                __syncwarp();
+                double xi[RI], yi[RI], zi[RI], mi[RI];
+#pragma unroll
+                for (int k = 0; k < RI; ++k) {
+                    const int i = warp * WI + lane + 32 * k;
+                    const TileF64& T = tiles[(long long)b * TPB + i / TJ];
+                    xi[k] = T.x[i % TJ] + sh[0]; yi[k] = T.y[i % TJ] + sh[1]; zi[k] = T.z[i % TJ] + sh[2];
+                    mi[k] = STEPS_FP64_FOLD * T.m[i % TJ];
+                }
+                for (int t = 0; t < WI / 32 && ncand > 0; ++t) {
+                    const int s0 = u * WI + t * 32;                                  // first source of the set, within the block
+                    double bx = 0.0, by = 0.0, bz = 0.0;
+#pragma unroll 1
+                    for (int st = 0; st < 32; ++st) {
+                        const int s = s0 + ((lane - st) & 31);
+                        const double* P = col + (s / TJ) * 4 * TJ + (s % TJ);
+                        const double xj = P[0], yj = P[TJ], zj = P[2 * TJ], mq = P[3 * TJ];
+                        if (mq != 0.0) {                                         // pads and massless sources add nothing
+                            const double mf = STEPS_FP64_FOLD * mq;
+#pragma unroll
+                            for (int k0 = 0; k0 < RI; k0 += 2) {
+                                double dx[2], dy[2], dz[2], px[2], py[2], pz[2];
+#pragma unroll
+                                for (int k = 0; k < 2; ++k) {
+                                    dx[k] = xj - xi[k0 + k]; dy[k] = yj - yi[k0 + k]; dz[k] = zj - zi[k0 + k];
+                                    px[k] = py[k] = pz[k] = 0.0;
+                                }
+                                double nox, noy, noz;
+                                { const int t3 = 3 * cand[0]; nox = cube_tab[t3]; noy = cube_tab[t3 + 1]; noz = cube_tab[t3 + 2]; }
+#pragma unroll 2
+                                for (int cq = 0; cq < ncand; ++cq) {
+                                    const double ox = nox, oy = noy, oz = noz;
+                                    { const int t3 = 3 * cand[min(cq + 1, ncand - 1)]; nox = cube_tab[t3]; noy = cube_tab[t3 + 1]; noz = cube_tab[t3 + 2]; }
+                                    double vx[2], vy[2], vz[2], r2[2], y0[2], y2[2], w[2];
+#pragma unroll
+                                    for (int k = 0; k < 2; ++k) { vx[k] = dx[k] - ox; vy[k] = dy[k] - oy; vz[k] = dz[k] - oz; }
+#pragma unroll
+                                    for (int k = 0; k < 2; ++k) r2[k] = fma(vz[k], vz[k], fma(vy[k], vy[k], vx[k] * vx[k]));
+#pragma unroll
+                                    for (int k = 0; k < 2; ++k) y0[k] = rsqrt_seed(r2[k]);
+#pragma unroll
+                                    for (int k = 0; k < 2; ++k) {
+                                        y2[k] = y0[k] * y0[k];
+                                        w[k] = fma(r2[k], y2[k], -A);
+                                        y2[k] = y0[k] * y2[k];
+                                        w[k] = fma(w[k], w[k], C0);
+                                        w[k] = y2[k] * w[k];
+                                        if (!(__double_as_longlong(r2[k]) < cut2_bits)) w[k] = 0.0;   // "|x - nL| < 2.6 L", strict
+                                    }
+#pragma unroll
+                                    for (int k = 0; k < 2; ++k) {
+                                        px[k] = fma(vx[k], w[k], px[k]); py[k] = fma(vy[k], w[k], py[k]); pz[k] = fma(vz[k], w[k], pz[k]);
+                                    }
+                                }
+#pragma unroll
+                                for (int k = 0; k < 2; ++k) {                     // a_i += m_j P (in shared memory), b_j += m_i P
+                                    Asm[(0 * RI + k0 + k) * THREADS] += mf * px[k];
+                                    Asm[(1 * RI + k0 + k) * THREADS] += mf * py[k];
+                                    Asm[(2 * RI + k0 + k) * THREADS] += mf * pz[k];
+                                    bx = fma(mi[k0 + k], px[k], bx); by = fma(mi[k0 + k], py[k], by); bz = fma(mi[k0 + k], pz[k], bz);
+                                }
+                            }
+                        }
+                        bx = __shfl_sync(0xffffffffu, bx, src_lane);
+                        by = __shfl_sync(0xffffffffu, by, src_lane);
+                        bz = __shfl_sync(0xffffffffu, bz, src_lane);
+                    }
+                    const int j = s0 + lane;
+                    Bsm[j] += bx; Bsm[IB + j] += by; Bsm[2 * IB + j] += bz;
+                }
+            }
+            __syncwarp();
+            if (lane == 0) round_publish(&round_done[warp], base + (q - part * rounds) + 1);
+        }
+        __syncthreads();                                      // every subgroup's reaction sums are complete
+
+        const long long rec = (kk0 + it - k_begin) * 3 * IB;
+#pragma unroll
+        for (int k = 0; k < RI; ++k) {
+            const int i = warp * WI + lane + 32 * k;
+#pragma unroll
+            for (int cc = 0; cc < 3; ++cc) rowrec[rec + cc * IB + i] = Asm[(cc * RI + k) * THREADS];
+        }
+        for (int j = threadIdx.x; j < IB; j += THREADS) {      // the reaction: a_j -= sum_i m_i P_ij
+            colrec[rec + j] = -Bsm[j]; colrec[rec + IB + j] = -Bsm[IB + j]; colrec[rec + 2 * IB + j] = -Bsm[2 * IB + j];
+        }
+        __syncthreads();                                      // the column stage, Asm and Bsm are free again
+        if ((kk0 + it + 1) % split == 0 && ++c == nb) { ++b; c = b + 1; }
+    }
+}
+
 // acc (double-double, SoA over all N particles) += the records of one panel, in fixed order; `last` writes acc_out = hi + lo.
 __global__ void __launch_bounds__(256)
 forces_sym_reduce_kernel(const SymPlan* __restrict__ plan, const double* __restrict__ rowrec, const double* __restrict__ colrec,

@@ -579,6 +579,65 @@ int launch_forces_box(const double* pos, const double* mass, const double* soft,
     return STEPS_OK;
 }
 
+// Image sum (steps_forces_periodic) from 16 blocks: every far meeting of two groups of different blocks ONCE
+// (forces_sym_img_kernel: the image sum of a pair is antisymmetric), the possibly-softened units by
+// forces_boxgen_kernel<Fp64Path, 2>, the groups' own blocks by the group-ring kernel in restricted mode.
+int launch_forces_images_sym(const double* pos, const double* mass, const double* soft, long long N, double L, double* acc_out,
+                             cudaStream_t st, Workspace& w)
+{
+    using Path = Fp64Path;
+    using Tile = Path::Tile;
+    const int nb = (int)nblocks_of(N), nt = (int)ntiles_of(N);
+    const int ntp = nb * TPB, ngm = nb * (IB / SPLITJ_GROUP);
+    Tile* tiles = reinterpret_cast<Tile*>(w.tiles);
+    const long long groups = (N + SPLITJ_GROUP - 1) / SPLITJ_GROUP;
+    if (groups > 0x7fffffffll) return STEPS_EINVAL;
+    static int grid_img = 0, unused = 0;
+    int rc = persistent_grid(forces_sym_img_kernel<SYM_FP64_THREADS, SYM_FP64_RI, false>, sym_img_smem_bytes(), w, grid_img, SYM_FP64_THREADS);
+    if (rc == STEPS_OK && unused == 0)
+        rc = persistent_grid(forces_sym_img_kernel<SYM_FP64_THREADS, SYM_FP64_RI, true>, sym_img_smem_bytes(), w, unused, SYM_FP64_THREADS);
+    if (rc != STEPS_OK) return rc;
+    const int Ps = std::min(grid_img, w.num_sms);
+    int split = 1;
+    while (split < SYM_FP64_THREADS / 32 && sym_items_max(N) * split < 24ll * Ps) split *= 2;
+    auto ring = forces_boxring_kernel<Path, 2>;
+    auto gen = forces_boxgen_kernel<Path, 2>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        STEPS_CUDA(cudaFuncSetAttribute(ring, cudaFuncAttributeMaxDynamicSharedMemorySize, boxring_smem_bytes<Path, 2>()));
+        STEPS_CUDA(cudaFuncSetAttribute(gen, cudaFuncAttributeMaxDynamicSharedMemorySize, boxgen_smem_bytes<Path>()));
+        attr_set = true;
+    }
+    prep_tiles<Tile><<<ntp, TJ, 0, st>>>(pos, mass, soft, N, tiles, &w.plan->W);          // W = 0: every block pair is an item
+    group_meta_kernel<Tile><<<(ngm + 3) / 4, 128, 0, st>>>(pos, soft, N, tiles, w.gm, ngm);
+    sym_plan_finalize<<<1, 1024, 0, st>>>(w.plan, nb, 8 * Ps, split);
+    double* hi = w.acc_dd;
+    double* lo = w.acc_dd + 3 * N;
+    long long gsplit = std::max(1, g_box_gsplit.load());
+    while (gsplit > 1 && (size_t)groups * gsplit * 6 * SPLITJ_GROUP * sizeof(double) > sym_record_bytes(w.sym_panel_items)) gsplit /= 2;
+    gen<<<dim3((unsigned)groups, (unsigned)gsplit), CTA_THREADS, boxgen_smem_bytes<Path>(), st>>>(pos, soft, N, tiles, nt, hi, lo, w.sym_records,
+                                                                                                   L, 1.0 / L, w.gm, w.plan);
+    if (gsplit > 1) {
+        forces_splitj_reduce<<<(unsigned)groups, SPLITJ_GROUP, 0, st>>>(w.sym_records, (int)gsplit, N, hi, NO_FUSE, lo);
+        g_launches++;
+    }
+    ring<<<(unsigned)groups, CTA_THREADS, boxring_smem_bytes<Path, 2>(), st>>>(pos, soft, N, tiles, nt, hi, w.partials, 0, L, 1.0 / L, w.gm, w.plan, lo);
+    g_launches += 5;
+    const long long items = w.sym_panel_items, kmax = sym_items_max(N) * split;
+    double* rowrec = w.sym_records;
+    double* colrec = w.sym_records + (size_t)items * 3 * IB;
+    for (long long k0 = 0; k0 < kmax; k0 += items) {
+        const long long k1 = std::min(kmax, k0 + items);
+        auto k = split == 1 ? forces_sym_img_kernel<SYM_FP64_THREADS, SYM_FP64_RI, false> : forces_sym_img_kernel<SYM_FP64_THREADS, SYM_FP64_RI, true>;
+        k<<<Ps, SYM_FP64_THREADS, sym_img_smem_bytes(), st>>>(tiles, w.plan, w.gm, k0, k1, rowrec, colrec, split, L, 1.0 / L);
+        forces_sym_reduce_kernel<<<(int)((N + 255) / 256), 256, 0, st>>>(w.plan, rowrec, colrec, k0, k1, N, hi, lo, k1 == kmax ? 1 : 0, acc_out,
+                                                                          split, NO_FUSE);
+        g_launches += 2;
+    }
+    STEPS_CUDA(cudaGetLastError());
+    return STEPS_OK;
+}
+
 template <typename Path, int BOX>
 int launch_forces_periodic(const double* pos, const double* mass, const double* soft, long long N, double L, double* acc_out,
                            cudaStream_t st, Workspace& w)
@@ -588,17 +647,20 @@ int launch_forces_periodic(const double* pos, const double* mass, const double* 
     Tile* tiles = reinterpret_cast<Tile*>(w.tiles);
     int rc = claim_scratch(w, st);
     if (rc != STEPS_OK) return rc;
-    if constexpr (BOX != 1) {
-        prep_tiles<Tile><<<nt, TJ, 0, st>>>(pos, mass, soft, N, tiles, nullptr);
-        g_launches++;
-    }
     if constexpr (BOX == 1) {
         rc = launch_forces_box<Path>(pos, mass, soft, N, L, acc_out, st, w);
         if (rc != STEPS_OK) return rc;
         return release_scratch(w, st);
     } else {
+        if (g_driver.load() == 0 && sym_eligible(N, false) && w.sym_records) {
+            rc = launch_forces_images_sym(pos, mass, soft, N, L, acc_out, st, w);
+            if (rc != STEPS_OK) return rc;
+            return release_scratch(w, st);
+        }
         // Image sum: the group-ring driver with BOX = 2.  The tile range is split over `jsplit` CTAs so that the grid is
         // (close to) whole waves of one CTA per SM -- an image-sum CTA runs for milliseconds, a ragged last wave shows.
+        prep_tiles<Tile><<<nt, TJ, 0, st>>>(pos, mass, soft, N, tiles, nullptr);
+        g_launches++;
         const long long groups = (N + SPLITJ_GROUP - 1) / SPLITJ_GROUP;
         const long long jsplit = boxring_jsplit(groups, nt, N, w);
         if (groups > 0x7fffffffll) return STEPS_EINVAL;

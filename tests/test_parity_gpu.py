@@ -964,6 +964,50 @@ def test_periodic_image_sum_several_i_blocks_sampled(S, oracle):
     assert float(p.norm()) < 1e-12 * float((dm * acc.norm(dim=0)).sum())
 
 
+@pytest.mark.parametrize("n,ordered", [(32768, True), (40001, True), (32768, False)])
+def test_periodic_image_sum_pair_symmetric_route(S, oracle, n, ordered):
+    """From 16 blocks the image sum evaluates every far meeting of two groups of different blocks once
+    (forces_sym_img_kernel), the possibly-softened units through forces_boxgen_kernel<., 2>, the own blocks through the
+    group-ring kernel.  Against the oracle on a sample (unequal masses: a swapped m_i / m_j in the reaction would show;
+    some larger softenings; unordered input: everything through the unpruned route), equality with the one-sided
+    evaluation (option "sym" = 0), bit-identical re-run, Newton's third law."""
+    import torch
+    L = 1.3
+    pos, mass, soft = _periodic_box(n, L, 6700 + n)
+    rng = np.random.default_rng(n)
+    mass = mass * rng.uniform(0.5, 2.0, size=n)
+    mass /= mass.sum()
+    soft = soft * rng.uniform(0.5, 3.0, size=n)
+    if ordered:
+        pos = np.ascontiguousarray(pos[:, synth.morton_order(pos, L)])
+    dpos, dm, dh = dev(pos), dev(mass), dev(soft)
+    acc, again, one = (torch.empty(3, n, dtype=torch.float64, device="cuda") for _ in range(3))
+    S.steps_forces_periodic(dpos, dm, dh, L, acc)
+    if not ordered:                                             # (slow route: the oracle comparison is enough)
+        idx = np.linspace(0, n - 1, 24).astype(np.int64)
+    else:
+        S.steps_forces_periodic(dpos, dm, dh, L, again)
+        assert torch.equal(acc, again)
+        try:
+            S.steps_set_option("sym", 0)
+            S.steps_forces_periodic(dpos, dm, dh, L, one)
+        finally:
+            S.steps_set_option("sym", 1)
+        edges = np.concatenate([[b * 2048, min(n, (b + 1) * 2048) - 1] for b in range((n + 2047) // 2048)])
+        idx = np.unique(np.concatenate([edges, np.linspace(0, n - 1, 40).astype(np.int64)]))
+    got = acc.cpu().numpy()[:, idx]
+    ref = oracle.forces_periodic_images(pos, mass, soft, L, idx=idx)
+    scale = _pair_force_abs_sum(pos, mass, np.full(n, soft.min()), L, idx)
+    e_abs = np.linalg.norm(got - ref, axis=0) / scale
+    print(f"[image sum, pair-symmetric route n={n} ordered={ordered}, {len(idx)} sampled] relative to sum_j|f_ij|: max {e_abs.max():.3e}")
+    assert e_abs.max() <= 1e-12
+    if ordered:
+        d = np.linalg.norm((acc - one).cpu().numpy()[:, idx], axis=0) / scale
+        assert d.max() <= 1e-13, d.max()
+    p = (dm * acc).sum(dim=1)
+    assert float(p.norm()) < 1e-12 * float((dm * acc.norm(dim=0)).sum())
+
+
 def test_config4_lockstep_200_steps_8192(S, oracle):
     """Config 4 at N = 8192, every one of the 200 comoving KDK steps (a: 1/51 -> 1): the library steps
     from the ORACLE's state (x_n, v_n, acc_n) and must land on the oracle's (x_{n+1}, v_{n+1},
