@@ -218,9 +218,10 @@ int steps_forces_quasi_periodic(const double *pos, const double *mass, const dou
  * pair softening soft_i + soft_j; fp64 path only (the images of a homogeneous box cancel to a small remainder).  Layout,
  * G = 1 and error behaviour as steps_forces_quasi_periodic; the result does not depend on which representative modulo L
  * the positions are given in (|x_j - x_i| < 2^51 L).  Cost: 74 images per pair inside the cut on average; a pair on its
- * own needs 179 candidates (all n.n <= 12 around its leading image), a (128-particle group, tile) pair of cell-ordered
- * input whose bounding boxes are compact and cannot hold a softened pair is pruned to the ~90-110 candidates that come
- * within the cut for some pair of the two boxes.  A particle's OWN images (j = i, n != 0) are summed like any other pair's: the triplet set is symmetric under
+ * own needs 179 candidates (all n.n <= 12 around its leading image), a pair of 128-particle groups of cell-ordered input
+ * whose bounding boxes are compact and cannot hold a softened pair is pruned to the ~90-110 candidates that come within
+ * the cut for some pair of the two boxes, and from N = 30,721 such pairs of groups of two different blocks of 2,048
+ * particles are evaluated ONCE for both groups (the image sum of a pair is antisymmetric).  A particle's OWN images (j = i, n != 0) are summed like any other pair's: the triplet set is symmetric under
  * n -> -n, so they cancel to rounding (the oracle skips j = i altogether).  Softening up to h_i + h_j <= L/2 takes the
  * fast route (only the nearest image can then be softened); larger softening is handled image by image. */
 int steps_forces_periodic(const double *pos, const double *mass, const double *soft, long long N, double L,
