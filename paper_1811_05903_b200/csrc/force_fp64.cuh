@@ -326,28 +326,36 @@ struct Fp64Path {
                 px[k] = dx[k] * s0; py[k] = dy[k] * s0; pz[k] = dz[k] * s0;
             }
             if (__all_sync(0xffffffffu, newtonian)) {
-#pragma unroll 1
-                for (int c = 1; c < EWALD_NTRIPLETS; ++c) {
-                    const double ox = tab[3 * c], oy = tab[3 * c + 1], oz = tab[3 * c + 2];
-                    double vx[R_I], vy[R_I], vz[R_I], r2[R_I], y0[R_I], y2[R_I], w[R_I];
+                // the 178 other triplets, for two of the thread's particles at a time (as in far_images: all four at once
+                // exceed the registers and their dependent chains run one after the other)
+                constexpr int H = 2;
+                static_assert(R_I % H == 0, "whole passes");
 #pragma unroll
-                    for (int k = 0; k < R_I; ++k) { vx[k] = dx[k] - ox; vy[k] = dy[k] - oy; vz[k] = dz[k] - oz; }
+                for (int k0 = 0; k0 < R_I; k0 += H) {
+#pragma unroll 2
+                    for (int c = 1; c < EWALD_NTRIPLETS; ++c) {
+                        const double ox = tab[3 * c], oy = tab[3 * c + 1], oz = tab[3 * c + 2];
+                        double vx[H], vy[H], vz[H], r2[H], y0[H], y2[H], w[H];
 #pragma unroll
-                    for (int k = 0; k < R_I; ++k) r2[k] = fma(vz[k], vz[k], fma(vy[k], vy[k], vx[k] * vx[k]));
+                        for (int k = 0; k < H; ++k) { vx[k] = dx[k0 + k] - ox; vy[k] = dy[k0 + k] - oy; vz[k] = dz[k0 + k] - oz; }
 #pragma unroll
-                    for (int k = 0; k < R_I; ++k) y0[k] = rsqrt_seed(r2[k]);
+                        for (int k = 0; k < H; ++k) r2[k] = fma(vz[k], vz[k], fma(vy[k], vy[k], vx[k] * vx[k]));
 #pragma unroll
-                    for (int k = 0; k < R_I; ++k) {
-                        y2[k] = y0[k] * y0[k];
-                        w[k] = fma(r2[k], y2[k], -A);
-                        y2[k] = y0[k] * y2[k];
-                        w[k] = fma(w[k], w[k], C0);
-                        w[k] = y2[k] * w[k];
-                        if (!(__double_as_longlong(r2[k]) < cut2_bits)) w[k] = 0.0;   // "|x - nL| < 2.6 L", strict (r2 >= 0)
-                    }
+                        for (int k = 0; k < H; ++k) y0[k] = rsqrt_seed(r2[k]);
 #pragma unroll
-                    for (int k = 0; k < R_I; ++k) {
-                        px[k] = fma(vx[k], w[k], px[k]); py[k] = fma(vy[k], w[k], py[k]); pz[k] = fma(vz[k], w[k], pz[k]);
+                        for (int k = 0; k < H; ++k) {
+                            y2[k] = y0[k] * y0[k];
+                            w[k] = fma(r2[k], y2[k], -A);
+                            y2[k] = y0[k] * y2[k];
+                            w[k] = fma(w[k], w[k], C0);
+                            w[k] = y2[k] * w[k];
+                            if (!(__double_as_longlong(r2[k]) < cut2_bits)) w[k] = 0.0;   // "|x - nL| < 2.6 L", strict (r2 >= 0)
+                        }
+#pragma unroll
+                        for (int k = 0; k < H; ++k) {
+                            px[k0 + k] = fma(vx[k], w[k], px[k0 + k]); py[k0 + k] = fma(vy[k], w[k], py[k0 + k]);
+                            pz[k0 + k] = fma(vz[k], w[k], pz[k0 + k]);
+                        }
                     }
                 }
             } else {                                                   // some h_i + h_j > L/2: every image through Eq. 4
