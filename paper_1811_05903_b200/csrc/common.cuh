@@ -196,6 +196,23 @@ __device__ __forceinline__ BoxShift pair_decision(const GroupMeta* __restrict__ 
     return d;
 }
 
+// Whether the boxes of the groups a and b span (nearly) a whole period in some component, or one of them is empty: then no
+// common lattice shift centres their separations.  Boxes in index order, like pair_decision: the kernels that split the
+// meetings between them by this test agree bit for bit.
+template <int GRAN>
+__device__ __forceinline__ bool pair_too_wide(const GroupMeta* __restrict__ gm, int a, int b, double L)
+{
+    const GroupMeta A = group_box<GRAN>(gm, a < b ? a : b), B = group_box<GRAN>(gm, a < b ? b : a);
+    const double eps = 1.0e-5 * L;
+    bool wide = false;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const double dmin = ((double)B.lo[c] - (double)A.hi[c]) - eps, dmax = ((double)B.hi[c] - (double)A.lo[c]) + eps;
+        wide = wide || !(dmax - dmin < 0.999 * L) || !(dmax >= dmin);
+    }
+    return wide;
+}
+
 // The fold of one separation component: e - copysign(h, e) as (|e| - h) with the sign of e (h = half the period, in the
 // units of e).  One DADD (|e| is an operand modifier) and one LOP3 on the high word.
 __device__ __forceinline__ double fold_f64(double e, double h)

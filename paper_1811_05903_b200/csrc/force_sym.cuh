@@ -927,11 +927,14 @@ forces_sym_mixed_box_kernel(const TileF32* __restrict__ tiles, const SymPlan* __
 // -- one pass over the ~100 candidate images per unordered pair instead of two.  Items, rounds, hand-over of the
 // reaction sums round the warp, neighbour hand-over of the subgroups and records as in forces_sym_box_kernel; the
 // candidates of a meeting are pruned from the two groups' bounding boxes as in forces_boxring_kernel<Fp64Path, 2> (no
-// per-pair wrap: one lattice shift centres the box difference).  Meetings that may hold a softened pair (pair_decision)
-// are skipped and evaluated by forces_boxgen_kernel<Fp64Path, 2>, the groups' own blocks by the group-ring kernel.
-// The column block arrives as its tiles' PLAIN sources (x, y, z, m); the particles' sums live in shared memory.
+// per-pair wrap: one lattice shift centres the box difference).  A candidate image whose lattice point comes closer to the
+// box of separations than the largest pair softening of the two groups MAY be softened: those few (usually none, or the
+// one nearest image of neighbouring groups) go through Eq. 4 in full per pair, all others through the branch-free body.
+// Only meetings whose boxes span a whole period (pair_too_wide: groups that straddle a jump of the cell order) are skipped
+// and evaluated by forces_boxgen_kernel<Fp64Path, 2>; the groups' own blocks by the group-ring kernel.
+// The column block arrives as its tiles' PLAIN sources (x, y, z, m, h); the particles' sums live in shared memory.
 constexpr int SYM_IMG_NCUBE = 343, SYM_IMG_CAND_STRIDE = 352;
-__host__ __device__ constexpr int sym_img_smem_bytes() { return 4 * IB * (int)sizeof(double) + 2 * 3 * IB * (int)sizeof(double); }
+__host__ __device__ constexpr int sym_img_smem_bytes() { return 5 * IB * (int)sizeof(double) + 2 * 3 * IB * (int)sizeof(double); }
 
 template <int THREADS, int RI, bool SPLIT>
 __global__ void __launch_bounds__(THREADS, 1)
@@ -950,8 +953,8 @@ forces_sym_img_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restri
     __shared__ double cube_tab[3 * SYM_IMG_NCUBE];                                 // offsets n L, n in [-3, 3]^3
     __shared__ unsigned short cand_all[SUBG * SYM_IMG_CAND_STRIDE];                // per warp: the candidates of its meeting
     __shared__ int round_done[SUBG];
-    double* col = reinterpret_cast<double*>(smem_raw);                             // [TPB][x, y, z, m][TJ]
-    double* Bsm = col + 4 * IB;                                                    // [3][IB]
+    double* col = reinterpret_cast<double*>(smem_raw);                             // [TPB][x, y, z, m, h][TJ]
+    double* Bsm = col + 5 * IB;                                                    // [3][IB]
     double* Asm = Bsm + 3 * IB + threadIdx.x;                                      // [3][RI][THREADS], this thread's column
     for (int q = threadIdx.x; q < SYM_IMG_NCUBE; q += THREADS) {
         cube_tab[3 * q] = (double)(q % 7 - 3) * box_L; cube_tab[3 * q + 1] = (double)((q / 7) % 7 - 3) * box_L;
@@ -996,10 +999,10 @@ forces_sym_img_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restri
         // the column block's plain sources: one stage (an item runs for milliseconds; the previous item's readers are past
         // the barrier at its end)
         if (threadIdx.x == 0) {
-            mbar_expect_tx(&full_bar, (uint32_t)(4 * IB * sizeof(double)));
+            mbar_expect_tx(&full_bar, (uint32_t)(5 * IB * sizeof(double)));
 #pragma unroll
             for (int t = 0; t < TPB; ++t)
-                bulk_load(col + t * 4 * TJ, &tiles[(long long)c * TPB + t].x[0], (uint32_t)(4 * TJ * sizeof(double)), &full_bar);
+                bulk_load(col + t * 5 * TJ, &tiles[(long long)c * TPB + t].x[0], (uint32_t)(5 * TJ * sizeof(double)), &full_bar);
         }
 #pragma unroll
         for (int q = 0; q < 3 * RI; ++q) Asm[q * THREADS] = 0.0;
@@ -1007,7 +1010,7 @@ forces_sym_img_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restri
         mbar_wait(&full_bar, it & 1);
         __syncthreads();
 
-        const uint32_t my_code = boxcode_pack(pair_decision<1>(gm, b * SUBG + warp, c * SUBG + (lane & (SUBG - 1)), box_L, box_invL), box_invL);
+        const bool my_skip = pair_too_wide<1>(gm, b * SUBG + warp, c * SUBG + (lane & (SUBG - 1)), box_L);
         const int part = SPLIT ? (int)((kk0 + it) % split) : 0, rounds = SPLIT ? SUBG / split : SUBG;
         const int base = it * rounds;
         for (int q = part * rounds; q < (part + 1) * rounds; ++q) {
@@ -1016,7 +1019,7 @@ forces_sym_img_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restri
                 if (lane == 0) round_wait(&round_done[(warp + 1) & (SUBG - 1)], base + (q - part * rounds));
                 __syncwarp();
             }
-            if (!(__shfl_sync(0xffffffffu, my_code, u) & BOXCODE_GENERAL)) {       // else: forces_boxgen_kernel<., 2> evaluates it
+            if (!__shfl_sync(0xffffffffu, (int)my_skip, u)) {                      // else: forces_boxgen_kernel<., 2> evaluates it
                 // the lattice shift that centres the box difference, and the candidates that come within the cut
                 const GroupMeta GI = gm[b * SUBG + warp], GJ = gm[c * SUBG + u];
                 double sh[3], lo3[3], hi3[3];
@@ -1026,10 +1029,12 @@ forces_sym_img_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restri
                     sh[cc] = box_L * rint(0.5 * (dmin + dmax) * box_invL);
                     lo3[cc] = dmin - sh[cc]; hi3[cc] = dmax - sh[cc];
                 }
-                int ncand = 0;
+                // candidates that may be softened go to the back of the list
+                const double need = ((double)GI.hmax + (double)GJ.hmax) * 1.0001 + eps, need2 = need * need;
+                int ncand = 0, nsoft = 0;
                 for (int q0 = 0; q0 < SYM_IMG_NCUBE; q0 += 32) {
                     const int tq = q0 + lane;
-                    bool keep = false;
+                    bool keep = false, softq = false;
                     if (tq < SYM_IMG_NCUBE) {
                         double g2 = 0.0;
 #pragma unroll
@@ -1038,28 +1043,30 @@ forces_sym_img_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restri
                             const double gap = fmax(0.0, fmax(lo3[cc] - o, o - hi3[cc]));
                             g2 = fma(gap, gap, g2);
                         }
-                        keep = g2 < cut2;
+                        softq = g2 < cut2 && !(g2 > need2);
+                        keep = g2 < cut2 && !softq;
                     }
-                    const unsigned m = __ballot_sync(0xffffffffu, keep);
+                    const unsigned m = __ballot_sync(0xffffffffu, keep), ms = __ballot_sync(0xffffffffu, softq);
                     if (keep) cand[ncand + __popc(m & ((1u << lane) - 1u))] = (unsigned short)tq;
-                    ncand += __popc(m);
+                    if (softq) cand[SYM_IMG_CAND_STRIDE - 1 - (nsoft + __popc(ms & ((1u << lane) - 1u)))] = (unsigned short)tq;
+                    ncand += __popc(m); nsoft += __popc(ms);
                 }
                 __syncwarp();
-                double xi[RI], yi[RI], zi[RI], mi[RI];
+                double xi[RI], yi[RI], zi[RI], mi[RI], hi[RI];
 #pragma unroll
                 for (int k = 0; k < RI; ++k) {
                     const int i = warp * WI + lane + 32 * k;
                     const TileF64& T = tiles[(long long)b * TPB + i / TJ];
                     xi[k] = T.x[i % TJ] + sh[0]; yi[k] = T.y[i % TJ] + sh[1]; zi[k] = T.z[i % TJ] + sh[2];
-                    mi[k] = STEPS_FP64_FOLD * T.m[i % TJ];
+                    mi[k] = STEPS_FP64_FOLD * T.m[i % TJ]; hi[k] = T.h[i % TJ];
                 }
-                for (int t = 0; t < WI / 32 && ncand > 0; ++t) {
+                for (int t = 0; t < WI / 32 && ncand + nsoft > 0; ++t) {
                     const int s0 = u * WI + t * 32;                                  // first source of the set, within the block
                     double bx = 0.0, by = 0.0, bz = 0.0;
 #pragma unroll 1
                     for (int st = 0; st < 32; ++st) {
                         const int s = s0 + ((lane - st) & 31);
-                        const double* P = col + (s / TJ) * 4 * TJ + (s % TJ);
+                        const double* P = col + (s / TJ) * 5 * TJ + (s % TJ);
                         const double xj = P[0], yj = P[TJ], zj = P[2 * TJ], mq = P[3 * TJ];
                         if (mq != 0.0) {                                         // pads and massless sources add nothing
                             const double mf = STEPS_FP64_FOLD * mq;
@@ -1071,8 +1078,8 @@ forces_sym_img_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restri
                                     dx[k] = xj - xi[k0 + k]; dy[k] = yj - yi[k0 + k]; dz[k] = zj - zi[k0 + k];
                                     px[k] = py[k] = pz[k] = 0.0;
                                 }
-                                double nox, noy, noz;
-                                { const int t3 = 3 * cand[0]; nox = cube_tab[t3]; noy = cube_tab[t3 + 1]; noz = cube_tab[t3 + 2]; }
+                                double nox = 0.0, noy = 0.0, noz = 0.0;
+                                if (ncand > 0) { const int t3 = 3 * cand[0]; nox = cube_tab[t3]; noy = cube_tab[t3 + 1]; noz = cube_tab[t3 + 2]; }
 #pragma unroll 2
                                 for (int cq = 0; cq < ncand; ++cq) {
                                     const double ox = nox, oy = noy, oz = noz;
@@ -1096,6 +1103,25 @@ forces_sym_img_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restri
 #pragma unroll
                                     for (int k = 0; k < 2; ++k) {
                                         px[k] = fma(vx[k], w[k], px[k]); py[k] = fma(vy[k], w[k], py[k]); pz[k] = fma(vz[k], w[k], pz[k]);
+                                    }
+                                }
+                                if (nsoft > 0) {                                  // the images that may be softened: Eq. 4 in full
+                                    const double hj = P[4 * TJ];
+#pragma unroll 1
+                                    for (int cq = 0; cq < nsoft; ++cq) {
+                                        const int t3 = 3 * cand[SYM_IMG_CAND_STRIDE - 1 - cq];
+                                        const double ox = cube_tab[t3], oy = cube_tab[t3 + 1], oz = cube_tab[t3 + 2];
+#pragma unroll
+                                        for (int k = 0; k < 2; ++k) {
+                                            const double vx = dx[k] - ox, vy = dy[k] - oy, vz = dz[k] - oz;
+                                            const double r2 = fma(vz, vz, fma(vy, vy, vx * vx));
+                                            const double hs = hi[k0 + k] + hj;
+                                            double sq = Fp64Path::rcube(r2);
+                                            if (r2 < hs * hs || r2 == 0.0) sq = (r2 == 0.0) ? 0.0 : spline_g_soft_f64(r2, hs);   // readings #2, #4
+                                            if (!(r2 < cut2)) sq = 0.0;
+                                            sq *= 1.0 / STEPS_FP64_FOLD;
+                                            px[k] = fma(vx, sq, px[k]); py[k] = fma(vy, sq, py[k]); pz[k] = fma(vz, sq, pz[k]);
+                                        }
                                     }
                                 }
 #pragma unroll
