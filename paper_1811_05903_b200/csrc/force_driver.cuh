@@ -867,9 +867,14 @@ forces_boxgen_kernel(const double* __restrict__ pos, const double* __restrict__ 
         auto wanted = [&](int q) {
             if (q >= cnt) return false;
             const int u = u0 + q;
-            if ((int)(((long long)u * UNIT) / IB) == my_block) return false;       // own block: forces_boxring_kernel
-            if constexpr (BOX == 2) return pair_too_wide<GRAN>(gm, me, u, box_L);     // the image-sum kernel softens in place
-            else return (boxcode_pack(pair_decision<GRAN>(gm, me, u, box_L, box_invL), box_invL) & BOXCODE_GENERAL) != 0;
+            if constexpr (BOX == 2) {
+                // the image-sum kernel softens in place and takes the groups' own blocks as well (diagonal items): left are the
+                // group's meeting with itself and the meetings whose boxes span a period
+                return u == me || pair_too_wide<GRAN>(gm, me, u, box_L);
+            } else {
+                if ((int)(((long long)u * UNIT) / IB) == my_block) return false;   // own block: forces_boxring_kernel
+                return (boxcode_pack(pair_decision<GRAN>(gm, me, u, box_L, box_invL), box_invL) & BOXCODE_GENERAL) != 0;
+            }
         };
         // (thread-interleaved: a CTA's share of a group is usually a few hundred units, one decision per thread; the list
         // is in unit order: the offsets come from the (round, warp) counts)

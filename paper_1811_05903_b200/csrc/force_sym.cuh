@@ -940,8 +940,13 @@ template <int THREADS, int RI, bool SPLIT>
 __global__ void __launch_bounds__(THREADS, 1)
 forces_sym_img_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__ plan, const GroupMeta* __restrict__ gm,
                       long long k_begin, long long k_end, double* __restrict__ rowrec, double* __restrict__ colrec, int split_arg,
-                      double box_L, double box_invL)
+                      double box_L, double box_invL, int diag)
 {
+    // diag != 0: the items are the blocks THEMSELVES, (b, b), b = 0 ... nb - 1: of the two meetings of an unordered pair of
+    // groups {w, u} of the block -- warp w with subgroup u, warp u with subgroup w -- the one with (u - w) mod 16 < 8 is
+    // evaluated (at distance 8 the one with w < u): every warp has 7 or 8 meetings, each pair of groups is evaluated once.
+    // A group's meeting with itself (and whatever pair_too_wide leaves out) is forces_boxgen_kernel's.  Both records of
+    // such an item belong to block b (forces_sym_diag_reduce).
     const int split = SPLIT ? split_arg : 1;
     static_assert(THREADS * RI == IB && RI % 2 == 0, "the CTA holds one block; the particles are taken two at a time");
     constexpr int WI = 32 * RI, SUBG = THREADS / 32;
@@ -962,10 +967,10 @@ forces_sym_img_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restri
     }
     if (threadIdx.x < SUBG) round_done[threadIdx.x] = 0;
 
-    const long long K = plan->K * split;
+    const int nb = plan->nb, Km = plan->Km;     // W = 0: item (b, c) for every c > b
+    const long long K = (diag ? (plan->K > 0 ? (long long)nb : 0ll) : plan->K) * split;
     if (k_end > K) k_end = K;
     if (k_begin >= k_end) return;
-    const int nb = plan->nb, Km = plan->Km;     // W = 0: item (b, c) for every c > b
     const long long n_items = k_end - k_begin;
     const long long kk0 = k_begin + (long long)blockIdx.x * n_items / gridDim.x;
     const long long kk1 = k_begin + ((long long)blockIdx.x + 1) * n_items / gridDim.x;
@@ -974,7 +979,9 @@ forces_sym_img_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restri
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     int b, c;
-    {
+    if (diag) {
+        b = c = (int)(kk0 / split);
+    } else {
         const double t = 2.0 * Km + 1.0;
         const long long item0 = kk0 / split;
         int bb = (int)((t - sqrt(fmax(t * t - 8.0 * (double)item0, 0.0))) * 0.5);
@@ -1010,7 +1017,12 @@ forces_sym_img_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restri
         mbar_wait(&full_bar, it & 1);
         __syncthreads();
 
-        const bool my_skip = pair_too_wide<1>(gm, b * SUBG + warp, c * SUBG + (lane & (SUBG - 1)), box_L);
+        bool my_skip;
+        {
+            const int uu = lane & (SUBG - 1), dist = (uu - warp) & (SUBG - 1);
+            if (diag && (dist == 0 || dist > SUBG / 2 || (dist == SUBG / 2 && warp > uu))) my_skip = true;   // the other meeting's, or the group itself
+            else my_skip = pair_too_wide<1>(gm, b * SUBG + warp, c * SUBG + uu, box_L);
+        }
         const int part = SPLIT ? (int)((kk0 + it) % split) : 0, rounds = SPLIT ? SUBG / split : SUBG;
         const int base = it * rounds;
         for (int q = part * rounds; q < (part + 1) * rounds; ++q) {
@@ -1157,7 +1169,36 @@ forces_sym_img_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restri
             colrec[rec + j] = -Bsm[j]; colrec[rec + IB + j] = -Bsm[IB + j]; colrec[rec + 2 * IB + j] = -Bsm[2 * IB + j];
         }
         __syncthreads();                                      // the column stage, Asm and Bsm are free again
-        if ((kk0 + it + 1) % split == 0 && ++c == nb) { ++b; c = b + 1; }
+        if ((kk0 + it + 1) % split == 0) {
+            if (diag) { ++b; c = b; }
+            else if (++c == nb) { ++b; c = b + 1; }
+        }
+    }
+}
+
+// The records of the diagonal items of forces_sym_img_kernel (item b, `split` parts: both records are block b's) added to
+// the double-double result in fixed order.
+__global__ void __launch_bounds__(256)
+forces_sym_diag_reduce(const SymPlan* __restrict__ plan, const double* __restrict__ rowrec, const double* __restrict__ colrec, int split,
+                       long long N, double* __restrict__ acc_hi, double* __restrict__ acc_lo)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N || plan->K <= 0) return;
+    const int b = (int)(i / IB), off = (int)(i - (long long)b * IB);
+#pragma unroll
+    for (int cc = 0; cc < 3; ++cc) {
+        double hi = acc_hi[cc * N + i], lo = acc_lo[cc * N + i];
+        for (int p = 0; p < split; ++p) {
+            const long long at = ((long long)b * split + p) * 3 * IB + (long long)cc * IB + off;
+#pragma unroll
+            for (int r = 0; r < 2; ++r) {
+                const double v = r == 0 ? rowrec[at] : colrec[at];
+                const double s = hi + v, bb = s - hi;
+                lo += (hi - (s - bb)) + (v - bb);              // TwoSum
+                hi = s;
+            }
+        }
+        acc_hi[cc * N + i] = hi; acc_lo[cc * N + i] = lo;
     }
 }
 

@@ -600,17 +600,15 @@ int launch_forces_images_sym(const double* pos, const double* mass, const double
     const int Ps = std::min(grid_img, w.num_sms);
     int split = 1;
     while (split < SYM_FP64_THREADS / 32 && sym_items_max(N) * split < 24ll * Ps) split *= 2;
-    auto ring = forces_boxring_kernel<Path, 2>;
     auto gen = forces_boxgen_kernel<Path, 2>;
     static bool attr_set = false;
     if (!attr_set) {
-        STEPS_CUDA(cudaFuncSetAttribute(ring, cudaFuncAttributeMaxDynamicSharedMemorySize, boxring_smem_bytes<Path, 2>()));
         STEPS_CUDA(cudaFuncSetAttribute(gen, cudaFuncAttributeMaxDynamicSharedMemorySize, boxgen_smem_bytes<Path>()));
         attr_set = true;
     }
     prep_tiles<Tile><<<ntp, TJ, 0, st>>>(pos, mass, soft, N, tiles, &w.plan->W);          // W = 0: every block pair is an item
     group_meta_kernel<Tile><<<(ngm + 3) / 4, 128, 0, st>>>(pos, soft, N, tiles, w.gm, ngm);
-    sym_plan_finalize<<<1, 1024, 0, st>>>(w.plan, nb, 8 * Ps, split);
+    sym_plan_finalize<<<1, 1024, 0, st>>>(w.plan, nb, 0, split);                        // (no minimum: this route has no one-sided fallback kernel)
     double* hi = w.acc_dd;
     double* lo = w.acc_dd + 3 * N;
     long long gsplit = std::max(1, g_box_gsplit.load());
@@ -621,15 +619,22 @@ int launch_forces_images_sym(const double* pos, const double* mass, const double
         forces_splitj_reduce<<<(unsigned)groups, SPLITJ_GROUP, 0, st>>>(w.sym_records, (int)gsplit, N, hi, NO_FUSE, lo);
         g_launches++;
     }
-    ring<<<(unsigned)groups, CTA_THREADS, boxring_smem_bytes<Path, 2>(), st>>>(pos, soft, N, tiles, nt, hi, w.partials, 0, L, 1.0 / L, w.gm, w.plan, lo);
-    g_launches += 5;
+    g_launches += 4;
     const long long items = w.sym_panel_items, kmax = sym_items_max(N) * split;
     double* rowrec = w.sym_records;
     double* colrec = w.sym_records + (size_t)items * 3 * IB;
+    auto k = split == 1 ? forces_sym_img_kernel<SYM_FP64_THREADS, SYM_FP64_RI, false> : forces_sym_img_kernel<SYM_FP64_THREADS, SYM_FP64_RI, true>;
+    // the blocks themselves (diagonal items: every pair of groups of a block once), then the block pairs, panel by panel
+    if ((long long)nb * split <= items) {
+        k<<<Ps, SYM_FP64_THREADS, sym_img_smem_bytes(), st>>>(tiles, w.plan, w.gm, 0, (long long)nb * split, rowrec, colrec, split, L, 1.0 / L, 1);
+        forces_sym_diag_reduce<<<(int)((N + 255) / 256), 256, 0, st>>>(w.plan, rowrec, colrec, split, N, hi, lo);
+        g_launches += 2;
+    } else {
+        return STEPS_EINVAL;                         // (sym_panel_items set below the number of blocks)
+    }
     for (long long k0 = 0; k0 < kmax; k0 += items) {
         const long long k1 = std::min(kmax, k0 + items);
-        auto k = split == 1 ? forces_sym_img_kernel<SYM_FP64_THREADS, SYM_FP64_RI, false> : forces_sym_img_kernel<SYM_FP64_THREADS, SYM_FP64_RI, true>;
-        k<<<Ps, SYM_FP64_THREADS, sym_img_smem_bytes(), st>>>(tiles, w.plan, w.gm, k0, k1, rowrec, colrec, split, L, 1.0 / L);
+        k<<<Ps, SYM_FP64_THREADS, sym_img_smem_bytes(), st>>>(tiles, w.plan, w.gm, k0, k1, rowrec, colrec, split, L, 1.0 / L, 0);
         forces_sym_reduce_kernel<<<(int)((N + 255) / 256), 256, 0, st>>>(w.plan, rowrec, colrec, k0, k1, N, hi, lo, k1 == kmax ? 1 : 0, acc_out,
                                                                           split, NO_FUSE);
         g_launches += 2;
