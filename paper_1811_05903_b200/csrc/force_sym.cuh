@@ -931,7 +931,8 @@ forces_sym_mixed_box_kernel(const TileF32* __restrict__ tiles, const SymPlan* __
 // box of separations than the largest pair softening of the two groups MAY be softened: those few (usually none, or the
 // one nearest image of neighbouring groups) go through Eq. 4 in full per pair, all others through the branch-free body.
 // Only meetings whose boxes span a whole period (pair_too_wide: groups that straddle a jump of the cell order) are skipped
-// and evaluated by forces_boxgen_kernel<Fp64Path, 2>; the groups' own blocks by the group-ring kernel.
+// and evaluated by forces_boxgen_kernel<Fp64Path, 2>, like every group's meeting with itself; the groups' own blocks are
+// the diagonal items of this kernel (`diag`).
 // The column block arrives as its tiles' PLAIN sources (x, y, z, m, h); the particles' sums live in shared memory.
 constexpr int SYM_IMG_NCUBE = 343, SYM_IMG_CAND_STRIDE = 352;
 __host__ __device__ constexpr int sym_img_smem_bytes() { return 5 * IB * (int)sizeof(double) + 2 * 3 * IB * (int)sizeof(double); }
