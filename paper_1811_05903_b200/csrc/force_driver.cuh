@@ -161,18 +161,38 @@ constexpr int persistent_smem_bytes()
 
 // ---- band mode (force_sym.cuh) ---------------------------------------------------------------------
 // Device-resident plan of a pair-symmetric force evaluation (written by sym_band_width + sym_plan_finalize in force_sym.cuh).
-// In BAND mode the persistent driver only visits, for i-block b, the tiles of the blocks c with |c - b| <= W; the far block
-// pairs beyond the band are the work items of forces_sym_kernel.
+// Row b's band is the blocks lo[b] ... edge[b]: edge[b] >= b is the last block that is not provably far from b or from an
+// earlier row (made non-decreasing in b, so that the band is symmetric: c <= edge[b]  <=>  b >= lo[c] for b <= c), and
+// lo[c] = the first row whose edge reaches c.  In BAND mode the persistent driver only visits, for i-block b, the tiles of
+// its band; the block pairs (b, c) with c > edge[b] are the work items of forces_sym_kernel, row after row.
 struct SymPlan {
-    int W;            // band half-width in blocks of IB particles
+    int W;            // widest band: max (edge[b] - b); nb - 1 = no symmetric items
     int nb;           // blocks
-    int Km;           // rows that own symmetric items: max(0, nb - 1 - W)
+    int Km;           // rows that own symmetric items (rows 0 ... Km - 1: edge[b] < nb - 1)
     int nt;           // j-tiles, padded to whole blocks: nb * (IB / TJ)
-    long long K;      // symmetric items: Km (Km + 1) / 2
+    long long K;      // symmetric items: rowstart[nb]
     long long T;      // band tile visits: cum[nb]
 };
-// followed in memory by  long long cum[nb + 1]: band tile visits of the rows before b
+// followed in memory by  long long cum[nb + 1]: band tile visits of the rows before b,
+//                        long long rowstart[nb + 1]: symmetric items of the rows before b,  int edge[nb],  int lo[nb]
+__host__ __device__ inline size_t sym_plan_bytes(long long nb)
+{
+    return sizeof(SymPlan) + 2 * sizeof(long long) * (size_t)(nb + 1) + 2 * sizeof(int) * (size_t)nb;
+}
 __device__ __forceinline__ const long long* plan_cum(const SymPlan* plan) { return reinterpret_cast<const long long*>(plan + 1); }
+__device__ __forceinline__ const long long* plan_rowstart(const SymPlan* plan, int nb) { return plan_cum(plan) + nb + 1; }
+__device__ __forceinline__ const int* plan_edge(const SymPlan* plan, int nb) { return reinterpret_cast<const int*>(plan_rowstart(plan, nb) + nb + 1); }
+__device__ __forceinline__ const int* plan_lo(const SymPlan* plan, int nb) { return plan_edge(plan, nb) + nb; }
+// the row of symmetric item k: the largest b < Km with rowstart[b] <= k
+__device__ __forceinline__ int sym_row_of(const long long* __restrict__ rowstart, int Km, long long k)
+{
+    int lo = 0, hi = max(Km - 1, 0);
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (rowstart[mid] <= k) lo = mid; else hi = mid - 1;
+    }
+    return lo;
+}
 // row b of the band with cum[b] <= w < cum[b + 1]
 __device__ __forceinline__ int band_row_of(const long long* __restrict__ cum, int nb, long long w)
 {
@@ -182,6 +202,22 @@ __device__ __forceinline__ int band_row_of(const long long* __restrict__ cum, in
         if (cum[mid] <= w) lo = mid; else hi = mid - 1;
     }
     return lo;
+}
+
+// The item list of the symmetric kernels (kept out of line: the kernels' register allocation is tuned to the body, and the
+// lookups run once per CTA / once per row).  Item k is the block pair (b, c): b = its row, c = edge[b] + 1 + (k - rowstart[b]).
+__device__ __noinline__ int2 sym_item_decode(const SymPlan* plan, long long k)
+{
+    const int nb = plan->nb;
+    const long long* rowstart = plan_rowstart(plan, nb);
+    const int b = sym_row_of(rowstart, plan->Km, k);
+    return make_int2(b, plan_edge(plan, nb)[b] + 1 + (int)(k - rowstart[b]));
+}
+// the column of the first item of row b
+__device__ __noinline__ int sym_row_first_col(const SymPlan* plan, int b)
+{
+    const int nb = plan->nb;
+    return plan_edge(plan, nb)[min(b, nb - 1)] + 1;
 }
 
 // ---- persistent stream-K driver ------------------------------------------------------------------
@@ -209,7 +245,6 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
     double* acc = reinterpret_cast<double*>(smem_raw + STAGES * STRIDE) + threadIdx.x;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const long long* cum = BAND ? plan_cum(plan) : nullptr;
-    const int bandW = BAND ? plan->W : 0;
     const long long Wall = BAND ? plan->T : (long long)nb * nt;
     const long long R0 = BAND ? Wall * share_rank / share_world : 0, R1 = BAND ? Wall * (share_rank + 1) / share_world : Wall;
     const long long W = R1 - R0;
@@ -233,7 +268,7 @@ forces_persistent_kernel(const double* __restrict__ pos, const double* __restric
         long long tile;
         if constexpr (BAND) {                                   // band mode: row of the linear index, then its tile
             const int pb = band_row_of(cum, nb, w0 + k);
-            tile = (long long)max(0, pb - bandW) * (IB / TJ) + (w0 + k - cum[pb]);
+            tile = (long long)plan_lo(plan, nb)[pb] * (IB / TJ) + (w0 + k - cum[pb]);
         } else {
             tile = (w0 + k) % nt;
         }
@@ -410,9 +445,9 @@ forces_splitj_kernel(const double* __restrict__ pos, const double* __restrict__ 
     const int per_tile = TJ / sub;
     int t_lo = 0, t_hi = nt;                                                // the tiles this group meets
     if (plan != nullptr) {
-        const int b = (int)(((long long)blockIdx.x * SPLITJ_GROUP) / IB), W = plan->W;
-        t_lo = max(0, b - W) * (IB / TJ);
-        t_hi = min(nt, (int)min((long long)plan->nb, (long long)b + W + 1) * (IB / TJ));
+        const int b = (int)(((long long)blockIdx.x * SPLITJ_GROUP) / IB), pnb = plan->nb;
+        t_lo = plan_lo(plan, pnb)[b] * (IB / TJ);
+        t_hi = min(nt, (plan_edge(plan, pnb)[b] + 1) * (IB / TJ));
     }
     const long long units = (long long)(t_hi - t_lo) * per_tile;
     const long long u0 = (long long)blockIdx.y * units / gridDim.y, u1 = ((long long)blockIdx.y + 1) * units / gridDim.y;

@@ -64,56 +64,109 @@ __device__ __forceinline__ BlockMeta block_meta(const Tile* __restrict__ tiles, 
     return m;
 }
 
-// W = max |c - b| over the block pairs that are not far.  plan->W must be 0 on entry (prep_tiles resets it).
+// edge[b] (raw) = the last block c >= b that is not far from block b; plan->W = the largest c - b (plan->W must be 0 on
+// entry: prep_tiles resets it).
 template <typename Tile>
 __global__ void __launch_bounds__(128) sym_band_width(const Tile* __restrict__ tiles, int nb, SymPlan* __restrict__ plan)
 {
     const int b = blockIdx.x;
     const BlockMeta I = block_meta(tiles, b);
-    int far_from = 0;
-    for (int c = threadIdx.x; c < nb; c += blockDim.x) {
+    int last = b;
+    for (int c = b + 1 + threadIdx.x; c < nb; c += blockDim.x) {
         const BlockMeta J = block_meta(tiles, c);
         const TileMeta Jm{J.rmin, J.rmax, J.hmax, 0.0f};
-        if (!tile_is_far(I.rmin, I.rmax, I.hmax, Jm)) far_from = max(far_from, abs(c - b));
+        if (!tile_is_far(I.rmin, I.rmax, I.hmax, Jm)) last = max(last, c);
     }
+    // a block that holds massless or unscalable particles (hmax = +inf) is not far from anything, ITSELF included: its own
+    // row must reach the last block too
+    if (!(I.hmax < __int_as_float(0x7f800000))) last = nb - 1;
+    __shared__ int wmax[4];
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) far_from = max(far_from, __shfl_xor_sync(0xffffffffu, far_from, o));
-    if ((threadIdx.x & 31) == 0 && far_from > 0) atomicMax(&plan->W, far_from);
+    for (int o = 16; o > 0; o >>= 1) last = max(last, __shfl_xor_sync(0xffffffffu, last, o));
+    if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = last;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        last = max(max(wmax[0], wmax[1]), max(wmax[2], wmax[3]));
+        const_cast<int*>(plan_edge(plan, nb))[b] = last;
+        if (last > b) atomicMax(&plan->W, last - b);
+    }
 }
 
-// One CTA: the item count and the band's cumulative tile counts from W.
-__global__ void __launch_bounds__(1024) sym_plan_finalize(SymPlan* __restrict__ plan, int nb, int sym_min_items, int split)
+// One CTA: the plan's arrays.  per_row != 0: edge[] holds sym_band_width's raw edges (made non-decreasing here);
+// per_row == 0: every row's band is plan->W blocks to either side (the periodic routes: W = 0, every block pair an item).
+__global__ void __launch_bounds__(1024) sym_plan_finalize(SymPlan* __restrict__ plan, int nb, int sym_min_items, int split, int per_row)
 {
     long long* cum = reinterpret_cast<long long*>(plan + 1);
-    __shared__ long long part[1024];
-    __shared__ int sW;
-    if (threadIdx.x == 0) {
-        int W = plan->W;
-        long long Km = nb - 1 - W;
-        if (Km < 0) Km = 0;
-        // too few items to balance over the SMs: everything through the band (W = nb - 1)
-        if (Km * (Km + 1) / 2 * split < sym_min_items) { W = nb - 1; Km = 0; }
-        plan->W = W; plan->nb = nb; plan->Km = (int)Km; plan->nt = nb * TPB; plan->K = Km * (Km + 1) / 2;
-        sW = W;
-    }
-    __syncthreads();
-    const int W = sW;
+    long long* rowstart = cum + nb + 1;
+    int* edge = reinterpret_cast<int*>(rowstart + nb + 1);
+    int* lo = edge + nb;
+    __shared__ long long part[1024], part2[1024];
+    __shared__ int pmax[1024];
+    __shared__ int all_band;
     const int per = (nb + blockDim.x - 1) / blockDim.x;
     const int b0 = min(nb, (int)threadIdx.x * per), b1 = min(nb, b0 + per);
-    auto width = [&](int b) { return (long long)(min(nb - 1, b + W) - max(0, b - W) + 1) * TPB; };
-    long long s = 0;
-    for (int b = b0; b < b1; ++b) s += width(b);
-    part[threadIdx.x] = s;
+    const int W0 = plan->W;
+    auto raw = [&](int b) { return per_row ? edge[b] : min(nb - 1, b + W0); };
+
+    // running maximum of the raw edges: chunk maxima, their exclusive scan (thread 0), then each chunk again
+    int m = 0;
+    for (int b = b0; b < b1; ++b) m = max(m, raw(b));
+    pmax[threadIdx.x] = m;
     __syncthreads();
     if (threadIdx.x == 0) {
-        long long run = 0;
-        for (int t = 0; t < (int)blockDim.x; ++t) { const long long v = part[t]; part[t] = run; run += v; }
-        plan->T = run;
-        cum[nb] = run;
+        int run = 0;
+        for (int t = 0; t < (int)blockDim.x; ++t) { const int v = pmax[t]; pmax[t] = run; run = max(run, v); }
     }
     __syncthreads();
-    s = part[threadIdx.x];
-    for (int b = b0; b < b1; ++b) { cum[b] = s; s += width(b); }
+    m = pmax[threadIdx.x];
+    long long items = 0;
+    for (int b = b0; b < b1; ++b) { m = max(m, raw(b)); edge[b] = m; items += nb - 1 - m; }
+    part[threadIdx.x] = items;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        long long K = 0;
+        for (int t = 0; t < (int)blockDim.x; ++t) K += part[t];
+        // too few items to balance over the SMs: everything through the band
+        all_band = K * split < sym_min_items ? 1 : 0;
+    }
+    __syncthreads();
+    if (all_band)
+        for (int b = b0; b < b1; ++b) edge[b] = nb - 1;
+    __syncthreads();                                          // edge[] complete (global writes of this CTA, read below)
+
+    // lo[c] = the first row whose edge reaches c (edge[] is non-decreasing, edge[c] >= c)
+    for (int c = b0; c < b1; ++c) {
+        int l = 0, h = c;
+        while (l < h) {
+            const int mid = (l + h) >> 1;
+            if (edge[mid] >= c) h = mid; else l = mid + 1;
+        }
+        lo[c] = l;
+    }
+    __syncthreads();
+    long long s = 0;
+    items = 0;
+    int wmax = 0;
+    for (int b = b0; b < b1; ++b) { s += (long long)(edge[b] - lo[b] + 1) * TPB; items += nb - 1 - edge[b]; wmax = max(wmax, edge[b] - b); }
+    part[threadIdx.x] = s; part2[threadIdx.x] = items; pmax[threadIdx.x] = wmax;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        long long run = 0, run2 = 0;
+        int W = 0;
+        for (int t = 0; t < (int)blockDim.x; ++t) {
+            const long long v = part[t], v2 = part2[t];
+            part[t] = run; part2[t] = run2; run += v; run2 += v2; W = max(W, pmax[t]);
+        }
+        cum[nb] = run; rowstart[nb] = run2;
+        plan->W = W; plan->nb = nb; plan->nt = nb * TPB; plan->K = run2; plan->T = run;
+        plan->Km = nb > 0 ? lo[nb - 1] : 0;                  // rows before the first one whose band reaches the last block
+    }
+    __syncthreads();
+    s = part[threadIdx.x]; items = part2[threadIdx.x];
+    for (int b = b0; b < b1; ++b) {
+        cum[b] = s; rowstart[b] = items;
+        s += (long long)(edge[b] - lo[b] + 1) * TPB; items += nb - 1 - edge[b];
+    }
 }
 
 __host__ __device__ constexpr int sym_smem_bytes() { return 2 * IB * (int)sizeof(FarSrcF64) + 3 * IB * (int)sizeof(double); }
@@ -148,7 +201,7 @@ forces_sym_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__
     k_begin += S0; k_end += S0;
     if (k_end > K) k_end = K;
     if (k_begin >= k_end) return;
-    const int W = plan->W, nb = plan->nb, Km = plan->Km;
+    const int nb = plan->nb;
     const long long n_items = k_end - k_begin;
     const long long kk0 = k_begin + (long long)blockIdx.x * n_items / gridDim.x;
     const long long kk1 = k_begin + ((long long)blockIdx.x + 1) * n_items / gridDim.x;
@@ -156,17 +209,11 @@ forces_sym_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__
     if (total <= 0) return;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    // decode the first item: row b = the largest b with sym_row_start(b) <= kk0
+    // decode the first item: row b = the largest b with rowstart[b] <= kk0
     int b, c;
     {
-        const double t = 2.0 * Km + 1.0;
-        const long long item0 = kk0 / split;
-        int bb = (int)((t - sqrt(fmax(t * t - 8.0 * (double)item0, 0.0))) * 0.5);
-        bb = max(0, min(bb, Km - 1));
-        while (bb + 1 < Km && sym_row_start(bb + 1, Km) <= item0) ++bb;
-        while (bb > 0 && sym_row_start(bb, Km) > item0) --bb;
-        b = bb;
-        c = bb + W + 1 + (int)(item0 - sym_row_start(bb, Km));
+        const int2 bc = sym_item_decode(plan, kk0 / split);
+        b = bc.x; c = bc.y;
     }
 
     if (threadIdx.x == 0) {
@@ -184,7 +231,7 @@ forces_sym_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__
         for (int t = 0; t < TPB; ++t)
             bulk_load(col + (size_t)s * IB + t * TJ, &tiles[(long long)pc * TPB + t].far[0], (uint32_t)(TJ * sizeof(FarSrcF64)),
                       &full_bar[s]);
-        if ((kk0 + it + 1) % split == 0 && ++pc == nb) { ++pb; pc = pb + W + 1; }     // the next sub-item starts a new item
+        if ((kk0 + it + 1) % split == 0 && ++pc == nb) { ++pb; pc = sym_row_first_col(plan, pb); }     // the next sub-item starts a new item
     };
     if (threadIdx.x == 0) {
         produce(0);
@@ -291,7 +338,7 @@ forces_sym_kernel(const TileF64* __restrict__ tiles, const SymPlan* __restrict__
         }
         __syncthreads();                                          // stage s and Bsm are free again
         if (threadIdx.x == 0 && it + 2 < total) produce(it + 2);
-        if ((kk0 + it + 1) % split == 0 && ++c == nb) { ++b; c = b + W + 1; }
+        if ((kk0 + it + 1) % split == 0 && ++c == nb) { ++b; c = sym_row_first_col(plan, b); }
     }
 }
 
@@ -341,7 +388,7 @@ forces_sym_mixed_kernel(const TileF32* __restrict__ tiles, const SymPlan* __rest
     k_begin += S0; k_end += S0;
     if (k_end > K) k_end = K;
     if (k_begin >= k_end) return;
-    const int W = plan->W, nb = plan->nb, Km = plan->Km;
+    const int nb = plan->nb;
     const long long n_items = k_end - k_begin;
     const long long kk0 = k_begin + (long long)blockIdx.x * n_items / gridDim.x;
     const long long kk1 = k_begin + ((long long)blockIdx.x + 1) * n_items / gridDim.x;
@@ -351,14 +398,8 @@ forces_sym_mixed_kernel(const TileF32* __restrict__ tiles, const SymPlan* __rest
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     int b, c;
     {
-        const double t = 2.0 * Km + 1.0;
-        const long long item0 = kk0 / split;
-        int bb = (int)((t - sqrt(fmax(t * t - 8.0 * (double)item0, 0.0))) * 0.5);
-        bb = max(0, min(bb, Km - 1));
-        while (bb + 1 < Km && sym_row_start(bb + 1, Km) <= item0) ++bb;
-        while (bb > 0 && sym_row_start(bb, Km) > item0) --bb;
-        b = bb;
-        c = bb + W + 1 + (int)(item0 - sym_row_start(bb, Km));
+        const int2 bc = sym_item_decode(plan, kk0 / split);
+        b = bc.x; c = bc.y;
     }
     if (threadIdx.x == 0) {
         mbar_init(&full_bar[0], 1); mbar_init(&full_bar[1], 1);
@@ -373,7 +414,7 @@ forces_sym_mixed_kernel(const TileF32* __restrict__ tiles, const SymPlan* __rest
         for (int t = 0; t < TPB; ++t)          // X[], Y[], Z[], c[] are the first 4 TJ floats of a tile record
             bulk_load(reinterpret_cast<unsigned char*>(col) + (size_t)s * STAGE + t * (4 * TJ * sizeof(float)),
                       &tiles[(long long)pc * TPB + t].X[0], (uint32_t)(4 * TJ * sizeof(float)), &full_bar[s]);
-        if ((kk0 + it + 1) % split == 0 && ++pc == nb) { ++pb; pc = pb + W + 1; }     // the next sub-item starts a new item
+        if ((kk0 + it + 1) % split == 0 && ++pc == nb) { ++pb; pc = sym_row_first_col(plan, pb); }     // the next sub-item starts a new item
     };
     if (threadIdx.x == 0) {
         produce(0);
@@ -475,7 +516,7 @@ forces_sym_mixed_kernel(const TileF32* __restrict__ tiles, const SymPlan* __rest
         }
         __syncthreads();
         if (threadIdx.x == 0 && it + 2 < total) produce(it + 2);
-        if ((kk0 + it + 1) % split == 0 && ++c == nb) { ++b; c = b + W + 1; }
+        if ((kk0 + it + 1) % split == 0 && ++c == nb) { ++b; c = sym_row_first_col(plan, b); }
     }
 }
 
@@ -1217,7 +1258,9 @@ forces_sym_reduce_kernel(const SymPlan* __restrict__ plan, const double* __restr
     const long long S0 = Kall * share_rank / share_world, K = Kall * (share_rank + 1) / share_world;
     k_begin += S0; k_end += S0;
     if (k_end > K) k_end = K;
-    const int W = plan->W, Km = plan->Km;
+    const int Km = plan->Km, pnb = plan->nb;
+    const long long* rowstart = plan_rowstart(plan, pnb);
+    const int* edge = plan_edge(plan, pnb);
     const int b = (int)(i / IB), off = (int)(i - (long long)b * IB);
     double hi[3], lo[3];
 #pragma unroll
@@ -1234,12 +1277,15 @@ forces_sym_reduce_kernel(const SymPlan* __restrict__ plan, const double* __restr
     };
     if (k_begin < k_end) {
         if (b < Km) {                                              // this block as the row of its items
-            const long long r0 = sym_row_start(b, Km) * split, r1 = r0 + (long long)(Km - b) * split;
+            const long long r0 = rowstart[b] * split, r1 = rowstart[b + 1] * split;
             for (long long k = max(r0, k_begin); k < min(r1, k_end); ++k) add(rowrec, k);
         }
-        const int rows = min(Km, b - W);                           // this block as the column of item (bb, b), bb + W < b
-        for (int bb = 0; bb < rows; ++bb) {
-            const long long k0 = (sym_row_start(bb, Km) + (b - bb - W - 1)) * split;
+        // this block as the column of item (bb, b): the rows bb with edge[bb] < b, i.e. bb < lo[b]; of those, the rows
+        // that have items inside [k_begin, k_end)
+        const int rows = min(Km, plan_lo(plan, pnb)[b]);
+        const int bb_first = sym_row_of(rowstart, Km, k_begin / split), bb_last = sym_row_of(rowstart, Km, (k_end - 1) / split);
+        for (int bb = bb_first; bb < min(rows, bb_last + 1); ++bb) {
+            const long long k0 = (rowstart[bb] + (b - edge[bb] - 1)) * split;
             for (long long k = max(k0, k_begin); k < min(k0 + split, k_end); ++k) add(colrec, k);
         }
     }

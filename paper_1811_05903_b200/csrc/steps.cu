@@ -65,7 +65,7 @@ struct Workspace {
     void* tiles = nullptr;          // max(sizeof(TileF32), sizeof(TileF64)) * ntiles (padded to whole blocks)
     double* partials = nullptr;     // (nb + grid) * 6 * IB doubles (persistent driver's split-j records)
     long long cap_particles = 0;
-    SymPlan* plan = nullptr;        // SymPlan + cum[nb + 1]
+    SymPlan* plan = nullptr;        // SymPlan + its arrays (sym_plan_bytes)
     GroupMeta* gm = nullptr;        // one per 128 particles, padded to whole blocks (periodic pair-symmetric evaluation)
     double* acc_dd = nullptr;       // 6 N doubles: (hi, lo) of the band result, the symmetric records are added to it
     double* sym_records = nullptr;  // 2 * panel_items * 3 * IB doubles (row records, then column records)
@@ -162,7 +162,7 @@ int ensure_workspace(int dev, long long N, cudaStream_t st)
         w.tiles = nullptr; w.partials = nullptr; w.plan = nullptr; w.gm = nullptr; w.cap_particles = 0;
         if (cudaMalloc(&w.tiles, tile_bytes_max() * (size_t)ntiles_padded(N)) != cudaSuccess ||
             cudaMalloc(&w.partials, partial_bytes(N)) != cudaSuccess ||
-            cudaMalloc(&w.plan, sizeof(SymPlan) + sizeof(long long) * (size_t)(nblocks_of(N) + 1)) != cudaSuccess ||
+            cudaMalloc(&w.plan, sym_plan_bytes(nblocks_of(N))) != cudaSuccess ||
             cudaMalloc(&w.gm, sizeof(GroupMeta) * (size_t)nblocks_of(N) * (IB / SPLITJ_GROUP)) != cudaSuccess) {
             cudaGetLastError();
             cudaFree(w.tiles); cudaFree(w.partials); cudaFree(w.plan); w.tiles = nullptr; w.partials = nullptr; w.plan = nullptr;
@@ -269,7 +269,7 @@ int launch_forces_sym(const double* pos, const double* mass, const double* soft,
 
     prep_tiles<Tile><<<ntp, TJ, 0, st>>>(pos, mass, soft, N, tiles, &w.plan->W);
     sym_band_width<Tile><<<nb, 128, 0, st>>>(tiles, nb, w.plan);
-    sym_plan_finalize<<<1, 1024, 0, st>>>(w.plan, nb, 8 * Ps, split);
+    sym_plan_finalize<<<1, 1024, 0, st>>>(w.plan, nb, 8 * Ps, split, 1);
     if (prof) STEPS_CUDA(cudaEventRecord(w.ev0, st));
     double* hi = w.acc_dd;
     double* lo = w.acc_dd + 3 * N;
@@ -536,7 +536,7 @@ int launch_forces_box(const double* pos, const double* mass, const double* soft,
     }
     prep_tiles<Tile><<<ntp, TJ, 0, st>>>(pos, mass, soft, N, tiles, &w.plan->W);          // W = 0: every block pair is an item
     group_meta_kernel<Tile><<<(ngm + 3) / 4, 128, 0, st>>>(pos, soft, N, tiles, w.gm, ngm);
-    sym_plan_finalize<<<1, 1024, 0, st>>>(w.plan, nb, 8 * Ps, split);
+    sym_plan_finalize<<<1, 1024, 0, st>>>(w.plan, nb, 8 * Ps, split, 0);
     if (prof) STEPS_CUDA(cudaEventRecord(w.ev0, st));
     double* hi = w.acc_dd;
     double* lo = w.acc_dd + 3 * N;
@@ -608,7 +608,7 @@ int launch_forces_images_sym(const double* pos, const double* mass, const double
     }
     prep_tiles<Tile><<<ntp, TJ, 0, st>>>(pos, mass, soft, N, tiles, &w.plan->W);          // W = 0: every block pair is an item
     group_meta_kernel<Tile><<<(ngm + 3) / 4, 128, 0, st>>>(pos, soft, N, tiles, w.gm, ngm);
-    sym_plan_finalize<<<1, 1024, 0, st>>>(w.plan, nb, 0, split);                        // (no minimum: this route has no one-sided fallback kernel)
+    sym_plan_finalize<<<1, 1024, 0, st>>>(w.plan, nb, 0, split, 0);                      // (no minimum: this route has no one-sided fallback kernel)
     double* hi = w.acc_dd;
     double* lo = w.acc_dd + 3 * N;
     long long gsplit = std::max(1, g_box_gsplit.load());
@@ -1126,7 +1126,7 @@ long long steps_workspace_bytes(long long N)
 {
     if (N < 1) return 0;
     size_t bytes = tile_bytes_max() * (size_t)ntiles_padded(N) + partial_bytes(N) + sizeof(double) * MOM_BLOCKS * 4 +
-                   sizeof(SymPlan) + sizeof(long long) * (size_t)(nblocks_of(N) + 1) +
+                   sym_plan_bytes(nblocks_of(N)) +
                    sizeof(GroupMeta) * (size_t)nblocks_of(N) * (IB / SPLITJ_GROUP);
     if (sym_eligible(N)) bytes += sizeof(double) * 6 * (size_t)N + sym_record_bytes(sym_panel_items_for(N));
     return (long long)bytes;

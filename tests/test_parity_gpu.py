@@ -145,14 +145,20 @@ def test_config3_one_million_sampled(S, oracle, mixed):
 
 
 @pytest.mark.parametrize("mixed", [False, True], ids=["fp64", "mixed"])
-@pytest.mark.parametrize("case", ["ragged", "unsorted", "massless", "stale_order", "one_sided"])
+@pytest.mark.parametrize("case", ["ragged", "unsorted", "massless", "massless_mid", "stale_order", "one_sided"])
 def test_pair_symmetric_path_and_its_fallbacks(S, oracle, mixed, case):
     """N >= 131,072 takes the pair-symmetric route (band + every far block pair once).  Against the oracle on a sample:
     ragged     N = 150,001: the last block holds 497 particles, the rest of its tiles are pads;
-    unsorted   a random permutation: no block pair is far, the device sets W = nb - 1 and everything runs one-sided;
+    unsorted   a random permutation: no block pair is far, every row's band reaches the last block and everything runs
+               one-sided;
     massless   three tracer particles (m = 0): their reaction sums could not be divided by m_j, so their tiles are marked
-               and the device falls back in the same way -- the tracers still feel the others;
-    stale_order every particle moved radially by up to 3 % (an order several steps old): a wider band, W > 1;
+               and the device falls back in the same way (one of them sits in the first block) -- the tracers still feel
+               the others;
+    massless_mid one tracer in the middle block: that block is "not far" from any other, so the rows before it have bands
+               that reach it (rows of very different widths), the rows after it have no items, and only the block pairs
+               (b, c) with b before and c after the tracer's block stay symmetric items;
+    stale_order every particle moved radially by up to 3 % (an order several steps old): wider bands, different from row
+               to row;
     one_sided  the "sym" option off: the one-sided kernels at this size, same answer to rounding."""
     import torch
     n = 150001 if case == "ragged" else 139264
@@ -164,6 +170,8 @@ def test_pair_symmetric_path_and_its_fallbacks(S, oracle, mixed, case):
         pos, mass, soft = np.ascontiguousarray(pos[:, perm]), mass[perm].copy(), soft[perm].copy()
     elif case == "massless":
         mass[[5, n // 2, n - 3]] = 0.0
+    elif case == "massless_mid":
+        mass[n // 2] = 0.0
     elif case == "stale_order":
         pos = np.ascontiguousarray(pos * (1.0 + 0.03 * rng.uniform(-1.0, 1.0, size=n)))
     idx = np.unique(np.concatenate([synth.stratified_sample(n, 1536), [5, n // 2, n - 3]]))
