@@ -67,8 +67,9 @@ enum {
     STEPS_ECUDA = -2,        /* CUDA runtime / launch error (steps_last_cuda_error() has the code) */
     STEPS_EUNSUPPORTED = -3, /* current device is not sm_100 */
     STEPS_ENOMEM = -4,       /* workspace allocation failed */
-    STEPS_ECAPTURE = -5      /* the call would have to allocate workspace while its stream is being captured into a CUDA
+    STEPS_ECAPTURE = -5,     /* the call would have to allocate workspace while its stream is being captured into a CUDA
                                 graph: call steps_reserve(N) (and, for steps_forces_periodic, one un-captured call) first */
+    STEPS_ETOOLARGE = -6     /* steps_forces_static: N > STEPS_STATIC_MAX_N (its scratch is a fixed array) */
 };
 
 /* ---- force evaluation --------------------------------- */
@@ -84,6 +85,23 @@ enum {
  * The symmetric part needs 48 B per particle + up to 1.5 GiB of partial records (steps_workspace_bytes). */
 int steps_forces(const double *pos, const double *mass, const double *soft, long long N,
                  double *acc, steps_stream_t stream);
+
+/* steps_forces (fp64 path, same operation, same bar, same argument meaning) for callers that cannot allocate device
+ * memory: code under CUDA-graph capture, tight loops, harnesses that forbid cudaMalloc.  This call never calls cudaMalloc,
+ * cudaFree or an allocating library routine, on the first call or any later one.  Its scratch (the tile records of
+ * PAPER.md Eq. 3-4's sources and the split-j partial records) is a file-scope __device__ array of the library:
+ * STEPS_STATIC_SCRATCH_BYTES (about 2.6 MiB) that every GPU which loads the library holds until the process exits.
+ *   - N <= STEPS_STATIC_MAX_N = 16,384 (the range of the split-j driver, one 128-particle group per CTA); a larger N
+ *     returns STEPS_ETOOLARGE and launches nothing.  Use steps_reserve + steps_forces there.
+ *   - pos, mass, soft, acc: device pointers, caller-owned, as for steps_forces.  The result equals steps_forces' at the
+ *     same N (same kernels, same launch shape).
+ *   - Every call on a device shares the one array, which keeps the previous call's contents.  Nothing in it has to start
+ *     at zero: each call rewrites every record it later reads.  Calls that OVERLAP on the GPU (two streams, two host
+ *     threads, a captured graph replayed next to a live call) race on it: give them one stream or order them with events. */
+#define STEPS_STATIC_MAX_N 16384
+#define STEPS_STATIC_SCRATCH_BYTES 2755584
+int steps_forces_static(const double *pos, const double *mass, const double *soft, long long N,
+                        double *acc, steps_stream_t stream);
 
 /* mixed path: pair arithmetic in fp32 (the paper's GPU runs were single precision, L159),
  * per-tile fp32 partial sums flushed into fp64 accumulators.

@@ -687,6 +687,49 @@ int launch_forces_periodic(const double* pos, const double* mass, const double* 
 
 }  // namespace
 
+// ---- steps_forces_static: the fp64 split-j evaluation with its scratch in a file-scope device array (include/steps.h) ----
+// [ STATIC_TILES tile records | STATIC_RECORDS split-j partial records of 6 x 128 doubles ].  In HOST code the array's name
+// is a host-side stand-in, not a device address: static_scratch_of() asks the runtime for the address once per device.
+constexpr int STATIC_TILES = STEPS_STATIC_MAX_N / TJ;                        // 64
+constexpr int STATIC_RECORDS = 256;                                          // >= groups x jsplit (<= SMs of the device)
+constexpr size_t STATIC_TILE_BYTES = sizeof(TileF64) * STATIC_TILES;
+constexpr size_t STATIC_RECORD_BYTES = sizeof(double) * 6 * SPLITJ_GROUP;
+static_assert(STEPS_STATIC_MAX_N % TJ == 0 && STATIC_TILE_BYTES % 256 == 0, "the records start on a 256 B boundary");
+static_assert(STATIC_TILE_BYTES + STATIC_RECORD_BYTES * STATIC_RECORDS == STEPS_STATIC_SCRATCH_BYTES, "include/steps.h states the size");
+static __device__ __align__(256) unsigned char g_static_scratch[STEPS_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+struct StaticState {
+    unsigned char* scratch = nullptr;   // device address of g_static_scratch on this device
+    int num_sms = 0;
+    bool ready = false;
+};
+StaticState g_static[MAX_DEVICES];
+std::mutex g_static_mutex;
+
+// Once per device, with that device current: the array's device address, the SM count, the kernel's shared-memory opt-in.
+// Nothing here allocates device memory.
+int static_scratch_of(int dev, StaticState** out)
+{
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticState& s = g_static[dev];
+    if (!s.ready) {
+        void* ptr = nullptr;
+        STEPS_CUDA(cudaGetSymbolAddress(&ptr, g_static_scratch));
+        if (ptr == nullptr) return STEPS_ECUDA;
+        STEPS_CUDA(cudaDeviceGetAttribute(&s.num_sms, cudaDevAttrMultiProcessorCount, dev));
+        constexpr int smem = Fp64Path::NOUT * R_I * CTA_THREADS * (int)sizeof(double);
+        STEPS_CUDA(cudaFuncSetAttribute(forces_splitj_kernel<Fp64Path, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        s.scratch = static_cast<unsigned char*>(ptr);
+        s.ready = true;
+    }
+    *out = &s;
+    return STEPS_OK;
+}
+
+}  // namespace
+
 extern "C" {
 
 int steps_forces_quasi_periodic(const double* pos, const double* mass, const double* soft, long long N, double L,
@@ -731,6 +774,47 @@ int steps_forces_mixed(const double* pos, const double* mass, const double* soft
                        steps_stream_t stream)
 {
     return forces_impl(pos, mass, soft, N, 0, N, acc, 1, stream);
+}
+
+int steps_forces_static(const double* pos, const double* mass, const double* soft, long long N, double* acc,
+                        steps_stream_t stream)
+{
+    if (!pos || !mass || !soft || !acc || N < 1) return STEPS_EINVAL;
+    if (misaligned(pos) || misaligned(mass) || misaligned(soft) || misaligned(acc)) return STEPS_EINVAL;
+    if (N > STEPS_STATIC_MAX_N) return STEPS_ETOOLARGE;
+    int dev;
+    int rc = current_device(&dev);                       // (device query only: sm_100 or STEPS_EUNSUPPORTED)
+    if (rc != STEPS_OK) return rc;
+    StaticState* s = nullptr;
+    rc = static_scratch_of(dev, &s);
+    if (rc != STEPS_OK) return rc;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    TileF64* tiles = reinterpret_cast<TileF64*>(s->scratch);
+    double* records = reinterpret_cast<double*>(s->scratch + STATIC_TILE_BYTES);
+
+    // the launch shape of launch_splitj<Fp64Path, 0> at this N (one wave: groups x jsplit <= SMs), so the result is
+    // steps_forces' at the same N
+    const int nt = (int)ntiles_of(N);
+    const long long groups = (N + SPLITJ_GROUP - 1) / SPLITJ_GROUP;
+    const long long warps = (long long)s->num_sms * (CTA_THREADS / 32);
+    int sub = TJ;
+    while (sub > 64 && groups * nt * (TJ / sub) < 4 * warps) sub /= 2;
+    const long long units = (long long)nt * (TJ / sub);
+    long long jsplit = groups < s->num_sms ? s->num_sms / groups : 1;
+    jsplit = std::max(1ll, std::min(jsplit, units / (CTA_THREADS / 32)));
+    if (groups * jsplit > STATIC_RECORDS) jsplit = std::max(1ll, STATIC_RECORDS / groups);
+    constexpr int smem = Fp64Path::NOUT * R_I * CTA_THREADS * (int)sizeof(double);
+
+    prep_tiles<TileF64><<<nt, TJ, 0, st>>>(pos, mass, soft, N, tiles, nullptr);
+    forces_splitj_kernel<Fp64Path, 0><<<dim3((unsigned)groups, (unsigned)jsplit), CTA_THREADS, smem, st>>>(
+        pos, soft, N, tiles, nt, sub, 0, N, acc, records, 0, 0.0, 0.0, NO_FUSE, nullptr, nullptr);
+    g_launches += 2;
+    if (jsplit > 1) {
+        forces_splitj_reduce<<<(unsigned)groups, SPLITJ_GROUP, 0, st>>>(records, (int)jsplit, N, acc, NO_FUSE);
+        g_launches++;
+    }
+    STEPS_CUDA(cudaGetLastError());
+    return STEPS_OK;
 }
 
 int steps_forces_range(const double* pos, const double* mass, const double* soft, long long N, long long i_begin,
@@ -1141,6 +1225,7 @@ const char* steps_strerror(int code)
         case STEPS_EUNSUPPORTED: return "device is not compute capability 10.x (sm_100a build, no fallback)";
         case STEPS_ENOMEM: return "workspace allocation failed";
         case STEPS_ECAPTURE: return "workspace must be allocated (steps_reserve) before the stream is captured into a CUDA graph";
+        case STEPS_ETOOLARGE: return "steps_forces_static: N exceeds STEPS_STATIC_MAX_N = 16384 (fixed scratch array); use steps_reserve + steps_forces";
         default: return "unknown error code";
     }
 }

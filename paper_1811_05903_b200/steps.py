@@ -11,10 +11,11 @@ import os
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsteps_b200.so")
 
-OK, EINVAL, ECUDA, EUNSUPPORTED, ENOMEM, ECAPTURE = 0, -1, -2, -3, -4, -5
+OK, EINVAL, ECUDA, EUNSUPPORTED, ENOMEM, ECAPTURE, ETOOLARGE = 0, -1, -2, -3, -4, -5, -6
+STATIC_MAX_N = 16384    # steps_forces_static (STEPS_STATIC_MAX_N of include/steps.h)
 
 EXPORTS = [
-    "steps_forces", "steps_forces_mixed", "steps_forces_range", "steps_forces_blocks", "steps_forces_share", "steps_block_size", "steps_forces_host", "steps_kick_drift",
+    "steps_forces", "steps_forces_static", "steps_forces_mixed", "steps_forces_range", "steps_forces_blocks", "steps_forces_share", "steps_block_size", "steps_forces_host", "steps_kick_drift",
     "steps_sort_radial", "steps_permute", "steps_near_fraction",
     "steps_kdk_step", "steps_hubble", "steps_scale_factor_rk4", "steps_kdk_schedule", "steps_momentum",
     "steps_timestep", "steps_timestep_coefficient", "steps_force_residual", "steps_forces_quasi_periodic", "steps_forces_periodic",
@@ -65,6 +66,7 @@ def load_library(path: str) -> C.CDLL:
     vp, ll, dbl, i32 = C.c_void_p, C.c_longlong, C.c_double, C.c_int
     L.steps_forces.argtypes = [vp, vp, vp, ll, vp, vp]
     L.steps_forces_mixed.argtypes = [vp, vp, vp, ll, vp, vp]
+    L.steps_forces_static.argtypes = [vp, vp, vp, ll, vp, vp]
     L.steps_forces_range.argtypes = [vp, vp, vp, ll, ll, ll, vp, i32, vp]
     L.steps_forces_host.argtypes = [vp, vp, vp, ll, vp, i32, vp]
     L.steps_forces_blocks.argtypes = [vp, vp, vp, ll, ll, ll, vp, i32, vp]
@@ -142,6 +144,12 @@ def _host(a, n_elem: int):
 def steps_forces(pos, mass, soft, acc, stream=None) -> None:
     n = mass.numel()
     _check(lib().steps_forces(_dev(pos, 3 * n), _dev(mass, n), _dev(soft, n), n, _dev(acc, 3 * n), _stream(stream)))
+
+
+def steps_forces_static(pos, mass, soft, acc, stream=None) -> None:
+    """steps_forces for N <= STATIC_MAX_N with the scratch in a device array of the library: never allocates."""
+    n = mass.numel()
+    _check(lib().steps_forces_static(_dev(pos, 3 * n), _dev(mass, n), _dev(soft, n), n, _dev(acc, 3 * n), _stream(stream)))
 
 
 def steps_forces_mixed(pos, mass, soft, acc, stream=None) -> None:
