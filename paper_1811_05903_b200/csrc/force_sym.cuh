@@ -6,12 +6,13 @@
 //   * The particles are cut into BLOCKS of IB = 2048 consecutive (radially sorted) particles = 8 j-tiles.  A block pair
 //     (b, c) is "far" when the radial intervals of the two blocks are separated by more than hmax_b + hmax_c (the same
 //     triangle-inequality test as tile_is_far, on block bounds): then no pair of it can be softened and every pair
-//     is exactly Newtonian.  W = max |c - b| over the block pairs that are NOT far (a device scalar, sym_band_width):
-//     for radially sorted input W = 1 ... 7 (N = 131,072 ... 1,048,576: the softening shell spans more of the ever thinner
-//     radial blocks), for unsorted input W = nb - 1.
-//   * Block pairs with |c - b| <= W (the "band": the diagonal, all softened pairs, the self pairs) go through the
-//     asymmetric persistent kernel of force_driver.cuh, restricted to the band's tiles.
-//   * Every block pair with c - b > W is ONE work item of forces_sym_kernel: the CTA's 16 warps hold the 2048 particles of
+//     is exactly Newtonian.  edge[b] = the last block that is not far from block b or from an earlier row (sym_band_width +
+//     sym_plan_finalize, on the device; SymPlan in force_driver.cuh): for radially sorted input edge[b] - b = 1 ... 7
+//     (N = 131,072 ... 1,048,576: the softening shell spans more of the ever thinner radial blocks) and differs from row to
+//     row, for unsorted input edge[b] = nb - 1.
+//   * Block pairs (b, c), b <= c <= edge[b], and their mirror images (the "band": the diagonal, all softened pairs, the self
+//     pairs) go through the asymmetric persistent kernel of force_driver.cuh, restricted to the band's tiles.
+//   * Every block pair with c > edge[b] is ONE work item of forces_sym_kernel: the CTA's 16 warps hold the 2048 particles of
 //     block b in registers (4 per lane, as the asymmetric kernel does), block c's scaled sources sit in shared memory, and
 //     warp w meets the sixteen 128-source subgroups of c in the order (w + q) mod 16, q = 0..15 (one __syncthreads per
 //     round, so each subgroup's reaction sums in shared memory have one owner at a time).  Inside a (warp, subgroup)
