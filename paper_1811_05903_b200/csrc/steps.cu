@@ -41,7 +41,9 @@ constexpr int MAX_GRID = 148 * 4;
 // its partial records are produced and consumed in panels of at most g_sym_panel_items items (96 KiB of records each).
 constexpr int SYM_MIN_BLOCKS = 16;         // fp64: from N = 30,721, with the items split into parts while the blocks are few
 constexpr int SYM_SPLITJ_BAND_MAX_BLOCKS = 64;   // up to here the band of a pair-symmetric evaluation runs on the split-j driver
-constexpr int SYM_MIN_BLOCKS_MIXED = 64;   // mixed: whole items only (its split variant is slower than the ring kernel): N >= 129,025
+constexpr int SYM_MIN_BLOCKS_MIXED = 16;   // mixed: from N = 30,721 too; whole items from 24 blocks (N >= 47,105), below that each item in 4 parts
+constexpr int SYM_BOX_MIN_BLOCKS_MIXED = 64;       // periodic boxes, mixed: whole items only, N >= 129,025
+constexpr int SYM_MIXED_WHOLE_ITEMS_BLOCKS = 24;   // (the split variant of the mixed kernel is slower per pair: measured, profiles/r02_sizes.md)
 std::atomic<long long> g_sym_panel_items{16384};
 std::atomic<int> g_sym_enabled{1};
 std::atomic<int> g_splitj{1};           // 0 = never use the split-j driver (testing)
@@ -266,10 +268,11 @@ int launch_forces_sym(const double* pos, const double* mass, const double* soft,
     const int max_split = (FP64 ? SYM_FP64_THREADS : SYM_MIXED_THREADS) / 32;
     if constexpr (FP64)
         while (split < max_split && sym_items_max(N) * split < 24ll * Ps) split *= 2;
+    else if (nb < SYM_MIXED_WHOLE_ITEMS_BLOCKS) split = 4;
 
     prep_tiles<Tile><<<ntp, TJ, 0, st>>>(pos, mass, soft, N, tiles, &w.plan->W);
     sym_band_width<Tile><<<nb, 128, 0, st>>>(tiles, nb, w.plan);
-    sym_plan_finalize<<<1, 1024, 0, st>>>(w.plan, nb, 8 * Ps, split, 1);
+    sym_plan_finalize<<<1, 1024, 0, st>>>(w.plan, nb, (FP64 ? 8 : 1) * Ps, split, 1);
     if (prof) STEPS_CUDA(cudaEventRecord(w.ev0, st));
     double* hi = w.acc_dd;
     double* lo = w.acc_dd + 3 * N;
@@ -490,7 +493,8 @@ int launch_forces_box(const double* pos, const double* mass, const double* soft,
     const int nb = (int)nblocks_of(N);
     const int nt = (int)ntiles_of(N);
     Tile* tiles = reinterpret_cast<Tile*>(w.tiles);
-    const bool sym = g_driver.load() == 0 && sym_eligible(N, !FP64) && w.sym_records && (FP64 || g_sym_enabled.load() != 2);
+    const bool sym = g_driver.load() == 0 && sym_eligible(N, !FP64) && nb >= (FP64 ? SYM_MIN_BLOCKS : SYM_BOX_MIN_BLOCKS_MIXED) && w.sym_records &&
+                     (FP64 || g_sym_enabled.load() != 2);
     const long long groups = (N + SPLITJ_GROUP - 1) / SPLITJ_GROUP;
     const long long jsplit = boxring_jsplit(groups, nt, N, w);
     if (groups > 0x7fffffffll || jsplit > 65535) return STEPS_EINVAL;
