@@ -223,7 +223,7 @@ int steps_momentum(const double *vec, const double *mass, long long N, double *o
  * synth.morton_order) -- the periodic counterpart of the radial order: groups of consecutive particles whose bounding
  * boxes are compact and cannot hold a softened pair share one image decision -- a lattice shift per component, plus a
  * FOLD (d' = e - copysign(L/2, e), one addition and one bit operation) of the components whose separations straddle half
- * the box -- and run the open-boundary far body; from N = 30,721 (fp64) / 129,025 (mixed) such pairs of groups of two
+ * the box -- and run the open-boundary far body; from N = 30,721 (fp64) / 161,793 (mixed) such pairs of groups of two
  * different blocks of 2,048 particles are evaluated ONCE and applied to both groups (Newton III, as steps_forces does).
  * Unordered input, or particles given many periods apart, go through the general wrapped body with the per-pair softening
  * test -- slower, never wrong.  Ties (a separation component of exactly L/2, measure zero) may pick either image.  The

@@ -42,7 +42,7 @@ constexpr int MAX_GRID = 148 * 4;
 constexpr int SYM_MIN_BLOCKS = 16;         // fp64: from N = 30,721, with the items split into parts while the blocks are few
 constexpr int SYM_SPLITJ_BAND_MAX_BLOCKS = 64;   // up to here the band of a pair-symmetric evaluation runs on the split-j driver
 constexpr int SYM_MIN_BLOCKS_MIXED = 16;   // mixed: from N = 30,721 too; whole items from 24 blocks (N >= 47,105), below that each item in 4 parts
-constexpr int SYM_BOX_MIN_BLOCKS_MIXED = 64;       // periodic boxes, mixed: whole items only, N >= 129,025
+constexpr int SYM_BOX_MIN_BLOCKS_MIXED = 80;       // periodic boxes, mixed: N >= 161,793 (measured crossover with the group-ring kernel)
 constexpr int SYM_MIXED_WHOLE_ITEMS_BLOCKS = 24;   // (the split variant of the mixed kernel is slower per pair: measured, profiles/r02_sizes.md)
 std::atomic<long long> g_sym_panel_items{16384};
 std::atomic<int> g_sym_enabled{1};
@@ -480,7 +480,7 @@ int forces_impl(const double* pos, const double* mass, const double* soft, long 
 }
 
 // Leading-image periodic box (steps_forces_quasi_periodic).  One 128-particle group per CTA column (forces_boxring_kernel);
-// from 16 (fp64) / 64 (mixed) blocks the far pairs of DIFFERENT blocks go through the pair-symmetric kernels
+// from 16 (fp64) / 80 (mixed) blocks the far pairs of DIFFERENT blocks go through the pair-symmetric kernels
 // (forces_sym_box_kernel / forces_sym_mixed_box_kernel), each evaluated once, and the group-ring kernel runs in restricted
 // mode (the groups' own blocks + the units that may hold a softened pair).  All decisions that depend on the data are taken
 // on the device (pair_decision on the group boxes; the plan falls back to "everything one-sided" when the items are too few).
