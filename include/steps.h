@@ -77,7 +77,7 @@ enum {
 /* fp64 path: every pair in fp64 (the reciprocal square root is seeded by the fp32 SFU and
  * refined in fp64).  Bar: max_i |acc_i - oracle_i| / |oracle_i| <= 1e-12.
  * Overwrites acc[0..3N).  pos/mass/soft are read only.
- * From N = 30,721 (16 blocks of 2,048 particles; both paths) the evaluation is PAIR-SYMMETRIC: every block pair whose radial
+ * From N = 16,385 (9 blocks of 2,048 particles; mixed path: from 30,721, 16 blocks) the evaluation is PAIR-SYMMETRIC: every block pair whose radial
  * intervals are further apart than the largest pair softening is evaluated once and applied to both blocks (Newton's
  * third law; PAPER.md L131 counts the cost as N(N-1)/2 pair evaluations), the band of block pairs around the diagonal
  * goes through the one-sided kernel.  The split is decided on the device from the data; unsorted input, massless
@@ -135,7 +135,7 @@ int steps_forces_blocks(const double *pos, const double *mass, const double *sof
  * Every rank holds all particles; the one exchange per step is a sum-reduction of 3N doubles (NCCL all-reduce, 25 MB at
  * N = 1M) instead of the all-gather of positions, and every rank then advances ALL particles (O(N), bit-identical on every
  * rank).  Each rank runs the pair-symmetric kernels at their single-GPU rate (steps_forces_blocks is one-sided).  Below the
- * pair-symmetric size (N < 30,721: under a millisecond of work) rank 0 evaluates everything and the
+ * pair-symmetric size (N < 16,385 fp64 / 30,721 mixed: under half a millisecond of work) rank 0 evaluates everything and the
  * other ranks return zeros.  STEPS_EINVAL for rank outside [0, world). */
 int steps_forces_share(const double *pos, const double *mass, const double *soft, long long N, int rank,
                        int world, double *acc_part, int mixed, steps_stream_t stream);
@@ -309,8 +309,8 @@ int steps_set_option(const char *key, long long value);
  * device (waits for it to finish); -1 if none was recorded.  For a pair-symmetric evaluation: from the
  * start of the band kernel to the end of the last panel's reduce (all force kernels of the evaluation). */
 double steps_last_force_kernel_ms(void);
-/* 1 if a full force evaluation of N particles on the given path is set up pair-symmetrically (see steps_forces: from
- * N = 30,721 on both paths, and the "sym" option on), else 0.  Host-side eligibility only: the device still routes
+/* 1 if a full force evaluation of N particles on the given path is set up pair-symmetrically (see steps_forces: fp64 from
+ * N = 16,385, mixed from N = 30,721, and the "sym" option on), else 0.  Host-side eligibility only: the device still routes
  * everything through the one-sided kernel when the data do not allow the split (unsorted input, massless particles). */
 int steps_pair_symmetric(long long N, int mixed);
 /* Grid (CTA count) of the persistent force kernel on the current device: SMs x resident CTAs;

@@ -39,7 +39,8 @@ constexpr int MAX_GRID = 148 * 4;
 
 // Pair-symmetric evaluation (force_sym.cuh) of the fp64 path: used for full evaluations of at least SYM_MIN_BLOCKS blocks;
 // its partial records are produced and consumed in panels of at most g_sym_panel_items items (96 KiB of records each).
-constexpr int SYM_MIN_BLOCKS = 16;         // fp64: from N = 30,721, with the items split into parts while the blocks are few
+constexpr int SYM_MIN_BLOCKS = 9;          // fp64: from N = 16,385, with the items split into parts while the blocks are few
+constexpr int SYM_BOX_MIN_BLOCKS = 16;     // periodic boxes, fp64 (leading image and image sum): from N = 30,721
 constexpr int SYM_SPLITJ_BAND_MAX_BLOCKS = 64;   // up to here the band of a pair-symmetric evaluation runs on the split-j driver
 constexpr int SYM_MIN_BLOCKS_MIXED = 16;   // mixed: from N = 30,721 too; whole items from 24 blocks (N >= 47,105), below that each item in 4 parts
 constexpr int SYM_BOX_MIN_BLOCKS_MIXED = 80;       // periodic boxes, mixed: N >= 161,793 (measured crossover with the group-ring kernel)
@@ -272,7 +273,7 @@ int launch_forces_sym(const double* pos, const double* mass, const double* soft,
 
     prep_tiles<Tile><<<ntp, TJ, 0, st>>>(pos, mass, soft, N, tiles, &w.plan->W);
     sym_band_width<Tile><<<nb, 128, 0, st>>>(tiles, nb, w.plan);
-    sym_plan_finalize<<<1, 1024, 0, st>>>(w.plan, nb, (FP64 ? 8 : 1) * Ps, split, 1);
+    sym_plan_finalize<<<1, 1024, 0, st>>>(w.plan, nb, (FP64 ? 2 : 1) * Ps, split, 1);
     if (prof) STEPS_CUDA(cudaEventRecord(w.ev0, st));
     double* hi = w.acc_dd;
     double* lo = w.acc_dd + 3 * N;
@@ -493,7 +494,7 @@ int launch_forces_box(const double* pos, const double* mass, const double* soft,
     const int nb = (int)nblocks_of(N);
     const int nt = (int)ntiles_of(N);
     Tile* tiles = reinterpret_cast<Tile*>(w.tiles);
-    const bool sym = g_driver.load() == 0 && sym_eligible(N, !FP64) && nb >= (FP64 ? SYM_MIN_BLOCKS : SYM_BOX_MIN_BLOCKS_MIXED) && w.sym_records &&
+    const bool sym = g_driver.load() == 0 && sym_eligible(N, !FP64) && nb >= (FP64 ? SYM_BOX_MIN_BLOCKS : SYM_BOX_MIN_BLOCKS_MIXED) && w.sym_records &&
                      (FP64 || g_sym_enabled.load() != 2);
     const long long groups = (N + SPLITJ_GROUP - 1) / SPLITJ_GROUP;
     const long long jsplit = boxring_jsplit(groups, nt, N, w);
@@ -661,7 +662,7 @@ int launch_forces_periodic(const double* pos, const double* mass, const double* 
         if (rc != STEPS_OK) return rc;
         return release_scratch(w, st);
     } else {
-        if (g_driver.load() == 0 && sym_eligible(N, false) && w.sym_records) {
+        if (g_driver.load() == 0 && sym_eligible(N, false) && nblocks_of(N) >= SYM_BOX_MIN_BLOCKS && w.sym_records) {
             rc = launch_forces_images_sym(pos, mass, soft, N, L, acc_out, st, w);
             if (rc != STEPS_OK) return rc;
             return release_scratch(w, st);

@@ -238,7 +238,12 @@ def test_simple_driver_cross_check(S, oracle, mixed):
     pair bodies; both must meet the bar and agree to summation-order rounding."""
     ps = synth.g0(20000, seed=31, eps0=0.03)
     ref = oracle.forces(ps.pos, ps.mass, ps.soft)
-    fast = gpu_forces(S, ps, mixed)
+    S.steps_set_option("sym", 0)                # (the fp64 path is pair-symmetric from 16,385 particles: this test is about the ring driver)
+    try:
+        fast = gpu_forces(S, ps, mixed)
+    finally:
+        S.steps_set_option("sym", 1)
+    check(gpu_forces(S, ps, mixed), ref, mixed, "default route")
     S.steps_set_option("driver", 1)
     try:
         simple = gpu_forces(S, ps, mixed)
