@@ -185,6 +185,29 @@ def test_pair_symmetric_path_and_its_fallbacks(S, oracle, mixed, case):
     check(got, ref, mixed, f"sym/{case}")
 
 
+@pytest.mark.parametrize("mixed,n", [(False, 16385), (False, 24577), (True, 30721), (True, 40001), (True, 50001)],
+                         ids=["fp64-16385", "fp64-24577", "mixed-30721", "mixed-40001", "mixed-50001"])
+def test_pair_symmetric_route_at_its_smallest_sizes(S, oracle, mixed, n):
+    """The smallest sizes of the pair-symmetric route, all ragged: fp64 from 9 blocks (items in 16 parts), mixed from 16 blocks
+    (4 parts per item up to 23 blocks, whole items from 24); the band of these sizes runs on the split-j driver.  Against
+    the oracle on a sample; the same bits on a second run; the one-sided evaluation to summation-order rounding."""
+    assert S.steps_pair_symmetric(n, mixed) == 1
+    if n in (16385, 30721):                     # the thresholds themselves
+        assert S.steps_pair_symmetric(n - 1, mixed) == 0
+    ps = synth.g0(n, seed=5150 + n)
+    idx = synth.stratified_sample(n, 1024)
+    ref = oracle.forces(ps.pos, ps.mass, ps.soft, idx=idx)
+    got = gpu_forces(S, ps, mixed)
+    check(got[:, idx], ref, mixed, f"sym-min n={n}")
+    assert np.array_equal(got, gpu_forces(S, ps, mixed))
+    S.steps_set_option("sym", 0)
+    try:
+        one = gpu_forces(S, ps, mixed)
+    finally:
+        S.steps_set_option("sym", 1)
+    assert rel_err(got, one).max() <= (1e-4 if mixed else 1e-13)
+
+
 def test_newtons_third_law_and_determinism_on_device(S):
     import torch
     ps = synth.config(1)
@@ -358,7 +381,8 @@ def test_outputs_stay_inside_their_buffers(S, n):
 
 
 @pytest.mark.parametrize("world", [2, 3, 8])
-@pytest.mark.parametrize("mixed,n", [(False, 65536), (False, 4096), (True, 150001)], ids=["fp64-65536", "fp64-4096", "mixed-150001"])
+@pytest.mark.parametrize("mixed,n", [(False, 65536), (False, 4096), (True, 150001), (True, 40001)],
+                         ids=["fp64-65536", "fp64-4096", "mixed-150001", "mixed-40001"])
 def test_work_shares_sum_to_the_full_evaluation(S, oracle, mixed, n, world):
     """steps_forces_share: the pair evaluations of one force evaluation cut into `world` equal parts (band visits and
     pair-symmetric items); the sum of the parts' partial accelerations is the full result to rounding (each part is
