@@ -223,7 +223,7 @@ int steps_momentum(const double *vec, const double *mass, long long N, double *o
  * synth.morton_order) -- the periodic counterpart of the radial order: groups of consecutive particles whose bounding
  * boxes are compact and cannot hold a softened pair share one image decision -- a lattice shift per component, plus a
  * FOLD (d' = e - copysign(L/2, e), one addition and one bit operation) of the components whose separations straddle half
- * the box -- and run the open-boundary far body; from N = 30,721 (fp64) / 161,793 (mixed) such pairs of groups of two
+ * the box -- and run the open-boundary far body; from N = 16,385 (fp64) / 161,793 (mixed) such pairs of groups of two
  * different blocks of 2,048 particles are evaluated ONCE and applied to both groups (Newton III, as steps_forces does).
  * Unordered input, or particles given many periods apart, go through the general wrapped body with the per-pair softening
  * test -- slower, never wrong.  Ties (a separation component of exactly L/2, measure zero) may pick either image.  The
@@ -238,7 +238,7 @@ int steps_forces_quasi_periodic(const double *pos, const double *mass, const dou
  * the positions are given in (|x_j - x_i| < 2^51 L).  Cost: 74 images per pair inside the cut on average; a pair on its
  * own needs 179 candidates (all n.n <= 12 around its leading image), a pair of 128-particle groups of cell-ordered input
  * whose bounding boxes are compact and cannot hold a softened pair is pruned to the ~90-110 candidates that come within
- * the cut for some pair of the two boxes, and from N = 30,721 such pairs of groups of two different blocks of 2,048
+ * the cut for some pair of the two boxes, and from N = 16,385 such pairs of groups of two different blocks of 2,048
  * particles are evaluated ONCE for both groups (the image sum of a pair is antisymmetric).  A particle's OWN images (j = i, n != 0) are summed like any other pair's: the triplet set is symmetric under
  * n -> -n, so they cancel to rounding (the oracle skips j = i altogether).  Softening up to h_i + h_j <= L/2 takes the
  * fast route (only the nearest image can then be softened); larger softening is handled image by image. */

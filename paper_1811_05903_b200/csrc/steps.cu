@@ -40,7 +40,7 @@ constexpr int MAX_GRID = 148 * 4;
 // Pair-symmetric evaluation (force_sym.cuh) of the fp64 path: used for full evaluations of at least SYM_MIN_BLOCKS blocks;
 // its partial records are produced and consumed in panels of at most g_sym_panel_items items (96 KiB of records each).
 constexpr int SYM_MIN_BLOCKS = 9;          // fp64: from N = 16,385, with the items split into parts while the blocks are few
-constexpr int SYM_BOX_MIN_BLOCKS = 16;     // periodic boxes, fp64 (leading image and image sum): from N = 30,721
+constexpr int SYM_BOX_MIN_BLOCKS = 9;      // periodic boxes, fp64 (leading image and image sum): from N = 16,385 as well
 constexpr int SYM_SPLITJ_BAND_MAX_BLOCKS = 64;   // up to here the band of a pair-symmetric evaluation runs on the split-j driver
 constexpr int SYM_MIN_BLOCKS_MIXED = 16;   // mixed: from N = 30,721 too; whole items from 24 blocks (N >= 47,105), below that each item in 4 parts
 constexpr int SYM_BOX_MIN_BLOCKS_MIXED = 80;       // periodic boxes, mixed: N >= 161,793 (measured crossover with the group-ring kernel)
@@ -481,7 +481,7 @@ int forces_impl(const double* pos, const double* mass, const double* soft, long 
 }
 
 // Leading-image periodic box (steps_forces_quasi_periodic).  One 128-particle group per CTA column (forces_boxring_kernel);
-// from 16 (fp64) / 80 (mixed) blocks the far pairs of DIFFERENT blocks go through the pair-symmetric kernels
+// from 9 (fp64) / 80 (mixed) blocks the far pairs of DIFFERENT blocks go through the pair-symmetric kernels
 // (forces_sym_box_kernel / forces_sym_mixed_box_kernel), each evaluated once, and the group-ring kernel runs in restricted
 // mode (the groups' own blocks + the units that may hold a softened pair).  All decisions that depend on the data are taken
 // on the device (pair_decision on the group boxes; the plan falls back to "everything one-sided" when the items are too few).
@@ -541,7 +541,7 @@ int launch_forces_box(const double* pos, const double* mass, const double* soft,
     }
     prep_tiles<Tile><<<ntp, TJ, 0, st>>>(pos, mass, soft, N, tiles, &w.plan->W);          // W = 0: every block pair is an item
     group_meta_kernel<Tile><<<(ngm + 3) / 4, 128, 0, st>>>(pos, soft, N, tiles, w.gm, ngm);
-    sym_plan_finalize<<<1, 1024, 0, st>>>(w.plan, nb, 8 * Ps, split, 0);
+    sym_plan_finalize<<<1, 1024, 0, st>>>(w.plan, nb, 2 * Ps, split, 0);
     if (prof) STEPS_CUDA(cudaEventRecord(w.ev0, st));
     double* hi = w.acc_dd;
     double* lo = w.acc_dd + 3 * N;
@@ -584,7 +584,7 @@ int launch_forces_box(const double* pos, const double* mass, const double* soft,
     return STEPS_OK;
 }
 
-// Image sum (steps_forces_periodic) from 16 blocks: every far meeting of two groups of different blocks ONCE
+// Image sum (steps_forces_periodic) from 9 blocks: every far meeting of two groups of different blocks ONCE
 // (forces_sym_img_kernel: the image sum of a pair is antisymmetric), the possibly-softened units by
 // forces_boxgen_kernel<Fp64Path, 2>, the groups' own blocks by the group-ring kernel in restricted mode.
 int launch_forces_images_sym(const double* pos, const double* mass, const double* soft, long long N, double L, double* acc_out,

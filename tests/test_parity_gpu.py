@@ -729,9 +729,10 @@ def _pair_force_abs_sum(pos, mass, soft, L, idx=None):
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("mixed,n", [(False, 40001), (False, 150001), (True, 150001)], ids=["fp64-40001", "fp64-150001", "mixed-150001"])
+@pytest.mark.parametrize("mixed,n", [(False, 18433), (False, 40001), (False, 150001), (True, 170001)],
+                         ids=["fp64-18433", "fp64-40001", "fp64-150001", "mixed-170001"])
 def test_quasi_periodic_pair_symmetric_route(S, mixed, n):
-    """From 16 (fp64) / 64 (mixed) blocks the far meetings of two different blocks are evaluated once and applied to both
+    """From 9 (fp64) / 80 (mixed) blocks the far meetings of two different blocks are evaluated once and applied to both
     groups (forces_sym_box_kernel), the possibly-softened units by forces_boxgen_kernel, the own blocks by the group-ring
     kernel.  Every pair must be evaluated by exactly one of them: the result equals the one-sided evaluation (option
     "sym" = 0: group-ring kernel alone) to rounding, is bit-identical run to run, and obeys Newton's third law."""
@@ -1001,9 +1002,9 @@ def test_periodic_image_sum_several_i_blocks_sampled(S, oracle):
     assert float(p.norm()) < 1e-12 * float((dm * acc.norm(dim=0)).sum())
 
 
-@pytest.mark.parametrize("n,ordered", [(32768, True), (40001, True), (32768, False)])
+@pytest.mark.parametrize("n,ordered", [(18433, True), (32768, True), (40001, True), (32768, False)])
 def test_periodic_image_sum_pair_symmetric_route(S, oracle, n, ordered):
-    """From 16 blocks the image sum evaluates every far meeting of two groups of different blocks once
+    """From 9 blocks (N = 16,385) the image sum evaluates every far meeting of two groups of different blocks once
     (forces_sym_img_kernel), the possibly-softened units through forces_boxgen_kernel<., 2>, the own blocks through the
     group-ring kernel.  Against the oracle on a sample (unequal masses: a swapped m_i / m_j in the reaction would show;
     some larger softenings; unordered input: everything through the unpruned route), equality with the one-sided
