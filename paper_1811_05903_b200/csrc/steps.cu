@@ -264,12 +264,23 @@ int launch_forces_sym(const double* pos, const double* mass, const double* soft,
     if (prof && !w.ev0) { STEPS_CUDA(cudaEventCreate(&w.ev0)); STEPS_CUDA(cudaEventCreate(&w.ev1)); }
 
     // Parts per item: with few blocks an item (0.3-0.7 ms) is too coarse a unit for 148 SMs, so its rounds are shared among
-    // `split` sub-items (a power of two, at most the warps per CTA) until there are about 24 of them per CTA.
+    // `split` sub-items (a power of two, at most the warps per CTA).
     int split = 1;
     const int max_split = (FP64 ? SYM_FP64_THREADS : SYM_MIXED_THREADS) / 32;
-    if constexpr (FP64)
-        while (split < max_split && sym_items_max(N) * split < 24ll * Ps) split *= 2;
-    else if (nb < SYM_MIXED_WHOLE_ITEMS_BLOCKS) split = 4;
+    if constexpr (FP64) {
+        // the part count that minimises  ceil(K s / CTAs) x (1 / s + c):  the slowest CTA's parts times the cost of a part, an
+        // s-th of an item plus a fixed cost c = 1/73 of an item (column copy, zeroing, 96 KiB of records: about 10 us, from
+        // the measured times at N = 32,768 ... 98,304, profiles/r02_sizes.md); K estimated for a band of one block to
+        // either side; whole items (the kernel variant with compile-time loop bounds) preferred by 3 %; at least the
+        // 2 sub-items per CTA below which the plan gives the items up (sym_plan_finalize)
+        const double Kest = (double)std::max(1ll, sym_items_max(N) - (nb - 1));
+        double best = 0.0;
+        for (int s = max_split; s >= 1; s /= 2) {
+            if (s < max_split && Kest * s < 2.0 * Ps) break;
+            const double cost = std::ceil(Kest * s / Ps) * (1.0 / s + 1.0 / 73.0) * (s == 1 ? 0.97 : 1.0);
+            if (best == 0.0 || cost < best) { best = cost; split = s; }
+        }
+    } else if (nb < SYM_MIXED_WHOLE_ITEMS_BLOCKS) split = 4;
 
     prep_tiles<Tile><<<ntp, TJ, 0, st>>>(pos, mass, soft, N, tiles, &w.plan->W);
     sym_band_width<Tile><<<nb, 128, 0, st>>>(tiles, nb, w.plan);
